@@ -1,0 +1,330 @@
+/*
+ * rw_oracle.c -- CPU ORACLE for the spectrum-reweighting likelihood hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or constant generator with the CUDA path in
+ * paper_2607_00488_b200/csrc; neither side includes or imports the other.
+ *
+ * What it is: the plain definitions of arxiv/paper_2607_00488 written
+ * out as loops -- no basis decomposition, no blocking, no BLAS, no reordering.
+ * Inputs and outputs are IEEE binary64; every intermediate and accumulator is
+ * `long double` (x87 80-bit, 64-bit significand on x86-64) so that the oracle is
+ * more accurate than the 1e-12 parity tolerance by several orders of magnitude.
+ * The single exception is the kinematic cut, which is *specified* in binary64
+ * (reading R2) so that both sides take the same yes/no decision.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`), per function:
+ *   orc_tmax          closed form + textbook Compton edges (7Be 665 keV, pp 261 keV)
+ *   orc_sm_couplings  Eq. (2)-(3) values, tests/golden/sm_couplings.txt
+ *   orc_dsigma_weak   antiderivative closed form vs adaptive quadrature; textbook
+ *                     sigma_e/E, sigma_mu/E high-energy slopes; sigma_0
+ *   orc_dsigma_mm     antiderivative ln(T2/T1)-(T2-T1)/E vs quadrature; zero at T=E
+ *   orc_spectrum      single-line reduction to dsigma; continuum limit vs scipy
+ *                     dblquad-free closed form; exact quadratic/linear structure in
+ *                     (eps, mu_nu^2); chirality sign-flip symmetry; mpmath brute force
+ *   orc_weights       theta=0 => w == 1 bit-exactly
+ *   orc_fold          identity / rank-1 responses; numpy matmul on random inputs;
+ *                     folded total = sum_i w_i N_i eff_i
+ *   orc_deviance      n == mu => 0; vs scipy.stats.poisson.logpmf; small-d expansion
+ *   orc_eq18          vs -2*sum(scipy.stats.poisson.logpmf)
+ *   orc_eval_batch    composition of the above; Asimov injection-recovery
+ *                     (PAPER.md:309-311); rank-K prefold identity
+ * No function here is "parity unpinned".
+ *
+ * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC rw_oracle.c -o librw_oracle.so -lm
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <float.h>
+#include <stdlib.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef long double xreal; /* extended working precision */
+
+typedef struct {
+    double sin2_theta_w; /* weak mixing angle, Eq. (2)-(3) PAPER.md:56-58 */
+    double m_e;          /* electron mass [MeV] */
+    double G_F;          /* Fermi constant [MeV^-2] */
+    double alpha_em;     /* fine-structure constant, Eq. (8) */
+} orc_consts;
+
+/* parameter kinds (values fixed by DESIGN.md "param_kind" table, not by a shared header) */
+enum {
+    ORC_EPS_EE_L = 0, ORC_EPS_EE_R = 1,
+    ORC_EPS_MM_L = 2, ORC_EPS_MM_R = 3,
+    ORC_EPS_TT_L = 4, ORC_EPS_TT_R = 5,
+    ORC_MU_NU    = 6,  /* mu_nu in Bohr magnetons */
+    ORC_N_KINDS  = 7
+};
+
+/* The paper gives no numerical constants (symbols only);
+ * DESIGN.md reading R1 fixes PDG-style values, natural units, MeV. */
+void orc_default_consts(orc_consts *c)
+{
+    c->sin2_theta_w = 0.23121;
+    c->m_e          = 0.51099895;
+    c->G_F          = 1.1663788e-11;
+    c->alpha_em     = 1.0 / 137.035999084;
+}
+
+int orc_long_double_mant_dig(void) { return LDBL_MANT_DIG; }
+
+/* Kinematic limit of the recoil energy for neutrino energy E: T <= 2E^2/(m_e+2E).
+ * Not printed in PAPER.md; fixed by BASELINE.json north_star (reading R2).
+ * Evaluated in binary64, one expression, exactly as written. */
+double orc_tmax(double E, double m_e)
+{
+    volatile double num = 2.0 * E * E;
+    volatile double den = m_e + 2.0 * E;
+    return num / den;
+}
+
+/* Eq. (2)-(3).  Flavour order: 0=e, 1=mu, 2=tau. */
+void orc_sm_couplings(const orc_consts *c, double gL[3], double gR[3])
+{
+    gL[0] = 0.5 + c->sin2_theta_w;   gR[0] = c->sin2_theta_w;
+    gL[1] = -0.5 + c->sin2_theta_w;  gR[1] = c->sin2_theta_w;
+    gL[2] = -0.5 + c->sin2_theta_w;  gR[2] = c->sin2_theta_w;
+}
+
+/* Eq. (4) / Eq. (7), PAPER.md:65,83:
+ *   dsigma/dT = (2 G_F^2 m_e / pi) [ gL^2 + gR^2 (1 - T/E)^2 - gL gR m_e T / E^2 ]
+ * (no kinematic cut applied here). */
+static xreal xdsigma_weak(const orc_consts *c, xreal E, xreal T, xreal gL, xreal gR)
+{
+    const xreal pi = acosl(-1.0L);
+    xreal pref = 2.0L * (xreal)c->G_F * (xreal)c->G_F * (xreal)c->m_e / pi;
+    xreal one_m = 1.0L - T / E;
+    return pref * (gL * gL + gR * gR * one_m * one_m - gL * gR * (xreal)c->m_e * T / (E * E));
+}
+
+/* Eq. (8):  dsigma^MM/dT = (pi alpha^2 / m_e^2) (mu_nu/mu_B)^2 (1/T - 1/E). */
+static xreal xdsigma_mm(const orc_consts *c, xreal E, xreal T, xreal mu_nu)
+{
+    const xreal pi = acosl(-1.0L);
+    xreal pref = pi * (xreal)c->alpha_em * (xreal)c->alpha_em / ((xreal)c->m_e * (xreal)c->m_e);
+    return pref * mu_nu * mu_nu * (1.0L / T - 1.0L / E);
+}
+
+double orc_dsigma_weak(const orc_consts *c, double E, double T, double gL, double gR)
+{
+    return (double)xdsigma_weak(c, E, T, gL, gR);
+}
+
+double orc_dsigma_mm(const orc_consts *c, double E, double T, double mu_nu)
+{
+    return (double)xdsigma_mm(c, E, T, mu_nu);
+}
+
+/* theta[7] indexed by the ORC_* kinds above. */
+static void xspectrum(const orc_consts *c, int n_E, const double *E, const double *flux_w,
+                      const double *P_e, const double *P_mu, const double *P_tau,
+                      int n_T, const double *T, const double *theta, xreal *S)
+{
+    double gL0[3], gR0[3];
+    xreal gL[3], gR[3];
+    orc_sm_couplings(c, gL0, gR0);
+    /* Eq. (6): g -> g + eps_{alpha alpha}^{eL,R} */
+    gL[0] = (xreal)gL0[0] + (xreal)theta[ORC_EPS_EE_L];
+    gR[0] = (xreal)gR0[0] + (xreal)theta[ORC_EPS_EE_R];
+    gL[1] = (xreal)gL0[1] + (xreal)theta[ORC_EPS_MM_L];
+    gR[1] = (xreal)gR0[1] + (xreal)theta[ORC_EPS_MM_R];
+    gL[2] = (xreal)gL0[2] + (xreal)theta[ORC_EPS_TT_L];
+    gR[2] = (xreal)gR0[2] + (xreal)theta[ORC_EPS_TT_R];
+    xreal mu_nu = (xreal)theta[ORC_MU_NU];
+
+    /* Eq. (12) with the flavour sum of Eq. (5) and the incoherent MM term of Eq. (9),
+     * PAPER.md:138-140, 69-71, 102.  flux_w[j] = phi(E_j) * dE_j; a line is one entry. */
+    for (int i = 0; i < n_T; ++i) {
+        xreal acc = 0.0L;
+        for (int j = 0; j < n_E; ++j) {
+            if (!(T[i] <= orc_tmax(E[j], c->m_e))) continue; /* kinematic cut (R2) */
+            xreal Ej = E[j], Ti = T[i];
+            xreal weak = (xreal)P_e[j]   * xdsigma_weak(c, Ej, Ti, gL[0], gR[0])
+                       + (xreal)P_mu[j]  * xdsigma_weak(c, Ej, Ti, gL[1], gR[1])
+                       + (xreal)P_tau[j] * xdsigma_weak(c, Ej, Ti, gL[2], gR[2]);
+            /* MM term is flavour independent; sum_alpha P_alpha = 1 */
+            xreal mm = xdsigma_mm(c, Ej, Ti, mu_nu);
+            acc += (xreal)flux_w[j] * (weak + mm);
+        }
+        S[i] = acc;
+    }
+}
+
+void orc_spectrum(const orc_consts *c, int n_E, const double *E, const double *flux_w,
+                  const double *P_e, const double *P_mu, const double *P_tau,
+                  int n_T, const double *T, const double *theta, double *S_out)
+{
+    xreal *S = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T > 0 ? n_T : 1));
+    xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, theta, S);
+    for (int i = 0; i < n_T; ++i) S_out[i] = (double)S[i];
+    free(S);
+}
+
+/* Bin-to-bin weights, Eq. (14) in the un-normalised north_star form w_i = S_theta/S_SM
+ * (readings R5, R9: w := 1 where S_SM == 0). */
+static void xweights(int n_T, const xreal *S, const xreal *S_sm, xreal *w)
+{
+    for (int i = 0; i < n_T; ++i)
+        w[i] = (S_sm[i] == 0.0L) ? 1.0L : S[i] / S_sm[i];
+}
+
+void orc_weights(const orc_consts *c, int n_E, const double *E, const double *flux_w,
+                 const double *P_e, const double *P_mu, const double *P_tau,
+                 int n_T, const double *T, const double *theta, double *w_out)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    size_t n = (size_t)(n_T > 0 ? n_T : 1);
+    xreal *S = (xreal *)malloc(sizeof(xreal) * 3 * n), *S0 = S + n, *w = S0 + n;
+    xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, theta, S);
+    xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, zero, S0);
+    xweights(n_T, S, S0, w);
+    for (int i = 0; i < n_T; ++i) w_out[i] = (double)w[i];
+    free(S);
+}
+
+/* Eq. (1)/(11): mu_k = sum_i R[i][k] * (w_i * N_mc,i) + bkg_k.
+ * R row-major [n_T][n_rec], conditional response (sum_k R[i][k] = efficiency_i). */
+static void xfold(int n_T, int n_rec, const xreal *w, const double *N_mc, const double *R,
+                  const double *bkg, xreal *mu)
+{
+    for (int k = 0; k < n_rec; ++k) {
+        xreal acc = 0.0L;
+        for (int i = 0; i < n_T; ++i)
+            acc += (w[i] * (xreal)N_mc[i]) * (xreal)R[(size_t)i * n_rec + k];
+        mu[k] = acc + (xreal)bkg[k];
+    }
+}
+
+void orc_fold(int n_T, int n_rec, const double *w, const double *N_mc, const double *R,
+              const double *bkg, double *mu_out)
+{
+    xreal *xw = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T + n_rec + 1)), *mu = xw + n_T;
+    for (int i = 0; i < n_T; ++i) xw[i] = w[i];
+    xfold(n_T, n_rec, xw, N_mc, R, bkg, mu);
+    for (int k = 0; k < n_rec; ++k) mu_out[k] = (double)mu[k];
+    free(xw);
+}
+
+/* Poisson deviance = Eq. (18) first sum minus its saturated value (reading R7):
+ *   2 sum_k [ mu - n + n ln(n/mu) ];  n = 0 => 2 mu;  mu = 0 < n => +inf  (R8). */
+static xreal xdeviance(int n_rec, const xreal *mu, const double *n)
+{
+    xreal acc = 0.0L;
+    for (int k = 0; k < n_rec; ++k) {
+        xreal nk = n[k], mk = mu[k];
+        if (nk > 0.0L) {
+            if (mk > 0.0L) {
+                xreal d = mk - nk;
+                acc += d - nk * log1pl(d / nk);
+            } else {
+                acc += (xreal)INFINITY;
+            }
+        } else {
+            acc += mk;
+        }
+    }
+    return 2.0L * acc;
+}
+
+/* Literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)]. */
+static xreal xeq18(int n_rec, const xreal *mu, const double *n)
+{
+    xreal acc = 0.0L;
+    for (int k = 0; k < n_rec; ++k) {
+        xreal nk = n[k], mk = mu[k];
+        xreal t = mk + lgammal(nk + 1.0L);
+        if (nk > 0.0L) t -= nk * logl(mk);
+        acc += t;
+    }
+    return 2.0L * acc;
+}
+
+double orc_deviance(int n_rec, const double *mu, const double *n)
+{
+    xreal *xmu = (xreal *)malloc(sizeof(xreal) * (size_t)(n_rec > 0 ? n_rec : 1));
+    for (int k = 0; k < n_rec; ++k) xmu[k] = mu[k];
+    double r = (double)xdeviance(n_rec, xmu, n);
+    free(xmu);
+    return r;
+}
+
+double orc_eq18(int n_rec, const double *mu, const double *n)
+{
+    xreal *xmu = (xreal *)malloc(sizeof(xreal) * (size_t)(n_rec > 0 ? n_rec : 1));
+    for (int k = 0; k < n_rec; ++k) xmu[k] = mu[k];
+    double r = (double)xeq18(n_rec, xmu, n);
+    free(xmu);
+    return r;
+}
+
+/* Whole path for a batch of points (one "likelihood call" per point).
+ *   params  [P][k] row-major, kinds[k] in ORC_* (absent kinds are 0)
+ *   N_mc    [n_periods][n_T];  R [n_periods][n_T][n_rec];  bkg, counts [n_periods][n_rec]
+ *   out     [P] deviance (or literal Eq. 18 sum if full_eq18 != 0), summed over periods
+ *   mu_out  NULL or [P][n_periods][n_rec]
+ *   abs_out NULL or [P]: sum_k 2|term_k| (conditioning scale for the tolerance, reading T)
+ * The SM denominator is computed once per call by the same spectrum routine at theta = 0
+ * ("computed once during initialization").  Returns 0, or -1 on bad kinds. */
+int orc_eval_batch(const orc_consts *c, int n_E, const double *E, const double *flux_w,
+                   const double *P_e, const double *P_mu, const double *P_tau,
+                   int n_T, const double *T, int n_rec, int n_periods,
+                   const double *N_mc, const double *R, const double *bkg, const double *counts,
+                   int64_t P, int k, const int32_t *kinds, const double *params,
+                   double *out, double *mu_out, double *abs_out, int full_eq18, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T > 0 ? n_T : 1));
+    xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, zero, S0);
+    if (nthreads < 1) nthreads = 1;
+
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        for (int a = 0; a < k; ++a) theta[kinds[a]] = params[p * k + a];
+        xreal *S = (xreal *)malloc(sizeof(xreal) * (size_t)(2 * n_T + n_rec + 1));
+        xreal *w = S + n_T, *mu = w + n_T;
+        xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, theta, S);
+        xweights(n_T, S, S0, w);
+        xreal total = 0.0L, total_abs = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            const double *Nd = N_mc + (size_t)d * n_T;
+            const double *Rd = R + (size_t)d * n_T * n_rec;
+            const double *Bd = bkg + (size_t)d * n_rec;
+            const double *Cd = counts + (size_t)d * n_rec;
+            xfold(n_T, n_rec, w, Nd, Rd, Bd, mu);
+            total += full_eq18 ? xeq18(n_rec, mu, Cd) : xdeviance(n_rec, mu, Cd);
+            if (mu_out)
+                for (int q = 0; q < n_rec; ++q)
+                    mu_out[((size_t)p * n_periods + d) * n_rec + q] = (double)mu[q];
+            if (abs_out)
+                for (int q = 0; q < n_rec; ++q) {
+                    xreal one = xdeviance(1, mu + q, Cd + q);
+                    total_abs += fabsl(one);
+                }
+        }
+        out[p] = (double)total;
+        if (abs_out) abs_out[p] = (double)total_abs;
+        free(S);
+    }
+    free(S0);
+    return 0;
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,397 @@
+"""Pins of the CPU oracle against things other than itself: closed forms, textbook numbers,
+library routines, invariants and brute force (prompt section (3); SURVEY.md 8(c) "What pins
+each part").  All CPU, all `-m "not gpu"`."""
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+from scipy import integrate, stats
+
+from paper_2607_00488_b200 import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _table(fn):
+    rows = {}
+    for line in open(os.path.join(GOLD, fn)):
+        line = line.split("#")[0].strip()
+        if line:
+            f = line.split()
+            rows[f[0]] = f[1:]
+    return rows
+
+
+TEXT = _table("textbook_values.txt")
+PAPER = _table("paper_values.txt")
+HBARC2 = float(TEXT["hbarc2_cm2_MeV2"][0])
+
+
+def _txt(name):
+    return float(TEXT[name][0]), float(TEXT[name][1])
+
+
+def test_long_double_is_extended(orc):
+    assert orc.long_double_mant_dig() >= 64
+
+
+# ----------------------------------------------------------------------------- T_max
+def test_tmax_closed_form_and_textbook_edges(orc):
+    c = orc.default_consts()
+    mp.mp.dps = 40
+    for E in (0.05, 0.42, 0.862, 1.44, 3.0, 16.0):
+        ref = 2 * mp.mpf(E) ** 2 / (mp.mpf(c.m_e) + 2 * mp.mpf(E))
+        assert abs(orc.tmax(E) - float(ref)) <= 2 * np.spacing(float(ref))
+    v, tol = _txt("be7_compton_edge_MeV")
+    assert abs(orc.tmax(float(PAPER["be7_line_MeV"][0])) / v - 1) < tol
+    v, tol = _txt("pp_endpoint_edge_MeV")
+    assert abs(orc.tmax(0.42) / v - 1) < tol
+    # E >> m_e: E - T_max -> m_e/2 (backward scattering leaves m_e/2 to the neutrino)
+    assert abs((1e4 - orc.tmax(1e4)) - c.m_e / 2) < 1e-4
+
+
+# ----------------------------------------------------------------------------- couplings
+def test_sm_couplings_eq2_eq3(orc):
+    c = orc.default_consts()
+    gL, gR = orc.sm_couplings()
+    rows = _table("sm_couplings.txt")
+    for a, fl in enumerate(("e", "mu", "tau")):
+        assert gL[a] == float(rows[fl][0]) + c.sin2_theta_w
+        assert gR[a] == float(rows[fl][1]) + c.sin2_theta_w
+
+
+# ----------------------------------------------------------------------------- Eq. (4)
+def _weak_antiderivative(c, E, T, gL, gR):
+    """F(T) with dF/dT = Eq.(4): C0 [gL^2 T - gR^2 (E/3)(1-T/E)^3 - gL gR m_e T^2/(2E^2)]."""
+    C0 = 2 * c.G_F ** 2 * c.m_e / np.pi
+    return C0 * (gL ** 2 * T - gR ** 2 * (E / 3.0) * (1 - T / E) ** 3 - gL * gR * c.m_e * T ** 2 / (2 * E * E))
+
+
+@pytest.mark.parametrize("E,gL,gR", [(0.862, 0.73121, 0.23121), (0.3, -0.26879, 0.23121),
+                                     (10.0, 0.9, -0.4), (2.0, -0.1, 0.7)])
+def test_dsigma_weak_integrates_to_closed_form(orc, E, gL, gR):
+    c = orc.default_consts()
+    T1, T2 = 0.02 * E, orc.tmax(E)
+    num, err = integrate.quad(lambda t: orc.dsigma_weak(E, t, gL, gR), T1, T2, epsabs=0, epsrel=1e-13)
+    ref = _weak_antiderivative(c, E, T2, gL, gR) - _weak_antiderivative(c, E, T1, gL, gR)
+    assert abs(num / ref - 1) < 1e-11
+
+
+def test_dsigma_weak_textbook_cross_sections(orc):
+    c = orc.default_consts()
+    gL, gR = orc.sm_couplings()
+    v, tol = _txt("sigma0_cm2")
+    # T = 0, gR = 0, gL = 1: dsigma/dT = 2 G_F^2 m_e / pi  ->  times m_e = sigma_0
+    assert abs(orc.dsigma_weak(1.0, 0.0, 1.0, 0.0) * c.m_e * HBARC2 / v - 1) < tol
+    for a, name in ((0, "sigma_nue_e_10MeV_cm2"), (1, "sigma_numu_e_10MeV_cm2")):
+        E = 10.0
+        sig, _ = integrate.quad(lambda t: orc.dsigma_weak(E, t, gL[a], gR[a]), 0.0, orc.tmax(E),
+                                epsabs=0, epsrel=1e-12)
+        v, tol = _txt(name)
+        assert abs(sig * HBARC2 / v - 1) < tol
+
+
+def test_dsigma_weak_term_structure(orc):
+    """Each bracket term of Eq.(4) in isolation: gL^2; gR^2 (1-T/E)^2; -gL gR m_e T/E^2."""
+    c = orc.default_consts()
+    C0 = 2 * c.G_F ** 2 * c.m_e / np.pi
+    E, T = 1.7, 0.6
+    assert abs(orc.dsigma_weak(E, T, 0.8, 0.0) / (C0 * 0.64) - 1) < 1e-15
+    assert abs(orc.dsigma_weak(E, T, 0.0, 0.5) / (C0 * 0.25 * (1 - T / E) ** 2) - 1) < 1e-15
+    cross = orc.dsigma_weak(E, T, 0.8, 0.5) - orc.dsigma_weak(E, T, 0.8, 0.0) - orc.dsigma_weak(E, T, 0.0, 0.5)
+    assert abs(cross / (-C0 * 0.4 * c.m_e * T / E ** 2) - 1) < 1e-13
+    assert cross < 0
+
+
+# ----------------------------------------------------------------------------- Eq. (8)
+def test_dsigma_mm_closed_forms(orc):
+    c = orc.default_consts()
+    v, tol = _txt("pi_re2_cm2")
+    # E >> T: T dsigma/dT -> pi alpha^2/m_e^2 mu^2 = pi r_e^2 (mu_nu/mu_B)^2
+    assert abs(orc.dsigma_mm(1e12, 1.0, 1.0) * HBARC2 / v - 1) < tol
+    assert orc.dsigma_mm(0.7, 0.7, 1.0) == 0.0          # bracket 1/T - 1/E vanishes at T = E
+    assert orc.dsigma_mm(0.862, 0.3, 2e-11) == orc.dsigma_mm(0.862, 0.3, -2e-11)   # even in mu_nu
+    assert abs(orc.dsigma_mm(0.862, 0.3, 4e-11) / orc.dsigma_mm(0.862, 0.3, 2e-11) - 4) < 1e-15
+    E, T1, T2, mu = 0.862, 0.01, orc.tmax(0.862), 2.8e-11
+    num, _ = integrate.quad(lambda t: orc.dsigma_mm(E, t, mu), T1, T2, epsabs=0, epsrel=1e-13)
+    Cmm = np.pi * c.alpha_em ** 2 / c.m_e ** 2
+    ref = Cmm * mu ** 2 * (np.log(T2 / T1) - (T2 - T1) / E)
+    assert abs(num / ref - 1) < 1e-11
+
+
+# ----------------------------------------------------------------------------- Eq. (12)
+def _tiny_inputs(seed=5, n_E=6, n_T=9):
+    rng = np.random.default_rng(seed)
+    E = np.sort(rng.uniform(0.3, 3.0, n_E))
+    return dict(E=E, flux_w=rng.uniform(0.5, 2.0, n_E), P_e=rng.uniform(0.3, 0.6, n_E), f_tau=0.37,
+                T=np.sort(rng.uniform(0.02, 2.5, n_T)))
+
+
+def test_spectrum_single_line_reduces_to_dsigma(orc):
+    gL, gR = orc.sm_couplings()
+    E0, fw, Pe = 0.862, 3.7, 0.52
+    T = np.array([0.05, 0.3, 0.66, 0.6649, 0.67, 0.9])
+    inp = dict(E=np.array([E0]), flux_w=np.array([fw]), P_e=np.array([Pe]), f_tau=0.25, T=T)
+    th = orc.theta_vector([0.1, -0.2, 0.05, 0.3, -0.15, 0.02, 2.8e-11], range(7))
+    S = orc.spectrum(inp, th)
+    Pmu, Ptau = (1 - Pe) * 0.75, (1 - Pe) * 0.25
+    for i, t in enumerate(T):
+        if t <= orc.tmax(E0):
+            ref = fw * (Pe * orc.dsigma_weak(E0, t, gL[0] + 0.1, gR[0] - 0.2)
+                        + Pmu * orc.dsigma_weak(E0, t, gL[1] + 0.05, gR[1] + 0.3)
+                        + Ptau * orc.dsigma_weak(E0, t, gL[2] - 0.15, gR[2] + 0.02)
+                        + orc.dsigma_mm(E0, t, 2.8e-11))
+            assert abs(S[i] / ref - 1) < 1e-15
+        else:
+            assert S[i] == 0.0            # kinematic cut: nothing above the Compton edge
+    assert S[4] == 0.0 and S[3] > 0.0     # 0.67 > T_max(0.862) = 0.66492 > 0.6649
+
+
+def test_spectrum_mpmath_brute_force(orc):
+    """Independent-precision brute force on a tiny grid (40 digits)."""
+    mp.mp.dps = 40
+    c = orc.default_consts()
+    inp = _tiny_inputs()
+    th = orc.theta_vector([0.21, -0.13, 0.4, 1.7e-11], [orc.EPS_EE_L, orc.EPS_TT_R, orc.EPS_MM_L, orc.MU_NU])
+    S = orc.spectrum(inp, th)
+    s2, me, GF, al = (mp.mpf(x) for x in (c.sin2_theta_w, c.m_e, c.G_F, c.alpha_em))
+    g = {"e": (mp.mpf(1) / 2 + s2 + mp.mpf(0.21), s2), "m": (-mp.mpf(1) / 2 + s2 + mp.mpf(0.4), s2),
+         "t": (-mp.mpf(1) / 2 + s2, s2 + mp.mpf(-0.13))}
+    C0, Cmm = 2 * GF ** 2 * me / mp.pi, mp.pi * al ** 2 / me ** 2
+    for i, Ti in enumerate(inp["T"]):
+        acc = mp.mpf(0)
+        for j, Ej in enumerate(inp["E"]):
+            Ej_, Ti_ = mp.mpf(Ej), mp.mpf(Ti)
+            if Ti_ > 2 * Ej_ ** 2 / (me + 2 * Ej_):
+                continue
+            Pe = mp.mpf(inp["P_e"][j])
+            P = {"e": Pe, "m": (1 - Pe) * (1 - mp.mpf(0.37)), "t": (1 - Pe) * mp.mpf(0.37)}
+            term = mp.mpf(0)
+            for a in "emt":
+                gL, gR = g[a]
+                term += P[a] * C0 * (gL ** 2 + gR ** 2 * (1 - Ti_ / Ej_) ** 2 - gL * gR * me * Ti_ / Ej_ ** 2)
+            term += Cmm * mp.mpf(1.7e-11) ** 2 * (1 / Ti_ - 1 / Ej_)
+            acc += mp.mpf(inp["flux_w"][j]) * term
+        if acc == 0:
+            assert S[i] == 0.0
+        else:
+            assert abs(S[i] / float(acc) - 1) < 4e-16
+
+
+def test_spectrum_continuum_limit_matches_integrated_cross_section(orc):
+    """sum_i S(T_i) dT -> sum_j flux_w[j] * int_{T_lo}^{T_max(E_j)} dsigma/dT dT (closed forms).
+    A missing kinematic cut, flux weight or flavour factor breaks this at O(1)."""
+    c = orc.default_consts()
+    gL, gR = orc.sm_couplings()
+    rng = np.random.default_rng(11)
+    E = np.array([0.5, 0.862, 1.3, 2.2, 4.0])
+    fw = rng.uniform(0.5, 2.0, E.size)
+    Pe = rng.uniform(0.3, 0.6, E.size)
+    T_lo, T_hi, n_T = 0.05, 4.0, 40000
+    edges = np.linspace(T_lo, T_hi, n_T + 1)
+    T = 0.5 * (edges[1:] + edges[:-1])
+    eps = [0.1, -0.05, 0.2, 0.1, -0.3, 0.15]
+    mu = 5e-11
+    S = orc.spectrum(dict(E=E, flux_w=fw, P_e=Pe, f_tau=0.5, T=T), orc.theta_vector(eps + [mu], range(7)))
+    lhs = S.sum() * (T_hi - T_lo) / n_T
+    Cmm = np.pi * c.alpha_em ** 2 / c.m_e ** 2
+    rhs = 0.0
+    for j in range(E.size):
+        Tm = orc.tmax(E[j])
+        P = (Pe[j], (1 - Pe[j]) * 0.5, (1 - Pe[j]) * 0.5)
+        for a in range(3):
+            l, r = gL[a] + eps[2 * a], gR[a] + eps[2 * a + 1]
+            rhs += fw[j] * P[a] * (_weak_antiderivative(c, E[j], Tm, l, r) - _weak_antiderivative(c, E[j], T_lo, l, r))
+        rhs += fw[j] * Cmm * mu ** 2 * (np.log(Tm / T_lo) - (Tm - T_lo) / E[j])
+    assert abs(lhs / rhs - 1) < 2e-4      # midpoint rule + all-or-nothing edge bins: O(dT)
+
+
+def test_spectrum_is_quadratic_in_eps_and_linear_in_mu2(orc):
+    inp = _tiny_inputs(seed=8, n_E=12, n_T=15)
+    for kind in range(6):
+        S = [orc.spectrum(inp, orc.theta_vector([e, 0.07], [kind, (kind + 1) % 6])) for e in (-0.3, -0.1, 0.1, 0.3)]
+        d3 = S[3] - 3 * S[2] + 3 * S[1] - S[0]
+        assert np.all(np.abs(d3) <= 1e-14 * np.abs(S[3]))
+        d2 = S[2] - 2 * S[1] + S[0]
+        assert np.any(np.abs(d2) > 1e-3 * np.abs(S[1]))   # genuinely quadratic, not linear
+    S0 = orc.spectrum(inp, orc.theta_vector([0.2], [orc.EPS_EE_R]))
+    S1 = orc.spectrum(inp, orc.theta_vector([0.2, 3e-11], [orc.EPS_EE_R, orc.MU_NU]))
+    S2 = orc.spectrum(inp, orc.theta_vector([0.2, 6e-11], [orc.EPS_EE_R, orc.MU_NU]))
+    live = S0 > 0
+    assert np.all(np.abs((S2 - S0)[live] / (S1 - S0)[live] - 4) < 1e-11)
+
+
+def test_spectrum_chirality_sign_flip_symmetry(orc):
+    """(gL,gR) -> (-gL,-gR) leaves Eq.(4) unchanged: eps -> -2g - eps is an exact partner point."""
+    inp = _tiny_inputs(seed=9, n_E=10, n_T=11)
+    gL, gR = orc.sm_couplings()
+    a = orc.theta_vector([0.11, -0.23], [orc.EPS_EE_L, orc.EPS_EE_R])
+    b = orc.theta_vector([-2 * gL[0] - 0.11, -2 * gR[0] + 0.23], [orc.EPS_EE_L, orc.EPS_EE_R])
+    Sa, Sb = orc.spectrum(inp, a), orc.spectrum(inp, b)
+    assert np.all(np.abs(Sa - Sb) <= 4e-16 * np.abs(Sa))
+
+
+def test_spectrum_flavour_routing(orc):
+    """P_e = 1: only eps_ee matters.  P_e = 0, f_tau = 0: only eps_mumu.  f_tau = 1: only eps_tautau."""
+    base = _tiny_inputs(seed=10)
+    for P_e, f_tau, live in ((1.0, 0.5, (0, 1)), (0.0, 0.0, (2, 3)), (0.0, 1.0, (4, 5))):
+        inp = dict(base, P_e=np.full_like(base["E"], P_e), f_tau=f_tau)
+        S0 = orc.spectrum(inp, np.zeros(7))
+        for kind in range(6):
+            S = orc.spectrum(inp, orc.theta_vector([0.2], [kind]))
+            if kind in live:
+                assert np.any(S != S0)
+            else:
+                assert np.array_equal(S, S0)
+
+
+# ----------------------------------------------------------------------------- weights
+def test_weights_are_one_at_sm_point_and_in_dead_bins(orc):
+    inp = _tiny_inputs(seed=12, n_E=8, n_T=30)
+    inp["T"] = np.linspace(0.05, 6.0, 30)          # bins above every T_max are dead
+    w = orc.weights(inp, np.zeros(7))
+    assert np.all(w == 1.0)
+    S0 = orc.spectrum(inp, np.zeros(7))
+    assert np.any(S0 == 0.0) and np.any(S0 > 0.0)
+    th = orc.theta_vector([0.3, 4e-11], [orc.EPS_EE_L, orc.MU_NU])
+    w = orc.weights(inp, th)
+    assert np.all(w[S0 == 0.0] == 1.0)
+    live = S0 > 0
+    assert np.all(np.abs(w[live] / (orc.spectrum(inp, th)[live] / S0[live]) - 1) < 4e-16)
+
+
+# ----------------------------------------------------------------------------- fold
+def test_fold_special_responses_and_library_matmul(orc):
+    rng = np.random.default_rng(3)
+    n_T, n_rec = 37, 23
+    w, N, bkg = rng.uniform(0.5, 1.5, n_T), rng.uniform(1, 100, n_T), rng.uniform(0, 5, n_rec)
+    R = rng.uniform(0, 1, (n_T, n_rec))
+    mu = orc.fold(w, N, R, bkg)
+    ref = (w * N) @ R + bkg                       # library routine on a non-square operand
+    assert np.all(np.abs(mu / ref - 1) < 1e-15)
+    # identity response: mu = N' + B
+    mu_id = orc.fold(w, N, np.eye(n_T), np.arange(n_T, dtype=float))
+    assert np.all(np.abs(mu_id - (w * N + np.arange(n_T))) <= 1e-13)
+    # rank-1 response eff_i * q_k
+    eff, q = rng.uniform(0.8, 1, n_T), rng.dirichlet(np.ones(n_rec))
+    mu_r1 = orc.fold(w, N, np.outer(eff, q), np.zeros(n_rec))
+    assert np.all(np.abs(mu_r1 / (q * np.sum(w * N * eff)) - 1) < 1e-15)
+    # folded total = sum_i w_i N_i * (row efficiency)   (north_star invariant)
+    assert abs((mu - bkg).sum() / np.sum(w * N * R.sum(axis=1)) - 1) < 1e-15
+
+
+# ----------------------------------------------------------------------------- likelihood
+def test_deviance_and_eq18_against_scipy_poisson(orc):
+    rng = np.random.default_rng(4)
+    mu = rng.uniform(0.5, 300.0, 64)
+    n = rng.poisson(mu).astype(float)
+    n[:3] = 0.0
+    full = -2.0 * stats.poisson.logpmf(n, mu).sum()
+    sat = -2.0 * stats.poisson.logpmf(n, np.where(n > 0, n, 1e-300)).sum()
+    assert abs(orc.eq18(mu, n) / full - 1) < 1e-13
+    assert abs(orc.deviance(mu, n) - (full - sat)) < 1e-10 * abs(full)
+    assert orc.deviance(n[3:], n[3:]) == 0.0                       # counts == mu  =>  0
+    assert orc.deviance(np.array([2.5, 0.0]), np.array([0.0, 0.0])) == 5.0   # n = 0 => 2 mu
+    assert orc.deviance(np.array([0.0]), np.array([1.0])) == np.inf
+    # small-d expansion 2[d - n log1p(d/n)] = d^2/n - (2/3) d^3/n^2 + ...
+    nn, d = 1000.0, 1e-3
+    assert abs(orc.deviance(np.array([nn + d]), np.array([nn])) / (d * d / nn - (2.0 / 3) * d ** 3 / nn ** 2) - 1) < 1e-9
+    # non-integer (Asimov) counts are accepted: PAPER.md:309
+    assert orc.deviance(np.array([10.25]), np.array([10.25])) == 0.0
+
+
+# ----------------------------------------------------------------------------- whole path
+def _small_problem(D=2):
+    return wl.make_custom(n_E=19, n_T=41, n_rec=29, n_periods=D, seed=77)
+
+
+def test_eval_batch_is_the_composition_of_its_steps(orc):
+    inp = _small_problem()
+    params, kinds = wl.random_points(5, [orc.EPS_TT_L, orc.MU_NU, orc.EPS_EE_R], seed=2)
+    out, mu, ab = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True)
+    for p in range(5):
+        th = orc.theta_vector(params[p], kinds)
+        w = orc.weights(inp, th)
+        tot = 0.0
+        for d in range(2):
+            m = orc.fold(w, inp["N_mc"][d], inp["R"][d], inp["bkg"][d])
+            assert np.all(np.abs(mu[p, d] / m - 1) < 1e-15)
+            tot += orc.deviance(m, inp["counts"][d])
+        assert abs(out[p] / tot - 1) < 1e-13
+        assert ab[p] >= out[p] > 0
+    # kind order is irrelevant; absent kinds are zero; threads do not change results
+    perm = [2, 0, 1]
+    out2 = orc.eval_batch(inp, params[:, perm], kinds[perm], nthreads=2)
+    assert np.array_equal(out, out2)
+    full = orc.eval_batch(inp, params, kinds, full_eq18=True)
+    sat_const = full - out
+    assert np.all(np.abs(sat_const - sat_const[0]) < 1e-9 * abs(sat_const[0]))   # theta independent
+    with pytest.raises(ValueError):
+        orc.eval_batch(inp, params, [0, 0, 1])
+
+
+def test_rank_K_prefold_identity(orc):
+    """SURVEY finding 0.2: mu - B is linear in the spectrum, so folding basis spectra first gives
+    the same prediction.  Checked with spectra at 3 points of a 1-D quadratic (exact Lagrange)."""
+    inp = _small_problem(D=1)
+    e = np.array([-0.4, 0.0, 0.4])
+    x = 0.17
+    lag = np.array([(x - e[1]) * (x - e[2]) / ((e[0] - e[1]) * (e[0] - e[2])),
+                    (x - e[0]) * (x - e[2]) / ((e[1] - e[0]) * (e[1] - e[2])),
+                    (x - e[0]) * (x - e[1]) / ((e[2] - e[0]) * (e[2] - e[1]))])
+    _, mu_nodes = orc.eval_batch(inp, e[:, None], [orc.EPS_EE_L], want_mu=True)
+    _, mu_x = orc.eval_batch(inp, np.array([[x]]), [orc.EPS_EE_L], want_mu=True)
+    B = inp["bkg"][0]
+    pred = np.tensordot(lag, mu_nodes[:, 0, :] - B, axes=1) + B
+    assert np.all(np.abs(pred / mu_x[0, 0] - 1) < 1e-13)
+
+
+def test_sm_point_gives_sm_prediction(orc):
+    inp = _small_problem(D=2)
+    _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
+    for d in range(2):
+        ref = inp["N_mc"][d] @ inp["R"][d] + inp["bkg"][d]
+        assert np.all(np.abs(mu[0, d] / ref - 1) < 1e-15)
+
+
+@pytest.mark.parametrize("kind,name", [(0, "inject_eps_ee_L"), (6, "inject_mu_nu")])
+def test_asimov_injection_recovery(orc, kind, name):
+    """Asimov data at the injected value => the scan minimum sits there (and is 0)."""
+    inj = float(PAPER[name][0])
+    inp = wl.make("cfg1_tiny_nsi") if kind == 0 else _small_problem(D=1)
+    _, mu = orc.eval_batch(inp, np.array([[inj]]), [kind], want_mu=True)
+    asimov = dict(inp, counts=mu[0])
+    scan = inj * np.linspace(0.0, 2.0, 41)
+    out = orc.eval_batch(asimov, scan[:, None], [kind])
+    assert np.argmin(out) == 20 and abs(out[20]) < 1e-12
+    assert np.all(np.delete(out, 20) > 1e-9)
+
+
+# ----------------------------------------------------------------------------- workloads
+def test_config1_recipe_and_stored_derived_inputs(orc):
+    """BASELINE config 1: the 0.862 MeV line holds 30 % of SM events; the stored S_hat / counts are
+    what the oracle produces today (they are written by oracle/write_derived_inputs.py only)."""
+    inp = wl.make("cfg1_tiny_nsi")
+    zero = np.zeros(7)
+    S = orc.spectrum(inp, zero)
+    line = dict(inp, E=inp["E"][-1:], flux_w=inp["flux_w"][-1:], P_e=inp["P_e"][-1:])
+    assert abs(orc.spectrum(line, zero).sum() / S.sum() - 0.30) < 1e-12
+    assert np.all(np.abs(inp["N_mc"][0] - 1e4 * S / S.sum()) <= 1e-12 * inp["N_mc"][0].max())
+    assert abs(inp["N_mc"].sum() - 1e4) < 1e-8
+    mu_sm = orc.fold(np.ones(100), inp["N_mc"][0], inp["R"][0], inp["bkg"][0])
+    assert np.array_equal(np.random.default_rng(0).poisson(mu_sm), inp["counts"][0])
+    # Gaussian response with efficiency 0.9 (interior rows), flat background 5
+    assert abs(inp["R"][0][50].sum() - 0.9) < 1e-12 and np.all(inp["bkg"] == 5.0)
+    p, kinds = wl.scan_points("cfg1_tiny_nsi")
+    assert p.shape == (121, 2) and list(kinds) == [0, 1] and p.min() == -0.5 and p.max() == 0.5
+
+
+def test_config2_stored_derived_inputs(orc):
+    inp = wl.make("cfg2_mm_lowE")
+    S = orc.spectrum(inp, np.zeros(7))
+    assert np.sum(S == 0.0) > 800          # bins above the 665 keV edge are dead (reading R9)
+    assert np.all(np.abs(inp["N_mc"][0] - 1e5 * S / S.sum()) <= 1e-12 * inp["N_mc"][0].max())
+    p, kinds = wl.scan_points("cfg2_mm_lowE")
+    assert p.shape == (1000, 1) and list(kinds) == [6]
+    assert abs(p[0, 0] / 1e-12 - 1) < 1e-12 and abs(p[-1, 0] / 1e-10 - 1) < 1e-12
