@@ -1,0 +1,150 @@
+/*
+ * rw.h -- C ABI of the B200-native spectrum-reweighting likelihood hot path
+ * (arxiv/paper_2607_00488; citations are PAPER.md:<line> + equation).
+ *
+ * One context (rw_ctx) = the device-resident, theta-independent tables of one analysis
+ * ("initialized once and remain resident on the target device throughout
+ * the fit").  rw_eval_batch runs, for P parameter points, the four steps of one
+ * likelihood call:
+ *   a1  couplings g~ = g + eps (Eq. 6) -> recoil spectrum S_theta(T_i) (Eq. 12,
+ *       PAPER.md:138; Eq. 4/8/9; cut T <= 2E^2/(m_e+2E))
+ *   a2  weights w_i = S_theta/S_SM applied to the MC recoil spectrum (Eq. 14, Eq. 1;
+ *       PAPER.md:151,35)
+ *   a3  fold mu[p,d,k] = sum_i w_i N_mc[d,i] R[d,i,k] + bkg[d,k]  (Eq. 11)
+ *   a4  binned Poisson -2lnL against the counts, summed over periods (Eq. 18)
+ * Every step runs in CUDA kernels (sm_100a); there is no CPU fallback.
+ *
+ * Conventions
+ *   - all functions return 0 (RW_OK) or a negative rw_status; no exception crosses the ABI;
+ *     there is no global state; rw_last_error(ctx) gives a human-readable message.
+ *   - "host"/"device" is stated for every pointer.  Arrays are row-major, FP64.
+ *   - the library never allocates device memory: the caller passes one workspace
+ *     (rw_workspace_bytes) which the context owns until rw_destroy.
+ *   - rw_eval_batch is asynchronous and stream-ordered: it only enqueues work on
+ *     `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and never synchronises,
+ *     except when RW_PARAM_HOST / RW_OUT_HOST ask for pageable/pinned host buffers, in
+ *     which case the copies are enqueued on the same stream (pinned memory => still async).
+ *   - one context must not be used from two streams at once; several contexts may coexist.
+ */
+#ifndef RW_H_
+#define RW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rw_ctx rw_ctx; /* opaque; created by rw_create, freed by rw_destroy */
+
+typedef enum {
+    RW_OK = 0,
+    RW_ERR_INVALID = -1,     /* bad argument / input table (see rw_last_error) */
+    RW_ERR_WORKSPACE = -2,   /* workspace NULL, misaligned or too small */
+    RW_ERR_CUDA = -3,        /* a CUDA runtime/driver call failed */
+    RW_ERR_UNSUPPORTED = -4, /* e.g. not an sm_100 device */
+    RW_ERR_NOMEM = -5        /* host allocation failed */
+} rw_status;
+
+/* parameter kinds: which new-physics parameter a column of param[P][k] holds.
+ * eps_{alpha alpha}^{eL,R} of Eq. (6); mu_nu in Bohr magnetons. */
+enum {
+    RW_EPS_EE_L = 0, RW_EPS_EE_R = 1,
+    RW_EPS_MM_L = 2, RW_EPS_MM_R = 3,
+    RW_EPS_TT_L = 4, RW_EPS_TT_R = 5,
+    RW_MU_NU = 6,
+    RW_N_KINDS = 7
+};
+
+enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
+
+/* rw_eval_batch flags */
+enum {
+    RW_DEVIANCE    = 0u,       /* default: 2 sum [mu - n + n ln(n/mu)] (Eq. 18 minus its saturated value) */
+    RW_FULL_EQ18   = 1u << 0,  /* literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)] */
+    RW_MODE_AUTO   = 0u,       /* P <= 16: streaming fold; else: DMMA batched contraction */
+    RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P) */
+    RW_MODE_GEMM   = 2u << 4,  /* force the FP64 tensor-core (DMMA) contraction */
+    RW_MODE_MASK   = 3u << 4,
+    RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
+    RW_OUT_HOST    = 1u << 9   /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
+};
+
+/* Physical constants.  The paper prints symbols only; any field that is 0
+ * takes the default: sin2_theta_w 0.23121, m_e 0.51099895 MeV, G_F 1.1663788e-11 MeV^-2,
+ * alpha_em 1/137.035999084.  Natural units, MeV. */
+typedef struct {
+    double sin2_theta_w, m_e_MeV, G_F_MeV2, alpha_em;
+} rw_constants;
+
+typedef struct {
+    int32_t n_E;            /* flux-grid entries: continuum cells + lines */
+    const double *E_MeV;    /* [n_E] neutrino energies, > 0 */
+    const double *flux_w;   /* [n_E] phi(E_j)*dE_j >= 0; a line is one entry with its integrated flux */
+    const double *P_e;      /* [n_E] nu_e survival probability in [0,1] */
+    const double *P_mu;     /* [n_E] or NULL -> (1-P_e)(1-f_tau) */
+    const double *P_tau;    /* [n_E] or NULL -> (1-P_e) f_tau */
+    double f_tau;           /* used only when P_mu/P_tau are NULL */
+    int32_t n_T;            /* recoil bins */
+    const double *T_MeV;    /* [n_T] representative recoil energy per bin, > 0 */
+    int32_t n_rec;          /* reconstructed-observable bins */
+    int32_t n_periods;      /* data periods D (>= 1), -2lnL is summed over them */
+    const double *N_mc;     /* [D][n_T]  MC recoil spectrum under the SM, >= 0 */
+    const double *R;        /* [D][n_T][n_rec] conditional response P(rec k | T_i), rec index fastest,
+                               >= 0, sum_k R[i][k] = efficiency_i */
+    const double *bkg;      /* [D][n_rec] theta-independent background, >= 0 */
+    const double *counts;   /* [D][n_rec] observed counts as doubles (Asimov allowed), >= 0 */
+    rw_constants consts;
+    int32_t mem_kind;       /* RW_MEM_HOST: all arrays are host pointers, copied into the workspace.
+                               RW_MEM_DEVICE: all arrays are device pointers; R is borrowed (caller keeps
+                               it alive until rw_destroy) when 16-byte aligned with even n_rec, the
+                               small tables are copied. */
+} rw_inputs;
+
+/* Bytes of device workspace rw_create needs for these inputs and batches of up to max_batch points.
+ * Only the sizes, n_periods and mem_kind fields of `in` are read. */
+int rw_workspace_bytes(const rw_inputs *in, int64_t max_batch, size_t *bytes);
+
+/* Validate inputs, place tables in the workspace, run the setup kernels (basis spectra, S_SM,
+ * pre-scaled basis W^, saturated constant) on `cuda_stream`, and synchronise that stream once.
+ * dev_workspace: device pointer, 256-byte aligned, >= rw_workspace_bytes; owned by ctx until destroy. */
+int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_t workspace_bytes,
+              void *cuda_stream, rw_ctx **out);
+
+/* Replace the observed counts ([D][n_rec], host or device per mem_kind); for toys / Asimov rescans. */
+int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cuda_stream);
+
+/* -2lnL for P points.
+ *   param       [P][k] row-major, device pointer (host if RW_PARAM_HOST)
+ *   param_kind  host [k], distinct values in RW_EPS_EE_L..RW_MU_NU; absent kinds are 0
+ *   out_m2lnL   [P] device pointer (host if RW_OUT_HOST)
+ *   out_mu      NULL, or [P][D][n_rec] predicted counts mu (same memory kind as out_m2lnL)
+ * P may be 0 (no-op) and may exceed max_batch (processed in slices).  Per-point numerical outcomes
+ * are values, not errors: mu_k = 0 with n_k > 0 gives +inf; non-finite parameters give NaN. */
+int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                  double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
+
+/* Device pointers to setup tables, for inspection/tests (valid until rw_destroy):
+ *   RW_TABLE_S_SM   [n_T]        SM recoil spectrum S_SM(T_i) (Eq. 12 at theta = 0)
+ *   RW_TABLE_BASIS  [10][n_T]    basis spectra A_e,B_e,C_e,A_mu,...,C_tau,D
+ *   RW_TABLE_WHAT   [D][12][n_T] pre-scaled basis W^ = basis * N_mc / S_SM (+ dead-bin row) */
+enum { RW_TABLE_S_SM = 0, RW_TABLE_BASIS = 1, RW_TABLE_WHAT = 2 };
+int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64_t *n_elems);
+
+/* Number of kernels this context has launched so far (setup + eval); for bench accounting. */
+int64_t rw_launch_count(const rw_ctx *ctx);
+
+int rw_destroy(rw_ctx *ctx);
+
+const char *rw_strerror(int status);
+const char *rw_last_error(const rw_ctx *ctx); /* ctx may be NULL: last rw_create failure of this thread */
+
+/* Measurement helper (not part of the method): register-resident FP64 issue-rate probe.
+ * kind 0 = DFMA, 1 = DMMA m8n8k4.  Runs on `cuda_stream`, synchronises, returns TFLOP/s. */
+int rw_probe_fp64_peak(int32_t kind, int32_t iters, double *tflops, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RW_H_ */

@@ -1,0 +1,243 @@
+"""Thin ctypes binding of include/rw.h -- argument marshalling only.
+
+Every step of the likelihood path runs in the CUDA kernels of librw.so; PyTorch is used here
+for device memory (the workspace, parameter and output tensors) and the CUDA stream, nothing
+else.  There is no CPU fallback: if librw.so is missing or the device is not sm_100 the calls
+raise.  Names mirror the C ABI: rw_workspace_bytes / rw_create / rw_set_counts /
+rw_eval_batch / rw_get_table / rw_destroy.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librw.so")
+
+# param kinds (include/rw.h)
+RW_EPS_EE_L, RW_EPS_EE_R, RW_EPS_MM_L, RW_EPS_MM_R, RW_EPS_TT_L, RW_EPS_TT_R, RW_MU_NU = range(7)
+RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
+RW_FULL_EQ18 = 1 << 0
+RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM = 0, 1 << 4, 2 << 4
+RW_PARAM_HOST, RW_OUT_HOST = 1 << 8, 1 << 9
+RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT = 0, 1, 2
+_MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM}
+
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
+           "rw_launch_count", "rw_destroy", "rw_strerror", "rw_last_error", "rw_probe_fp64_peak")
+
+_dp = C.POINTER(C.c_double)
+
+
+class rw_constants(C.Structure):
+    _fields_ = [("sin2_theta_w", C.c_double), ("m_e_MeV", C.c_double), ("G_F_MeV2", C.c_double),
+                ("alpha_em", C.c_double)]
+
+
+class rw_inputs(C.Structure):
+    _fields_ = [("n_E", C.c_int32), ("E_MeV", C.c_void_p), ("flux_w", C.c_void_p), ("P_e", C.c_void_p),
+                ("P_mu", C.c_void_p), ("P_tau", C.c_void_p), ("f_tau", C.c_double),
+                ("n_T", C.c_int32), ("T_MeV", C.c_void_p), ("n_rec", C.c_int32), ("n_periods", C.c_int32),
+                ("N_mc", C.c_void_p), ("R", C.c_void_p), ("bkg", C.c_void_p), ("counts", C.c_void_p),
+                ("consts", rw_constants), ("mem_kind", C.c_int32)]
+
+
+class RwError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("rw status %d: %s" % (status, msg))
+        self.status = status
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen librw.so and declare the prototypes.  Fails loudly when the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("%s not found: build it with `python -m paper_2607_00488_b200.build` "
+                           "(there is no CPU fallback)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    L.rw_workspace_bytes.argtypes = [C.POINTER(rw_inputs), C.c_int64, C.POINTER(C.c_size_t)]
+    L.rw_create.argtypes = [C.POINTER(rw_inputs), C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p,
+                            C.POINTER(C.c_void_p)]
+    L.rw_set_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.rw_eval_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32),
+                                C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_get_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
+    L.rw_launch_count.argtypes = [C.c_void_p]
+    L.rw_launch_count.restype = C.c_int64
+    L.rw_destroy.argtypes = [C.c_void_p]
+    L.rw_strerror.argtypes = [C.c_int]
+    L.rw_strerror.restype = C.c_char_p
+    L.rw_last_error.argtypes = [C.c_void_p]
+    L.rw_last_error.restype = C.c_char_p
+    L.rw_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
+    for f in ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
+              "rw_destroy", "rw_probe_fp64_peak"):
+        getattr(L, f).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _stream_ptr():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def probe_fp64_peak(kind, iters=20000):
+    """TFLOP/s of the register-resident FP64 probe (0 = DFMA, 1 = DMMA m8n8k4)."""
+    L = load_library()
+    out = C.c_double(0.0)
+    rc = L.rw_probe_fp64_peak(int(kind), int(iters), C.byref(out), _stream_ptr())
+    if rc != 0:
+        raise RwError(rc, L.rw_strerror(rc).decode())
+    return out.value
+
+
+class Reweighter:
+    """One rw_ctx: device-resident tables of one analysis + its workspace (a torch uint8 tensor).
+
+    `inputs` is a dict with E, flux_w, P_e, [P_mu, P_tau | f_tau], T, N_mc[D][n_T], R[D][n_T][n_rec],
+    bkg[D][n_rec], counts[D][n_rec] as numpy arrays (host: copied at create) or, with
+    tables_on_device=True, CUDA float64 torch tensors (R is borrowed, the rest copied)."""
+
+    def __init__(self, inputs, max_batch, device="cuda:0", consts=None):
+        self._L = load_library()
+        self._ctx = C.c_void_p(None)
+        self.device = torch.device(device)
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2607_00488_b200 needs a CUDA device (sm_100a); no CPU fallback exists")
+        torch.cuda.set_device(self.device)
+        on_device = isinstance(inputs["R"], torch.Tensor)
+        keep = {}
+
+        def arr(name, required=True):
+            v = inputs.get(name)
+            if v is None:
+                if required:
+                    raise KeyError(name)
+                return None
+            if on_device:
+                t = v.to(device=self.device, dtype=torch.float64).contiguous()
+                keep[name] = t
+                return C.c_void_p(t.data_ptr())
+            a = np.ascontiguousarray(v, dtype=np.float64)
+            keep[name] = a
+            return C.c_void_p(a.ctypes.data)
+
+        R = inputs["R"]
+        if R.ndim == 2:
+            R = R[None]
+            inputs = dict(inputs, R=R)
+        D, n_T, n_rec = (int(x) for x in R.shape)
+        inp = rw_inputs()
+        inp.n_E = int(np.prod(inputs["E"].shape))
+        inp.E_MeV, inp.flux_w, inp.P_e = arr("E"), arr("flux_w"), arr("P_e")
+        inp.P_mu, inp.P_tau = arr("P_mu", False), arr("P_tau", False)
+        inp.f_tau = float(inputs.get("f_tau", 0.5))
+        inp.n_T, inp.T_MeV = n_T, arr("T")
+        inp.n_rec, inp.n_periods = n_rec, D
+        inp.N_mc, inp.R, inp.bkg, inp.counts = arr("N_mc"), arr("R"), arr("bkg"), arr("counts")
+        if consts:
+            inp.consts = rw_constants(*[float(consts.get(k, 0.0)) for k in
+                                        ("sin2_theta_w", "m_e_MeV", "G_F_MeV2", "alpha_em")])
+        inp.mem_kind = RW_MEM_DEVICE if on_device else RW_MEM_HOST
+        self.n_E, self.n_T, self.n_rec, self.n_periods = inp.n_E, n_T, n_rec, D
+        self.max_batch = int(max_batch)
+        nbytes = C.c_size_t(0)
+        self._check(self._L.rw_workspace_bytes(C.byref(inp), self.max_batch, C.byref(nbytes)), None)
+        self.workspace = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self._keep = keep            # borrowed device R must outlive the context
+        ctx = C.c_void_p(None)
+        self._check(self._L.rw_create(C.byref(inp), self.max_batch, C.c_void_p(base), nbytes.value,
+                                      _stream_ptr(), C.byref(ctx)), None)
+        self._ctx = ctx
+        if not on_device:
+            self._keep = {}
+
+    # ------------------------------------------------------------------------------------------
+    def _check(self, rc, ctx):
+        if rc != 0:
+            msg = self._L.rw_last_error(ctx).decode() or self._L.rw_strerror(rc).decode()
+            raise RwError(rc, msg)
+
+    def eval_batch(self, param, kinds, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
+        """-2lnL[P] for param[P][k] (CUDA float64 tensor, or numpy/pinned CPU tensor => host path).
+
+        Device params: asynchronous on the current stream, returns a CUDA tensor.
+        Host params: H2D + kernels + D2H are enqueued on the current stream; returns a CPU tensor
+        (pinned), valid after the stream is synchronised."""
+        kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        host = not (isinstance(param, torch.Tensor) and param.is_cuda)
+        if host:
+            if isinstance(param, np.ndarray):
+                param = torch.from_numpy(np.ascontiguousarray(param, dtype=np.float64))
+            param = param.to(torch.float64).contiguous()
+            if param.ndim == 1:
+                param = param[:, None]
+            P, k = param.shape
+            if out is None:
+                out = torch.empty(P, dtype=torch.float64, pin_memory=True)
+            flags |= RW_PARAM_HOST | RW_OUT_HOST
+            if want_mu or out_mu is not None:
+                raise RwError(-4, "out_mu is only available with device-resident params/out")
+        else:
+            param = param.to(torch.float64).contiguous()
+            if param.ndim == 1:
+                param = param[:, None]
+            P, k = param.shape
+            if out is None:
+                out = torch.empty(P, dtype=torch.float64, device=self.device)
+            if want_mu and out_mu is None:
+                out_mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device)
+        assert k == len(kinds), "param has %d columns but %d kinds were given" % (k, len(kinds))
+        rc = self._L.rw_eval_batch(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr,
+                                   C.c_void_p(out.data_ptr()),
+                                   C.c_void_p(out_mu.data_ptr()) if out_mu is not None else None,
+                                   flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = param          # keep alive until the stream has consumed it
+        return (out, out_mu) if (want_mu or out_mu is not None) else out
+
+    def set_counts(self, counts):
+        if isinstance(counts, torch.Tensor) and counts.is_cuda:
+            c = counts.to(torch.float64).contiguous()
+            rc = self._L.rw_set_counts(self._ctx, C.c_void_p(c.data_ptr()), RW_MEM_DEVICE, _stream_ptr())
+        else:
+            c = np.ascontiguousarray(counts.cpu().numpy() if isinstance(counts, torch.Tensor) else counts,
+                                     dtype=np.float64)
+            rc = self._L.rw_set_counts(self._ctx, C.c_void_p(c.ctypes.data), RW_MEM_HOST, _stream_ptr())
+        self._check(rc, self._ctx)
+
+    def table(self, which):
+        """Copy of a setup table as a CUDA tensor (RW_TABLE_S_SM / _BASIS / _WHAT)."""
+        ptr, n = C.c_void_p(None), C.c_int64(0)
+        self._check(self._L.rw_get_table(self._ctx, int(which), C.byref(ptr), C.byref(n)), self._ctx)
+        out = torch.empty(n.value, dtype=torch.float64, device=self.device)
+        torch.cuda.current_stream().synchronize()
+        rc = torch.cuda.cudart().cudaMemcpy(out.data_ptr(), ptr.value, n.value * 8, 3)   # cudaMemcpyDeviceToDevice
+        if int(rc) != 0:
+            raise RuntimeError("cudaMemcpy failed: %s" % rc)
+        return out
+
+    def launch_count(self):
+        return int(self._L.rw_launch_count(self._ctx))
+
+    def close(self):
+        if self._ctx:
+            torch.cuda.synchronize(self.device)
+            self._L.rw_destroy(self._ctx)
+            self._ctx = C.c_void_p(None)
+            self.workspace = None
+            self._keep = {}
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,384 @@
+// rw_api.cu -- the C ABI of include/rw.h: validation, workspace planning, table placement and
+// the stream-ordered launch sequence of one rw_eval_batch.  No arithmetic of the method lives
+// here; every step of the path runs in the kernels of rw_setup/rw_coef/rw_fold_*.cu.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "rw_internal.h"
+
+namespace rw {
+
+static thread_local char g_create_err[512] = "";
+
+int fail(rw_ctx *ctx, int status, const char *fmt, ...)
+{
+    char *dst = ctx ? ctx->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    if (ctx) memcpy(g_create_err, ctx->err, 512);
+    return status;
+}
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+constexpr int kPlanSMs = 148;            // B200; only used to size the streaming-fold row split
+constexpr int64_t kMaxChunkRows = 8192;  // points per contraction chunk (A_packed <= 1 GiB)
+
+static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
+{
+    if (!in || !L) return RW_ERR_INVALID;
+    if (in->n_E <= 0 || in->n_T <= 0 || in->n_rec <= 0 || in->n_periods <= 0 || max_batch <= 0)
+        return RW_ERR_INVALID;
+    if (in->mem_kind != RW_MEM_HOST && in->mem_kind != RW_MEM_DEVICE) return RW_ERR_INVALID;
+    const size_t n_E = in->n_E, n_T = in->n_T, n_rec = in->n_rec, D = in->n_periods;
+    memset(L, 0, sizeof(*L));
+    L->max_batch = max_batch;
+    L->copy_R = (in->mem_kind == RW_MEM_HOST) || (n_rec & 1);
+    L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
+    L->KPAD = (int)((n_T + kBK - 1) / kBK * kBK);
+    int64_t cap = ((int64_t)1 << 30) / ((int64_t)L->KPAD * 8) / kBM * kBM;
+    if (cap < kBM) cap = kBM;
+    if (cap > kMaxChunkRows) cap = kMaxChunkRows;
+    int64_t mc = (max_batch + kBM - 1) / kBM * kBM;
+    L->MC = mc < cap ? mc : cap;
+    L->n_tiles_n = (int)((n_rec + kBN - 1) / kBN);
+    L->stream_strips = (int)((n_rec + kStreamCols - 1) / kStreamCols);
+    int splits = (int)((kPlanSMs * 4 + L->stream_strips * D - 1) / (L->stream_strips * D));
+    int max_splits = (int)((n_T + 63) / 64);
+    if (splits > max_splits) splits = max_splits;
+    if (splits < 1) splits = 1;
+    L->stream_splits = splits;
+    const size_t nstrip2 = (n_rec + 255) / 256;
+    const size_t mu_ld = (n_rec + 1) & ~(size_t)1;
+
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
+    L->E = take(n_E * 8);
+    L->fw = take(n_E * 8);
+    L->P3 = take(3 * n_E * 8);
+    L->T = take(n_T * 8);
+    L->Tmax_invE = take(3 * n_E * 8);
+    L->N_mc = take(D * n_T * 8);
+    L->bkg = take(D * n_rec * 8);
+    L->counts = take(D * n_rec * 8);
+    L->R_copy = take(L->copy_R ? D * n_T * (size_t)L->ldR * 8 : 0);
+    L->basis = take(kNumBasis * n_T * 8);
+    L->S_sm = take(n_T * 8);
+    L->What = take(D * kCoefStride * n_T * 8);
+    L->sat_const = take(8);
+    L->flag = take(4);
+    L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
+    L->coef = take((size_t)max_batch * kCoefStride * 8);
+    L->A_packed = take((size_t)L->MC * L->KPAD * 8);
+    size_t part_gemm = D * (size_t)L->n_tiles_n * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
+    L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
+    L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
+    L->out_stage = take((size_t)max_batch * 8);
+    L->total = off;
+    return RW_OK;
+}
+
+static bool host_bad_nonneg(const double *x, size_t n)
+{
+    for (size_t q = 0; q < n; ++q)
+        if (!(x[q] >= 0.0) || isinf(x[q])) return true;
+    return false;
+}
+static bool host_bad_pos(const double *x, size_t n)
+{
+    for (size_t q = 0; q < n; ++q)
+        if (!(x[q] > 0.0) || isinf(x[q])) return true;
+    return false;
+}
+static bool host_bad_prob(const double *x, size_t n)
+{
+    for (size_t q = 0; q < n; ++q)
+        if (!(x[q] >= 0.0 && x[q] <= 1.0)) return true;
+    return false;
+}
+
+static const char *flag_message(int f)
+{
+    if (f & 1) return "E_MeV must be finite and > 0";
+    if (f & 2) return "flux_w must be finite and >= 0";
+    if (f & 4) return "P_e/P_mu/P_tau must lie in [0,1]";
+    if (f & 8) return "T_MeV must be finite and > 0 (PAPER.md:108)";
+    if (f & 16) return "N_mc must be finite and >= 0";
+    if (f & 32) return "bkg must be finite and >= 0";
+    if (f & 64) return "counts must be finite and >= 0";
+    if (f & 128) return "R must be finite and >= 0";
+    return "invalid input";
+}
+
+}  // namespace rw
+
+using namespace rw;
+
+extern "C" {
+
+int rw_workspace_bytes(const rw_inputs *in, int64_t max_batch, size_t *bytes)
+{
+    Layout L;
+    int rc = plan(in, max_batch, &L);
+    if (rc != RW_OK) return fail(nullptr, rc, "rw_workspace_bytes: invalid sizes/mem_kind/max_batch");
+    if (!bytes) return fail(nullptr, RW_ERR_INVALID, "rw_workspace_bytes: bytes is NULL");
+    *bytes = L.total;
+    return RW_OK;
+}
+
+int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_t workspace_bytes,
+              void *cuda_stream, rw_ctx **out)
+{
+    if (!out) return fail(nullptr, RW_ERR_INVALID, "rw_create: out is NULL");
+    *out = nullptr;
+    Layout L;
+    int rc = plan(in, max_batch, &L);
+    if (rc != RW_OK) return fail(nullptr, rc, "rw_create: invalid sizes/mem_kind/max_batch");
+    if (!in->E_MeV || !in->flux_w || !in->P_e || !in->T_MeV || !in->N_mc || !in->R || !in->bkg || !in->counts)
+        return fail(nullptr, RW_ERR_INVALID, "rw_create: a required input array is NULL");
+    if ((in->P_mu == nullptr) != (in->P_tau == nullptr))
+        return fail(nullptr, RW_ERR_INVALID, "rw_create: P_mu and P_tau must both be given or both be NULL");
+    const bool have_mt = in->P_mu != nullptr;
+    double f_tau = in->f_tau;
+    if (!have_mt && !(f_tau >= 0.0 && f_tau <= 1.0))
+        return fail(nullptr, RW_ERR_INVALID, "rw_create: f_tau must lie in [0,1]");
+    if (!dev_workspace || ((uintptr_t)dev_workspace & 255) || workspace_bytes < L.total)
+        return fail(nullptr, RW_ERR_WORKSPACE, "rw_create: workspace NULL, not 256-byte aligned, or smaller than %zu bytes",
+                    L.total);
+    const rw_constants &k = in->consts;
+    double vals[4] = {k.sin2_theta_w, k.m_e_MeV, k.G_F_MeV2, k.alpha_em};
+    for (double v : vals)
+        if (!(v >= 0.0) || isinf(v)) return fail(nullptr, RW_ERR_INVALID, "rw_create: constants must be finite and >= 0");
+
+    int dev = 0, major = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return fail(nullptr, RW_ERR_CUDA, "rw_create: no usable CUDA device: %s", cudaGetErrorString(cudaGetLastError()));
+    if (major != 10) return fail(nullptr, RW_ERR_UNSUPPORTED, "rw_create: built for sm_100a, device is sm_%d", major * 10);
+
+    const size_t n_E = in->n_E, n_T = in->n_T, n_rec = in->n_rec, D = in->n_periods;
+    const bool host = in->mem_kind == RW_MEM_HOST;
+    if (host) {
+        int f = 0;
+        if (host_bad_pos(in->E_MeV, n_E)) f |= 1;
+        if (host_bad_nonneg(in->flux_w, n_E)) f |= 2;
+        if (host_bad_prob(in->P_e, n_E) || (have_mt && (host_bad_prob(in->P_mu, n_E) || host_bad_prob(in->P_tau, n_E)))) f |= 4;
+        if (host_bad_pos(in->T_MeV, n_T)) f |= 8;
+        if (host_bad_nonneg(in->N_mc, D * n_T)) f |= 16;
+        if (host_bad_nonneg(in->bkg, D * n_rec)) f |= 32;
+        if (host_bad_nonneg(in->counts, D * n_rec)) f |= 64;
+        if (host_bad_nonneg(in->R, D * n_T * n_rec)) f |= 128;
+        if (f) return fail(nullptr, RW_ERR_INVALID, "rw_create: %s", flag_message(f));
+    } else if (!L.copy_R && ((uintptr_t)in->R & 15)) {
+        return fail(nullptr, RW_ERR_INVALID, "rw_create: a borrowed device R must be 16-byte aligned");
+    }
+
+    rw_ctx *ctx = (rw_ctx *)calloc(1, sizeof(rw_ctx));
+    if (!ctx) return fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory");
+    ctx->tmapR = (CUtensorMap *)calloc(D, sizeof(CUtensorMap));
+    if (!ctx->tmapR) { free(ctx); return fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory"); }
+    ctx->n_E = in->n_E; ctx->n_T = in->n_T; ctx->n_rec = in->n_rec; ctx->D = in->n_periods;
+    ctx->lay = L;
+    ctx->num_sms = sms;
+    ctx->ws = (char *)dev_workspace;
+    Consts &c = ctx->cst;
+    c.sin2w = k.sin2_theta_w > 0 ? k.sin2_theta_w : 0.23121;
+    c.m_e = k.m_e_MeV > 0 ? k.m_e_MeV : 0.51099895;
+    c.G_F = k.G_F_MeV2 > 0 ? k.G_F_MeV2 : 1.1663788e-11;
+    c.alpha = k.alpha_em > 0 ? k.alpha_em : 1.0 / 137.035999084;
+    const double pi = 3.14159265358979323846;
+    c.C0 = 2.0 * c.G_F * c.G_F * c.m_e / pi;                 // Eq. (4) prefactor
+    c.Cmm = pi * c.alpha * c.alpha / (c.m_e * c.m_e);        // Eq. (8) prefactor
+    c.gL[0] = 0.5 + c.sin2w;  c.gR[0] = c.sin2w;              // Eq. (2)
+    c.gL[1] = -0.5 + c.sin2w; c.gR[1] = c.sin2w;              // Eq. (3)
+    c.gL[2] = -0.5 + c.sin2w; c.gR[2] = c.sin2w;
+
+    char *ws = ctx->ws;
+    ctx->E = (double *)(ws + L.E);          ctx->fw = (double *)(ws + L.fw);
+    ctx->P3 = (double *)(ws + L.P3);        ctx->T = (double *)(ws + L.T);
+    ctx->Tmax_invE = (double *)(ws + L.Tmax_invE);
+    ctx->N_mc = (double *)(ws + L.N_mc);    ctx->bkg = (double *)(ws + L.bkg);
+    ctx->counts = (double *)(ws + L.counts);
+    ctx->basis = (double *)(ws + L.basis);  ctx->S_sm = (double *)(ws + L.S_sm);
+    ctx->What = (double *)(ws + L.What);    ctx->sat_const = (double *)(ws + L.sat_const);
+    ctx->flag = (int *)(ws + L.flag);
+    ctx->param_stage = (double *)(ws + L.param_stage);
+    ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);
+    ctx->partial = (double *)(ws + L.partial);
+    ctx->mu_part = (double *)(ws + L.mu_part);
+    ctx->out_stage = (double *)(ws + L.out_stage);
+    ctx->ldR = L.ldR;
+    ctx->R_period_stride = n_T * (size_t)L.ldR;
+    ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const cudaMemcpyKind kind = host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+#define RW_TRY(call)                                                                            \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            fail(nullptr, RW_ERR_CUDA, "rw_create: %s failed: %s", #call, cudaGetErrorString(e__)); \
+            free(ctx->tmapR); free(ctx);                                                        \
+            return RW_ERR_CUDA;                                                                 \
+        }                                                                                       \
+    } while (0)
+    RW_TRY(cudaMemcpyAsync(ctx->E, in->E_MeV, n_E * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->fw, in->flux_w, n_E * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->P3, in->P_e, n_E * 8, kind, s));
+    if (have_mt) {
+        RW_TRY(cudaMemcpyAsync(ctx->P3 + n_E, in->P_mu, n_E * 8, kind, s));
+        RW_TRY(cudaMemcpyAsync(ctx->P3 + 2 * n_E, in->P_tau, n_E * 8, kind, s));
+    }
+    RW_TRY(cudaMemcpyAsync(ctx->T, in->T_MeV, n_T * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->N_mc, in->N_mc, D * n_T * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->bkg, in->bkg, D * n_rec * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->counts, in->counts, D * n_rec * 8, kind, s));
+    if (L.copy_R) {
+        if ((size_t)L.ldR != n_rec) RW_TRY(cudaMemsetAsync(ws + L.R_copy, 0, D * n_T * (size_t)L.ldR * 8, s));
+        RW_TRY(cudaMemcpy2DAsync(ws + L.R_copy, (size_t)L.ldR * 8, in->R, n_rec * 8, n_rec * 8, D * n_T, kind, s));
+    }
+    RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
+    RW_TRY(launch_flavour(ctx, have_mt ? 1 : 0, f_tau, s));
+    if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
+    RW_TRY(launch_setup(ctx, s));
+    RW_TRY(launch_sat_const(ctx, s));
+    int flag = 0;
+    RW_TRY(cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
+    RW_TRY(cudaStreamSynchronize(s));
+#undef RW_TRY
+    if (flag) {
+        fail(nullptr, RW_ERR_INVALID, "rw_create: %s", flag_message(flag));
+        free(ctx->tmapR); free(ctx);
+        return RW_ERR_INVALID;
+    }
+    rc = make_tensor_maps(ctx);
+    if (rc != RW_OK) { free(ctx->tmapR); free(ctx); return rc; }
+    ctx->err[0] = 0;
+    *out = ctx;
+    return RW_OK;
+}
+
+int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_set_counts: ctx is NULL");
+    if (!counts || (mem_kind != RW_MEM_HOST && mem_kind != RW_MEM_DEVICE))
+        return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts NULL or bad mem_kind");
+    const size_t n = (size_t)ctx->D * ctx->n_rec;
+    if (mem_kind == RW_MEM_HOST && host_bad_nonneg(counts, n))
+        return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts must be finite and >= 0");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    RW_CUDA(ctx, cudaMemsetAsync(ctx->flag, 0, 4, s));
+    RW_CUDA(ctx, cudaMemcpyAsync(ctx->counts, counts, n * 8,
+                                 mem_kind == RW_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
+    RW_CUDA(ctx, launch_sat_const(ctx, s));
+    int flag = 0;
+    RW_CUDA(ctx, cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
+    RW_CUDA(ctx, cudaStreamSynchronize(s));
+    if (flag) return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts must be finite and >= 0");
+    return RW_OK;
+}
+
+int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                  double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_batch: ctx is NULL");
+    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: P < 0 or k outside [0,7]");
+    if (P == 0) return RW_OK;
+    if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param, param_kind or out_m2lnL is NULL");
+    int kinds[RW_N_KINDS];
+    for (int a = 0; a < k; ++a) {
+        kinds[a] = param_kind[a];
+        if (kinds[a] < 0 || kinds[a] >= RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param_kind[%d] = %d out of range", a, kinds[a]);
+        for (int b = 0; b < a; ++b)
+            if (kinds[b] == kinds[a]) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: duplicate param_kind %d", kinds[a]);
+    }
+    const uint32_t mode = flags & RW_MODE_MASK;
+    if (mode == RW_MODE_MASK) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: bad mode flags");
+    const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
+    if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Layout &L = ctx->lay;
+    const int D = ctx->D, n_rec = ctx->n_rec;
+    for (int64_t s0 = 0; s0 < P; s0 += L.max_batch) {
+        const int64_t Ps = (P - s0 < L.max_batch) ? P - s0 : L.max_batch;
+        const double *dparam = nullptr;
+        if (k > 0) {
+            dparam = param + s0 * k;
+            if (param_host) {
+                RW_CUDA(ctx, cudaMemcpyAsync(ctx->param_stage, dparam, (size_t)Ps * k * 8, cudaMemcpyHostToDevice, s));
+                dparam = ctx->param_stage;
+            }
+        }
+        double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
+        RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
+        const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && Ps <= 32);
+        if (stream_mode) {
+            const int nstrip2 = (n_rec + 255) / 256;
+            for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
+                const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
+                double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
+                RW_CUDA(ctx, launch_fold_stream(ctx, g0, Pb, mu, s));
+                RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, dout + g0, full, s));
+            }
+        } else {
+            for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
+                const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
+                double *mu = out_mu ? out_mu + (size_t)(s0 + c0) * D * n_rec : nullptr;
+                for (int d = 0; d < D; ++d) {
+                    RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
+                    RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                }
+                RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, dout + c0, full, s));
+            }
+        }
+        if (out_host)
+            RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
+    }
+    return RW_OK;
+}
+
+int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64_t *n_elems)
+{
+    if (!ctx || !dev_ptr || !n_elems) return RW_ERR_INVALID;
+    switch (which) {
+    case RW_TABLE_S_SM: *dev_ptr = ctx->S_sm; *n_elems = ctx->n_T; return RW_OK;
+    case RW_TABLE_BASIS: *dev_ptr = ctx->basis; *n_elems = (int64_t)kNumBasis * ctx->n_T; return RW_OK;
+    case RW_TABLE_WHAT: *dev_ptr = ctx->What; *n_elems = (int64_t)ctx->D * kCoefStride * ctx->n_T; return RW_OK;
+    default: return RW_ERR_INVALID;
+    }
+}
+
+int64_t rw_launch_count(const rw_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int rw_destroy(rw_ctx *ctx)
+{
+    if (!ctx) return RW_OK;
+    free(ctx->tmapR);
+    free(ctx);
+    return RW_OK;
+}
+
+const char *rw_strerror(int status)
+{
+    switch (status) {
+    case RW_OK: return "ok";
+    case RW_ERR_INVALID: return "invalid argument or input table";
+    case RW_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case RW_ERR_CUDA: return "CUDA call failed";
+    case RW_ERR_UNSUPPORTED: return "unsupported device or option";
+    case RW_ERR_NOMEM: return "out of host memory";
+    default: return "unknown status";
+    }
+}
+
+const char *rw_last_error(const rw_ctx *ctx) { return ctx ? ctx->err : g_create_err; }
+
+}  // extern "C"

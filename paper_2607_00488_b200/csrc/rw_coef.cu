@@ -1,0 +1,113 @@
+// rw_coef.cu -- steps a1 + a2: per-point coefficients and the reweighted MC spectrum.
+//
+//   k_coef    param[P][k] -> coef[P][12]:  g~ = g + eps (Eq. 6), then the monomials the
+//             cross section is polynomial in: g~L^2, g~R^2, g~L g~R per flavour (Eq. 4/7,
+//             PAPER.md:65,83) and mu_nu^2 (Eq. 8-9)
+//   k_gen_A   N'[p][i] = w_i(theta_p) N_mc[i] = sum_b coef[p][b] W^[b][i]  (Eq. 14 and the
+//             diag(r) E_true of Eq. 1), written in the 8x8-blocked layout the
+//             DMMA contraction reads (rw_fold_gemm.cu).  Materialised once per (chunk, period):
+//             regenerating it per output tile would redo these flops n_rec/128 times.
+#include "rw_internal.h"
+
+namespace rw {
+
+struct Kinds { int k; int kind[RW_N_KINDS]; };
+
+__global__ void k_coef(const double *__restrict__ param, int64_t P, Kinds kd, Consts cst,
+                       double *__restrict__ coef)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    double th[RW_N_KINDS];
+#pragma unroll
+    for (int q = 0; q < RW_N_KINDS; ++q) th[q] = 0.0;
+    for (int a = 0; a < kd.k; ++a) {
+        double v = param[p * kd.k + a];
+#pragma unroll
+        for (int q = 0; q < RW_N_KINDS; ++q)
+            if (kd.kind[a] == q) th[q] = v;
+    }
+    double *c = coef + p * kCoefStride;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double gl = cst.gL[a] + th[2 * a], gr = cst.gR[a] + th[2 * a + 1];
+        c[3 * a + 0] = gl * gl;
+        c[3 * a + 1] = gr * gr;
+        c[3 * a + 2] = gl * gr;
+    }
+    c[9] = th[RW_MU_NU] * th[RW_MU_NU];
+    c[10] = 1.0;
+    c[11] = 0.0;
+}
+
+constexpr int kGenThreads = 256;   // 32 row-blocks of 8 points
+constexpr int kGenKT = 128;        // recoil bins staged per CTA
+
+// A_packed[mb][kb][r][kk] = N'[p0 + 8 mb + r][8 kb + kk]; rows >= Pc and bins >= n_T are zero.
+__global__ void __launch_bounds__(kGenThreads)
+k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pad,
+        const double *__restrict__ What /*[12][n_T] of this period*/, int n_T, int KPAD,
+        double *__restrict__ A)
+{
+    __shared__ __align__(16) double sW[kNumTerms][kGenKT];
+    const int k0 = blockIdx.y * kGenKT;
+    for (int q = threadIdx.x; q < kNumTerms * kGenKT; q += kGenThreads) {
+        int b = q / kGenKT, kk = q - b * kGenKT;
+        int i = k0 + kk;
+        sW[b][kk] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;
+    }
+    __syncthreads();
+    const int r = threadIdx.x & 7;
+    const int64_t mb = blockIdx.x * (int64_t)(kGenThreads / 8) + (threadIdx.x >> 3);
+    const int64_t row = mb * 8 + r;
+    if (row >= rows_pad) return;
+    double c[kNumTerms];
+    const bool valid = row < Pc;
+#pragma unroll
+    for (int b = 0; b < kNumTerms; ++b) c[b] = valid ? coef[(p0 + row) * kCoefStride + b] : 0.0;
+    const int KB = KPAD / 8;
+    const int nkb = min(kGenKT, KPAD - k0) / 8;
+    for (int kb = 0; kb < nkb; ++kb) {
+        double v[8];
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) v[kk] = 0.0;
+#pragma unroll
+        for (int b = 0; b < kNumTerms; ++b) {
+            const double2 *w2 = reinterpret_cast<const double2 *>(&sW[b][kb * 8]);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                double2 w = w2[h];
+                v[2 * h] = fma(c[b], w.x, v[2 * h]);
+                v[2 * h + 1] = fma(c[b], w.y, v[2 * h + 1]);
+            }
+        }
+        double2 *dst = reinterpret_cast<double2 *>(A + ((mb * KB + (k0 / 8 + kb)) * 64 + r * 8));
+#pragma unroll
+        for (int h = 0; h < 4; ++h) dst[h] = make_double2(v[2 * h], v[2 * h + 1]);
+    }
+}
+
+cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
+                        cudaStream_t s)
+{
+    Kinds kd;
+    kd.k = k;
+    for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
+    k_coef<<<(unsigned)((P + 127) / 128), 128, 0, s>>>(param, P, kd, ctx->cst, ctx->coef);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_t s)
+{
+    const int64_t rows_pad = (Pc + kBM - 1) / kBM * kBM;
+    dim3 grid((unsigned)((rows_pad + kGenThreads - 1) / kGenThreads),
+              (unsigned)((ctx->lay.KPAD + kGenKT - 1) / kGenKT));
+    k_gen_A<<<grid, kGenThreads, 0, s>>>(ctx->coef, p0, Pc, rows_pad,
+                                         ctx->What + (size_t)d * kCoefStride * ctx->n_T, ctx->n_T,
+                                         ctx->lay.KPAD, ctx->A_packed);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace rw

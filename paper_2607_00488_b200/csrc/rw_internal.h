@@ -1,0 +1,124 @@
+// rw_internal.h -- private declarations shared by the translation units of librw.so.
+// Nothing here is visible through the C ABI (include/rw.h), and nothing under oracle/
+// includes it.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/rw.h"
+
+namespace rw {
+
+// ---- basis / coefficient layout -----------------------------------------
+// dsigma of Eq. (4) is quadratic in (g~L, g~R) per flavour and Eq. (8) is linear in mu_nu^2, so
+//   S_theta(T_i) = sum_b c_b(theta) * Basis_b(T_i),   b = 0..9
+//   b = 3a+0: g~L_a^2   b = 3a+1: g~R_a^2   b = 3a+2: g~L_a g~R_a   (a = e, mu, tau)   b = 9: mu_nu^2
+// Row 10 carries coefficient 1 and holds N_mc in dead bins (S_SM = 0 => w := 1); row 11 is padding.
+constexpr int kNumBasis = 10;
+constexpr int kCoefStride = 12;   // doubles per point in coef[P][12] and rows per period in What[D][12][n_T]
+constexpr int kNumTerms = 11;     // rows of What that are ever non-zero
+
+// ---- DMMA contraction tile geometry (rw_fold_gemm.cu) ------------------------------------------
+constexpr int kBM = 128;          // points per CTA tile
+constexpr int kBN = 128;          // reconstructed bins per CTA tile
+constexpr int kBK = 16;           // recoil bins per pipeline stage
+constexpr int kStages = 6;
+constexpr int kGemmConsumerWarps = 8;
+constexpr int kGemmThreads = (kGemmConsumerWarps + 1) * 32;   // + 1 TMA producer warp
+
+// ---- streaming fold geometry (rw_fold_stream.cu) -----------------------------------------------
+constexpr int kStreamThreads = 256;
+constexpr int kStreamCols = 2 * kStreamThreads;   // columns per CTA strip (one double2 per thread)
+constexpr int kStreamMaxPB = 16;                  // points folded per pass over R
+
+struct Consts {
+    double sin2w, m_e, G_F, alpha;
+    double C0;        // 2 G_F^2 m_e / pi        (Eq. 4 prefactor)
+    double Cmm;       // pi alpha^2 / m_e^2      (Eq. 8 prefactor)
+    double gL[3], gR[3];   // Eq. (2)-(3)
+};
+
+struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
+    size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
+    size_t basis, S_sm, What, sat_const, flag;
+    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage;
+    size_t total;
+    int ldR;              // row pitch of the workspace copy of R (doubles)
+    int KPAD;             // n_T rounded up to kBK
+    int64_t MC;           // points per GEMM chunk (multiple of kBM)
+    int n_tiles_n;        // ceil(n_rec / kBN)
+    int stream_strips;    // ceil(n_rec / kStreamCols)
+    int stream_splits;    // row splits of the streaming fold
+    int64_t max_batch;
+    bool copy_R;
+};
+
+}  // namespace rw
+
+struct rw_ctx {
+    int n_E, n_T, n_rec, D;
+    rw::Consts cst;
+    rw::Layout lay;
+    char *ws;                 // device workspace base
+    // device tables
+    double *E, *fw, *P3, *T, *Tmax_invE, *N_mc, *bkg, *counts;
+    const double *R;          // [D][n_T][ldR]
+    int ldR;
+    size_t R_period_stride;   // doubles between periods
+    double *basis, *S_sm, *What, *sat_const;
+    int *flag;
+    // per-call scratch
+    double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
+    CUtensorMap *tmapR;       // host array [D]
+    CUtensorMap tmapA;
+    int num_sms;
+    int64_t launches;
+    char err[512];
+};
+
+namespace rw {
+
+// error helpers -----------------------------------------------------------------------------------
+int fail(rw_ctx *ctx, int status, const char *fmt, ...);
+#define RW_CUDA(ctx, call)                                                                   \
+    do {                                                                                     \
+        cudaError_t e__ = (call);                                                            \
+        if (e__ != cudaSuccess)                                                              \
+            return rw::fail((ctx), RW_ERR_CUDA, "%s failed: %s (%s:%d)", #call,              \
+                            cudaGetErrorString(e__), __FILE__, __LINE__);                    \
+    } while (0)
+
+// kernels' host launchers (each returns a cudaError_t from the launch) ---------------------------
+cudaError_t launch_setup(rw_ctx *ctx, cudaStream_t s);                       // rw_setup.cu
+cudaError_t launch_sat_const(rw_ctx *ctx, cudaStream_t s);                   // rw_setup.cu
+cudaError_t launch_validate_device(rw_ctx *ctx, const double *R_src, int ld_src,
+                                   size_t period_stride_src, cudaStream_t s); // rw_setup.cu
+cudaError_t launch_flavour(rw_ctx *ctx, int have_mu_tau, double f_tau, cudaStream_t s);  // rw_setup.cu
+cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
+                        cudaStream_t s);                                     // rw_coef.cu
+cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_t s);   // rw_coef.cu
+cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int64_t mu_p0,
+                             cudaStream_t s);                                // rw_fold_gemm.cu
+cudaError_t launch_fold_stream(rw_ctx *ctx, int64_t p0, int Pb, double *out_mu,
+                               cudaStream_t s);                              // rw_fold_stream.cu
+cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
+                          bool full_eq18, cudaStream_t s);                   // rw_fold_stream.cu
+int make_tensor_maps(rw_ctx *ctx);                                           // rw_fold_gemm.cu
+
+// Poisson term of Eq. (18) relative to its saturated value: mu - n + n ln(n/mu) (x2 applied later).
+__device__ __forceinline__ double poisson_term(double mu, double n)
+{
+    if (n > 0.0) {
+        if (mu > 0.0) {
+            double d = mu - n;
+            return d - n * log1p(d / n);
+        }
+        return (mu == mu) ? __longlong_as_double(0x7ff0000000000000LL) : mu;   // +inf, NaN stays NaN
+    }
+    return mu;
+}
+
+}  // namespace rw
