@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- likelihood evaluations per second on BASELINE.json's dense-contraction config.
+
+One *step* = one pass of the whole hot path (coefficients -> reweighted MC spectrum -> response
+fold -> Poisson -2lnL) over one batch of the config's scan points.  Default workload: config 4
+("cfg4_dense": 16384 recoil bins x 8192 reconstructed bins, 1.07 GB FP64 response, 65536 points),
+the configuration the batched-throughput metric is quoted on; the others are parity cases.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config NAME]
+
+N > 1 is launched by torchrun (one rank per GPU); the points are sharded, the tables replicated,
+there is no data-path collective (weak scaling: every rank folds its own 65536-point batch).
+`--impl reference` times the CPU oracle (oracle/) on the box's host cores -- a deliberately slow,
+plain program; see DESIGN.md section 8.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "likelihood evals/sec (batched)"
+UNIT = "evals/s"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per k_fold_gemm launch from the committed
+# `ncu --set full` capture (profiles/r01_fold_gemm_full.md), or None if not captured yet.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": None}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=p["hbm_gbs"], bf16=p["bf16_tflops"], bf16_sus=p.get("bf16_tflops_sustained"),
+                    source="measured")
+    return dict(hbm_gbs=6650.0, bf16=1590.0, bf16_sus=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        out = self.proc.communicate()[0]
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def rank_points(wl, name, rank):
+    """Rank 0 folds the config's own scan; further ranks an independent seeded draw of the same shape."""
+    params, kinds = wl.scan_points(name)
+    if rank > 0:
+        params, kinds = wl.random_points(params.shape[0], kinds, seed=100003 * rank + 7)
+    return np.ascontiguousarray(params), kinds
+
+
+def oracle_sample_run(name, n_points, nthreads, repeats=1):
+    """Times the oracle as it stands on the first n_points scan points; returns (evals/s, seconds)."""
+    from oracle import rw_oracle as orc
+    from paper_2607_00488_b200 import workloads as wl
+    inp = wl.make(name)
+    params, kinds = wl.scan_points(name)
+    sample = params[:n_points]
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        orc.eval_batch(inp, sample, kinds, nthreads=nthreads)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return n_points / best, best
+
+
+def run_reference(args, rank, world):
+    """CPU oracle arm: rank 0 alone works; each step folds a bounded sample of the config."""
+    if rank != 0:
+        return
+    from oracle import rw_oracle as orc
+    from paper_2607_00488_b200 import workloads as wl
+    orc.build()
+    cores = os.cpu_count() or 1
+    name = args.config
+    inp = wl.make(name)
+    params, kinds = wl.scan_points(name)
+    n_sample = max(1, min(params.shape[0], cores))        # one point per core and step
+    for w in range(args.warmup):
+        orc.eval_batch(inp, params[:n_sample], kinds, nthreads=cores)
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        lo = (s * n_sample) % max(1, params.shape[0] - n_sample + 1)
+        orc.eval_batch(inp, params[lo:lo + n_sample], kinds, nthreads=cores)
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    sample = "%d scan points per step (of %d), OpenMP over points on %d threads" % (n_sample, params.shape[0], cores)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(name, inp, params.shape[0], args.gpus, sample=sample),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(name, inp, P, n_gpus, sample=None):
+    D, n_T, n_rec = inp["R"].shape
+    cfg = {"workload": name, "n_E": int(inp["E"].size), "n_T": int(n_T), "n_rec": int(n_rec), "n_periods": int(D),
+           "points_per_step_per_gpu": int(P), "response_bytes": int(D * n_T * n_rec * 8),
+           "parallelism": "points sharded over %d GPU(s), tables replicated, no collective" % n_gpus,
+           "l2": "response (%.2f GB) and reweighted spectrum exceed the 126 MB L2: no flush needed" % (D * n_T * n_rec * 8 / 1e9)}
+    if sample:
+        cfg["sample"] = sample
+    return cfg
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg4_dense")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2607_00488_b200 import binding, workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.load_library()
+    name = args.config
+    inp = wl.make(name)
+    D, n_T, n_rec = inp["R"].shape
+    params, kinds = rank_points(wl, name, rank)
+    P, k = params.shape
+
+    # tables resident in HBM before anything is timed (R is borrowed by the context, not copied)
+    dev_inp = {key: torch.from_numpy(np.ascontiguousarray(inp[key])).to(dev)
+               for key in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
+    dev_inp["f_tau"] = inp["f_tau"]
+    ctx = binding.Reweighter(dev_inp, max_batch=P, device=dev)
+    param_dev = torch.from_numpy(params).to(dev)
+    out_dev = torch.empty(P, dtype=torch.float64, device=dev)
+    param_pin = torch.from_numpy(params).pin_memory()
+    out_pin = torch.empty(P, dtype=torch.float64).pin_memory()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def maxreduce(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---------------------------------------------------------------- device-resident throughput
+    for _ in range(args.warmup):
+        ctx.eval_batch(param_dev, kinds, out=out_dev)
+    barrier()
+    sampler = ClockSampler("GPU-" + str(torch.cuda.get_device_properties(dev).uuid))
+    if rank == 0:
+        sampler.start()
+    launches0 = ctx.launch_count()
+    ctx.profile_begin()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        ctx.eval_batch(param_dev, kinds, out=out_dev)
+    e1.record()
+    barrier()
+    ms = maxreduce(e0.elapsed_time(e1))
+    fold_ms, fold_launches = ctx.profile_end()
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    value = world * P * args.steps / (ms * 1e-3)
+    finite = bool(torch.isfinite(out_dev).all().item())
+
+    # ---------------------------------------------------------------- end to end with host buffers
+    for _ in range(2):
+        ctx.eval_batch(param_pin, kinds, out=out_pin)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        ctx.eval_batch(param_pin, kinds, out=out_pin)     # H2D params, kernels, D2H -2lnL: all on the stream
+    e1.record()
+    barrier()
+    ms_e2e = maxreduce(e0.elapsed_time(e1))
+    e2e_value = world * P * args.steps / (ms_e2e * 1e-3)
+    same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
+
+    # ---------------------------------------------------------------- single evaluation (HBM-bound regime)
+    one = param_dev[:1].contiguous()
+    out1 = torch.empty(1, dtype=torch.float64, device=dev)
+    for _ in range(5):
+        ctx.eval_batch(one, kinds, out=out1, mode="stream")
+    torch.cuda.synchronize()
+    reps = 30
+    ctx.profile_begin()
+    e0.record()
+    for _ in range(reps):
+        ctx.eval_batch(one, kinds, out=out1, mode="stream")
+    e1.record()
+    torch.cuda.synchronize()
+    single_ms = e0.elapsed_time(e1) / reps
+    sfold_ms, sfold_n = ctx.profile_end()
+    peaks = load_peaks()
+    r_bytes = D * n_T * n_rec * 8
+    single = {"ms_per_eval": single_ms, "fold_kernel_ms": sfold_ms / max(1, sfold_n),
+              "hbm_gbs": r_bytes / (sfold_ms / max(1, sfold_n) * 1e-3) / 1e9,
+              "hbm_peak_gbs": peaks["hbm_gbs"], "note": "P=1, streaming fold; R (%.2f GB) >> L2, so every eval reads it from HBM" % (r_bytes / 1e9)}
+    single["hbm_frac"] = single["hbm_gbs"] / peaks["hbm_gbs"]
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel
+    dmma_peak = binding.probe_fp64_peak(1)
+    dfma_peak = binding.probe_fp64_peak(0)
+    flops_timed = 2.0 * n_T * n_rec * D * P * args.steps           # algorithmic: 2 N_T N_rec per point and period
+    achieved = flops_timed / (fold_ms * 1e-3) / 1e12
+    traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(name)
+    roofline = {"bound": "tensor", "kernel": "k_fold_gemm", "achieved": achieved, "peak": dmma_peak, "unit": "TFLOP/s",
+                "frac": achieved / dmma_peak, "traffic": traffic,
+                "peak_source": "FP64 DMMA.8x8x4 issue-rate probe measured live (rw_probe_fp64_peak); DFMA probe %.2f; "
+                               "bf16 %s peak x nominal FP64/bf16 ratio (45/2250) = %.1f burst / %.1f sustained"
+                               % (dfma_peak, peaks["source"], peaks["bf16"] * 0.02, (peaks["bf16_sus"] or 0) * 0.02),
+                "launches_timed": int(fold_launches), "avg_launch_ms": fold_ms / max(1, fold_launches),
+                "flops_per_launch": flops_timed / max(1, fold_launches),
+                "kernel_share_of_step": fold_ms / ms}
+
+    # ---------------------------------------------------------------- CPU oracle beside it
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import rw_oracle as orc
+        orc.build()
+        cores = os.cpu_count() or 1
+        n_sample = min(P, 4 * cores)
+        v, secs = oracle_sample_run(name, n_sample, cores)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "first %d of %d scan points, OpenMP over points on %d threads, %.1f s wall" % (n_sample, P, cores, secs)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": workload_config(name, inp, P, world),
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(P * k * 8),
+                        "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
+                        "matches_device_path": same},
+                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
+                "clocks": clocks, "all_finite": finite,
+                "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
+                                 "the authors' own multi-component model; other hardware and inputs, not comparable"}
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

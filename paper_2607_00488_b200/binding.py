@@ -25,7 +25,8 @@ RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT = 0, 1, 2
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM}
 
 EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
-           "rw_launch_count", "rw_destroy", "rw_strerror", "rw_last_error", "rw_probe_fp64_peak")
+           "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
+           "rw_last_error", "rw_probe_fp64_peak")
 
 _dp = C.POINTER(C.c_double)
 
@@ -71,13 +72,15 @@ def load_library():
     L.rw_launch_count.argtypes = [C.c_void_p]
     L.rw_launch_count.restype = C.c_int64
     L.rw_destroy.argtypes = [C.c_void_p]
+    L.rw_profile_begin.argtypes = [C.c_void_p]
+    L.rw_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.rw_strerror.argtypes = [C.c_int]
     L.rw_strerror.restype = C.c_char_p
     L.rw_last_error.argtypes = [C.c_void_p]
     L.rw_last_error.restype = C.c_char_p
     L.rw_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
     for f in ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
-              "rw_destroy", "rw_probe_fp64_peak"):
+              "rw_destroy", "rw_probe_fp64_peak", "rw_profile_begin", "rw_profile_end"):
         getattr(L, f).restype = C.c_int
     _lib = L
     return L
@@ -224,6 +227,15 @@ class Reweighter:
         if int(rc) != 0:
             raise RuntimeError("cudaMemcpy failed: %s" % rc)
         return out
+
+    def profile_begin(self):
+        self._check(self._L.rw_profile_begin(self._ctx), self._ctx)
+
+    def profile_end(self):
+        """(summed fold-kernel ms, launches timed) since profile_begin; synchronises."""
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        self._check(self._L.rw_profile_end(self._ctx, C.byref(ms), C.byref(n)), self._ctx)
+        return ms.value, n.value
 
     def launch_count(self):
         return int(self._L.rw_launch_count(self._ctx))

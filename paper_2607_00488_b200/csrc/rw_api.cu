@@ -358,9 +358,44 @@ int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64
 
 int64_t rw_launch_count(const rw_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
+int rw_profile_begin(rw_ctx *ctx)
+{
+    if (!ctx) return RW_ERR_INVALID;
+    if (!ctx->prof_ev) {
+        const int cap = 4096;
+        ctx->prof_ev = (cudaEvent_t *)calloc(2 * cap, sizeof(cudaEvent_t));
+        if (!ctx->prof_ev) return fail(ctx, RW_ERR_NOMEM, "rw_profile_begin: out of host memory");
+        for (int q = 0; q < 2 * cap; ++q) RW_CUDA(ctx, cudaEventCreate(&ctx->prof_ev[q]));
+        ctx->prof_cap = cap;
+    }
+    ctx->prof_n = 0;
+    ctx->profiling = true;
+    return RW_OK;
+}
+
+int rw_profile_end(rw_ctx *ctx, double *fold_ms_total, int64_t *fold_launches)
+{
+    if (!ctx || !fold_ms_total || !fold_launches) return RW_ERR_INVALID;
+    ctx->profiling = false;
+    double total = 0.0;
+    for (int q = 0; q < ctx->prof_n; ++q) {
+        float ms = 0.f;
+        RW_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[2 * q + 1]));
+        RW_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->prof_ev[2 * q], ctx->prof_ev[2 * q + 1]));
+        total += ms;
+    }
+    *fold_ms_total = total;
+    *fold_launches = ctx->prof_n;
+    return RW_OK;
+}
+
 int rw_destroy(rw_ctx *ctx)
 {
     if (!ctx) return RW_OK;
+    if (ctx->prof_ev) {
+        for (int q = 0; q < 2 * ctx->prof_cap; ++q) cudaEventDestroy(ctx->prof_ev[q]);
+        free(ctx->prof_ev);
+    }
     free(ctx->tmapR);
     free(ctx);
     return RW_OK;

@@ -298,6 +298,7 @@ cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int
     const int total = tiles_m * tiles_n;
     const int grid = total < ctx->num_sms ? total : ctx->num_sms;
     double *part = ctx->partial + (size_t)d * tiles_n * L.MC;
+    ProfScope prof(ctx, s);
     k_fold_gemm<<<grid, kGemmThreads, kGemmSmem, s>>>(
         ctx->tmapA, ctx->tmapR[d], ctx->n_T, ctx->n_rec, Pc, tiles_m, tiles_n,
         ctx->bkg + (size_t)d * ctx->n_rec, ctx->counts + (size_t)d * ctx->n_rec, part, L.MC, out_mu, ctx->D, d);

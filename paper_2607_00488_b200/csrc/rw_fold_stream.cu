@@ -146,11 +146,14 @@ cudaError_t launch_fold_stream(rw_ctx *ctx, int64_t p0, int Pb, double *out_mu, 
 {
     const Layout &L = ctx->lay;
     int PB;
-    if (Pb <= 1) { PB = 1; launch_stream_t<1>(ctx, p0, Pb, s); }
-    else if (Pb <= 2) { PB = 2; launch_stream_t<2>(ctx, p0, Pb, s); }
-    else if (Pb <= 4) { PB = 4; launch_stream_t<4>(ctx, p0, Pb, s); }
-    else if (Pb <= 8) { PB = 8; launch_stream_t<8>(ctx, p0, Pb, s); }
-    else { PB = 16; launch_stream_t<16>(ctx, p0, Pb, s); }
+    {
+        ProfScope prof(ctx, s);
+        if (Pb <= 1) { PB = 1; launch_stream_t<1>(ctx, p0, Pb, s); }
+        else if (Pb <= 2) { PB = 2; launch_stream_t<2>(ctx, p0, Pb, s); }
+        else if (Pb <= 4) { PB = 4; launch_stream_t<4>(ctx, p0, Pb, s); }
+        else if (Pb <= 8) { PB = 8; launch_stream_t<8>(ctx, p0, Pb, s); }
+        else { PB = 16; launch_stream_t<16>(ctx, p0, Pb, s); }
+    }
     const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
     const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;
     const int mu_ld = (ctx->n_rec + 1) & ~1;

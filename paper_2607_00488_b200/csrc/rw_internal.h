@@ -76,6 +76,10 @@ struct rw_ctx {
     CUtensorMap tmapA;
     int num_sms;
     int64_t launches;
+    // measurement hooks (rw_profile_begin/end)
+    cudaEvent_t *prof_ev;     // pairs: [2q] before, [2q+1] after fold launch q
+    int prof_cap, prof_n;     // pairs allocated / recorded
+    bool profiling;
     char err[512];
 };
 
@@ -107,6 +111,19 @@ cudaError_t launch_fold_stream(rw_ctx *ctx, int64_t p0, int Pb, double *out_mu,
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
                           bool full_eq18, cudaStream_t s);                   // rw_fold_stream.cu
 int make_tensor_maps(rw_ctx *ctx);                                           // rw_fold_gemm.cu
+
+// Brackets one fold-kernel launch with CUDA events while profiling is on (rw_api.cu).
+struct ProfScope {
+    rw_ctx *ctx; cudaStream_t s; bool on;
+    ProfScope(rw_ctx *c, cudaStream_t st) : ctx(c), s(st), on(c->profiling && c->prof_n < c->prof_cap)
+    {
+        if (on) cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n], s);
+    }
+    ~ProfScope()
+    {
+        if (on) { cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n + 1], s); ctx->prof_n++; }
+    }
+};
 
 // Poisson term of Eq. (18) relative to its saturated value: mu - n + n ln(n/mu) (x2 applied later).
 __device__ __forceinline__ double poisson_term(double mu, double n)
