@@ -84,14 +84,6 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def rank_points(wl, name, rank):
-    """Rank 0 folds the config's own scan; further ranks an independent seeded draw of the same shape."""
-    params, kinds = wl.scan_points(name)
-    if rank > 0:
-        params, kinds = wl.random_points(params.shape[0], kinds, seed=100003 * rank + 7)
-    return np.ascontiguousarray(params), kinds
-
-
 def oracle_sample_run(name, n_points, nthreads, repeats=1):
     """Times the oracle as it stands on the first n_points scan points; returns (evals/s, seconds)."""
     from oracle import rw_oracle as orc
@@ -170,7 +162,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2607_00488_b200 import binding, workloads as wl
+    from paper_2607_00488_b200 import binding, sharding, workloads as wl
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
@@ -182,7 +174,7 @@ def main():
     name = args.config
     inp = wl.make(name)
     D, n_T, n_rec = inp["R"].shape
-    params, kinds = rank_points(wl, name, rank)
+    params, kinds = sharding.rank_points(name, rank)
     P, k = params.shape
 
     # tables resident in HBM before anything is timed (R is borrowed by the context, not copied)
@@ -202,11 +194,7 @@ def main():
             torch.cuda.synchronize()
 
     def maxreduce(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, dev, world)
 
     # ---------------------------------------------------------------- device-resident throughput
     for _ in range(args.warmup):
@@ -228,7 +216,7 @@ def main():
     fold_ms, fold_launches = ctx.profile_end()
     launches = ctx.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    value = world * P * args.steps / (ms * 1e-3)
+    value = sharding.whole_job_value(world, P, args.steps, ms)
     finite = bool(torch.isfinite(out_dev).all().item())
 
     # ---------------------------------------------------------------- end to end with host buffers
@@ -241,7 +229,7 @@ def main():
     e1.record()
     barrier()
     ms_e2e = maxreduce(e0.elapsed_time(e1))
-    e2e_value = world * P * args.steps / (ms_e2e * 1e-3)
+    e2e_value = sharding.whole_job_value(world, P, args.steps, ms_e2e)
     same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
 
     # ---------------------------------------------------------------- single evaluation (HBM-bound regime)

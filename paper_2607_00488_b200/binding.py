@@ -100,6 +100,14 @@ def probe_fp64_peak(kind, iters=20000):
     return out.value
 
 
+class _DevicePointer:
+    """A float64 device array owned by the library, exposed through __cuda_array_interface__."""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f8", "data": (int(ptr), False),
+                                         "version": 3, "strides": None}
+
+
 class Reweighter:
     """One rw_ctx: device-resident tables of one analysis + its workspace (a torch uint8 tensor).
 
@@ -221,12 +229,8 @@ class Reweighter:
         """Copy of a setup table as a CUDA tensor (RW_TABLE_S_SM / _BASIS / _WHAT)."""
         ptr, n = C.c_void_p(None), C.c_int64(0)
         self._check(self._L.rw_get_table(self._ctx, int(which), C.byref(ptr), C.byref(n)), self._ctx)
-        out = torch.empty(n.value, dtype=torch.float64, device=self.device)
-        torch.cuda.current_stream().synchronize()
-        rc = torch.cuda.cudart().cudaMemcpy(out.data_ptr(), ptr.value, n.value * 8, 3)   # cudaMemcpyDeviceToDevice
-        if int(rc) != 0:
-            raise RuntimeError("cudaMemcpy failed: %s" % rc)
-        return out
+        view = _DevicePointer(ptr.value, n.value)
+        return torch.as_tensor(view, device=self.device).clone()
 
     def profile_begin(self):
         self._check(self._L.rw_profile_begin(self._ctx), self._ctx)

@@ -27,7 +27,9 @@ int fail(rw_ctx *ctx, int status, const char *fmt, ...)
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 constexpr int kPlanSMs = 148;            // B200; only used to size the streaming-fold row split
-constexpr int64_t kMaxChunkRows = 8192;  // points per contraction chunk (A_packed <= 1 GiB)
+constexpr int64_t kMaxChunkRows = 32768;             // points per contraction chunk
+constexpr int64_t kMaxChunkBytes = (int64_t)4 << 30;  // ... and A_packed <= 4 GiB: 180 GB of HBM make large
+                                                      // chunks cheap, and the last wave of a launch is <0.5%
 
 static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
 {
@@ -41,7 +43,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->copy_R = (in->mem_kind == RW_MEM_HOST) || (n_rec & 1);
     L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
     L->KPAD = (int)((n_T + kBK - 1) / kBK * kBK);
-    int64_t cap = ((int64_t)1 << 30) / ((int64_t)L->KPAD * 8) / kBM * kBM;
+    int64_t cap = kMaxChunkBytes / ((int64_t)L->KPAD * 8) / kBM * kBM;
     if (cap < kBM) cap = kBM;
     if (cap > kMaxChunkRows) cap = kMaxChunkRows;
     int64_t mc = (max_batch + kBM - 1) / kBM * kBM;

@@ -6,7 +6,8 @@
 // Blackwell has no FP64 path in tcgen05/TMEM; FP64 tensor work is the warp-level DMMA.8x8x4
 // (mma.sync.m8n8k4.f64), measured at 37.1 TFLOP/s on B200.  Design:
 //   * persistent CTAs (one per SM), 128x128 output tile, BK = 16, 6-stage TMA/mbarrier pipeline
-//   * warp 8 = TMA producer (one elected lane); warps 0-7 = DMMA consumers, 64x32 warp tiles
+//   * 8 DMMA warps (two per SM sub-partition), 64x32 warp tiles; lane 0 of warp 0 also issues the
+//     TMA loads, kStages-2 stage-iterations ahead of the math
 //   * R tiles arrive by TMA as eight 16-column sub-tiles with the 128-byte swizzle; N' arrives as
 //     one 2-D box of the 8x8-blocked A_packed (rw_coef.cu).  The contraction index inside every
 //     group of 8 recoil bins is visited in the order {0,2,4,6},{1,3,5,7}: with that permutation
@@ -26,6 +27,7 @@ constexpr int kSubTileBytes = kBK * 128;               // one 16-column swizzled
 constexpr int kSmemRed = 4 * kBM * 8;                  // [4 column warps][128 rows]
 constexpr int kSmemBars = 2 * kStages * 8;
 constexpr int kGemmSmem = kStages * kStageBytes + kSmemRed + kSmemBars + 1024;
+constexpr int kPrefetch = kStages - 2;                 // stage-iterations the TMA issue runs ahead
 static_assert(kBK == 16 && kBM == 128 && kBN == 128, "fragment indexing below assumes this tile");
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
@@ -109,28 +111,35 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
     const int k_iters = (n_T + kBK - 1) / kBK;
     const int total_tiles = tiles_m * tiles_n;
 
-    if (warp == kGemmConsumerWarps) {
-        // ------------------------------------------------------------------ TMA producer
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-                const TileCoord tc = tile_coord(t, tiles_m, tiles_n);
-                for (int kt = 0; kt < k_iters; ++kt) {
-                    mbar_wait(empty_bar + 8 * stage, phase ^ 1);
-                    const uint32_t fb = full_bar + 8 * stage;
-                    mbar_expect_tx(fb, kStageBytes);
-                    const uint32_t dstA = sbase + stage * kStageBytes;
-                    tma_load_2d(dstA, &tmapA, kt * kBK * 8, tc.m * (kBM / 8), fb);
-                    const uint32_t dstB = dstA + kStageBytesA;
+    // ---------------------------------------------------------------------- TMA producer duty
+    // Lane 0 of warp 0 runs kPrefetch stage-iterations ahead of the consumers.  (A dedicated
+    // producer warp would put three warps on one SM sub-partition and cap every thread at 168
+    // registers; the 64x32 FP64 warp tile needs ~230.)
+    const bool is_producer = threadIdx.x == 0;
+    int p_t = blockIdx.x, p_kt = 0, p_stage = 0;
+    uint32_t p_phase = 0;
+    TileCoord p_tc = tile_coord(p_t < total_tiles ? p_t : 0, tiles_m, tiles_n);
+    auto produce_one = [&]() {
+        if (p_t >= total_tiles) return;
+        mbar_wait(empty_bar + 8 * p_stage, p_phase ^ 1);
+        const uint32_t fb = full_bar + 8 * p_stage;
+        mbar_expect_tx(fb, kStageBytes);
+        const uint32_t dstA = sbase + p_stage * kStageBytes;
+        tma_load_2d(dstA, &tmapA, p_kt * kBK * 8, p_tc.m * (kBM / 8), fb);
+        const uint32_t dstB = dstA + kStageBytesA;
 #pragma unroll
-                    for (int j = 0; j < kBN / 16; ++j)
-                        tma_load_2d(dstB + j * kSubTileBytes, &tmapR, tc.n * kBN + 16 * j, kt * kBK, fb);
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
-                }
-            }
+        for (int j = 0; j < kBN / 16; ++j)
+            tma_load_2d(dstB + j * kSubTileBytes, &tmapR, p_tc.n * kBN + 16 * j, p_kt * kBK, fb);
+        if (++p_stage == kStages) { p_stage = 0; p_phase ^= 1; }
+        if (++p_kt == k_iters) {
+            p_kt = 0;
+            p_t += gridDim.x;
+            if (p_t < total_tiles) p_tc = tile_coord(p_t, tiles_m, tiles_n);
         }
-        return;
+    };
+    if (is_producer) {
+#pragma unroll 1
+        for (int q = 0; q < kPrefetch; ++q) produce_one();
     }
 
     // ---------------------------------------------------------------------- DMMA consumers
@@ -158,6 +167,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                 for (int nb = 0; nb < 2; ++nb) acc[mb][sj][nb][0] = acc[mb][sj][nb][1] = 0.0;
 
         for (int kt = 0; kt < k_iters; ++kt) {
+            if (is_producer) produce_one();
             mbar_wait(full_bar + 8 * stage, phase);
             const uint32_t st = sbase + stage * kStageBytes;
 #pragma unroll

@@ -27,7 +27,7 @@ constexpr int kBN = 128;          // reconstructed bins per CTA tile
 constexpr int kBK = 16;           // recoil bins per pipeline stage
 constexpr int kStages = 6;
 constexpr int kGemmConsumerWarps = 8;
-constexpr int kGemmThreads = (kGemmConsumerWarps + 1) * 32;   // + 1 TMA producer warp
+constexpr int kGemmThreads = kGemmConsumerWarps * 32;
 
 // ---- streaming fold geometry (rw_fold_stream.cu) -----------------------------------------------
 constexpr int kStreamThreads = 256;
