@@ -48,7 +48,7 @@ def test_abi_argument_errors_without_a_gpu():
     inp.n_T, inp.n_rec = 16384, 8192
     inp.mem_kind = binding.RW_MEM_DEVICE
     assert L.rw_workspace_bytes(ctypes.byref(inp), 65536, ctypes.byref(nbytes)) == 0
-    assert small < nbytes.value < 4 << 30          # borrowed R: chunked scratch only, not 1 GiB of copy x2
+    assert small < nbytes.value < 5 << 30          # borrowed R: no copy; scratch = one <= 4 GiB chunk of N' + partials
     ctx = ctypes.c_void_p(None)
     assert L.rw_create(ctypes.byref(inp), 65536, None, 0, None, ctypes.byref(ctx)) in (-1, -2)
     assert ctx.value is None
@@ -122,7 +122,8 @@ v = sharding.whole_job_value(world, 121, 4, ms)
 assert abs(v - 2 * 121 * 4 / 0.015) < 1e-9
 dist.barrier()
 dist.destroy_process_group()
-print("rank", rank, "ok")
+sys.stdout.write("rank" + str(rank) + "-ok\n")
+sys.stdout.flush()
 """
 
 
@@ -134,7 +135,7 @@ def test_two_rank_gloo_plumbing(tmp_path):
     env = dict(os.environ, OMP_NUM_THREADS="1")
     p = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env)
     assert p.returncode == 0, p.stdout + p.stderr
-    assert "rank 0 ok" in p.stdout and "rank 1 ok" in p.stdout
+    assert "rank0-ok" in p.stdout and "rank1-ok" in p.stdout
 
 
 def test_reference_arm_non_zero_ranks_exit_quietly():
