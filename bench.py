@@ -30,8 +30,8 @@ METRIC = "likelihood evals/sec (batched)"
 UNIT = "evals/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_fold_gemm launch from the committed
-# `ncu --set full` capture (profiles/r01_fold_gemm_full.md), or None if not captured yet.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": None}
+# `ncu --set full` capture (profiles/r01_fold_kernels_full.md), or None if not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 87.107397e9 + 0.033670e9}
 
 
 def load_peaks():
