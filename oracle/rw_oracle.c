@@ -30,6 +30,8 @@
  *   orc_eq18          vs -2*sum(scipy.stats.poisson.logpmf)
  *   orc_eval_batch    composition of the above; Asimov injection-recovery
  *                     (PAPER.md:309-311); rank-K prefold identity
+ *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
+ *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC rw_oracle.c -o librw_oracle.so -lm
@@ -317,6 +319,40 @@ int orc_eval_batch(const orc_consts *c, int n_E, const double *E, const double *
         free(S);
     }
     free(S0);
+    return 0;
+}
+
+/* Steps a3 + a4 for caller-supplied weights: Eq. (1), E_obs = R diag(r) E_true with an
+ * arbitrary per-point weight vector r = w[p][.] (the case where a per-point nuisance -- oscillation
+ * parameters, flux shape, PAPER.md:220 -- makes the weights something other than the spectrum
+ * ratio of Eq. 14), then Eq. (18).  The same w is applied to every period's MC spectrum.
+ *   w [P][n_T];  out [P];  mu_out NULL or [P][n_periods][n_rec];  abs_out NULL or [P]. */
+int orc_eval_weights(int n_T, int n_rec, int n_periods, const double *N_mc, const double *R,
+                     const double *bkg, const double *counts, int64_t P, const double *w,
+                     double *out, double *mu_out, double *abs_out, int full_eq18, int nthreads)
+{
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        xreal *xw = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T + n_rec + 1));
+        xreal *mu = xw + n_T;
+        for (int i = 0; i < n_T; ++i) xw[i] = (xreal)w[(size_t)p * n_T + i];
+        xreal total = 0.0L, total_abs = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            const double *Cd = counts + (size_t)d * n_rec;
+            xfold(n_T, n_rec, xw, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec,
+                  bkg + (size_t)d * n_rec, mu);
+            total += full_eq18 ? xeq18(n_rec, mu, Cd) : xdeviance(n_rec, mu, Cd);
+            if (mu_out)
+                for (int q = 0; q < n_rec; ++q)
+                    mu_out[((size_t)p * n_periods + d) * n_rec + q] = (double)mu[q];
+            if (abs_out)
+                for (int q = 0; q < n_rec; ++q) total_abs += fabsl(xdeviance(1, mu + q, Cd + q));
+        }
+        out[p] = (double)total;
+        if (abs_out) abs_out[p] = (double)total_abs;
+        free(xw);
+    }
     return 0;
 }
 

@@ -204,3 +204,33 @@ def eval_batch(inp, params, kinds, want_mu=False, want_abs=False, full_eq18=Fals
     if want_abs:
         res.append(ab)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def eval_weights(inp, w, want_mu=False, want_abs=False, full_eq18=False, nthreads=1):
+    """Fold + likelihood for caller-supplied weights w[P][n_T] (Eq. 1 with an arbitrary diag(r))."""
+    R = _a(inp["R"])
+    if R.ndim == 2:
+        R = R[None]
+    D, n_T, n_rec = R.shape
+    N_mc = _a(inp["N_mc"]).reshape(D, n_T)
+    bkg = _a(inp["bkg"]).reshape(D, n_rec)
+    counts = _a(inp["counts"]).reshape(D, n_rec)
+    w = _a(w)
+    if w.ndim == 1:
+        w = w[None]
+    P = w.shape[0]
+    assert w.shape[1] == n_T
+    out = np.empty(P)
+    mu = np.empty((P, D, n_rec)) if want_mu else None
+    ab = np.empty(P) if want_abs else None
+    L = lib()
+    L.orc_eval_weights.restype = C.c_int
+    L.orc_eval_weights(C.c_int(n_T), C.c_int(n_rec), C.c_int(D), _p(N_mc), _p(R), _p(bkg), _p(counts),
+                       C.c_int64(P), _p(w), _p(out), _p(mu) if want_mu else None,
+                       _p(ab) if want_abs else None, C.c_int(1 if full_eq18 else 0), C.c_int(int(nthreads)))
+    res = [out]
+    if want_mu:
+        res.append(mu)
+    if want_abs:
+        res.append(ab)
+    return res[0] if len(res) == 1 else tuple(res)

@@ -43,7 +43,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->copy_R = (in->mem_kind == RW_MEM_HOST) || (n_rec & 1);
     L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
     L->KPAD = (int)((n_T + kBK - 1) / kBK * kBK);
-    int64_t cap = kMaxChunkBytes / ((int64_t)L->KPAD * 8) / kBM * kBM;
+    L->A_pitch = (int64_t)L->KPAD * 8;
+    int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;
     if (cap > kMaxChunkRows) cap = kMaxChunkRows;
     int64_t mc = (max_batch + kBM - 1) / kBM * kBM;
@@ -76,7 +77,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->flag = take(4);
     L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
     L->coef = take((size_t)max_batch * kCoefStride * 8);
-    L->A_packed = take((size_t)L->MC * L->KPAD * 8);
+    L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
     size_t part_gemm = D * (size_t)L->n_tiles_n * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
     L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);

@@ -46,7 +46,7 @@ constexpr int kGenKT = 128;        // recoil bins staged per CTA
 // A_packed[mb][kb][r][kk] = N'[p0 + 8 mb + r][8 kb + kk]; rows >= Pc and bins >= n_T are zero.
 __global__ void __launch_bounds__(kGenThreads)
 k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pad,
-        const double *__restrict__ What /*[12][n_T] of this period*/, int n_T, int KPAD,
+        const double *__restrict__ What /*[12][n_T] of this period*/, int n_T, int KPAD, int64_t A_pitch,
         double *__restrict__ A)
 {
     __shared__ __align__(16) double sW[kNumTerms][kGenKT];
@@ -65,7 +65,6 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
     const bool valid = row < Pc;
 #pragma unroll
     for (int b = 0; b < kNumTerms; ++b) c[b] = valid ? coef[(p0 + row) * kCoefStride + b] : 0.0;
-    const int KB = KPAD / 8;
     const int nkb = min(kGenKT, KPAD - k0) / 8;
     for (int kb = 0; kb < nkb; ++kb) {
         double v[8];
@@ -81,7 +80,7 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
                 v[2 * h + 1] = fma(c[b], w.y, v[2 * h + 1]);
             }
         }
-        double2 *dst = reinterpret_cast<double2 *>(A + ((mb * KB + (k0 / 8 + kb)) * 64 + r * 8));
+        double2 *dst = reinterpret_cast<double2 *>(A + (mb * A_pitch + (size_t)(k0 / 8 + kb) * 64 + r * 8));
 #pragma unroll
         for (int h = 0; h < 4; ++h) dst[h] = make_double2(v[2 * h], v[2 * h + 1]);
     }
@@ -105,7 +104,7 @@ cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_
               (unsigned)((ctx->lay.KPAD + kGenKT - 1) / kGenKT));
     k_gen_A<<<grid, kGenThreads, 0, s>>>(ctx->coef, p0, Pc, rows_pad,
                                          ctx->What + (size_t)d * kCoefStride * ctx->n_T, ctx->n_T,
-                                         ctx->lay.KPAD, ctx->A_packed);
+                                         ctx->lay.KPAD, ctx->lay.A_pitch, ctx->A_packed);
     ctx->launches++;
     return cudaGetLastError();
 }

@@ -27,8 +27,9 @@ constexpr int kSubTileBytes = kBK * 128;               // one 16-column swizzled
 constexpr int kSmemRed = 4 * kBM * 8;                  // [4 column warps][128 rows]
 constexpr int kSmemBars = 2 * kStages * 8;
 constexpr int kGemmSmem = kStages * kStageBytes + kSmemRed + kSmemBars + 1024;
-constexpr int kPrefetch = kStages - 2;                 // stage-iterations the TMA issue runs ahead
-static_assert(kBK == 16 && kBM == 128 && kBN == 128, "fragment indexing below assumes this tile");
+constexpr int kPrefetch = (kStages > 3) ? kStages - 2 : kStages - 1;                 // stage-iterations the TMA issue runs ahead
+static_assert((kBK == 16 || kBK == 32) && kBM == 128 && kBN == 128, "fragment indexing below assumes this tile");
+constexpr int kKB = kBK / 8;                           // 8-bin groups per stage
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -58,6 +59,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok;
+}
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
 {
     asm volatile(
@@ -70,10 +82,15 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
+#ifdef RW_GEMM_STATS
+__device__ unsigned long long g_gemm_stats[148 * 8];
+__device__ __forceinline__ long long clk() { long long t; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t)); return t; }
+#endif
+
 struct TileCoord { int m, n; };
 __device__ __forceinline__ TileCoord tile_coord(int t, int tiles_m, int tiles_n)
 {
-    constexpr int GM = 8;                       // m-tiles per raster group: a wave shares A and R panels in L2
+    constexpr int GM = 8;     // m-tiles per raster group: a wave of 148 CTAs shares 8 N' and ~19 R panels in L2
     const int per_group = GM * tiles_n;
     const int g = t / per_group, rem = t - g * per_group;
     const int first_m = g * GM;
@@ -146,7 +163,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
     const int wm = warp >> 2, wn = warp & 3;
     const int r = lane >> 2, c = lane & 3;
     // A: block (8 wm + mb, kb) is 512 contiguous bytes, lane reads its 16 bytes
-    const uint32_t a_off = (uint32_t)(wm * 8 * 2) * 512 + lane * 16;
+    const uint32_t a_off = (uint32_t)(wm * 8 * kKB) * 512 + lane * 16;
     // R: sub-tile (2 wn + sj), row 8 kb + 2c + s, 16-byte chunk (r ^ (2c + s))
     uint32_t b_off[2];
 #pragma unroll
@@ -156,6 +173,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
 
     int stage = 0;
     uint32_t phase = 0;
+    uint32_t ready = 0;      // result of the early poll of the next stage's full barrier
     for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
         const TileCoord tc = tile_coord(t, tiles_m, tiles_n);
         double acc[8][2][2][2];
@@ -168,16 +186,32 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
 
         for (int kt = 0; kt < k_iters; ++kt) {
             if (is_producer) produce_one();
-            mbar_wait(full_bar + 8 * stage, phase);
+#ifdef RW_GEMM_STATS
+            {
+                long long t0 = clk();
+                mbar_wait(full_bar + 8 * stage, phase);
+                long long dt = clk() - t0;
+                if (threadIdx.x == 32 && blockIdx.x < 148) {
+                    unsigned long long *st = g_gemm_stats + blockIdx.x * 8;
+                    st[0] += dt; st[1] += 1;
+                    if (dt > 500) st[2] += 1;
+                    if (dt > 4000) st[3] += 1;
+                    if ((unsigned long long)dt > st[4]) st[4] = dt;
+                    if (kt < 4) st[5] += dt;
+                }
+            }
+#else
+            if (!ready) mbar_wait(full_bar + 8 * stage, phase);
+#endif
             const uint32_t st = sbase + stage * kStageBytes;
 #pragma unroll
-            for (int kb = 0; kb < 2; ++kb) {
+            for (int kb = 0; kb < kKB; ++kb) {
                 double2 a[8], b[2][2];
 #pragma unroll
                 for (int mb = 0; mb < 8; ++mb)
                     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];"
                                  : "=d"(a[mb].x), "=d"(a[mb].y)
-                                 : "r"(st + a_off + (uint32_t)(mb * 2 + kb) * 512));
+                                 : "r"(st + a_off + (uint32_t)(mb * kKB + kb) * 512));
 #pragma unroll
                 for (int sj = 0; sj < 2; ++sj)
 #pragma unroll
@@ -185,6 +219,12 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                         asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];"
                                      : "=d"(b[sj][s].x), "=d"(b[sj][s].y)
                                      : "r"(st + b_off[s] + (uint32_t)sj * kSubTileBytes + (uint32_t)kb * 1024));
+                if (kb == kKB - 1) {
+                    // poll the next stage's barrier now: the result is back by the time the last
+                    // 64 DMMAs of this stage have issued, so the wait below costs no pipe bubble
+                    const int ns = (stage + 1 == kStages) ? 0 : stage + 1;
+                    ready = mbar_test(full_bar + 8 * ns, (stage + 1 == kStages) ? (phase ^ 1) : phase);
+                }
 #pragma unroll
                 for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -269,6 +309,16 @@ static PFN_encodeTiled get_encode()
     return fn;
 }
 
+#ifdef RW_GEMM_STATS
+extern "C" int rw_debug_gemm_stats(unsigned long long *host_out, int reset)
+{
+    cudaDeviceSynchronize();
+    if (host_out) cudaMemcpyFromSymbol(host_out, g_gemm_stats, sizeof(unsigned long long) * 148 * 8);
+    if (reset) { static unsigned long long z[148 * 8]; cudaMemcpyToSymbol(g_gemm_stats, z, sizeof(z)); }
+    return 0;
+}
+#endif
+
 int make_tensor_maps(rw_ctx *ctx)
 {
     PFN_encodeTiled enc = get_encode();
@@ -276,7 +326,7 @@ int make_tensor_maps(rw_ctx *ctx)
     const Layout &L = ctx->lay;
     {
         cuuint64_t dims[2] = {(cuuint64_t)L.KPAD * 8, (cuuint64_t)(L.MC / 8)};
-        cuuint64_t strides[1] = {(cuuint64_t)L.KPAD * 8 * sizeof(double)};
+        cuuint64_t strides[1] = {(cuuint64_t)L.A_pitch * sizeof(double)};
         cuuint32_t box[2] = {kBK * 8, kBM / 8};
         cuuint32_t estr[2] = {1, 1};
         CUresult r = enc(&ctx->tmapA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, ctx->A_packed, dims, strides, box, estr,

@@ -48,6 +48,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
+    int64_t A_pitch;      // doubles between consecutive 8-point row blocks of A_packed (>= 8 KPAD)
     int64_t MC;           // points per GEMM chunk (multiple of kBM)
     int n_tiles_n;        // ceil(n_rec / kBN)
     int stream_strips;    // ceil(n_rec / kStreamCols)

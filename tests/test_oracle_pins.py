@@ -347,6 +347,35 @@ def test_rank_K_prefold_identity(orc):
     assert np.all(np.abs(pred / mu_x[0, 0] - 1) < 1e-13)
 
 
+def test_eval_weights_pins(orc):
+    """Caller-supplied weights (Eq. 1 with an arbitrary diag(r)): (i) fed the spectrum-ratio weights
+    it reproduces eval_batch; (ii) on random weights mu = (w*N_mc) @ R + bkg by numpy and the
+    likelihood is -2 sum logpmf by scipy; (iii) w == 1 is the SM prediction; (iv) a transposed or
+    period-swapped operand fails (ii)."""
+    from scipy.stats import poisson
+    inp = _small_problem(D=2)
+    params, kinds = wl.random_points(4, [orc.EPS_EE_L, orc.MU_NU], seed=9)
+    ref, mu_ref = orc.eval_batch(inp, params, kinds, want_mu=True)
+    w = np.stack([orc.weights(inp, orc.theta_vector(params[p], kinds)) for p in range(4)])
+    out, mu = orc.eval_weights(inp, w, want_mu=True, nthreads=2)
+    assert np.all(np.abs(mu / mu_ref - 1) < 1e-15) and np.all(np.abs(out / ref - 1) < 1e-13)
+    rng = np.random.default_rng(10)
+    w = rng.uniform(0.2, 3.0, size=(3, inp["T"].size))
+    out, mu, ab = orc.eval_weights(inp, w, want_mu=True, want_abs=True)
+    full = orc.eval_weights(inp, w, full_eq18=True)
+    for p in range(3):
+        tot = 0.0
+        for d in range(2):
+            m = (w[p] * inp["N_mc"][d]) @ inp["R"][d] + inp["bkg"][d]
+            assert np.all(np.abs(mu[p, d] / m - 1) < 1e-14)
+            tot += -2.0 * poisson.logpmf(inp["counts"][d], m).sum()
+        assert abs(full[p] / tot - 1) < 1e-12
+        assert ab[p] >= out[p] > 0
+    _, mu1 = orc.eval_weights(inp, np.ones((1, inp["T"].size)), want_mu=True)
+    for d in range(2):
+        assert np.all(np.abs(mu1[0, d] / (inp["N_mc"][d] @ inp["R"][d] + inp["bkg"][d]) - 1) < 1e-15)
+
+
 def test_sm_point_gives_sm_prediction(orc):
     inp = _small_problem(D=2)
     _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
