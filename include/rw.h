@@ -63,9 +63,10 @@ enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
 enum {
     RW_DEVIANCE    = 0u,       /* default: 2 sum [mu - n + n ln(n/mu)] (Eq. 18 minus its saturated value) */
     RW_FULL_EQ18   = 1u << 0,  /* literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)] */
-    RW_MODE_AUTO   = 0u,       /* P <= 16: streaming fold; else: DMMA batched contraction */
+    RW_MODE_AUTO   = 0u,       /* P <= 32: streaming fold; else: DMMA batched contraction */
     RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P) */
     RW_MODE_GEMM   = 2u << 4,  /* force the FP64 tensor-core (DMMA) contraction */
+    RW_MODE_COLLAPSED = 3u << 4, /* opt-in: rank-K prefolded templates (exact, O(K n_rec) per point); see below */
     RW_MODE_MASK   = 3u << 4,
     RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
     RW_OUT_HOST    = 1u << 9   /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
@@ -125,11 +126,30 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
 int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                   double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
 
+/* RW_MODE_COLLAPSED (rw_eval_batch only).  Eq. (4) is quadratic in the couplings, Eq. (8)
+ * linear in mu_nu^2 and the fold of Eq. (11) linear in the spectrum, so
+ *   mu[p][d][k] - bkg[d][k] = sum_b c_b(theta_p) G[d][b][k],   G[d][b][k] = sum_i W^[d][b][i] R[d][i][k]
+ * exactly (up to rounding order).  rw_create folds the 11 templates G once; this mode then evaluates a point
+ * in O(11 n_rec D) instead of O(n_T n_rec D).  It is NOT what RW_MODE_AUTO/STREAM/GEMM run (those execute the
+ * full fold for every point, which is the only valid path once weights are not low-rank -- rw_eval_weights).
+ *
+ * rw_eval_weights: steps a3 + a4 for caller-supplied weights (Eq. 1, with an arbitrary
+ * diag(r)): mu[p][d][k] = sum_i w[p][i] N_mc[d][i] R[d][i][k] + bkg[d][k], then Eq. (18).  For per-point
+ * nuisances that make the weights something other than the spectrum ratio of Eq. (14) (oscillation
+ * parameters, flux shapes: PAPER.md:220).
+ *   w          [P][n_T] row-major DEVICE pointer, finite and >= 0 (not validated; garbage in, garbage out)
+ *   out_m2lnL  [P] device pointer;  out_mu NULL or [P][D][n_rec] device pointer
+ *   flags      RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM (COLLAPSED, RW_PARAM_HOST, RW_OUT_HOST: RW_ERR_UNSUPPORTED)
+ * Asynchronous and stream-ordered like rw_eval_batch; P may be 0 and may exceed max_batch. */
+int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
+                    uint32_t flags, void *cuda_stream);
+
 /* Device pointers to setup tables, for inspection/tests (valid until rw_destroy):
  *   RW_TABLE_S_SM   [n_T]        SM recoil spectrum S_SM(T_i) (Eq. 12 at theta = 0)
  *   RW_TABLE_BASIS  [10][n_T]    basis spectra A_e,B_e,C_e,A_mu,...,C_tau,D
- *   RW_TABLE_WHAT   [D][12][n_T] pre-scaled basis W^ = basis * N_mc / S_SM (+ dead-bin row) */
-enum { RW_TABLE_S_SM = 0, RW_TABLE_BASIS = 1, RW_TABLE_WHAT = 2 };
+ *   RW_TABLE_WHAT   [D][12][n_T] pre-scaled basis W^ = basis * N_mc / S_SM (+ dead-bin row)
+ *   RW_TABLE_G      [D][12][ldG] prefolded templates G (ldG = n_rec rounded up to even; rows 11 unused) */
+enum { RW_TABLE_S_SM = 0, RW_TABLE_BASIS = 1, RW_TABLE_WHAT = 2, RW_TABLE_G = 3 };
 int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64_t *n_elems);
 
 /* Number of kernels this context has launched so far (setup + eval); for bench accounting. */

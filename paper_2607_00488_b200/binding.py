@@ -19,12 +19,12 @@ LIB_PATH = os.path.join(_HERE, "librw.so")
 RW_EPS_EE_L, RW_EPS_EE_R, RW_EPS_MM_L, RW_EPS_MM_R, RW_EPS_TT_L, RW_EPS_TT_R, RW_MU_NU = range(7)
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
-RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM = 0, 1 << 4, 2 << 4
+RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED = 0, 1 << 4, 2 << 4, 3 << 4
 RW_PARAM_HOST, RW_OUT_HOST = 1 << 8, 1 << 9
-RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT = 0, 1, 2
-_MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM}
+RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
+_MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
-EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
            "rw_last_error", "rw_probe_fp64_peak")
 
@@ -68,6 +68,8 @@ def load_library():
     L.rw_set_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.rw_eval_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32),
                                 C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_weights.restype = C.c_int
     L.rw_get_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
     L.rw_launch_count.argtypes = [C.c_void_p]
     L.rw_launch_count.restype = C.c_int64
@@ -213,6 +215,28 @@ class Reweighter:
                                    flags, _stream_ptr())
         self._check(rc, self._ctx)
         self._last_param = param          # keep alive until the stream has consumed it
+        return (out, out_mu) if (want_mu or out_mu is not None) else out
+
+    def eval_weights(self, w, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
+        """-2lnL[P] for caller-supplied weights w[P][n_T] (CUDA float64 tensor): the dense fold on arbitrary
+        weights (rw_eval_weights).  Asynchronous on the current stream."""
+        if not (isinstance(w, torch.Tensor) and w.is_cuda):
+            raise RwError(-4, "eval_weights needs a CUDA tensor w[P][n_T]")
+        w = w.to(torch.float64).contiguous()
+        if w.ndim == 1:
+            w = w[None]
+        P, n_T = w.shape
+        assert n_T == self.n_T, "w has %d columns, the recoil grid has %d bins" % (n_T, self.n_T)
+        if out is None:
+            out = torch.empty(P, dtype=torch.float64, device=self.device)
+        if want_mu and out_mu is None:
+            out_mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        rc = self._L.rw_eval_weights(self._ctx, C.c_void_p(w.data_ptr()), P, C.c_void_p(out.data_ptr()),
+                                     C.c_void_p(out_mu.data_ptr()) if out_mu is not None else None,
+                                     flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = w
         return (out, out_mu) if (want_mu or out_mu is not None) else out
 
     def set_counts(self, counts):

@@ -75,6 +75,9 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->What = take(D * kCoefStride * n_T * 8);
     L->sat_const = take(8);
     L->flag = take(4);
+    L->ldG = (int)mu_ld;
+    L->G = take(D * kCoefStride * mu_ld * 8);
+    L->ident = take(kStreamMaxPB * kCoefStride * 8);
     L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
     L->coef = take((size_t)max_batch * kCoefStride * 8);
     L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
@@ -211,6 +214,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->basis = (double *)(ws + L.basis);  ctx->S_sm = (double *)(ws + L.S_sm);
     ctx->What = (double *)(ws + L.What);    ctx->sat_const = (double *)(ws + L.sat_const);
     ctx->flag = (int *)(ws + L.flag);
+    ctx->G = (double *)(ws + L.G);          ctx->ident = (double *)(ws + L.ident);
     ctx->param_stage = (double *)(ws + L.param_stage);
     ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);
     ctx->partial = (double *)(ws + L.partial);
@@ -251,6 +255,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
     RW_TRY(launch_setup(ctx, s));
     RW_TRY(launch_sat_const(ctx, s));
+    RW_TRY(launch_prefold(ctx, s));
     int flag = 0;
     RW_TRY(cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
     RW_TRY(cudaStreamSynchronize(s));
@@ -303,7 +308,6 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             if (kinds[b] == kinds[a]) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: duplicate param_kind %d", kinds[a]);
     }
     const uint32_t mode = flags & RW_MODE_MASK;
-    if (mode == RW_MODE_MASK) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: bad mode flags");
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
 
@@ -323,12 +327,20 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
         const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && Ps <= 32);
-        if (stream_mode) {
+        if (mode == RW_MODE_COLLAPSED) {
+            const int nstrip = (n_rec + 511) / 512;
+            for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
+                const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
+                double *mu = out_mu ? out_mu + (size_t)(s0 + c0) * D * n_rec : nullptr;
+                RW_CUDA(ctx, launch_collapsed(ctx, c0, Pc, mu, s));
+                RW_CUDA(ctx, launch_reduce(ctx, D * nstrip, L.MC, Pc, dout + c0, full, s));
+            }
+        } else if (stream_mode) {
             const int nstrip2 = (n_rec + 255) / 256;
             for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
                 const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
                 double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
-                RW_CUDA(ctx, launch_fold_stream(ctx, g0, Pb, mu, s));
+                RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, Pb, mu, s));
                 RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, dout + g0, full, s));
             }
         } else {
@@ -348,6 +360,45 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     return RW_OK;
 }
 
+int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
+                    uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_weights: ctx is NULL");
+    if (P < 0) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: P < 0");
+    if (P == 0) return RW_OK;
+    if (!w || !out_m2lnL) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: w or out_m2lnL is NULL");
+    const uint32_t mode = flags & RW_MODE_MASK;
+    if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST)))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_weights: collapsed mode and host buffers are not supported "
+                                             "(arbitrary weights are not low-rank; w is a device array)");
+    const bool full = flags & RW_FULL_EQ18;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Layout &L = ctx->lay;
+    const int D = ctx->D, n_rec = ctx->n_rec;
+    const size_t n_T = ctx->n_T;
+    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && P <= 32);
+    if (stream_mode) {
+        const int nstrip2 = (n_rec + 255) / 256;
+        for (int64_t g0 = 0; g0 < P; g0 += kStreamMaxPB) {
+            const int Pb = (int)((P - g0 < kStreamMaxPB) ? P - g0 : kStreamMaxPB);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, w + (size_t)g0 * n_T, Pb, mu, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, out_m2lnL + g0, full, s));
+        }
+    } else {
+        for (int64_t c0 = 0; c0 < P; c0 += L.MC) {
+            const int64_t Pc = (P - c0 < L.MC) ? P - c0 : L.MC;
+            double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
+            for (int d = 0; d < D; ++d) {
+                RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
+                RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+            }
+            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, out_m2lnL + c0, full, s));
+        }
+    }
+    return RW_OK;
+}
+
 int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64_t *n_elems)
 {
     if (!ctx || !dev_ptr || !n_elems) return RW_ERR_INVALID;
@@ -355,6 +406,7 @@ int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64
     case RW_TABLE_S_SM: *dev_ptr = ctx->S_sm; *n_elems = ctx->n_T; return RW_OK;
     case RW_TABLE_BASIS: *dev_ptr = ctx->basis; *n_elems = (int64_t)kNumBasis * ctx->n_T; return RW_OK;
     case RW_TABLE_WHAT: *dev_ptr = ctx->What; *n_elems = (int64_t)ctx->D * kCoefStride * ctx->n_T; return RW_OK;
+    case RW_TABLE_G: *dev_ptr = ctx->G; *n_elems = (int64_t)ctx->D * kCoefStride * ctx->lay.ldG; return RW_OK;
     default: return RW_ERR_INVALID;
     }
 }

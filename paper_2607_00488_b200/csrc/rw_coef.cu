@@ -86,6 +86,54 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
     }
 }
 
+// Caller-supplied weights (rw_eval_weights): A_packed[mb][kb][r][kk] = w[8 mb + r][8 kb + kk] * N_mc[8 kb + kk]
+// (Eq. 1: diag(r) E_true).  A CTA transposes a 64-point x 64-bin tile through shared
+// memory: rows of w are read 512 contiguous bytes per warp, the 8x8 blocks are written 512 contiguous bytes each.
+constexpr int kGwRows = 64, kGwCols = 64;
+__global__ void __launch_bounds__(256)
+k_gen_A_weights(const double *__restrict__ w /*[Pc][n_T]*/, int64_t Pc, int64_t rows_pad,
+                const double *__restrict__ N_mc /*[n_T] of this period*/, int n_T, int KPAD, int64_t A_pitch,
+                double *__restrict__ A)
+{
+    __shared__ double tile[kGwRows][kGwCols + 1];
+    const int64_t row0 = (int64_t)blockIdx.x * kGwRows;
+    const int k0 = blockIdx.y * kGwCols;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int rr = warp; rr < kGwRows; rr += 8) {
+        const int64_t row = row0 + rr;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int i = k0 + lane + 32 * h;
+            double v = 0.0;
+            if (row < Pc && i < n_T) v = w[(size_t)row * n_T + i] * N_mc[i];
+            tile[rr][lane + 32 * h] = v;
+        }
+    }
+    __syncthreads();
+    // 8 x 8 blocks of this tile; warp `warp` writes the blocks of row block mb = warp
+    const int64_t mb = row0 / 8 + warp;
+    if (mb * 8 >= rows_pad) return;
+    for (int kb = 0; kb < kGwCols / 8; ++kb) {
+        if (k0 + kb * 8 >= KPAD) break;
+        double *dst = A + (mb * A_pitch + (size_t)(k0 / 8 + kb) * 64);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int e = lane + 32 * h;               // element of the block: r = e / 8, kk = e % 8
+            dst[e] = tile[warp * 8 + (e >> 3)][kb * 8 + (e & 7)];
+        }
+    }
+}
+
+cudaError_t launch_gen_A_weights(rw_ctx *ctx, int d, const double *w, int64_t Pc, cudaStream_t s)
+{
+    const int64_t rows_pad = (Pc + kBM - 1) / kBM * kBM;
+    dim3 grid((unsigned)((rows_pad + kGwRows - 1) / kGwRows), (unsigned)((ctx->lay.KPAD + kGwCols - 1) / kGwCols));
+    k_gen_A_weights<<<grid, 256, 0, s>>>(w, Pc, rows_pad, ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T,
+                                         ctx->lay.KPAD, ctx->lay.A_pitch, ctx->A_packed);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
                         cudaStream_t s)
 {

@@ -1,0 +1,133 @@
+// rw_collapsed.cu -- opt-in RW_MODE_COLLAPSED: rank-K prefolded templates.
+//
+// Eq. (4) is quadratic in the couplings, Eq. (8) linear in mu_nu^2, and the
+// fold of Eq. (11) is linear in the recoil spectrum, so
+//     mu[p][d][k] - bkg[d][k] = sum_{b<11} c_b(theta_p) G[d][b][k],   G[d][b][k] = sum_i W^[d][b][i] R[d][i][k]
+// holds exactly.  rw_create folds the 11 templates once (k_fold_stream with identity coefficients: the
+// templates are "points" whose coefficient vectors are unit vectors), and a point then costs
+// 2*11*n_rec*D flop plus the Poisson terms of Eq. (18) instead of 2*n_T*n_rec*D.
+// This path is bound by plain FP64 ALU work (the log1p of every bin), not by HBM or the tensor pipe;
+// bench.py reports it on its own line and never mixes it into the dense-fold figure.
+#include "rw_internal.h"
+
+namespace rw {
+
+constexpr int kColThreads = 256;
+constexpr int kColCols = 2 * kColThreads;   // reconstructed bins per CTA strip, two per thread
+constexpr int kColPB = 64;                  // points per CTA
+
+// G[d][b][k] = sum over row splits of the streaming fold's partial sums (fixed order).
+__global__ void k_sum_splits(const double *__restrict__ mu_part, int n_splits, int PB, int mu_ld, int n_rec,
+                             int ldG, double *__restrict__ G /*[D][12][ldG]*/)
+{
+    const int b = blockIdx.y, d = blockIdx.z;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= ldG) return;
+    double v = 0.0;
+    if (col < n_rec && b < kNumTerms)
+        for (int s = 0; s < n_splits; ++s) v += mu_part[(((size_t)d * n_splits + s) * PB + b) * mu_ld + col];
+    G[((size_t)d * kCoefStride + b) * ldG + col] = v;
+}
+
+__global__ void k_identity(double *__restrict__ ident /*[16][12]*/)
+{
+    const int q = threadIdx.x;
+    if (q < kStreamMaxPB * kCoefStride) ident[q] = (q / kCoefStride == q % kCoefStride) ? 1.0 : 0.0;
+}
+
+// One CTA: kColPB points x one 512-column strip of one period.  The 11 template values of the thread's two
+// columns stay in registers; per point: 11-term dot product, + bkg, Poisson term, warp-shuffle sum, then one
+// shared-memory pass over the 8 warps.  partial[(d * nstrip + strip)][p] feeds k_reduce (fixed order).
+__global__ void __launch_bounds__(kColThreads)
+k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const double *__restrict__ coef,
+            int64_t Pc, const double *__restrict__ bkg, const double *__restrict__ counts,
+            double *__restrict__ partial, int64_t part_stride, double *__restrict__ out_mu)
+{
+    __shared__ double sC[kColPB][kCoefStride];
+    __shared__ double red[kColThreads / 32][kColPB];
+    const int d = blockIdx.z;
+    const int64_t p0 = (int64_t)blockIdx.y * kColPB;
+    const int np = (int)min((int64_t)kColPB, Pc - p0);
+    const int col = blockIdx.x * kColCols + 2 * threadIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    for (int q = threadIdx.x; q < kColPB * kCoefStride; q += kColThreads) {
+        const int p = q / kCoefStride, b = q - p * kCoefStride;
+        sC[p][b] = (p < np) ? coef[(p0 + p) * kCoefStride + b] : 0.0;
+    }
+    double g[kNumTerms][2], bk[2], cn[2];
+    const bool ok0 = col < n_rec, ok1 = col + 1 < n_rec;
+    {
+        const double *Gd = G + (size_t)d * kCoefStride * ldG;
+#pragma unroll
+        for (int b = 0; b < kNumTerms; ++b) {
+            // ldG is even and col is even: one 16-byte load; columns >= n_rec hold zeros
+            const double2 v = ok0 ? *reinterpret_cast<const double2 *>(Gd + (size_t)b * ldG + col)
+                                  : make_double2(0.0, 0.0);
+            g[b][0] = v.x; g[b][1] = v.y;
+        }
+        bk[0] = ok0 ? bkg[(size_t)d * n_rec + col] : 0.0;
+        bk[1] = ok1 ? bkg[(size_t)d * n_rec + col + 1] : 0.0;
+        cn[0] = ok0 ? counts[(size_t)d * n_rec + col] : 0.0;
+        cn[1] = ok1 ? counts[(size_t)d * n_rec + col + 1] : 0.0;
+    }
+    __syncthreads();
+    for (int p = 0; p < np; ++p) {
+        double m0 = 0.0, m1 = 0.0;
+#pragma unroll
+        for (int b = 0; b < kNumTerms; ++b) {
+            const double c = sC[p][b];
+            m0 = fma(c, g[b][0], m0);
+            m1 = fma(c, g[b][1], m1);
+        }
+        m0 += bk[0];
+        m1 += bk[1];
+        if (out_mu) {
+            double *dst = out_mu + ((size_t)(p0 + p) * D + d) * n_rec + col;
+            if (ok0) dst[0] = m0;
+            if (ok1) dst[1] = m1;
+        }
+        double t = (ok0 ? poisson_term(m0, cn[0]) : 0.0) + (ok1 ? poisson_term(m1, cn[1]) : 0.0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) red[warp][p] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < np) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < kColThreads / 32; ++w) v += red[w][threadIdx.x];
+        partial[((size_t)d * gridDim.x + blockIdx.x) * part_stride + p0 + threadIdx.x] = v;
+    }
+}
+
+cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    k_identity<<<1, 256, 0, s>>>(ctx->ident);
+    ctx->launches++;
+    // the 11 templates are folded as 11 "points" with unit coefficient vectors (no deviance pass)
+    cudaError_t e = launch_fold_stream(ctx, ctx->ident, nullptr, -kNumTerms, nullptr, s);
+    if (e != cudaSuccess) return e;
+    const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + 63) / 64 * 64;
+    const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;
+    const int mu_ld = (ctx->n_rec + 1) & ~1;
+    dim3 grid((L.ldG + 255) / 256, kCoefStride, ctx->D);
+    k_sum_splits<<<grid, 256, 0, s>>>(ctx->mu_part, n_splits, kStreamMaxPB, mu_ld, ctx->n_rec, L.ldG, ctx->G);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    const int nstrip = (ctx->n_rec + kColCols - 1) / kColCols;
+    dim3 grid(nstrip, (unsigned)((Pc + kColPB - 1) / kColPB), ctx->D);
+    ProfScope prof(ctx, s);
+    k_collapsed<<<grid, kColThreads, 0, s>>>(ctx->G, L.ldG, ctx->n_rec, ctx->D, ctx->coef + p0 * kCoefStride, Pc,
+                                             ctx->bkg, ctx->counts, ctx->partial, L.MC, out_mu);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace rw

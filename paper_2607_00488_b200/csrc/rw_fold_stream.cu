@@ -19,6 +19,8 @@ template <int PB>
 __global__ void __launch_bounds__(kStreamThreads)
 k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int n_T, int n_rec,
               const double *__restrict__ coef, int Pb, const double *__restrict__ What,
+              const double *__restrict__ wts /*NULL, or caller weights [Pb][n_T] (rw_eval_weights)*/,
+              const double *__restrict__ N_mc /*[D][n_T], used with wts*/,
               int rows_per_split, int n_splits, int mu_ld, double *__restrict__ mu_part)
 {
     __shared__ __align__(16) double sN[kRC][PB];
@@ -31,10 +33,11 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
     const double *Rd = R + (size_t)d * R_period_stride;
     const double *Wd = What + (size_t)d * kCoefStride * n_T;
 
-    for (int q = threadIdx.x; q < PB * kNumTerms; q += kStreamThreads) {
-        int p = q / kNumTerms, b = q - p * kNumTerms;
-        sC[p][b] = (p < Pb) ? coef[(size_t)p * kCoefStride + b] : 0.0;
-    }
+    if (!wts)
+        for (int q = threadIdx.x; q < PB * kNumTerms; q += kStreamThreads) {
+            int p = q / kNumTerms, b = q - p * kNumTerms;
+            sC[p][b] = (p < Pb) ? coef[(size_t)p * kCoefStride + b] : 0.0;
+        }
     double acc[PB][2];
 #pragma unroll
     for (int p = 0; p < PB; ++p) acc[p][0] = acc[p][1] = 0.0;
@@ -47,8 +50,12 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
             const int i = ic + row;
             double v = 0.0;
             if (i < i1) {
+                if (wts) {          // N' = w N_mc (Eq. 1 with caller-supplied weights)
+                    if (p < Pb) v = wts[(size_t)p * n_T + i] * N_mc[(size_t)d * n_T + i];
+                } else {            // N' = sum_b c_b W^_b (Eq. 14 folded into the pre-scaled basis)
 #pragma unroll
-                for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p][b], Wd[(size_t)b * n_T + i], v);
+                    for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p][b], Wd[(size_t)b * n_T + i], v);
+                }
             }
             sN[row][p] = v;
         }
@@ -130,7 +137,7 @@ __global__ void k_reduce(const double *__restrict__ partial, int n_parts, int64_
 }
 
 template <int PB>
-static void launch_stream_t(rw_ctx *ctx, int64_t p0, int Pb, cudaStream_t s)
+static void launch_stream_t(rw_ctx *ctx, const double *coef, const double *wts, int Pb, cudaStream_t s)
 {
     const Layout &L = ctx->lay;
     const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
@@ -138,21 +145,30 @@ static void launch_stream_t(rw_ctx *ctx, int64_t p0, int Pb, cudaStream_t s)
     dim3 grid(L.stream_strips, n_splits, ctx->D);
     const int mu_ld = (ctx->n_rec + 1) & ~1;
     k_fold_stream<PB><<<grid, kStreamThreads, 0, s>>>(
-        ctx->R, ctx->R_period_stride, ctx->ldR, ctx->n_T, ctx->n_rec, ctx->coef + p0 * kCoefStride, Pb,
-        ctx->What, rows_per_split, n_splits, mu_ld, ctx->mu_part);
+        ctx->R, ctx->R_period_stride, ctx->ldR, ctx->n_T, ctx->n_rec, coef, Pb,
+        ctx->What, wts, ctx->N_mc, rows_per_split, n_splits, mu_ld, ctx->mu_part);
 }
 
-cudaError_t launch_fold_stream(rw_ctx *ctx, int64_t p0, int Pb, double *out_mu, cudaStream_t s)
+// Pb > 0: fold Pb points (coefficients `coef`, or caller weights `wts`) and reduce the Poisson terms.
+// Pb < 0: fold -Pb coefficient vectors only (the template prefold of rw_collapsed.cu; partials stay in mu_part
+//         laid out for PB = 16).
+cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *wts, int Pb, double *out_mu,
+                               cudaStream_t s)
 {
     const Layout &L = ctx->lay;
+    if (Pb < 0) {
+        launch_stream_t<16>(ctx, coef, nullptr, -Pb, s);
+        ctx->launches++;
+        return cudaGetLastError();
+    }
     int PB;
     {
         ProfScope prof(ctx, s);
-        if (Pb <= 1) { PB = 1; launch_stream_t<1>(ctx, p0, Pb, s); }
-        else if (Pb <= 2) { PB = 2; launch_stream_t<2>(ctx, p0, Pb, s); }
-        else if (Pb <= 4) { PB = 4; launch_stream_t<4>(ctx, p0, Pb, s); }
-        else if (Pb <= 8) { PB = 8; launch_stream_t<8>(ctx, p0, Pb, s); }
-        else { PB = 16; launch_stream_t<16>(ctx, p0, Pb, s); }
+        if (Pb <= 1) { PB = 1; launch_stream_t<1>(ctx, coef, wts, Pb, s); }
+        else if (Pb <= 2) { PB = 2; launch_stream_t<2>(ctx, coef, wts, Pb, s); }
+        else if (Pb <= 4) { PB = 4; launch_stream_t<4>(ctx, coef, wts, Pb, s); }
+        else if (Pb <= 8) { PB = 8; launch_stream_t<8>(ctx, coef, wts, Pb, s); }
+        else { PB = 16; launch_stream_t<16>(ctx, coef, wts, Pb, s); }
     }
     const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
     const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;

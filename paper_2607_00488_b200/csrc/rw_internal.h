@@ -43,7 +43,7 @@ struct Consts {
 
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
-    size_t basis, S_sm, What, sat_const, flag;
+    size_t basis, S_sm, What, sat_const, flag, G, ident;
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
@@ -53,6 +53,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int n_tiles_n;        // ceil(n_rec / kBN)
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
+    int ldG;              // row pitch of the prefolded templates G[D][12][ldG] (n_rec rounded up to even)
     int64_t max_batch;
     bool copy_R;
 };
@@ -70,6 +71,7 @@ struct rw_ctx {
     int ldR;
     size_t R_period_stride;   // doubles between periods
     double *basis, *S_sm, *What, *sat_const;
+    double *G, *ident;        // prefolded templates [D][12][ldG]; identity coefficients [16][12] used to fold them
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
@@ -107,8 +109,12 @@ cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, cons
 cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_t s);   // rw_coef.cu
 cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int64_t mu_p0,
                              cudaStream_t s);                                // rw_fold_gemm.cu
-cudaError_t launch_fold_stream(rw_ctx *ctx, int64_t p0, int Pb, double *out_mu,
+cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *wts, int Pb, double *out_mu,
                                cudaStream_t s);                              // rw_fold_stream.cu
+cudaError_t launch_gen_A_weights(rw_ctx *ctx, int d, const double *w, int64_t Pc, cudaStream_t s);  // rw_coef.cu
+cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // rw_collapsed.cu
+cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,
+                             cudaStream_t s);                                // rw_collapsed.cu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
                           bool full_eq18, cudaStream_t s);                   // rw_fold_stream.cu
 int make_tensor_maps(rw_ctx *ctx);                                           // rw_fold_gemm.cu

@@ -1,0 +1,175 @@
+"""GPU parity of the SURVEY.md section 8(f) rows against the oracle, through the C ABI:
+  f-1  RW_MODE_COLLAPSED (rank-K prefolded templates)     vs orc.eval_batch
+  f-3  rw_eval_weights (dense fold on caller weights)     vs orc.eval_weights
+Same bars as the main path: mu 1e-12 relative, -2lnL 1e-9 + 1e-12 * sum 2|term| (reading T)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2607_00488_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+CORES = os.cpu_count() or 4
+
+
+@pytest.fixture(scope="module")
+def rw():
+    import torch
+    from paper_2607_00488_b200 import binding
+    assert torch.cuda.is_available()
+    binding.load_library()
+    return binding
+
+
+def _cuda(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _assert_parity(out, mu, ref, mu_ref, scale):
+    rel = np.abs(mu - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= 1e-12, "mu rel err %.3e" % rel.max()
+    err = np.abs(out - ref)
+    assert np.all(err <= 1e-9 + 1e-12 * scale), "-2lnL err %.3e at %.6e" % (err.max(), ref[err.argmax()])
+
+
+# ------------------------------------------------------------------------------------- f-1 collapsed
+@pytest.mark.parametrize("shape", [dict(n_E=31, n_T=77, n_rec=53, n_periods=2, P=37),
+                                   dict(n_E=40, n_T=203, n_rec=1030, n_periods=3, P=300)])
+def test_collapsed_mode_small_and_ragged(rw, orc, shape):
+    """Odd n_rec (padded template rows), several 512-column strips with a ragged tail, several 64-point
+    groups with a ragged tail, several periods, dead bins, all seven parameter kinds."""
+    import torch
+    P = shape.pop("P")
+    inp = wl.make_custom(seed=11, dead_fraction=0.15, **shape)
+    params, kinds = wl.random_points(P, list(range(7)), seed=12)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=P)
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="collapsed")
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    # literal Eq. 18 form through the collapsed path
+    full = ctx.eval_batch(_cuda(params[:5]), kinds, full_eq18=True, mode="collapsed")
+    ref_full = orc.eval_batch(inp, params[:5], kinds, full_eq18=True)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(full.cpu().numpy() - ref_full) <= 1e-9 + 1e-12 * (scale[:5] + np.abs(ref_full)))
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_tiny_nsi", "cfg2_mm_lowE"])
+def test_collapsed_mode_configs_1_2_all_points(rw, orc, name):
+    import torch
+    inp = wl.make(name)
+    params, kinds = wl.scan_points(name)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=params.shape[0])
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="collapsed")
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    ctx.close()
+
+
+def test_collapsed_templates_are_the_fold_of_the_prescaled_basis(rw):
+    """G[d][b][k] = sum_i W^[d][b][i] R[d][i][k]: the stored templates against a float64 torch matmul of the
+    stored pre-scaled basis (both device tables of the same context; property of the setup step)."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=150, n_rec=61, n_periods=2, seed=13)
+    ctx = rw.Reweighter(inp, max_batch=4)
+    D, n_T, n_rec = inp["R"].shape
+    What = ctx.table(rw.RW_TABLE_WHAT).reshape(D, 12, n_T)
+    G = ctx.table(rw.RW_TABLE_G).reshape(D, 12, -1)
+    R = _cuda(inp["R"])
+    for d in range(D):
+        ref = What[d, :11] @ R[d]
+        got = G[d, :11, :n_rec]
+        assert torch.all((got - ref).abs() <= 1e-13 * ref.abs().max())
+        assert torch.all(G[d, :, n_rec:] == 0) and torch.all(G[d, 11] == 0)
+    ctx.close()
+
+
+def test_collapsed_mode_full_config3_sampled(rw, orc):
+    """Config 3 at full size (10^4 points, 4096 x 2048) in one call; sampled points against the oracle and all
+    points against the dense contraction of the same context."""
+    import torch
+    inp = wl.make("cfg3_nsi4")
+    params, kinds = wl.scan_points("cfg3_nsi4")
+    dev_inp = {k: _cuda(inp[k]) for k in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
+    dev_inp["f_tau"] = inp["f_tau"]
+    ctx = rw.Reweighter(dev_inp, max_batch=10000)
+    p_dev = _cuda(params)
+    out_c = ctx.eval_batch(p_dev, kinds, mode="collapsed")
+    out_g = ctx.eval_batch(p_dev, kinds, mode="gemm")
+    torch.cuda.synchronize()
+    out_c, out_g = out_c.cpu().numpy(), out_g.cpu().numpy()
+    idx = np.unique(np.concatenate([[0, 63, 64, 9999], np.random.default_rng(33).integers(0, 10000, 20)]))
+    ref, scale = orc.eval_batch(inp, params[idx], kinds, want_abs=True, nthreads=CORES)
+    assert np.all(np.abs(out_c[idx] - ref) <= 1e-9 + 1e-12 * scale)
+    assert np.all(np.abs(out_c - out_g) <= 2e-9 + 1e-11 * np.abs(out_g))
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------- f-3 weights
+@pytest.mark.parametrize("mode,P", [("stream", 1), ("stream", 21), ("gemm", 37), ("gemm", 300), ("auto", 33)])
+def test_eval_weights_ragged(rw, orc, mode, P):
+    """Random (not low-rank) weights; n_T = 203 (partial 64-bin transpose tile and partial k-stage),
+    n_rec = 330, 2 periods; ragged 16-point groups / 128-point tiles."""
+    import torch
+    inp = wl.make_custom(n_E=20, n_T=203, n_rec=330, n_periods=2, seed=21)
+    w = np.random.default_rng(22).uniform(0.0, 3.0, size=(P, 203))
+    w[0, :7] = 0.0
+    ref, mu_ref, scale = orc.eval_weights(inp, w, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=max(P, 1))
+    out, mu = ctx.eval_weights(_cuda(w), want_mu=True, mode=mode)
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    ctx.close()
+
+
+def test_eval_weights_reproduces_eval_batch_and_sm_point(rw, orc):
+    """Fed the oracle's spectrum-ratio weights, the weights path gives the oracle's eval_batch numbers;
+    w == 1 gives the SM prediction; the Eq. 18 form and chunking (P > max_batch) work."""
+    import torch
+    inp = wl.make_custom(n_E=31, n_T=77, n_rec=53, n_periods=2, seed=5)
+    params, kinds = wl.random_points(40, [wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU], seed=6)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    w = np.stack([orc.weights(inp, orc.theta_vector(params[p], kinds)) for p in range(40)])
+    ctx = rw.Reweighter(inp, max_batch=16)
+    for mode in ("stream", "gemm"):
+        out, mu = ctx.eval_weights(_cuda(w), want_mu=True, mode=mode)
+        torch.cuda.synchronize()
+        # w itself is rounded to binary64 once: 1 ulp on every term
+        rel = np.abs(mu.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+        assert rel.max() <= 1e-12
+        assert np.all(np.abs(out.cpu().numpy() - ref) <= 1e-9 + 2e-12 * scale)
+    _, mu1 = ctx.eval_weights(_cuda(np.ones((1, 77))), want_mu=True)
+    torch.cuda.synchronize()
+    for d in range(2):
+        sm = inp["N_mc"][d] @ inp["R"][d] + inp["bkg"][d]
+        assert np.all(np.abs(mu1.cpu().numpy()[0, d] / sm - 1) <= 1e-13)
+    full = ctx.eval_weights(_cuda(w[:3]), full_eq18=True)
+    ref_full = orc.eval_weights(inp, w[:3], full_eq18=True)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(full.cpu().numpy() - ref_full) <= 1e-9 + 1e-12 * (scale[:3] + np.abs(ref_full)))
+    with pytest.raises(rw.RwError):
+        ctx.eval_weights(_cuda(w), mode="collapsed")
+    ctx.close()
+
+
+def test_eval_weights_config3_size_sampled(rw, orc):
+    """Config-3-sized dense fold on random weights (4096 x 2048, 1000 points through the DMMA contraction,
+    8 through the streaming fold); sampled rows against the oracle."""
+    import torch
+    inp = wl.make("cfg3_nsi4")
+    rng = np.random.default_rng(44)
+    P = 1000
+    w = rng.uniform(0.5, 1.5, size=(P, 4096))
+    ctx = rw.Reweighter(inp, max_batch=P)
+    out = ctx.eval_weights(_cuda(w))
+    out_s = ctx.eval_weights(_cuda(w[:8]), mode="stream")
+    torch.cuda.synchronize()
+    idx = np.array([0, 1, 7, 127, 128, 999, 500])
+    ref, scale = orc.eval_weights(inp, w[idx], want_abs=True, nthreads=CORES)
+    assert np.all(np.abs(out.cpu().numpy()[idx] - ref) <= 1e-9 + 1e-12 * scale)
+    assert np.all(np.abs(out_s.cpu().numpy()[idx[:3]] - ref[:3]) <= 1e-9 + 1e-12 * scale[:3])
+    ctx.close()
