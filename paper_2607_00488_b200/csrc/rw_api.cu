@@ -85,6 +85,12 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
     L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
     L->out_stage = take((size_t)max_batch * 8);
+    {   // split-K scratch: at most 8 work items per SM, and never more than 16 k-ranges of every 16-point tile
+        int64_t items = (int64_t)L->n_tiles_n * ((L->MC + 15) / 16) * 16;
+        if (items > 8 * kPlanSMs) items = 8 * kPlanSMs;
+        L->mu_tile_items = (int)items;
+        L->mu_tile = take((size_t)items * kBM * kBN * 8);
+    }
     L->total = off;
     return RW_OK;
 }
@@ -119,6 +125,14 @@ static const char *flag_message(int f)
     if (f & 64) return "counts must be finite and >= 0";
     if (f & 128) return "R must be finite and >= 0";
     return "invalid input";
+}
+
+// RW_MODE_AUTO: the HBM-streaming fold for a handful of points (measured on B200: it wins up to 8 points while
+// R is L2-sized, up to 4 points for a 1 GiB R), the DMMA contraction (tile height 16..128, split-K) beyond.
+static bool auto_stream(const rw_ctx *ctx, int64_t P)
+{
+    const size_t r_bytes = (size_t)ctx->D * ctx->n_T * (size_t)ctx->n_rec * 8;
+    return P <= ((r_bytes >= ((size_t)512 << 20)) ? 4 : 8);
 }
 
 }  // namespace rw
@@ -220,6 +234,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->partial = (double *)(ws + L.partial);
     ctx->mu_part = (double *)(ws + L.mu_part);
     ctx->out_stage = (double *)(ws + L.out_stage);
+    ctx->mu_tile = (double *)(ws + L.mu_tile);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;
@@ -326,7 +341,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
         }
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
-        const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && Ps <= 32);
+        const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps));
         if (mode == RW_MODE_COLLAPSED) {
             const int nstrip = (n_rec + 511) / 512;
             for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
@@ -376,7 +391,7 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
     const size_t n_T = ctx->n_T;
-    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && P <= 32);
+    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, P));
     if (stream_mode) {
         const int nstrip2 = (n_rec + 255) / 256;
         for (int64_t g0 = 0; g0 < P; g0 += kStreamMaxPB) {

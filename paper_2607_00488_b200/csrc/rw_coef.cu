@@ -43,7 +43,8 @@ __global__ void k_coef(const double *__restrict__ param, int64_t P, Kinds kd, Co
 constexpr int kGenThreads = 256;   // 32 row-blocks of 8 points
 constexpr int kGenKT = 128;        // recoil bins staged per CTA
 
-// A_packed[mb][kb][r][kk] = N'[p0 + 8 mb + r][8 kb + kk]; rows >= Pc and bins >= n_T are zero.
+// A_packed[mb][kb][r][2 c + e] = N'[p0 + 8 mb + r][8 kb + c + 4 e] (the DMMA A fragment of k-step e is the
+// even/odd half of one 16-byte load); rows >= Pc and bins >= n_T are zero.
 __global__ void __launch_bounds__(kGenThreads)
 k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pad,
         const double *__restrict__ What /*[12][n_T] of this period*/, int n_T, int KPAD, int64_t A_pitch,
@@ -82,11 +83,11 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
         }
         double2 *dst = reinterpret_cast<double2 *>(A + (mb * A_pitch + (size_t)(k0 / 8 + kb) * 64 + r * 8));
 #pragma unroll
-        for (int h = 0; h < 4; ++h) dst[h] = make_double2(v[2 * h], v[2 * h + 1]);
+        for (int h = 0; h < 4; ++h) dst[h] = make_double2(v[h], v[h + 4]);   // bins k and k+4 interleaved
     }
 }
 
-// Caller-supplied weights (rw_eval_weights): A_packed[mb][kb][r][kk] = w[8 mb + r][8 kb + kk] * N_mc[8 kb + kk]
+// Caller-supplied weights (rw_eval_weights): A_packed[mb][kb][r][2 c + e] = (w N_mc)[8 mb + r][8 kb + c + 4 e]
 // (Eq. 1: diag(r) E_true).  A CTA transposes a 64-point x 64-bin tile through shared
 // memory: rows of w are read 512 contiguous bytes per warp, the 8x8 blocks are written 512 contiguous bytes each.
 constexpr int kGwRows = 64, kGwCols = 64;
@@ -118,8 +119,8 @@ k_gen_A_weights(const double *__restrict__ w /*[Pc][n_T]*/, int64_t Pc, int64_t 
         double *dst = A + (mb * A_pitch + (size_t)(k0 / 8 + kb) * 64);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const int e = lane + 32 * h;               // element of the block: r = e / 8, kk = e % 8
-            dst[e] = tile[warp * 8 + (e >> 3)][kb * 8 + (e & 7)];
+            const int e = lane + 32 * h;               // element of the block: r = e / 8, position 2 c + e' = e % 8
+            dst[e] = tile[warp * 8 + (e >> 3)][kb * 8 + ((e & 7) >> 1) + 4 * (e & 1)];
         }
     }
 }

@@ -1,35 +1,45 @@
-// rw_fold_gemm.cu -- steps a3 + a4 for large batches: the response fold as a dense FP64 contraction
+// rw_fold_gemm.cu -- steps a3 + a4 for batched points: the response fold as a dense FP64 contraction
 //   mu[p][k] = sum_i N'[p][i] R[i][k] + bkg[k]      (Eq. 11 / Eq. 1)
 // with the binned Poisson terms of Eq. (18) reduced in the epilogue, so mu never
 // touches HBM.  This is the operation the paper names as its bottleneck.
 //
 // Blackwell has no FP64 path in tcgen05/TMEM; FP64 tensor work is the warp-level DMMA.8x8x4
 // (mma.sync.m8n8k4.f64), measured at 37.1 TFLOP/s on B200.  Design:
-//   * persistent CTAs (one per SM), 128x128 output tile, BK = 16, 6-stage TMA/mbarrier pipeline
-//   * 8 DMMA warps (two per SM sub-partition), 64x32 warp tiles; lane 0 of warp 0 also issues the
+//   * persistent CTAs (one per SM), (16 MB) x 128 output tiles with MB in {1,2,4,8} 8-point row blocks per
+//     warp (tile heights 16/32/64/128 follow the batch size), BK = 16, TMA/mbarrier ring of 6-10 stages
+//   * 8 DMMA warps (two per SM sub-partition) as 2 (points) x 4 (bins); lane 0 of warp 0 also issues the
 //     TMA loads, kStages-2 stage-iterations ahead of the math
-//   * R tiles arrive by TMA as eight 16-column sub-tiles with the 128-byte swizzle; N' arrives as
-//     one 2-D box of the 8x8-blocked A_packed (rw_coef.cu).  The contraction index inside every
-//     group of 8 recoil bins is visited in the order {0,2,4,6},{1,3,5,7}: with that permutation
-//     (legal because it is applied to both operands) every fragment load is one conflict-free
-//     LDS.128 -- A gives the fragments of two k-steps, R gives two adjacent output columns.
-//   * epilogue: + bkg, Poisson term, sum over the thread's 4 adjacent columns, shuffle over the
+//   * an R tile arrives as ONE TMA box of 16 rows x 132 columns (1056-byte rows: long L2 requests instead of
+//     128-byte swizzle atoms; the 4 extra columns make the row pitch = 32 mod 128 bytes, so the four
+//     k-rows a quarter-warp reads fall in four different 32-byte bank groups); N' arrives as one 2-D box
+//     of the 8x8-blocked A_packed (rw_coef.cu), whose blocks interleave k and k+4.  Every fragment load is one
+//     conflict-free LDS.128 -- A gives the fragments of two k-steps, R gives two adjacent output columns.
+//   * the next stage's full barrier is polled before the last DMMA block of a stage, so its latency is hidden
+//   * fused epilogue: + bkg, Poisson term, sum over the thread's 4 adjacent columns, shuffle over the
 //     4 lanes of a row, shared-memory sum over the 4 column warps, one partial per (row, n-tile)
 //     written to partial[d][n_tile][row]; k_reduce adds tiles and periods in a fixed order.
+//   * split-K for what does not fill the machine (small batches; the last partial wave of a large one):
+//     a work item is (tile, k-range), the accumulators go to a per-item scratch tile, and
+//     k_tile_deviance adds the k-ranges in a fixed order, then does the same + bkg / Poisson / row sum.
 #include "rw_internal.h"
 
 namespace rw {
 
-constexpr int kStageBytesA = kBM * kBK * 8;            // 16 KB
-constexpr int kStageBytesB = kBK * kBN * 8;            // 16 KB
-constexpr int kStageBytes = kStageBytesA + kStageBytesB;
-constexpr int kSubTileBytes = kBK * 128;               // one 16-column swizzled sub-tile
-constexpr int kSmemRed = 4 * kBM * 8;                  // [4 column warps][128 rows]
-constexpr int kSmemBars = 2 * kStages * 8;
-constexpr int kGemmSmem = kStages * kStageBytes + kSmemRed + kSmemBars + 1024;
-constexpr int kPrefetch = (kStages > 3) ? kStages - 2 : kStages - 1;                 // stage-iterations the TMA issue runs ahead
-static_assert((kBK == 16 || kBK == 32) && kBM == 128 && kBN == 128, "fragment indexing below assumes this tile");
+constexpr int kBoxCols = kBN + 4;                      // columns per R box: 128 + 4 (pitch 1056 B = 32 mod 128)
+constexpr int kRowBytesB = kBoxCols * 8;
+constexpr int kStageBytesB = kBK * kRowBytesB;         // 16.5 KB of R per stage
 constexpr int kKB = kBK / 8;                           // 8-bin groups per stage
+static_assert(kBK == 16 && kBN == 128, "fragment indexing below assumes this tile");
+
+template <int MB> struct GemmCfg {
+    static constexpr int BM = 16 * MB;                              // points per tile
+    static constexpr int StageBytesA = BM * kBK * 8;                // 2 KB x MB of N' per stage
+    static constexpr int StageBytes = StageBytesA + kStageBytesB;
+    static constexpr int Stages = (MB == 8) ? 6 : (MB == 4) ? 8 : 10;
+    static constexpr int Prefetch = Stages - 2;                     // stage-iterations the TMA issue runs ahead
+    static constexpr int SmemRed = 4 * BM * 8;                      // [4 column warps][BM rows]
+    static constexpr int Smem = Stages * StageBytes + SmemRed + 2 * Stages * 8 + 1024;
+};
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -82,11 +92,6 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-#ifdef RW_GEMM_STATS
-__device__ unsigned long long g_gemm_stats[148 * 8];
-__device__ __forceinline__ long long clk() { long long t; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t)); return t; }
-#endif
-
 struct TileCoord { int m, n; };
 __device__ __forceinline__ TileCoord tile_coord(int t, int tiles_m, int tiles_n)
 {
@@ -101,19 +106,28 @@ __device__ __forceinline__ TileCoord tile_coord(int t, int tiles_m, int tiles_n)
     return tc;
 }
 
+// One launch covers tiles [tile0, tile0 + n_tiles) of the (tiles_m x tiles_n) grid, each cut into S k-ranges of
+// kps stage-iterations.  S == 1: fused Poisson epilogue.  S > 1: accumulators -> mu_tile[item][BM][128].
+struct GemmWork {
+    int n_T, n_rec, tiles_m, tiles_n, tile0, n_tiles, S, kps, D, d;
+    int64_t Pc, part_stride;
+    const double *bkg, *counts;
+    double *partial, *out_mu, *mu_tile;
+};
+
+template <int MB>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapR,
-            int n_T, int n_rec, int64_t Pc, int tiles_m, int tiles_n,
-            const double *__restrict__ bkg, const double *__restrict__ counts,
-            double *__restrict__ partial /*[tiles_n][part_stride]*/, int64_t part_stride,
-            double *__restrict__ out_mu /*NULL or rows of this chunk, [.][D][n_rec]*/, int D, int d)
+            const GemmWork W)
 {
+    using Cfg = GemmCfg<MB>;
+    constexpr int BM = Cfg::BM, kStages = Cfg::Stages;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t sbase = smem_u32(smem);
-    const uint32_t full_bar = sbase + kStages * kStageBytes + kSmemRed;
+    const uint32_t full_bar = sbase + kStages * Cfg::StageBytes + Cfg::SmemRed;
     const uint32_t empty_bar = full_bar + kStages * 8;
-    double *red = reinterpret_cast<double *>(smem + kStages * kStageBytes);
+    double *red = reinterpret_cast<double *>(smem + kStages * Cfg::StageBytes);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -125,90 +139,80 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
     }
     __syncthreads();
 
-    const int k_iters = (n_T + kBK - 1) / kBK;
-    const int total_tiles = tiles_m * tiles_n;
+    const int k_iters = (W.n_T + kBK - 1) / kBK;
+    const int total_items = W.n_tiles * W.S;
+    const int tiles_m = W.tiles_m, tiles_n = W.tiles_n, S = W.S, kps = W.kps;
 
     // ---------------------------------------------------------------------- TMA producer duty
-    // Lane 0 of warp 0 runs kPrefetch stage-iterations ahead of the consumers.  (A dedicated
+    // Lane 0 of warp 0 runs Prefetch stage-iterations ahead of the consumers.  (A dedicated
     // producer warp would put three warps on one SM sub-partition and cap every thread at 168
-    // registers; the 64x32 FP64 warp tile needs ~230.)
+    // registers; the 64x32 FP64 warp tile of MB = 8 needs ~236.)
     const bool is_producer = threadIdx.x == 0;
-    int p_t = blockIdx.x, p_kt = 0, p_stage = 0;
+    int p_item = blockIdx.x, p_kt = 0, p_kt1 = 0, p_stage = 0;
     uint32_t p_phase = 0;
-    TileCoord p_tc = tile_coord(p_t < total_tiles ? p_t : 0, tiles_m, tiles_n);
+    TileCoord p_tc = {0, 0};
+    auto producer_open = [&]() {      // position the producer on item p_item
+        if (p_item >= total_items) return;
+        const int tl = p_item / S, ks = p_item - tl * S;
+        p_tc = tile_coord(W.tile0 + tl, tiles_m, tiles_n);
+        p_kt = ks * kps;
+        p_kt1 = min(k_iters, p_kt + kps);
+    };
     auto produce_one = [&]() {
-        if (p_t >= total_tiles) return;
+        if (p_item >= total_items) return;
         mbar_wait(empty_bar + 8 * p_stage, p_phase ^ 1);
         const uint32_t fb = full_bar + 8 * p_stage;
-        mbar_expect_tx(fb, kStageBytes);
-        const uint32_t dstA = sbase + p_stage * kStageBytes;
-        tma_load_2d(dstA, &tmapA, p_kt * kBK * 8, p_tc.m * (kBM / 8), fb);
-        const uint32_t dstB = dstA + kStageBytesA;
-#pragma unroll
-        for (int j = 0; j < kBN / 16; ++j)
-            tma_load_2d(dstB + j * kSubTileBytes, &tmapR, p_tc.n * kBN + 16 * j, p_kt * kBK, fb);
+        mbar_expect_tx(fb, Cfg::StageBytes);
+        const uint32_t dstA = sbase + p_stage * Cfg::StageBytes;
+        tma_load_2d(dstA, &tmapA, p_kt * kBK * 8, p_tc.m * (BM / 8), fb);
+        tma_load_2d(dstA + Cfg::StageBytesA, &tmapR, p_tc.n * kBN, p_kt * kBK, fb);
         if (++p_stage == kStages) { p_stage = 0; p_phase ^= 1; }
-        if (++p_kt == k_iters) {
-            p_kt = 0;
-            p_t += gridDim.x;
-            if (p_t < total_tiles) p_tc = tile_coord(p_t, tiles_m, tiles_n);
+        if (++p_kt == p_kt1) {
+            p_item += gridDim.x;
+            producer_open();
         }
     };
     if (is_producer) {
+        producer_open();
 #pragma unroll 1
-        for (int q = 0; q < kPrefetch; ++q) produce_one();
+        for (int q = 0; q < Cfg::Prefetch; ++q) produce_one();
     }
 
     // ---------------------------------------------------------------------- DMMA consumers
     const int wm = warp >> 2, wn = warp & 3;
     const int r = lane >> 2, c = lane & 3;
-    // A: block (8 wm + mb, kb) is 512 contiguous bytes, lane reads its 16 bytes
-    const uint32_t a_off = (uint32_t)(wm * 8 * kKB) * 512 + lane * 16;
-    // R: sub-tile (2 wn + sj), row 8 kb + 2c + s, 16-byte chunk (r ^ (2c + s))
+    // A: block (MB wm + mb, kb) is 512 contiguous bytes, lane reads its 16 bytes
+    const uint32_t a_off = (uint32_t)(wm * MB * kKB) * 512 + lane * 16;
+    // R: row 8 kb + c + 4 s, columns 32 wn + 16 sj + 2 r + {0,1}
     uint32_t b_off[2];
 #pragma unroll
     for (int s = 0; s < 2; ++s)
-        b_off[s] = kStageBytesA + (uint32_t)(2 * wn) * kSubTileBytes + (uint32_t)(2 * c + s) * 128 +
-                   (uint32_t)((r ^ (2 * c + s)) * 16);
+        b_off[s] = Cfg::StageBytesA + (uint32_t)(c + 4 * s) * kRowBytesB + (uint32_t)(32 * wn + 2 * r) * 8;
 
     int stage = 0;
     uint32_t phase = 0;
     uint32_t ready = 0;      // result of the early poll of the next stage's full barrier
-    for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-        const TileCoord tc = tile_coord(t, tiles_m, tiles_n);
-        double acc[8][2][2][2];
+    for (int item = blockIdx.x; item < total_items; item += gridDim.x) {
+        const int tl = item / S, ks = item - tl * S;
+        const TileCoord tc = tile_coord(W.tile0 + tl, tiles_m, tiles_n);
+        const int kt0 = ks * kps, kt1 = min(k_iters, kt0 + kps);
+        double acc[MB][2][2][2];
 #pragma unroll
-        for (int mb = 0; mb < 8; ++mb)
+        for (int mb = 0; mb < MB; ++mb)
 #pragma unroll
             for (int sj = 0; sj < 2; ++sj)
 #pragma unroll
                 for (int nb = 0; nb < 2; ++nb) acc[mb][sj][nb][0] = acc[mb][sj][nb][1] = 0.0;
 
-        for (int kt = 0; kt < k_iters; ++kt) {
+        for (int kt = kt0; kt < kt1; ++kt) {
             if (is_producer) produce_one();
-#ifdef RW_GEMM_STATS
-            {
-                long long t0 = clk();
-                mbar_wait(full_bar + 8 * stage, phase);
-                long long dt = clk() - t0;
-                if (threadIdx.x == 32 && blockIdx.x < 148) {
-                    unsigned long long *st = g_gemm_stats + blockIdx.x * 8;
-                    st[0] += dt; st[1] += 1;
-                    if (dt > 500) st[2] += 1;
-                    if (dt > 4000) st[3] += 1;
-                    if ((unsigned long long)dt > st[4]) st[4] = dt;
-                    if (kt < 4) st[5] += dt;
-                }
-            }
-#else
             if (!ready) mbar_wait(full_bar + 8 * stage, phase);
-#endif
-            const uint32_t st = sbase + stage * kStageBytes;
+            const uint32_t st = sbase + stage * Cfg::StageBytes;
 #pragma unroll
             for (int kb = 0; kb < kKB; ++kb) {
-                double2 a[8], b[2][2];
+                double2 a[MB], b[2][2];
 #pragma unroll
-                for (int mb = 0; mb < 8; ++mb)
+                for (int mb = 0; mb < MB; ++mb)
                     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];"
                                  : "=d"(a[mb].x), "=d"(a[mb].y)
                                  : "r"(st + a_off + (uint32_t)(mb * kKB + kb) * 512));
@@ -218,17 +222,17 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                     for (int s = 0; s < 2; ++s)
                         asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];"
                                      : "=d"(b[sj][s].x), "=d"(b[sj][s].y)
-                                     : "r"(st + b_off[s] + (uint32_t)sj * kSubTileBytes + (uint32_t)kb * 1024));
+                                     : "r"(st + b_off[s] + (uint32_t)sj * 128 + (uint32_t)kb * (8 * kRowBytesB)));
                 if (kb == kKB - 1) {
                     // poll the next stage's barrier now: the result is back by the time the last
-                    // 64 DMMAs of this stage have issued, so the wait below costs no pipe bubble
+                    // DMMA block of this stage has issued, so the wait above costs no pipe bubble
                     const int ns = (stage + 1 == kStages) ? 0 : stage + 1;
                     ready = mbar_test(full_bar + 8 * ns, (stage + 1 == kStages) ? (phase ^ 1) : phase);
                 }
 #pragma unroll
                 for (int s = 0; s < 2; ++s)
 #pragma unroll
-                    for (int mb = 0; mb < 8; ++mb) {
+                    for (int mb = 0; mb < MB; ++mb) {
                         const double av = s ? a[mb].y : a[mb].x;
 #pragma unroll
                         for (int sj = 0; sj < 2; ++sj) {
@@ -242,21 +246,36 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
             if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
 
+        const int lrow0 = wm * (8 * MB) + r;                    // row within the tile, + 8 mb
+        const int lcol0 = wn * 32 + 4 * c;                      // column within the tile, + 16 sj + {0,1,2,3}
+        if (S > 1) {
+            // ---------------------------------------------------------------- split-K: park the accumulators
+            double *dst = W.mu_tile + (size_t)item * (BM * kBN);
+#pragma unroll
+            for (int mb = 0; mb < MB; ++mb)
+#pragma unroll
+                for (int sj = 0; sj < 2; ++sj) {
+                    double2 *q = reinterpret_cast<double2 *>(dst + (size_t)(lrow0 + 8 * mb) * kBN + lcol0 + 16 * sj);
+                    q[0] = make_double2(acc[mb][sj][0][0], acc[mb][sj][1][0]);
+                    q[1] = make_double2(acc[mb][sj][0][1], acc[mb][sj][1][1]);
+                }
+            continue;
+        }
         // ------------------------------------------------------------------ fused epilogue
-        const int row0 = tc.m * kBM + wm * 64 + r;              // + 8 mb
-        const int col0 = tc.n * kBN + wn * 32 + 4 * c;          // + 16 sj + {0,1,2,3}
+        const int row0 = tc.m * BM + lrow0;
+        const int col0 = tc.n * kBN + lcol0;
         double bk[2][4], cn[2][4];
 #pragma unroll
         for (int sj = 0; sj < 2; ++sj)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int col = col0 + 16 * sj + q;
-                const bool ok = col < n_rec;
-                bk[sj][q] = ok ? __ldg(bkg + col) : 0.0;
-                cn[sj][q] = ok ? __ldg(counts + col) : 0.0;
+                const bool ok = col < W.n_rec;
+                bk[sj][q] = ok ? __ldg(W.bkg + col) : 0.0;
+                cn[sj][q] = ok ? __ldg(W.counts + col) : 0.0;
             }
 #pragma unroll
-        for (int mb = 0; mb < 8; ++mb) {
+        for (int mb = 0; mb < MB; ++mb) {
             double sum = 0.0;
 #pragma unroll
             for (int sj = 0; sj < 2; ++sj)
@@ -267,26 +286,67 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                         const int q = 2 * e + nb;
                         const double mu = acc[mb][sj][nb][e] + bk[sj][q];
                         const int col = col0 + 16 * sj + q;
-                        if (col < n_rec) {
+                        if (col < W.n_rec) {
                             sum += poisson_term(mu, cn[sj][q]);
-                            if (out_mu) {
+                            if (W.out_mu) {
                                 const int64_t row = row0 + 8 * mb;
-                                if (row < Pc) out_mu[((size_t)row * D + d) * n_rec + col] = mu;
+                                if (row < W.Pc) W.out_mu[((size_t)row * W.D + W.d) * W.n_rec + col] = mu;
                             }
                         }
                     }
             sum += __shfl_xor_sync(0xffffffffu, sum, 1);
             sum += __shfl_xor_sync(0xffffffffu, sum, 2);
-            if (c == 0) red[wn * kBM + wm * 64 + 8 * mb + r] = sum;
+            if (c == 0) red[wn * BM + lrow0 + 8 * mb] = sum;
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (threadIdx.x < kBM) {
-            const int64_t row = (int64_t)tc.m * kBM + threadIdx.x;
-            const double v = (red[threadIdx.x] + red[kBM + threadIdx.x]) +
-                             (red[2 * kBM + threadIdx.x] + red[3 * kBM + threadIdx.x]);
-            if (row < Pc) partial[(size_t)tc.n * part_stride + row] = v;
+        if (threadIdx.x < BM) {
+            const int64_t row = (int64_t)tc.m * BM + threadIdx.x;
+            const double v = (red[threadIdx.x] + red[BM + threadIdx.x]) +
+                             (red[2 * BM + threadIdx.x] + red[3 * BM + threadIdx.x]);
+            if (row < W.Pc) W.partial[(size_t)tc.n * W.part_stride + row] = v;
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
+    }
+}
+
+// Split-K finish: mu = sum over the S k-ranges (fixed order) + bkg, Poisson term, row sum over the tile's 128
+// columns -> partial[n_tile][row], exactly the slot the fused epilogue fills.  One CTA per tile, one warp per row.
+__global__ void __launch_bounds__(256)
+k_tile_deviance(const double *__restrict__ mu_tile, int BM, int S, int tile0, int tiles_m, int tiles_n,
+                int n_rec, int64_t Pc, const double *__restrict__ bkg, const double *__restrict__ counts,
+                double *__restrict__ partial, int64_t part_stride, double *__restrict__ out_mu, int D, int d)
+{
+    const TileCoord tc = tile_coord(tile0 + blockIdx.x, tiles_m, tiles_n);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int col = tc.n * kBN + 4 * lane;
+    double bk[4], cn[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const bool ok = col + q < n_rec;
+        bk[q] = ok ? bkg[col + q] : 0.0;
+        cn[q] = ok ? counts[col + q] : 0.0;
+    }
+    const double *base = mu_tile + (size_t)blockIdx.x * S * (BM * kBN);
+    for (int lr = warp; lr < BM; lr += 8) {
+        const int64_t row = (int64_t)tc.m * BM + lr;
+        double m[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int s = 0; s < S; ++s) {
+            const double2 *q = reinterpret_cast<const double2 *>(base + ((size_t)s * BM + lr) * kBN + 4 * lane);
+            const double2 u = q[0], v = q[1];
+            m[0] += u.x; m[1] += u.y; m[2] += v.x; m[3] += v.y;
+        }
+        double sum = 0.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const double mu = m[q] + bk[q];
+            if (col + q < n_rec) {
+                sum += poisson_term(mu, cn[q]);
+                if (out_mu && row < Pc) out_mu[((size_t)row * D + d) * n_rec + col + q] = mu;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0 && row < Pc) partial[(size_t)tc.n * part_stride + row] = sum;
     }
 }
 
@@ -309,27 +369,17 @@ static PFN_encodeTiled get_encode()
     return fn;
 }
 
-#ifdef RW_GEMM_STATS
-extern "C" int rw_debug_gemm_stats(unsigned long long *host_out, int reset)
-{
-    cudaDeviceSynchronize();
-    if (host_out) cudaMemcpyFromSymbol(host_out, g_gemm_stats, sizeof(unsigned long long) * 148 * 8);
-    if (reset) { static unsigned long long z[148 * 8]; cudaMemcpyToSymbol(g_gemm_stats, z, sizeof(z)); }
-    return 0;
-}
-#endif
-
 int make_tensor_maps(rw_ctx *ctx)
 {
     PFN_encodeTiled enc = get_encode();
     if (!enc) return fail(ctx, RW_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
     const Layout &L = ctx->lay;
-    {
+    for (int v = 0; v < 4; ++v) {            // one map of N' per tile height 16 << v (the box is part of the map)
         cuuint64_t dims[2] = {(cuuint64_t)L.KPAD * 8, (cuuint64_t)(L.MC / 8)};
         cuuint64_t strides[1] = {(cuuint64_t)L.A_pitch * sizeof(double)};
-        cuuint32_t box[2] = {kBK * 8, kBM / 8};
+        cuuint32_t box[2] = {kBK * 8, (cuuint32_t)(2 << v)};
         cuuint32_t estr[2] = {1, 1};
-        CUresult r = enc(&ctx->tmapA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, ctx->A_packed, dims, strides, box, estr,
+        CUresult r = enc(&ctx->tmapA[v], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, ctx->A_packed, dims, strides, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(ctx, RW_ERR_CUDA, "cuTensorMapEncodeTiled(A) failed: %d", (int)r);
@@ -337,32 +387,99 @@ int make_tensor_maps(rw_ctx *ctx)
     for (int d = 0; d < ctx->D; ++d) {
         cuuint64_t dims[2] = {(cuuint64_t)ctx->n_rec, (cuuint64_t)ctx->n_T};
         cuuint64_t strides[1] = {(cuuint64_t)ctx->ldR * sizeof(double)};
-        cuuint32_t box[2] = {16, kBK};
+        cuuint32_t box[2] = {kBoxCols, kBK};
         cuuint32_t estr[2] = {1, 1};
         void *base = const_cast<double *>(ctx->R + (size_t)d * ctx->R_period_stride);
         CUresult r = enc(&ctx->tmapR[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(ctx, RW_ERR_CUDA, "cuTensorMapEncodeTiled(R[%d]) failed: %d", d, (int)r);
     }
-    cudaError_t e = cudaFuncSetAttribute(k_fold_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    cudaError_t e = cudaFuncSetAttribute(k_fold_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<1>::Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<2>::Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<4>::Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_gemm<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<8>::Smem);
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
     return RW_OK;
+}
+
+template <int MB>
+static void launch_gemm_t(rw_ctx *ctx, int d, const GemmWork &W, int grid, cudaStream_t s)
+{
+    ProfScope prof(ctx, s);
+    k_fold_gemm<MB><<<grid, kGemmThreads, GemmCfg<MB>::Smem, s>>>(ctx->tmapA[MB == 1 ? 0 : MB == 2 ? 1 : MB == 4 ? 2 : 3],
+                                                                  ctx->tmapR[d], W);
+    ctx->launches++;
+}
+
+static void launch_gemm_any(rw_ctx *ctx, int MB, int d, const GemmWork &W, cudaStream_t s)
+{
+    const int items = W.n_tiles * W.S;
+    const int grid = items < ctx->num_sms ? items : ctx->num_sms;
+    switch (MB) {
+    case 1: launch_gemm_t<1>(ctx, d, W, grid, s); break;
+    case 2: launch_gemm_t<2>(ctx, d, W, grid, s); break;
+    case 4: launch_gemm_t<4>(ctx, d, W, grid, s); break;
+    default: launch_gemm_t<8>(ctx, d, W, grid, s); break;
+    }
+}
+
+// Tile height for a chunk of Pc points: the smallest of 16/32/64/128 that holds it, 128 beyond.
+int gemm_rows_per_warp_block(int64_t Pc) { return Pc <= 16 ? 1 : Pc <= 32 ? 2 : Pc <= 64 ? 4 : 8; }
+
+// Split factor for `tail` tiles that do not fill the machine: the smallest S <= s_max whose S*tail work items
+// use >= 90 % of the SM slots of the waves they occupy, else the best one.
+int gemm_tail_split(int tail, int num_sms, int k_iters, int max_items)
+{
+    int s_max = k_iters / 8;
+    if (s_max > 16) s_max = 16;
+    if (s_max > max_items / tail) s_max = max_items / tail;
+    if (s_max < 1) s_max = 1;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int S = 1; S <= s_max; ++S) {
+        const int kps = (k_iters + S - 1) / S;
+        if ((S - 1) * kps >= k_iters) continue;                       // an empty k-range
+        const int items = tail * S;
+        const double eff = (double)items / ((double)((items + num_sms - 1) / num_sms) * num_sms);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = S; }
+        if (eff >= 0.9) break;
+    }
+    return best;
 }
 
 cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int64_t /*mu_p0*/, cudaStream_t s)
 {
     const Layout &L = ctx->lay;
-    const int tiles_m = (int)((Pc + kBM - 1) / kBM);
-    const int tiles_n = L.n_tiles_n;
-    const int total = tiles_m * tiles_n;
-    const int grid = total < ctx->num_sms ? total : ctx->num_sms;
-    double *part = ctx->partial + (size_t)d * tiles_n * L.MC;
-    ProfScope prof(ctx, s);
-    k_fold_gemm<<<grid, kGemmThreads, kGemmSmem, s>>>(
-        ctx->tmapA, ctx->tmapR[d], ctx->n_T, ctx->n_rec, Pc, tiles_m, tiles_n,
-        ctx->bkg + (size_t)d * ctx->n_rec, ctx->counts + (size_t)d * ctx->n_rec, part, L.MC, out_mu, ctx->D, d);
-    ctx->launches++;
+    const int MB = gemm_rows_per_warp_block(Pc);
+    const int BM = 16 * MB;
+    GemmWork W;
+    W.n_T = ctx->n_T; W.n_rec = ctx->n_rec; W.D = ctx->D; W.d = d;
+    W.tiles_m = (int)((Pc + BM - 1) / BM);
+    W.tiles_n = L.n_tiles_n;
+    W.Pc = Pc; W.part_stride = L.MC;
+    W.bkg = ctx->bkg + (size_t)d * ctx->n_rec;
+    W.counts = ctx->counts + (size_t)d * ctx->n_rec;
+    W.partial = ctx->partial + (size_t)d * W.tiles_n * L.MC;
+    W.out_mu = out_mu;
+    W.mu_tile = ctx->mu_tile;
+    const int k_iters = (ctx->n_T + kBK - 1) / kBK;
+    const int total = W.tiles_m * W.tiles_n;
+    int full = total / ctx->num_sms * ctx->num_sms;
+    int tail = total - full;
+    int S = tail ? gemm_tail_split(tail, ctx->num_sms, k_iters, L.mu_tile_items) : 1;
+    if (S == 1) { full = total; tail = 0; }
+    if (full) {
+        W.tile0 = 0; W.n_tiles = full; W.S = 1; W.kps = k_iters;
+        launch_gemm_any(ctx, MB, d, W, s);
+    }
+    if (tail) {
+        W.tile0 = full; W.n_tiles = tail; W.S = S; W.kps = (k_iters + S - 1) / S;
+        launch_gemm_any(ctx, MB, d, W, s);
+        k_tile_deviance<<<tail, 256, 0, s>>>(ctx->mu_tile, BM, S, full, W.tiles_m, W.tiles_n, ctx->n_rec, Pc, W.bkg,
+                                             W.counts, W.partial, W.part_stride, out_mu, ctx->D, d);
+        ctx->launches++;
+    }
     return cudaGetLastError();
 }
 

@@ -44,7 +44,7 @@ struct Consts {
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident;
-    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage;
+    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
@@ -53,6 +53,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int n_tiles_n;        // ceil(n_rec / kBN)
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
+    int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
     int ldG;              // row pitch of the prefolded templates G[D][12][ldG] (n_rec rounded up to even)
     int64_t max_batch;
     bool copy_R;
@@ -75,8 +76,9 @@ struct rw_ctx {
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
+    double *mu_tile;          // split-K scratch: [mu_tile_items][<=128][128] parked accumulators
     CUtensorMap *tmapR;       // host array [D]
-    CUtensorMap tmapA;
+    CUtensorMap tmapA[4];     // N' maps for tile heights 16, 32, 64, 128
     int num_sms;
     int64_t launches;
     // measurement hooks (rw_profile_begin/end)
@@ -118,6 +120,8 @@ cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
                           bool full_eq18, cudaStream_t s);                   // rw_fold_stream.cu
 int make_tensor_maps(rw_ctx *ctx);                                           // rw_fold_gemm.cu
+int gemm_rows_per_warp_block(int64_t Pc);                                    // rw_fold_gemm.cu
+int gemm_tail_split(int tail, int num_sms, int k_iters, int max_items);      // rw_fold_gemm.cu
 
 // Brackets one fold-kernel launch with CUDA events while profiling is on (rw_api.cu).
 struct ProfScope {

@@ -58,6 +58,16 @@ def test_multi_tile_problem(rw, orc, mode):
     _check(rw, orc, inp, params, kinds, mode)
 
 
+@pytest.mark.parametrize("P", [5, 16, 17, 32, 50, 64, 100, 129])
+def test_contraction_tile_heights_and_split_k(rw, orc, P):
+    """Every tile height of the DMMA contraction (16/32/64/128 points) with a contraction long enough to be
+    split into k-ranges (n_T = 1500: 94 stage-iterations, ragged last one), 3 column tiles with a ragged tail,
+    2 periods: the parked accumulators of the k-ranges must add up to the oracle's mu."""
+    inp = wl.make_custom(n_E=24, n_T=1500, n_rec=330, n_periods=2, seed=17, dead_fraction=0.1)
+    params, kinds = wl.random_points(P, list(range(7)), seed=18)
+    _check(rw, orc, inp, params, kinds, "gemm")
+
+
 @pytest.mark.parametrize("mode", ["stream", "gemm"])
 def test_config1_all_points(rw, orc, mode):
     inp = wl.make("cfg1_tiny_nsi")
