@@ -144,39 +144,42 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
     const int tiles_m = W.tiles_m, tiles_n = W.tiles_n, S = W.S, kps = W.kps;
 
     // ---------------------------------------------------------------------- TMA producer duty
-    // Lane 0 of warp 0 runs Prefetch stage-iterations ahead of the consumers.  (A dedicated
-    // producer warp would put three warps on one SM sub-partition and cap every thread at 168
+    // Every warp tracks the load sequence (one load = one stage of one work item), Prefetch loads ahead of its
+    // own math; load number q is issued by lane 0 of warp q % 8.  Rotating the duty keeps the eight warps'
+    // work equal: with a fixed producer warp that warp is the slowest, the other seven run ahead until they
+    // all wait on the load it has just issued, and the pipeline depth hides its lag instead of the latency.
+    // (A dedicated producer warp would put three warps on one SM sub-partition and cap every thread at 168
     // registers; the 64x32 FP64 warp tile of MB = 8 needs ~236.)
-    const bool is_producer = threadIdx.x == 0;
-    int p_item = blockIdx.x, p_kt = 0, p_kt1 = 0, p_stage = 0;
+    int p_item = blockIdx.x, p_kt = 0, p_kt1 = 0, p_stage = 0, p_seq = 0;
     uint32_t p_phase = 0;
     TileCoord p_tc = {0, 0};
-    auto producer_open = [&]() {      // position the producer on item p_item
+    auto producer_open = [&]() {      // position the load sequence on item p_item
         if (p_item >= total_items) return;
         const int tl = p_item / S, ks = p_item - tl * S;
         p_tc = tile_coord(W.tile0 + tl, tiles_m, tiles_n);
         p_kt = ks * kps;
         p_kt1 = min(k_iters, p_kt + kps);
     };
-    auto produce_one = [&]() {
+    auto produce_step = [&]() {
         if (p_item >= total_items) return;
-        mbar_wait(empty_bar + 8 * p_stage, p_phase ^ 1);
-        const uint32_t fb = full_bar + 8 * p_stage;
-        mbar_expect_tx(fb, Cfg::StageBytes);
-        const uint32_t dstA = sbase + p_stage * Cfg::StageBytes;
-        tma_load_2d(dstA, &tmapA, p_kt * kBK * 8, p_tc.m * (BM / 8), fb);
-        tma_load_2d(dstA + Cfg::StageBytesA, &tmapR, p_tc.n * kBN, p_kt * kBK, fb);
+        if ((p_seq & (kGemmConsumerWarps - 1)) == warp && lane == 0) {
+            mbar_wait(empty_bar + 8 * p_stage, p_phase ^ 1);
+            const uint32_t fb = full_bar + 8 * p_stage;
+            mbar_expect_tx(fb, Cfg::StageBytes);
+            const uint32_t dstA = sbase + p_stage * Cfg::StageBytes;
+            tma_load_2d(dstA, &tmapA, p_kt * kBK * 8, p_tc.m * (BM / 8), fb);
+            tma_load_2d(dstA + Cfg::StageBytesA, &tmapR, p_tc.n * kBN, p_kt * kBK, fb);
+        }
+        ++p_seq;
         if (++p_stage == kStages) { p_stage = 0; p_phase ^= 1; }
         if (++p_kt == p_kt1) {
             p_item += gridDim.x;
             producer_open();
         }
     };
-    if (is_producer) {
-        producer_open();
+    producer_open();
 #pragma unroll 1
-        for (int q = 0; q < Cfg::Prefetch; ++q) produce_one();
-    }
+    for (int q = 0; q < Cfg::Prefetch; ++q) produce_step();
 
     // ---------------------------------------------------------------------- DMMA consumers
     const int wm = warp >> 2, wn = warp & 3;
@@ -205,7 +208,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                 for (int nb = 0; nb < 2; ++nb) acc[mb][sj][nb][0] = acc[mb][sj][nb][1] = 0.0;
 
         for (int kt = kt0; kt < kt1; ++kt) {
-            if (is_producer) produce_one();
+            produce_step();
             if (!ready) mbar_wait(full_bar + 8 * stage, phase);
             const uint32_t st = sbase + stage * Cfg::StageBytes;
 #pragma unroll
