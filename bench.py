@@ -254,6 +254,35 @@ def main():
               "hbm_peak_gbs": peaks["hbm_gbs"], "note": "P=1, streaming fold; R (%.2f GB) >> L2, so every eval reads it from HBM" % (r_bytes / 1e9)}
     single["hbm_frac"] = single["hbm_gbs"] / peaks["hbm_gbs"]
 
+    # ---------------------------------------------------------------- other regimes of the same path (context lines)
+    def timed(fn, reps):
+        fn(); fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    sweep = []
+    for Pb in (1, 4, 16, 64, 256, 2048):
+        if Pb > P:
+            break
+        pb = param_dev[:Pb].contiguous()
+        ob = torch.empty(Pb, dtype=torch.float64, device=dev)
+        t = timed(lambda: ctx.eval_batch(pb, kinds, out=ob), 20 if Pb <= 256 else 5)
+        sweep.append({"points": Pb, "ms_per_call": t, "evals_per_s": Pb / t * 1e3,
+                      "fold_tflops": 2.0 * n_T * n_rec * D * Pb / t / 1e9, "response_gbs": r_bytes / t / 1e6})
+    # opt-in rank-K collapsed mode: exact, O(11 n_rec) per point, FP64-ALU bound; never mixed into `value`
+    out_c = torch.empty(P, dtype=torch.float64, device=dev)
+    t_c = timed(lambda: ctx.eval_batch(param_dev, kinds, out=out_c, mode="collapsed"), 5)
+    dmax = float((out_c - out_dev).abs().max().item())
+    collapsed = {"ms_per_call": t_c, "evals_per_s": P / t_c * 1e3, "bound": "alu",
+                 "algorithmic_gflops": 2.0 * 11 * n_rec * D * P / t_c / 1e6,
+                 "max_abs_diff_vs_dense_fold": dmax,
+                 "note": "2*11*n_rec*D flop per point plus one log1p per bin; see profiles/ for the FP64-pipe utilisation"}
+
     # ---------------------------------------------------------------- roofline of the dominant kernel
     dmma_peak = binding.probe_fp64_peak(1)
     dfma_peak = binding.probe_fp64_peak(0)
@@ -289,6 +318,7 @@ def main():
                         "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path": same},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
+                "batch_sweep": sweep, "collapsed_mode": collapsed,
                 "clocks": clocks, "all_finite": finite,
                 "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
                                  "the authors' own multi-component model; other hardware and inputs, not comparable"}

@@ -30,6 +30,9 @@
  *   orc_eq18          vs -2*sum(scipy.stats.poisson.logpmf)
  *   orc_eval_batch    composition of the above; Asimov injection-recovery
  *                     (PAPER.md:309-311); rank-K prefold identity
+ *   orc_profile_scale closed form s^ = sum n / sum S (no background, no pull); Asimov data at s* => s^ = s*,
+ *                     value 0; scipy.optimize.minimize_scalar on a numpy objective;
+ *                     pull limits sigma -> 0 (s^ -> s0) and sigma -> inf; boundary s^ = 0
  *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
  *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
@@ -319,6 +322,117 @@ int orc_eval_batch(const orc_consts *c, int n_E, const double *E, const double *
         free(S);
     }
     free(S0);
+    return 0;
+}
+
+/* Profiled overall rate normalisation (Sec. VI B: "profiling an overall rate normalization at
+ * each scan point"; rate_k of Eq. 17; Gaussian constraint of Eq. 18).
+ * Given the signal prediction S[j] >= 0 (fold at unit normalisation, background removed), background B[j] and
+ * counts n[j] over all bins of all periods:
+ *     mu_j(s) = s S_j + B_j,   f(s) = 2 sum_j [mu_j - n_j + n_j ln(n_j/mu_j)] + ((s - s0)/sigma)^2   (pull iff sigma > 0)
+ * returns s^ = argmin_{s >= 0} f(s) and f(s^).  f is convex in s (reading R13), so the minimiser is
+ * the root of f' (or 0 when f'(0) >= 0); it is bracketed by doubling and found by bisection in long double.
+ * With full_eq18 the value is the literal Eq. (18) sum at s^ instead of the deviance (same minimiser). */
+static xreal xprofile_dfds(int n, const xreal *S, const double *B, const double *cnt, xreal s, xreal s0, xreal sigma)
+{
+    xreal acc = 0.0L;
+    for (int j = 0; j < n; ++j) {
+        xreal mu = s * S[j] + (xreal)B[j];
+        if (cnt[j] > 0.0) {
+            if (S[j] != 0.0L) acc += S[j] * (1.0L - (xreal)cnt[j] / mu);   /* mu = 0 => -inf: pushes s up */
+        } else {
+            acc += S[j];
+        }
+    }
+    acc *= 2.0L;
+    if (sigma > 0.0L) acc += 2.0L * (s - s0) / (sigma * sigma);
+    return acc;
+}
+
+static xreal xprofile_scale(int n, const xreal *S, const double *B, const double *cnt, xreal s0, xreal sigma,
+                            int full_eq18, xreal *f_min)
+{
+    xreal s_hat;
+    xreal lo = 0.0L, hi = 1.0L;
+    if (!(xprofile_dfds(n, S, B, cnt, 0.0L, s0, sigma) < 0.0L)) {
+        s_hat = 0.0L;                                  /* f increasing on s >= 0: boundary minimum */
+    } else {
+        int guard = 0;
+        while (xprofile_dfds(n, S, B, cnt, hi, s0, sigma) < 0.0L && guard++ < 4000) { lo = hi; hi *= 2.0L; }
+        for (int it = 0; it < 200; ++it) {
+            xreal mid = 0.5L * (lo + hi);
+            if (xprofile_dfds(n, S, B, cnt, mid, s0, sigma) < 0.0L) lo = mid; else hi = mid;
+        }
+        s_hat = 0.5L * (lo + hi);
+    }
+    xreal *mu = (xreal *)malloc(sizeof(xreal) * (size_t)(n > 0 ? n : 1));
+    for (int j = 0; j < n; ++j) mu[j] = s_hat * S[j] + (xreal)B[j];
+    xreal f = full_eq18 ? xeq18(n, mu, cnt) : xdeviance(n, mu, cnt);
+    if (sigma > 0.0L) f += (s_hat - s0) * (s_hat - s0) / (sigma * sigma);
+    free(mu);
+    *f_min = f;
+    return s_hat;
+}
+
+/* Stand-alone entry for the pins: S, B, cnt of length n. */
+double orc_profile_scale(int n, const double *S, const double *B, const double *cnt, double s0, double sigma,
+                         int full_eq18, double *f_min)
+{
+    xreal *xS = (xreal *)malloc(sizeof(xreal) * (size_t)(n > 0 ? n : 1));
+    for (int j = 0; j < n; ++j) xS[j] = S[j];
+    xreal f;
+    xreal s = xprofile_scale(n, xS, B, cnt, s0, sigma, full_eq18, &f);
+    free(xS);
+    *f_min = (double)f;
+    return (double)s;
+}
+
+/* Whole path with the normalisation profiled per point: steps a1-a3 as in orc_eval_batch (signal S = fold
+ * without background, kept in long double), then orc_profile_scale over the bins of all periods.
+ *   out [P] profiled -2lnL;  scale_out [P] s^;  abs_out NULL or [P] sum 2|term| at s^. */
+int orc_eval_profile(const orc_consts *c, int n_E, const double *E, const double *flux_w,
+                     const double *P_e, const double *P_mu, const double *P_tau,
+                     int n_T, const double *T, int n_rec, int n_periods,
+                     const double *N_mc, const double *R, const double *bkg, const double *counts,
+                     int64_t P, int k, const int32_t *kinds, const double *params, double s0, double sigma,
+                     double *out, double *scale_out, double *abs_out, int full_eq18, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T > 0 ? n_T : 1));
+    xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, zero, S0);
+    double *zero_bkg = (double *)calloc((size_t)(n_rec > 0 ? n_rec : 1), sizeof(double));
+    if (nthreads < 1) nthreads = 1;
+    const int nb = n_periods * n_rec;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        for (int a = 0; a < k; ++a) theta[kinds[a]] = params[p * k + a];
+        xreal *Sp = (xreal *)malloc(sizeof(xreal) * (size_t)(2 * n_T + nb + 1));
+        xreal *w = Sp + n_T, *sig = w + n_T;
+        xspectrum(c, n_E, E, flux_w, P_e, P_mu, P_tau, n_T, T, theta, Sp);
+        xweights(n_T, Sp, S0, w);
+        for (int d = 0; d < n_periods; ++d)
+            xfold(n_T, n_rec, w, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, zero_bkg, sig + (size_t)d * n_rec);
+        xreal f;
+        xreal s_hat = xprofile_scale(nb, sig, bkg, counts, s0, sigma, full_eq18, &f);
+        out[p] = (double)f;
+        if (scale_out) scale_out[p] = (double)s_hat;
+        if (abs_out) {
+            xreal tot = 0.0L;
+            for (int j = 0; j < nb; ++j) {
+                xreal mu = s_hat * sig[j] + (xreal)bkg[j];
+                tot += fabsl(xdeviance(1, &mu, counts + j));
+            }
+            abs_out[p] = (double)tot;
+        }
+        free(Sp);
+    }
+    free(S0);
+    free(zero_bkg);
     return 0;
 }
 

@@ -234,3 +234,47 @@ def eval_weights(inp, w, want_mu=False, want_abs=False, full_eq18=False, nthread
     if want_abs:
         res.append(ab)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def profile_scale(S, B, n, s0=1.0, sigma=0.0, full_eq18=False):
+    """(s_hat, f_min) of f(s) = deviance(s S + B, n) + ((s - s0)/sigma)^2 over s >= 0 (pull iff sigma > 0)."""
+    S, B, n = _a(S).ravel(), _a(B).ravel(), _a(n).ravel()
+    assert S.size == B.size == n.size
+    L = lib()
+    L.orc_profile_scale.restype = C.c_double
+    f = C.c_double(0.0)
+    s = L.orc_profile_scale(C.c_int(S.size), _p(S), _p(B), _p(n), C.c_double(s0), C.c_double(sigma),
+                            C.c_int(1 if full_eq18 else 0), C.byref(f))
+    return s, f.value
+
+
+def eval_profile(inp, params, kinds, s0=1.0, sigma=0.0, want_abs=False, full_eq18=False, nthreads=1, consts=None):
+    """Whole path with the overall rate normalisation profiled per point. Returns (out[P], s_hat[P][, abs[P]])."""
+    c = consts or default_consts()
+    E, fw, T = _a(inp["E"]), _a(inp["flux_w"]), _a(inp["T"])
+    P_e, P_mu, P_tau = _flavour_probs(inp)
+    R = _a(inp["R"])
+    if R.ndim == 2:
+        R = R[None]
+    D, n_T, n_rec = R.shape
+    N_mc = _a(inp["N_mc"]).reshape(D, n_T)
+    bkg = _a(inp["bkg"]).reshape(D, n_rec)
+    counts = _a(inp["counts"]).reshape(D, n_rec)
+    params = _a(params)
+    if params.ndim == 1:
+        params = params[:, None]
+    P, k = params.shape
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    out, sc = np.empty(P), np.empty(P)
+    ab = np.empty(P) if want_abs else None
+    L = lib()
+    L.orc_eval_profile.restype = C.c_int
+    rc = L.orc_eval_profile(
+        C.byref(c), C.c_int(E.size), _p(E), _p(fw), _p(P_e), _p(P_mu), _p(P_tau),
+        C.c_int(n_T), _p(T), C.c_int(n_rec), C.c_int(D), _p(N_mc), _p(R), _p(bkg), _p(counts),
+        C.c_int64(P), C.c_int(k), kinds.ctypes.data_as(C.POINTER(C.c_int32)), _p(params),
+        C.c_double(s0), C.c_double(sigma), _p(out), _p(sc), _p(ab) if want_abs else None,
+        C.c_int(1 if full_eq18 else 0), C.c_int(int(nthreads)))
+    if rc != 0:
+        raise ValueError("orc_eval_profile: invalid param kinds")
+    return (out, sc, ab) if want_abs else (out, sc)

@@ -376,6 +376,66 @@ def test_eval_weights_pins(orc):
         assert np.all(np.abs(mu1[0, d] / (inp["N_mc"][d] @ inp["R"][d] + inp["bkg"][d]) - 1) < 1e-15)
 
 
+def test_profile_scale_pins(orc):
+    """Profiled rate normalisation (rate_k of Eq. 17, pull of Eq. 18):
+    (i) no background, no pull: Poisson MLE of a scale, s^ = sum n / sum S (closed form);
+    (ii) Asimov data n = s* S + B: s^ = s*, value 0;  (iii) scipy minimize_scalar on a numpy objective,
+    with and without pull;  (iv) sigma -> 0 pins s^ to s0, huge sigma = no pull;  (v) boundary s^ = 0;
+    (vi) the Eq. 18 form has the same minimiser and differs by the saturated constant."""
+    from scipy.optimize import minimize_scalar
+    from scipy.special import gammaln, xlogy
+    rng = np.random.default_rng(3)
+    S = rng.uniform(1.0, 300.0, 57)
+    B = rng.uniform(0.5, 20.0, 57)
+    n = rng.poisson(1.3 * S + B).astype(float)
+    s, f = orc.profile_scale(S, np.zeros(57), n)
+    assert abs(s / (n.sum() / S.sum()) - 1) < 1e-15
+    s, f = orc.profile_scale(S, B, 0.83 * S + B)
+    assert abs(s - 0.83) < 1e-15 and abs(f) < 1e-12
+
+    def obj(x, s0=1.0, sig=0.0):
+        mu = x * S + B
+        v = 2.0 * np.sum(mu - n + xlogy(n, n) - xlogy(n, mu))
+        return v + ((x - s0) / sig) ** 2 if sig > 0 else v
+    for s0, sig in ((1.0, 0.0), (1.0, 0.05), (0.7, 0.01)):
+        s, f = orc.profile_scale(S, B, n, s0=s0, sigma=sig)
+        r = minimize_scalar(lambda x: obj(x, s0, sig), bounds=(0.0, 5.0), method="bounded", options={"xatol": 1e-12})
+        assert abs(s - r.x) < 1e-6 and abs(f - r.fun) < 1e-8 * max(1.0, abs(r.fun))
+        assert abs(f - obj(s, s0, sig)) < 1e-9 * max(1.0, abs(f))
+        assert f <= obj(1.0, s0, sig) + 1e-9                      # profiling never raises the value
+    s_tight, _ = orc.profile_scale(S, B, n, s0=0.9, sigma=1e-9)
+    assert abs(s_tight - 0.9) < 1e-9
+    s_free, f_free = orc.profile_scale(S, B, n)
+    s_loose, f_loose = orc.profile_scale(S, B, n, s0=0.9, sigma=1e9)
+    assert abs(s_loose - s_free) < 1e-9 and abs(f_loose - f_free) < 1e-9
+    # boundary: data below the background everywhere => no signal wanted
+    s0_, f0_ = orc.profile_scale(S, B, 0.5 * B)
+    assert s0_ == 0.0 and abs(f0_ - orc.deviance(B, 0.5 * B)) < 1e-12
+    sf, ff = orc.profile_scale(S, B, n, full_eq18=True)
+    const = 2.0 * np.sum(gammaln(n + 1) - xlogy(n, n) + n)
+    assert abs(sf - s_free) < 1e-15 and abs(ff - f_free - const) < 1e-9 * abs(ff)
+
+
+def test_eval_profile_composition_and_asimov(orc):
+    """eval_profile = (fold without background) -> profile_scale over the bins of all periods; Asimov data made
+    at (theta*, s*) are recovered with value 0 at theta* (PAPER.md:309-311); value <= the unprofiled one."""
+    inp = _small_problem(D=2)
+    params, kinds = wl.random_points(4, [orc.EPS_EE_L, orc.MU_NU], seed=31)
+    out, sc, ab = orc.eval_profile(inp, params, kinds, want_abs=True, nthreads=2)
+    plain, mu = orc.eval_batch(inp, params, kinds, want_mu=True)
+    for p in range(4):
+        S = (mu[p] - inp["bkg"]).ravel()
+        s, f = orc.profile_scale(S, inp["bkg"].ravel(), inp["counts"].ravel())
+        assert abs(s / sc[p] - 1) < 1e-12 and abs(f - out[p]) < 1e-9 * max(1.0, f)
+        assert out[p] <= plain[p] + 1e-9 and ab[p] >= out[p]
+    asim = dict(inp)
+    asim["counts"] = 1.7 * (mu[2] - inp["bkg"]) + inp["bkg"]
+    out, sc = orc.eval_profile(asim, params, kinds)
+    assert abs(sc[2] - 1.7) < 1e-12 and abs(out[2]) < 1e-9 and np.all(out[[0, 1, 3]] > 1e-3)
+    pulled, scp = orc.eval_profile(asim, params, kinds, s0=1.0, sigma=0.1)
+    assert pulled[2] > out[2] and 1.0 < scp[2] < 1.7
+
+
 def test_sm_point_gives_sm_prediction(orc):
     inp = _small_problem(D=2)
     _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
