@@ -144,6 +144,22 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
 int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
                     uint32_t flags, void *cuda_stream);
 
+/* rw_eval_profile: -2lnL with the overall rate normalisation of the signal profiled out per point (PAPER.md:309,
+ * "profiling an overall rate normalization at each scan point"; rate_k of Eq. 17; the Gaussian
+ * constraint of Eq. 18, on that one nuisance).  With S = mu - bkg the fold of the point at unit
+ * normalisation, over the bins of all periods,
+ *     out[p]   = min over s >= 0 of  2 sum [mu_s - n + n ln(n/mu_s)] + ((s - s0)/sigma)^2,   mu_s = s S + bkg
+ *     scale[p] = the minimiser s^ (0 when the data want no signal)
+ * The objective is convex in s; the minimiser is found by a bracketed Newton iteration to double precision.
+ *   param, param_kind, P, k   as rw_eval_batch (DEVICE param only)
+ *   s0, sigma                 centre and width of the Gaussian pull on s; sigma <= 0 or +inf-like: no pull
+ *   out_m2lnL [P], out_scale [P] or NULL   device pointers
+ *   flags                     RW_FULL_EQ18; RW_MODE_AUTO/STREAM/GEMM (dense fold) or RW_MODE_COLLAPSED
+ * Asynchronous and stream-ordered; P may exceed max_batch. */
+int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                    double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,
+                    void *cuda_stream);
+
 /* Device pointers to setup tables, for inspection/tests (valid until rw_destroy):
  *   RW_TABLE_S_SM   [n_T]        SM recoil spectrum S_SM(T_i) (Eq. 12 at theta = 0)
  *   RW_TABLE_BASIS  [10][n_T]    basis spectra A_e,B_e,C_e,A_mu,...,C_tau,D

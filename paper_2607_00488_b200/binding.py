@@ -24,7 +24,7 @@ RW_PARAM_HOST, RW_OUT_HOST = 1 << 8, 1 << 9
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
-EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_get_table",
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
            "rw_last_error", "rw_probe_fp64_peak")
 
@@ -70,6 +70,9 @@ def load_library():
                                 C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     L.rw_eval_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     L.rw_eval_weights.restype = C.c_int
+    L.rw_eval_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_double,
+                                  C.c_double, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_profile.restype = C.c_int
     L.rw_get_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
     L.rw_launch_count.argtypes = [C.c_void_p]
     L.rw_launch_count.restype = C.c_int64
@@ -216,6 +219,26 @@ class Reweighter:
         self._check(rc, self._ctx)
         self._last_param = param          # keep alive until the stream has consumed it
         return (out, out_mu) if (want_mu or out_mu is not None) else out
+
+    def eval_profile(self, param, kinds, s0=1.0, sigma=0.0, full_eq18=False, mode="auto"):
+        """(-2lnL[P] with the overall signal normalisation profiled out, s_hat[P]) for CUDA param[P][k]
+        (rw_eval_profile); sigma > 0 adds the Gaussian pull ((s - s0)/sigma)^2."""
+        if not (isinstance(param, torch.Tensor) and param.is_cuda):
+            raise RwError(-4, "eval_profile needs a CUDA tensor param[P][k]")
+        param = param.to(torch.float64).contiguous()
+        if param.ndim == 1:
+            param = param[:, None]
+        P, k = param.shape
+        assert k == len(kinds)
+        kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
+        out = torch.empty(P, dtype=torch.float64, device=self.device)
+        scale = torch.empty(P, dtype=torch.float64, device=self.device)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        rc = self._L.rw_eval_profile(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, float(s0), float(sigma),
+                                     C.c_void_p(out.data_ptr()), C.c_void_p(scale.data_ptr()), flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = param
+        return out, scale
 
     def eval_weights(self, w, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
         """-2lnL[P] for caller-supplied weights w[P][n_T] (CUDA float64 tensor): the dense fold on arbitrary

@@ -91,6 +91,13 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         L->mu_tile_items = (int)items;
         L->mu_tile = take((size_t)items * kBM * kBN * 8);
     }
+    {   // rw_eval_profile scratch: mu of one pass, about 256 MB (at least 128 points, at most max_batch)
+        int64_t rows = ((int64_t)256 << 20) / (int64_t)(D * n_rec * 8);
+        if (rows < 128) rows = 128;
+        if (rows > max_batch) rows = max_batch;
+        L->prof_rows = rows;
+        L->mu_prof = take((size_t)rows * D * n_rec * 8);
+    }
     L->total = off;
     return RW_OK;
 }
@@ -133,6 +140,55 @@ static bool auto_stream(const rw_ctx *ctx, int64_t P)
 {
     const size_t r_bytes = (size_t)ctx->D * ctx->n_T * (size_t)ctx->n_rec * 8;
     return P <= ((r_bytes >= ((size_t)512 << 20)) ? 4 : 8);
+}
+
+// Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
+// out_mu[Ps][D][n_rec] when asked.
+static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    const int D = ctx->D, n_rec = ctx->n_rec;
+    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps));
+    if (mode == RW_MODE_COLLAPSED) {
+        const int nstrip = (n_rec + 511) / 512;
+        for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
+            const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
+            double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_collapsed(ctx, c0, Pc, mu, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * nstrip, L.MC, Pc, dout + c0, full, s));
+        }
+    } else if (stream_mode) {
+        const int nstrip2 = (n_rec + 255) / 256;
+        for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
+            const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, Pb, mu, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, dout + g0, full, s));
+        }
+    } else {
+        for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
+            const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
+            double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
+            for (int d = 0; d < D; ++d) {
+                RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
+                RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+            }
+            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, dout + c0, full, s));
+        }
+    }
+    return RW_OK;
+}
+
+static int check_kinds(rw_ctx *ctx, const char *fn, int32_t k, const int32_t *param_kind, int *kinds)
+{
+    for (int a = 0; a < k; ++a) {
+        kinds[a] = param_kind[a];
+        if (kinds[a] < 0 || kinds[a] >= RW_N_KINDS)
+            return fail(ctx, RW_ERR_INVALID, "%s: param_kind[%d] = %d out of range", fn, a, kinds[a]);
+        for (int b = 0; b < a; ++b)
+            if (kinds[b] == kinds[a]) return fail(ctx, RW_ERR_INVALID, "%s: duplicate param_kind %d", fn, kinds[a]);
+    }
+    return RW_OK;
 }
 
 }  // namespace rw
@@ -235,6 +291,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->mu_part = (double *)(ws + L.mu_part);
     ctx->out_stage = (double *)(ws + L.out_stage);
     ctx->mu_tile = (double *)(ws + L.mu_tile);
+    ctx->mu_prof = (double *)(ws + L.mu_prof);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;
@@ -281,6 +338,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         return RW_ERR_INVALID;
     }
     rc = make_tensor_maps(ctx);
+    if (rc == RW_OK) rc = profile_setup(ctx);
     if (rc != RW_OK) { free(ctx->tmapR); free(ctx); return rc; }
     ctx->err[0] = 0;
     *out = ctx;
@@ -316,12 +374,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
         return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param, param_kind or out_m2lnL is NULL");
     int kinds[RW_N_KINDS];
-    for (int a = 0; a < k; ++a) {
-        kinds[a] = param_kind[a];
-        if (kinds[a] < 0 || kinds[a] >= RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param_kind[%d] = %d out of range", a, kinds[a]);
-        for (int b = 0; b < a; ++b)
-            if (kinds[b] == kinds[a]) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: duplicate param_kind %d", kinds[a]);
-    }
+    { int rc = check_kinds(ctx, "rw_eval_batch", k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
@@ -341,36 +394,40 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
         }
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
-        const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps));
-        if (mode == RW_MODE_COLLAPSED) {
-            const int nstrip = (n_rec + 511) / 512;
-            for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
-                const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
-                double *mu = out_mu ? out_mu + (size_t)(s0 + c0) * D * n_rec : nullptr;
-                RW_CUDA(ctx, launch_collapsed(ctx, c0, Pc, mu, s));
-                RW_CUDA(ctx, launch_reduce(ctx, D * nstrip, L.MC, Pc, dout + c0, full, s));
-            }
-        } else if (stream_mode) {
-            const int nstrip2 = (n_rec + 255) / 256;
-            for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
-                const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
-                double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
-                RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, Pb, mu, s));
-                RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, dout + g0, full, s));
-            }
-        } else {
-            for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
-                const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
-                double *mu = out_mu ? out_mu + (size_t)(s0 + c0) * D * n_rec : nullptr;
-                for (int d = 0; d < D; ++d) {
-                    RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
-                    RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
-                }
-                RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, dout + c0, full, s));
-            }
-        }
+        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s); if (rc != RW_OK) return rc; }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
+    }
+    return RW_OK;
+}
+
+int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                    double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,
+                    void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_profile: ctx is NULL");
+    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: P < 0 or k outside [0,7]");
+    if (P == 0) return RW_OK;
+    if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: param, param_kind or out_m2lnL is NULL");
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_profile: host buffers are not supported");
+    if (!(s0 == s0) || !(sigma == sigma) || isinf(s0) || (sigma > 0.0 && s0 < 0.0))
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: s0 must be finite (and >= 0 with a pull), sigma not NaN");
+    int kinds[RW_N_KINDS];
+    { int rc = check_kinds(ctx, "rw_eval_profile", k, param_kind, kinds); if (rc != RW_OK) return rc; }
+    const uint32_t mode = flags & RW_MODE_MASK;
+    const bool full = flags & RW_FULL_EQ18;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Layout &L = ctx->lay;
+    // passes of <= prof_rows points: fold with mu written to the scratch, then one CTA per point profiles s
+    for (int64_t q0 = 0; q0 < P; q0 += L.prof_rows) {
+        const int64_t Pq = (P - q0 < L.prof_rows) ? P - q0 : L.prof_rows;
+        RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
+        int rc = fold_slice(ctx, Pq, mode, false, ctx->out_stage, ctx->mu_prof, s);
+        if (rc != RW_OK) return rc;
+        RW_CUDA(ctx, launch_profile(ctx, ctx->mu_prof, Pq, s0, sigma, full, out_m2lnL + q0,
+                                    out_scale ? out_scale + q0 : nullptr, s));
     }
     return RW_OK;
 }

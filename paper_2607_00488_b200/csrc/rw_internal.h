@@ -44,7 +44,7 @@ struct Consts {
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident;
-    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile;
+    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
@@ -53,6 +53,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int n_tiles_n;        // ceil(n_rec / kBN)
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
+    int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
     int ldG;              // row pitch of the prefolded templates G[D][12][ldG] (n_rec rounded up to even)
     int64_t max_batch;
@@ -76,6 +77,7 @@ struct rw_ctx {
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
+    double *mu_prof;          // rw_eval_profile scratch: mu[prof_rows][D][n_rec]
     double *mu_tile;          // split-K scratch: [mu_tile_items][<=128][128] parked accumulators
     CUtensorMap *tmapR;       // host array [D]
     CUtensorMap tmapA[4];     // N' maps for tile heights 16, 32, 64, 128
@@ -115,6 +117,9 @@ cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *wt
                                cudaStream_t s);                              // rw_fold_stream.cu
 cudaError_t launch_gen_A_weights(rw_ctx *ctx, int d, const double *w, int64_t Pc, cudaStream_t s);  // rw_coef.cu
 cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // rw_collapsed.cu
+cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, double s0, double sigma,
+                           bool full_eq18, double *out, double *out_scale, cudaStream_t s);   // rw_profile.cu
+int profile_setup(rw_ctx *ctx);                                              // rw_profile.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,
                              cudaStream_t s);                                // rw_collapsed.cu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,

@@ -173,3 +173,66 @@ def test_eval_weights_config3_size_sampled(rw, orc):
     assert np.all(np.abs(out.cpu().numpy()[idx] - ref) <= 1e-9 + 1e-12 * scale)
     assert np.all(np.abs(out_s.cpu().numpy()[idx[:3]] - ref[:3]) <= 1e-9 + 1e-12 * scale[:3])
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------- f-2 profiled normalisation
+def _profile_check(rw, orc, inp, params, kinds, mode, s0=1.0, sigma=0.0, max_batch=None):
+    import torch
+    ref, sc_ref, scale = orc.eval_profile(inp, params, kinds, s0=s0, sigma=sigma, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=max_batch or params.shape[0])
+    out, sc = ctx.eval_profile(_cuda(params), kinds, s0=s0, sigma=sigma, mode=mode)
+    torch.cuda.synchronize()
+    out, sc = out.cpu().numpy(), sc.cpu().numpy()
+    ctx.close()
+    # the minimiser to 1e-10 relative (the value is flat there), the value to the usual bar (+ the pull term's rounding)
+    assert np.all(np.abs(sc - sc_ref) <= 1e-10 * np.maximum(sc_ref, 1e-3)), np.abs(sc - sc_ref).max()
+    err = np.abs(out - ref)
+    assert np.all(err <= 1e-9 + 1e-12 * (scale + np.abs(ref))), "profiled -2lnL err %.3e" % err.max()
+    return out, sc
+
+
+@pytest.mark.parametrize("mode", ["stream", "gemm", "collapsed"])
+def test_profile_ragged_with_and_without_pull(rw, orc, mode):
+    inp = wl.make_custom(n_E=31, n_T=203, n_rec=330, n_periods=2, seed=51, dead_fraction=0.1)
+    params, kinds = wl.random_points(45, [wl.EPS_EE_L, wl.EPS_EE_R, wl.EPS_TT_L, wl.MU_NU], seed=52)
+    out_free, sc_free = _profile_check(rw, orc, inp, params, kinds, mode)
+    out_pull, sc_pull = _profile_check(rw, orc, inp, params, kinds, mode, s0=1.0, sigma=0.02, max_batch=16)
+    assert np.all(out_pull >= out_free - 1e-9)                       # a constraint never lowers the minimum
+    assert np.all(np.abs(sc_pull - 1.0) <= np.abs(sc_free - 1.0) + 1e-12)
+
+
+def test_profile_asimov_recovery_and_boundary(rw, orc):
+    """PAPER.md:309-311: Asimov data built at (theta*, s* = 1.4) are recovered with value 0 and s^ = s*;
+    data below the background give the boundary s^ = 0; the Eq. 18 form adds the saturated constant."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=120, n_rec=90, n_periods=2, seed=53)
+    params, kinds = wl.random_points(6, [wl.EPS_EE_L, wl.MU_NU], seed=54)
+    _, mu = orc.eval_batch(inp, params, kinds, want_mu=True)
+    asim = dict(inp)
+    asim["counts"] = 1.4 * (mu[3] - inp["bkg"]) + inp["bkg"]
+    out, sc = _profile_check(rw, orc, asim, params, kinds, "gemm")
+    assert abs(sc[3] - 1.4) < 1e-10 and abs(out[3]) < 1e-9 and np.all(np.delete(out, 3) > 1e-6)
+    low = dict(inp)
+    low["counts"] = 0.5 * inp["bkg"]
+    out, sc = _profile_check(rw, orc, low, params, kinds, "stream")
+    assert np.all(sc == 0.0)
+    ctx = rw.Reweighter(inp, max_batch=6)
+    full, _ = ctx.eval_profile(_cuda(params), kinds, full_eq18=True)
+    plain, _ = ctx.eval_profile(_cuda(params), kinds)
+    torch.cuda.synchronize()
+    ref_full = orc.eval_profile(inp, params, kinds, full_eq18=True)[0]
+    assert np.all(np.abs(full.cpu().numpy() - ref_full) <= 1e-9 * np.abs(ref_full))
+    const = (full - plain).cpu().numpy()
+    assert np.all(np.abs(const - const[0]) <= 1e-9 * abs(const[0]))
+    with pytest.raises(rw.RwError):
+        ctx.eval_profile(_cuda(params), kinds, s0=float("nan"))
+    ctx.close()
+
+
+def test_profile_config2_all_points(rw, orc):
+    """Config 2 (1000 mu_nu points, 867 dead recoil bins, exact zeros in R): dense and collapsed folds."""
+    inp = wl.make("cfg2_mm_lowE")
+    params, kinds = wl.scan_points("cfg2_mm_lowE")
+    a, _ = _profile_check(rw, orc, inp, params, kinds, "auto")
+    b, _ = _profile_check(rw, orc, inp, params, kinds, "collapsed", s0=1.0, sigma=0.1)
+    assert np.all(b >= a - 1e-9)
