@@ -30,8 +30,9 @@ METRIC = "likelihood evals/sec (batched)"
 UNIT = "evals/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_fold_gemm launch from the committed
-# `ncu --set full` capture (profiles/r01_fold_kernels_full.md), or None if not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 87.107397e9 + 0.033670e9}
+# `ncu --set full` capture (profiles/r01b_fold_gemm_full.md: the fused launch over the 110 full waves of one
+# 32768-point chunk), or None if not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 54.395468e9 + 0.030036e9}
 
 
 def load_peaks():

@@ -77,6 +77,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->flag = take(4);
     L->ldG = (int)mu_ld;
     L->G = take(D * kCoefStride * mu_ld * 8);
+    L->stream_cnt = take((D * (size_t)L->stream_strips + 1) * 4);
+    L->strip_part = take(D * (size_t)L->stream_strips * kStreamMaxPB * 8);
     L->ident = take(kStreamMaxPB * kCoefStride * 8);
     L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
     L->coef = take((size_t)max_batch * kCoefStride * 8);
@@ -134,13 +136,9 @@ static const char *flag_message(int f)
     return "invalid input";
 }
 
-// RW_MODE_AUTO: the HBM-streaming fold for a handful of points (measured on B200: it wins up to 8 points while
-// R is L2-sized, up to 4 points for a 1 GiB R), the DMMA contraction (tile height 16..128, split-K) beyond.
-static bool auto_stream(const rw_ctx *ctx, int64_t P)
-{
-    const size_t r_bytes = (size_t)ctx->D * ctx->n_T * (size_t)ctx->n_rec * 8;
-    return P <= ((r_bytes >= ((size_t)512 << 20)) ? 4 : 8);
-}
+// RW_MODE_AUTO: the one-launch HBM-streaming path for up to 4 points (measured on B200: it wins there at every
+// response size), the DMMA contraction (tile height 16..128, split-K) beyond.
+static bool auto_stream(const rw_ctx *, int64_t P) { return P <= 4; }
 
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
@@ -158,12 +156,11 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             RW_CUDA(ctx, launch_reduce(ctx, D * nstrip, L.MC, Pc, dout + c0, full, s));
         }
     } else if (stream_mode) {
-        const int nstrip2 = (n_rec + 255) / 256;
         for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
             const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
-            RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, Pb, mu, s));
-            RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, dout + g0, full, s));
+            RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
+                                            dout + g0, full, mu, s));
         }
     } else {
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
@@ -285,6 +282,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->What = (double *)(ws + L.What);    ctx->sat_const = (double *)(ws + L.sat_const);
     ctx->flag = (int *)(ws + L.flag);
     ctx->G = (double *)(ws + L.G);          ctx->ident = (double *)(ws + L.ident);
+    ctx->stream_cnt = (int *)(ws + L.stream_cnt);
+    ctx->strip_part = (double *)(ws + L.strip_part);
     ctx->param_stage = (double *)(ws + L.param_stage);
     ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);
     ctx->partial = (double *)(ws + L.partial);
@@ -323,6 +322,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         RW_TRY(cudaMemcpy2DAsync(ws + L.R_copy, (size_t)L.ldR * 8, in->R, n_rec * 8, n_rec * 8, D * n_T, kind, s));
     }
     RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
+    RW_TRY(cudaMemsetAsync(ctx->stream_cnt, 0, (D * (size_t)L.stream_strips + 1) * 4, s));
     RW_TRY(launch_flavour(ctx, have_mt ? 1 : 0, f_tau, s));
     if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
     RW_TRY(launch_setup(ctx, s));
@@ -393,8 +393,25 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             }
         }
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
+        if ((mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps))) {
+            // a handful of points: one launch per <= 16 points does a1-a4 (coefficients computed in the kernel)
+            Kinds kd;
+            kd.k = k;
+            for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
+            for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
+                const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
+                double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
+                if (k > 0)
+                    RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, dparam + g0 * k, &kd, nullptr, Pb, dout + g0, full, mu, s));
+                else {
+                    RW_CUDA(ctx, launch_coef(ctx, nullptr, Pb, 0, kinds, s));
+                    RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef, nullptr, nullptr, nullptr, Pb, dout + g0, full, mu, s));
+                }
+            }
+        } else {
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
         { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s); if (rc != RW_OK) return rc; }
+        }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
     }
@@ -450,12 +467,11 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
     const size_t n_T = ctx->n_T;
     const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, P));
     if (stream_mode) {
-        const int nstrip2 = (n_rec + 255) / 256;
         for (int64_t g0 = 0; g0 < P; g0 += kStreamMaxPB) {
             const int Pb = (int)((P - g0 < kStreamMaxPB) ? P - g0 : kStreamMaxPB);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
-            RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, w + (size_t)g0 * n_T, Pb, mu, s));
-            RW_CUDA(ctx, launch_reduce(ctx, D * nstrip2, kStreamMaxPB, Pb, out_m2lnL + g0, full, s));
+            RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb,
+                                            out_m2lnL + g0, full, mu, s));
         }
     } else {
         for (int64_t c0 = 0; c0 < P; c0 += L.MC) {

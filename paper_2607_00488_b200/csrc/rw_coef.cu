@@ -11,33 +11,15 @@
 
 namespace rw {
 
-struct Kinds { int k; int kind[RW_N_KINDS]; };
-
 __global__ void k_coef(const double *__restrict__ param, int64_t P, Kinds kd, Consts cst,
                        double *__restrict__ coef)
 {
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= P) return;
-    double th[RW_N_KINDS];
+    double c[kCoefStride];
+    coef_from_param(param + p * kd.k, kd, cst, c);
 #pragma unroll
-    for (int q = 0; q < RW_N_KINDS; ++q) th[q] = 0.0;
-    for (int a = 0; a < kd.k; ++a) {
-        double v = param[p * kd.k + a];
-#pragma unroll
-        for (int q = 0; q < RW_N_KINDS; ++q)
-            if (kd.kind[a] == q) th[q] = v;
-    }
-    double *c = coef + p * kCoefStride;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double gl = cst.gL[a] + th[2 * a], gr = cst.gR[a] + th[2 * a + 1];
-        c[3 * a + 0] = gl * gl;
-        c[3 * a + 1] = gr * gr;
-        c[3 * a + 2] = gl * gr;
-    }
-    c[9] = th[RW_MU_NU] * th[RW_MU_NU];
-    c[10] = 1.0;
-    c[11] = 0.0;
+    for (int b = 0; b < kCoefStride; ++b) coef[p * kCoefStride + b] = c[b];
 }
 
 constexpr int kGenThreads = 256;   // 32 row-blocks of 8 points

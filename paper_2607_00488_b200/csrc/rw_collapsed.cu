@@ -107,7 +107,7 @@ cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s)
     k_identity<<<1, 256, 0, s>>>(ctx->ident);
     ctx->launches++;
     // the 11 templates are folded as 11 "points" with unit coefficient vectors (no deviance pass)
-    cudaError_t e = launch_fold_stream(ctx, ctx->ident, nullptr, -kNumTerms, nullptr, s);
+    cudaError_t e = launch_fold_stream(ctx, ctx->ident, nullptr, nullptr, nullptr, kNumTerms, nullptr, false, nullptr, s);
     if (e != cudaSuccess) return e;
     const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + 63) / 64 * 64;
     const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;

@@ -1,43 +1,76 @@
-// rw_fold_stream.cu -- steps a3 + a4 for small batches (P <= 16 per pass): HBM-streaming fold.
+// rw_fold_stream.cu -- the whole path for a handful of points (Pb <= 16 per launch) in ONE kernel:
+// HBM-streaming fold with the coefficient step in front and the likelihood reduction behind it.
 //
 // With few points the fold mu[p][k] = sum_i N'[p][i] R[i][k] + bkg[k] (Eq. 11) reads
 // every byte of R once and does 2P flop per 8 bytes: it is bound by HBM bandwidth, not arithmetic.
 // R is row-major with the reconstructed index fastest, so a thread owns two adjacent columns
 // (one 16-byte load per row), a CTA owns a 512-column strip, and the recoil rows are split over
-// gridDim.y so that the grid fills all SMs several times over.  N'[p][i] (Eq. 14 / Eq. 1) is
-// formed on the fly from the 11-term pre-scaled basis and staged in shared memory.
-// The row-split partial sums are combined in a fixed order by k_stream_deviance, which adds the
-// background and reduces the Poisson terms of Eq. (18) per point: warp shuffles,
-// then one shared-memory pass per CTA; k_reduce finishes over strips and periods.
+// gridDim.y so that the grid fills all SMs several times over.
+//   a1  the CTA computes the coefficients of its points from the raw parameters (Eq. 6)
+//   a2  N'[p][i] (Eq. 14 / Eq. 1) is formed on the fly from the 11-term pre-scaled basis into shared memory
+//   a3  each CTA folds its row range; the partial sums of a strip go to mu_part
+//   a4  the LAST CTA of a strip to finish (ticket counter) adds the row ranges in a fixed order, adds the
+//       background and reduces the Poisson terms of Eq. (18) of its 512 columns; the LAST strip
+//       to finish adds the strips and periods in a fixed order and writes -2lnL.  Results do not depend on
+//       which CTA is last: only who does the (fixed-order) sums changes.  The counters reset themselves.
+// A single evaluation -- the call a minimiser makes -- is therefore one launch.
 #include "rw_internal.h"
 
 namespace rw {
 
 constexpr int kRC = 64;   // recoil rows staged per iteration
 
+struct StreamArgs {
+    const double *R; size_t R_period_stride; int ldR, n_T, n_rec, D;
+    const double *coef;       // [Pb][12], or NULL
+    const double *param;      // [Pb][k] raw parameters (coefficients computed here), or NULL
+    const double *wts;        // [Pb][n_T] caller weights (rw_eval_weights), or NULL
+    const double *What, *N_mc, *bkg, *counts, *sat_const;
+    int Pb, rows_per_split, n_splits, mu_ld;
+    double *mu_part;          // [D][n_splits][PB][mu_ld]
+    double *strip_part;       // [D * strips][16]
+    int *cnt;                 // [D * strips] strip tickets, then one global ticket
+    double *out;              // [Pb] -2lnL, or NULL: fold only
+    double *out_mu;           // NULL or [Pb][D][n_rec]
+};
+
 template <int PB>
 __global__ void __launch_bounds__(kStreamThreads)
-k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int n_T, int n_rec,
-              const double *__restrict__ coef, int Pb, const double *__restrict__ What,
-              const double *__restrict__ wts /*NULL, or caller weights [Pb][n_T] (rw_eval_weights)*/,
-              const double *__restrict__ N_mc /*[D][n_T], used with wts*/,
-              int rows_per_split, int n_splits, int mu_ld, double *__restrict__ mu_part)
+k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
 {
     __shared__ __align__(16) double sN[kRC][PB];
-    __shared__ double sC[PB][kNumTerms];
-    const int d = blockIdx.z;
-    const int split = blockIdx.y;
-    const int col = blockIdx.x * kStreamCols + 2 * threadIdx.x;
-    const int i0 = split * rows_per_split;
-    const int i1 = min(n_T, i0 + rows_per_split);
-    const double *Rd = R + (size_t)d * R_period_stride;
-    const double *Wd = What + (size_t)d * kCoefStride * n_T;
+    __shared__ double sC[PB][kCoefStride];
+    __shared__ double red[kStreamThreads / 32][PB];
+    __shared__ int s_last;
+    const int d = blockIdx.z, split = blockIdx.y, strip = blockIdx.x;
+    const int n_T = A.n_T, n_rec = A.n_rec, Pb = A.Pb;
+    const int col = strip * kStreamCols + 2 * threadIdx.x;
+    const int i0 = split * A.rows_per_split;
+    const int i1 = min(n_T, i0 + A.rows_per_split);
+    const double *Rd = A.R + (size_t)d * A.R_period_stride;
+    const double *Wd = A.What + (size_t)d * kCoefStride * n_T;
+    const double *wts = A.wts;
 
-    if (!wts)
-        for (int q = threadIdx.x; q < PB * kNumTerms; q += kStreamThreads) {
-            int p = q / kNumTerms, b = q - p * kNumTerms;
-            sC[p][b] = (p < Pb) ? coef[(size_t)p * kCoefStride + b] : 0.0;
+    if (!wts) {
+        if (A.param) {
+            if (threadIdx.x < PB) {
+                double c[kCoefStride];
+                if (threadIdx.x < Pb) {
+                    coef_from_param(A.param + (size_t)threadIdx.x * kd.k, kd, cst, c);
+                } else {
+#pragma unroll
+                    for (int b = 0; b < kCoefStride; ++b) c[b] = 0.0;
+                }
+#pragma unroll
+                for (int b = 0; b < kCoefStride; ++b) sC[threadIdx.x][b] = c[b];
+            }
+        } else {
+            for (int q = threadIdx.x; q < PB * kCoefStride; q += kStreamThreads) {
+                int p = q / kCoefStride, b = q - p * kCoefStride;
+                sC[p][b] = (p < Pb) ? A.coef[(size_t)p * kCoefStride + b] : 0.0;
+            }
         }
+    }
     double acc[PB][2];
 #pragma unroll
     for (int p = 0; p < PB; ++p) acc[p][0] = acc[p][1] = 0.0;
@@ -51,7 +84,7 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
             double v = 0.0;
             if (i < i1) {
                 if (wts) {          // N' = w N_mc (Eq. 1 with caller-supplied weights)
-                    if (p < Pb) v = wts[(size_t)p * n_T + i] * N_mc[(size_t)d * n_T + i];
+                    if (p < Pb) v = wts[(size_t)p * n_T + i] * A.N_mc[(size_t)d * n_T + i];
                 } else {            // N' = sum_b c_b W^_b (Eq. 14 folded into the pre-scaled basis)
 #pragma unroll
                     for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p][b], Wd[(size_t)b * n_T + i], v);
@@ -61,7 +94,7 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
         }
         __syncthreads();
         if (col_ok) {
-            const double *Rp = Rd + (size_t)ic * ldR + col;
+            const double *Rp = Rd + (size_t)ic * A.ldR + col;
             const int nrows = min(kRC, i1 - ic);
 #pragma unroll 1
             for (int r0 = 0; r0 < nrows; r0 += 8) {
@@ -69,7 +102,7 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
 #pragma unroll
                 for (int u = 0; u < 8; ++u)
                     rv[u] = (r0 + u < nrows)
-                                ? __ldg(reinterpret_cast<const double2 *>(Rp + (size_t)(r0 + u) * ldR))
+                                ? __ldg(reinterpret_cast<const double2 *>(Rp + (size_t)(r0 + u) * A.ldR))
                                 : make_double2(0.0, 0.0);
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
@@ -83,44 +116,122 @@ k_fold_stream(const double *__restrict__ R, size_t R_period_stride, int ldR, int
             }
         }
     }
+    const int n_splits = A.n_splits, mu_ld = A.mu_ld;
     if (col_ok) {
 #pragma unroll
         for (int p = 0; p < PB; ++p) {
-            double *dst = mu_part + (((size_t)d * n_splits + split) * PB + p) * mu_ld + col;
-            *reinterpret_cast<double2 *>(dst) = make_double2(acc[p][0], acc[p][1]);
+            double *dst = A.mu_part + (((size_t)d * n_splits + split) * PB + p) * mu_ld + col;
+            __stcg(reinterpret_cast<double2 *>(dst), make_double2(acc[p][0], acc[p][1]));
         }
     }
-}
+    if (!A.out) return;                      // fold only (template prefold)
 
-// mu = sum_split partial + bkg; Poisson term; per-CTA reduction -> partial[(d*nstrip + strip)][p].
-__global__ void __launch_bounds__(256)
-k_stream_deviance(const double *__restrict__ mu_part, int n_splits, int PB, int mu_ld, int n_rec,
-                  const double *__restrict__ bkg, const double *__restrict__ counts, int D,
-                  double *__restrict__ out_mu /*[P][D][n_rec] rows of this group, or NULL*/,
-                  double *__restrict__ partial /*[D*nstrip][kStreamMaxPB]*/)
-{
-    const int p = blockIdx.y, d = blockIdx.z;
-    const int col = blockIdx.x * 256 + threadIdx.x;
-    double term = 0.0;
-    if (col < n_rec) {
-        double mu = 0.0;
-        for (int s = 0; s < n_splits; ++s)
-            mu += mu_part[(((size_t)d * n_splits + s) * PB + p) * mu_ld + col];
-        mu += bkg[(size_t)d * n_rec + col];
-        if (out_mu) out_mu[((size_t)p * D + d) * n_rec + col] = mu;
-        term = poisson_term(mu, counts[(size_t)d * n_rec + col]);
-    }
-    __shared__ double red[8];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) term += __shfl_down_sync(0xffffffffu, term, o);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = term;
+    // ---------------------------------------------------------------- last CTA of this strip: a4 for 512 columns
+    const int n_strips = gridDim.x, sid = d * n_strips + strip;
+    __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0) s_last = (atomicAdd(A.cnt + sid, 1) == n_splits - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double bk0 = 0.0, bk1 = 0.0, cn0 = 0.0, cn1 = 0.0;
+    const bool ok1 = col + 1 < n_rec;
+    if (col_ok) { bk0 = A.bkg[(size_t)d * n_rec + col]; cn0 = A.counts[(size_t)d * n_rec + col]; }
+    if (ok1) { bk1 = A.bkg[(size_t)d * n_rec + col + 1]; cn1 = A.counts[(size_t)d * n_rec + col + 1]; }
+    double m0[PB], m1[PB];
+#pragma unroll
+    for (int p = 0; p < PB; ++p) m0[p] = m1[p] = 0.0;
+    if (col_ok)
+        for (int s = 0; s < n_splits; ++s) {          // row ranges in a fixed order; the PB loads of a step overlap
+#pragma unroll
+            for (int p = 0; p < PB; ++p) {
+                const double2 v = __ldcg(reinterpret_cast<const double2 *>(
+                    A.mu_part + (((size_t)d * n_splits + s) * PB + p) * mu_ld + col));
+                m0[p] += v.x; m1[p] += v.y;
+            }
+        }
+#pragma unroll
+    for (int p = 0; p < PB; ++p) {
+        double t = 0.0;
+        if (col_ok && p < Pb) {
+            const double a0 = m0[p] + bk0, a1 = m1[p] + bk1;
+            if (A.out_mu) {
+                double *dst = A.out_mu + ((size_t)p * A.D + d) * n_rec + col;
+                dst[0] = a0;
+                if (ok1) dst[1] = a1;
+            }
+            t = poisson_term(a0, cn0) + (ok1 ? poisson_term(a1, cn1) : 0.0);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) red[warp][p] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < PB) {
         double v = 0.0;
 #pragma unroll
-        for (int w = 0; w < 8; ++w) v += red[w];
-        partial[((size_t)d * gridDim.x + blockIdx.x) * kStreamMaxPB + p] = v;
+        for (int w = 0; w < kStreamThreads / 32; ++w) v += red[w][threadIdx.x];
+        __stcg(A.strip_part + (size_t)sid * kStreamMaxPB + threadIdx.x, v);
     }
+
+    // ---------------------------------------------------------------- last strip: sum strips and periods, write
+    const int n_sid = n_strips * A.D;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(A.cnt + n_sid, 1) == n_sid - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (threadIdx.x < Pb) {
+        double v = 0.0;
+        for (int q = 0; q < n_sid; ++q) v += __ldcg(A.strip_part + (size_t)q * kStreamMaxPB + threadIdx.x);
+        v *= 2.0;
+        if (A.sat_const) v += A.sat_const[0];
+        A.out[threadIdx.x] = v;
+    }
+    for (int q = threadIdx.x; q <= n_sid; q += kStreamThreads) A.cnt[q] = 0;     // ready for the next launch
+}
+
+template <int PB>
+static void launch_stream_t(const StreamArgs &A, const Kinds &kd, const Consts &cst, dim3 grid, cudaStream_t s)
+{
+    k_fold_stream<PB><<<grid, kStreamThreads, 0, s>>>(A, kd, cst);
+}
+
+cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
+                               const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
+                               cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    StreamArgs A;
+    A.R = ctx->R; A.R_period_stride = ctx->R_period_stride; A.ldR = ctx->ldR;
+    A.n_T = ctx->n_T; A.n_rec = ctx->n_rec; A.D = ctx->D;
+    A.coef = coef; A.param = param; A.wts = wts;
+    A.What = ctx->What; A.N_mc = ctx->N_mc; A.bkg = ctx->bkg; A.counts = ctx->counts;
+    A.sat_const = full_eq18 ? ctx->sat_const : nullptr;
+    A.Pb = Pb;
+    A.rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
+    A.n_splits = (ctx->n_T + A.rows_per_split - 1) / A.rows_per_split;
+    A.mu_ld = (ctx->n_rec + 1) & ~1;
+    A.mu_part = ctx->mu_part; A.strip_part = ctx->strip_part; A.cnt = ctx->stream_cnt;
+    A.out = out; A.out_mu = out_mu;
+    Kinds none;
+    none.k = 0;
+    for (int a = 0; a < RW_N_KINDS; ++a) none.kind[a] = -1;
+    const Kinds &k = kd ? *kd : none;
+    dim3 grid(L.stream_strips, A.n_splits, ctx->D);
+    {
+        ProfScope prof(ctx, s);
+        if (!out) launch_stream_t<16>(A, k, ctx->cst, grid, s);           // prefold: PB = 16 layout of mu_part
+        else if (Pb <= 1) launch_stream_t<1>(A, k, ctx->cst, grid, s);
+        else if (Pb <= 2) launch_stream_t<2>(A, k, ctx->cst, grid, s);
+        else if (Pb <= 4) launch_stream_t<4>(A, k, ctx->cst, grid, s);
+        else if (Pb <= 8) launch_stream_t<8>(A, k, ctx->cst, grid, s);
+        else launch_stream_t<16>(A, k, ctx->cst, grid, s);
+    }
+    ctx->launches++;
+    return cudaGetLastError();
 }
 
 // out[p] = 2 * sum_parts partial[part][p] (+ saturated constant for the literal Eq. 18), fixed order.
@@ -134,51 +245,6 @@ __global__ void k_reduce(const double *__restrict__ partial, int n_parts, int64_
     v *= 2.0;
     if (sat_const) v += sat_const[0];
     out[p] = v;
-}
-
-template <int PB>
-static void launch_stream_t(rw_ctx *ctx, const double *coef, const double *wts, int Pb, cudaStream_t s)
-{
-    const Layout &L = ctx->lay;
-    const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
-    const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;
-    dim3 grid(L.stream_strips, n_splits, ctx->D);
-    const int mu_ld = (ctx->n_rec + 1) & ~1;
-    k_fold_stream<PB><<<grid, kStreamThreads, 0, s>>>(
-        ctx->R, ctx->R_period_stride, ctx->ldR, ctx->n_T, ctx->n_rec, coef, Pb,
-        ctx->What, wts, ctx->N_mc, rows_per_split, n_splits, mu_ld, ctx->mu_part);
-}
-
-// Pb > 0: fold Pb points (coefficients `coef`, or caller weights `wts`) and reduce the Poisson terms.
-// Pb < 0: fold -Pb coefficient vectors only (the template prefold of rw_collapsed.cu; partials stay in mu_part
-//         laid out for PB = 16).
-cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *wts, int Pb, double *out_mu,
-                               cudaStream_t s)
-{
-    const Layout &L = ctx->lay;
-    if (Pb < 0) {
-        launch_stream_t<16>(ctx, coef, nullptr, -Pb, s);
-        ctx->launches++;
-        return cudaGetLastError();
-    }
-    int PB;
-    {
-        ProfScope prof(ctx, s);
-        if (Pb <= 1) { PB = 1; launch_stream_t<1>(ctx, coef, wts, Pb, s); }
-        else if (Pb <= 2) { PB = 2; launch_stream_t<2>(ctx, coef, wts, Pb, s); }
-        else if (Pb <= 4) { PB = 4; launch_stream_t<4>(ctx, coef, wts, Pb, s); }
-        else if (Pb <= 8) { PB = 8; launch_stream_t<8>(ctx, coef, wts, Pb, s); }
-        else { PB = 16; launch_stream_t<16>(ctx, coef, wts, Pb, s); }
-    }
-    const int rows_per_split = ((ctx->n_T + L.stream_splits - 1) / L.stream_splits + kRC - 1) / kRC * kRC;
-    const int n_splits = (ctx->n_T + rows_per_split - 1) / rows_per_split;
-    const int mu_ld = (ctx->n_rec + 1) & ~1;
-    const int nstrip2 = (ctx->n_rec + 255) / 256;
-    dim3 grid2(nstrip2, Pb, ctx->D);
-    k_stream_deviance<<<grid2, 256, 0, s>>>(ctx->mu_part, n_splits, PB, mu_ld, ctx->n_rec, ctx->bkg,
-                                            ctx->counts, ctx->D, out_mu, ctx->partial);
-    ctx->launches += 2;
-    return cudaGetLastError();
 }
 
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,

@@ -41,9 +41,12 @@ struct Consts {
     double gL[3], gR[3];   // Eq. (2)-(3)
 };
 
+// Which parameter a column of param[P][k] holds (include/rw.h RW_EPS_EE_L ... RW_MU_NU); -1 = unused.
+struct Kinds { int k; int kind[RW_N_KINDS]; };
+
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
-    size_t basis, S_sm, What, sat_const, flag, G, ident;
+    size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part;
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
@@ -73,6 +76,8 @@ struct rw_ctx {
     int ldR;
     size_t R_period_stride;   // doubles between periods
     double *basis, *S_sm, *What, *sat_const;
+    int *stream_cnt;          // last-CTA-done tickets of the streaming fold: [D * strips] + 1, self-resetting
+    double *strip_part;       // [D * strips][16] Poisson sums per column strip
     double *G, *ident;        // prefolded templates [D][12][ldG]; identity coefficients [16][12] used to fold them
     int *flag;
     // per-call scratch
@@ -113,7 +118,10 @@ cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, cons
 cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_t s);   // rw_coef.cu
 cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int64_t mu_p0,
                              cudaStream_t s);                                // rw_fold_gemm.cu
-cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *wts, int Pb, double *out_mu,
+// One launch: fold + Poisson terms + final sum for Pb <= 16 points given by coefficients `coef`, raw parameters
+// `param` (+ kinds; step a1 then runs inside the kernel) or caller weights `wts`.  out == NULL: fold only (prefold).
+cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
+                               const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
                                cudaStream_t s);                              // rw_fold_stream.cu
 cudaError_t launch_gen_A_weights(rw_ctx *ctx, int d, const double *w, int64_t Pc, cudaStream_t s);  // rw_coef.cu
 cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // rw_collapsed.cu
@@ -140,6 +148,33 @@ struct ProfScope {
         if (on) { cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n + 1], s); ctx->prof_n++; }
     }
 };
+
+// Step a1 for one point: g~ = g + eps (Eq. 6), then the monomials the cross section is polynomial
+// in: g~L^2, g~R^2, g~L g~R per flavour (Eq. 4/7) and mu_nu^2 (Eq. 8-9).
+// c[10] = 1 multiplies the dead-bin row of W^, c[11] = 0 is padding.
+__device__ __forceinline__ void coef_from_param(const double *__restrict__ prow, const Kinds &kd, const Consts &cst,
+                                                double *c /*[12]*/)
+{
+    double th[RW_N_KINDS];
+#pragma unroll
+    for (int q = 0; q < RW_N_KINDS; ++q) th[q] = 0.0;
+    for (int a = 0; a < kd.k; ++a) {
+        const double v = prow[a];
+#pragma unroll
+        for (int q = 0; q < RW_N_KINDS; ++q)
+            if (kd.kind[a] == q) th[q] = v;
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double gl = cst.gL[a] + th[2 * a], gr = cst.gR[a] + th[2 * a + 1];
+        c[3 * a + 0] = gl * gl;
+        c[3 * a + 1] = gr * gr;
+        c[3 * a + 2] = gl * gr;
+    }
+    c[9] = th[RW_MU_NU] * th[RW_MU_NU];
+    c[10] = 1.0;
+    c[11] = 0.0;
+}
 
 // Poisson term of Eq. (18) relative to its saturated value: mu - n + n ln(n/mu) (x2 applied later).
 __device__ __forceinline__ double poisson_term(double mu, double n)
