@@ -132,12 +132,15 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
-def workload_config(name, inp, P, n_gpus, sample=None):
+def workload_config(name, inp, P, n_gpus, sample=None, max_batch=0):
     D, n_T, n_rec = inp["R"].shape
     cfg = {"workload": name, "n_E": int(inp["E"].size), "n_T": int(n_T), "n_rec": int(n_rec), "n_periods": int(D),
            "points_per_step_per_gpu": int(P), "response_bytes": int(D * n_T * n_rec * 8),
+           "library_slice_points": int(max_batch) if max_batch else int(P),
            "parallelism": "points sharded over %d GPU(s), tables replicated, no collective" % n_gpus,
-           "l2": "response (%.2f GB) and reweighted spectrum exceed the 126 MB L2: no flush needed" % (D * n_T * n_rec * 8 / 1e9)}
+           "l2": ("response (%.2f GB) and reweighted spectrum exceed the 126 MB L2: no flush needed" % (D * n_T * n_rec * 8 / 1e9))
+                 if D * n_T * n_rec * 8 + 8.0 * P * n_T > 252e6 else
+                 "working set fits the 126 MB L2: a 256 MB buffer is rewritten between timed steps (L2 flush)"}
     if sample:
         cfg["sample"] = sample
     return cfg
@@ -151,6 +154,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg4_dense")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--max-batch", type=int, default=0,
+                    help="points per library slice (default: the whole scan; 16384 for cfg5_joint6, as BASELINE.json says)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -182,7 +187,8 @@ def main():
     dev_inp = {key: torch.from_numpy(np.ascontiguousarray(inp[key])).to(dev)
                for key in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
     dev_inp["f_tau"] = inp["f_tau"]
-    ctx = binding.Reweighter(dev_inp, max_batch=P, device=dev)
+    max_batch = args.max_batch or (16384 if name == "cfg5_joint6" else P)
+    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev)
     param_dev = torch.from_numpy(params).to(dev)
     out_dev = torch.empty(P, dtype=torch.float64, device=dev)
     param_pin = torch.from_numpy(params).pin_memory()
@@ -207,13 +213,31 @@ def main():
     launches0 = ctx.launch_count()
     ctx.profile_begin()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        ctx.eval_batch(param_dev, kinds, out=out_dev)
-    e1.record()
-    barrier()
-    ms = maxreduce(e0.elapsed_time(e1))
+    need_flush = D * n_T * n_rec * 8 + 8.0 * P * n_T <= 252e6      # working set could stay in the 126 MB L2
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if need_flush else None
+
+    def timed_steps(fn):
+        """K steps timed on the device; with an L2 flush (256 MB rewrite, untimed) before each one if needed."""
+        barrier()
+        if not need_flush:
+            e0.record()
+            for _ in range(args.steps):
+                fn()
+            e1.record()
+            barrier()
+            return e0.elapsed_time(e1)
+        total = 0.0
+        for _ in range(args.steps):
+            flush_buf.zero_()
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            total += e0.elapsed_time(e1)
+        barrier()
+        return total
+
+    ms = maxreduce(timed_steps(lambda: ctx.eval_batch(param_dev, kinds, out=out_dev)))
     fold_ms, fold_launches = ctx.profile_end()
     launches = ctx.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
@@ -223,13 +247,8 @@ def main():
     # ---------------------------------------------------------------- end to end with host buffers
     for _ in range(2):
         ctx.eval_batch(param_pin, kinds, out=out_pin)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        ctx.eval_batch(param_pin, kinds, out=out_pin)     # H2D params, kernels, D2H -2lnL: all on the stream
-    e1.record()
-    barrier()
-    ms_e2e = maxreduce(e0.elapsed_time(e1))
+    # H2D params, kernels, D2H -2lnL: all on the stream, inside the timed region
+    ms_e2e = maxreduce(timed_steps(lambda: ctx.eval_batch(param_pin, kinds, out=out_pin)))
     e2e_value = sharding.whole_job_value(world, P, args.steps, ms_e2e)
     same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
 
@@ -252,8 +271,15 @@ def main():
     r_bytes = D * n_T * n_rec * 8
     single = {"ms_per_eval": single_ms, "fold_kernel_ms": sfold_ms / max(1, sfold_n),
               "hbm_gbs": r_bytes / (sfold_ms / max(1, sfold_n) * 1e-3) / 1e9,
-              "hbm_peak_gbs": peaks["hbm_gbs"], "note": "P=1, streaming fold; R (%.2f GB) >> L2, so every eval reads it from HBM" % (r_bytes / 1e9)}
-    single["hbm_frac"] = single["hbm_gbs"] / peaks["hbm_gbs"]
+              "hbm_peak_gbs": peaks["hbm_gbs"]}
+    if r_bytes > 252e6:
+        single["note"] = ("P=1, one-launch streaming path (fold + likelihood); R (%.2f GB) >> L2, so every eval reads it "
+                          "from HBM; kernel time includes the last-CTA reduction" % (r_bytes / 1e9))
+        single["hbm_frac"] = single["hbm_gbs"] / peaks["hbm_gbs"]
+    else:
+        single["note"] = ("P=1, one-launch streaming path; R (%.1f MB) stays in the 126 MB L2 between back-to-back "
+                          "evaluations: latency-bound, no HBM fraction is claimed" % (r_bytes / 1e6))
+        single["hbm_frac"] = None
 
     # ---------------------------------------------------------------- other regimes of the same path (context lines)
     def timed(fn, reps):
@@ -314,7 +340,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": workload_config(name, inp, P, world),
+                "config": workload_config(name, inp, P, world, max_batch=max_batch),
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(P * k * 8),
                         "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path": same},

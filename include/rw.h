@@ -174,7 +174,7 @@ int64_t rw_launch_count(const rw_ctx *ctx);
 /* Measurement hooks (bench.py roofline): between begin and end every fold-kernel launch
  * (k_fold_gemm / k_fold_stream, the dominant kernels) is bracketed by CUDA events recorded on the
  * launching stream.  rw_profile_end synchronises those events and returns the summed kernel time
- * in ms and the number of launches timed (at most 4096; later launches are not bracketed). */
+ * in ms and the number of launches timed (at most 32768; later launches are not bracketed). */
 int rw_profile_begin(rw_ctx *ctx);
 int rw_profile_end(rw_ctx *ctx, double *fold_ms_total, int64_t *fold_launches);
 

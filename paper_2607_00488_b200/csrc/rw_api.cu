@@ -505,7 +505,7 @@ int rw_profile_begin(rw_ctx *ctx)
 {
     if (!ctx) return RW_ERR_INVALID;
     if (!ctx->prof_ev) {
-        const int cap = 4096;
+        const int cap = 32768;
         ctx->prof_ev = (cudaEvent_t *)calloc(2 * cap, sizeof(cudaEvent_t));
         if (!ctx->prof_ev) return fail(ctx, RW_ERR_NOMEM, "rw_profile_begin: out of host memory");
         for (int q = 0; q < 2 * cap; ++q) RW_CUDA(ctx, cudaEventCreate(&ctx->prof_ev[q]));

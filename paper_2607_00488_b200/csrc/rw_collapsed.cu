@@ -55,7 +55,7 @@ k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const doubl
         const int p = q / kCoefStride, b = q - p * kCoefStride;
         sC[p][b] = (p < np) ? coef[(p0 + p) * kCoefStride + b] : 0.0;
     }
-    double g[kNumTerms][2], bk[2], cn[2];
+    double g[kNumTerms][2], bk[2], cn[2], ci[2];
     const bool ok0 = col < n_rec, ok1 = col + 1 < n_rec;
     {
         const double *Gd = G + (size_t)d * kCoefStride * ldG;
@@ -70,27 +70,40 @@ k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const doubl
         bk[1] = ok1 ? bkg[(size_t)d * n_rec + col + 1] : 0.0;
         cn[0] = ok0 ? counts[(size_t)d * n_rec + col] : 0.0;
         cn[1] = ok1 ? counts[(size_t)d * n_rec + col + 1] : 0.0;
+        ci[0] = cn[0] > 0.0 ? 1.0 / cn[0] : 0.0;
+        ci[1] = cn[1] > 0.0 ? 1.0 / cn[1] : 0.0;
     }
     __syncthreads();
-    for (int p = 0; p < np; ++p) {
-        double m0 = 0.0, m1 = 0.0;
+    // two points per trip: four independent log1p chains per thread keep the FP64 pipe fed at 16 warps per SM
+    for (int p = 0; p < np; p += 2) {
+        double m[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
         for (int b = 0; b < kNumTerms; ++b) {
-            const double c = sC[p][b];
-            m0 = fma(c, g[b][0], m0);
-            m1 = fma(c, g[b][1], m1);
-        }
-        m0 += bk[0];
-        m1 += bk[1];
-        if (out_mu) {
-            double *dst = out_mu + ((size_t)(p0 + p) * D + d) * n_rec + col;
-            if (ok0) dst[0] = m0;
-            if (ok1) dst[1] = m1;
-        }
-        double t = (ok0 ? poisson_term(m0, cn[0]) : 0.0) + (ok1 ? poisson_term(m1, cn[1]) : 0.0);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-        if (lane == 0) red[warp][p] = t;
+            for (int u = 0; u < 2; ++u) {
+                const double c = sC[p + u][b];            // rows >= np hold zeros
+                m[u][0] = fma(c, g[b][0], m[u][0]);
+                m[u][1] = fma(c, g[b][1], m[u][1]);
+            }
+        }
+        double t[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const double m0 = m[u][0] + bk[0], m1 = m[u][1] + bk[1];
+            if (out_mu && p + u < np) {
+                double *dst = out_mu + ((size_t)(p0 + p + u) * D + d) * n_rec + col;
+                if (ok0) dst[0] = m0;
+                if (ok1) dst[1] = m1;
+            }
+            // columns >= n_rec carry template 0, bkg 0, n 0: their term is exactly 0
+            t[u] = poisson_term_inv(m0, cn[0], ci[0]) + poisson_term_inv(m1, cn[1], ci[1]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            t[0] += __shfl_xor_sync(0xffffffffu, t[0], o);
+            t[1] += __shfl_xor_sync(0xffffffffu, t[1], o);
+        }
+        if (lane == 0) { red[warp][p] = t[0]; red[warp][p + 1] = t[1]; }
     }
     __syncthreads();
     if (threadIdx.x < np) {

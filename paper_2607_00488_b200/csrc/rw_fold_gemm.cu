@@ -267,7 +267,8 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
         // ------------------------------------------------------------------ fused epilogue
         const int row0 = tc.m * BM + lrow0;
         const int col0 = tc.n * kBN + lcol0;
-        double bk[2][4], cn[2][4];
+        // columns >= n_rec: R is zero-filled there (TMA), so with bkg = n = 1/n = 0 their term is exactly 0
+        double bk[2][4], cn[2][4], ci[2][4];
 #pragma unroll
         for (int sj = 0; sj < 2; ++sj)
 #pragma unroll
@@ -276,27 +277,31 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                 const bool ok = col < W.n_rec;
                 bk[sj][q] = ok ? __ldg(W.bkg + col) : 0.0;
                 cn[sj][q] = ok ? __ldg(W.counts + col) : 0.0;
+                ci[sj][q] = cn[sj][q] > 0.0 ? 1.0 / cn[sj][q] : 0.0;
             }
+        if (W.out_mu) {
+#pragma unroll
+            for (int mb = 0; mb < MB; ++mb) {
+                const int64_t row = row0 + 8 * mb;
+#pragma unroll
+                for (int sj = 0; sj < 2; ++sj)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int col = col0 + 16 * sj + q;
+                        if (row < W.Pc && col < W.n_rec)
+                            W.out_mu[((size_t)row * W.D + W.d) * W.n_rec + col] = acc[mb][sj][q & 1][q >> 1] + bk[sj][q];
+                    }
+            }
+        }
 #pragma unroll
         for (int mb = 0; mb < MB; ++mb) {
             double sum = 0.0;
 #pragma unroll
-            for (int sj = 0; sj < 2; ++sj)
-#pragma unroll
-                for (int e = 0; e < 2; ++e)
-#pragma unroll
-                    for (int nb = 0; nb < 2; ++nb) {
-                        const int q = 2 * e + nb;
-                        const double mu = acc[mb][sj][nb][e] + bk[sj][q];
-                        const int col = col0 + 16 * sj + q;
-                        if (col < W.n_rec) {
-                            sum += poisson_term(mu, cn[sj][q]);
-                            if (W.out_mu) {
-                                const int64_t row = row0 + 8 * mb;
-                                if (row < W.Pc) W.out_mu[((size_t)row * W.D + W.d) * W.n_rec + col] = mu;
-                            }
-                        }
-                    }
+            for (int sj = 0; sj < 2; ++sj)      // column q = 2 e + nb of the group holds acc[mb][sj][nb][e]
+                sum += poisson_sum4(acc[mb][sj][0][0] + bk[sj][0], acc[mb][sj][1][0] + bk[sj][1],
+                                    acc[mb][sj][0][1] + bk[sj][2], acc[mb][sj][1][1] + bk[sj][3],
+                                    cn[sj][0], cn[sj][1], cn[sj][2], cn[sj][3],
+                                    ci[sj][0], ci[sj][1], ci[sj][2], ci[sj][3]);
             sum += __shfl_xor_sync(0xffffffffu, sum, 1);
             sum += __shfl_xor_sync(0xffffffffu, sum, 2);
             if (c == 0) red[wn * BM + lrow0 + 8 * mb] = sum;
@@ -322,12 +327,13 @@ k_tile_deviance(const double *__restrict__ mu_tile, int BM, int S, int tile0, in
     const TileCoord tc = tile_coord(tile0 + blockIdx.x, tiles_m, tiles_n);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int col = tc.n * kBN + 4 * lane;
-    double bk[4], cn[4];
+    double bk[4], cn[4], ci[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         const bool ok = col + q < n_rec;
         bk[q] = ok ? bkg[col + q] : 0.0;
         cn[q] = ok ? counts[col + q] : 0.0;
+        ci[q] = cn[q] > 0.0 ? 1.0 / cn[q] : 0.0;
     }
     const double *base = mu_tile + (size_t)blockIdx.x * S * (BM * kBN);
     for (int lr = warp; lr < BM; lr += 8) {
@@ -338,15 +344,14 @@ k_tile_deviance(const double *__restrict__ mu_tile, int BM, int S, int tile0, in
             const double2 u = q[0], v = q[1];
             m[0] += u.x; m[1] += u.y; m[2] += v.x; m[3] += v.y;
         }
-        double sum = 0.0;
+        if (out_mu && row < Pc) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const double mu = m[q] + bk[q];
-            if (col + q < n_rec) {
-                sum += poisson_term(mu, cn[q]);
-                if (out_mu && row < Pc) out_mu[((size_t)row * D + d) * n_rec + col + q] = mu;
-            }
+            for (int q = 0; q < 4; ++q)
+                if (col + q < n_rec) out_mu[((size_t)row * D + d) * n_rec + col + q] = m[q] + bk[q];
         }
+        // columns >= n_rec hold 0 + 0 with n = 0: term 0
+        double sum = poisson_sum4(m[0] + bk[0], m[1] + bk[1], m[2] + bk[2], m[3] + bk[3], cn[0], cn[1], cn[2], cn[3],
+                                  ci[0], ci[1], ci[2], ci[3]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
         if (lane == 0 && row < Pc) partial[(size_t)tc.n * part_stride + row] = sum;
