@@ -69,7 +69,16 @@ enum {
     RW_MODE_COLLAPSED = 3u << 4, /* opt-in: rank-K prefolded templates (exact, O(K n_rec) per point); see below */
     RW_MODE_MASK   = 3u << 4,
     RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
-    RW_OUT_HOST    = 1u << 9   /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
+    RW_OUT_HOST    = 1u << 9,  /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
+    RW_FP32        = 1u << 10  /* opt-in reduced precision for the batched contraction (rw_eval_batch, > 4 points, dense
+                                  fold): operands split in two TF32 pieces, three tcgen05 tensor-core products, FP32
+                                  accumulation in 128-bin chunks; mu within 1e-5 relative of the FP64 path (values below
+                                  the FP32 range flush to 0).  Needs a context created with RW_CREATE_FP32. */
+};
+
+/* rw_inputs.create_flags */
+enum {
+    RW_CREATE_FP32 = 1u << 0   /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
 };
 
 /* Physical constants.  The paper prints symbols only; any field that is 0
@@ -101,10 +110,11 @@ typedef struct {
                                RW_MEM_DEVICE: all arrays are device pointers; R is borrowed (caller keeps
                                it alive until rw_destroy) when 16-byte aligned with even n_rec, the
                                small tables are copied. */
+    uint32_t create_flags;  /* 0 or RW_CREATE_FP32 */
 } rw_inputs;
 
 /* Bytes of device workspace rw_create needs for these inputs and batches of up to max_batch points.
- * Only the sizes, n_periods and mem_kind fields of `in` are read. */
+ * Only the sizes, n_periods, mem_kind and create_flags fields of `in` are read. */
 int rw_workspace_bytes(const rw_inputs *in, int64_t max_batch, size_t *bytes);
 
 /* Validate inputs, place tables in the workspace, run the setup kernels (basis spectra, S_SM,

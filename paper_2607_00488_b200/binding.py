@@ -20,7 +20,8 @@ RW_EPS_EE_L, RW_EPS_EE_R, RW_EPS_MM_L, RW_EPS_MM_R, RW_EPS_TT_L, RW_EPS_TT_R, RW
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
 RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED = 0, 1 << 4, 2 << 4, 3 << 4
-RW_PARAM_HOST, RW_OUT_HOST = 1 << 8, 1 << 9
+RW_PARAM_HOST, RW_OUT_HOST, RW_FP32 = 1 << 8, 1 << 9, 1 << 10
+RW_CREATE_FP32 = 1
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
@@ -41,7 +42,7 @@ class rw_inputs(C.Structure):
                 ("P_mu", C.c_void_p), ("P_tau", C.c_void_p), ("f_tau", C.c_double),
                 ("n_T", C.c_int32), ("T_MeV", C.c_void_p), ("n_rec", C.c_int32), ("n_periods", C.c_int32),
                 ("N_mc", C.c_void_p), ("R", C.c_void_p), ("bkg", C.c_void_p), ("counts", C.c_void_p),
-                ("consts", rw_constants), ("mem_kind", C.c_int32)]
+                ("consts", rw_constants), ("mem_kind", C.c_int32), ("create_flags", C.c_uint32)]
 
 
 class RwError(RuntimeError):
@@ -120,7 +121,7 @@ class Reweighter:
     bkg[D][n_rec], counts[D][n_rec] as numpy arrays (host: copied at create) or, with
     tables_on_device=True, CUDA float64 torch tensors (R is borrowed, the rest copied)."""
 
-    def __init__(self, inputs, max_batch, device="cuda:0", consts=None):
+    def __init__(self, inputs, max_batch, device="cuda:0", consts=None, fp32=False):
         self._L = load_library()
         self._ctx = C.c_void_p(None)
         self.device = torch.device(device)
@@ -161,6 +162,7 @@ class Reweighter:
             inp.consts = rw_constants(*[float(consts.get(k, 0.0)) for k in
                                         ("sin2_theta_w", "m_e_MeV", "G_F_MeV2", "alpha_em")])
         inp.mem_kind = RW_MEM_DEVICE if on_device else RW_MEM_HOST
+        inp.create_flags = RW_CREATE_FP32 if fp32 else 0
         self.n_E, self.n_T, self.n_rec, self.n_periods = inp.n_E, n_T, n_rec, D
         self.max_batch = int(max_batch)
         nbytes = C.c_size_t(0)
@@ -181,14 +183,14 @@ class Reweighter:
             msg = self._L.rw_last_error(ctx).decode() or self._L.rw_strerror(rc).decode()
             raise RwError(rc, msg)
 
-    def eval_batch(self, param, kinds, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
+    def eval_batch(self, param, kinds, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto", fp32=False):
         """-2lnL[P] for param[P][k] (CUDA float64 tensor, or numpy/pinned CPU tensor => host path).
 
         Device params: asynchronous on the current stream, returns a CUDA tensor.
         Host params: H2D + kernels + D2H are enqueued on the current stream; returns a CPU tensor
         (pinned), valid after the stream is synchronised."""
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_FP32 if fp32 else 0)
         host = not (isinstance(param, torch.Tensor) and param.is_cuda)
         if host:
             if isinstance(param, np.ndarray):

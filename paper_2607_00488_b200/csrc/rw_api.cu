@@ -44,6 +44,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
     L->KPAD = (int)((n_T + kBK - 1) / kBK * kBK);
     L->A_pitch = (int64_t)L->KPAD * 8;
+    L->KP32 = (int)((n_T + 3) / 4 * 4);
+    L->fp32 = (in->create_flags & RW_CREATE_FP32) != 0;
     int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;
     if (cap > kMaxChunkRows) cap = kMaxChunkRows;
@@ -100,6 +102,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         L->prof_rows = rows;
         L->mu_prof = take((size_t)rows * D * n_rec * 8);
     }
+    L->R32 = take(L->fp32 ? D * 2 * n_rec * (size_t)L->KP32 * 4 : 0);
     L->total = off;
     return RW_OK;
 }
@@ -142,7 +145,8 @@ static bool auto_stream(const rw_ctx *, int64_t P) { return P <= 4; }
 
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
-static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s)
+static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s,
+                      bool fp32 = false)
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
@@ -167,8 +171,12 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
-                RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
-                RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                if (fp32) {
+                    RW_CUDA(ctx, launch_fold_tf32(ctx, d, c0, Pc, mu, s));
+                } else {
+                    RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
+                    RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                }
             }
             RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, dout + c0, full, s));
         }
@@ -291,6 +299,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->out_stage = (double *)(ws + L.out_stage);
     ctx->mu_tile = (double *)(ws + L.mu_tile);
     ctx->mu_prof = (double *)(ws + L.mu_prof);
+    ctx->R32 = (float *)(ws + L.R32);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;
@@ -339,7 +348,14 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     }
     rc = make_tensor_maps(ctx);
     if (rc == RW_OK) rc = profile_setup(ctx);
-    if (rc != RW_OK) { free(ctx->tmapR); free(ctx); return rc; }
+    if (rc == RW_OK && L.fp32) {
+        ctx->tmapB32 = (CUtensorMap *)calloc(2 * D, sizeof(CUtensorMap));
+        if (!ctx->tmapB32) rc = fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory");
+        if (rc == RW_OK) rc = tf32_setup(ctx, s);
+        if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
+            rc = fail(nullptr, RW_ERR_CUDA, "rw_create: TF32 split of R failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    if (rc != RW_OK) { free(ctx->tmapB32); free(ctx->tmapR); free(ctx); return rc; }
     ctx->err[0] = 0;
     *out = ctx;
     return RW_OK;
@@ -378,6 +394,9 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
+    const bool fp32 = flags & RW_FP32;
+    if (fp32 && !ctx->lay.fp32)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_FP32 needs a context created with RW_CREATE_FP32");
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -410,7 +429,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             }
         } else {
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
-        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s); if (rc != RW_OK) return rc; }
+        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, fp32); if (rc != RW_OK) return rc; }
         }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
@@ -539,6 +558,7 @@ int rw_destroy(rw_ctx *ctx)
         for (int q = 0; q < 2 * ctx->prof_cap; ++q) cudaEventDestroy(ctx->prof_ev[q]);
         free(ctx->prof_ev);
     }
+    free(ctx->tmapB32);
     free(ctx->tmapR);
     free(ctx);
     return RW_OK;

@@ -47,7 +47,7 @@ struct Kinds { int k; int kind[RW_N_KINDS]; };
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part;
-    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof;
+    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof, R32;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
@@ -56,6 +56,8 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int n_tiles_n;        // ceil(n_rec / kBN)
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
+    int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
+    bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
     int ldG;              // row pitch of the prefolded templates G[D][12][ldG] (n_rec rounded up to even)
@@ -82,6 +84,9 @@ struct rw_ctx {
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
+    float *R32;               // [D][2 (hi, lo)][n_rec][KP32] transposed TF32 split of R (RW_CREATE_FP32)
+    CUtensorMap tmapA32[2];   // hi, lo of N' (aliases A_packed)
+    CUtensorMap *tmapB32;     // host array [2 D]
     double *mu_prof;          // rw_eval_profile scratch: mu[prof_rows][D][n_rec]
     double *mu_tile;          // split-K scratch: [mu_tile_items][<=128][128] parked accumulators
     CUtensorMap *tmapR;       // host array [D]
@@ -128,6 +133,8 @@ cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // 
 cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, double s0, double sigma,
                            bool full_eq18, double *out, double *out_scale, cudaStream_t s);   // rw_profile.cu
 int profile_setup(rw_ctx *ctx);                                              // rw_profile.cu
+int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
+cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,
                              cudaStream_t s);                                // rw_collapsed.cu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
