@@ -30,9 +30,9 @@ METRIC = "likelihood evals/sec (batched)"
 UNIT = "evals/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_fold_gemm launch from the committed
-# `ncu --set full` capture (profiles/r01b_fold_gemm_full.md: the fused launch over the 110 full waves of one
+# `ncu --set full` capture (profiles/r01c_fold_gemm_full.md: the fused launch over the 110 full waves of one
 # 32768-point chunk), or None if not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 54.395468e9 + 0.030036e9}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 69.584991e9 + 0.032040e9}
 
 
 def load_peaks():
@@ -188,7 +188,7 @@ def main():
                for key in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
     dev_inp["f_tau"] = inp["f_tau"]
     max_batch = args.max_batch or (16384 if name == "cfg5_joint6" else P)
-    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev)
+    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=True)   # + TF32 copy of R for the opt-in leg
     param_dev = torch.from_numpy(params).to(dev)
     out_dev = torch.empty(P, dtype=torch.float64, device=dev)
     param_pin = torch.from_numpy(params).pin_memory()
@@ -310,6 +310,22 @@ def main():
                  "max_abs_diff_vs_dense_fold": dmax,
                  "note": "2*11*n_rec*D flop per point plus one log1p per bin; see profiles/ for the FP64-pipe utilisation"}
 
+    # opt-in RW_FP32 contraction: TF32 x 3 on tcgen05, 1e-5 relative on mu; never mixed into `value`
+    fp32_leg = None
+    if P > 4:
+        out_f = torch.empty(P, dtype=torch.float64, device=dev)
+        t_f = timed(lambda: ctx.eval_batch(param_dev, kinds, out=out_f, fp32=True), 5)
+        ns = min(P, 128)
+        _, mu32 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm", fp32=True)
+        _, mu64 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm")
+        rel = ((mu32 - mu64).abs() / mu64.abs())
+        fp32_leg = {"ms_per_call": t_f, "evals_per_s": P / t_f * 1e3, "bound": "tensor (tf32) / L2",
+                    "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_f / 1e9,
+                    "executed_tf32_tflops": 6.0 * n_T * n_rec * D * P / t_f / 1e9,
+                    "mu_rel_err_vs_fp64_max": float(rel.max().item()), "mu_rel_err_vs_fp64_mean": float(rel.mean().item()),
+                    "note": "three tcgen05.mma.kind::tf32 products per k-step (hi*hi, hi*lo, lo*hi), FP32 accumulation in "
+                            "128-bin TMEM chunks; the three-fold executed flops are not counted in effective_fold_tflops"}
+
     # ---------------------------------------------------------------- roofline of the dominant kernel
     dmma_peak = binding.probe_fp64_peak(1)
     dfma_peak = binding.probe_fp64_peak(0)
@@ -345,7 +361,7 @@ def main():
                         "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path": same},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
-                "batch_sweep": sweep, "collapsed_mode": collapsed,
+                "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg,
                 "clocks": clocks, "all_finite": finite,
                 "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
                                  "the authors' own multi-component model; other hardware and inputs, not comparable"}
