@@ -203,6 +203,9 @@ def main():
     def maxreduce(x):
         return sharding.max_over_ranks(x, dev, world)
 
+    dmma_peak0 = binding.probe_fp64_peak(1)
+    dfma_peak0 = binding.probe_fp64_peak(0)
+
     # ---------------------------------------------------------------- device-resident throughput
     for _ in range(args.warmup):
         ctx.eval_batch(param_dev, kinds, out=out_dev)
@@ -327,8 +330,10 @@ def main():
                             "128-bin TMEM chunks; the three-fold executed flops are not counted in effective_fold_tflops"}
 
     # ---------------------------------------------------------------- roofline of the dominant kernel
-    dmma_peak = binding.probe_fp64_peak(1)
-    dfma_peak = binding.probe_fp64_peak(0)
+    # the probe is taken before the timed region and again here; the higher reading is the denominator (a probe
+    # right after the TF32 leg can catch a lower clock)
+    dmma_peak = max(dmma_peak0, binding.probe_fp64_peak(1))
+    dfma_peak = max(dfma_peak0, binding.probe_fp64_peak(0))
     flops_timed = 2.0 * n_T * n_rec * D * P * args.steps           # algorithmic: 2 N_T N_rec per point and period
     achieved = flops_timed / (fold_ms * 1e-3) / 1e12
     traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(name)
