@@ -33,6 +33,9 @@
  *   orc_profile_scale closed form s^ = sum n / sum S (no background, no pull); Asimov data at s* => s^ = s*,
  *                     value 0; scipy.optimize.minimize_scalar on a numpy objective;
  *                     pull limits sigma -> 0 (s^ -> s0) and sigma -> inf; boundary s^ = 0
+ *   orc_eval_components  n_comp = 1 reproduces orc_eval_batch; identical tables split over two components
+ *                     reproduce it too; mu - bkg is linear in the per-component rates with the single-component
+ *                     predictions as coefficients; a component's bins get the weights of its own flux table
  *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
  *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
@@ -467,6 +470,70 @@ int orc_eval_weights(int n_T, int n_rec, int n_periods, const double *N_mc, cons
         if (abs_out) abs_out[p] = (double)total_abs;
         free(xw);
     }
+    return 0;
+}
+
+/* Several signal components (Eq. 17: mu_j = MT M_j sum_k rate_k f^(k)(j; eps); Sec. IV B a-b,
+ * every neutrino component has its own flux, survival probability, recoil spectrum and
+ * response).  The recoil bins of all components are concatenated along the contraction index: bin i belongs to
+ * component comp_of_T[i], its spectrum (Eq. 12) and SM reference use that component's flux table
+ * flux_w[comp][.], P_alpha[comp][.] on the shared E grid, its response rows are R[.][i][.], and a per-point
+ * rate scale multiplies its reweighted MC content.  Parameter kinds 0..6 as orc_eval_batch; kind 7 + c is the
+ * rate scale of component c (absent => 1).  n_comp <= 4. */
+int orc_eval_components(const orc_consts *c, int n_E, const double *E, int n_comp, const double *flux_w,
+                        const double *P_e, const double *P_mu, const double *P_tau,
+                        int n_T, const double *T, const int32_t *comp_of_T, int n_rec, int n_periods,
+                        const double *N_mc, const double *R, const double *bkg, const double *counts,
+                        int64_t P, int k, const int32_t *kinds, const double *params,
+                        double *out, double *mu_out, double *abs_out, int full_eq18, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    if (n_comp < 1 || n_comp > 4) return -1;
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS + n_comp) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    for (int i = 0; i < n_T; ++i) if (comp_of_T[i] < 0 || comp_of_T[i] >= n_comp) return -1;
+    size_t nT = (size_t)(n_T > 0 ? n_T : 1);
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * nT * 2), *tmp0 = S0 + nT;
+    for (int q = 0; q < n_comp; ++q) {      /* SM reference of every bin from its own component's table */
+        xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E, P_mu + (size_t)q * n_E,
+                  P_tau + (size_t)q * n_E, n_T, T, zero, tmp0);
+        for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S0[i] = tmp0[i];
+    }
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        double rate[4] = {1.0, 1.0, 1.0, 1.0};
+        for (int a = 0; a < k; ++a) {
+            if (kinds[a] < ORC_N_KINDS) theta[kinds[a]] = params[p * k + a];
+            else rate[kinds[a] - ORC_N_KINDS] = params[p * k + a];
+        }
+        xreal *S = (xreal *)malloc(sizeof(xreal) * (3 * nT + (size_t)n_rec + 1));
+        xreal *tmp = S + nT, *w = tmp + nT, *mu = w + nT;
+        for (int q = 0; q < n_comp; ++q) {
+            xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E, P_mu + (size_t)q * n_E,
+                      P_tau + (size_t)q * n_E, n_T, T, theta, tmp);
+            for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S[i] = tmp[i];
+        }
+        xweights(n_T, S, S0, w);
+        for (int i = 0; i < n_T; ++i) w[i] *= (xreal)rate[comp_of_T[i]];      /* rate_k of Eq. (17) */
+        xreal total = 0.0L, total_abs = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            const double *Cd = counts + (size_t)d * n_rec;
+            xfold(n_T, n_rec, w, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, bkg + (size_t)d * n_rec, mu);
+            total += full_eq18 ? xeq18(n_rec, mu, Cd) : xdeviance(n_rec, mu, Cd);
+            if (mu_out)
+                for (int q = 0; q < n_rec; ++q) mu_out[((size_t)p * n_periods + d) * n_rec + q] = (double)mu[q];
+            if (abs_out)
+                for (int q = 0; q < n_rec; ++q) total_abs += fabsl(xdeviance(1, mu + q, Cd + q));
+        }
+        out[p] = (double)total;
+        if (abs_out) abs_out[p] = (double)total_abs;
+        free(S);
+    }
+    free(S0);
     return 0;
 }
 

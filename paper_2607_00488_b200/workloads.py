@@ -215,6 +215,37 @@ def make_custom(n_E=31, n_T=77, n_rec=53, n_periods=1, seed=1234, n_lines=1, tai
                 exposure=np.ones(n_periods), N_tot=1.0, N_mc=N_mc, counts=counts)
 
 
+def make_components(n_comp=2, n_E=41, n_T=96, n_rec=53, n_periods=1, seed=4321):
+    """Small multi-component raw tables (Eq. 17 structure): n_comp flux tables on one E grid (a continuum with a
+    different endpoint each, component 0 also a line), component-specific survival probabilities, and the recoil bins
+    of the components concatenated (comp_of_T), each block with its own recoil grid and response rows."""
+    rng = np.random.default_rng(seed)
+    E, _ = _midpoints(0.2, 14.0, n_E - 1)
+    E = np.append(E, 0.862)
+    dE = (14.0 - 0.2) / (n_E - 1)
+    fw = np.zeros((n_comp, n_E))
+    P_e = np.zeros((n_comp, n_E))
+    for c in range(n_comp):
+        end = 14.0 / (1 + c)
+        fw[c, :-1] = np.where(E[:-1] < end, E[:-1] ** 2 * (end - E[:-1]) ** 2, 0.0) * dE
+        if c == 0:
+            fw[c, -1] = 0.3 * fw[c, :-1].sum()
+        P_e[c] = np.clip(p_ee(E) + 0.03 * c, 0.0, 1.0)
+    sizes = [n_T // n_comp + (1 if c < n_T % n_comp else 0) for c in range(n_comp)]
+    comp = np.concatenate([np.full(sz, c, np.int32) for c, sz in enumerate(sizes)])
+    T = np.concatenate([_midpoints(0.0, 12.0 / (1 + c), sz)[0] for c, sz in enumerate(sizes)])
+    _, rec_edges = _midpoints(0.0, 12.0, n_rec)
+    R = np.empty((n_periods, n_T, n_rec))
+    for d in range(n_periods):
+        eff = rng.uniform(0.85, 0.95, size=n_T)
+        R[d] = gaussian_response(T, rec_edges, 0.08 * (1 + 0.1 * d) * np.sqrt(T) + 0.05, eff, tail=0.01)
+    bkg = rng.uniform(1.0, 6.0, size=(n_periods, n_rec))
+    N_mc = rng.uniform(10.0, 500.0, size=(n_periods, n_T))
+    counts = rng.poisson(rng.uniform(5.0, 400.0, size=(n_periods, n_rec))).astype(np.float64)
+    return dict(E=E, flux_w=fw, P_e=P_e, f_tau=0.5, T=T, comp_of_T=comp, rec_edges=rec_edges, R=R, bkg=bkg,
+                N_mc=N_mc, counts=counts)
+
+
 def random_points(P, kinds, seed):
     """P random scan points for the given kinds: eps ~ U(-0.5,0.5), mu_nu log-uniform [1e-12,1e-10]."""
     rng = np.random.default_rng(seed)
@@ -223,4 +254,6 @@ def random_points(P, kinds, seed):
     for a, kd in enumerate(kinds):
         if kd == MU_NU:
             p[:, a] = 10.0 ** rng.uniform(-12.0, -10.0, size=P)
+        elif kd > MU_NU:                       # rate scales of signal components
+            p[:, a] = rng.uniform(0.5, 1.5, size=P)
     return p, kinds

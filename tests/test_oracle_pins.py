@@ -436,6 +436,43 @@ def test_eval_profile_composition_and_asimov(orc):
     assert pulled[2] > out[2] and 1.0 < scp[2] < 1.7
 
 
+def test_eval_components_pins(orc):
+    """Multi-component path (Eq. 17): (i) one component = eval_batch; (ii) two components with the same
+    tables = eval_batch on the concatenated bins; (iii) mu - bkg is linear in the rates, with the single-component
+    predictions as coefficients; (iv) a component's bins are weighted with its own flux table."""
+    one = _small_problem(D=2)
+    params, kinds = wl.random_points(4, [orc.EPS_EE_L, orc.EPS_TT_R, orc.MU_NU], seed=41)
+    ref, mu_ref = orc.eval_batch(one, params, kinds, want_mu=True)
+    as1 = dict(one, comp_of_T=np.zeros(one["T"].size, np.int32))
+    out, mu = orc.eval_components(as1, params, kinds, want_mu=True)
+    assert np.array_equal(out, ref) and np.array_equal(mu, mu_ref)
+    split = dict(one, flux_w=np.stack([one["flux_w"]] * 2), P_e=np.stack([one["P_e"]] * 2),
+                 comp_of_T=(np.arange(one["T"].size) % 2).astype(np.int32))
+    out, mu = orc.eval_components(split, params, kinds, want_mu=True, nthreads=2)
+    assert np.array_equal(out, ref) and np.array_equal(mu, mu_ref)
+
+    mc = wl.make_components(n_comp=3, n_E=30, n_T=60, n_rec=31, n_periods=2, seed=42)
+    kinds3 = np.array([orc.EPS_EE_L, orc.MU_NU, orc.RATE_0, orc.RATE_0 + 2], np.int32)
+    p3, _ = wl.random_points(3, kinds3, seed=43)
+    out, mu = orc.eval_components(mc, p3, kinds3, want_mu=True)
+    for p in range(3):
+        pred = np.zeros_like(mu[p])
+        rates = [p3[p, 2], 1.0, p3[p, 3]]
+        for c in range(3):
+            only = dict(mc, N_mc=np.where(mc["comp_of_T"] == c, mc["N_mc"], 0.0))
+            _, mu_c = orc.eval_components(only, p3[p:p + 1, :2], kinds3[:2], want_mu=True)
+            pred += rates[c] * (mu_c[0] - mc["bkg"])
+            # (iv) component c alone = a single-component problem with its own table on its own bins
+            sel = mc["comp_of_T"] == c
+            single = dict(E=mc["E"], flux_w=mc["flux_w"][c], P_e=mc["P_e"][c], f_tau=0.5, T=mc["T"][sel],
+                          N_mc=mc["N_mc"][:, sel], R=mc["R"][:, sel, :], bkg=mc["bkg"], counts=mc["counts"])
+            _, mu_s = orc.eval_batch(single, p3[p:p + 1, :2], kinds3[:2], want_mu=True)
+            assert np.all(np.abs(mu_s[0] / mu_c[0] - 1) < 1e-15)
+        assert np.all(np.abs((pred + mc["bkg"]) / mu[p] - 1) < 1e-14)
+    with pytest.raises(ValueError):
+        orc.eval_components(mc, p3, [0, 6, 7, 10])          # rate kind of a component that does not exist
+
+
 def test_sm_point_gives_sm_prediction(orc):
     inp = _small_problem(D=2)
     _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
