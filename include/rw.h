@@ -54,8 +54,13 @@ enum {
     RW_EPS_MM_L = 2, RW_EPS_MM_R = 3,
     RW_EPS_TT_L = 4, RW_EPS_TT_R = 5,
     RW_MU_NU = 6,
-    RW_N_KINDS = 7
+    RW_RATE_0 = 7,          /* RW_RATE_0 + c: rate scale of signal component c (rate_k of Eq. 17); */
+    RW_RATE_1 = 8,          /* multiplies that component's reweighted MC content; absent => 1.  c < n_comp <= 4 */
+    RW_RATE_2 = 9,
+    RW_RATE_3 = 10,
+    RW_N_KINDS = 11
 };
+enum { RW_MAX_COMPONENTS = 4 };
 
 enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
 
@@ -111,6 +116,11 @@ typedef struct {
                                it alive until rw_destroy) when 16-byte aligned with even n_rec, the
                                small tables are copied. */
     uint32_t create_flags;  /* 0 or RW_CREATE_FP32 */
+    int32_t n_comp;         /* signal components (Eq. 17; Sec. IV B); 0 or 1: one.
+                               With n_comp > 1, flux_w, P_e (and P_mu, P_tau) are [n_comp][n_E] tables on the shared
+                               E grid, and the recoil bins of all components are concatenated along n_T. */
+    const int32_t *comp_of_T; /* [n_T] component of every recoil bin (same memory kind as the other arrays);
+                               ignored (may be NULL) when n_comp <= 1.  RW_MODE_COLLAPSED needs n_comp <= 1. */
 } rw_inputs;
 
 /* Bytes of device workspace rw_create needs for these inputs and batches of up to max_batch points.
@@ -128,7 +138,7 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
 
 /* -2lnL for P points.
  *   param       [P][k] row-major, device pointer (host if RW_PARAM_HOST)
- *   param_kind  host [k], distinct values in RW_EPS_EE_L..RW_MU_NU; absent kinds are 0
+ *   param_kind  host [k], distinct values in RW_EPS_EE_L..RW_MU_NU (absent: 0) and RW_RATE_0 + c, c < n_comp (absent: 1)
  *   out_m2lnL   [P] device pointer (host if RW_OUT_HOST)
  *   out_mu      NULL, or [P][D][n_rec] predicted counts mu (same memory kind as out_m2lnL)
  * P may be 0 (no-op) and may exceed max_batch (processed in slices).  Per-point numerical outcomes

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "librw.so")
 
 # param kinds (include/rw.h)
 RW_EPS_EE_L, RW_EPS_EE_R, RW_EPS_MM_L, RW_EPS_MM_R, RW_EPS_TT_L, RW_EPS_TT_R, RW_MU_NU = range(7)
+RW_RATE_0 = 7        # RW_RATE_0 + c: rate scale of signal component c
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
 RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED = 0, 1 << 4, 2 << 4, 3 << 4
@@ -42,7 +43,8 @@ class rw_inputs(C.Structure):
                 ("P_mu", C.c_void_p), ("P_tau", C.c_void_p), ("f_tau", C.c_double),
                 ("n_T", C.c_int32), ("T_MeV", C.c_void_p), ("n_rec", C.c_int32), ("n_periods", C.c_int32),
                 ("N_mc", C.c_void_p), ("R", C.c_void_p), ("bkg", C.c_void_p), ("counts", C.c_void_p),
-                ("consts", rw_constants), ("mem_kind", C.c_int32), ("create_flags", C.c_uint32)]
+                ("consts", rw_constants), ("mem_kind", C.c_int32), ("create_flags", C.c_uint32),
+                ("n_comp", C.c_int32), ("comp_of_T", C.c_void_p)]
 
 
 class RwError(RuntimeError):
@@ -118,8 +120,9 @@ class Reweighter:
     """One rw_ctx: device-resident tables of one analysis + its workspace (a torch uint8 tensor).
 
     `inputs` is a dict with E, flux_w, P_e, [P_mu, P_tau | f_tau], T, N_mc[D][n_T], R[D][n_T][n_rec],
-    bkg[D][n_rec], counts[D][n_rec] as numpy arrays (host: copied at create) or, with
-    tables_on_device=True, CUDA float64 torch tensors (R is borrowed, the rest copied)."""
+    bkg[D][n_rec], counts[D][n_rec] as numpy arrays (host: copied at create) or CUDA float64 torch tensors
+    (R is borrowed, the rest copied).  Several signal components (Eq. 17): flux_w, P_e[, P_mu, P_tau] as
+    [n_comp][n_E] plus comp_of_T[n_T]; parameter kinds RW_RATE_0 + c then scale component c."""
 
     def __init__(self, inputs, max_batch, device="cuda:0", consts=None, fp32=False):
         self._L = load_library()
@@ -163,6 +166,19 @@ class Reweighter:
                                         ("sin2_theta_w", "m_e_MeV", "G_F_MeV2", "alpha_em")])
         inp.mem_kind = RW_MEM_DEVICE if on_device else RW_MEM_HOST
         inp.create_flags = RW_CREATE_FP32 if fp32 else 0
+        fw = inputs["flux_w"]
+        inp.n_comp = int(fw.shape[0]) if fw.ndim == 2 else 1
+        if inp.n_comp > 1:
+            comp = inputs["comp_of_T"]
+            if on_device:
+                t = torch.as_tensor(comp).to(device=self.device, dtype=torch.int32).contiguous()
+                keep["comp_of_T"] = t
+                inp.comp_of_T = C.c_void_p(t.data_ptr())
+            else:
+                a = np.ascontiguousarray(comp.cpu().numpy() if isinstance(comp, torch.Tensor) else comp, dtype=np.int32)
+                keep["comp_of_T"] = a
+                inp.comp_of_T = C.c_void_p(a.ctypes.data)
+        self.n_comp = inp.n_comp
         self.n_E, self.n_T, self.n_rec, self.n_periods = inp.n_E, n_T, n_rec, D
         self.max_batch = int(max_batch)
         nbytes = C.c_size_t(0)

@@ -38,6 +38,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         return RW_ERR_INVALID;
     if (in->mem_kind != RW_MEM_HOST && in->mem_kind != RW_MEM_DEVICE) return RW_ERR_INVALID;
     const size_t n_E = in->n_E, n_T = in->n_T, n_rec = in->n_rec, D = in->n_periods;
+    if (in->n_comp < 0 || in->n_comp > RW_MAX_COMPONENTS) return RW_ERR_INVALID;
+    const size_t n_comp = in->n_comp > 1 ? in->n_comp : 1;
     memset(L, 0, sizeof(*L));
     L->max_batch = max_batch;
     L->copy_R = (in->mem_kind == RW_MEM_HOST) || (n_rec & 1);
@@ -64,8 +66,10 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     L->E = take(n_E * 8);
-    L->fw = take(n_E * 8);
-    L->P3 = take(3 * n_E * 8);
+    L->fw = take(n_comp * n_E * 8);
+    L->P3 = take(n_comp * 3 * n_E * 8);
+    L->comp8 = take(n_comp > 1 ? n_T : 0);
+    L->rate = take((size_t)max_batch * RW_MAX_COMPONENTS * 8);
     L->T = take(n_T * 8);
     L->Tmax_invE = take(3 * n_E * 8);
     L->N_mc = take(D * n_T * 8);
@@ -136,6 +140,7 @@ static const char *flag_message(int f)
     if (f & 32) return "bkg must be finite and >= 0";
     if (f & 64) return "counts must be finite and >= 0";
     if (f & 128) return "R must be finite and >= 0";
+    if (f & 256) return "comp_of_T must lie in [0, n_comp)";
     return "invalid input";
 }
 
@@ -188,7 +193,7 @@ static int check_kinds(rw_ctx *ctx, const char *fn, int32_t k, const int32_t *pa
 {
     for (int a = 0; a < k; ++a) {
         kinds[a] = param_kind[a];
-        if (kinds[a] < 0 || kinds[a] >= RW_N_KINDS)
+        if (kinds[a] < 0 || kinds[a] >= RW_RATE_0 + ctx->n_comp)
             return fail(ctx, RW_ERR_INVALID, "%s: param_kind[%d] = %d out of range", fn, a, kinds[a]);
         for (int b = 0; b < a; ++b)
             if (kinds[b] == kinds[a]) return fail(ctx, RW_ERR_INVALID, "%s: duplicate param_kind %d", fn, kinds[a]);
@@ -225,6 +230,9 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     if ((in->P_mu == nullptr) != (in->P_tau == nullptr))
         return fail(nullptr, RW_ERR_INVALID, "rw_create: P_mu and P_tau must both be given or both be NULL");
     const bool have_mt = in->P_mu != nullptr;
+    const size_t n_comp = in->n_comp > 1 ? in->n_comp : 1;
+    if (n_comp > 1 && !in->comp_of_T)
+        return fail(nullptr, RW_ERR_INVALID, "rw_create: comp_of_T is NULL with n_comp = %d", in->n_comp);
     double f_tau = in->f_tau;
     if (!have_mt && !(f_tau >= 0.0 && f_tau <= 1.0))
         return fail(nullptr, RW_ERR_INVALID, "rw_create: f_tau must lie in [0,1]");
@@ -248,8 +256,12 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     if (host) {
         int f = 0;
         if (host_bad_pos(in->E_MeV, n_E)) f |= 1;
-        if (host_bad_nonneg(in->flux_w, n_E)) f |= 2;
-        if (host_bad_prob(in->P_e, n_E) || (have_mt && (host_bad_prob(in->P_mu, n_E) || host_bad_prob(in->P_tau, n_E)))) f |= 4;
+        if (host_bad_nonneg(in->flux_w, n_comp * n_E)) f |= 2;
+        if (host_bad_prob(in->P_e, n_comp * n_E) ||
+            (have_mt && (host_bad_prob(in->P_mu, n_comp * n_E) || host_bad_prob(in->P_tau, n_comp * n_E)))) f |= 4;
+        if (n_comp > 1)
+            for (size_t i = 0; i < n_T; ++i)
+                if (in->comp_of_T[i] < 0 || in->comp_of_T[i] >= (int32_t)n_comp) f |= 256;
         if (host_bad_pos(in->T_MeV, n_T)) f |= 8;
         if (host_bad_nonneg(in->N_mc, D * n_T)) f |= 16;
         if (host_bad_nonneg(in->bkg, D * n_rec)) f |= 32;
@@ -265,6 +277,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->tmapR = (CUtensorMap *)calloc(D, sizeof(CUtensorMap));
     if (!ctx->tmapR) { free(ctx); return fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory"); }
     ctx->n_E = in->n_E; ctx->n_T = in->n_T; ctx->n_rec = in->n_rec; ctx->D = in->n_periods;
+    ctx->n_comp = (int)n_comp;
     ctx->lay = L;
     ctx->num_sms = sms;
     ctx->ws = (char *)dev_workspace;
@@ -283,6 +296,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     char *ws = ctx->ws;
     ctx->E = (double *)(ws + L.E);          ctx->fw = (double *)(ws + L.fw);
     ctx->P3 = (double *)(ws + L.P3);        ctx->T = (double *)(ws + L.T);
+    ctx->comp8 = n_comp > 1 ? (uint8_t *)(ws + L.comp8) : nullptr;
+    ctx->rate = (double *)(ws + L.rate);
     ctx->Tmax_invE = (double *)(ws + L.Tmax_invE);
     ctx->N_mc = (double *)(ws + L.N_mc);    ctx->bkg = (double *)(ws + L.bkg);
     ctx->counts = (double *)(ws + L.counts);
@@ -316,11 +331,23 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         }                                                                                       \
     } while (0)
     RW_TRY(cudaMemcpyAsync(ctx->E, in->E_MeV, n_E * 8, kind, s));
-    RW_TRY(cudaMemcpyAsync(ctx->fw, in->flux_w, n_E * 8, kind, s));
-    RW_TRY(cudaMemcpyAsync(ctx->P3, in->P_e, n_E * 8, kind, s));
-    if (have_mt) {
-        RW_TRY(cudaMemcpyAsync(ctx->P3 + n_E, in->P_mu, n_E * 8, kind, s));
-        RW_TRY(cudaMemcpyAsync(ctx->P3 + 2 * n_E, in->P_tau, n_E * 8, kind, s));
+    RW_TRY(cudaMemcpyAsync(ctx->fw, in->flux_w, n_comp * n_E * 8, kind, s));
+    for (size_t q = 0; q < n_comp; ++q) {                      // [n_comp][n_E] tables -> P3[n_comp][3][n_E]
+        RW_TRY(cudaMemcpyAsync(ctx->P3 + q * 3 * n_E, in->P_e + q * n_E, n_E * 8, kind, s));
+        if (have_mt) {
+            RW_TRY(cudaMemcpyAsync(ctx->P3 + q * 3 * n_E + n_E, in->P_mu + q * n_E, n_E * 8, kind, s));
+            RW_TRY(cudaMemcpyAsync(ctx->P3 + q * 3 * n_E + 2 * n_E, in->P_tau + q * n_E, n_E * 8, kind, s));
+        }
+    }
+    uint8_t *comp_host = nullptr;                              // host staging of comp_of_T, freed after the sync
+    if (n_comp > 1) {
+        RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
+        if (host) {
+            comp_host = (uint8_t *)malloc(n_T);
+            if (!comp_host) { free(ctx->tmapR); free(ctx); return fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory"); }
+            for (size_t i = 0; i < n_T; ++i) comp_host[i] = (uint8_t)in->comp_of_T[i];
+            RW_TRY(cudaMemcpyAsync(ctx->comp8, comp_host, n_T, cudaMemcpyHostToDevice, s));
+        }
     }
     RW_TRY(cudaMemcpyAsync(ctx->T, in->T_MeV, n_T * 8, kind, s));
     RW_TRY(cudaMemcpyAsync(ctx->N_mc, in->N_mc, D * n_T * 8, kind, s));
@@ -331,6 +358,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         RW_TRY(cudaMemcpy2DAsync(ws + L.R_copy, (size_t)L.ldR * 8, in->R, n_rec * 8, n_rec * 8, D * n_T, kind, s));
     }
     RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
+    if (n_comp > 1 && !host) RW_TRY(launch_comp8(ctx, in->comp_of_T, s));
     RW_TRY(cudaMemsetAsync(ctx->stream_cnt, 0, (D * (size_t)L.stream_strips + 1) * 4, s));
     RW_TRY(launch_flavour(ctx, have_mt ? 1 : 0, f_tau, s));
     if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
@@ -340,6 +368,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     int flag = 0;
     RW_TRY(cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
     RW_TRY(cudaStreamSynchronize(s));
+    free(comp_host);
 #undef RW_TRY
     if (flag) {
         fail(nullptr, RW_ERR_INVALID, "rw_create: %s", flag_message(flag));
@@ -385,7 +414,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
                   double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
 {
     if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_batch: ctx is NULL");
-    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: P < 0 or k outside [0,7]");
+    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: P < 0 or k outside [0,11]");
     if (P == 0) return RW_OK;
     if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
         return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param, param_kind or out_m2lnL is NULL");
@@ -394,6 +423,8 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
+    if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_MODE_COLLAPSED needs a single signal component");
     const bool fp32 = flags & RW_FP32;
     if (fp32 && !ctx->lay.fp32)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_FP32 needs a context created with RW_CREATE_FP32");
@@ -442,7 +473,9 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
                     void *cuda_stream)
 {
     if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_profile: ctx is NULL");
-    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: P < 0 or k outside [0,7]");
+    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: P < 0 or k outside [0,11]");
+    if ((flags & RW_MODE_MASK) == RW_MODE_COLLAPSED && ctx->n_comp > 1)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_profile: RW_MODE_COLLAPSED needs a single signal component");
     if (P == 0) return RW_OK;
     if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
         return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: param, param_kind or out_m2lnL is NULL");

@@ -12,14 +12,16 @@
 namespace rw {
 
 __global__ void k_coef(const double *__restrict__ param, int64_t P, Kinds kd, Consts cst,
-                       double *__restrict__ coef)
+                       double *__restrict__ coef, double *__restrict__ rate)
 {
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= P) return;
-    double c[kCoefStride];
-    coef_from_param(param + p * kd.k, kd, cst, c);
+    double c[kCoefStride], r[RW_MAX_COMPONENTS];
+    coef_from_param(param + p * kd.k, kd, cst, c, r);
 #pragma unroll
     for (int b = 0; b < kCoefStride; ++b) coef[p * kCoefStride + b] = c[b];
+#pragma unroll
+    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) rate[p * RW_MAX_COMPONENTS + q] = r[q];
 }
 
 constexpr int kGenThreads = 256;   // 32 row-blocks of 8 points
@@ -30,9 +32,16 @@ constexpr int kGenKT = 128;        // recoil bins staged per CTA
 __global__ void __launch_bounds__(kGenThreads)
 k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pad,
         const double *__restrict__ What /*[12][n_T] of this period*/, int n_T, int KPAD, int64_t A_pitch,
+        const double *__restrict__ rate /*[P][4]*/, const uint8_t *__restrict__ comp8 /*[n_T] or NULL*/,
         double *__restrict__ A)
 {
     __shared__ __align__(16) double sW[kNumTerms][kGenKT];
+    __shared__ uint8_t sComp[kGenKT];
+    if (comp8)
+        for (int q = threadIdx.x; q < kGenKT; q += kGenThreads) {
+            const int i = blockIdx.y * kGenKT + q;
+            sComp[q] = (i < n_T) ? comp8[i] : 0;
+        }
     const int k0 = blockIdx.y * kGenKT;
     for (int q = threadIdx.x; q < kNumTerms * kGenKT; q += kGenThreads) {
         int b = q / kGenKT, kk = q - b * kGenKT;
@@ -48,6 +57,9 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
     const bool valid = row < Pc;
 #pragma unroll
     for (int b = 0; b < kNumTerms; ++b) c[b] = valid ? coef[(p0 + row) * kCoefStride + b] : 0.0;
+    double rt[RW_MAX_COMPONENTS];
+#pragma unroll
+    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) rt[q] = (valid && comp8) ? rate[(p0 + row) * RW_MAX_COMPONENTS + q] : 1.0;
     const int nkb = min(kGenKT, KPAD - k0) / 8;
     for (int kb = 0; kb < nkb; ++kb) {
         double v[8];
@@ -61,6 +73,13 @@ k_gen_A(const double *__restrict__ coef, int64_t p0, int64_t Pc, int64_t rows_pa
                 double2 w = w2[h];
                 v[2 * h] = fma(c[b], w.x, v[2 * h]);
                 v[2 * h + 1] = fma(c[b], w.y, v[2 * h + 1]);
+            }
+        }
+        if (comp8) {            // rate_k of Eq. (17): scale every bin by its component's rate
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk) {
+                const int cq = sComp[kb * 8 + kk];
+                v[kk] *= (cq == 0) ? rt[0] : (cq == 1) ? rt[1] : (cq == 2) ? rt[2] : rt[3];
             }
         }
         double2 *dst = reinterpret_cast<double2 *>(A + (mb * A_pitch + (size_t)(k0 / 8 + kb) * 64 + r * 8));
@@ -123,7 +142,7 @@ cudaError_t launch_coef(rw_ctx *ctx, const double *param, int64_t P, int k, cons
     Kinds kd;
     kd.k = k;
     for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
-    k_coef<<<(unsigned)((P + 127) / 128), 128, 0, s>>>(param, P, kd, ctx->cst, ctx->coef);
+    k_coef<<<(unsigned)((P + 127) / 128), 128, 0, s>>>(param, P, kd, ctx->cst, ctx->coef, ctx->rate);
     ctx->launches++;
     return cudaGetLastError();
 }
@@ -135,7 +154,7 @@ cudaError_t launch_gen_A(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, cudaStream_
               (unsigned)((ctx->lay.KPAD + kGenKT - 1) / kGenKT));
     k_gen_A<<<grid, kGenThreads, 0, s>>>(ctx->coef, p0, Pc, rows_pad,
                                          ctx->What + (size_t)d * kCoefStride * ctx->n_T, ctx->n_T,
-                                         ctx->lay.KPAD, ctx->lay.A_pitch, ctx->A_packed);
+                                         ctx->lay.KPAD, ctx->lay.A_pitch, ctx->rate, ctx->comp8, ctx->A_packed);
     ctx->launches++;
     return cudaGetLastError();
 }

@@ -117,6 +117,7 @@ k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const doubl
 cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s)
 {
     const Layout &L = ctx->lay;
+    if (ctx->n_comp > 1) return cudaSuccess;      // templates would be per component: collapsed mode is off
     k_identity<<<1, 256, 0, s>>>(ctx->ident);
     ctx->launches++;
     // the 11 templates are folded as 11 "points" with unit coefficient vectors (no deviance pass)

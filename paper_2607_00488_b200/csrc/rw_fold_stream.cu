@@ -25,6 +25,8 @@ struct StreamArgs {
     const double *coef;       // [Pb][12], or NULL
     const double *param;      // [Pb][k] raw parameters (coefficients computed here), or NULL
     const double *wts;        // [Pb][n_T] caller weights (rw_eval_weights), or NULL
+    const double *rate;       // [Pb][4] rate scales matching `coef` (ignored with `param`: computed here), or NULL
+    const uint8_t *comp8;     // [n_T] component of every recoil bin, or NULL (one component)
     const double *What, *N_mc, *bkg, *counts, *sat_const;
     int Pb, rows_per_split, n_splits, mu_ld;
     double *mu_part;          // [D][n_splits][PB][mu_ld]
@@ -40,6 +42,7 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
 {
     __shared__ __align__(16) double sN[kRC][PB];
     __shared__ double sC[PB][kCoefStride];
+    __shared__ double sRate[PB][RW_MAX_COMPONENTS];
     __shared__ double red[kStreamThreads / 32][PB];
     __shared__ int s_last;
     const int d = blockIdx.z, split = blockIdx.y, strip = blockIdx.x;
@@ -54,20 +57,28 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
     if (!wts) {
         if (A.param) {
             if (threadIdx.x < PB) {
-                double c[kCoefStride];
+                double c[kCoefStride], r[RW_MAX_COMPONENTS];
                 if (threadIdx.x < Pb) {
-                    coef_from_param(A.param + (size_t)threadIdx.x * kd.k, kd, cst, c);
+                    coef_from_param(A.param + (size_t)threadIdx.x * kd.k, kd, cst, c, r);
                 } else {
 #pragma unroll
                     for (int b = 0; b < kCoefStride; ++b) c[b] = 0.0;
+#pragma unroll
+                    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) r[q] = 1.0;
                 }
 #pragma unroll
                 for (int b = 0; b < kCoefStride; ++b) sC[threadIdx.x][b] = c[b];
+#pragma unroll
+                for (int q = 0; q < RW_MAX_COMPONENTS; ++q) sRate[threadIdx.x][q] = r[q];
             }
         } else {
             for (int q = threadIdx.x; q < PB * kCoefStride; q += kStreamThreads) {
                 int p = q / kCoefStride, b = q - p * kCoefStride;
                 sC[p][b] = (p < Pb) ? A.coef[(size_t)p * kCoefStride + b] : 0.0;
+            }
+            for (int q = threadIdx.x; q < PB * RW_MAX_COMPONENTS; q += kStreamThreads) {
+                int p = q / RW_MAX_COMPONENTS, cq = q - p * RW_MAX_COMPONENTS;
+                sRate[p][cq] = (p < Pb && A.rate) ? A.rate[(size_t)p * RW_MAX_COMPONENTS + cq] : 1.0;
             }
         }
     }
@@ -88,6 +99,7 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
                 } else {            // N' = sum_b c_b W^_b (Eq. 14 folded into the pre-scaled basis)
 #pragma unroll
                     for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p][b], Wd[(size_t)b * n_T + i], v);
+                    if (A.comp8) v *= sRate[p][A.comp8[i]];        // rate_k of Eq. (17)
                 }
             }
             sN[row][p] = v;
@@ -203,11 +215,17 @@ cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *pa
                                const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
                                cudaStream_t s)
 {
+    // `coef` is ctx->coef + 12 g0 for the group starting at point g0 (or the identity of the prefold, which is
+    // never run with several components): its rates are ctx->rate + 4 g0
+    const double *rate = nullptr;
+    if (coef && ctx->comp8 && coef >= ctx->coef && coef < ctx->coef + (size_t)ctx->lay.max_batch * kCoefStride)
+        rate = ctx->rate + (coef - ctx->coef) / kCoefStride * RW_MAX_COMPONENTS;
     const Layout &L = ctx->lay;
     StreamArgs A;
     A.R = ctx->R; A.R_period_stride = ctx->R_period_stride; A.ldR = ctx->ldR;
     A.n_T = ctx->n_T; A.n_rec = ctx->n_rec; A.D = ctx->D;
     A.coef = coef; A.param = param; A.wts = wts;
+    A.rate = rate; A.comp8 = ctx->comp8;
     A.What = ctx->What; A.N_mc = ctx->N_mc; A.bkg = ctx->bkg; A.counts = ctx->counts;
     A.sat_const = full_eq18 ? ctx->sat_const : nullptr;
     A.Pb = Pb;

@@ -136,10 +136,17 @@ k_split_R(const double *__restrict__ R, int ldR, int n_T, int n_rec, int KP, flo
 // [rows_pad][KP]; rows >= Pc and bins >= n_T are zero.  8 points x 256 bins per CTA, W^ staged in shared memory.
 __global__ void __launch_bounds__(256)
 k_gen_A32(const double *__restrict__ coef, int64_t p0, int64_t Pc, const double *__restrict__ What, int n_T,
-          int KP, float *__restrict__ hi, float *__restrict__ lo)
+          int KP, const double *__restrict__ rate, const uint8_t *__restrict__ comp8, float *__restrict__ hi,
+          float *__restrict__ lo)
 {
     __shared__ double sW[kNumTerms][256];
     __shared__ double sC[8][kCoefStride];
+    __shared__ double sRate[8][RW_MAX_COMPONENTS];
+    if (threadIdx.x < 8 * RW_MAX_COMPONENTS) {
+        const int r = threadIdx.x / RW_MAX_COMPONENTS, cq = threadIdx.x % RW_MAX_COMPONENTS;
+        const int64_t row = (int64_t)blockIdx.x * 8 + r;
+        sRate[r][cq] = (comp8 && row < Pc) ? rate[(p0 + row) * RW_MAX_COMPONENTS + cq] : 1.0;
+    }
     const int i0 = blockIdx.y * 256;
     const int64_t row0 = (int64_t)blockIdx.x * 8;
     for (int q = threadIdx.x; q < kNumTerms * 256; q += 256) {
@@ -153,11 +160,13 @@ k_gen_A32(const double *__restrict__ coef, int64_t p0, int64_t Pc, const double 
     __syncthreads();
     const int i = i0 + threadIdx.x;
     if (i >= KP) return;
+    const int cq = (comp8 && i < n_T) ? comp8[i] : 0;
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         double v = 0.0;
 #pragma unroll
         for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][threadIdx.x], v);
+        v *= sRate[r][cq];                                   // rate_k of Eq. (17); 1 with a single component
         float h, l;
         split_tf32(v, h, l);
         hi[(size_t)(row0 + r) * KP + i] = h;
@@ -389,7 +398,7 @@ cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double 
     const int64_t rows_pad = (Pc + 127) / 128 * 128;
     dim3 ggrid((unsigned)(rows_pad / 8), (unsigned)((KP + 255) / 256));
     k_gen_A32<<<ggrid, 256, 0, s>>>(ctx->coef, p0, Pc, ctx->What + (size_t)d * kCoefStride * ctx->n_T, ctx->n_T, KP,
-                                    a_hi, a_lo);
+                                    ctx->rate, ctx->comp8, a_hi, a_lo);
     ctx->launches++;
     F32Work W;
     W.n_T = ctx->n_T; W.n_rec = ctx->n_rec; W.D = ctx->D; W.d = d;

@@ -46,7 +46,7 @@ struct Kinds { int k; int kind[RW_N_KINDS]; };
 
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
-    size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part;
+    size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part, comp8, rate;
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof, R32;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
@@ -69,6 +69,9 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
 
 struct rw_ctx {
     int n_E, n_T, n_rec, D;
+    int n_comp;               // signal components (>= 1)
+    uint8_t *comp8;           // [n_T] component of every recoil bin (device); NULL when n_comp == 1
+    double *rate;             // [max_batch][4] per-point rate scales of the components (k_coef)
     rw::Consts cst;
     rw::Layout lay;
     char *ws;                 // device workspace base
@@ -115,6 +118,7 @@ int fail(rw_ctx *ctx, int status, const char *fmt, ...);
 // kernels' host launchers (each returns a cudaError_t from the launch) ---------------------------
 cudaError_t launch_setup(rw_ctx *ctx, cudaStream_t s);                       // rw_setup.cu
 cudaError_t launch_sat_const(rw_ctx *ctx, cudaStream_t s);                   // rw_setup.cu
+cudaError_t launch_comp8(rw_ctx *ctx, const int32_t *comp_dev, cudaStream_t s);   // rw_setup.cu
 cudaError_t launch_validate_device(rw_ctx *ctx, const double *R_src, int ld_src,
                                    size_t period_stride_src, cudaStream_t s); // rw_setup.cu
 cudaError_t launch_flavour(rw_ctx *ctx, int have_mu_tau, double f_tau, cudaStream_t s);  // rw_setup.cu
@@ -159,16 +163,24 @@ struct ProfScope {
 // Step a1 for one point: g~ = g + eps (Eq. 6), then the monomials the cross section is polynomial
 // in: g~L^2, g~R^2, g~L g~R per flavour (Eq. 4/7) and mu_nu^2 (Eq. 8-9).
 // c[10] = 1 multiplies the dead-bin row of W^, c[11] = 0 is padding.
+// r[c] = rate scale of signal component c (rate_k of Eq. 17; 1 when not scanned).
 __device__ __forceinline__ void coef_from_param(const double *__restrict__ prow, const Kinds &kd, const Consts &cst,
-                                                double *c /*[12]*/)
+                                                double *c /*[12]*/, double *r /*[4]*/)
 {
-    double th[RW_N_KINDS];
 #pragma unroll
-    for (int q = 0; q < RW_N_KINDS; ++q) th[q] = 0.0;
+    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) r[q] = 1.0;
+    for (int a = 0; a < kd.k; ++a) {
+#pragma unroll
+        for (int q = 0; q < RW_MAX_COMPONENTS; ++q)
+            if (kd.kind[a] == RW_RATE_0 + q) r[q] = prow[a];
+    }
+    double th[RW_RATE_0];
+#pragma unroll
+    for (int q = 0; q < RW_RATE_0; ++q) th[q] = 0.0;
     for (int a = 0; a < kd.k; ++a) {
         const double v = prow[a];
 #pragma unroll
-        for (int q = 0; q < RW_N_KINDS; ++q)
+        for (int q = 0; q < RW_RATE_0; ++q)
             if (kd.kind[a] == q) th[q] = v;
     }
 #pragma unroll

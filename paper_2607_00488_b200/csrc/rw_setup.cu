@@ -31,13 +31,15 @@ __global__ void k_energy_tables(int n_E, const double *__restrict__ E, double m_
 }
 
 // Flavour probabilities: row 0 = P_e; rows 1,2 = P_mu, P_tau or the f_tau split of 1 - P_e (R3).
+// Layout P3[n_comp][3][n_E]; blockIdx.y = component.
 __global__ void k_flavour(int n_E, double *__restrict__ P3, int have_mu_tau, double f_tau)
 {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_E || have_mu_tau) return;
-    double pe = P3[j];
-    P3[n_E + j] = (1.0 - pe) * (1.0 - f_tau);
-    P3[2 * n_E + j] = (1.0 - pe) * f_tau;
+    double *Pc = P3 + (size_t)blockIdx.y * 3 * n_E;
+    double pe = Pc[j];
+    Pc[n_E + j] = (1.0 - pe) * (1.0 - f_tau);
+    Pc[2 * n_E + j] = (1.0 - pe) * f_tau;
 }
 
 constexpr int kBasisThreads = 128;
@@ -46,9 +48,13 @@ constexpr int kBasisThreads = 128;
 __global__ void __launch_bounds__(kBasisThreads)
 k_basis(int n_E, const double *__restrict__ fw, const double *__restrict__ P3,
         const double *__restrict__ etab, int n_T, const double *__restrict__ T, double C0, double Cmm,
-        double *__restrict__ basis /*[10][n_T]*/)
+        const uint8_t *__restrict__ comp8 /*NULL: one component*/, double *__restrict__ basis /*[10][n_T]*/)
 {
     const int i = blockIdx.x;
+    if (comp8) {                  // the bin's own component: its flux table and flavour probabilities (Eq. 17)
+        fw += (size_t)comp8[i] * n_E;
+        P3 += (size_t)comp8[i] * 3 * n_E;
+    }
     const double Ti = T[i];
     const double invT = 1.0 / Ti;
     const double *Tmax = etab, *invE = etab + n_E, *meE2 = etab + 2 * n_E;
@@ -144,19 +150,17 @@ enum { F_E = 1, F_FW = 2, F_P = 4, F_T = 8, F_NMC = 16, F_BKG = 32, F_CNT = 64, 
 
 __device__ __forceinline__ bool bad_nonneg(double x) { return !(x >= 0.0) || isinf(x); }
 
-__global__ void k_validate_small(int n_E, const double *E, const double *fw, const double *P3, int n_T,
+__global__ void k_validate_small(int n_E, int n_comp, const double *E, const double *fw, const double *P3, int n_T,
                                  const double *T, int64_t nN, const double *N_mc, int64_t nB,
                                  const double *bkg, const double *counts, int *flag)
 {
     int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     int f = 0;
-    if (t < n_E) {
-        if (!(E[t] > 0.0) || isinf(E[t])) f |= F_E;
-        if (bad_nonneg(fw[t])) f |= F_FW;
-        for (int a = 0; a < 3; ++a) {
-            double p = P3[a * (int64_t)n_E + t];
-            if (!(p >= 0.0 && p <= 1.0)) f |= F_P;
-        }
+    if (t < n_E && (!(E[t] > 0.0) || isinf(E[t]))) f |= F_E;
+    if (t < (int64_t)n_comp * n_E && bad_nonneg(fw[t])) f |= F_FW;
+    if (t < (int64_t)n_comp * 3 * n_E) {
+        double p = P3[t];
+        if (!(p >= 0.0 && p <= 1.0)) f |= F_P;
     }
     if (t < n_T && (!(T[t] > 0.0) || isinf(T[t]))) f |= F_T;
     if (t < nN && bad_nonneg(N_mc[t])) f |= F_NMC;
@@ -191,12 +195,12 @@ cudaError_t launch_validate_device(rw_ctx *ctx, const double *R_src, int ld_src,
                                    size_t period_stride_src, cudaStream_t s)
 {
     int64_t nN = (int64_t)ctx->D * ctx->n_T, nB = (int64_t)ctx->D * ctx->n_rec;
-    int64_t m = ctx->n_E;
+    int64_t m = (int64_t)ctx->n_comp * 3 * ctx->n_E;
     if (ctx->n_T > m) m = ctx->n_T;
     if (nN > m) m = nN;
     if (nB > m) m = nB;
     k_validate_small<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(
-        ctx->n_E, ctx->E, ctx->fw, ctx->P3, ctx->n_T, ctx->T, nN, ctx->N_mc, nB, ctx->bkg, ctx->counts,
+        ctx->n_E, ctx->n_comp, ctx->E, ctx->fw, ctx->P3, ctx->n_T, ctx->T, nN, ctx->N_mc, nB, ctx->bkg, ctx->counts,
         ctx->flag);
     ctx->launches++;
     for (int d = 0; d < ctx->D; ++d) {
@@ -204,6 +208,23 @@ cudaError_t launch_validate_device(rw_ctx *ctx, const double *R_src, int ld_src,
                                                       ctx->n_rec, ld_src, ctx->flag);
         ctx->launches++;
     }
+    return cudaGetLastError();
+}
+
+// comp_of_T (int32, device) -> comp8, flagging indices outside [0, n_comp)
+__global__ void k_comp8(int n_T, int n_comp, const int32_t *__restrict__ comp, uint8_t *__restrict__ comp8, int *flag)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_T) return;
+    const int c = comp[i];
+    if (c < 0 || c >= n_comp) { atomicOr(flag, 256); comp8[i] = 0; }
+    else comp8[i] = (uint8_t)c;
+}
+
+cudaError_t launch_comp8(rw_ctx *ctx, const int32_t *comp_dev, cudaStream_t s)
+{
+    k_comp8<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->n_T, ctx->n_comp, comp_dev, ctx->comp8, ctx->flag);
+    ctx->launches++;
     return cudaGetLastError();
 }
 
@@ -221,7 +242,7 @@ cudaError_t launch_setup(rw_ctx *ctx, cudaStream_t s)
     const int n_E = ctx->n_E, n_T = ctx->n_T;
     k_energy_tables<<<(n_E + 255) / 256, 256, 0, s>>>(n_E, ctx->E, ctx->cst.m_e, ctx->Tmax_invE);
     k_basis<<<n_T, kBasisThreads, 0, s>>>(n_E, ctx->fw, ctx->P3, ctx->Tmax_invE, n_T, ctx->T,
-                                          ctx->cst.C0, ctx->cst.Cmm, ctx->basis);
+                                          ctx->cst.C0, ctx->cst.Cmm, ctx->comp8, ctx->basis);
     Coef0 c0;
     for (int a = 0; a < 3; ++a) {
         c0.c[3 * a + 0] = ctx->cst.gL[a] * ctx->cst.gL[a];
@@ -237,7 +258,7 @@ cudaError_t launch_setup(rw_ctx *ctx, cudaStream_t s)
 
 cudaError_t launch_flavour(rw_ctx *ctx, int have_mu_tau, double f_tau, cudaStream_t s)
 {
-    k_flavour<<<(ctx->n_E + 255) / 256, 256, 0, s>>>(ctx->n_E, ctx->P3, have_mu_tau, f_tau);
+    k_flavour<<<dim3((ctx->n_E + 255) / 256, ctx->n_comp), 256, 0, s>>>(ctx->n_E, ctx->P3, have_mu_tau, f_tau);
     ctx->launches++;
     return cudaGetLastError();
 }

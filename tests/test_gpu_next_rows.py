@@ -236,3 +236,52 @@ def test_profile_config2_all_points(rw, orc):
     a, _ = _profile_check(rw, orc, inp, params, kinds, "auto")
     b, _ = _profile_check(rw, orc, inp, params, kinds, "collapsed", s0=1.0, sigma=0.1)
     assert np.all(b >= a - 1e-9)
+
+
+# ------------------------------------------------------------------------------------- f-2 several signal components
+@pytest.mark.parametrize("mode,P", [("stream", 3), ("stream", 21), ("gemm", 40), ("gemm", 300), ("auto", 9)])
+def test_multi_component_rates(rw, orc, mode, P):
+    """Three signal components (own flux tables and survival probabilities, concatenated recoil bins), rate scales of
+    components 0 and 2 scanned together with couplings (Eq. 17) against orc.eval_components."""
+    import torch
+    inp = wl.make_components(n_comp=3, n_E=33, n_T=203, n_rec=330, n_periods=2, seed=71)
+    kinds = np.array([wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU, 7, 9], np.int32)
+    params, _ = wl.random_points(P, kinds, seed=72)
+    ref, mu_ref, scale = orc.eval_components(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=max(P, 16))
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode=mode)
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    with pytest.raises(rw.RwError):
+        ctx.eval_batch(_cuda(params), kinds, mode="collapsed")
+    with pytest.raises(rw.RwError):
+        ctx.eval_batch(_cuda(params[:, :1]), [10])               # rate of a component that does not exist
+    ctx.close()
+
+
+def test_multi_component_device_tables_profile_and_fp32(rw, orc):
+    """Device-resident multi-component tables; the profiled normalisation and the TF32 contraction on top."""
+    import torch
+    inp = wl.make_components(n_comp=2, n_E=29, n_T=160, n_rec=140, n_periods=1, seed=73)
+    kinds = np.array([wl.EPS_EE_R, 8], np.int32)
+    params, _ = wl.random_points(50, kinds, seed=74)
+    ref, mu_ref, scale = orc.eval_components(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    dev = {k: _cuda(inp[k]) for k in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
+    dev["comp_of_T"] = torch.from_numpy(inp["comp_of_T"]).cuda()
+    dev["f_tau"] = 0.5
+    ctx = rw.Reweighter(dev, max_batch=50, fp32=True)
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="gemm")
+    out32, mu32 = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="gemm", fp32=True)
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    assert (np.abs(mu32.cpu().numpy() - mu_ref) / mu_ref).max() <= 1e-5
+    # profiling the overall normalisation on top of fixed relative rates: minimum over s of the oracle's objective
+    prof, sc = ctx.eval_profile(_cuda(params[:6]), kinds)
+    torch.cuda.synchronize()
+    for p in range(6):
+        s_ref, f_ref = orc.profile_scale((mu_ref[p] - inp["bkg"]).ravel(), inp["bkg"].ravel(), inp["counts"].ravel())
+        assert abs(sc[p].item() - s_ref) <= 1e-10 * s_ref and abs(prof[p].item() - f_ref) <= 1e-9 + 1e-12 * scale[p]
+    bad = dict(inp, comp_of_T=np.where(np.arange(160) == 7, 5, inp["comp_of_T"]).astype(np.int32))
+    with pytest.raises(rw.RwError, match="comp_of_T"):
+        rw.Reweighter(bad, max_batch=4)
+    ctx.close()
