@@ -36,6 +36,8 @@
  *   orc_eval_components  n_comp = 1 reproduces orc_eval_batch; identical tables split over two components
  *                     reproduce it too; mu - bkg is linear in the per-component rates with the single-component
  *                     predictions as coefficients; a component's bins get the weights of its own flux table
+ *   orc_eval_grad     central finite differences (Richardson) of orc_eval_components in every parameter kind;
+ *                     zero gradient at an Asimov point; value output identical to orc_eval_components
  *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
  *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
@@ -534,6 +536,116 @@ int orc_eval_components(const orc_consts *c, int n_E, const double *E, int n_com
         free(S);
     }
     free(S0);
+    return 0;
+}
+
+/* Gradient of -2lnL with respect to the scanned parameters (for gradient-based minimisers; the paper fits
+ * Eq. 18 with MIGRAD).  Written from the derivatives of the definitions:
+ *   d/dgL of Eq. (4) bracket = 2 gL - gR m_e T/E^2,   d/dgR = 2 gR (1 - T/E)^2 - gL m_e T/E^2
+ *   d/dmu_nu of Eq. (8) = 2 mu_nu (pi alpha^2/m_e^2)(1/T - 1/E)
+ *   d mu_j = sum_i R_ij N_mc,i rate_c(i) dS_i/S_SM,i  (rate parameter: the component's own prediction / rate)
+ *   d(-2lnL)/dtheta = sum_j 2 (1 - n_j/mu_j) dmu_j/dtheta                        (Eq. 18; n_j = 0: 2 dmu_j)
+ * grad_out [P][k] in the order of `kinds`; out [P] as orc_eval_components. */
+static xreal xdspectrum_bin(const orc_consts *c, int n_E, const double *E, const double *flux_w, const double *P_e,
+                            const double *P_mu, const double *P_tau, double Ti, const double *theta, int kind)
+{
+    double gL0[3], gR0[3];
+    orc_sm_couplings(c, gL0, gR0);
+    const xreal pi = acosl(-1.0L);
+    const xreal pref = 2.0L * (xreal)c->G_F * (xreal)c->G_F * (xreal)c->m_e / pi;
+    const xreal pmm = pi * (xreal)c->alpha_em * (xreal)c->alpha_em / ((xreal)c->m_e * (xreal)c->m_e);
+    xreal acc = 0.0L;
+    for (int j = 0; j < n_E; ++j) {
+        if (!(Ti <= orc_tmax(E[j], c->m_e))) continue;
+        xreal Ej = E[j], T = Ti, d;
+        if (kind == ORC_MU_NU) {
+            d = 2.0L * (xreal)theta[ORC_MU_NU] * pmm * (1.0L / T - 1.0L / Ej);
+        } else {
+            const int fl = kind / 2;                       /* 0 e, 1 mu, 2 tau */
+            const double *Pf = fl == 0 ? P_e : (fl == 1 ? P_mu : P_tau);
+            xreal gL = (xreal)gL0[fl] + (xreal)theta[2 * fl], gR = (xreal)gR0[fl] + (xreal)theta[2 * fl + 1];
+            xreal one_m = 1.0L - T / Ej, x = (xreal)c->m_e * T / (Ej * Ej);
+            d = (kind % 2 == 0) ? (2.0L * gL - gR * x) : (2.0L * gR * one_m * one_m - gL * x);
+            d *= pref * (xreal)Pf[j];
+        }
+        acc += (xreal)flux_w[j] * d;
+    }
+    return acc;
+}
+
+int orc_eval_grad(const orc_consts *c, int n_E, const double *E, int n_comp, const double *flux_w,
+                  const double *P_e, const double *P_mu, const double *P_tau,
+                  int n_T, const double *T, const int32_t *comp_of_T, int n_rec, int n_periods,
+                  const double *N_mc, const double *R, const double *bkg, const double *counts,
+                  int64_t P, int k, const int32_t *kinds, const double *params,
+                  double *out, double *grad_out, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    if (n_comp < 1 || n_comp > 4) return -1;
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS + n_comp) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    size_t nT = (size_t)(n_T > 0 ? n_T : 1);
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * nT * 2), *tmp0 = S0 + nT;
+    for (int q = 0; q < n_comp; ++q) {
+        xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E, P_mu + (size_t)q * n_E,
+                  P_tau + (size_t)q * n_E, n_T, T, zero, tmp0);
+        for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S0[i] = tmp0[i];
+    }
+    double *zero_bkg = (double *)calloc((size_t)(n_rec > 0 ? n_rec : 1), sizeof(double));
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        double rate[4] = {1.0, 1.0, 1.0, 1.0};
+        for (int a = 0; a < k; ++a) {
+            if (kinds[a] < ORC_N_KINDS) theta[kinds[a]] = params[p * k + a];
+            else rate[kinds[a] - ORC_N_KINDS] = params[p * k + a];
+        }
+        xreal *S = (xreal *)malloc(sizeof(xreal) * (4 * nT + 2 * (size_t)n_rec * (size_t)n_periods + 2));
+        xreal *tmp = S + nT, *w = tmp + nT, *dw = w + nT, *mu = dw + nT, *dmu = mu + (size_t)n_rec * n_periods;
+        for (int q = 0; q < n_comp; ++q) {
+            xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E, P_mu + (size_t)q * n_E,
+                      P_tau + (size_t)q * n_E, n_T, T, theta, tmp);
+            for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S[i] = tmp[i];
+        }
+        xweights(n_T, S, S0, w);                           /* unscaled weights S_theta/S_SM (1 in dead bins) */
+        for (int i = 0; i < n_T; ++i) tmp[i] = w[i] * (xreal)rate[comp_of_T[i]];
+        xreal total = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            xfold(n_T, n_rec, tmp, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, bkg + (size_t)d * n_rec,
+                  mu + (size_t)d * n_rec);
+            total += xdeviance(n_rec, mu + (size_t)d * n_rec, counts + (size_t)d * n_rec);
+        }
+        out[p] = (double)total;
+        for (int a = 0; a < k; ++a) {
+            for (int i = 0; i < n_T; ++i) {
+                const int q = comp_of_T[i];
+                if (kinds[a] >= ORC_N_KINDS) {             /* rate of one component: its own unscaled content */
+                    dw[i] = (q == kinds[a] - ORC_N_KINDS) ? w[i] : 0.0L;
+                } else if (S0[i] == 0.0L) {
+                    dw[i] = 0.0L;                          /* dead bin: w = 1 for every theta */
+                } else {
+                    dw[i] = (xreal)rate[q] * xdspectrum_bin(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E,
+                                                            P_mu + (size_t)q * n_E, P_tau + (size_t)q * n_E, T[i],
+                                                            theta, kinds[a]) / S0[i];
+                }
+            }
+            xreal g = 0.0L;
+            for (int d = 0; d < n_periods; ++d) {
+                xfold(n_T, n_rec, dw, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, zero_bkg, dmu);
+                for (int j = 0; j < n_rec; ++j) {
+                    xreal m = mu[(size_t)d * n_rec + j], n = counts[(size_t)d * n_rec + j];
+                    g += 2.0L * (n > 0.0L ? (1.0L - n / m) : 1.0L) * dmu[j];
+                }
+            }
+            grad_out[p * k + a] = (double)g;
+        }
+        free(S);
+    }
+    free(S0);
+    free(zero_bkg);
     return 0;
 }
 

@@ -326,3 +326,42 @@ def eval_components(inp, params, kinds, want_mu=False, want_abs=False, full_eq18
     if want_abs:
         res.append(ab)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def eval_grad(inp, params, kinds, nthreads=1, consts=None):
+    """(-2lnL[P], d(-2lnL)/dtheta [P][k]) for the (multi-)component path; inputs as eval_components
+    (a single component may pass 1-D flux_w / P_e and no comp_of_T)."""
+    c = consts or default_consts()
+    E, T = _a(inp["E"]), _a(inp["T"])
+    fw = np.atleast_2d(_a(inp["flux_w"]))
+    n_comp, n_E = fw.shape
+    P_e = np.atleast_2d(_a(inp["P_e"]))
+    if inp.get("P_mu") is not None and inp.get("P_tau") is not None:
+        P_mu, P_tau = np.atleast_2d(_a(inp["P_mu"])), np.atleast_2d(_a(inp["P_tau"]))
+    else:
+        f_tau = inp.get("f_tau", 0.5)
+        P_mu, P_tau = _a((1.0 - P_e) * (1.0 - f_tau)), _a((1.0 - P_e) * f_tau)
+    comp = np.ascontiguousarray(inp.get("comp_of_T", np.zeros(T.size)), dtype=np.int32)
+    R = _a(inp["R"])
+    if R.ndim == 2:
+        R = R[None]
+    D, n_T, n_rec = R.shape
+    N_mc = _a(inp["N_mc"]).reshape(D, n_T)
+    bkg = _a(inp["bkg"]).reshape(D, n_rec)
+    counts = _a(inp["counts"]).reshape(D, n_rec)
+    params = _a(params)
+    if params.ndim == 1:
+        params = params[:, None]
+    P, k = params.shape
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    out, grad = np.empty(P), np.empty((P, k))
+    L = lib()
+    L.orc_eval_grad.restype = C.c_int
+    rc = L.orc_eval_grad(
+        C.byref(c), C.c_int(n_E), _p(E), C.c_int(n_comp), _p(fw), _p(P_e), _p(P_mu), _p(P_tau),
+        C.c_int(n_T), _p(T), comp.ctypes.data_as(C.POINTER(C.c_int32)), C.c_int(n_rec), C.c_int(D),
+        _p(N_mc), _p(R), _p(bkg), _p(counts), C.c_int64(P), C.c_int(k),
+        kinds.ctypes.data_as(C.POINTER(C.c_int32)), _p(params), _p(out), _p(grad), C.c_int(int(nthreads)))
+    if rc != 0:
+        raise ValueError("orc_eval_grad: invalid kinds / component indices")
+    return out, grad
