@@ -180,6 +180,15 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
                     double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,
                     void *cuda_stream);
 
+/* rw_eval_grad: -2lnL and its gradient with respect to the k scanned parameters, for gradient-based minimisers
+ * (the paper minimises Eq. 18 with MIGRAD).  The path is linear in the coefficient vector of
+ * Eq. (4)/(8) and in the rates of Eq. (17), so d mu / d theta_m is the same fold applied to derivative coefficients;
+ *     out_grad[p][m] = sum over bins and periods of 2 (1 - n/mu) d mu / d theta_m      (n = 0: 2 d mu / d theta_m).
+ * A point costs 1 + k rows of the batched fold.  DEVICE pointers only; flags: RW_FULL_EQ18 (value only) and the
+ * fold modes; max_batch must be >= 1 + k.  Asynchronous and stream-ordered; P may exceed max_batch. */
+int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                 double *out_m2lnL, double *out_grad /*[P][k]*/, uint32_t flags, void *cuda_stream);
+
 /* Device pointers to setup tables, for inspection/tests (valid until rw_destroy):
  *   RW_TABLE_S_SM   [n_T]        SM recoil spectrum S_SM(T_i) (Eq. 12 at theta = 0)
  *   RW_TABLE_BASIS  [10][n_T]    basis spectra A_e,B_e,C_e,A_mu,...,C_tau,D

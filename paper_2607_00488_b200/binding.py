@@ -26,7 +26,7 @@ RW_CREATE_FP32 = 1
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
-EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_get_table",
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
            "rw_last_error", "rw_probe_fp64_peak")
 
@@ -76,6 +76,9 @@ def load_library():
     L.rw_eval_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_double,
                                   C.c_double, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     L.rw_eval_profile.restype = C.c_int
+    L.rw_eval_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_void_p,
+                               C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_grad.restype = C.c_int
     L.rw_get_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
     L.rw_launch_count.argtypes = [C.c_void_p]
     L.rw_launch_count.restype = C.c_int64
@@ -257,6 +260,25 @@ class Reweighter:
         self._check(rc, self._ctx)
         self._last_param = param
         return out, scale
+
+    def eval_grad(self, param, kinds, full_eq18=False, mode="auto"):
+        """(-2lnL[P], gradient[P][k]) for CUDA param[P][k] (rw_eval_grad)."""
+        if not (isinstance(param, torch.Tensor) and param.is_cuda):
+            raise RwError(-4, "eval_grad needs a CUDA tensor param[P][k]")
+        param = param.to(torch.float64).contiguous()
+        if param.ndim == 1:
+            param = param[:, None]
+        P, k = param.shape
+        assert k == len(kinds)
+        kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
+        out = torch.empty(P, dtype=torch.float64, device=self.device)
+        grad = torch.empty((P, k), dtype=torch.float64, device=self.device)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        rc = self._L.rw_eval_grad(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr,
+                                  C.c_void_p(out.data_ptr()), C.c_void_p(grad.data_ptr()), flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = param
+        return out, grad
 
     def eval_weights(self, w, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
         """-2lnL[P] for caller-supplied weights w[P][n_T] (CUDA float64 tensor): the dense fold on arbitrary

@@ -68,7 +68,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->E = take(n_E * 8);
     L->fw = take(n_comp * n_E * 8);
     L->P3 = take(n_comp * 3 * n_E * 8);
-    L->comp8 = take(n_comp > 1 ? n_T : 0);
+    L->comp8 = take(n_T);
     L->rate = take((size_t)max_batch * RW_MAX_COMPONENTS * 8);
     L->T = take(n_T * 8);
     L->Tmax_invE = take(3 * n_E * 8);
@@ -296,7 +296,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     char *ws = ctx->ws;
     ctx->E = (double *)(ws + L.E);          ctx->fw = (double *)(ws + L.fw);
     ctx->P3 = (double *)(ws + L.P3);        ctx->T = (double *)(ws + L.T);
-    ctx->comp8 = n_comp > 1 ? (uint8_t *)(ws + L.comp8) : nullptr;
+    ctx->comp8 = (uint8_t *)(ws + L.comp8);       // all zero with a single component
     ctx->rate = (double *)(ws + L.rate);
     ctx->Tmax_invE = (double *)(ws + L.Tmax_invE);
     ctx->N_mc = (double *)(ws + L.N_mc);    ctx->bkg = (double *)(ws + L.bkg);
@@ -340,6 +340,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         }
     }
     uint8_t *comp_host = nullptr;                              // host staging of comp_of_T, freed after the sync
+    if (n_comp == 1) RW_TRY(cudaMemsetAsync(ctx->comp8, 0, n_T, s));
     if (n_comp > 1) {
         RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
         if (host) {
@@ -497,6 +498,39 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
         if (rc != RW_OK) return rc;
         RW_CUDA(ctx, launch_profile(ctx, ctx->mu_prof, Pq, s0, sigma, full, out_m2lnL + q0,
                                     out_scale ? out_scale + q0 : nullptr, s));
+    }
+    return RW_OK;
+}
+
+int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                 double *out_m2lnL, double *out_grad, uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_grad: ctx is NULL");
+    if (P < 0 || k < 1 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_grad: P < 0 or k outside [1,11]");
+    if (P == 0) return RW_OK;
+    if (!out_m2lnL || !out_grad || !param || !param_kind)
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_grad: param, param_kind, out_m2lnL or out_grad is NULL");
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers and RW_FP32 are not supported");
+    int kinds[RW_N_KINDS];
+    { int rc = check_kinds(ctx, "rw_eval_grad", k, param_kind, kinds); if (rc != RW_OK) return rc; }
+    const uint32_t mode = flags & RW_MODE_MASK;
+    if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: RW_MODE_COLLAPSED needs a single signal component");
+    const bool full = flags & RW_FULL_EQ18;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Layout &L = ctx->lay;
+    // a point is 1 + k rows of the ordinary fold (value row + one derivative row per parameter)
+    int64_t per_pass = L.prof_rows / (1 + k);
+    if (per_pass < 1)
+        return fail(ctx, RW_ERR_WORKSPACE, "rw_eval_grad: max_batch (%lld) is smaller than 1 + k = %d rows",
+                    (long long)L.max_batch, 1 + k);
+    for (int64_t q0 = 0; q0 < P; q0 += per_pass) {
+        const int64_t Pq = (P - q0 < per_pass) ? P - q0 : per_pass;
+        RW_CUDA(ctx, launch_coef_grad(ctx, param + q0 * k, Pq, k, kinds, s));
+        int rc = fold_slice(ctx, Pq * (1 + k), mode, false, ctx->out_stage, ctx->mu_prof, s);
+        if (rc != RW_OK) return rc;
+        RW_CUDA(ctx, launch_grad(ctx, ctx->mu_prof, Pq, k, full, out_m2lnL + q0, out_grad + q0 * k, s));
     }
     return RW_OK;
 }

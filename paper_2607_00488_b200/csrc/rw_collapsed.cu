@@ -40,7 +40,7 @@ __global__ void k_identity(double *__restrict__ ident /*[16][12]*/)
 // shared-memory pass over the 8 warps.  partial[(d * nstrip + strip)][p] feeds k_reduce (fixed order).
 __global__ void __launch_bounds__(kColThreads)
 k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const double *__restrict__ coef,
-            int64_t Pc, const double *__restrict__ bkg, const double *__restrict__ counts,
+            const double *__restrict__ rate /*[.][4]: rate[.][0] scales the single component*/, int64_t Pc, const double *__restrict__ bkg, const double *__restrict__ counts,
             double *__restrict__ partial, int64_t part_stride, double *__restrict__ out_mu)
 {
     __shared__ double sC[kColPB][kCoefStride];
@@ -53,7 +53,8 @@ k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const doubl
 
     for (int q = threadIdx.x; q < kColPB * kCoefStride; q += kColThreads) {
         const int p = q / kCoefStride, b = q - p * kCoefStride;
-        sC[p][b] = (p < np) ? coef[(p0 + p) * kCoefStride + b] : 0.0;
+        // slot 11 of the coefficient row is padding: it carries the point's rate scale here
+        sC[p][b] = (p < np) ? (b == kCoefStride - 1 ? rate[(p0 + p) * RW_MAX_COMPONENTS] : coef[(p0 + p) * kCoefStride + b]) : 0.0;
     }
     double g[kNumTerms][2], bk[2], cn[2], ci[2];
     const bool ok0 = col < n_rec, ok1 = col + 1 < n_rec;
@@ -89,7 +90,8 @@ k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const doubl
         double t[2];
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
-            const double m0 = m[u][0] + bk[0], m1 = m[u][1] + bk[1];
+            const double rt = sC[p + u][kCoefStride - 1];             // rate_k of Eq. (17), 1 when not scanned
+            const double m0 = fma(rt, m[u][0], bk[0]), m1 = fma(rt, m[u][1], bk[1]);
             if (out_mu && p + u < np) {
                 double *dst = out_mu + ((size_t)(p0 + p + u) * D + d) * n_rec + col;
                 if (ok0) dst[0] = m0;
@@ -138,7 +140,8 @@ cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu
     const int nstrip = (ctx->n_rec + kColCols - 1) / kColCols;
     dim3 grid(nstrip, (unsigned)((Pc + kColPB - 1) / kColPB), ctx->D);
     ProfScope prof(ctx, s);
-    k_collapsed<<<grid, kColThreads, 0, s>>>(ctx->G, L.ldG, ctx->n_rec, ctx->D, ctx->coef + p0 * kCoefStride, Pc,
+    k_collapsed<<<grid, kColThreads, 0, s>>>(ctx->G, L.ldG, ctx->n_rec, ctx->D, ctx->coef + p0 * kCoefStride,
+                                             ctx->rate + p0 * RW_MAX_COMPONENTS, Pc,
                                              ctx->bkg, ctx->counts, ctx->partial, L.MC, out_mu);
     ctx->launches++;
     return cudaGetLastError();

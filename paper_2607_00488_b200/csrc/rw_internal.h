@@ -70,7 +70,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
 struct rw_ctx {
     int n_E, n_T, n_rec, D;
     int n_comp;               // signal components (>= 1)
-    uint8_t *comp8;           // [n_T] component of every recoil bin (device); NULL when n_comp == 1
+    uint8_t *comp8;           // [n_T] component of every recoil bin (device); all zero when n_comp == 1
     double *rate;             // [max_batch][4] per-point rate scales of the components (k_coef)
     rw::Consts cst;
     rw::Layout lay;
@@ -137,6 +137,10 @@ cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // 
 cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, double s0, double sigma,
                            bool full_eq18, double *out, double *out_scale, cudaStream_t s);   // rw_profile.cu
 int profile_setup(rw_ctx *ctx);                                              // rw_profile.cu
+cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
+                             cudaStream_t s);                                // rw_grad.cu
+cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,
+                        double *grad, cudaStream_t s);                       // rw_grad.cu
 int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
 cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,

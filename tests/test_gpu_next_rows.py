@@ -285,3 +285,43 @@ def test_multi_component_device_tables_profile_and_fp32(rw, orc):
     with pytest.raises(rw.RwError, match="comp_of_T"):
         rw.Reweighter(bad, max_batch=4)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------- f-2 analytic gradient
+def _grad_check(rw, orc, inp, params, kinds, mode, max_batch):
+    import torch
+    ref, gref = orc.eval_grad(inp, params, kinds, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=max_batch)
+    out, grad = ctx.eval_grad(_cuda(params), kinds, mode=mode)
+    torch.cuda.synchronize()
+    out, grad = out.cpu().numpy(), grad.cpu().numpy()
+    ctx.close()
+    assert np.all(np.abs(out - ref) <= 1e-9 + 1e-11 * np.abs(ref))
+    # the derivative rows come back as (d mu + bkg) - bkg: absolute rounding of the background scale per bin
+    floor = 1e-11 * np.asarray(inp["bkg"]).sum()
+    assert np.all(np.abs(grad - gref) <= 1e-10 * np.abs(gref) + floor), np.abs(grad - gref).max()
+    return out, grad
+
+
+@pytest.mark.parametrize("mode", ["stream", "gemm", "collapsed"])
+def test_gradient_single_component(rw, orc, mode):
+    inp = wl.make_custom(n_E=31, n_T=203, n_rec=130, n_periods=2, seed=91, dead_fraction=0.1)
+    kinds = np.array([0, 1, 4, 5, 6, 7], np.int32)                # couplings, mu_nu and the rate of the component
+    params, _ = wl.random_points(23, kinds, seed=92)
+    _grad_check(rw, orc, inp, params, kinds, mode, max_batch=64)
+
+
+def test_gradient_multi_component_and_asimov_zero(rw, orc):
+    import torch
+    inp = wl.make_components(n_comp=3, n_E=27, n_T=120, n_rec=90, n_periods=1, seed=93)
+    kinds = np.array([0, 2, 3, 6, 7, 8, 9], np.int32)
+    params, _ = wl.random_points(40, kinds, seed=94)
+    _grad_check(rw, orc, inp, params, kinds, "auto", max_batch=300)
+    _, mu = orc.eval_components(inp, params[:1], kinds, want_mu=True)
+    asim = dict(inp, counts=mu[0])
+    ctx = rw.Reweighter(asim, max_batch=16)
+    out, grad = ctx.eval_grad(_cuda(params[:1]), kinds)
+    torch.cuda.synchronize()
+    scale = np.abs(orc.eval_grad(inp, params[:1], kinds)[1])
+    assert abs(out.item()) < 1e-9 and np.all(np.abs(grad.cpu().numpy()) <= 1e-9 * scale)
+    ctx.close()
