@@ -175,6 +175,20 @@ k_gen_A32(const double *__restrict__ coef, int64_t p0, int64_t Pc, const double 
 }
 
 // ---------------------------------------------------------------------------------------------- the contraction
+// Raster: groups of 8 m-tiles sweep n, so a wave of 148 CTAs shares 8 N' panels and ~19 R panels in L2 (with
+// m fastest over the whole grid every n-tile re-streams all of N' from HBM: 290 GB per launch at config-4 size,
+// HBM-bound at 5.5 TB/s -- ncu, round 1).
+__device__ __forceinline__ void f32_tile_coord(int t, int tiles_m, int tiles_n, int &tm, int &tn)
+{
+    constexpr int GM = 8;
+    const int per_group = GM * tiles_n;
+    const int g = t / per_group, rem = t - g * per_group;
+    const int first_m = g * GM;
+    const int gm = min(GM, tiles_m - first_m);
+    tm = first_m + rem % gm;
+    tn = rem / gm;
+}
+
 struct F32Work {
     int n_T, n_rec, tiles_m, tiles_n, D, d;
     int64_t Pc, part_stride;
@@ -220,7 +234,8 @@ k_fold_tf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant__ 
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-                const int tm = t % W.tiles_m, tn = t / W.tiles_m;
+                int tm, tn;
+                f32_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
                 for (int ks = 0; ks < k_stages; ++ks) {
                     f32_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
                     const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kF32StageBytes;
@@ -277,7 +292,8 @@ k_fold_tf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant__ 
         const int et = threadIdx.x - 64;                         // 0..127
         uint32_t cseq = 0;
         for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-            const int tm = t % W.tiles_m, tn = t / W.tiles_m;
+            int tm, tn;
+            f32_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
             {   // per-tile column constants; columns >= n_rec get bkg = n = 1/n = 0 (their mu is 0: term 0)
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 const int col = tn * 128 + et;
