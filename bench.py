@@ -270,9 +270,32 @@ def main():
     torch.cuda.synchronize()
     single_ms = e0.elapsed_time(e1) / reps
     sfold_ms, sfold_n = ctx.profile_end()
+    # the same single evaluation replayed from a CUDA graph: device-side latency without the Python/ctypes call
+    graph_us = None
+    try:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            ctx.eval_batch(one, kinds, out=out1, mode="stream")
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            ctx.eval_batch(one, kinds, out=out1, mode="stream")
+        for _ in range(5):
+            g.replay()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        graph_us = e0.elapsed_time(e1) / reps * 1e3
+    except Exception as exc:                                  # capture is a convenience, not part of the metric
+        graph_us = "unavailable: %s" % exc
     peaks = load_peaks()
     r_bytes = D * n_T * n_rec * 8
-    single = {"ms_per_eval": single_ms, "fold_kernel_ms": sfold_ms / max(1, sfold_n),
+    single = {"ms_per_eval": single_ms, "graph_replay_us_per_eval": graph_us, "fold_kernel_ms": sfold_ms / max(1, sfold_n),
               "hbm_gbs": r_bytes / (sfold_ms / max(1, sfold_n) * 1e-3) / 1e9,
               "hbm_peak_gbs": peaks["hbm_gbs"]}
     if r_bytes > 252e6:

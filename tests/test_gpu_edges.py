@@ -204,3 +204,32 @@ def test_symmetries_hold_on_the_gpu(rw, orc):
         out = ctx.eval_batch(_cuda(a), [0, 1, 6], mode=mode).cpu().numpy()
         assert abs(out[0] - out[1]) <= 1e-9 + 1e-12 * abs(out[0])
     ctx.close()
+
+
+def test_eval_batch_is_cuda_graph_capturable(rw, orc):
+    """rw_eval_batch only enqueues work (no allocation, no synchronisation): a minimiser loop can capture it in a
+    CUDA graph and replay it with new parameters written into the same device buffer."""
+    import torch
+    inp = wl.make("cfg1_tiny_nsi")
+    params, kinds = wl.scan_points("cfg1_tiny_nsi")
+    ref = orc.eval_batch(inp, params, kinds, nthreads=4)
+    ctx = rw.Reweighter(inp, max_batch=121)
+    for P, mode in ((1, "auto"), (121, "auto"), (121, "collapsed")):
+        buf = _cuda(params[:P].copy())
+        out = torch.empty(P, dtype=torch.float64, device="cuda")
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            ctx.eval_batch(buf, kinds, out=out, mode=mode)          # warm-up outside capture
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            ctx.eval_batch(buf, kinds, out=out, mode=mode)
+        for lo in (0, 60):                                           # replay with other points in the same buffer
+            sel = np.arange(lo, lo + P) % 121
+            buf.copy_(_cuda(params[sel]))
+            g.replay()
+            torch.cuda.synchronize()
+            assert np.all(np.abs(out.cpu().numpy() - ref[sel]) <= 1e-9), (P, mode)
+    ctx.close()
