@@ -38,6 +38,9 @@
  *                     predictions as coefficients; a component's bins get the weights of its own flux table
  *   orc_eval_grad     central finite differences (Richardson) of orc_eval_components in every parameter kind;
  *                     zero gradient at an Asimov point; value output identical to orc_eval_components
+ *   orc_eval_pee      reference P_ee for every point reproduces orc_eval_batch; equals orc_eval_weights fed
+ *                     the spectrum ratio computed with orc_spectrum on the point's table; P_ee = 1 / 0 on a
+ *                     single line give the pure nu_e / nu_mu,tau cross-section ratio of Eq. (4)
  *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
  *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
@@ -646,6 +649,60 @@ int orc_eval_grad(const orc_consts *c, int n_E, const double *E, int n_comp, con
     }
     free(S0);
     free(zero_bkg);
+    return 0;
+}
+
+/* Per-point survival probabilities (the "physics update" of PAPER.md:220 evaluates the oscillation
+ * probabilities for every parameter vector; here they arrive as a table P_e_pts[p][.] per point).  The MC sample
+ * and the SM reference stay those of the nominal table P_e (the denominator is computed once), so
+ *     w_i(p) = S_theta(T_i; P_e_pts[p]) / S_SM(T_i; P_e)          (Eq. 12 / Eq. 14; reading R16)
+ * with P_mu, P_tau = (1 - P_e)(1 - f_tau), (1 - P_e) f_tau for the point's and the nominal table alike.  These
+ * weights are not a low-rank function of theta: the dense fold is required.  Single component. */
+int orc_eval_pee(const orc_consts *c, int n_E, const double *E, const double *flux_w, const double *P_e,
+                 double f_tau, int n_T, const double *T, int n_rec, int n_periods,
+                 const double *N_mc, const double *R, const double *bkg, const double *counts,
+                 int64_t P, int k, const int32_t *kinds, const double *params, const double *P_e_pts,
+                 double *out, double *mu_out, double *abs_out, int full_eq18, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    size_t nE = (size_t)(n_E > 0 ? n_E : 1);
+    double *Pm0 = (double *)malloc(sizeof(double) * 2 * nE), *Pt0 = Pm0 + nE;
+    for (int j = 0; j < n_E; ++j) { Pm0[j] = (1.0 - P_e[j]) * (1.0 - f_tau); Pt0[j] = (1.0 - P_e[j]) * f_tau; }
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * (size_t)(n_T > 0 ? n_T : 1));
+    xspectrum(c, n_E, E, flux_w, P_e, Pm0, Pt0, n_T, T, zero, S0);
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        for (int a = 0; a < k; ++a) theta[kinds[a]] = params[p * k + a];
+        const double *Pp = P_e_pts + (size_t)p * n_E;
+        double *Pm = (double *)malloc(sizeof(double) * 2 * nE), *Pt = Pm + nE;
+        for (int j = 0; j < n_E; ++j) { Pm[j] = (1.0 - Pp[j]) * (1.0 - f_tau); Pt[j] = (1.0 - Pp[j]) * f_tau; }
+        xreal *S = (xreal *)malloc(sizeof(xreal) * (size_t)(2 * n_T + n_rec + 1));
+        xreal *w = S + n_T, *mu = w + n_T;
+        xspectrum(c, n_E, E, flux_w, Pp, Pm, Pt, n_T, T, theta, S);
+        xweights(n_T, S, S0, w);
+        xreal total = 0.0L, total_abs = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            const double *Cd = counts + (size_t)d * n_rec;
+            xfold(n_T, n_rec, w, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, bkg + (size_t)d * n_rec, mu);
+            total += full_eq18 ? xeq18(n_rec, mu, Cd) : xdeviance(n_rec, mu, Cd);
+            if (mu_out)
+                for (int q = 0; q < n_rec; ++q) mu_out[((size_t)p * n_periods + d) * n_rec + q] = (double)mu[q];
+            if (abs_out)
+                for (int q = 0; q < n_rec; ++q) total_abs += fabsl(xdeviance(1, mu + q, Cd + q));
+        }
+        out[p] = (double)total;
+        if (abs_out) abs_out[p] = (double)total_abs;
+        free(S);
+        free(Pm);
+    }
+    free(S0);
+    free(Pm0);
     return 0;
 }
 

@@ -365,3 +365,42 @@ def eval_grad(inp, params, kinds, nthreads=1, consts=None):
     if rc != 0:
         raise ValueError("orc_eval_grad: invalid kinds / component indices")
     return out, grad
+
+
+def eval_pee(inp, params, kinds, P_e_pts, want_mu=False, want_abs=False, full_eq18=False, nthreads=1, consts=None):
+    """Whole path with a survival-probability table per point, P_e_pts[P][n_E]; the SM reference keeps inp["P_e"]."""
+    c = consts or default_consts()
+    E, fw, T, P_e = _a(inp["E"]), _a(inp["flux_w"]), _a(inp["T"]), _a(inp["P_e"])
+    R = _a(inp["R"])
+    if R.ndim == 2:
+        R = R[None]
+    D, n_T, n_rec = R.shape
+    N_mc = _a(inp["N_mc"]).reshape(D, n_T)
+    bkg = _a(inp["bkg"]).reshape(D, n_rec)
+    counts = _a(inp["counts"]).reshape(D, n_rec)
+    params = _a(params)
+    if params.ndim == 1:
+        params = params[:, None]
+    P, k = params.shape
+    Pp = _a(P_e_pts)
+    assert Pp.shape == (P, E.size)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    out = np.empty(P)
+    mu = np.empty((P, D, n_rec)) if want_mu else None
+    ab = np.empty(P) if want_abs else None
+    L = lib()
+    L.orc_eval_pee.restype = C.c_int
+    rc = L.orc_eval_pee(
+        C.byref(c), C.c_int(E.size), _p(E), _p(fw), _p(P_e), C.c_double(inp.get("f_tau", 0.5)),
+        C.c_int(n_T), _p(T), C.c_int(n_rec), C.c_int(D), _p(N_mc), _p(R), _p(bkg), _p(counts),
+        C.c_int64(P), C.c_int(k), kinds.ctypes.data_as(C.POINTER(C.c_int32)), _p(params), _p(Pp),
+        _p(out), _p(mu) if want_mu else None, _p(ab) if want_abs else None,
+        C.c_int(1 if full_eq18 else 0), C.c_int(int(nthreads)))
+    if rc != 0:
+        raise ValueError("orc_eval_pee: invalid param kinds")
+    res = [out]
+    if want_mu:
+        res.append(mu)
+    if want_abs:
+        res.append(ab)
+    return res[0] if len(res) == 1 else tuple(res)

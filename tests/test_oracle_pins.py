@@ -501,6 +501,38 @@ def test_eval_grad_pins(orc):
     assert abs(out0[0]) < 1e-9 and np.all(np.abs(g0) <= 1e-10 * scale)
 
 
+def test_eval_pee_pins(orc):
+    """Per-point survival probabilities: (i) the nominal table for every point = eval_batch; (ii) = eval_weights fed
+    spectrum(point's table, theta) / spectrum(nominal table, 0), both from orc.spectrum; (iii) on a single line,
+    P_ee = 1 and P_ee = 0 give the pure nu_e and nu_mu,tau cross sections of Eq. (4) over the nominal mixture."""
+    inp = _small_problem(D=2)
+    params, kinds = wl.random_points(4, [orc.EPS_EE_L, orc.EPS_TT_R, orc.MU_NU], seed=51)
+    n_E = inp["E"].size
+    ref, mu_ref = orc.eval_batch(inp, params, kinds, want_mu=True)
+    out, mu = orc.eval_pee(inp, params, kinds, np.tile(inp["P_e"], (4, 1)), want_mu=True)
+    assert np.array_equal(out, ref) and np.array_equal(mu, mu_ref)
+    rng = np.random.default_rng(52)
+    Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.2, 0.2, size=(4, n_E)), 0.0, 1.0)
+    out, mu = orc.eval_pee(inp, params, kinds, Pp, want_mu=True, nthreads=2)
+    S0 = orc.spectrum(inp, np.zeros(7))
+    live = S0 > 0                                                    # dead bins keep w = 1 (reading R9)
+    w = np.stack([np.where(live, orc.spectrum(dict(inp, P_e=Pp[p]), orc.theta_vector(params[p], kinds)) /
+                           np.where(live, S0, 1.0), 1.0) for p in range(4)])
+    out_w, mu_w = orc.eval_weights(inp, w, want_mu=True)
+    assert np.all(np.abs(mu / mu_w - 1) < 1e-14) and np.all(np.abs(out / out_w - 1) < 1e-12)
+    assert not np.allclose(out, ref, rtol=1e-6)                      # the tables do matter
+    # (iii) a single line, one recoil bin below the Compton edge
+    E0, T0, pe0 = 0.862, 0.3, 0.54
+    gL, gR = orc.sm_couplings()
+    line = dict(E=np.array([E0]), flux_w=np.array([2.0]), P_e=np.array([pe0]), f_tau=0.5, T=np.array([T0]),
+                N_mc=np.array([[100.0]]), R=np.array([[[0.9]]]), bkg=np.array([[1.0]]), counts=np.array([[50.0]]))
+    se, sm = orc.dsigma_weak(E0, T0, gL[0], gR[0]), orc.dsigma_weak(E0, T0, gL[1], gR[1])
+    nominal = pe0 * se + (1 - pe0) * sm
+    _, mu1 = orc.eval_pee(line, np.zeros((2, 1)), [0], np.array([[1.0], [0.0]]), want_mu=True)
+    assert abs(mu1[0, 0, 0] - (1.0 + 0.9 * 100.0 * se / nominal)) < 1e-12 * mu1[0, 0, 0]
+    assert abs(mu1[1, 0, 0] - (1.0 + 0.9 * 100.0 * sm / nominal)) < 1e-12 * mu1[1, 0, 0]
+
+
 def test_sm_point_gives_sm_prediction(orc):
     inp = _small_problem(D=2)
     _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
