@@ -164,6 +164,20 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
 int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
                     uint32_t flags, void *cuda_stream);
 
+/* rw_eval_pee: the path with a survival-probability table per point (the "physics update" of PAPER.md:220 evaluates
+ * the oscillation probabilities for every parameter vector; here they arrive tabulated on the flux grid).
+ *     w[p][i] = S_theta_p(T_i; P_e_pts[p]) / S_SM(T_i; nominal P_e)       (Eq. 12 / Eq. 14; the MC sample and the SM
+ * reference stay those of the nominal table given to rw_create), P_mu, P_tau = (1 - P_e)(1 - f_tau), (1 - P_e) f_tau.
+ * The spectrum is computed on the (E_nu x T) grid per point (these weights are not low-rank), then folded by the
+ * dense path of rw_eval_weights.
+ *   param, param_kind, P, k   as rw_eval_batch (DEVICE param; kinds RW_EPS_* and RW_MU_NU only)
+ *   P_e_pts                   [P][n_E] device pointer, values in [0,1] (not validated)
+ *   out_m2lnL [P], out_mu NULL or [P][D][n_rec]   device pointers
+ *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM
+ * Needs a single-component context created without explicit P_mu / P_tau.  Asynchronous and stream-ordered. */
+int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                const double *P_e_pts, double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
+
 /* rw_eval_profile: -2lnL with the overall rate normalisation of the signal profiled out per point (PAPER.md:309,
  * "profiling an overall rate normalization at each scan point"; rate_k of Eq. 17; the Gaussian
  * constraint of Eq. 18, on that one nuisance).  With S = mu - bkg the fold of the point at unit

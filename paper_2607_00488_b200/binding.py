@@ -26,7 +26,7 @@ RW_CREATE_FP32 = 1
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
-EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_get_table",
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_eval_pee", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
            "rw_last_error", "rw_probe_fp64_peak")
 
@@ -79,6 +79,9 @@ def load_library():
     L.rw_eval_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_void_p,
                                C.c_void_p, C.c_uint32, C.c_void_p]
     L.rw_eval_grad.restype = C.c_int
+    L.rw_eval_pee.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_void_p,
+                              C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_pee.restype = C.c_int
     L.rw_get_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
     L.rw_launch_count.argtypes = [C.c_void_p]
     L.rw_launch_count.restype = C.c_int64
@@ -260,6 +263,27 @@ class Reweighter:
         self._check(rc, self._ctx)
         self._last_param = param
         return out, scale
+
+    def eval_pee(self, param, kinds, P_e_pts, want_mu=False, full_eq18=False, mode="auto"):
+        """-2lnL[P] (and mu) with a survival-probability table per point, P_e_pts[P][n_E] (CUDA tensors; rw_eval_pee)."""
+        if not (isinstance(param, torch.Tensor) and param.is_cuda and isinstance(P_e_pts, torch.Tensor) and P_e_pts.is_cuda):
+            raise RwError(-4, "eval_pee needs CUDA tensors param[P][k] and P_e_pts[P][n_E]")
+        param = param.to(torch.float64).contiguous()
+        if param.ndim == 1:
+            param = param[:, None]
+        P, k = param.shape
+        pts = P_e_pts.to(torch.float64).contiguous()
+        assert pts.shape == (P, self.n_E) and k == len(kinds)
+        kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
+        out = torch.empty(P, dtype=torch.float64, device=self.device)
+        mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device) if want_mu else None
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        rc = self._L.rw_eval_pee(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, C.c_void_p(pts.data_ptr()),
+                                 C.c_void_p(out.data_ptr()), C.c_void_p(mu.data_ptr()) if want_mu else None,
+                                 flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = (param, pts)
+        return (out, mu) if want_mu else out
 
     def eval_grad(self, param, kinds, full_eq18=False, mode="auto"):
         """(-2lnL[P], gradient[P][k]) for CUDA param[P][k] (rw_eval_grad)."""

@@ -278,6 +278,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     if (!ctx->tmapR) { free(ctx); return fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory"); }
     ctx->n_E = in->n_E; ctx->n_T = in->n_T; ctx->n_rec = in->n_rec; ctx->D = in->n_periods;
     ctx->n_comp = (int)n_comp;
+    ctx->f_tau = f_tau; ctx->have_mu_tau = have_mt;
     ctx->lay = L;
     ctx->num_sms = sms;
     ctx->ws = (char *)dev_workspace;
@@ -535,19 +536,10 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
     return RW_OK;
 }
 
-int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
-                    uint32_t flags, void *cuda_stream)
+// Dense fold + likelihood for P rows of caller-visible weights w[P][n_T] (device).
+static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, bool full, double *out, double *out_mu,
+                        cudaStream_t s)
 {
-    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_weights: ctx is NULL");
-    if (P < 0) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: P < 0");
-    if (P == 0) return RW_OK;
-    if (!w || !out_m2lnL) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: w or out_m2lnL is NULL");
-    const uint32_t mode = flags & RW_MODE_MASK;
-    if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST)))
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_weights: collapsed mode and host buffers are not supported "
-                                             "(arbitrary weights are not low-rank; w is a device array)");
-    const bool full = flags & RW_FULL_EQ18;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
     const size_t n_T = ctx->n_T;
@@ -556,8 +548,7 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
         for (int64_t g0 = 0; g0 < P; g0 += kStreamMaxPB) {
             const int Pb = (int)((P - g0 < kStreamMaxPB) ? P - g0 : kStreamMaxPB);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
-            RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb,
-                                            out_m2lnL + g0, full, mu, s));
+            RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
     } else {
         for (int64_t c0 = 0; c0 < P; c0 += L.MC) {
@@ -567,8 +558,58 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
                 RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
                 RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
             }
-            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, out_m2lnL + c0, full, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, out + c0, full, s));
         }
+    }
+    return RW_OK;
+}
+
+int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
+                    uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_weights: ctx is NULL");
+    if (P < 0) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: P < 0");
+    if (P == 0) return RW_OK;
+    if (!w || !out_m2lnL) return fail(ctx, RW_ERR_INVALID, "rw_eval_weights: w or out_m2lnL is NULL");
+    const uint32_t mode = flags & RW_MODE_MASK;
+    if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32)))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_weights: collapsed mode, RW_FP32 and host buffers are not supported "
+                                             "(arbitrary weights are not low-rank; w is a device array)");
+    return weights_rows(ctx, w, P, mode, flags & RW_FULL_EQ18, out_m2lnL, out_mu, (cudaStream_t)cuda_stream);
+}
+
+int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                const double *P_e_pts, double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_pee: ctx is NULL");
+    if (P < 0 || k < 0 || k > RW_RATE_0) return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: P < 0 or k outside [0,7]");
+    if (P == 0) return RW_OK;
+    if (!out_m2lnL || !P_e_pts || (k > 0 && (!param || !param_kind)))
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: param, param_kind, P_e_pts or out_m2lnL is NULL");
+    const uint32_t mode = flags & RW_MODE_MASK;
+    if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32)))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: collapsed mode, RW_FP32 and host buffers are not supported");
+    if (ctx->n_comp > 1 || ctx->have_mu_tau)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: needs a single component created without explicit P_mu/P_tau "
+                                             "(the point's 1 - P_e is split by f_tau)");
+    int kinds[RW_N_KINDS];
+    { int rc = check_kinds(ctx, "rw_eval_pee", k, param_kind, kinds); if (rc != RW_OK) return rc; }
+    for (int a = 0; a < k; ++a)
+        if (kinds[a] >= RW_RATE_0) return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: rate kinds are not accepted");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Layout &L = ctx->lay;
+    // passes sized by the mu scratch, which holds the weights w[Pq][n_T] here
+    int64_t per_pass = (int64_t)((size_t)L.prof_rows * ctx->D * ctx->n_rec / (size_t)ctx->n_T);
+    if (per_pass > L.max_batch) per_pass = L.max_batch;
+    if (per_pass < 1)
+        return fail(ctx, RW_ERR_WORKSPACE, "rw_eval_pee: the scratch cannot hold one row of weights (n_T = %d)", ctx->n_T);
+    for (int64_t q0 = 0; q0 < P; q0 += per_pass) {
+        const int64_t Pq = (P - q0 < per_pass) ? P - q0 : per_pass;
+        RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
+        RW_CUDA(ctx, launch_weights_pee(ctx, P_e_pts + (size_t)q0 * ctx->n_E, Pq, ctx->mu_prof, s));
+        int rc = weights_rows(ctx, ctx->mu_prof, Pq, mode, flags & RW_FULL_EQ18, out_m2lnL + q0,
+                              out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s);
+        if (rc != RW_OK) return rc;
     }
     return RW_OK;
 }

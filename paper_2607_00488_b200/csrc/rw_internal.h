@@ -70,6 +70,8 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
 struct rw_ctx {
     int n_E, n_T, n_rec, D;
     int n_comp;               // signal components (>= 1)
+    double f_tau;             // tau share of 1 - P_e when no explicit P_mu / P_tau tables were given
+    bool have_mu_tau;         // explicit P_mu / P_tau tables (then rw_eval_pee cannot split a per-point P_e)
     uint8_t *comp8;           // [n_T] component of every recoil bin (device); all zero when n_comp == 1
     double *rate;             // [max_batch][4] per-point rate scales of the components (k_coef)
     rw::Consts cst;
@@ -137,6 +139,7 @@ cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // 
 cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, double s0, double sigma,
                            bool full_eq18, double *out, double *out_scale, cudaStream_t s);   // rw_profile.cu
 int profile_setup(rw_ctx *ctx);                                              // rw_profile.cu
+cudaError_t launch_weights_pee(rw_ctx *ctx, const double *P_e_pts, int64_t Pq, double *w, cudaStream_t s);  // rw_pee.cu
 cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
                              cudaStream_t s);                                // rw_grad.cu
 cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,

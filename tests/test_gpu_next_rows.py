@@ -325,3 +325,44 @@ def test_gradient_multi_component_and_asimov_zero(rw, orc):
     scale = np.abs(orc.eval_grad(inp, params[:1], kinds)[1])
     assert abs(out.item()) < 1e-9 and np.all(np.abs(grad.cpu().numpy()) <= 1e-9 * scale)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------- f-3 per-point survival probabilities
+@pytest.mark.parametrize("mode,P", [("stream", 3), ("gemm", 45), ("auto", 150)])
+def test_per_point_survival_probability(rw, orc, mode, P):
+    """P_ee table per point: spectrum on the (E_nu x T) grid per point (n_E = 300: three staging chunks with a
+    ragged tail; dead bins), then the dense fold; against orc.eval_pee."""
+    import torch
+    inp = wl.make_custom(n_E=300, n_T=203, n_rec=130, n_periods=2, seed=101, dead_fraction=0.15)
+    params, kinds = wl.random_points(P, [wl.EPS_EE_L, wl.EPS_EE_R, wl.EPS_TT_L, wl.MU_NU], seed=102)
+    rng = np.random.default_rng(103)
+    Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.25, 0.25, size=(P, 300)), 0.0, 1.0)
+    Pp[0] = inp["P_e"]
+    ref, mu_ref, scale = orc.eval_pee(inp, params, kinds, Pp, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=max(P, 16))
+    out, mu = ctx.eval_pee(_cuda(params), kinds, _cuda(Pp), want_mu=True, mode=mode)
+    plain = ctx.eval_batch(_cuda(params[:1]), kinds)
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    assert abs(plain.item() - out[0].item()) <= 1e-9 + 1e-11 * abs(plain.item())     # nominal table = ordinary path
+    with pytest.raises(rw.RwError):
+        ctx.eval_pee(_cuda(params), kinds, _cuda(Pp), mode="collapsed")
+    ctx.close()
+
+
+def test_per_point_survival_probability_config3_size(rw, orc):
+    """Config-3-sized grids (4096 flux entries x 4096 recoil bins x 2048 rec bins), 40 points with their own tables."""
+    import torch
+    inp = wl.make("cfg3_nsi4")
+    params, kinds = wl.scan_points("cfg3_nsi4")
+    params = params[:40]
+    rng = np.random.default_rng(104)
+    shift = rng.uniform(-0.1, 0.1, size=(40, 1))
+    Pp = np.clip(inp["P_e"][None, :] + shift, 0.0, 1.0)
+    ctx = rw.Reweighter(inp, max_batch=64)
+    out = ctx.eval_pee(_cuda(params), kinds, _cuda(Pp))
+    torch.cuda.synchronize()
+    idx = np.array([0, 1, 17, 39])
+    ref, scale = orc.eval_pee(inp, params[idx], kinds, Pp[idx], want_abs=True, nthreads=CORES)
+    assert np.all(np.abs(out.cpu().numpy()[idx] - ref) <= 1e-9 + 1e-12 * scale)
+    ctx.close()
