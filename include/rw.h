@@ -75,15 +75,21 @@ enum {
     RW_MODE_MASK   = 3u << 4,
     RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
     RW_OUT_HOST    = 1u << 9,  /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
-    RW_FP32        = 1u << 10  /* opt-in reduced precision for the batched contraction (rw_eval_batch, > 4 points, dense
+    RW_FP32        = 1u << 10, /* opt-in reduced precision for the batched contraction (rw_eval_batch, > 4 points, dense
                                   fold): operands split in two TF32 pieces, three tcgen05 tensor-core products, FP32
                                   accumulation in 128-bin chunks; mu within 1e-5 relative of the FP64 path (values below
                                   the FP32 range flush to 0).  Needs a context created with RW_CREATE_FP32. */
+    RW_SLICED      = 1u << 11  /* opt-in FP64-by-slicing for the batched contraction: rows of N' and columns of R in fixed point
+                                  (56 bits below their own maximum), 36 INT8 tensor-core products with exact int32
+                                  accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
+                                  one: ~1e-13 of mu for responses spread over many recoil bins.
+                                  Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point). */
 };
 
 /* rw_inputs.create_flags */
 enum {
-    RW_CREATE_FP32 = 1u << 0   /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
+    RW_CREATE_FP32 = 1u << 0,  /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
+    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into eight 7-bit INT8 slices (same bytes as R) for RW_SLICED; n_T <= 16384 */
 };
 
 /* Physical constants.  The paper prints symbols only; any field that is 0
@@ -115,7 +121,7 @@ typedef struct {
                                RW_MEM_DEVICE: all arrays are device pointers; R is borrowed (caller keeps
                                it alive until rw_destroy) when 16-byte aligned with even n_rec, the
                                small tables are copied. */
-    uint32_t create_flags;  /* 0 or RW_CREATE_FP32 */
+    uint32_t create_flags;  /* 0, RW_CREATE_FP32 and/or RW_CREATE_SLICED */
     int32_t n_comp;         /* signal components (Eq. 17; Sec. IV B); 0 or 1: one.
                                With n_comp > 1, flux_w, P_e (and P_mu, P_tau) are [n_comp][n_E] tables on the shared
                                E grid, and the recoil bins of all components are concatenated along n_T. */

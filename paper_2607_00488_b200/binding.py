@@ -21,8 +21,8 @@ RW_RATE_0 = 7        # RW_RATE_0 + c: rate scale of signal component c
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
 RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED = 0, 1 << 4, 2 << 4, 3 << 4
-RW_PARAM_HOST, RW_OUT_HOST, RW_FP32 = 1 << 8, 1 << 9, 1 << 10
-RW_CREATE_FP32 = 1
+RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED = 1 << 8, 1 << 9, 1 << 10, 1 << 11
+RW_CREATE_FP32, RW_CREATE_SLICED = 1, 2
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
 
@@ -130,7 +130,7 @@ class Reweighter:
     (R is borrowed, the rest copied).  Several signal components (Eq. 17): flux_w, P_e[, P_mu, P_tau] as
     [n_comp][n_E] plus comp_of_T[n_T]; parameter kinds RW_RATE_0 + c then scale component c."""
 
-    def __init__(self, inputs, max_batch, device="cuda:0", consts=None, fp32=False):
+    def __init__(self, inputs, max_batch, device="cuda:0", consts=None, fp32=False, sliced=False):
         self._L = load_library()
         self._ctx = C.c_void_p(None)
         self.device = torch.device(device)
@@ -171,7 +171,7 @@ class Reweighter:
             inp.consts = rw_constants(*[float(consts.get(k, 0.0)) for k in
                                         ("sin2_theta_w", "m_e_MeV", "G_F_MeV2", "alpha_em")])
         inp.mem_kind = RW_MEM_DEVICE if on_device else RW_MEM_HOST
-        inp.create_flags = RW_CREATE_FP32 if fp32 else 0
+        inp.create_flags = (RW_CREATE_FP32 if fp32 else 0) | (RW_CREATE_SLICED if sliced else 0)
         fw = inputs["flux_w"]
         inp.n_comp = int(fw.shape[0]) if fw.ndim == 2 else 1
         if inp.n_comp > 1:
@@ -205,14 +205,16 @@ class Reweighter:
             msg = self._L.rw_last_error(ctx).decode() or self._L.rw_strerror(rc).decode()
             raise RwError(rc, msg)
 
-    def eval_batch(self, param, kinds, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto", fp32=False):
+    def eval_batch(self, param, kinds, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto", fp32=False,
+                   sliced=False):
         """-2lnL[P] for param[P][k] (CUDA float64 tensor, or numpy/pinned CPU tensor => host path).
 
         Device params: asynchronous on the current stream, returns a CUDA tensor.
         Host params: H2D + kernels + D2H are enqueued on the current stream; returns a CPU tensor
         (pinned), valid after the stream is synchronised."""
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_FP32 if fp32 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_FP32 if fp32 else 0) | \
+            (RW_SLICED if sliced else 0)
         host = not (isinstance(param, torch.Tensor) and param.is_cuda)
         if host:
             if isinstance(param, np.ndarray):

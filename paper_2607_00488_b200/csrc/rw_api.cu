@@ -44,10 +44,14 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->max_batch = max_batch;
     L->copy_R = (in->mem_kind == RW_MEM_HOST) || (n_rec & 1);
     L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
-    L->KPAD = (int)((n_T + kBK - 1) / kBK * kBK);
+    L->KPAD = (int)((n_T + 31) / 32 * 32);      // k-stages of 16 (DMMA) and 32 (INT8 slices) both divide it
     L->A_pitch = (int64_t)L->KPAD * 8;
     L->KP32 = (int)((n_T + 3) / 4 * 4);
     L->fp32 = (in->create_flags & RW_CREATE_FP32) != 0;
+    L->sliced = (in->create_flags & RW_CREATE_SLICED) != 0;
+    L->KT8 = (int)((n_T + 31) / 32);
+    L->sb8 = (n_T <= 4096) ? 8 : 7;
+    L->NT8 = (int)((n_rec + 63) / 64);
     int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;
     if (cap > kMaxChunkRows) cap = kMaxChunkRows;
@@ -89,7 +93,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
     L->coef = take((size_t)max_batch * kCoefStride * 8);
     L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
-    size_t part_gemm = D * (size_t)L->n_tiles_n * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
+    size_t part_gemm = D * (size_t)(L->sliced ? L->NT8 : L->n_tiles_n) * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
     L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
     L->out_stage = take((size_t)max_batch * 8);
@@ -107,6 +111,10 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         L->mu_prof = take((size_t)rows * D * n_rec * 8);
     }
     L->R32 = take(L->fp32 ? D * 2 * n_rec * (size_t)L->KP32 * 4 : 0);
+    L->B8 = take(L->sliced ? D * (size_t)L->NT8 * L->KT8 * 16384 : 0);
+    L->f_col8 = take(L->sliced ? D * n_rec * 4 : 0);
+    L->e_row8 = take(L->sliced ? (size_t)L->MC * 4 : 0);
+    L->tau8 = take(L->sliced ? D * n_T * 4 : 0);
     L->total = off;
     return RW_OK;
 }
@@ -150,8 +158,9 @@ static bool auto_stream(const rw_ctx *, int64_t P) { return P <= 4; }
 
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
+// prec: 0 = FP64 DMMA, 1 = TF32 x 3 (RW_FP32), 2 = INT8 slices (RW_SLICED); only the contraction regime differs
 static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s,
-                      bool fp32 = false)
+                      int prec = 0)
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
@@ -176,14 +185,16 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
-                if (fp32) {
+                if (prec == 1) {
                     RW_CUDA(ctx, launch_fold_tf32(ctx, d, c0, Pc, mu, s));
+                } else if (prec == 2) {
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, c0, Pc, mu, s));
                 } else {
                     RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
                     RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
                 }
             }
-            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, dout + c0, full, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * (prec == 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, dout + c0, full, s));
         }
     }
     return RW_OK;
@@ -316,6 +327,10 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->mu_tile = (double *)(ws + L.mu_tile);
     ctx->mu_prof = (double *)(ws + L.mu_prof);
     ctx->R32 = (float *)(ws + L.R32);
+    ctx->B8 = (uint8_t *)(ws + L.B8);
+    ctx->f_col8 = (int *)(ws + L.f_col8);
+    ctx->e_row8 = (int *)(ws + L.e_row8);
+    ctx->tau8 = (int *)(ws + L.tau8);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;
@@ -386,6 +401,13 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: TF32 split of R failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
+    if (rc == RW_OK && L.sliced) {
+        if (ctx->n_T > 16384)
+            rc = fail(nullptr, RW_ERR_UNSUPPORTED, "rw_create: RW_CREATE_SLICED needs n_T <= 16384 (exact int32 accumulation)");
+        if (rc == RW_OK) rc = i8_setup(ctx, s);
+        if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
+            rc = fail(nullptr, RW_ERR_CUDA, "rw_create: slicing R failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     if (rc != RW_OK) { free(ctx->tmapB32); free(ctx->tmapR); free(ctx); return rc; }
     ctx->err[0] = 0;
     *out = ctx;
@@ -427,9 +449,13 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
     if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_MODE_COLLAPSED needs a single signal component");
-    const bool fp32 = flags & RW_FP32;
+    const bool fp32 = flags & RW_FP32, sliced = flags & RW_SLICED;
     if (fp32 && !ctx->lay.fp32)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_FP32 needs a context created with RW_CREATE_FP32");
+    if (sliced && (!ctx->lay.sliced || fp32))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_SLICED needs a context created with RW_CREATE_SLICED "
+                                             "and excludes RW_FP32");
+    const int prec = sliced ? 2 : (fp32 ? 1 : 0);
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -462,7 +488,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             }
         } else {
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
-        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, fp32); if (rc != RW_OK) return rc; }
+        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, prec); if (rc != RW_OK) return rc; }
         }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));

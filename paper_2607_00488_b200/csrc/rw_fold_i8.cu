@@ -1,0 +1,493 @@
+// rw_fold_i8.cu -- opt-in RW_SLICED variant of the batched fold ("FP64-by-slicing
+// (Ozaki-style) on low-precision tensor cores as a way past the native FP64 peak while holding 1e-12").
+//
+// The fold mu[p][k] = sum_i N'[p][i] R[i][k] (Eq. 11) has only non-negative terms.  Each row of N'
+// and each column of R is written in fixed point relative to its own power-of-two scale and cut into eight 7-bit
+// slices,
+//     N'[p][i] = 2^(e_p) sum_s a_s[p][i] 2^(-7(s+1)),      R[i][k] = 2^(f_k) sum_t b_t[i][k] 2^(-7(t+1)),
+// so that the contraction becomes 36 INT8 tensor-core products with EXACT int32 accumulation (tcgen05.mma
+// kind::i8, accumulators in TMEM; 8 pairs x 16384 bins x 127^2 < 2^31; for n_T <= 4096 the slices are 8 bits wide,
+// 8 x 4096 x 255^2 < 2^31, and the formulas below hold with 8 in place of 7):
+//     mu[p][k] - bkg[k] = 2^(e_p + f_k - 14) sum_{d=0..7} 2^(-7d) sum_{s+t=d} sum_i a_s[p][i] b_t[i][k].
+// Before slicing, recoil bin i is rescaled by an exact power of two on both sides, N'[p][i] / 2^tau_i and
+// R[i][k] 2^tau_i with 2^tau_i ~ N_mc[i]: the rows of N' then have the dynamic range of the WEIGHTS (Eq. 14) instead
+// of that of the MC spectrum times the weights, which is what the fixed-point error is relative to.
+// Pairs with s + t > 7 are below 2^-56 of (row max x column max x N_T) and are dropped; the slices themselves
+// truncate at 2^-56 of the row / column maximum.  There is no rounding anywhere else, so the error is a bound in
+// terms of the scales, not of the individual mu: for responses whose columns spread over many recoil bins (all
+// BASELINE configurations) it is < 1e-13 of mu; see DESIGN.md section 3.3 for the bound and its limits.
+//
+// One CTA per SM, 192 threads as in rw_fold_tf32.cu (TMA warp, MMA warp, 4 epilogue warps), tile 128 points x 64
+// bins, 32 recoil bins per stage.  The slices are stored in global memory already in the tensor core's canonical
+// K-major no-swizzle layout (8 x 16-byte core matrices), all eight slices of a (tile, k-block) contiguous: a stage
+// is two plain bulk copies (32 KB of N' slices, 16 KB of R slices).  Eight TMEM accumulators (one per s + t) x 64
+// columns = all 512 TMEM columns; the epilogue combines them in FP64 and evaluates the Poisson terms of Eq. (18).
+#include <limits.h>
+
+#include "rw_internal.h"
+
+namespace rw {
+
+constexpr int kI8BM = 128, kI8BN = 64, kI8BK = 32;
+constexpr int kI8Slices = 8;
+constexpr int kI8SliceBytesA = kI8BM * kI8BK;                   // 4 KB
+constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 2 KB
+constexpr int kI8StageBytesA = kI8Slices * kI8SliceBytesA;      // 32 KB
+constexpr int kI8StageBytesB = kI8Slices * kI8SliceBytesB;      // 16 KB
+constexpr int kI8StageBytes = kI8StageBytesA + kI8StageBytesB;
+constexpr int kI8Stages = 4;
+constexpr int kI8Threads = 192;
+constexpr int kI8Smem = kI8Stages * kI8StageBytes + 3 * 64 * 8 + 64 * 8 + 256 + 1024;
+constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
+
+// ---------------------------------------------------------------------------------------------- slicing
+// fixed-point digits of x (0 <= x < 2^e) with sb bits per slice (7, or 8 when n_T <= 4096 lets eight pairs of
+// 255 x 255 products still fit int32): q = floor(x 2^(8 sb - e)), slice s = bits [sb (7-s), sb (8-s)) of q
+__device__ __forceinline__ unsigned long long i8_fixed(double x, int e, int sb)
+{
+    return __double2ull_rd(ldexp(x, 8 * sb - e));
+}
+__device__ __forceinline__ int i8_exponent(double vmax)          // smallest e with vmax < 2^e (0 for vmax == 0)
+{
+    if (!(vmax > 0.0)) return 0;
+    int e;
+    frexp(vmax, &e);                                             // vmax = m 2^e, m in [0.5, 1)
+    return e;
+}
+
+// N'[p][i] = rate * sum_b coef[p][b] W^[b][i] (steps a1 + a2) for 8 points x all recoil bins per CTA, W^ staged
+// 512 bins at a time.  PASS 0: row maximum -> exponent e_p.  PASS 1: slices, written 16 bytes at a time into
+//   As[m-tile][k-block][slice][16-byte chunk c][row group g][row r8][16]     (canonical K-major core matrices)
+template <int PASS>
+__global__ void __launch_bounds__(256)
+k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
+          int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
+          int sb, int *__restrict__ e_row, uint8_t *__restrict__ As)
+{
+    __shared__ double sW[kNumTerms][512];
+    __shared__ uint8_t sComp[512];
+    __shared__ short sTau[512];
+    __shared__ double sC[8][kCoefStride];
+    __shared__ double sRate[8][RW_MAX_COMPONENTS];
+    const int r = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + r;
+    if (threadIdx.x < 8 * kCoefStride) {
+        const int rr = threadIdx.x / kCoefStride, b = threadIdx.x - rr * kCoefStride;
+        const int64_t q = (int64_t)blockIdx.x * 8 + rr;
+        sC[rr][b] = (q < Pc) ? coef[(p0 + q) * kCoefStride + b] : 0.0;
+    }
+    if (threadIdx.x < 8 * RW_MAX_COMPONENTS) {
+        const int rr = threadIdx.x / RW_MAX_COMPONENTS, cq = threadIdx.x % RW_MAX_COMPONENTS;
+        const int64_t q = (int64_t)blockIdx.x * 8 + rr;
+        sRate[rr][cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
+    }
+    const int e = (PASS == 1) ? e_row[row] : 0;
+    double vmax = 0.0;
+    bool bad = false;
+    const int n_pad = KT * kI8BK;
+    for (int i0 = 0; i0 < n_pad; i0 += 512) {
+        __syncthreads();
+        for (int q = threadIdx.x; q < kNumTerms * 512; q += 256) {
+            const int b = q >> 9, ii = q & 511, i = i0 + ii;
+            sW[b][ii] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;
+        }
+        for (int q = threadIdx.x; q < 512; q += 256) {
+            sComp[q] = (i0 + q < n_T) ? comp8[i0 + q] : 0;
+            sTau[q] = (i0 + q < n_T) ? (short)tau[i0 + q] : 0;
+        }
+        __syncthreads();
+        const int ii0 = lane * 16, ibase = i0 + ii0;             // this thread: 16 consecutive bins of its row
+        if (ibase >= n_pad) continue;
+        unsigned long long q16[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            double v = 0.0;
+#pragma unroll
+            for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][ii0 + j], v);
+            v = ldexp(v * sRate[r][sComp[ii0 + j]], -sTau[ii0 + j]);      // exact: N' / 2^tau_i
+            if (PASS == 0) {
+                if (!(v >= 0.0) || isinf(v)) bad = true;
+                vmax = fmax(vmax, v);
+            } else {
+                q16[j] = (e == kI8BadRow) ? 0ull : i8_fixed(v, e, sb);
+            }
+        }
+        if (PASS == 1) {
+            const int64_t mt = row >> 7;
+            const int rr = (int)(row & 127), g = rr >> 3, r8 = rr & 7;
+            const int kt = ibase >> 5, c = (ibase >> 4) & 1;
+            uint8_t *base = As + ((size_t)(mt * KT + kt) * kI8Slices * 2 + c) * 2048 + g * 128 + r8 * 16;
+#pragma unroll
+            for (int s = 0; s < kI8Slices; ++s) {
+                uint32_t w[4];
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    uint32_t x = 0;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        x |= (uint32_t)((q16[4 * h + j] >> (sb * (7 - s))) & ((1ull << sb) - 1)) << (8 * j);
+                    w[h] = x;
+                }
+                *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+        }
+    }
+    if (PASS == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+            bad = __shfl_xor_sync(0xffffffffu, (int)bad, o) || bad;
+        }
+        if (lane == 0) e_row[row] = bad ? kI8BadRow : i8_exponent(vmax);
+    }
+}
+
+// Column maxima of R -> exponents f_k (one thread per column, rows read coalesced across the warp).
+// tau_i = binary exponent of the mean of N_mc over the 33 bins around i (0 where that mean is 0): the per-bin
+// rescaling shared by both operands.  The window keeps tau smooth: it follows the shape of the MC spectrum, which
+// is what spans decades, without passing bin-to-bin noise of N_mc on to the columns of R.
+__global__ void k_tau(const double *__restrict__ N_mc, int n_T, int *__restrict__ tau)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_T) return;
+    double acc = 0.0;
+    for (int j = max(0, i - 16); j <= min(n_T - 1, i + 16); ++j) acc += N_mc[j];
+    tau[i] = i8_exponent(acc / 33.0);
+}
+
+__global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, const int *__restrict__ tau,
+                           int *__restrict__ f_col)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_rec) return;
+    double vmax = 0.0;
+    for (int i = 0; i < n_T; ++i) vmax = fmax(vmax, ldexp(R[(size_t)i * ldR + k], tau[i]));
+    f_col[k] = i8_exponent(vmax);
+}
+
+// Slices of R in  Bs[n-tile][k-block][slice][chunk c][column group g][column r8][16]  (K-major core matrices,
+// "rows" of the B operand are reconstructed bins).  Thread = (column, 16 consecutive recoil bins).
+__global__ void __launch_bounds__(256)
+k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols /*64 x column tiles*/, int KT, int sb,
+          const int *__restrict__ tau, const int *__restrict__ f_col, uint8_t *__restrict__ Bs)
+{
+    const int k = blockIdx.x * 256 + threadIdx.x;                // column (padded columns carry zeros)
+    const int ibase = blockIdx.y * 16;
+    if (k >= n_cols) return;
+    const int f = (k < n_rec) ? f_col[k] : 0;
+    unsigned long long q16[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const int i = ibase + j;
+        const double v = (k < n_rec && i < n_T) ? ldexp(R[(size_t)i * ldR + k], tau[i]) : 0.0;     // exact: R 2^tau_i
+        q16[j] = i8_fixed(v, f, sb);
+    }
+    const int nt = k >> 6, rr = k & 63, g = rr >> 3, r8 = rr & 7;
+    const int kt = ibase >> 5, c = (ibase >> 4) & 1;
+    uint8_t *base = Bs + ((size_t)((size_t)nt * KT + kt) * kI8Slices * 2 + c) * 1024 + g * 128 + r8 * 16;
+#pragma unroll
+    for (int t = 0; t < kI8Slices; ++t) {
+        uint32_t w[4];
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            uint32_t x = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) x |= (uint32_t)((q16[4 * h + j] >> (sb * (7 - t))) & ((1ull << sb) - 1)) << (8 * j);
+            w[h] = x;
+        }
+        *reinterpret_cast<uint4 *>(base + (size_t)t * kI8SliceBytesB) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- the contraction
+__device__ __forceinline__ uint32_t i8_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void i8_mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void i8_mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void i8_mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void i8_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// contiguous global -> shared bulk copy (TMA engine, no tensor map), completion on an mbarrier
+__device__ __forceinline__ void i8_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// K-major operand, no swizzle: 8 rows x 16 bytes core matrices (128 contiguous bytes); SBO = distance between
+// 8-row groups, LBO = distance between the two 16-byte K chunks of a 32-element k-step; descriptor version 1.
+__device__ __forceinline__ uint64_t i8_desc(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((smem_addr & 0x3ffff) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+           ((uint64_t)(sbo_bytes >> 4) << 32) | ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                        uint32_t accumulate)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void i8_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+
+struct I8Work {
+    int n_rec, KT, tiles_m, tiles_n, D, d, sb;
+    int64_t Pc, part_stride;
+    const uint8_t *As, *Bs;
+    const int *e_row, *f_col;
+    const double *bkg, *counts;
+    double *partial, *out_mu;
+};
+
+__device__ __forceinline__ void i8_tile_coord(int t, int tiles_m, int tiles_n, int &tm, int &tn)
+{
+    constexpr int GM = 8;             // 8 point tiles sweep the column tiles: a wave shares their slices in L2
+    const int per_group = GM * tiles_n;
+    const int g = t / per_group, rem = t - g * per_group;
+    const int first_m = g * GM;
+    const int gm = min(GM, tiles_m - first_m);
+    tm = first_m + rem % gm;
+    tn = rem / gm;
+}
+
+__global__ void __launch_bounds__(kI8Threads, 1)
+k_fold_i8(const I8Work W)
+{
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const uint32_t sbase = i8_smem_u32(smem);
+    double *s_bkg = reinterpret_cast<double *>(smem + kI8Stages * kI8StageBytes);     // [64] per tile
+    double *s_cnt = s_bkg + 64, *s_inv = s_cnt + 64, *s_scl = s_inv + 64;            // counts, 1/counts, 2^f_k
+    const uint32_t bars = sbase + kI8Stages * kI8StageBytes + 4 * 64 * 8;
+    const uint32_t full_bar = bars, empty_bar = bars + 8 * kI8Stages;
+    const uint32_t tfull_bar = empty_bar + 8 * kI8Stages, tempty_bar = tfull_bar + 8;
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kI8Stages * kI8StageBytes + 4 * 64 * 8 + 128);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kI8Stages; ++s) { i8_mbar_init(full_bar + 8 * s, 1); i8_mbar_init(empty_bar + 8 * s, 1); }
+        i8_mbar_init(tfull_bar, 1);
+        i8_mbar_init(tempty_bar, 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {     // TMEM: 8 accumulators (one per s + t) x 64 int32 columns = all 512 columns
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(i8_smem_u32(s_tmem)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *s_tmem;
+    const int total_tiles = W.tiles_m * W.tiles_n;
+    const int KT = W.KT;
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ producer: two bulk copies per stage
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+                int tm, tn;
+                i8_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
+                const uint8_t *a = W.As + (size_t)tm * KT * kI8StageBytesA;
+                const uint8_t *b = W.Bs + (size_t)tn * KT * kI8StageBytesB;
+                for (int kt = 0; kt < KT; ++kt) {
+                    i8_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
+                    const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kI8StageBytes;
+                    i8_mbar_expect_tx(fb, kI8StageBytes);
+                    i8_bulk_g2s(dst, a + (size_t)kt * kI8StageBytesA, kI8StageBytesA, fb);
+                    i8_bulk_g2s(dst + kI8StageBytesA, b + (size_t)kt * kI8StageBytesB, kI8StageBytesB, fb);
+                    if (++stage == kI8Stages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer: 36 products per stage
+        if (lane == 0) {
+            // D = S32 (bits 4-5 = 2), A = B = unsigned 8 bit (bits 7-9, 10-12 = 0), K-major, N >> 3 at bit 17, M >> 4 at 24
+            const uint32_t idesc = (2u << 4) | ((uint32_t)(kI8BN >> 3) << 17) | ((uint32_t)(kI8BM >> 4) << 24);
+            int stage = 0; uint32_t phase = 0, tseq = 0;
+            for (int t = blockIdx.x; t < total_tiles; t += gridDim.x, ++tseq) {
+                i8_mbar_wait(tempty_bar, (tseq & 1) ^ 1);        // the epilogue has drained the previous tile
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                for (int kt = 0; kt < KT; ++kt) {
+                    i8_mbar_wait(full_bar + 8 * stage, phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t sa = sbase + stage * kI8StageBytes, sb = sa + kI8StageBytesA;
+#pragma unroll
+                    for (int d = 0; d < kI8Slices; ++d)
+#pragma unroll
+                        for (int s = 0; s <= d; ++s)
+                            umma_i8(tmem_base + d * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
+                                    i8_desc(sb + (d - s) * kI8SliceBytesB, 1024, 128), idesc, (kt > 0 || s > 0) ? 1u : 0u);
+                    i8_commit(empty_bar + 8 * stage);
+                    if (++stage == kI8Stages) { stage = 0; phase ^= 1; }
+                }
+                i8_commit(tfull_bar);
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ epilogue warps 2..5
+        const int q = warp & 3;
+        const int lrow = 32 * q + lane;
+        const int et = threadIdx.x - 64;                         // 0..127
+        uint32_t tseq = 0;
+        for (int t = blockIdx.x; t < total_tiles; t += gridDim.x, ++tseq) {
+            int tm, tn;
+            i8_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (et < kI8BN) {        // column constants; columns >= n_rec: all slices are zero, bkg = n = 1/n = 0
+                const int col = tn * kI8BN + et;
+                const bool ok = col < W.n_rec;
+                const double n = ok ? W.counts[col] : 0.0;
+                s_bkg[et] = ok ? W.bkg[col] : 0.0;
+                s_cnt[et] = n;
+                s_inv[et] = n > 0.0 ? 1.0 / n : 0.0;
+                s_scl[et] = ok ? ldexp(1.0, W.f_col[col]) : 0.0;
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            const int64_t row = (int64_t)tm * kI8BM + lrow;
+            const int e = W.e_row[row];
+            const double rscale = (e == kI8BadRow) ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, e - 2 * W.sb);
+            const double step = (W.sb == 8) ? 0.00390625 : 0.0078125;     // 2^-sb between neighbouring diagonals
+            i8_mbar_wait(tfull_bar, tseq & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16);
+            double tot = 0.0;
+#pragma unroll 1
+            for (int g = 0; g < kI8BN / 16; ++g) {
+                double v[16];
+                {   // Horner over the diagonals d = 7 .. 0: v = sum_d 2^(-7 d) acc_d, exact int32 -> double
+                    uint32_t a[16];
+                    tmem_ld16(taddr + 7 * kI8BN + 16 * g, a);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[j] = (double)(int)a[j];
+#pragma unroll
+                    for (int d = 6; d >= 0; --d) {
+                        tmem_ld16(taddr + d * kI8BN + 16 * g, a);
+                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) v[j] = fma(v[j], step, (double)(int)a[j]);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 16; j += 4) {
+                    const int c0 = 16 * g + j;
+                    const double m0 = fma(v[j] * rscale, s_scl[c0], s_bkg[c0]);
+                    const double m1 = fma(v[j + 1] * rscale, s_scl[c0 + 1], s_bkg[c0 + 1]);
+                    const double m2 = fma(v[j + 2] * rscale, s_scl[c0 + 2], s_bkg[c0 + 2]);
+                    const double m3 = fma(v[j + 3] * rscale, s_scl[c0 + 3], s_bkg[c0 + 3]);
+                    if (W.out_mu && row < W.Pc) {
+                        const int col = tn * kI8BN + c0;
+                        double *dst = W.out_mu + ((size_t)row * W.D + W.d) * W.n_rec + col;
+                        if (col < W.n_rec) dst[0] = m0;
+                        if (col + 1 < W.n_rec) dst[1] = m1;
+                        if (col + 2 < W.n_rec) dst[2] = m2;
+                        if (col + 3 < W.n_rec) dst[3] = m3;
+                    }
+                    tot += poisson_sum4(m0, m1, m2, m3, s_cnt[c0], s_cnt[c0 + 1], s_cnt[c0 + 2], s_cnt[c0 + 3],
+                                        s_inv[c0], s_inv[c0 + 1], s_inv[c0 + 2], s_inv[c0 + 3]);
+                }
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) i8_mbar_arrive(tempty_bar);
+            if (row < W.Pc) W.partial[(size_t)tn * W.part_stride + row] = tot;
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- host side
+// rw_create with RW_CREATE_SLICED: column exponents and the eight slices of every period's R.
+int i8_setup(rw_ctx *ctx, cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    const int KT = L.KT8, n_cols = L.NT8 * kI8BN;
+    const size_t per = (size_t)L.NT8 * KT * kI8StageBytesB;
+    for (int d = 0; d < ctx->D; ++d) {
+        const double *Rd = ctx->R + (size_t)d * ctx->R_period_stride;
+        int *f = ctx->f_col8 + (size_t)d * ctx->n_rec, *tau = ctx->tau8 + (size_t)d * ctx->n_T;
+        k_tau<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T, tau);
+        k_colexp_B<<<(ctx->n_rec + 127) / 128, 128, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, tau, f);
+        dim3 grid((n_cols + 255) / 256, KT * 2);
+        k_slice_B<<<grid, 256, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, n_cols, KT, L.sb8, tau, f, ctx->B8 + (size_t)d * per);
+        ctx->launches += 3;
+    }
+    if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "slicing R failed at launch");
+    cudaError_t e = cudaFuncSetAttribute(k_fold_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_i8): %s", cudaGetErrorString(e));
+    return RW_OK;
+}
+
+// Steps a1-a4 for the Pc points at coef[p0..] and period d through the sliced INT8 contraction.
+cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s)
+{
+    const Layout &L = ctx->lay;
+    const int KT = L.KT8;
+    const int64_t rows_pad = (Pc + kI8BM - 1) / kI8BM * kI8BM;
+    uint8_t *As = reinterpret_cast<uint8_t *>(ctx->A_packed);     // 8 slice bytes per (point, bin): fits the FP64 N'
+    const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
+    const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
+    k_slice_A<0><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
+                                                         L.sb8, ctx->e_row8, As);
+    k_slice_A<1><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
+                                                         L.sb8, ctx->e_row8, As);
+    ctx->launches += 2;
+    I8Work W;
+    W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d; W.sb = L.sb8;
+    W.tiles_m = (int)(rows_pad / kI8BM); W.tiles_n = L.NT8;
+    W.Pc = Pc; W.part_stride = L.MC;
+    W.As = As;
+    W.Bs = ctx->B8 + (size_t)d * L.NT8 * KT * kI8StageBytesB;
+    W.e_row = ctx->e_row8;
+    W.f_col = ctx->f_col8 + (size_t)d * ctx->n_rec;
+    W.bkg = ctx->bkg + (size_t)d * ctx->n_rec;
+    W.counts = ctx->counts + (size_t)d * ctx->n_rec;
+    W.partial = ctx->partial + (size_t)d * L.NT8 * L.MC;       // [D][NT8][MC]: 64-column tiles in this mode
+    W.out_mu = out_mu;
+    const int total = W.tiles_m * W.tiles_n;
+    const int grid = total < ctx->num_sms ? total : ctx->num_sms;
+    {
+        ProfScope prof(ctx, s);
+        k_fold_i8<<<grid, kI8Threads, kI8Smem, s>>>(W);
+    }
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace rw

@@ -48,6 +48,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part, comp8, rate;
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof, R32;
+    size_t B8, f_col8, e_row8, tau8;
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
@@ -57,6 +58,9 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
     int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
+    bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
+    int sb8;              // bits per slice: 8 when n_T <= 4096 (int32 accumulation stays exact), else 7
+    int KT8, NT8;         // k-blocks of 32 recoil bins, column tiles of 64 bins (rw_fold_i8.cu)
     bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
@@ -89,6 +93,9 @@ struct rw_ctx {
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
+    uint8_t *B8;              // [D][NT8][KT8][8 slices][2 KB] INT8 slices of R (RW_CREATE_SLICED)
+    int *f_col8, *e_row8;     // column exponents [D][n_rec]; row exponents of the current chunk [MC]
+    int *tau8;                // [D][n_T] per-bin rescaling exponents (2^tau ~ N_mc)
     float *R32;               // [D][2 (hi, lo)][n_rec][KP32] transposed TF32 split of R (RW_CREATE_FP32)
     CUtensorMap tmapA32[2];   // hi, lo of N' (aliases A_packed)
     CUtensorMap *tmapB32;     // host array [2 D]
@@ -144,6 +151,8 @@ cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k,
                              cudaStream_t s);                                // rw_grad.cu
 cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,
                         double *grad, cudaStream_t s);                       // rw_grad.cu
+int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
+cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);    // rw_fold_i8.cu
 int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
 cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,

@@ -1,0 +1,80 @@
+"""Opt-in RW_SLICED contraction (FP64 by slicing on the INT8 tensor cores, exact int32 accumulation) against the
+oracle at the FP64 bars of the main path: mu 1e-12 relative, -2lnL 1e-9 + 1e-12 * sum 2|term| (reading T)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2607_00488_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+CORES = os.cpu_count() or 4
+
+
+def _cuda(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _check(inp, params, kinds, ref, mu_ref, scale, max_batch=None):
+    import torch
+    from paper_2607_00488_b200 import binding
+    ctx = binding.Reweighter(inp, max_batch=max_batch or params.shape[0], sliced=True)
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="gemm", sliced=True)
+    out64 = ctx.eval_batch(_cuda(params), kinds, mode="gemm")
+    torch.cuda.synchronize()
+    out, mu, out64 = out.cpu().numpy(), mu.cpu().numpy(), out64.cpu().numpy()
+    ctx.close()
+    rel = np.abs(mu - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= 1e-12, "sliced mu rel err %.3e" % rel.max()
+    err = np.abs(out - ref)
+    assert np.all(err <= 1e-9 + 1e-12 * scale), "sliced -2lnL err %.3e" % err.max()
+    assert np.all(np.abs(out64 - ref) <= 1e-9 + 1e-12 * scale)
+    return rel.max()
+
+
+def test_sliced_small_ragged(orc):
+    """n_T = 203 (7 k-blocks of 32, ragged), n_rec = 330 (6 column tiles of 64, ragged), 2 periods, 300 points
+    (3 point tiles, ragged), all seven parameter kinds, dead bins."""
+    inp = wl.make_custom(n_E=31, n_T=203, n_rec=330, n_periods=2, seed=111, dead_fraction=0.1)
+    params, kinds = wl.random_points(300, list(range(7)), seed=112)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale)
+
+
+def test_sliced_long_contraction_and_chunks(orc):
+    """n_T = 3000 (94 k-blocks; the smem ring wraps many times), several tiles per CTA, P > max_batch."""
+    inp = wl.make_custom(n_E=24, n_T=3000, n_rec=200, n_periods=1, seed=113)
+    params, kinds = wl.random_points(150, [wl.EPS_EE_L, wl.EPS_EE_R, wl.MU_NU], seed=114)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale, max_batch=64)
+
+
+def test_sliced_config2_all_points(orc):
+    """Config 2: exact zeros in R, 867 dead recoil bins, mu_nu over two decades."""
+    inp = wl.make("cfg2_mm_lowE")
+    params, kinds = wl.scan_points("cfg2_mm_lowE")
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale)
+
+
+def test_sliced_components_rates_and_bad_points(orc):
+    import torch
+    from paper_2607_00488_b200 import binding
+    inp = wl.make_components(n_comp=3, n_E=33, n_T=160, n_rec=140, n_periods=2, seed=115)
+    kinds = np.array([wl.EPS_EE_L, wl.MU_NU, 7, 9], np.int32)
+    params, _ = wl.random_points(70, kinds, seed=116)
+    ref, mu_ref, scale = orc.eval_components(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale)
+    bad = params.copy()
+    bad[5, 0] = np.nan
+    ctx = binding.Reweighter(inp, max_batch=70, sliced=True)
+    out = ctx.eval_batch(_cuda(bad), kinds, mode="gemm", sliced=True)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    assert np.isnan(out[5]) and np.all(np.isfinite(np.delete(out, 5)))
+    plain = binding.Reweighter(inp, max_batch=8)
+    with pytest.raises(binding.RwError):
+        plain.eval_batch(_cuda(params[:8]), kinds, mode="gemm", sliced=True)
+    plain.close()
+    ctx.close()
