@@ -12,21 +12,21 @@ pytestmark = pytest.mark.gpu
 CORES = os.cpu_count() or 4
 
 
-def _device_ctx(binding, inp, max_batch):
+def _device_ctx(binding, inp, max_batch, sliced=False):
     import torch
     dev_inp = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()
                for k in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
     dev_inp["f_tau"] = inp["f_tau"]
-    return binding.Reweighter(dev_inp, max_batch=max_batch)
+    return binding.Reweighter(dev_inp, max_batch=max_batch, sliced=sliced)
 
 
-def _full_vs_sample(orc, name, sample_idx, max_batch, mu_check=True):
+def _full_vs_sample(orc, name, sample_idx, max_batch, mu_check=True, sliced=False):
     import torch
     from paper_2607_00488_b200 import binding
     inp = wl.make(name)
     params, kinds = wl.scan_points(name)
     P = params.shape[0]
-    ctx = _device_ctx(binding, inp, max_batch)
+    ctx = _device_ctx(binding, inp, max_batch, sliced=sliced)
     out = ctx.eval_batch(torch.from_numpy(params).cuda(), kinds)
     torch.cuda.synchronize()
     out = out.cpu().numpy()
@@ -44,6 +44,12 @@ def _full_vs_sample(orc, name, sample_idx, max_batch, mu_check=True):
         out_s = ctx.eval_batch(torch.from_numpy(params[idx[:8]]).cuda(), kinds, mode="stream")
         torch.cuda.synchronize()
         assert np.all(np.abs(out_s.cpu().numpy() - ref[:8]) <= 1e-9 + 1e-12 * scale[:8])
+    if sliced:      # the INT8-sliced contraction on the sampled points: same FP64 bars
+        out_i8, mu_i8 = ctx.eval_batch(torch.from_numpy(params[idx]).cuda(), kinds, want_mu=True, mode="gemm", sliced=True)
+        torch.cuda.synchronize()
+        rel = np.abs(mu_i8.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+        assert rel.max() <= 1e-12, "sliced mu rel err %.3e" % rel.max()
+        assert np.all(np.abs(out_i8.cpu().numpy() - ref) <= 1e-9 + 1e-12 * scale)
     ctx.close()
     return err.max()
 
@@ -51,14 +57,14 @@ def _full_vs_sample(orc, name, sample_idx, max_batch, mu_check=True):
 def test_config3_full_scan_sampled(orc):
     rng = np.random.default_rng(303)
     idx = np.concatenate([[0, 9999, 8191, 8192], rng.integers(0, 10000, 28)])
-    _full_vs_sample(orc, "cfg3_nsi4", idx, max_batch=10000)
+    _full_vs_sample(orc, "cfg3_nsi4", idx, max_batch=10000, sliced=True)
 
 
 def test_config4_bench_configuration_sampled(orc):
     """65536 points, 16384 x 8192 response: exactly what bench.py times (8 chunks of 8192 points)."""
     rng = np.random.default_rng(404)
     idx = np.concatenate([[0, 65535, 8191, 8192, 32767, 32768], rng.integers(0, 65536, 18)])
-    _full_vs_sample(orc, "cfg4_dense", idx, max_batch=65536)
+    _full_vs_sample(orc, "cfg4_dense", idx, max_batch=65536, sliced=True)
 
 
 def test_config5_streamed_in_batches_of_16384(orc):
