@@ -188,7 +188,8 @@ def main():
                for key in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
     dev_inp["f_tau"] = inp["f_tau"]
     max_batch = args.max_batch or (16384 if name == "cfg5_joint6" else P)
-    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=True)   # + TF32 copy of R for the opt-in leg
+    sliced_ok = n_T <= 16384
+    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=True, sliced=sliced_ok)   # + operand copies for the opt-in legs
     param_dev = torch.from_numpy(params).to(dev)
     out_dev = torch.empty(P, dtype=torch.float64, device=dev)
     param_pin = torch.from_numpy(params).pin_memory()
@@ -352,6 +353,27 @@ def main():
                     "note": "three tcgen05.mma.kind::tf32 products per k-step (hi*hi, hi*lo, lo*hi), FP32 accumulation in "
                             "128-bin TMEM chunks; the three-fold executed flops are not counted in effective_fold_tflops"}
 
+    # opt-in RW_SLICED contraction: FP64 by slicing on the INT8 tensor cores, exact int32 accumulation,
+    # same 1e-12 bar as the DMMA path; a context line, never mixed into `value`
+    sliced_leg = None
+    if P > 4 and sliced_ok:
+        out_s = torch.empty(P, dtype=torch.float64, device=dev)
+        ctx.profile_begin()
+        t_s = timed(lambda: ctx.eval_batch(param_dev, kinds, out=out_s, sliced=True), 5)
+        k_ms, k_n = ctx.profile_end()
+        ns = min(P, 128)
+        _, mu8 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm", sliced=True)
+        _, mu64 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm")
+        rel = ((mu8 - mu64).abs() / mu64.abs())
+        sliced_leg = {"ms_per_call": t_s, "evals_per_s": P / t_s * 1e3, "bound": "tensor (int8)",
+                      "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_s / 1e9,
+                      "kernel_effective_fold_tflops": 2.0 * n_T * n_rec * D * P * 7 / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None,
+                      "executed_int8_tops": 72.0 * n_T * n_rec * D * P / t_s / 1e9,
+                      "mu_rel_diff_vs_dmma_max": float(rel.max().item()),
+                      "max_abs_diff_m2lnL_vs_dmma": float((out_s - out_dev).abs().max().item()),
+                      "note": "eight 7/8-bit slices per operand, 36 tcgen05.mma.kind::i8 products per k-step with exact int32 "
+                              "accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % dmma_peak0}
+
     # ---------------------------------------------------------------- roofline of the dominant kernel
     # the probe is taken before the timed region and again here; the higher reading is the denominator (a probe
     # right after the TF32 leg can catch a lower clock)
@@ -389,7 +411,7 @@ def main():
                         "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path": same},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
-                "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg,
+                "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg, "sliced_mode": sliced_leg,
                 "clocks": clocks, "all_finite": finite,
                 "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
                                  "the authors' own multi-component model; other hardware and inputs, not comparable"}
