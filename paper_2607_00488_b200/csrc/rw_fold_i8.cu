@@ -58,6 +58,10 @@ __device__ __forceinline__ int i8_exponent(double vmax)          // smallest e w
 // N'[p][i] = rate * sum_b coef[p][b] W^[b][i] (steps a1 + a2) for 8 points x all recoil bins per CTA, W^ staged
 // 512 bins at a time.  PASS 0: row maximum -> exponent e_p.  PASS 1: slices, written 16 bytes at a time into
 //   As[m-tile][k-block][slice][16-byte chunk c][row group g][row r8][16]     (canonical K-major core matrices)
+// shared-memory column swizzle: a thread reads 16 consecutive bins (lane stride 128 bytes = one bank for the whole
+// warp); XOR-ing the low 4 index bits with the 16-bin group number spreads 16 lanes over 16 banks
+__device__ __forceinline__ int i8_sw(int ii) { return ii ^ ((ii >> 4) & 15); }
+
 template <int PASS>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
@@ -65,8 +69,8 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
           int sb, int *__restrict__ e_row, uint8_t *__restrict__ As)
 {
     __shared__ double sW[kNumTerms][512];
-    __shared__ uint8_t sComp[512];
-    __shared__ short sTau[512];
+    __shared__ __align__(16) uint8_t sComp[512];
+    __shared__ float sScl[512];                                  // 2^-tau_i (exact in FP32 too), swizzled like sW
     __shared__ double sC[8][kCoefStride];
     __shared__ double sRate[8][RW_MAX_COMPONENTS];
     const int r = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -89,22 +93,24 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
         __syncthreads();
         for (int q = threadIdx.x; q < kNumTerms * 512; q += 256) {
             const int b = q >> 9, ii = q & 511, i = i0 + ii;
-            sW[b][ii] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;
+            sW[b][i8_sw(ii)] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;
         }
         for (int q = threadIdx.x; q < 512; q += 256) {
             sComp[q] = (i0 + q < n_T) ? comp8[i0 + q] : 0;
-            sTau[q] = (i0 + q < n_T) ? (short)tau[i0 + q] : 0;
+            sScl[i8_sw(q)] = (i0 + q < n_T) ? ldexpf(1.0f, -tau[i0 + q]) : 1.0f;
         }
         __syncthreads();
         const int ii0 = lane * 16, ibase = i0 + ii0;             // this thread: 16 consecutive bins of its row
         if (ibase >= n_pad) continue;
         unsigned long long q16[16];
+        const uint4 cw = *reinterpret_cast<const uint4 *>(sComp + ii0);
+        const uint32_t cws[4] = {cw.x, cw.y, cw.z, cw.w};
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             double v = 0.0;
 #pragma unroll
-            for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][ii0 + j], v);
-            v = ldexp(v * sRate[r][sComp[ii0 + j]], -sTau[ii0 + j]);      // exact: N' / 2^tau_i
+            for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][i8_sw(ii0 + j)], v);
+            v = v * sRate[r][(cws[j >> 2] >> (8 * (j & 3))) & 0xffu] * (double)sScl[i8_sw(ii0 + j)];   // N' / 2^tau_i
             if (PASS == 0) {
                 if (!(v >= 0.0) || isinf(v)) bad = true;
                 vmax = fmax(vmax, v);
@@ -152,7 +158,7 @@ __global__ void k_tau(const double *__restrict__ N_mc, int n_T, int *__restrict_
     if (i >= n_T) return;
     double acc = 0.0;
     for (int j = max(0, i - 16); j <= min(n_T - 1, i + 16); ++j) acc += N_mc[j];
-    tau[i] = i8_exponent(acc / 33.0);
+    tau[i] = max(-120, min(120, i8_exponent(acc / 33.0)));      // any tau is valid (shared by both operands); keep 2^-tau an FP32 normal
 }
 
 __global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, const int *__restrict__ tau,
