@@ -365,14 +365,17 @@ def main():
         _, mu8 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm", sliced=True)
         _, mu64 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm")
         rel = ((mu8 - mu64).abs() / mu64.abs())
+        n_sl = 8 if n_T <= 8192 else 7                              # balanced 8-bit slices per operand (rw_fold_i8.cu)
+        n_prod = n_sl * (n_sl + 1) // 2
         sliced_leg = {"ms_per_call": t_s, "evals_per_s": P / t_s * 1e3, "bound": "tensor (int8)",
                       "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_s / 1e9,
                       "kernel_effective_fold_tflops": 2.0 * n_T * n_rec * D * P * 7 / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None,
-                      "executed_int8_tops": 72.0 * n_T * n_rec * D * P / t_s / 1e9,
+                      "executed_int8_tops": 2.0 * n_prod * n_T * n_rec * D * P / t_s / 1e9,
                       "mu_rel_diff_vs_dmma_max": float(rel.max().item()),
                       "max_abs_diff_m2lnL_vs_dmma": float((out_s - out_dev).abs().max().item()),
-                      "note": "eight 7/8-bit slices per operand, 36 tcgen05.mma.kind::i8 products per k-step with exact int32 "
-                              "accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % dmma_peak0}
+                      "slices": n_sl, "int8_products_per_k_step": n_prod,
+                      "note": "%d balanced 8-bit slices per operand, %d tcgen05.mma.kind::i8 products per k-step with exact "
+                              "int32 accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % (n_sl, n_prod, dmma_peak0)}
 
     # ---------------------------------------------------------------- roofline of the dominant kernel
     # the probe is taken before the timed region and again here; the higher reading is the denominator (a probe

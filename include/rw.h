@@ -80,8 +80,8 @@ enum {
                                   accumulation in 128-bin chunks; mu within 1e-5 relative of the FP64 path (values below
                                   the FP32 range flush to 0).  Needs a context created with RW_CREATE_FP32. */
     RW_SLICED      = 1u << 11  /* opt-in FP64-by-slicing for the batched contraction: rows of N' and columns of R in fixed point
-                                  (56 bits below their own maximum), 36 INT8 tensor-core products with exact int32
-                                  accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
+                                  (8 balanced base-256 digits for n_T <= 8192, else 7: 63 / 55 bits below their own maximum),
+                                  36 / 28 INT8 tensor-core products per 32 recoil bins with exact int32 accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
                                   one: ~1e-13 of mu for responses spread over many recoil bins.
                                   Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point). */
 };
@@ -89,7 +89,8 @@ enum {
 /* rw_inputs.create_flags */
 enum {
     RW_CREATE_FP32 = 1u << 0,  /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
-    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into eight 7-bit INT8 slices (same bytes as R) for RW_SLICED; n_T <= 16384 */
+    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into 8 (7 for n_T > 8192) INT8 slices (at most the bytes of R) for RW_SLICED;
+                                  n_T <= 18560 */
 };
 
 /* Physical constants.  The paper prints symbols only; any field that is 0

@@ -50,7 +50,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->fp32 = (in->create_flags & RW_CREATE_FP32) != 0;
     L->sliced = (in->create_flags & RW_CREATE_SLICED) != 0;
     L->KT8 = (int)((n_T + 31) / 32);
-    L->sb8 = (n_T <= 4096) ? 8 : 7;
+    L->ns8 = (n_T <= 8192) ? 8 : 7;
     L->NT8 = (int)((n_rec + 63) / 64);
     int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;
@@ -402,8 +402,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: TF32 split of R failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
     if (rc == RW_OK && L.sliced) {
-        if (ctx->n_T > 16384)
-            rc = fail(nullptr, RW_ERR_UNSUPPORTED, "rw_create: RW_CREATE_SLICED needs n_T <= 16384 (exact int32 accumulation)");
+        if (ctx->n_T > 18560)
+            rc = fail(nullptr, RW_ERR_UNSUPPORTED, "rw_create: RW_CREATE_SLICED needs n_T <= 18560 (exact int32 accumulation)");
         if (rc == RW_OK) rc = i8_setup(ctx, s);
         if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: slicing R failed: %s", cudaGetErrorString(cudaGetLastError()));

@@ -2,26 +2,29 @@
 // (Ozaki-style) on low-precision tensor cores as a way past the native FP64 peak while holding 1e-12").
 //
 // The fold mu[p][k] = sum_i N'[p][i] R[i][k] (Eq. 11) has only non-negative terms.  Each row of N'
-// and each column of R is written in fixed point relative to its own power-of-two scale and cut into eight 7-bit
-// slices,
-//     N'[p][i] = 2^(e_p) sum_s a_s[p][i] 2^(-7(s+1)),      R[i][k] = 2^(f_k) sum_t b_t[i][k] 2^(-7(t+1)),
-// so that the contraction becomes 36 INT8 tensor-core products with EXACT int32 accumulation (tcgen05.mma
-// kind::i8, accumulators in TMEM; 8 pairs x 16384 bins x 127^2 < 2^31; for n_T <= 4096 the slices are 8 bits wide,
-// 8 x 4096 x 255^2 < 2^31, and the formulas below hold with 8 in place of 7):
-//     mu[p][k] - bkg[k] = 2^(e_p + f_k - 14) sum_{d=0..7} 2^(-7d) sum_{s+t=d} sum_i a_s[p][i] b_t[i][k].
+// and each column of R is written in fixed point relative to its own power-of-two scale and cut into NS base-256
+// digits ("slices"; NS = 8 for n_T <= 8192, else 7),
+//     N'[p][i] = 2^(e_p - 7) sum_s a_s[p][i] 2^(-8 s),      R[i][k] = 2^(f_k - 7) sum_t b_t[i][k] 2^(-8 t),
+// with BALANCED digits: a_0 in [0, 129] (unsigned; one spare bit keeps the carry), a_s in [-128, 127] for s > 0.
+// The contraction becomes NS (NS + 1) / 2 INT8 tensor-core products with EXACT int32 accumulation (tcgen05.mma
+// kind::i8, accumulators in TMEM; |digit product| <= 129 x 128, NS pairs per accumulator:
+// 7 x 16512 x 18560 bins < 2^31 and 8 x 16512 x 8192 < 2^31):
+//     mu[p][k] - bkg[k] = 2^(e_p + f_k - 14) sum_{d=0..NS-1} 2^(-8d) sum_{s+t=d} sum_i a_s[p][i] b_t[i][k].
+// Balanced digits are what lets 8-bit slices through at n_T = 16384 (unsigned ones would need 7-bit slices, i.e.
+// 8 slices and 36 products for the same 55 bits that 7 slices and 28 products give here).
 // Before slicing, recoil bin i is rescaled by an exact power of two on both sides, N'[p][i] / 2^tau_i and
 // R[i][k] 2^tau_i with 2^tau_i ~ N_mc[i]: the rows of N' then have the dynamic range of the WEIGHTS (Eq. 14) instead
 // of that of the MC spectrum times the weights, which is what the fixed-point error is relative to.
-// Pairs with s + t > 7 are below 2^-56 of (row max x column max x N_T) and are dropped; the slices themselves
-// truncate at 2^-56 of the row / column maximum.  There is no rounding anywhere else, so the error is a bound in
-// terms of the scales, not of the individual mu: for responses whose columns spread over many recoil bins (all
-// BASELINE configurations) it is < 1e-13 of mu; see DESIGN.md section 3.3 for the bound and its limits.
+// Pairs with s + t >= NS are below 2^-(8 NS - 1) of (row max x column max x N_T) and are dropped; the fixed-point
+// values are rounded to nearest at 2^-(8 NS - 1) of the row / column maximum.  There is no rounding anywhere
+// else, so the error is a bound in terms of the scales, not of the individual mu: for responses whose columns
+// spread over many recoil bins (all BASELINE configurations) it is < 1e-13 of mu; see DESIGN.md section 3.3.
 //
 // One CTA per SM, 192 threads as in rw_fold_tf32.cu (TMA warp, MMA warp, 4 epilogue warps), tile 128 points x 64
 // bins, 32 recoil bins per stage.  The slices are stored in global memory already in the tensor core's canonical
-// K-major no-swizzle layout (8 x 16-byte core matrices), all eight slices of a (tile, k-block) contiguous: a stage
-// is two plain bulk copies (32 KB of N' slices, 16 KB of R slices).  Eight TMEM accumulators (one per s + t) x 64
-// columns = all 512 TMEM columns; the epilogue combines them in FP64 and evaluates the Poisson terms of Eq. (18).
+// K-major no-swizzle layout (8 x 16-byte core matrices), all slices of a (tile, k-block) contiguous: a stage is
+// two plain bulk copies (NS x 4 KB of N' slices, NS x 2 KB of R slices).  NS TMEM accumulators (one per s + t) x
+// 64 columns; the epilogue combines them in FP64 (Horner) and evaluates the Poisson terms of Eq. (18).
 #include <limits.h>
 
 #include "rw_internal.h"
@@ -29,23 +32,28 @@
 namespace rw {
 
 constexpr int kI8BM = 128, kI8BN = 64, kI8BK = 32;
-constexpr int kI8Slices = 8;
 constexpr int kI8SliceBytesA = kI8BM * kI8BK;                   // 4 KB
 constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 2 KB
-constexpr int kI8StageBytesA = kI8Slices * kI8SliceBytesA;      // 32 KB
-constexpr int kI8StageBytesB = kI8Slices * kI8SliceBytesB;      // 16 KB
-constexpr int kI8StageBytes = kI8StageBytesA + kI8StageBytesB;
-constexpr int kI8Stages = 4;
 constexpr int kI8Threads = 192;
-constexpr int kI8Smem = kI8Stages * kI8StageBytes + 3 * 64 * 8 + 64 * 8 + 256 + 1024;
+constexpr int kI8TailBytes = 4 * kI8BN * 8 + 256 + 1024;        // column constants, barriers, alignment slack
+__host__ __device__ constexpr int i8_stage_bytes(int ns) { return ns * (kI8SliceBytesA + kI8SliceBytesB); }
+__host__ __device__ constexpr int i8_stages(int ns) { return ns == 8 ? 4 : 5; }      // 4 x 48 KB / 5 x 42 KB
+__host__ __device__ constexpr int i8_smem(int ns) { return i8_stages(ns) * i8_stage_bytes(ns) + kI8TailBytes; }
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
 
 // ---------------------------------------------------------------------------------------------- slicing
-// fixed-point digits of x (0 <= x < 2^e) with sb bits per slice (7, or 8 when n_T <= 4096 lets eight pairs of
-// 255 x 255 products still fit int32): q = floor(x 2^(8 sb - e)), slice s = bits [sb (7-s), sb (8-s)) of q
-__device__ __forceinline__ unsigned long long i8_fixed(double x, int e, int sb)
+// Fixed point: q = round(x 2^(8 ns - 1 - e)) for 0 <= x < 2^e, so q <= 2^(8 ns - 1); scale2 = 2^(8 ns - 1 - e).
+// Adding 0x80 to every digit below the top one and reading bytes gives the balanced digits: byte ^ 0x80 is the
+// two's-complement int8 of (digit - 128 + carry handling done by the addition); the top byte (<= 129) stays unsigned.
+__device__ __forceinline__ unsigned long long i8_fixed(double x, double scale2, int ns)
 {
-    return __double2ull_rd(ldexp(x, 8 * sb - e));
+    const unsigned long long bias = 0x0080808080808080ull >> (8 * (8 - ns));
+    return __double2ull_rn(x * scale2) + bias;
+}
+__device__ __forceinline__ uint32_t i8_digit(unsigned long long qb, int s, int ns)    // slice s (0 = top) as a byte
+{
+    const uint32_t u = (uint32_t)(qb >> (8 * (ns - 1 - s))) & 0xffu;
+    return s == 0 ? u : (u ^ 0x80u);
 }
 __device__ __forceinline__ int i8_exponent(double vmax)          // smallest e with vmax < 2^e (0 for vmax == 0)
 {
@@ -66,7 +74,7 @@ template <int PASS>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
           int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
-          int sb, int *__restrict__ e_row, uint8_t *__restrict__ As)
+          int ns, int *__restrict__ e_row, uint8_t *__restrict__ As)
 {
     __shared__ double sW[kNumTerms][512];
     __shared__ __align__(16) uint8_t sComp[512];
@@ -86,6 +94,7 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
         sRate[rr][cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
     }
     const int e = (PASS == 1) ? e_row[row] : 0;
+    const double scale2 = (PASS == 1 && e != kI8BadRow) ? ldexp(1.0, 8 * ns - 1 - e) : 0.0;
     double vmax = 0.0;
     bool bad = false;
     const int n_pad = KT * kI8BK;
@@ -115,23 +124,24 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
                 if (!(v >= 0.0) || isinf(v)) bad = true;
                 vmax = fmax(vmax, v);
             } else {
-                q16[j] = (e == kI8BadRow) ? 0ull : i8_fixed(v, e, sb);
+                q16[j] = i8_fixed((e == kI8BadRow) ? 0.0 : v, scale2, ns);
             }
         }
         if (PASS == 1) {
             const int64_t mt = row >> 7;
             const int rr = (int)(row & 127), g = rr >> 3, r8 = rr & 7;
             const int kt = ibase >> 5, c = (ibase >> 4) & 1;
-            uint8_t *base = As + ((size_t)(mt * KT + kt) * kI8Slices * 2 + c) * 2048 + g * 128 + r8 * 16;
+            uint8_t *base = As + ((size_t)(mt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
-            for (int s = 0; s < kI8Slices; ++s) {
+            for (int s = 0; s < 8; ++s) {
+                if (s >= ns) break;
                 uint32_t w[4];
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
                     uint32_t x = 0;
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
-                        x |= (uint32_t)((q16[4 * h + j] >> (sb * (7 - s))) & ((1ull << sb) - 1)) << (8 * j);
+                        x |= i8_digit(q16[4 * h + j], s, ns) << (8 * j);
                     w[h] = x;
                 }
                 *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) = make_uint4(w[0], w[1], w[2], w[3]);
@@ -174,31 +184,33 @@ __global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n
 // Slices of R in  Bs[n-tile][k-block][slice][chunk c][column group g][column r8][16]  (K-major core matrices,
 // "rows" of the B operand are reconstructed bins).  Thread = (column, 16 consecutive recoil bins).
 __global__ void __launch_bounds__(256)
-k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols /*64 x column tiles*/, int KT, int sb,
+k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols /*64 x column tiles*/, int KT, int ns,
           const int *__restrict__ tau, const int *__restrict__ f_col, uint8_t *__restrict__ Bs)
 {
     const int k = blockIdx.x * 256 + threadIdx.x;                // column (padded columns carry zeros)
     const int ibase = blockIdx.y * 16;
     if (k >= n_cols) return;
     const int f = (k < n_rec) ? f_col[k] : 0;
+    const double scale2 = ldexp(1.0, 8 * ns - 1 - f);
     unsigned long long q16[16];
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
         const int i = ibase + j;
         const double v = (k < n_rec && i < n_T) ? ldexp(R[(size_t)i * ldR + k], tau[i]) : 0.0;     // exact: R 2^tau_i
-        q16[j] = i8_fixed(v, f, sb);
+        q16[j] = i8_fixed(v, scale2, ns);
     }
     const int nt = k >> 6, rr = k & 63, g = rr >> 3, r8 = rr & 7;
     const int kt = ibase >> 5, c = (ibase >> 4) & 1;
-    uint8_t *base = Bs + ((size_t)((size_t)nt * KT + kt) * kI8Slices * 2 + c) * 1024 + g * 128 + r8 * 16;
+    uint8_t *base = Bs + ((size_t)((size_t)nt * KT + kt) * ns * 2 + c) * 1024 + g * 128 + r8 * 16;
 #pragma unroll
-    for (int t = 0; t < kI8Slices; ++t) {
+    for (int t = 0; t < 8; ++t) {
+        if (t >= ns) break;
         uint32_t w[4];
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
             uint32_t x = 0;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) x |= (uint32_t)((q16[4 * h + j] >> (sb * (7 - t))) & ((1ull << sb) - 1)) << (8 * j);
+            for (int j = 0; j < 4; ++j) x |= i8_digit(q16[4 * h + j], t, ns) << (8 * j);
             w[h] = x;
         }
         *reinterpret_cast<uint4 *>(base + (size_t)t * kI8SliceBytesB) = make_uint4(w[0], w[1], w[2], w[3]);
@@ -269,7 +281,7 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
 }
 
 struct I8Work {
-    int n_rec, KT, tiles_m, tiles_n, D, d, sb;
+    int n_rec, KT, tiles_m, tiles_n, D, d;
     int64_t Pc, part_stride;
     const uint8_t *As, *Bs;
     const int *e_row, *f_col;
@@ -288,9 +300,12 @@ __device__ __forceinline__ void i8_tile_coord(int t, int tiles_m, int tiles_n, i
     tn = rem / gm;
 }
 
+template <int NS>
 __global__ void __launch_bounds__(kI8Threads, 1)
 k_fold_i8(const I8Work W)
 {
+    constexpr int kI8Stages = i8_stages(NS), kI8StageBytes = i8_stage_bytes(NS);
+    constexpr int kI8StageBytesA = NS * kI8SliceBytesA, kI8StageBytesB = NS * kI8SliceBytesB;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t sbase = i8_smem_u32(smem);
@@ -308,7 +323,7 @@ k_fold_i8(const I8Work W)
         i8_mbar_init(tempty_bar, 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {     // TMEM: 8 accumulators (one per s + t) x 64 int32 columns = all 512 columns
+    if (warp == 1) {     // TMEM: NS accumulators (one per s + t) x 64 int32 columns (NS = 8: all 512 columns)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(i8_smem_u32(s_tmem)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -341,7 +356,8 @@ k_fold_i8(const I8Work W)
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer: 36 products per stage
         if (lane == 0) {
-            // D = S32 (bits 4-5 = 2), A = B = unsigned 8 bit (bits 7-9, 10-12 = 0), K-major, N >> 3 at bit 17, M >> 4 at 24
+            // D = S32 (bits 4-5 = 2), A / B format at bits 7-9 / 10-12 (0 = unsigned 8 bit: the top slice, 1 = signed:
+            // the balanced lower slices), K-major, N >> 3 at bit 17, M >> 4 at bit 24
             const uint32_t idesc = (2u << 4) | ((uint32_t)(kI8BN >> 3) << 17) | ((uint32_t)(kI8BM >> 4) << 24);
             int stage = 0; uint32_t phase = 0, tseq = 0;
             for (int t = blockIdx.x; t < total_tiles; t += gridDim.x, ++tseq) {
@@ -352,11 +368,12 @@ k_fold_i8(const I8Work W)
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t sa = sbase + stage * kI8StageBytes, sb = sa + kI8StageBytesA;
 #pragma unroll
-                    for (int d = 0; d < kI8Slices; ++d)
+                    for (int d = 0; d < NS; ++d)
 #pragma unroll
                         for (int s = 0; s <= d; ++s)
                             umma_i8(tmem_base + d * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
-                                    i8_desc(sb + (d - s) * kI8SliceBytesB, 1024, 128), idesc, (kt > 0 || s > 0) ? 1u : 0u);
+                                    i8_desc(sb + (d - s) * kI8SliceBytesB, 1024, 128),
+                                    idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u), (kt > 0 || s > 0) ? 1u : 0u);
                     i8_commit(empty_bar + 8 * stage);
                     if (++stage == kI8Stages) { stage = 0; phase ^= 1; }
                 }
@@ -385,8 +402,8 @@ k_fold_i8(const I8Work W)
             asm volatile("bar.sync 1, 128;" ::: "memory");
             const int64_t row = (int64_t)tm * kI8BM + lrow;
             const int e = W.e_row[row];
-            const double rscale = (e == kI8BadRow) ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, e - 2 * W.sb);
-            const double step = (W.sb == 8) ? 0.00390625 : 0.0078125;     // 2^-sb between neighbouring diagonals
+            const double rscale = (e == kI8BadRow) ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, e - 14);
+            const double step = 0.00390625;                      // 2^-8 between neighbouring diagonals
             i8_mbar_wait(tfull_bar, tseq & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16);
@@ -394,14 +411,14 @@ k_fold_i8(const I8Work W)
 #pragma unroll 1
             for (int g = 0; g < kI8BN / 16; ++g) {
                 double v[16];
-                {   // Horner over the diagonals d = 7 .. 0: v = sum_d 2^(-7 d) acc_d, exact int32 -> double
+                {   // Horner over the diagonals d = NS-1 .. 0: v = sum_d 2^(-8 d) acc_d, exact int32 -> double
                     uint32_t a[16];
-                    tmem_ld16(taddr + 7 * kI8BN + 16 * g, a);
+                    tmem_ld16(taddr + (NS - 1) * kI8BN + 16 * g, a);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                     for (int j = 0; j < 16; ++j) v[j] = (double)(int)a[j];
 #pragma unroll
-                    for (int d = 6; d >= 0; --d) {
+                    for (int d = NS - 2; d >= 0; --d) {
                         tmem_ld16(taddr + d * kI8BN + 16 * g, a);
                         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
@@ -444,18 +461,19 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
 {
     const Layout &L = ctx->lay;
     const int KT = L.KT8, n_cols = L.NT8 * kI8BN;
-    const size_t per = (size_t)L.NT8 * KT * kI8StageBytesB;
+    const size_t per = (size_t)L.NT8 * KT * L.ns8 * kI8SliceBytesB;
     for (int d = 0; d < ctx->D; ++d) {
         const double *Rd = ctx->R + (size_t)d * ctx->R_period_stride;
         int *f = ctx->f_col8 + (size_t)d * ctx->n_rec, *tau = ctx->tau8 + (size_t)d * ctx->n_T;
         k_tau<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T, tau);
         k_colexp_B<<<(ctx->n_rec + 127) / 128, 128, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, tau, f);
         dim3 grid((n_cols + 255) / 256, KT * 2);
-        k_slice_B<<<grid, 256, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, n_cols, KT, L.sb8, tau, f, ctx->B8 + (size_t)d * per);
+        k_slice_B<<<grid, 256, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, n_cols, KT, L.ns8, tau, f, ctx->B8 + (size_t)d * per);
         ctx->launches += 3;
     }
     if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "slicing R failed at launch");
-    cudaError_t e = cudaFuncSetAttribute(k_fold_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_smem(8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_smem(7));
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_i8): %s", cudaGetErrorString(e));
     return RW_OK;
 }
@@ -470,16 +488,16 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
     const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
     k_slice_A<0><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
-                                                         L.sb8, ctx->e_row8, As);
+                                                         L.ns8, ctx->e_row8, As);
     k_slice_A<1><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
-                                                         L.sb8, ctx->e_row8, As);
+                                                         L.ns8, ctx->e_row8, As);
     ctx->launches += 2;
     I8Work W;
-    W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d; W.sb = L.sb8;
+    W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d;
     W.tiles_m = (int)(rows_pad / kI8BM); W.tiles_n = L.NT8;
     W.Pc = Pc; W.part_stride = L.MC;
     W.As = As;
-    W.Bs = ctx->B8 + (size_t)d * L.NT8 * KT * kI8StageBytesB;
+    W.Bs = ctx->B8 + (size_t)d * L.NT8 * KT * L.ns8 * kI8SliceBytesB;
     W.e_row = ctx->e_row8;
     W.f_col = ctx->f_col8 + (size_t)d * ctx->n_rec;
     W.bkg = ctx->bkg + (size_t)d * ctx->n_rec;
@@ -490,7 +508,8 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const int grid = total < ctx->num_sms ? total : ctx->num_sms;
     {
         ProfScope prof(ctx, s);
-        k_fold_i8<<<grid, kI8Threads, kI8Smem, s>>>(W);
+        if (L.ns8 == 8) k_fold_i8<8><<<grid, kI8Threads, i8_smem(8), s>>>(W);
+        else k_fold_i8<7><<<grid, kI8Threads, i8_smem(7), s>>>(W);
     }
     ctx->launches++;
     return cudaGetLastError();
