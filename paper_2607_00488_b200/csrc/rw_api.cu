@@ -51,7 +51,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->sliced = (in->create_flags & RW_CREATE_SLICED) != 0;
     L->KT8 = (int)((n_T + 31) / 32);
     L->ns8 = (n_T <= 8192) ? 8 : 7;
-    L->NT8 = (int)((n_rec + 63) / 64);
+    L->NT8 = 2 * (int)((n_rec + 127) / 128);     // 64-column units (one epilogue warp set each); tiles are 128 wide
     int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;
     if (cap > kMaxChunkRows) cap = kMaxChunkRows;

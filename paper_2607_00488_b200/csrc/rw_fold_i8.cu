@@ -31,14 +31,12 @@
 
 namespace rw {
 
-constexpr int kI8BM = 128, kI8BN = 64, kI8BK = 32;
+constexpr int kI8BM = 128, kI8BN = 128, kI8BK = 32;
 constexpr int kI8SliceBytesA = kI8BM * kI8BK;                   // 4 KB
-constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 2 KB
-constexpr int kI8Threads = 192;
-constexpr int kI8TailBytes = 4 * kI8BN * 8 + 256 + 1024;        // column constants, barriers, alignment slack
-__host__ __device__ constexpr int i8_stage_bytes(int ns) { return ns * (kI8SliceBytesA + kI8SliceBytesB); }
-__host__ __device__ constexpr int i8_stages(int ns) { return ns == 8 ? 4 : 5; }      // 4 x 48 KB / 5 x 42 KB
-__host__ __device__ constexpr int i8_smem(int ns) { return i8_stages(ns) * i8_stage_bytes(ns) + kI8TailBytes; }
+constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 4 KB
+constexpr int kI8Threads = 320;                                 // TMA warp, MMA warp, 8 epilogue warps
+constexpr int kI8SlotBytes = 65536, kI8Stages = 3;              // a slot: N' slices in its first half, R slices in its second
+constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 4 * kI8BN * 8 + 256 + 1024;
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
 
 // ---------------------------------------------------------------------------------------------- slicing
@@ -184,7 +182,7 @@ __global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n
 // Slices of R in  Bs[n-tile][k-block][slice][chunk c][column group g][column r8][16]  (K-major core matrices,
 // "rows" of the B operand are reconstructed bins).  Thread = (column, 16 consecutive recoil bins).
 __global__ void __launch_bounds__(256)
-k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols /*64 x column tiles*/, int KT, int ns,
+k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols /*128 x column tiles*/, int KT, int ns,
           const int *__restrict__ tau, const int *__restrict__ f_col, uint8_t *__restrict__ Bs)
 {
     const int k = blockIdx.x * 256 + threadIdx.x;                // column (padded columns carry zeros)
@@ -199,9 +197,9 @@ k_slice_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, int n_cols 
         const double v = (k < n_rec && i < n_T) ? ldexp(R[(size_t)i * ldR + k], tau[i]) : 0.0;     // exact: R 2^tau_i
         q16[j] = i8_fixed(v, scale2, ns);
     }
-    const int nt = k >> 6, rr = k & 63, g = rr >> 3, r8 = rr & 7;
+    const int nt = k >> 7, rr = k & 127, g = rr >> 3, r8 = rr & 7;
     const int kt = ibase >> 5, c = (ibase >> 4) & 1;
-    uint8_t *base = Bs + ((size_t)((size_t)nt * KT + kt) * ns * 2 + c) * 1024 + g * 128 + r8 * 16;
+    uint8_t *base = Bs + ((size_t)((size_t)nt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
     for (int t = 0; t < 8; ++t) {
         if (t >= ns) break;
@@ -300,30 +298,45 @@ __device__ __forceinline__ void i8_tile_coord(int t, int tiles_m, int tiles_n, i
     tn = rem / gm;
 }
 
+// Horner step over one accumulator: v = v * 2^-8 + acc (exact int32 -> double), 16 columns
+__device__ __forceinline__ void i8_horner16(uint32_t taddr, double (&v)[16], bool first)
+{
+    uint32_t a[16];
+    tmem_ld16(taddr, a);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = first ? (double)(int)a[j] : fma(v[j], 0.00390625, (double)(int)a[j]);
+}
+
+// Tile = 128 points x 128 bins.  A product with N = 64 columns cannot be issued faster than every ~50 cycles (its
+// tensor-pipe slot is 32), one with N = 128 fills its 64-cycle slot, so the tile is 128 columns wide and the NS
+// diagonals (one 128-column int32 accumulator each; TMEM holds four) are done in TWO PASSES over the recoil bins:
+// pass 0 the diagonals 0..3 (10 products per 32 bins, slices 0..3 of both operands), pass 1 the diagonals 4..NS-1
+// (18 or 26 products, all slices).  Eight epilogue warps (lane quadrant x column half) keep the pass-0 Horner sums
+// of their 64 columns in registers until pass 1 has drained.
 template <int NS>
 __global__ void __launch_bounds__(kI8Threads, 1)
 k_fold_i8(const I8Work W)
 {
-    constexpr int kI8Stages = i8_stages(NS), kI8StageBytes = i8_stage_bytes(NS);
-    constexpr int kI8StageBytesA = NS * kI8SliceBytesA, kI8StageBytesB = NS * kI8SliceBytesB;
+    constexpr int kSlot = kI8SlotBytes, kStages = kI8Stages, kBOff = kI8SlotBytes / 2;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t sbase = i8_smem_u32(smem);
-    double *s_bkg = reinterpret_cast<double *>(smem + kI8Stages * kI8StageBytes);     // [64] per tile
-    double *s_cnt = s_bkg + 64, *s_inv = s_cnt + 64, *s_scl = s_inv + 64;            // counts, 1/counts, 2^f_k
-    const uint32_t bars = sbase + kI8Stages * kI8StageBytes + 4 * 64 * 8;
-    const uint32_t full_bar = bars, empty_bar = bars + 8 * kI8Stages;
-    const uint32_t tfull_bar = empty_bar + 8 * kI8Stages, tempty_bar = tfull_bar + 8;
-    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kI8Stages * kI8StageBytes + 4 * 64 * 8 + 128);
+    double *s_bkg = reinterpret_cast<double *>(smem + kStages * kSlot);                // [128] per tile
+    double *s_cnt = s_bkg + kI8BN, *s_inv = s_cnt + kI8BN, *s_scl = s_inv + kI8BN;    // counts, 1/counts, 2^f_k
+    const uint32_t bars = sbase + kStages * kSlot + 4 * kI8BN * 8;
+    const uint32_t full_bar = bars, empty_bar = bars + 8 * kStages;
+    const uint32_t tfull_bar = empty_bar + 8 * kStages, tempty_bar = tfull_bar + 8;
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kStages * kSlot + 4 * kI8BN * 8 + 128);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kI8Stages; ++s) { i8_mbar_init(full_bar + 8 * s, 1); i8_mbar_init(empty_bar + 8 * s, 1); }
+        for (int s = 0; s < kStages; ++s) { i8_mbar_init(full_bar + 8 * s, 1); i8_mbar_init(empty_bar + 8 * s, 1); }
         i8_mbar_init(tfull_bar, 1);
-        i8_mbar_init(tempty_bar, 4);
+        i8_mbar_init(tempty_bar, 8);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {     // TMEM: NS accumulators (one per s + t) x 64 int32 columns (NS = 8: all 512 columns)
+    if (warp == 1) {     // TMEM: 4 accumulators x 128 int32 columns = all 512 columns
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(i8_smem_u32(s_tmem)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -333,63 +346,102 @@ k_fold_i8(const I8Work W)
     const uint32_t tmem_base = *s_tmem;
     const int total_tiles = W.tiles_m * W.tiles_n;
     const int KT = W.KT;
+    constexpr size_t kPerKtA = (size_t)NS * kI8SliceBytesA, kPerKtB = (size_t)NS * kI8SliceBytesB;
 
     if (warp == 0) {
-        // ------------------------------------------------------------------ producer: two bulk copies per stage
+        // ------------------------------------------------------------------ producer: bulk copies, no tensor maps
+        // pass 0: a stage is TWO 32-bin blocks (slices 0..3: 16 KB + 16 KB each); pass 1: one block, all slices
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
                 int tm, tn;
                 i8_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
-                const uint8_t *a = W.As + (size_t)tm * KT * kI8StageBytesA;
-                const uint8_t *b = W.Bs + (size_t)tn * KT * kI8StageBytesB;
+                const uint8_t *a = W.As + (size_t)tm * KT * kPerKtA;
+                const uint8_t *b = W.Bs + (size_t)tn * KT * kPerKtB;
+                for (int kt = 0; kt < KT; kt += 2) {
+                    i8_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
+                    const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kSlot;
+                    const int nk = min(2, KT - kt);
+                    i8_mbar_expect_tx(fb, nk * 8 * 4096);
+                    for (int h = 0; h < nk; ++h) {
+                        i8_bulk_g2s(dst + h * 16384, a + (size_t)(kt + h) * kPerKtA, 4 * kI8SliceBytesA, fb);
+                        i8_bulk_g2s(dst + kBOff + h * 16384, b + (size_t)(kt + h) * kPerKtB, 4 * kI8SliceBytesB, fb);
+                    }
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
                 for (int kt = 0; kt < KT; ++kt) {
                     i8_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
-                    const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kI8StageBytes;
-                    i8_mbar_expect_tx(fb, kI8StageBytes);
-                    i8_bulk_g2s(dst, a + (size_t)kt * kI8StageBytesA, kI8StageBytesA, fb);
-                    i8_bulk_g2s(dst + kI8StageBytesA, b + (size_t)kt * kI8StageBytesB, kI8StageBytesB, fb);
-                    if (++stage == kI8Stages) { stage = 0; phase ^= 1; }
+                    const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kSlot;
+                    i8_mbar_expect_tx(fb, (uint32_t)(kPerKtA + kPerKtB));
+                    i8_bulk_g2s(dst, a + (size_t)kt * kPerKtA, (uint32_t)kPerKtA, fb);
+                    i8_bulk_g2s(dst + kBOff, b + (size_t)kt * kPerKtB, (uint32_t)kPerKtB, fb);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ------------------------------------------------------------------ MMA issuer: 36 products per stage
+        // ------------------------------------------------------------------ MMA issuer
         if (lane == 0) {
             // D = S32 (bits 4-5 = 2), A / B format at bits 7-9 / 10-12 (0 = unsigned 8 bit: the top slice, 1 = signed:
             // the balanced lower slices), K-major, N >> 3 at bit 17, M >> 4 at bit 24
             const uint32_t idesc = (2u << 4) | ((uint32_t)(kI8BN >> 3) << 17) | ((uint32_t)(kI8BM >> 4) << 24);
-            int stage = 0; uint32_t phase = 0, tseq = 0;
-            for (int t = blockIdx.x; t < total_tiles; t += gridDim.x, ++tseq) {
-                i8_mbar_wait(tempty_bar, (tseq & 1) ^ 1);        // the epilogue has drained the previous tile
+            int stage = 0; uint32_t phase = 0, pseq = 0;
+            for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+                // ---- pass 0: diagonals 0..3 into accumulators 0..3
+                i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);        // the epilogue has drained the previous pass
+                ++pseq;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                for (int kt = 0; kt < KT; kt += 2) {
+                    i8_mbar_wait(full_bar + 8 * stage, phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const int nk = min(2, KT - kt);
+                    for (int h = 0; h < nk; ++h) {
+                        const uint32_t sa = sbase + stage * kSlot + h * 16384, sb = sa + kBOff;
+#pragma unroll
+                        for (int d = 0; d < 4; ++d)
+#pragma unroll
+                            for (int s = 0; s <= d; ++s)
+                                umma_i8(tmem_base + d * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
+                                        i8_desc(sb + (d - s) * kI8SliceBytesB, 2048, 128),
+                                        idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u),
+                                        (kt + h > 0 || s > 0) ? 1u : 0u);
+                    }
+                    i8_commit(empty_bar + 8 * stage);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+                i8_commit(tfull_bar);
+                // ---- pass 1: diagonals 4..NS-1 into accumulators 0..NS-5
+                i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);
+                ++pseq;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 for (int kt = 0; kt < KT; ++kt) {
                     i8_mbar_wait(full_bar + 8 * stage, phase);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t sa = sbase + stage * kI8StageBytes, sb = sa + kI8StageBytesA;
+                    const uint32_t sa = sbase + stage * kSlot, sb = sa + kBOff;
 #pragma unroll
-                    for (int d = 0; d < NS; ++d)
+                    for (int d = 4; d < NS; ++d)
 #pragma unroll
                         for (int s = 0; s <= d; ++s)
-                            umma_i8(tmem_base + d * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
-                                    i8_desc(sb + (d - s) * kI8SliceBytesB, 1024, 128),
+                            umma_i8(tmem_base + (d - 4) * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
+                                    i8_desc(sb + (d - s) * kI8SliceBytesB, 2048, 128),
                                     idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u), (kt > 0 || s > 0) ? 1u : 0u);
                     i8_commit(empty_bar + 8 * stage);
-                    if (++stage == kI8Stages) { stage = 0; phase ^= 1; }
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
                 i8_commit(tfull_bar);
             }
         }
     } else {
-        // ------------------------------------------------------------------ epilogue warps 2..5
-        const int q = warp & 3;
+        // ------------------------------------------------------------------ epilogue warps 2..9
+        const int q = warp & 3;                                  // TMEM lane quadrant this warp may read
+        const int half = (warp - 2) >> 2;                        // its 64 of the tile's 128 columns
         const int lrow = 32 * q + lane;
-        const int et = threadIdx.x - 64;                         // 0..127
-        uint32_t tseq = 0;
-        for (int t = blockIdx.x; t < total_tiles; t += gridDim.x, ++tseq) {
+        const int et = threadIdx.x - 64;                         // 0..255
+        uint32_t pseq = 0;
+        for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
             int tm, tn;
             i8_tile_coord(t, W.tiles_m, W.tiles_n, tm, tn);
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            asm volatile("bar.sync 1, 256;" ::: "memory");
             if (et < kI8BN) {        // column constants; columns >= n_rec: all slices are zero, bkg = n = 1/n = 0
                 const int col = tn * kI8BN + et;
                 const bool ok = col < W.n_rec;
@@ -399,39 +451,49 @@ k_fold_i8(const I8Work W)
                 s_inv[et] = n > 0.0 ? 1.0 / n : 0.0;
                 s_scl[et] = ok ? ldexp(1.0, W.f_col[col]) : 0.0;
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            asm volatile("bar.sync 1, 256;" ::: "memory");
             const int64_t row = (int64_t)tm * kI8BM + lrow;
             const int e = W.e_row[row];
             const double rscale = (e == kI8BadRow) ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, e - 14);
-            const double step = 0.00390625;                      // 2^-8 between neighbouring diagonals
-            i8_mbar_wait(tfull_bar, tseq & 1);
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + 64 * half;
+            double v[4][16];
+            // ---- pass 0: v = sum_{d=0..3} 2^(-8d) acc_d, kept in registers
+            i8_mbar_wait(tfull_bar, pseq & 1);
+            ++pseq;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16);
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+#pragma unroll
+                for (int d = 3; d >= 0; --d) i8_horner16(taddr + d * kI8BN + 16 * g, v[g], d == 3);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) i8_mbar_arrive(tempty_bar);
+            // ---- pass 1: v += 2^-32 sum_{d=4..NS-1} 2^(-8(d-4)) acc_(d-4)
+            i8_mbar_wait(tfull_bar, pseq & 1);
+            ++pseq;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                double u[16];
+#pragma unroll
+                for (int d = NS - 1; d >= 4; --d) i8_horner16(taddr + (d - 4) * kI8BN + 16 * g, u, d == NS - 1);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) v[g][j] = fma(u[j], 2.3283064365386963e-10 /* 2^-32 */, v[g][j]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) i8_mbar_arrive(tempty_bar);           // the next tile's products run under the Poisson terms
             double tot = 0.0;
-#pragma unroll 1
-            for (int g = 0; g < kI8BN / 16; ++g) {
-                double v[16];
-                {   // Horner over the diagonals d = NS-1 .. 0: v = sum_d 2^(-8 d) acc_d, exact int32 -> double
-                    uint32_t a[16];
-                    tmem_ld16(taddr + (NS - 1) * kI8BN + 16 * g, a);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) v[j] = (double)(int)a[j];
-#pragma unroll
-                    for (int d = NS - 2; d >= 0; --d) {
-                        tmem_ld16(taddr + d * kI8BN + 16 * g, a);
-                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) v[j] = fma(v[j], step, (double)(int)a[j]);
-                    }
-                }
+            for (int g = 0; g < 4; ++g) {
 #pragma unroll
                 for (int j = 0; j < 16; j += 4) {
-                    const int c0 = 16 * g + j;
-                    const double m0 = fma(v[j] * rscale, s_scl[c0], s_bkg[c0]);
-                    const double m1 = fma(v[j + 1] * rscale, s_scl[c0 + 1], s_bkg[c0 + 1]);
-                    const double m2 = fma(v[j + 2] * rscale, s_scl[c0 + 2], s_bkg[c0 + 2]);
-                    const double m3 = fma(v[j + 3] * rscale, s_scl[c0 + 3], s_bkg[c0 + 3]);
+                    const int c0 = 64 * half + 16 * g + j;
+                    const double m0 = fma(v[g][j] * rscale, s_scl[c0], s_bkg[c0]);
+                    const double m1 = fma(v[g][j + 1] * rscale, s_scl[c0 + 1], s_bkg[c0 + 1]);
+                    const double m2 = fma(v[g][j + 2] * rscale, s_scl[c0 + 2], s_bkg[c0 + 2]);
+                    const double m3 = fma(v[g][j + 3] * rscale, s_scl[c0 + 3], s_bkg[c0 + 3]);
                     if (W.out_mu && row < W.Pc) {
                         const int col = tn * kI8BN + c0;
                         double *dst = W.out_mu + ((size_t)row * W.D + W.d) * W.n_rec + col;
@@ -444,10 +506,7 @@ k_fold_i8(const I8Work W)
                                         s_inv[c0], s_inv[c0 + 1], s_inv[c0 + 2], s_inv[c0 + 3]);
                 }
             }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) i8_mbar_arrive(tempty_bar);
-            if (row < W.Pc) W.partial[(size_t)tn * W.part_stride + row] = tot;
+            if (row < W.Pc) W.partial[(size_t)(2 * tn + half) * W.part_stride + row] = tot;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -460,8 +519,8 @@ k_fold_i8(const I8Work W)
 int i8_setup(rw_ctx *ctx, cudaStream_t s)
 {
     const Layout &L = ctx->lay;
-    const int KT = L.KT8, n_cols = L.NT8 * kI8BN;
-    const size_t per = (size_t)L.NT8 * KT * L.ns8 * kI8SliceBytesB;
+    const int KT = L.KT8, n_cols = L.NT8 * 64;                  // NT8 counts 64-column units and is even
+    const size_t per = (size_t)(L.NT8 / 2) * KT * L.ns8 * kI8SliceBytesB;
     for (int d = 0; d < ctx->D; ++d) {
         const double *Rd = ctx->R + (size_t)d * ctx->R_period_stride;
         int *f = ctx->f_col8 + (size_t)d * ctx->n_rec, *tau = ctx->tau8 + (size_t)d * ctx->n_T;
@@ -472,8 +531,8 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
         ctx->launches += 3;
     }
     if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "slicing R failed at launch");
-    cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_smem(8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_smem(7));
+    cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_i8): %s", cudaGetErrorString(e));
     return RW_OK;
 }
@@ -494,22 +553,22 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     ctx->launches += 2;
     I8Work W;
     W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d;
-    W.tiles_m = (int)(rows_pad / kI8BM); W.tiles_n = L.NT8;
+    W.tiles_m = (int)(rows_pad / kI8BM); W.tiles_n = L.NT8 / 2;
     W.Pc = Pc; W.part_stride = L.MC;
     W.As = As;
-    W.Bs = ctx->B8 + (size_t)d * L.NT8 * KT * L.ns8 * kI8SliceBytesB;
+    W.Bs = ctx->B8 + (size_t)d * (L.NT8 / 2) * KT * L.ns8 * kI8SliceBytesB;
     W.e_row = ctx->e_row8;
     W.f_col = ctx->f_col8 + (size_t)d * ctx->n_rec;
     W.bkg = ctx->bkg + (size_t)d * ctx->n_rec;
     W.counts = ctx->counts + (size_t)d * ctx->n_rec;
-    W.partial = ctx->partial + (size_t)d * L.NT8 * L.MC;       // [D][NT8][MC]: 64-column tiles in this mode
+    W.partial = ctx->partial + (size_t)d * L.NT8 * L.MC;       // [D][NT8][MC]: 64-column half tiles in this mode
     W.out_mu = out_mu;
     const int total = W.tiles_m * W.tiles_n;
     const int grid = total < ctx->num_sms ? total : ctx->num_sms;
     {
         ProfScope prof(ctx, s);
-        if (L.ns8 == 8) k_fold_i8<8><<<grid, kI8Threads, i8_smem(8), s>>>(W);
-        else k_fold_i8<7><<<grid, kI8Threads, i8_smem(7), s>>>(W);
+        if (L.ns8 == 8) k_fold_i8<8><<<grid, kI8Threads, kI8Smem, s>>>(W);
+        else k_fold_i8<7><<<grid, kI8Threads, kI8Smem, s>>>(W);
     }
     ctx->launches++;
     return cudaGetLastError();
