@@ -20,11 +20,11 @@
 // else, so the error is a bound in terms of the scales, not of the individual mu: for responses whose columns
 // spread over many recoil bins (all BASELINE configurations) it is < 1e-13 of mu; see DESIGN.md section 3.3.
 //
-// One CTA per SM, 192 threads as in rw_fold_tf32.cu (TMA warp, MMA warp, 4 epilogue warps), tile 128 points x 64
-// bins, 32 recoil bins per stage.  The slices are stored in global memory already in the tensor core's canonical
-// K-major no-swizzle layout (8 x 16-byte core matrices), all slices of a (tile, k-block) contiguous: a stage is
-// two plain bulk copies (NS x 4 KB of N' slices, NS x 2 KB of R slices).  NS TMEM accumulators (one per s + t) x
-// 64 columns; the epilogue combines them in FP64 (Horner) and evaluates the Poisson terms of Eq. (18).
+// One CTA per SM, 320 threads (TMA warp, MMA warp, 8 epilogue warps), tile 128 points x 128 bins, 32 recoil bins per
+// k-block.  The slices are stored in global memory already in the tensor core's canonical K-major no-swizzle layout
+// (8 x 16-byte core matrices), all slices of a (tile, k-block) contiguous: a stage is plain bulk copies into a 64 KB
+// slot.  One 128-column TMEM accumulator per diagonal s + t, four at a time (two passes, see k_fold_i8); the
+// epilogue combines them in FP64 (Horner) and evaluates the Poisson terms of Eq. (18).
 #include <limits.h>
 
 #include "rw_internal.h"
