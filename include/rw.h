@@ -83,7 +83,9 @@ enum {
                                   (8 balanced base-256 digits for n_T <= 8192, else 7: 63 / 55 bits below their own maximum),
                                   36 / 28 INT8 tensor-core products per 32 recoil bins with exact int32 accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
                                   one: ~1e-13 of mu for responses spread over many recoil bins.
-                                  Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point). */
+                                  Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point).  Accepted by
+                                  rw_eval_batch, rw_eval_profile, rw_eval_weights and rw_eval_pee (dense fold only; the
+                                  streaming and collapsed regimes ignore it); rw_eval_grad refuses it. */
 };
 
 /* rw_inputs.create_flags */

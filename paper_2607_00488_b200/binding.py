@@ -246,7 +246,7 @@ class Reweighter:
         self._last_param = param          # keep alive until the stream has consumed it
         return (out, out_mu) if (want_mu or out_mu is not None) else out
 
-    def eval_profile(self, param, kinds, s0=1.0, sigma=0.0, full_eq18=False, mode="auto"):
+    def eval_profile(self, param, kinds, s0=1.0, sigma=0.0, full_eq18=False, mode="auto", sliced=False):
         """(-2lnL[P] with the overall signal normalisation profiled out, s_hat[P]) for CUDA param[P][k]
         (rw_eval_profile); sigma > 0 adds the Gaussian pull ((s - s0)/sigma)^2."""
         if not (isinstance(param, torch.Tensor) and param.is_cuda):
@@ -259,14 +259,14 @@ class Reweighter:
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         scale = torch.empty(P, dtype=torch.float64, device=self.device)
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
         rc = self._L.rw_eval_profile(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, float(s0), float(sigma),
                                      C.c_void_p(out.data_ptr()), C.c_void_p(scale.data_ptr()), flags, _stream_ptr())
         self._check(rc, self._ctx)
         self._last_param = param
         return out, scale
 
-    def eval_pee(self, param, kinds, P_e_pts, want_mu=False, full_eq18=False, mode="auto"):
+    def eval_pee(self, param, kinds, P_e_pts, want_mu=False, full_eq18=False, mode="auto", sliced=False):
         """-2lnL[P] (and mu) with a survival-probability table per point, P_e_pts[P][n_E] (CUDA tensors; rw_eval_pee)."""
         if not (isinstance(param, torch.Tensor) and param.is_cuda and isinstance(P_e_pts, torch.Tensor) and P_e_pts.is_cuda):
             raise RwError(-4, "eval_pee needs CUDA tensors param[P][k] and P_e_pts[P][n_E]")
@@ -279,7 +279,7 @@ class Reweighter:
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device) if want_mu else None
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
         rc = self._L.rw_eval_pee(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, C.c_void_p(pts.data_ptr()),
                                  C.c_void_p(out.data_ptr()), C.c_void_p(mu.data_ptr()) if want_mu else None,
                                  flags, _stream_ptr())
@@ -306,7 +306,7 @@ class Reweighter:
         self._last_param = param
         return out, grad
 
-    def eval_weights(self, w, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto"):
+    def eval_weights(self, w, out=None, out_mu=None, want_mu=False, full_eq18=False, mode="auto", sliced=False):
         """-2lnL[P] for caller-supplied weights w[P][n_T] (CUDA float64 tensor): the dense fold on arbitrary
         weights (rw_eval_weights).  Asynchronous on the current stream."""
         if not (isinstance(w, torch.Tensor) and w.is_cuda):
@@ -320,7 +320,7 @@ class Reweighter:
             out = torch.empty(P, dtype=torch.float64, device=self.device)
         if want_mu and out_mu is None:
             out_mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device)
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
         rc = self._L.rw_eval_weights(self._ctx, C.c_void_p(w.data_ptr()), P, C.c_void_p(out.data_ptr()),
                                      C.c_void_p(out_mu.data_ptr()) if out_mu is not None else None,
                                      flags, _stream_ptr())

@@ -200,6 +200,20 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
     return RW_OK;
 }
 
+// Contraction regime asked for by the flags: 0 = FP64 DMMA, 1 = RW_FP32, 2 = RW_SLICED.
+static int pick_prec(rw_ctx *ctx, const char *fn, uint32_t flags, bool fp32_ok, int *prec)
+{
+    const bool fp32 = flags & RW_FP32, sliced = flags & RW_SLICED;
+    if (fp32 && !fp32_ok) return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 is not supported here", fn);
+    if (fp32 && !ctx->lay.fp32)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 needs a context created with RW_CREATE_FP32", fn);
+    if (sliced && (!ctx->lay.sliced || fp32))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_SLICED needs a context created with RW_CREATE_SLICED "
+                                             "and excludes RW_FP32", fn);
+    *prec = sliced ? 2 : (fp32 ? 1 : 0);
+    return RW_OK;
+}
+
 static int check_kinds(rw_ctx *ctx, const char *fn, int32_t k, const int32_t *param_kind, int *kinds)
 {
     for (int a = 0; a < k; ++a) {
@@ -449,13 +463,8 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
     if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_MODE_COLLAPSED needs a single signal component");
-    const bool fp32 = flags & RW_FP32, sliced = flags & RW_SLICED;
-    if (fp32 && !ctx->lay.fp32)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_FP32 needs a context created with RW_CREATE_FP32");
-    if (sliced && (!ctx->lay.sliced || fp32))
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_SLICED needs a context created with RW_CREATE_SLICED "
-                                             "and excludes RW_FP32");
-    const int prec = sliced ? 2 : (fp32 ? 1 : 0);
+    int prec = 0;
+    { int rc = pick_prec(ctx, "rw_eval_batch", flags, true, &prec); if (rc != RW_OK) return rc; }
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -515,13 +524,15 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
     { int rc = check_kinds(ctx, "rw_eval_profile", k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool full = flags & RW_FULL_EQ18;
+    int prec = 0;
+    { int rc = pick_prec(ctx, "rw_eval_profile", flags, true, &prec); if (rc != RW_OK) return rc; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
     // passes of <= prof_rows points: fold with mu written to the scratch, then one CTA per point profiles s
     for (int64_t q0 = 0; q0 < P; q0 += L.prof_rows) {
         const int64_t Pq = (P - q0 < L.prof_rows) ? P - q0 : L.prof_rows;
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
-        int rc = fold_slice(ctx, Pq, mode, false, ctx->out_stage, ctx->mu_prof, s);
+        int rc = fold_slice(ctx, Pq, mode, false, ctx->out_stage, ctx->mu_prof, s, prec);
         if (rc != RW_OK) return rc;
         RW_CUDA(ctx, launch_profile(ctx, ctx->mu_prof, Pq, s0, sigma, full, out_m2lnL + q0,
                                     out_scale ? out_scale + q0 : nullptr, s));
@@ -537,8 +548,9 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
     if (P == 0) return RW_OK;
     if (!out_m2lnL || !out_grad || !param || !param_kind)
         return fail(ctx, RW_ERR_INVALID, "rw_eval_grad: param, param_kind, out_m2lnL or out_grad is NULL");
-    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32))
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers and RW_FP32 are not supported");
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32 | RW_SLICED))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers, RW_FP32 and RW_SLICED are not supported "
+                                             "(derivative rows change sign)");
     int kinds[RW_N_KINDS];
     { int rc = check_kinds(ctx, "rw_eval_grad", k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
@@ -564,7 +576,7 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
 
 // Dense fold + likelihood for P rows of caller-visible weights w[P][n_T] (device).
 static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, bool full, double *out, double *out_mu,
-                        cudaStream_t s)
+                        cudaStream_t s, int prec)
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
@@ -581,10 +593,14 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             const int64_t Pc = (P - c0 < L.MC) ? P - c0 : L.MC;
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
-                RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
-                RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                if (prec == 2) {
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, 0, Pc, mu, s, w + (size_t)c0 * n_T));
+                } else {
+                    RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
+                    RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                }
             }
-            RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, out + c0, full, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * (prec == 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, out + c0, full, s));
         }
     }
     return RW_OK;
@@ -601,7 +617,9 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
     if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32)))
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_weights: collapsed mode, RW_FP32 and host buffers are not supported "
                                              "(arbitrary weights are not low-rank; w is a device array)");
-    return weights_rows(ctx, w, P, mode, flags & RW_FULL_EQ18, out_m2lnL, out_mu, (cudaStream_t)cuda_stream);
+    int prec = 0;
+    { int rc = pick_prec(ctx, "rw_eval_weights", flags, false, &prec); if (rc != RW_OK) return rc; }
+    return weights_rows(ctx, w, P, mode, flags & RW_FULL_EQ18, out_m2lnL, out_mu, (cudaStream_t)cuda_stream, prec);
 }
 
 int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
@@ -618,8 +636,9 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
     if (ctx->n_comp > 1 || ctx->have_mu_tau)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: needs a single component created without explicit P_mu/P_tau "
                                              "(the point's 1 - P_e is split by f_tau)");
-    int kinds[RW_N_KINDS];
+    int kinds[RW_N_KINDS], prec = 0;
     { int rc = check_kinds(ctx, "rw_eval_pee", k, param_kind, kinds); if (rc != RW_OK) return rc; }
+    { int rc = pick_prec(ctx, "rw_eval_pee", flags, false, &prec); if (rc != RW_OK) return rc; }
     for (int a = 0; a < k; ++a)
         if (kinds[a] >= RW_RATE_0) return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: rate kinds are not accepted");
     cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -634,7 +653,7 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
         RW_CUDA(ctx, launch_weights_pee(ctx, P_e_pts + (size_t)q0 * ctx->n_E, Pq, ctx->mu_prof, s));
         int rc = weights_rows(ctx, ctx->mu_prof, Pq, mode, flags & RW_FULL_EQ18, out_m2lnL + q0,
-                              out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s);
+                              out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s, prec);
         if (rc != RW_OK) return rc;
     }
     return RW_OK;

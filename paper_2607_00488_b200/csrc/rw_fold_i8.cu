@@ -68,7 +68,9 @@ __device__ __forceinline__ int i8_exponent(double vmax)          // smallest e w
 // warp); XOR-ing the low 4 index bits with the 16-bin group number spreads 16 lanes over 16 banks
 __device__ __forceinline__ int i8_sw(int ii) { return ii ^ ((ii >> 4) & 15); }
 
-template <int PASS>
+// SRC 1 (rw_eval_weights, rw_eval_pee): N'[p][i] = w[p][i] N_mc[i] from caller-visible weights instead (`What` is
+// N_mc[n_T] of the period then, `coef` the weights of the chunk's first point).
+template <int PASS, int SRC>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
           int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
@@ -81,12 +83,12 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
     __shared__ double sRate[8][RW_MAX_COMPONENTS];
     const int r = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + r;
-    if (threadIdx.x < 8 * kCoefStride) {
+    if (SRC == 0 && threadIdx.x < 8 * kCoefStride) {
         const int rr = threadIdx.x / kCoefStride, b = threadIdx.x - rr * kCoefStride;
         const int64_t q = (int64_t)blockIdx.x * 8 + rr;
         sC[rr][b] = (q < Pc) ? coef[(p0 + q) * kCoefStride + b] : 0.0;
     }
-    if (threadIdx.x < 8 * RW_MAX_COMPONENTS) {
+    if (SRC == 0 && threadIdx.x < 8 * RW_MAX_COMPONENTS) {
         const int rr = threadIdx.x / RW_MAX_COMPONENTS, cq = threadIdx.x % RW_MAX_COMPONENTS;
         const int64_t q = (int64_t)blockIdx.x * 8 + rr;
         sRate[rr][cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
@@ -98,12 +100,12 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
     const int n_pad = KT * kI8BK;
     for (int i0 = 0; i0 < n_pad; i0 += 512) {
         __syncthreads();
-        for (int q = threadIdx.x; q < kNumTerms * 512; q += 256) {
+        for (int q = threadIdx.x; q < (SRC == 0 ? kNumTerms : 1) * 512; q += 256) {
             const int b = q >> 9, ii = q & 511, i = i0 + ii;
-            sW[b][i8_sw(ii)] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;
+            sW[b][i8_sw(ii)] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;       // SRC 1: row 0 = N_mc
         }
         for (int q = threadIdx.x; q < 512; q += 256) {
-            sComp[q] = (i0 + q < n_T) ? comp8[i0 + q] : 0;
+            sComp[q] = (SRC == 0 && i0 + q < n_T) ? comp8[i0 + q] : 0;
             sScl[i8_sw(q)] = (i0 + q < n_T) ? ldexpf(1.0f, -tau[i0 + q]) : 1.0f;
         }
         __syncthreads();
@@ -115,9 +117,13 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             double v = 0.0;
+            if (SRC == 0) {
 #pragma unroll
-            for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][i8_sw(ii0 + j)], v);
-            v = v * sRate[r][(cws[j >> 2] >> (8 * (j & 3))) & 0xffu] * (double)sScl[i8_sw(ii0 + j)];   // N' / 2^tau_i
+                for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][i8_sw(ii0 + j)], v);
+                v = v * sRate[r][(cws[j >> 2] >> (8 * (j & 3))) & 0xffu] * (double)sScl[i8_sw(ii0 + j)];   // N' / 2^tau_i
+            } else if (row < Pc && ibase + j < n_T) {
+                v = coef[(size_t)row * n_T + ibase + j] * sW[0][i8_sw(ii0 + j)] * (double)sScl[i8_sw(ii0 + j)];
+            }
             if (PASS == 0) {
                 if (!(v >= 0.0) || isinf(v)) bad = true;
                 vmax = fmax(vmax, v);
@@ -538,7 +544,8 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
 }
 
 // Steps a1-a4 for the Pc points at coef[p0..] and period d through the sliced INT8 contraction.
-cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s)
+// With `w` (weights of the chunk's Pc points, [Pc][n_T]) the rows are N' = w N_mc instead of the coefficient rows.
+cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s, const double *w)
 {
     const Layout &L = ctx->lay;
     const int KT = L.KT8;
@@ -546,10 +553,17 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     uint8_t *As = reinterpret_cast<uint8_t *>(ctx->A_packed);     // 8 slice bytes per (point, bin): fits the FP64 N'
     const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
     const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
-    k_slice_A<0><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
-                                                         L.ns8, ctx->e_row8, As);
-    k_slice_A<1><<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT,
-                                                         L.ns8, ctx->e_row8, As);
+    const unsigned sgrid = (unsigned)(rows_pad / 8);
+    if (w) {
+        const double *N_mc = ctx->N_mc + (size_t)d * ctx->n_T;
+        k_slice_A<0, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, ctx->e_row8, As);
+        k_slice_A<1, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, ctx->e_row8, As);
+    } else {
+        k_slice_A<0, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
+                                              ctx->e_row8, As);
+        k_slice_A<1, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
+                                              ctx->e_row8, As);
+    }
     ctx->launches += 2;
     I8Work W;
     W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d;

@@ -60,7 +60,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
     bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
     int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 8192 (int32 accumulation stays exact), else 7
-    int KT8, NT8;         // k-blocks of 32 recoil bins, column tiles of 64 bins (rw_fold_i8.cu)
+    int KT8, NT8;         // k-blocks of 32 recoil bins; 64-column units = 2 x (128-column tiles) (rw_fold_i8.cu)
     bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
@@ -93,7 +93,7 @@ struct rw_ctx {
     int *flag;
     // per-call scratch
     double *param_stage, *coef, *A_packed, *partial, *mu_part, *out_stage, *mu_stage;
-    uint8_t *B8;              // [D][NT8][KT8][8 slices][2 KB] INT8 slices of R (RW_CREATE_SLICED)
+    uint8_t *B8;              // [D][NT8 / 2][KT8][ns8 slices][4 KB] INT8 slices of R (RW_CREATE_SLICED)
     int *f_col8, *e_row8;     // column exponents [D][n_rec]; row exponents of the current chunk [MC]
     int *tau8;                // [D][n_T] per-bin rescaling exponents (2^tau ~ N_mc)
     float *R32;               // [D][2 (hi, lo)][n_rec][KP32] transposed TF32 split of R (RW_CREATE_FP32)
@@ -152,7 +152,8 @@ cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k,
 cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,
                         double *grad, cudaStream_t s);                       // rw_grad.cu
 int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
-cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);    // rw_fold_i8.cu
+cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s,
+                           const double *w = nullptr);    // rw_fold_i8.cu
 int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
 cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,

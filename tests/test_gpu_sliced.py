@@ -94,3 +94,60 @@ def test_sliced_components_rates_and_bad_points(orc):
         plain.eval_batch(_cuda(params[:8]), kinds, mode="gemm", sliced=True)
     plain.close()
     ctx.close()
+
+
+def test_sliced_weights_profile_and_pee(orc):
+    """RW_SLICED through the other entry points that feed the dense fold non-negative rows: rw_eval_weights
+    (N' = w N_mc sliced from caller weights, a zero-weight stretch and an all-zero row included), rw_eval_profile
+    (mu of the sliced fold into the profiling kernel) and rw_eval_pee; rw_eval_grad refuses it (derivative rows
+    change sign)."""
+    import torch
+    from paper_2607_00488_b200 import binding
+    inp = wl.make_custom(n_E=300, n_T=203, n_rec=330, n_periods=2, seed=121, dead_fraction=0.1)
+    ctx = binding.Reweighter(inp, max_batch=160, sliced=True)
+    # weights
+    P = 150
+    w = np.random.default_rng(122).uniform(0.0, 3.0, size=(P, 203))
+    w[0, :7] = 0.0
+    w[3] = 0.0
+    ref, mu_ref, scale = orc.eval_weights(inp, w, want_mu=True, want_abs=True, nthreads=CORES)
+    out, mu = ctx.eval_weights(_cuda(w), want_mu=True, mode="gemm", sliced=True)
+    torch.cuda.synchronize()
+    out, mu = out.cpu().numpy(), mu.cpu().numpy()
+    assert (np.abs(mu - mu_ref) <= 1e-12 * np.abs(mu_ref)).all(), (np.abs(mu - mu_ref) / np.abs(mu_ref)).max()
+    assert np.all(np.abs(out - ref) <= 1e-9 + 1e-12 * scale)
+    # profiled normalisation with a pull
+    params, kinds = wl.random_points(45, [wl.EPS_EE_L, wl.EPS_EE_R, wl.EPS_TT_L, wl.MU_NU], seed=123)
+    ref, sc_ref, scale = orc.eval_profile(inp, params, kinds, s0=1.0, sigma=0.05, want_abs=True, nthreads=CORES)
+    out, sc = ctx.eval_profile(_cuda(params), kinds, s0=1.0, sigma=0.05, mode="gemm", sliced=True)
+    torch.cuda.synchronize()
+    out, sc = out.cpu().numpy(), sc.cpu().numpy()
+    assert np.all(np.abs(sc - sc_ref) <= 1e-10 * np.maximum(sc_ref, 1e-3)), np.abs(sc - sc_ref).max()
+    assert np.all(np.abs(out - ref) <= 1e-9 + 1e-12 * (scale + np.abs(ref)))
+    # survival-probability table per point
+    rng = np.random.default_rng(124)
+    Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.25, 0.25, size=(45, 300)), 0.0, 1.0)
+    ref, mu_ref, scale = orc.eval_pee(inp, params, kinds, Pp, want_mu=True, want_abs=True, nthreads=CORES)
+    out, mu = ctx.eval_pee(_cuda(params), kinds, _cuda(Pp), want_mu=True, mode="gemm", sliced=True)
+    torch.cuda.synchronize()
+    out, mu = out.cpu().numpy(), mu.cpu().numpy()
+    assert (np.abs(mu - mu_ref) <= 1e-12 * np.abs(mu_ref)).all(), (np.abs(mu - mu_ref) / np.abs(mu_ref)).max()
+    assert np.all(np.abs(out - ref) <= 1e-9 + 1e-12 * scale)
+    # negative weights cannot be sliced: that point is NaN, the others are unaffected
+    wneg = w[:20].copy()
+    wneg[4, 10] = -0.5
+    out = ctx.eval_weights(_cuda(wneg), mode="gemm", sliced=True)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    assert np.isnan(out[4]) and np.all(np.isfinite(np.delete(out, 4)))
+    with pytest.raises(binding.RwError):
+        flags = binding.RW_SLICED
+        import ctypes as C
+        p = _cuda(params)
+        o = torch.empty(45, dtype=torch.float64, device="cuda")
+        g = torch.empty((45, 4), dtype=torch.float64, device="cuda")
+        ka = (C.c_int32 * 4)(*[int(x) for x in kinds])
+        rc = ctx._L.rw_eval_grad(ctx._ctx, C.c_void_p(p.data_ptr()), 45, 4, ka, C.c_void_p(o.data_ptr()),
+                                 C.c_void_p(g.data_ptr()), flags, None)
+        ctx._check(rc, ctx._ctx)
+    ctx.close()
