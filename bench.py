@@ -365,6 +365,14 @@ def main():
         _, mu8 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm", sliced=True)
         _, mu64 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm")
         rel = ((mu8 - mu64).abs() / mu64.abs())
+        # RW_SLICED_FAST: the top four slices of the same operands (10 products), the FP32 bar
+        out_f = torch.empty(P, dtype=torch.float64, device=dev)
+        t_f = timed(lambda: ctx.eval_batch(param_dev, kinds, out=out_f, sliced="fast"), 5)
+        _, muf = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm", sliced="fast")
+        relf = ((muf - mu64).abs() / mu64.abs())
+        fast_leg = {"ms_per_call": t_f, "evals_per_s": P / t_f * 1e3,
+                    "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_f / 1e9,
+                    "mu_rel_err_vs_fp64_max": float(relf.max().item()), "int8_products_per_k_step": 10}
         n_sl = 8 if n_T <= 8192 else 7                              # balanced 8-bit slices per operand (rw_fold_i8.cu)
         n_prod = n_sl * (n_sl + 1) // 2
         sliced_leg = {"ms_per_call": t_s, "evals_per_s": P / t_s * 1e3, "bound": "tensor (int8)",
@@ -373,7 +381,7 @@ def main():
                       "executed_int8_tops": 2.0 * n_prod * n_T * n_rec * D * P / t_s / 1e9,
                       "mu_rel_diff_vs_dmma_max": float(rel.max().item()),
                       "max_abs_diff_m2lnL_vs_dmma": float((out_s - out_dev).abs().max().item()),
-                      "slices": n_sl, "int8_products_per_k_step": n_prod,
+                      "slices": n_sl, "int8_products_per_k_step": n_prod, "fast": fast_leg,
                       "note": "%d balanced 8-bit slices per operand, %d tcgen05.mma.kind::i8 products per k-step with exact "
                               "int32 accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % (n_sl, n_prod, dmma_peak0)}
 

@@ -79,13 +79,18 @@ enum {
                                   fold): operands split in two TF32 pieces, three tcgen05 tensor-core products, FP32
                                   accumulation in 128-bin chunks; mu within 1e-5 relative of the FP64 path (values below
                                   the FP32 range flush to 0).  Needs a context created with RW_CREATE_FP32. */
-    RW_SLICED      = 1u << 11  /* opt-in FP64-by-slicing for the batched contraction: rows of N' and columns of R in fixed point
+    RW_SLICED      = 1u << 11, /* opt-in FP64-by-slicing for the batched contraction: rows of N' and columns of R in fixed point
                                   (8 balanced base-256 digits for n_T <= 8192, else 7: 63 / 55 bits below their own maximum),
                                   36 / 28 INT8 tensor-core products per 32 recoil bins with exact int32 accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
                                   one: ~1e-13 of mu for responses spread over many recoil bins.
                                   Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point).  Accepted by
                                   rw_eval_batch, rw_eval_profile, rw_eval_weights and rw_eval_pee (dense fold only; the
                                   streaming and collapsed regimes ignore it); rw_eval_grad refuses it. */
+    RW_SLICED_FAST = 1u << 12  /* opt-in reduced precision on the same slices: only their top four (31-bit fixed point) and
+                                  the four leading diagonals, 10 INT8 products per 32 recoil bins.  Error
+                                  ~1e-9 (row max)(column max) n_T per bin: mu within 1e-5 relative wherever RW_SLICED
+                                  holds 1e-12 (the FP32 bar of this library).  Same requirements and scope as RW_SLICED,
+                                  which it excludes. */
 };
 
 /* rw_inputs.create_flags */

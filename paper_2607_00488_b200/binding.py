@@ -21,7 +21,7 @@ RW_RATE_0 = 7        # RW_RATE_0 + c: rate scale of signal component c
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
 RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED = 0, 1 << 4, 2 << 4, 3 << 4
-RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED = 1 << 8, 1 << 9, 1 << 10, 1 << 11
+RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED, RW_SLICED_FAST = 1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12
 RW_CREATE_FP32, RW_CREATE_SLICED = 1, 2
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED}
@@ -45,6 +45,13 @@ class rw_inputs(C.Structure):
                 ("N_mc", C.c_void_p), ("R", C.c_void_p), ("bkg", C.c_void_p), ("counts", C.c_void_p),
                 ("consts", rw_constants), ("mem_kind", C.c_int32), ("create_flags", C.c_uint32),
                 ("n_comp", C.c_int32), ("comp_of_T", C.c_void_p)]
+
+
+def _sliced_flag(sliced):
+    """sliced = False | True (FP64-grade, RW_SLICED) | "fast" (top four slices, FP32-grade, RW_SLICED_FAST)."""
+    if sliced == "fast":
+        return RW_SLICED_FAST
+    return RW_SLICED if sliced else 0
 
 
 class RwError(RuntimeError):
@@ -214,7 +221,7 @@ class Reweighter:
         (pinned), valid after the stream is synchronised."""
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_FP32 if fp32 else 0) | \
-            (RW_SLICED if sliced else 0)
+            _sliced_flag(sliced)
         host = not (isinstance(param, torch.Tensor) and param.is_cuda)
         if host:
             if isinstance(param, np.ndarray):
@@ -259,7 +266,7 @@ class Reweighter:
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         scale = torch.empty(P, dtype=torch.float64, device=self.device)
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | _sliced_flag(sliced)
         rc = self._L.rw_eval_profile(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, float(s0), float(sigma),
                                      C.c_void_p(out.data_ptr()), C.c_void_p(scale.data_ptr()), flags, _stream_ptr())
         self._check(rc, self._ctx)
@@ -279,7 +286,7 @@ class Reweighter:
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device) if want_mu else None
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | _sliced_flag(sliced)
         rc = self._L.rw_eval_pee(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr, C.c_void_p(pts.data_ptr()),
                                  C.c_void_p(out.data_ptr()), C.c_void_p(mu.data_ptr()) if want_mu else None,
                                  flags, _stream_ptr())
@@ -320,7 +327,7 @@ class Reweighter:
             out = torch.empty(P, dtype=torch.float64, device=self.device)
         if want_mu and out_mu is None:
             out_mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device)
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_SLICED if sliced else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | _sliced_flag(sliced)
         rc = self._L.rw_eval_weights(self._ctx, C.c_void_p(w.data_ptr()), P, C.c_void_p(out.data_ptr()),
                                      C.c_void_p(out_mu.data_ptr()) if out_mu is not None else None,
                                      flags, _stream_ptr())

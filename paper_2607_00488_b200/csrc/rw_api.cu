@@ -158,7 +158,8 @@ static bool auto_stream(const rw_ctx *, int64_t P) { return P <= 4; }
 
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
-// prec: 0 = FP64 DMMA, 1 = TF32 x 3 (RW_FP32), 2 = INT8 slices (RW_SLICED); only the contraction regime differs
+// prec: 0 = FP64 DMMA, 1 = TF32 x 3 (RW_FP32), 2 = INT8 slices (RW_SLICED), 3 = their top four (RW_SLICED_FAST);
+// only the contraction regime differs
 static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s,
                       int prec = 0)
 {
@@ -187,30 +188,32 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             for (int d = 0; d < D; ++d) {
                 if (prec == 1) {
                     RW_CUDA(ctx, launch_fold_tf32(ctx, d, c0, Pc, mu, s));
-                } else if (prec == 2) {
-                    RW_CUDA(ctx, launch_fold_i8(ctx, d, c0, Pc, mu, s));
+                } else if (prec >= 2) {
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, c0, Pc, mu, s, nullptr, prec == 3));
                 } else {
                     RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
                     RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
                 }
             }
-            RW_CUDA(ctx, launch_reduce(ctx, D * (prec == 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, dout + c0, full, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * (prec >= 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, dout + c0, full, s));
         }
     }
     return RW_OK;
 }
 
-// Contraction regime asked for by the flags: 0 = FP64 DMMA, 1 = RW_FP32, 2 = RW_SLICED.
+// Contraction regime asked for by the flags: 0 = FP64 DMMA, 1 = RW_FP32, 2 = RW_SLICED, 3 = RW_SLICED_FAST.
 static int pick_prec(rw_ctx *ctx, const char *fn, uint32_t flags, bool fp32_ok, int *prec)
 {
-    const bool fp32 = flags & RW_FP32, sliced = flags & RW_SLICED;
+    const bool fp32 = flags & RW_FP32, fast = flags & RW_SLICED_FAST, sliced = (flags & RW_SLICED) || fast;
+    if ((flags & RW_SLICED) && fast)
+        return fail(ctx, RW_ERR_INVALID, "%s: RW_SLICED and RW_SLICED_FAST exclude each other", fn);
     if (fp32 && !fp32_ok) return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 is not supported here", fn);
     if (fp32 && !ctx->lay.fp32)
         return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 needs a context created with RW_CREATE_FP32", fn);
     if (sliced && (!ctx->lay.sliced || fp32))
         return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_SLICED needs a context created with RW_CREATE_SLICED "
                                              "and excludes RW_FP32", fn);
-    *prec = sliced ? 2 : (fp32 ? 1 : 0);
+    *prec = fast ? 3 : (sliced ? 2 : (fp32 ? 1 : 0));
     return RW_OK;
 }
 
@@ -548,7 +551,7 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
     if (P == 0) return RW_OK;
     if (!out_m2lnL || !out_grad || !param || !param_kind)
         return fail(ctx, RW_ERR_INVALID, "rw_eval_grad: param, param_kind, out_m2lnL or out_grad is NULL");
-    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32 | RW_SLICED))
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32 | RW_SLICED | RW_SLICED_FAST))
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers, RW_FP32 and RW_SLICED are not supported "
                                              "(derivative rows change sign)");
     int kinds[RW_N_KINDS];
@@ -593,14 +596,14 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             const int64_t Pc = (P - c0 < L.MC) ? P - c0 : L.MC;
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
-                if (prec == 2) {
-                    RW_CUDA(ctx, launch_fold_i8(ctx, d, 0, Pc, mu, s, w + (size_t)c0 * n_T));
+                if (prec >= 2) {
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, 0, Pc, mu, s, w + (size_t)c0 * n_T, prec == 3));
                 } else {
                     RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
                     RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
                 }
             }
-            RW_CUDA(ctx, launch_reduce(ctx, D * (prec == 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, out + c0, full, s));
+            RW_CUDA(ctx, launch_reduce(ctx, D * (prec >= 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, out + c0, full, s));
         }
     }
     return RW_OK;

@@ -74,7 +74,8 @@ template <int PASS, int SRC>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
           int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
-          int ns, int *__restrict__ e_row, uint8_t *__restrict__ As)
+          int ns, int ns_store /*slices written: ns, or 4 for the fast mode*/, int *__restrict__ e_row,
+          uint8_t *__restrict__ As)
 {
     __shared__ double sW[kNumTerms][512];
     __shared__ __align__(16) uint8_t sComp[512];
@@ -138,7 +139,7 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
             uint8_t *base = As + ((size_t)(mt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
             for (int s = 0; s < 8; ++s) {
-                if (s >= ns) break;
+                if (s >= ns_store) break;
                 uint32_t w[4];
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
@@ -320,7 +321,10 @@ __device__ __forceinline__ void i8_horner16(uint32_t taddr, double (&v)[16], boo
 // pass 0 the diagonals 0..3 (10 products per 32 bins, slices 0..3 of both operands), pass 1 the diagonals 4..NS-1
 // (18 or 26 products, all slices).  Eight epilogue warps (lane quadrant x column half) keep the pass-0 Horner sums
 // of their 64 columns in registers until pass 1 has drained.
-template <int NS>
+// FAST (RW_SLICED_FAST): pass 0 only.  Balanced digits round to nearest at every truncation point, so the top four
+// slices of the same operands are the 31-bit fixed-point values and the four diagonals kept are everything above
+// 2^-32 of (row max x column max): an FP32-class result from 10 of the 28 / 36 products.
+template <int NS, bool FAST>
 __global__ void __launch_bounds__(kI8Threads, 1)
 k_fold_i8(const I8Work W)
 {
@@ -375,7 +379,7 @@ k_fold_i8(const I8Work W)
                     }
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
-                for (int kt = 0; kt < KT; ++kt) {
+                for (int kt = 0; kt < (FAST ? 0 : KT); ++kt) {
                     i8_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
                     const uint32_t fb = full_bar + 8 * stage, dst = sbase + stage * kSlot;
                     i8_mbar_expect_tx(fb, (uint32_t)(kPerKtA + kPerKtB));
@@ -416,6 +420,7 @@ k_fold_i8(const I8Work W)
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
                 i8_commit(tfull_bar);
+                if (FAST) continue;
                 // ---- pass 1: diagonals 4..NS-1 into accumulators 0..NS-5
                 i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);
                 ++pseq;
@@ -476,20 +481,22 @@ k_fold_i8(const I8Work W)
             __syncwarp();
             if (lane == 0) i8_mbar_arrive(tempty_bar);
             // ---- pass 1: v += 2^-32 sum_{d=4..NS-1} 2^(-8(d-4)) acc_(d-4)
-            i8_mbar_wait(tfull_bar, pseq & 1);
-            ++pseq;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            if (!FAST) {
+                i8_mbar_wait(tfull_bar, pseq & 1);
+                ++pseq;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-            for (int g = 0; g < 4; ++g) {
-                double u[16];
+                for (int g = 0; g < 4; ++g) {
+                    double u[16];
 #pragma unroll
-                for (int d = NS - 1; d >= 4; --d) i8_horner16(taddr + (d - 4) * kI8BN + 16 * g, u, d == NS - 1);
+                    for (int d = NS - 1; d >= 4; --d) i8_horner16(taddr + (d - 4) * kI8BN + 16 * g, u, d == NS - 1);
 #pragma unroll
-                for (int j = 0; j < 16; ++j) v[g][j] = fma(u[j], 2.3283064365386963e-10 /* 2^-32 */, v[g][j]);
+                    for (int j = 0; j < 16; ++j) v[g][j] = fma(u[j], 2.3283064365386963e-10 /* 2^-32 */, v[g][j]);
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) i8_mbar_arrive(tempty_bar);       // the next tile's products run under the Poisson terms
             }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) i8_mbar_arrive(tempty_bar);           // the next tile's products run under the Poisson terms
             double tot = 0.0;
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
@@ -537,15 +544,18 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
         ctx->launches += 3;
     }
     if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "slicing R failed at launch");
-    cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_i8): %s", cudaGetErrorString(e));
     return RW_OK;
 }
 
 // Steps a1-a4 for the Pc points at coef[p0..] and period d through the sliced INT8 contraction.
 // With `w` (weights of the chunk's Pc points, [Pc][n_T]) the rows are N' = w N_mc instead of the coefficient rows.
-cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s, const double *w)
+cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s, const double *w,
+                           bool fast)
 {
     const Layout &L = ctx->lay;
     const int KT = L.KT8;
@@ -554,15 +564,16 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
     const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
     const unsigned sgrid = (unsigned)(rows_pad / 8);
+    const int nst = fast ? 4 : L.ns8;
     if (w) {
         const double *N_mc = ctx->N_mc + (size_t)d * ctx->n_T;
-        k_slice_A<0, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, ctx->e_row8, As);
-        k_slice_A<1, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, ctx->e_row8, As);
+        k_slice_A<0, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
+        k_slice_A<1, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
     } else {
         k_slice_A<0, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
-                                              ctx->e_row8, As);
+                                              nst, ctx->e_row8, As);
         k_slice_A<1, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
-                                              ctx->e_row8, As);
+                                              nst, ctx->e_row8, As);
     }
     ctx->launches += 2;
     I8Work W;
@@ -581,8 +592,10 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const int grid = total < ctx->num_sms ? total : ctx->num_sms;
     {
         ProfScope prof(ctx, s);
-        if (L.ns8 == 8) k_fold_i8<8><<<grid, kI8Threads, kI8Smem, s>>>(W);
-        else k_fold_i8<7><<<grid, kI8Threads, kI8Smem, s>>>(W);
+        if (L.ns8 == 8 && !fast) k_fold_i8<8, false><<<grid, kI8Threads, kI8Smem, s>>>(W);
+        else if (L.ns8 == 8) k_fold_i8<8, true><<<grid, kI8Threads, kI8Smem, s>>>(W);
+        else if (!fast) k_fold_i8<7, false><<<grid, kI8Threads, kI8Smem, s>>>(W);
+        else k_fold_i8<7, true><<<grid, kI8Threads, kI8Smem, s>>>(W);
     }
     ctx->launches++;
     return cudaGetLastError();

@@ -153,7 +153,7 @@ cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool 
                         double *grad, cudaStream_t s);                       // rw_grad.cu
 int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
 cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s,
-                           const double *w = nullptr);    // rw_fold_i8.cu
+                           const double *w = nullptr, bool fast = false);    // rw_fold_i8.cu
 int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
 cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,

@@ -50,6 +50,11 @@ def _full_vs_sample(orc, name, sample_idx, max_batch, mu_check=True, sliced=Fals
         rel = np.abs(mu_i8.cpu().numpy() - mu_ref) / np.abs(mu_ref)
         assert rel.max() <= 1e-12, "sliced mu rel err %.3e" % rel.max()
         assert np.all(np.abs(out_i8.cpu().numpy() - ref) <= 1e-9 + 1e-12 * scale)
+        # their top four slices only (RW_SLICED_FAST): the FP32 bar
+        _, mu_f = ctx.eval_batch(torch.from_numpy(params[idx]).cuda(), kinds, want_mu=True, mode="gemm", sliced="fast")
+        torch.cuda.synchronize()
+        rel = np.abs(mu_f.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+        assert rel.max() <= 1e-5, "fast sliced mu rel err %.3e" % rel.max()
     ctx.close()
     return err.max()
 

@@ -151,3 +151,49 @@ def test_sliced_weights_profile_and_pee(orc):
                                  C.c_void_p(g.data_ptr()), flags, None)
         ctx._check(rc, ctx._ctx)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------- RW_SLICED_FAST (FP32 bar)
+def _check_fast(orc, inp, params, kinds, max_batch=None, components=False):
+    """Top four slices only: mu within 1e-5 relative, -2lnL within the first-order propagation of that bound
+    (the bar of tests/test_gpu_fp32.py)."""
+    import torch
+    from paper_2607_00488_b200 import binding
+    fn = orc.eval_components if components else orc.eval_batch
+    ref, mu_ref = fn(inp, params, kinds, want_mu=True, nthreads=CORES)
+    ctx = binding.Reweighter(inp, max_batch=max_batch or params.shape[0], sliced=True)
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="gemm", sliced="fast")
+    torch.cuda.synchronize()
+    out, mu = out.cpu().numpy(), mu.cpu().numpy()
+    with pytest.raises(binding.RwError):
+        ctx.eval_batch(_cuda(params), kinds, mode="gemm", fp32=True, sliced="fast")
+    ctx.close()
+    rel = np.abs(mu - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= 1e-5, "fast sliced mu rel err %.3e" % rel.max()
+    counts = np.asarray(inp["counts"], float).reshape(mu_ref.shape[1:])
+    tol = 1e-9 + (2.0 * np.abs(1.0 - counts[None] / mu_ref) * 1e-5 * mu_ref).sum(axis=(1, 2))
+    assert np.all(np.abs(out - ref) <= tol), "fast sliced -2lnL err %.3e (tol %.3e)" % (np.abs(out - ref).max(), tol.min())
+    return rel.max()
+
+
+def test_sliced_fast_small_ragged(orc):
+    inp = wl.make_custom(n_E=31, n_T=203, n_rec=330, n_periods=2, seed=131, dead_fraction=0.1)
+    params, kinds = wl.random_points(300, list(range(7)), seed=132)
+    _check_fast(orc, inp, params, kinds)
+
+
+def test_sliced_fast_long_contraction_seven_slice_layout(orc):
+    """n_T = 8300: the operands are stored as 7 slices, the fast mode reads the first 4 of each k-block."""
+    inp = wl.make_custom(n_E=24, n_T=8300, n_rec=100, n_periods=1, seed=133, tail=0.0)
+    params, kinds = wl.random_points(130, [wl.EPS_EE_L, wl.EPS_MM_R, wl.MU_NU], seed=134)
+    _check_fast(orc, inp, params, kinds, max_batch=64)
+
+
+def test_sliced_fast_config2_and_components(orc):
+    inp = wl.make("cfg2_mm_lowE")
+    params, kinds = wl.scan_points("cfg2_mm_lowE")
+    _check_fast(orc, inp, params, kinds)
+    inp = wl.make_components(n_comp=3, n_E=33, n_T=160, n_rec=140, n_periods=2, seed=135)
+    kinds = np.array([wl.EPS_EE_L, wl.MU_NU, 7, 9], np.int32)
+    params, _ = wl.random_points(70, kinds, seed=136)
+    _check_fast(orc, inp, params, kinds, components=True)
