@@ -385,6 +385,23 @@ def main():
                       "note": "%d balanced 8-bit slices per operand, %d tcgen05.mma.kind::i8 products per k-step with exact "
                               "int32 accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % (n_sl, n_prod, dmma_peak0)}
 
+    # library DGEMM of the shape of one chunk of the fold (cuBLAS FP64 as a reference point for the
+    # denominator).  Context only: no N' generation, no Poisson epilogue, no reduction, and mu goes to HBM.
+    lib_dgemm = None
+    if P > 4 and rank == 0:
+        Pl = int(min(P, max_batch, 32768))
+        try:
+            gen = torch.Generator(device=dev).manual_seed(7)
+            A_l = torch.rand((Pl, n_T), dtype=torch.float64, device=dev, generator=gen)
+            B_l = torch.rand((n_T, n_rec), dtype=torch.float64, device=dev, generator=gen)
+            C_l = torch.empty((Pl, n_rec), dtype=torch.float64, device=dev)
+            t_l = timed(lambda: torch.matmul(A_l, B_l, out=C_l), 3)
+            lib_dgemm = {"shape": [Pl, n_T, n_rec], "ms": t_l, "tflops": 2.0 * Pl * n_T * n_rec / t_l / 1e9,
+                         "note": "torch.matmul float64 (cuBLAS DGEMM), one period, operands resident; not on the product path"}
+            del A_l, B_l, C_l
+        except RuntimeError as exc:                                  # out of memory on a crowded box: context only
+            lib_dgemm = {"unavailable": str(exc)[:120]}
+
     # ---------------------------------------------------------------- roofline of the dominant kernel
     # the probe is taken before the timed region and again here; the higher reading is the denominator (a probe
     # right after the TF32 leg can catch a lower clock)
@@ -423,7 +440,7 @@ def main():
                         "matches_device_path": same},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
                 "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg, "sliced_mode": sliced_leg,
-                "clocks": clocks, "all_finite": finite,
+                "library_dgemm": lib_dgemm, "clocks": clocks, "all_finite": finite,
                 "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
                                  "the authors' own multi-component model; other hardware and inputs, not comparable"}
         print(json.dumps(line))

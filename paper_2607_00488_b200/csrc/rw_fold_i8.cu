@@ -35,7 +35,10 @@ constexpr int kI8BM = 128, kI8BN = 128, kI8BK = 32;
 constexpr int kI8SliceBytesA = kI8BM * kI8BK;                   // 4 KB
 constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 4 KB
 constexpr int kI8Threads = 320;                                 // TMA warp, MMA warp, 8 epilogue warps
-constexpr int kI8SlotBytes = 65536, kI8Stages = 3;              // a slot: N' slices in its first half, R slices in its second
+#ifndef RW_I8_STAGES
+#define RW_I8_STAGES 3
+#endif
+constexpr int kI8SlotBytes = 65536, kI8Stages = RW_I8_STAGES;              // a slot: N' slices in its first half, R slices in its second
 constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 4 * kI8BN * 8 + 256 + 1024;
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
 
