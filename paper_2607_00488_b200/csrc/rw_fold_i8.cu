@@ -73,6 +73,8 @@ __device__ __forceinline__ int i8_sw(int ii) { return ii ^ ((ii >> 4) & 15); }
 
 // SRC 1 (rw_eval_weights, rw_eval_pee): N'[p][i] = w[p][i] N_mc[i] from caller-visible weights instead (`What` is
 // N_mc[n_T] of the period then, `coef` the weights of the chunk's first point).
+constexpr int kI8SliceRows = 16;      // rows per CTA: 2 per warp, so that every staged W^ value read from shared memory serves two rows
+
 template <int PASS, int SRC>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
@@ -80,27 +82,34 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
           int ns, int ns_store /*slices written: ns, or 4 for the fast mode*/, int *__restrict__ e_row,
           uint8_t *__restrict__ As)
 {
+    constexpr int RPW = kI8SliceRows / 8;
     __shared__ double sW[kNumTerms][512];
     __shared__ __align__(16) uint8_t sComp[512];
-    __shared__ float sScl[512];                                  // 2^-tau_i (exact in FP32 too), swizzled like sW
-    __shared__ double sC[8][kCoefStride];
-    __shared__ double sRate[8][RW_MAX_COMPONENTS];
-    const int r = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * 8 + r;
-    if (SRC == 0 && threadIdx.x < 8 * kCoefStride) {
+    __shared__ __align__(16) int8_t sTau[512];                   // tau_i (clamped to +-120 by k_tau)
+    __shared__ double sC[kI8SliceRows][kCoefStride];
+    __shared__ double sRate[kI8SliceRows][RW_MAX_COMPONENTS];
+    const int r0 = (threadIdx.x >> 5) * RPW, lane = threadIdx.x & 31;
+    const int64_t row0 = (int64_t)blockIdx.x * kI8SliceRows + r0;
+    if (SRC == 0 && threadIdx.x < kI8SliceRows * kCoefStride) {
         const int rr = threadIdx.x / kCoefStride, b = threadIdx.x - rr * kCoefStride;
-        const int64_t q = (int64_t)blockIdx.x * 8 + rr;
+        const int64_t q = (int64_t)blockIdx.x * kI8SliceRows + rr;
         sC[rr][b] = (q < Pc) ? coef[(p0 + q) * kCoefStride + b] : 0.0;
     }
-    if (SRC == 0 && threadIdx.x < 8 * RW_MAX_COMPONENTS) {
+    if (SRC == 0 && threadIdx.x < kI8SliceRows * RW_MAX_COMPONENTS) {
         const int rr = threadIdx.x / RW_MAX_COMPONENTS, cq = threadIdx.x % RW_MAX_COMPONENTS;
-        const int64_t q = (int64_t)blockIdx.x * 8 + rr;
+        const int64_t q = (int64_t)blockIdx.x * kI8SliceRows + rr;
         sRate[rr][cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
     }
-    const int e = (PASS == 1) ? e_row[row] : 0;
-    const double scale2 = (PASS == 1 && e != kI8BadRow) ? ldexp(1.0, 8 * ns - 1 - e) : 0.0;
-    double vmax = 0.0;
-    bool bad = false;
+    int e[RPW];
+    double scale2[RPW], vmax[RPW];
+    bool bad[RPW];
+#pragma unroll
+    for (int u = 0; u < RPW; ++u) {
+        e[u] = (PASS == 1) ? e_row[row0 + u] : 0;
+        scale2[u] = (PASS == 1 && e[u] != kI8BadRow) ? ldexp(1.0, 8 * ns - 1 - e[u]) : 0.0;
+        vmax[u] = 0.0;
+        bad[u] = false;
+    }
     const int n_pad = KT * kI8BK;
     for (int i0 = 0; i0 < n_pad; i0 += 512) {
         __syncthreads();
@@ -110,59 +119,85 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
         }
         for (int q = threadIdx.x; q < 512; q += 256) {
             sComp[q] = (SRC == 0 && i0 + q < n_T) ? comp8[i0 + q] : 0;
-            sScl[i8_sw(q)] = (i0 + q < n_T) ? ldexpf(1.0f, -tau[i0 + q]) : 1.0f;
+            sTau[q] = (i0 + q < n_T) ? (int8_t)tau[i0 + q] : (int8_t)0;
         }
         __syncthreads();
-        const int ii0 = lane * 16, ibase = i0 + ii0;             // this thread: 16 consecutive bins of its row
+        const int ii0 = lane * 16, ibase = i0 + ii0;             // this thread: 16 consecutive bins of its rows
         if (ibase >= n_pad) continue;
-        unsigned long long q16[16];
+        unsigned long long q16[RPW][16];
         const uint4 cw = *reinterpret_cast<const uint4 *>(sComp + ii0);
         const uint32_t cws[4] = {cw.x, cw.y, cw.z, cw.w};
+        const uint4 tw = *reinterpret_cast<const uint4 *>(sTau + ii0);
+        const uint32_t tws[4] = {tw.x, tw.y, tw.z, tw.w};
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-            double v = 0.0;
+            const int sj = i8_sw(ii0 + j);
+            const int tj = (int)(int8_t)((tws[j >> 2] >> (8 * (j & 3))) & 0xffu);
+            const double scl = __hiloint2double((1023 - tj) << 20, 0);       // 2^-tau_i, exact
+            double v[RPW];
             if (SRC == 0) {
+                double wv[kNumTerms];
 #pragma unroll
-                for (int b = 0; b < kNumTerms; ++b) v = fma(sC[r][b], sW[b][i8_sw(ii0 + j)], v);
-                v = v * sRate[r][(cws[j >> 2] >> (8 * (j & 3))) & 0xffu] * (double)sScl[i8_sw(ii0 + j)];   // N' / 2^tau_i
-            } else if (row < Pc && ibase + j < n_T) {
-                v = coef[(size_t)row * n_T + ibase + j] * sW[0][i8_sw(ii0 + j)] * (double)sScl[i8_sw(ii0 + j)];
-            }
-            if (PASS == 0) {
-                if (!(v >= 0.0) || isinf(v)) bad = true;
-                vmax = fmax(vmax, v);
+                for (int b = 0; b < kNumTerms; ++b) wv[b] = sW[b][sj];
+                const uint32_t cmp = (cws[j >> 2] >> (8 * (j & 3))) & 0xffu;
+#pragma unroll
+                for (int u = 0; u < RPW; ++u) {
+                    double acc = 0.0;
+#pragma unroll
+                    for (int b = 0; b < kNumTerms; ++b) acc = fma(sC[r0 + u][b], wv[b], acc);
+                    v[u] = acc * sRate[r0 + u][cmp] * scl;       // N' / 2^tau_i
+                }
             } else {
-                q16[j] = i8_fixed((e == kI8BadRow) ? 0.0 : v, scale2, ns);
+                const double nm = sW[0][sj] * scl;
+#pragma unroll
+                for (int u = 0; u < RPW; ++u)
+                    v[u] = (row0 + u < Pc && ibase + j < n_T) ? coef[(size_t)(row0 + u) * n_T + ibase + j] * nm : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < RPW; ++u) {
+                if (PASS == 0) {
+                    if (!(v[u] >= 0.0) || isinf(v[u])) bad[u] = true;
+                    vmax[u] = fmax(vmax[u], v[u]);
+                } else {
+                    q16[u][j] = i8_fixed((e[u] == kI8BadRow) ? 0.0 : v[u], scale2[u], ns);
+                }
             }
         }
         if (PASS == 1) {
-            const int64_t mt = row >> 7;
-            const int rr = (int)(row & 127), g = rr >> 3, r8 = rr & 7;
-            const int kt = ibase >> 5, c = (ibase >> 4) & 1;
-            uint8_t *base = As + ((size_t)(mt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
-            for (int s = 0; s < 8; ++s) {
-                if (s >= ns_store) break;
-                uint32_t w[4];
+            for (int u = 0; u < RPW; ++u) {
+                const int64_t row = row0 + u, mt = row >> 7;
+                const int rr = (int)(row & 127), g = rr >> 3, r8 = rr & 7;
+                const int kt = ibase >> 5, c = (ibase >> 4) & 1;
+                uint8_t *base = As + ((size_t)(mt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    uint32_t x = 0;
+                for (int s = 0; s < 8; ++s) {
+                    if (s >= ns_store) break;
+                    uint32_t w[4];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        x |= i8_digit(q16[4 * h + j], s, ns) << (8 * j);
-                    w[h] = x;
+                    for (int h = 0; h < 4; ++h) {
+                        uint32_t x = 0;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) x |= i8_digit(q16[u][4 * h + j], s, ns) << (8 * j);
+                        w[h] = x;
+                    }
+                    *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) = make_uint4(w[0], w[1], w[2], w[3]);
                 }
-                *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) = make_uint4(w[0], w[1], w[2], w[3]);
             }
         }
     }
     if (PASS == 0) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
-            bad = __shfl_xor_sync(0xffffffffu, (int)bad, o) || bad;
+        for (int u = 0; u < RPW; ++u) {
+            double vm = vmax[u];
+            int bd = bad[u];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                vm = fmax(vm, __shfl_xor_sync(0xffffffffu, vm, o));
+                bd |= __shfl_xor_sync(0xffffffffu, bd, o);
+            }
+            if (lane == 0) e_row[row0 + u] = bd ? kI8BadRow : i8_exponent(vm);
         }
-        if (lane == 0) e_row[row] = bad ? kI8BadRow : i8_exponent(vmax);
     }
 }
 
@@ -566,7 +601,7 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     uint8_t *As = reinterpret_cast<uint8_t *>(ctx->A_packed);     // 8 slice bytes per (point, bin): fits the FP64 N'
     const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
     const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
-    const unsigned sgrid = (unsigned)(rows_pad / 8);
+    const unsigned sgrid = (unsigned)(rows_pad / kI8SliceRows);
     const int nst = fast ? 4 : L.ns8;
     if (w) {
         const double *N_mc = ctx->N_mc + (size_t)d * ctx->n_T;
