@@ -40,7 +40,7 @@ template <int PB>
 __global__ void __launch_bounds__(kStreamThreads)
 k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
 {
-    __shared__ __align__(16) double sN[kRC][PB];
+    __shared__ __align__(16) double sN[2][kRC][PB];
     __shared__ double sC[PB][kCoefStride];
     __shared__ double sRate[PB][RW_MAX_COMPONENTS];
     __shared__ double red[kStreamThreads / 32][PB];
@@ -87,24 +87,31 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
     for (int p = 0; p < PB; ++p) acc[p][0] = acc[p][1] = 0.0;
     const bool col_ok = col < n_rec;
 
-    for (int ic = i0; ic < i1; ic += kRC) {
-        __syncthreads();
+    // N' of a 64-row chunk: N' = sum_b c_b W^_b (Eq. 14 folded into the pre-scaled basis) or w N_mc (Eq. 1 with
+    // caller-supplied weights).  Double-buffered: chunk ic + 64 is staged after chunk ic has been streamed, so one
+    // barrier per chunk and the warps that finish streaming early stage while the others still load R.
+    auto stage = [&](int ic, int buf) {
         for (int q = threadIdx.x; q < kRC * PB; q += kStreamThreads) {
             const int p = q / kRC, row = q - p * kRC;     // consecutive threads -> consecutive bins
             const int i = ic + row;
             double v = 0.0;
             if (i < i1) {
-                if (wts) {          // N' = w N_mc (Eq. 1 with caller-supplied weights)
+                if (wts) {
                     if (p < Pb) v = wts[(size_t)p * n_T + i] * A.N_mc[(size_t)d * n_T + i];
-                } else {            // N' = sum_b c_b W^_b (Eq. 14 folded into the pre-scaled basis)
+                } else {
 #pragma unroll
                     for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p][b], Wd[(size_t)b * n_T + i], v);
                     if (A.comp8) v *= sRate[p][A.comp8[i]];        // rate_k of Eq. (17)
                 }
             }
-            sN[row][p] = v;
+            sN[buf][row][p] = v;
         }
-        __syncthreads();
+    };
+    __syncthreads();                                               // sC, sRate
+    if (i0 < i1) stage(i0, 0);
+    int buf = 0;
+    for (int ic = i0; ic < i1; ic += kRC, buf ^= 1) {
+        __syncthreads();                                           // sN[buf] staged; sN[buf ^ 1] no longer read
         if (col_ok) {
             const double *Rp = Rd + (size_t)ic * A.ldR + col;
             const int nrows = min(kRC, i1 - ic);
@@ -120,13 +127,14 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
                 for (int u = 0; u < 8; ++u) {
 #pragma unroll
                     for (int p = 0; p < PB; ++p) {
-                        const double n = sN[r0 + u][p];
+                        const double n = sN[buf][r0 + u][p];
                         acc[p][0] = fma(n, rv[u].x, acc[p][0]);
                         acc[p][1] = fma(n, rv[u].y, acc[p][1]);
                     }
                 }
             }
         }
+        if (ic + kRC < i1) stage(ic + kRC, buf ^ 1);
     }
     const int n_splits = A.n_splits, mu_ld = A.mu_ld;
     if (col_ok) {
