@@ -15,7 +15,7 @@
 
 namespace rw {
 
-constexpr int kProfThreads = 256;
+constexpr int kProfThreads = 1024;   // a Newton step is a latency chain (pass + block reduction): keep the pass short
 constexpr int kProfSmemRow = 20480;     // doubles of S cached in shared memory (160 KB); larger rows re-read HBM/L2
 
 struct Pair { double a, b; };
@@ -56,6 +56,7 @@ k_profile(const double *__restrict__ mu_rows /*[rows][nb]: mu at s = 1*/, int nb
 
     auto eval_g = [&](double s) {          // (g, g') at s
         double g = 0.0, dg = 0.0;
+#pragma unroll 4
         for (int j = threadIdx.x; j < nb; j += kProfThreads) {
             const double S = sig(j), n = counts[j];
             if (S != 0.0) {
@@ -75,18 +76,25 @@ k_profile(const double *__restrict__ mu_rows /*[rows][nb]: mu at s = 1*/, int nb
     };
 
     double s_hat = 0.0;
+    int n_it = 0;
     Pair r = eval_g(0.0);
     if (r.a < 0.0) {                       // interior minimum (NaN inputs fall through to the value pass)
         double lo = 0.0, hi = -1.0;        // hi < 0: no upper bracket yet
         double s = (sigma > 0.0 && s0 > 0.0) ? s0 : 1.0;
         for (int it = 0; it < 100; ++it) {
+            ++n_it;
             r = eval_g(s);
             if (r.a == 0.0) break;
             if (r.a < 0.0) lo = s; else hi = s;
             double sn = s - r.a / r.b;
-            if (!(sn > lo) || (hi > 0.0 && !(sn < hi)) || !(r.b > 0.0))
-                sn = (hi > 0.0) ? 0.5 * (lo + hi) : 2.0 * s;
-            const bool done = fabs(sn - s) <= 1e-15 * fabs(sn) || (hi > 0.0 && hi - lo <= 1e-15 * hi);
+            if (sn == s) break;            // the step is below one ulp of s: converged (without this test a step
+                                           // from the left with no upper bracket yet would be "rejected", s doubled,
+                                           // and ~50 bisections spent coming back)
+            const bool rejected = !(sn > lo) || (hi > 0.0 && !(sn < hi)) || !(r.b > 0.0);
+            if (rejected) sn = (hi > 0.0) ? 0.5 * (lo + hi) : 2.0 * s;
+            // Newton converges quadratically here: once a step is below 1e-12 relative, the point it lands on is
+            // exact to rounding, so that step is the last one
+            const bool done = (!rejected && fabs(sn - s) <= 1e-12 * fabs(sn)) || (hi > 0.0 && hi - lo <= 1e-15 * hi);
             s = sn;
             if (done) break;
         }
@@ -104,7 +112,12 @@ k_profile(const double *__restrict__ mu_rows /*[rows][nb]: mu at s = 1*/, int nb
         if (sigma > 0.0) f += (s_hat - s0) * (s_hat - s0) * inv_var;
         if (sat_const) f += sat_const[0];
         out[blockIdx.x] = f;
+#ifdef RW_PROF_DEBUG
+        if (out_scale) out_scale[blockIdx.x] = n_it;
+#else
+        (void)n_it;
         if (out_scale) out_scale[blockIdx.x] = s_hat;
+#endif
     }
 }
 
