@@ -78,4 +78,4 @@ def test_config5_streamed_in_batches_of_16384(orc):
     rng = np.random.default_rng(505)
     edges = [0, 16383, 16384, 61 * 16384 - 1, 61 * 16384, 999999, 100 * 16384 // 2]
     idx = np.concatenate([edges, rng.integers(0, 1000000, 17)])
-    _full_vs_sample(orc, "cfg5_joint6", idx, max_batch=16384, mu_check=False)
+    _full_vs_sample(orc, "cfg5_joint6", idx, max_batch=16384, mu_check=False, sliced=True)
