@@ -33,6 +33,8 @@ UNIT = "evals/s"
 # `ncu --set full` capture (profiles/r01c_fold_gemm_full.md: the fused launch over the 110 full waves of one
 # 32768-point chunk), or None if not captured.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4_dense": 69.584991e9 + 0.032040e9}
+# the same for the single-evaluation kernel k_fold_stream<1> (profiles/r01e_fold_stream_full.md)
+NCU_TRAFFIC_BYTES_SINGLE_EVAL = {"cfg4_dense": 1.075726e9 + 0.0112768e9}
 
 
 def load_peaks():
@@ -303,6 +305,8 @@ def main():
         single["note"] = ("P=1, one-launch streaming path (fold + likelihood); R (%.2f GB) >> L2, so every eval reads it "
                           "from HBM; kernel time includes the last-CTA reduction" % (r_bytes / 1e9))
         single["hbm_frac"] = single["hbm_gbs"] / peaks["hbm_gbs"]
+        single["algorithmic_bytes"] = r_bytes
+        single["traffic"] = NCU_TRAFFIC_BYTES_SINGLE_EVAL.get(name)
     else:
         single["note"] = ("P=1, one-launch streaming path; R (%.1f MB) stays in the 126 MB L2 between back-to-back "
                           "evaluations: latency-bound, no HBM fraction is claimed" % (r_bytes / 1e6))
