@@ -33,6 +33,36 @@ def test_library_exports_every_declared_symbol():
     assert set(binding.EXPORTS) == set(names)
 
 
+def test_binding_constants_match_the_header():
+    """Every RW_* enumerator of include/rw.h that the binding also defines has the same value there (the binding
+    retypes them; a drift would send the wrong flag or parameter kind through the ABI)."""
+    from paper_2607_00488_b200 import binding
+    text = open(os.path.join(ROOT, "include", "rw.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    header = {}
+    for body in re.findall(r"enum\s*\w*\s*\{(.*?)\}", text, flags=re.S):
+        nxt = 0
+        for item in body.split(","):
+            item = item.strip()
+            if not item:
+                continue
+            m = re.match(r"(RW_[A-Z0-9_]+)\s*(?:=\s*(.+))?$", item, flags=re.S)
+            assert m, item
+            if m.group(2) is not None:
+                expr = re.sub(r"(\d+)u\b", r"\1", m.group(2))
+                expr = re.sub(r"RW_[A-Z0-9_]+", lambda mm: str(header[mm.group(0)]), expr)
+                nxt = int(eval(expr, {"__builtins__": {}}))            # noqa: S307 (header arithmetic only)
+            header[m.group(1)] = nxt
+            nxt += 1
+    assert header["RW_SLICED"] == 1 << 11 and header["RW_MU_NU"] == 6 and header["RW_N_KINDS"] == 11
+    checked = 0
+    for name, value in header.items():
+        if hasattr(binding, name):
+            assert getattr(binding, name) == value, "%s: header %d, binding %d" % (name, value, getattr(binding, name))
+            checked += 1
+    assert checked >= 12, checked
+
+
 def test_abi_argument_errors_without_a_gpu():
     """Pure host-side validation paths return statuses, never crash (no kernel is launched)."""
     from paper_2607_00488_b200 import binding
