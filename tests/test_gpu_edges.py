@@ -233,3 +233,35 @@ def test_eval_batch_is_cuda_graph_capturable(rw, orc):
             torch.cuda.synchronize()
             assert np.all(np.abs(out.cpu().numpy() - ref[sel]) <= 1e-9), (P, mode)
     ctx.close()
+
+
+def test_every_regime_is_bit_reproducible_run_to_run(rw):
+    """The design has no floating-point atomics: reductions across tiles, k-ranges, row ranges and periods run in a
+    fixed order (tickets only decide WHO sums).  The same call twice must therefore give the same bits, in every
+    regime: streaming (1, 4 and 16 points per launch), DMMA contraction with and without split-K, collapsed, TF32 x 3,
+    sliced, fast sliced, profile, gradient."""
+    import torch
+    inp = wl.make_custom(n_E=31, n_T=1500, n_rec=700, n_periods=2, seed=141, dead_fraction=0.05)
+    params, kinds = wl.random_points(700, [wl.EPS_EE_L, wl.EPS_EE_R, wl.EPS_TT_L, wl.MU_NU], seed=142)
+    ctx = rw.Reweighter(inp, max_batch=512, fp32=True, sliced=True)
+    p = _cuda(params)
+
+    def twice(fn):
+        a = fn()
+        torch.cuda.synchronize()
+        a = [t.clone() for t in (a if isinstance(a, tuple) else (a,))]
+        b = fn()
+        torch.cuda.synchronize()
+        b = b if isinstance(b, tuple) else (b,)
+        for x, y in zip(a, b):
+            assert torch.equal(x, y)
+
+    for n, mode in ((1, "stream"), (4, "stream"), (16, "stream"), (16, "gemm"), (40, "gemm"), (300, "gemm"),
+                    (700, "gemm"), (700, "collapsed")):
+        twice(lambda: ctx.eval_batch(p[:n], kinds, want_mu=True, mode=mode))
+    twice(lambda: ctx.eval_batch(p, kinds, mode="gemm", fp32=True))
+    twice(lambda: ctx.eval_batch(p, kinds, want_mu=True, mode="gemm", sliced=True))
+    twice(lambda: ctx.eval_batch(p, kinds, mode="gemm", sliced="fast"))
+    twice(lambda: ctx.eval_profile(p[:200], kinds, s0=1.0, sigma=0.1))
+    twice(lambda: ctx.eval_grad(p[:100], kinds))
+    ctx.close()
