@@ -36,9 +36,9 @@ constexpr int kI8SliceBytesA = kI8BM * kI8BK;                   // 4 KB
 constexpr int kI8SliceBytesB = kI8BN * kI8BK;                   // 4 KB
 constexpr int kI8Threads = 320;                                 // TMA warp, MMA warp, 8 epilogue warps
 #ifndef RW_I8_STAGES
-#define RW_I8_STAGES 3
+#define RW_I8_STAGES 3              // measured: 2 slots cost 0.7 %, a 4th does not fit
 #endif
-constexpr int kI8SlotBytes = 65536, kI8Stages = RW_I8_STAGES;              // a slot: N' slices in its first half, R slices in its second
+constexpr int kI8SlotBytes = 65536, kI8Stages = RW_I8_STAGES;   // a slot: N' slices in its first half, R slices in its second
 constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 4 * kI8BN * 8 + 256 + 1024;
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
 
@@ -64,7 +64,7 @@ __device__ __forceinline__ int i8_exponent(double vmax)          // smallest e w
     return e;
 }
 
-// N'[p][i] = rate * sum_b coef[p][b] W^[b][i] (steps a1 + a2) for 8 points x all recoil bins per CTA, W^ staged
+// N'[p][i] = rate * sum_b coef[p][b] W^[b][i] (steps a1 + a2) for 16 points x all recoil bins per CTA, W^ staged
 // 512 bins at a time.  PASS 0: row maximum -> exponent e_p.  PASS 1: slices, written 16 bytes at a time into
 //   As[m-tile][k-block][slice][16-byte chunk c][row group g][row r8][16]     (canonical K-major core matrices)
 // shared-memory column swizzle: a thread reads 16 consecutive bins (lane stride 128 bytes = one bank for the whole
