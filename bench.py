@@ -381,7 +381,7 @@ def main():
             fast_leg = {"ms_per_call": t_f, "evals_per_s": P / t_f * 1e3,
                         "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_f / 1e9,
                         "mu_rel_err_vs_fp64_max": float(relf.max().item()), "int8_products_per_k_step": 10}
-            n_sl = 8 if n_T <= 8192 else 7                              # balanced 8-bit slices per operand (rw_fold_i8.cu)
+            n_sl = 8 if n_T <= 2048 else 7                              # balanced 8-bit slices per operand (rw_fold_i8.cu)
             n_prod = n_sl * (n_sl + 1) // 2
             sliced_leg = {"ms_per_call": t_s, "evals_per_s": P / t_s * 1e3, "bound": "tensor (int8)",
                           "effective_fold_tflops": 2.0 * n_T * n_rec * D * P / t_s / 1e9,

@@ -50,7 +50,10 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->fp32 = (in->create_flags & RW_CREATE_FP32) != 0;
     L->sliced = (in->create_flags & RW_CREATE_SLICED) != 0;
     L->KT8 = (int)((n_T + 31) / 32);
-    L->ns8 = (n_T <= 8192) ? 8 : 7;
+    // 8 slices (63 bits) are exact in int32 up to n_T = 8192; they are used where the contraction is too short for
+    // the tensor pipe to matter.  Beyond, 7 slices (55 bits, 28 instead of 36 products): measured 5e-15 .. 1.2e-13 of mu
+    // on configs 3-5 against the 1e-12 bar.
+    L->ns8 = (n_T <= 2048) ? 8 : 7;
     L->NT8 = 2 * (int)((n_rec + 127) / 128);     // 64-column units (one epilogue warp set each); tiles are 128 wide
     int64_t cap = kMaxChunkBytes / (L->A_pitch) / kBM * kBM;
     if (cap < kBM) cap = kBM;

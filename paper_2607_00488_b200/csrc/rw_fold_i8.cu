@@ -3,7 +3,7 @@
 //
 // The fold mu[p][k] = sum_i N'[p][i] R[i][k] (Eq. 11) has only non-negative terms.  Each row of N'
 // and each column of R is written in fixed point relative to its own power-of-two scale and cut into NS base-256
-// digits ("slices"; NS = 8 for n_T <= 8192, else 7),
+// digits ("slices"; NS = 8 for n_T <= 2048, else 7),
 //     N'[p][i] = 2^(e_p - 7) sum_s a_s[p][i] 2^(-8 s),      R[i][k] = 2^(f_k - 7) sum_t b_t[i][k] 2^(-8 t),
 // with BALANCED digits: a_0 in [0, 129] (unsigned; one spare bit keeps the carry), a_s in [-128, 127] for s > 0.
 // The contraction becomes NS (NS + 1) / 2 INT8 tensor-core products with EXACT int32 accumulation (tcgen05.mma

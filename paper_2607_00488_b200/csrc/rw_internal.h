@@ -59,7 +59,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int stream_splits;    // row splits of the streaming fold
     int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
     bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
-    int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 8192 (int32 accumulation stays exact), else 7
+    int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 2048, else 7 (rw_api.cu plan())
     int KT8, NT8;         // k-blocks of 32 recoil bins; 64-column units = 2 x (128-column tiles) (rw_fold_i8.cu)
     bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)

@@ -50,16 +50,17 @@ def test_sliced_long_contraction_and_chunks(orc):
     _check(inp, params, kinds, ref, mu_ref, scale, max_batch=64)
 
 
-def test_sliced_eight_slices_mid_length(orc):
-    """n_T = 5000: eight balanced 8-bit slices (eight pairs of 129 x 128 products over 8192 bins stay below 2^31)."""
-    inp = wl.make_custom(n_E=24, n_T=5000, n_rec=130, n_periods=1, seed=117, tail=0.0)
+def test_sliced_eight_slices_at_their_largest_size(orc):
+    """n_T = 2048: the longest contraction that still takes eight balanced 8-bit slices (36 products per k-step)."""
+    inp = wl.make_custom(n_E=24, n_T=2048, n_rec=130, n_periods=1, seed=117, tail=0.0)
     params, kinds = wl.random_points(140, [wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU], seed=118)
     ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
     _check(inp, params, kinds, ref, mu_ref, scale)
 
 
 def test_sliced_seven_slices(orc):
-    """n_T = 8300 > 8192: seven balanced 8-bit slices (28 products per k-step, 55 bits below the row / column scale)."""
+    """n_T = 8300: seven balanced 8-bit slices (28 products per k-step, 55 bits below the row / column scale), as for
+    every n_T > 2048 (n_T = 3000 and config 2's dead-bin-heavy 1000 x 500 are covered above and below)."""
     inp = wl.make_custom(n_E=24, n_T=8300, n_rec=100, n_periods=1, seed=119, tail=0.0)
     params, kinds = wl.random_points(130, [wl.EPS_EE_L, wl.EPS_MM_R, wl.MU_NU], seed=120)
     ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
