@@ -198,3 +198,37 @@ def test_sliced_fast_config2_and_components(orc):
     kinds = np.array([wl.EPS_EE_L, wl.MU_NU, 7, 9], np.int32)
     params, _ = wl.random_points(70, kinds, seed=136)
     _check_fast(orc, inp, params, kinds, components=True)
+
+
+def test_sliced_agrees_with_the_dmma_path_on_odd_shapes():
+    """Shape sweep around every boundary of the sliced kernels (k-blocks of 32 bins, tiles of 128 points x 128 bins,
+    64-column epilogue halves, chunked batches, several periods).  The DMMA path is held to the oracle elsewhere;
+    here the sliced, fast-sliced, sliced-weights and sliced-profile results are held to it."""
+    import torch
+    from paper_2607_00488_b200 import binding
+    rng = np.random.default_rng(151)
+    shapes = [(1, 1, 5, 1), (2, 3, 6, 2), (31, 63, 17, 1), (32, 64, 127, 3), (33, 65, 128, 1), (64, 127, 129, 2),
+              (65, 128, 255, 1), (255, 129, 256, 1), (256, 130, 300, 2), (257, 255, 17, 3), (1000, 256, 128, 1),
+              (2047, 257, 129, 1), (2048, 500, 300, 1), (2049, 700, 127, 2)]
+    for n_T, n_rec, P, D in shapes:
+        inp = wl.make_custom(n_E=int(rng.integers(3, 40)), n_T=n_T, n_rec=n_rec, n_periods=D,
+                             seed=int(rng.integers(1, 10**6)), dead_fraction=float(rng.choice([0.0, 0.1])))
+        params, kinds = wl.random_points(P, [wl.EPS_EE_L, wl.EPS_EE_R, wl.EPS_TT_L, wl.MU_NU], seed=int(rng.integers(1, 10**6)))
+        ctx = binding.Reweighter(inp, max_batch=int(rng.choice([P, max(5, P // 2), 64])), sliced=True)
+        p = _cuda(params)
+        w = _cuda(rng.uniform(0.0, 2.0, size=(P, n_T)))
+        o64, m64 = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm")
+        o8, m8 = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm", sliced=True)
+        _, mf = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm", sliced="fast")
+        _, mw64 = ctx.eval_weights(w, want_mu=True, mode="gemm")
+        _, mw8 = ctx.eval_weights(w, want_mu=True, mode="gemm", sliced=True)
+        _, s64 = ctx.eval_profile(p, kinds, mode="gemm")
+        _, s8 = ctx.eval_profile(p, kinds, mode="gemm", sliced=True)
+        torch.cuda.synchronize()
+        tag = "n_T %d n_rec %d P %d D %d" % (n_T, n_rec, P, D)
+        assert ((m8 - m64).abs() <= 2e-12 * m64.abs()).all(), tag
+        assert ((mf - m64).abs() <= 1e-5 * m64.abs()).all(), tag
+        assert ((mw8 - mw64).abs() <= 2e-12 * mw64.abs()).all(), tag
+        assert ((o8 - o64).abs() <= 1e-9 + 1e-10 * o64.abs()).all() and bool(torch.isfinite(o8).all()), tag
+        assert ((s8 - s64).abs() <= 1e-9 * s64.abs().clamp_min(1e-3)).all(), tag
+        ctx.close()
