@@ -76,13 +76,11 @@ k_profile(const double *__restrict__ mu_rows /*[rows][nb]: mu at s = 1*/, int nb
     };
 
     double s_hat = 0.0;
-    int n_it = 0;
     Pair r = eval_g(0.0);
     if (r.a < 0.0) {                       // interior minimum (NaN inputs fall through to the value pass)
         double lo = 0.0, hi = -1.0;        // hi < 0: no upper bracket yet
         double s = (sigma > 0.0 && s0 > 0.0) ? s0 : 1.0;
         for (int it = 0; it < 100; ++it) {
-            ++n_it;
             r = eval_g(s);
             if (r.a == 0.0) break;
             if (r.a < 0.0) lo = s; else hi = s;
@@ -112,12 +110,7 @@ k_profile(const double *__restrict__ mu_rows /*[rows][nb]: mu at s = 1*/, int nb
         if (sigma > 0.0) f += (s_hat - s0) * (s_hat - s0) * inv_var;
         if (sat_const) f += sat_const[0];
         out[blockIdx.x] = f;
-#ifdef RW_PROF_DEBUG
-        if (out_scale) out_scale[blockIdx.x] = n_it;
-#else
-        (void)n_it;
         if (out_scale) out_scale[blockIdx.x] = s_hat;
-#endif
     }
 }
 
