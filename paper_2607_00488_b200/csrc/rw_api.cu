@@ -118,6 +118,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->f_col8 = take(L->sliced ? D * n_rec * 4 : 0);
     L->e_row8 = take(L->sliced ? (size_t)L->MC * 4 : 0);
     L->tau8 = take(L->sliced ? D * n_T * 4 : 0);
+    L->blk_hl8 = take(L->sliced ? D * 2 * (size_t)kNumTerms * L->KT8 * 8 : 0);
+    L->blk_cm8 = take(L->sliced ? (size_t)L->KT8 * 4 : 0);
     L->total = off;
     return RW_OK;
 }
@@ -351,6 +353,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->f_col8 = (int *)(ws + L.f_col8);
     ctx->e_row8 = (int *)(ws + L.e_row8);
     ctx->tau8 = (int *)(ws + L.tau8);
+    ctx->blk_hl8 = (double *)(ws + L.blk_hl8);
+    ctx->blk_cm8 = (int *)(ws + L.blk_cm8);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;

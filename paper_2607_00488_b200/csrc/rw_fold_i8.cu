@@ -111,6 +111,7 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
         bad[u] = false;
     }
     const int n_pad = KT * kI8BK;
+    const double limit = ldexp(1.0, 8 * ns - 1);                  // q <= 2^(8 ns - 1) keeps the top digit <= 128
     for (int i0 = 0; i0 < n_pad; i0 += 512) {
         __syncthreads();
         for (int q = threadIdx.x; q < (SRC == 0 ? kNumTerms : 1) * 512; q += 256) {
@@ -159,7 +160,10 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
                     if (!(v[u] >= 0.0) || isinf(v[u])) bad[u] = true;
                     vmax[u] = fmax(vmax[u], v[u]);
                 } else {
-                    q16[u][j] = i8_fixed((e[u] == kI8BadRow) ? 0.0 : v[u], scale2[u], ns);
+                    // the exponent may come from k_row_bound (an upper bound, never below the row maximum): a negative
+                    // or non-finite N', or -- should the bound ever fail -- a value past 2^e, makes the row NaN
+                    if (!(v[u] >= 0.0) || !(v[u] * scale2[u] <= limit)) bad[u] = e[u] != kI8BadRow;
+                    q16[u][j] = i8_fixed((e[u] == kI8BadRow || bad[u]) ? 0.0 : v[u], scale2[u], ns);
                 }
             }
         }
@@ -186,6 +190,15 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
             }
         }
     }
+    if (PASS == 1) {
+#pragma unroll
+        for (int u = 0; u < RPW; ++u) {
+            int bd = bad[u];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) bd |= __shfl_xor_sync(0xffffffffu, bd, o);
+            if (bd && lane == 0) e_row[row0 + u] = kI8BadRow;    // read by the fold's epilogue: NaN for that point
+        }
+    }
     if (PASS == 0) {
 #pragma unroll
         for (int u = 0; u < RPW; ++u) {
@@ -199,6 +212,76 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
             if (lane == 0) e_row[row0 + u] = bd ? kI8BadRow : i8_exponent(vm);
         }
     }
+}
+
+// ---- row exponents of N' without a pass over N' (coefficient rows only) ----
+// Per 32-bin block B and basis term b: hi / lo = max / min over the block of W^_b[i] 2^-tau_i; cmask = components
+// present.  Then for a point   max_i N'[p][i] 2^-tau_i  <=  max_B rate_B(p) sum_b max(c_b hi_b[B], c_b lo_b[B]),
+// a sum of maxima in place of the maximum of the sum: 16 x cheaper than evaluating N', and tight because all W^_b
+// carry the same N_mc[i] / S_SM[i] factor (the exponent comes out one larger than the exact one in a few per cent
+// of the rows: one bit of 55).
+__global__ void __launch_bounds__(32)
+k_block_tables(const double *__restrict__ What /*[12][n_T]*/, const int *__restrict__ tau, const uint8_t *__restrict__ comp8,
+               int n_T, int n_blk, double *__restrict__ hi /*[11][n_blk]*/, double *__restrict__ lo, int *__restrict__ cmask)
+{
+    const int B = blockIdx.x, i = B * 32 + threadIdx.x;
+    const bool in = i < n_T;
+    const double scl = in ? ldexp(1.0, -tau[i]) : 0.0;
+    for (int b = 0; b < kNumTerms; ++b) {
+        const double v = in ? What[(size_t)b * n_T + i] * scl : 0.0;
+        double h = in ? v : -INFINITY, l = in ? v : INFINITY;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            h = fmax(h, __shfl_xor_sync(0xffffffffu, h, o));
+            l = fmin(l, __shfl_xor_sync(0xffffffffu, l, o));
+        }
+        if (threadIdx.x == 0) { hi[(size_t)b * n_blk + B] = h; lo[(size_t)b * n_blk + B] = l; }
+    }
+    int m = in ? (1 << comp8[i]) : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m |= __shfl_xor_sync(0xffffffffu, m, o);
+    if (threadIdx.x == 0) cmask[B] = m;
+}
+
+// One warp per point of the chunk: e_row[p] from the bound above (NaN / infinite coefficients: bad row).
+__global__ void __launch_bounds__(256)
+k_row_bound(const double *__restrict__ coef, const double *__restrict__ rate, int64_t p0, int64_t Pc, int64_t rows_pad,
+            const double *__restrict__ hi, const double *__restrict__ lo, const int *__restrict__ cmask, int n_blk,
+            int *__restrict__ e_row)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (row >= rows_pad) return;
+    if (row >= Pc) { if (lane == 0) e_row[row] = 0; return; }      // padding rows of the last tile: all-zero slices
+    double c[kNumTerms], r[RW_MAX_COMPONENTS];
+#pragma unroll
+    for (int b = 0; b < kNumTerms; ++b) c[b] = coef[(p0 + row) * kCoefStride + b];
+#pragma unroll
+    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) r[q] = rate[(p0 + row) * RW_MAX_COMPONENTS + q];
+    double vmax = 0.0;
+    bool bad = false;
+    for (int B = lane; B < n_blk; B += 32) {
+        double sum = 0.0;
+#pragma unroll
+        for (int b = 0; b < kNumTerms; ++b) sum += fmax(c[b] * hi[(size_t)b * n_blk + B], c[b] * lo[(size_t)b * n_blk + B]);
+        const int m = cmask[B];
+        double rm = 0.0;
+#pragma unroll
+        for (int q = 0; q < RW_MAX_COMPONENTS; ++q)
+            if (m >> q & 1) rm = fmax(rm, r[q]);
+        const double v = sum * rm;
+        if (!(v == v) || isinf(v) || !(rm == rm)) bad = true;
+        vmax = fmax(vmax, v);
+    }
+#pragma unroll
+    for (int b = 0; b < kNumTerms; ++b) bad = bad || !(c[b] == c[b]) || isinf(c[b]);
+    int bd = bad;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+        bd |= __shfl_xor_sync(0xffffffffu, bd, o);
+    }
+    if (lane == 0) e_row[row] = bd ? kI8BadRow : i8_exponent(vmax * (1.0 + 1e-9));     // rounding slack of the 11-term sums
 }
 
 // Column maxima of R -> exponents f_k (one thread per column, rows read coalesced across the warp).
@@ -576,6 +659,10 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
         const double *Rd = ctx->R + (size_t)d * ctx->R_period_stride;
         int *f = ctx->f_col8 + (size_t)d * ctx->n_rec, *tau = ctx->tau8 + (size_t)d * ctx->n_T;
         k_tau<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T, tau);
+        k_block_tables<<<KT, 32, 0, s>>>(ctx->What + (size_t)d * kCoefStride * ctx->n_T, tau, ctx->comp8, ctx->n_T, KT,
+                                         ctx->blk_hl8 + (size_t)d * 2 * kNumTerms * KT,
+                                         ctx->blk_hl8 + ((size_t)d * 2 + 1) * kNumTerms * KT, ctx->blk_cm8);
+        ctx->launches++;
         k_colexp_B<<<(ctx->n_rec + 127) / 128, 128, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, tau, f);
         dim3 grid((n_cols + 255) / 256, KT * 2);
         k_slice_B<<<grid, 256, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, n_cols, KT, L.ns8, tau, f, ctx->B8 + (size_t)d * per);
@@ -608,8 +695,10 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
         k_slice_A<0, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
         k_slice_A<1, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
     } else {
-        k_slice_A<0, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
-                                              nst, ctx->e_row8, As);
+        k_row_bound<<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, p0, Pc, rows_pad,
+                                                             ctx->blk_hl8 + (size_t)d * 2 * kNumTerms * KT,
+                                                             ctx->blk_hl8 + ((size_t)d * 2 + 1) * kNumTerms * KT,
+                                                             ctx->blk_cm8, KT, ctx->e_row8);
         k_slice_A<1, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
                                               nst, ctx->e_row8, As);
     }
