@@ -75,13 +75,29 @@ __device__ __forceinline__ int i8_sw(int ii) { return ii ^ ((ii >> 4) & 15); }
 // N_mc[n_T] of the period then, `coef` the weights of the chunk's first point).
 constexpr int kI8SliceRows = 16;      // rows per CTA: 2 per warp, so that every staged W^ value read from shared memory serves two rows
 
-template <int PASS, int SRC>
+// slice s (0 = top) of four fixed-point values as one 32-bit word of the operand: the digit is byte NS - 1 - s of
+// each value, gathered with three byte permutes (NS is a template parameter so the selectors are immediates)
+template <int NS>
+__device__ __forceinline__ uint32_t i8_pack4(const unsigned long long (&q)[16], int j0, int s)
+{
+    const int bidx = NS - 1 - s, bsel = bidx & 3;
+    const uint32_t sel = (uint32_t)bsel | ((uint32_t)(4 + bsel) << 4);
+    uint32_t w[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) w[j] = bidx < 4 ? (uint32_t)q[j0 + j] : (uint32_t)(q[j0 + j] >> 32);
+    const uint32_t t01 = __byte_perm(w[0], w[1], sel), t23 = __byte_perm(w[2], w[3], sel);
+    const uint32_t r = __byte_perm(t01, t23, 0x5410);
+    return s == 0 ? r : (r ^ 0x80808080u);
+}
+
+template <int PASS, int SRC, int NS>
 __global__ void __launch_bounds__(256)
 k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
           int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
-          int ns, int ns_store /*slices written: ns, or 4 for the fast mode*/, int *__restrict__ e_row,
+          int ns_store /*slices written: NS, or 4 for the fast mode*/, int *__restrict__ e_row,
           uint8_t *__restrict__ As)
 {
+    constexpr int ns = NS;
     constexpr int RPW = kI8SliceRows / 8;
     __shared__ double sW[kNumTerms][512];
     __shared__ __align__(16) uint8_t sComp[512];
@@ -175,17 +191,11 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
                 const int kt = ibase >> 5, c = (ibase >> 4) & 1;
                 uint8_t *base = As + ((size_t)(mt * KT + kt) * ns * 2 + c) * 2048 + g * 128 + r8 * 16;
 #pragma unroll
-                for (int s = 0; s < 8; ++s) {
+                for (int s = 0; s < NS; ++s) {
                     if (s >= ns_store) break;
-                    uint32_t w[4];
-#pragma unroll
-                    for (int h = 0; h < 4; ++h) {
-                        uint32_t x = 0;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) x |= i8_digit(q16[u][4 * h + j], s, ns) << (8 * j);
-                        w[h] = x;
-                    }
-                    *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) = make_uint4(w[0], w[1], w[2], w[3]);
+                    *reinterpret_cast<uint4 *>(base + (size_t)s * kI8SliceBytesA) =
+                        make_uint4(i8_pack4<NS>(q16[u], 0, s), i8_pack4<NS>(q16[u], 4, s), i8_pack4<NS>(q16[u], 8, s),
+                                   i8_pack4<NS>(q16[u], 12, s));
                 }
             }
         }
@@ -690,18 +700,21 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
     const unsigned sgrid = (unsigned)(rows_pad / kI8SliceRows);
     const int nst = fast ? 4 : L.ns8;
+#define RW_SLICE_LAUNCH(PASS, SRC, NS, c0, r0, m0, pp, W0)                                                          \
+    k_slice_A<PASS, SRC, NS><<<sgrid, 256, 0, s>>>(c0, r0, m0, pp, Pc, W0, tau, ctx->n_T, KT, nst, ctx->e_row8, As)
     if (w) {
         const double *N_mc = ctx->N_mc + (size_t)d * ctx->n_T;
-        k_slice_A<0, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
-        k_slice_A<1, 1><<<sgrid, 256, 0, s>>>(w, nullptr, nullptr, 0, Pc, N_mc, tau, ctx->n_T, KT, L.ns8, nst, ctx->e_row8, As);
+        if (L.ns8 == 8) { RW_SLICE_LAUNCH(0, 1, 8, w, nullptr, nullptr, 0, N_mc); RW_SLICE_LAUNCH(1, 1, 8, w, nullptr, nullptr, 0, N_mc); }
+        else { RW_SLICE_LAUNCH(0, 1, 7, w, nullptr, nullptr, 0, N_mc); RW_SLICE_LAUNCH(1, 1, 7, w, nullptr, nullptr, 0, N_mc); }
     } else {
         k_row_bound<<<(unsigned)(rows_pad / 8), 256, 0, s>>>(ctx->coef, ctx->rate, p0, Pc, rows_pad,
                                                              ctx->blk_hl8 + (size_t)d * 2 * kNumTerms * KT,
                                                              ctx->blk_hl8 + ((size_t)d * 2 + 1) * kNumTerms * KT,
                                                              ctx->blk_cm8, KT, ctx->e_row8);
-        k_slice_A<1, 0><<<sgrid, 256, 0, s>>>(ctx->coef, ctx->rate, ctx->comp8, p0, Pc, What, tau, ctx->n_T, KT, L.ns8,
-                                              nst, ctx->e_row8, As);
+        if (L.ns8 == 8) RW_SLICE_LAUNCH(1, 0, 8, ctx->coef, ctx->rate, ctx->comp8, p0, What);
+        else RW_SLICE_LAUNCH(1, 0, 7, ctx->coef, ctx->rate, ctx->comp8, p0, What);
     }
+#undef RW_SLICE_LAUNCH
     ctx->launches += 2;
     I8Work W;
     W.n_rec = ctx->n_rec; W.KT = KT; W.D = ctx->D; W.d = d;
