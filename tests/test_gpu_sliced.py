@@ -232,3 +232,12 @@ def test_sliced_agrees_with_the_dmma_path_on_odd_shapes():
         assert ((o8 - o64).abs() <= 1e-9 + 1e-10 * o64.abs()).all() and bool(torch.isfinite(o8).all()), tag
         assert ((s8 - s64).abs() <= 1e-9 * s64.abs().clamp_min(1e-3)).all(), tag
         ctx.close()
+
+
+@pytest.mark.parametrize("n_T,n_rec,P,D", [(1, 1, 5, 1), (33, 65, 129, 2), (257, 129, 130, 1)])
+def test_sliced_degenerate_and_boundary_shapes_against_the_oracle(orc, n_T, n_rec, P, D):
+    """One recoil bin and one reconstructed bin; one bin / one point past a k-block, a tile row and a tile column."""
+    inp = wl.make_custom(n_E=9, n_T=n_T, n_rec=n_rec, n_periods=D, seed=161 + n_T)
+    params, kinds = wl.random_points(P, [wl.EPS_EE_L, wl.EPS_MM_L, wl.MU_NU], seed=162 + n_T)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale)
