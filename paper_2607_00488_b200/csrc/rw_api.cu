@@ -120,6 +120,9 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->tau8 = take(L->sliced ? D * n_T * 4 : 0);
     L->blk_hl8 = take(L->sliced ? D * 2 * (size_t)kNumTerms * L->KT8 * 8 : 0);
     L->blk_cm8 = take(L->sliced ? (size_t)L->KT8 * 4 : 0);
+    L->KP512 = (int)((n_T + 511) / 512 * 512);
+    L->tau8b = take(L->sliced ? D * (size_t)L->KP512 : 0);
+    L->comp8p = take(L->sliced ? (size_t)L->KP512 : 0);
     L->total = off;
     return RW_OK;
 }
@@ -355,6 +358,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->tau8 = (int *)(ws + L.tau8);
     ctx->blk_hl8 = (double *)(ws + L.blk_hl8);
     ctx->blk_cm8 = (int *)(ws + L.blk_cm8);
+    ctx->tau8b = (int8_t *)(ws + L.tau8b);
+    ctx->comp8p = (uint8_t *)(ws + L.comp8p);
     ctx->ldR = L.ldR;
     ctx->R_period_stride = n_T * (size_t)L.ldR;
     ctx->R = L.copy_R ? (const double *)(ws + L.R_copy) : in->R;

@@ -73,6 +73,10 @@ __device__ __forceinline__ int i8_sw(int ii) { return ii ^ ((ii >> 4) & 15); }
 
 // SRC 1 (rw_eval_weights, rw_eval_pee): N'[p][i] = w[p][i] N_mc[i] from caller-visible weights instead (`What` is
 // N_mc[n_T] of the period then, `coef` the weights of the chunk's first point).
+constexpr int i8_slice_smem(int src)   // k_slice_A: two staging buffers + coefficient / rate rows
+{
+    return 2 * ((src == 0 ? kNumTerms : 1) * 512 * 8 + 1024) + 16 * (kCoefStride + RW_MAX_COMPONENTS) * 8;
+}
 constexpr int kI8SliceRows = 16;      // rows per CTA: 2 per warp, so that every staged W^ value read from shared memory serves two rows
 
 // slice s (0 = top) of four fixed-point values as one 32-bit word of the operand: the digit is byte NS - 1 - s of
@@ -92,29 +96,31 @@ __device__ __forceinline__ uint32_t i8_pack4(const unsigned long long (&q)[16], 
 
 template <int PASS, int SRC, int NS>
 __global__ void __launch_bounds__(256)
-k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8,
-          int64_t p0, int64_t Pc, const double *__restrict__ What, const int *__restrict__ tau /*[n_T]*/, int n_T, int KT,
-          int ns_store /*slices written: NS, or 4 for the fast mode*/, int *__restrict__ e_row,
+k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, const uint8_t *__restrict__ comp8 /*padded*/,
+          int64_t p0, int64_t Pc, const double *__restrict__ What, const int8_t *__restrict__ tau /*[n_T], padded*/,
+          int n_T, int KT, int ns_store /*slices written: NS, or 4 for the fast mode*/, int *__restrict__ e_row,
           uint8_t *__restrict__ As)
 {
     constexpr int ns = NS;
     constexpr int RPW = kI8SliceRows / 8;
-    __shared__ double sW[kNumTerms][512];
-    __shared__ __align__(16) uint8_t sComp[512];
-    __shared__ __align__(16) int8_t sTau[512];                   // tau_i (clamped to +-120 by k_tau)
-    __shared__ double sC[kI8SliceRows][kCoefStride];
-    __shared__ double sRate[kI8SliceRows][RW_MAX_COMPONENTS];
+    constexpr int NW = (SRC == 0) ? kNumTerms : 1;               // staged rows of W^ (SRC 1: N_mc only)
+    // dynamic shared memory: two staging buffers {W^ rows [NW][512], comp [512] bytes, tau [512] bytes}, filled with
+    // cp.async one 512-bin chunk ahead of the arithmetic (the kernel was latency-bound on these loads)
+    extern __shared__ __align__(16) uint8_t slice_smem[];
+    constexpr int kBufBytes = NW * 512 * 8 + 512 + 512;
+    double *sC = reinterpret_cast<double *>(slice_smem + 2 * kBufBytes);                  // [16][12]
+    double *sRate = sC + kI8SliceRows * kCoefStride;                                      // [16][4]
     const int r0 = (threadIdx.x >> 5) * RPW, lane = threadIdx.x & 31;
     const int64_t row0 = (int64_t)blockIdx.x * kI8SliceRows + r0;
     if (SRC == 0 && threadIdx.x < kI8SliceRows * kCoefStride) {
         const int rr = threadIdx.x / kCoefStride, b = threadIdx.x - rr * kCoefStride;
         const int64_t q = (int64_t)blockIdx.x * kI8SliceRows + rr;
-        sC[rr][b] = (q < Pc) ? coef[(p0 + q) * kCoefStride + b] : 0.0;
+        sC[rr * kCoefStride + b] = (q < Pc) ? coef[(p0 + q) * kCoefStride + b] : 0.0;
     }
     if (SRC == 0 && threadIdx.x < kI8SliceRows * RW_MAX_COMPONENTS) {
         const int rr = threadIdx.x / RW_MAX_COMPONENTS, cq = threadIdx.x % RW_MAX_COMPONENTS;
         const int64_t q = (int64_t)blockIdx.x * kI8SliceRows + rr;
-        sRate[rr][cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
+        sRate[rr * RW_MAX_COMPONENTS + cq] = (q < Pc) ? rate[(p0 + q) * RW_MAX_COMPONENTS + cq] : 1.0;
     }
     int e[RPW];
     double scale2[RPW], vmax[RPW];
@@ -128,17 +134,37 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
     }
     const int n_pad = KT * kI8BK;
     const double limit = ldexp(1.0, 8 * ns - 1);                  // q <= 2^(8 ns - 1) keeps the top digit <= 128
-    for (int i0 = 0; i0 < n_pad; i0 += 512) {
-        __syncthreads();
-        for (int q = threadIdx.x; q < (SRC == 0 ? kNumTerms : 1) * 512; q += 256) {
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(slice_smem);
+    auto stage = [&](int i0, int buf) {          // chunk [i0, i0 + 512) -> buffer buf; bins >= n_T read as zero
+        const uint32_t dW = sbase + buf * kBufBytes;
+        for (int q = threadIdx.x; q < NW * 512; q += 256) {
             const int b = q >> 9, ii = q & 511, i = i0 + ii;
-            sW[b][i8_sw(ii)] = (i < n_T) ? What[(size_t)b * n_T + i] : 0.0;       // SRC 1: row 0 = N_mc
+            const bool in = i < n_T;
+            const double *src = What + (in ? (size_t)b * n_T + i : 0);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dW + (b * 512 + i8_sw(ii)) * 8), "l"(src),
+                         "r"(in ? 8 : 0) : "memory");
         }
-        for (int q = threadIdx.x; q < 512; q += 256) {
-            sComp[q] = (SRC == 0 && i0 + q < n_T) ? comp8[i0 + q] : 0;
-            sTau[q] = (i0 + q < n_T) ? (int8_t)tau[i0 + q] : (int8_t)0;
+        if (threadIdx.x < 128) {                 // comp / tau bytes: padded to a multiple of 512 bins at rw_create
+            const uint32_t dC = dW + NW * 512 * 8 + 4 * threadIdx.x;
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4, 4;" ::"r"(dC), "l"(comp8 + i0 + 4 * threadIdx.x) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4, 4;" ::"r"(dC + 512), "l"(tau + i0 + 4 * threadIdx.x) : "memory");
         }
-        __syncthreads();
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    stage(0, 0);
+    int buf = 0;
+    for (int i0 = 0; i0 < n_pad; i0 += 512, buf ^= 1) {
+        if (i0 > 0) __syncthreads();                               // everyone is done with the buffer refilled next
+        if (i0 + 512 < n_pad) {
+            stage(i0 + 512, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();                                           // chunk i0 is in buffer buf for every thread
+        const double(*sW)[512] = reinterpret_cast<const double(*)[512]>(slice_smem + buf * kBufBytes);
+        const uint8_t *sComp = slice_smem + buf * kBufBytes + NW * 512 * 8;
+        const uint8_t *sTau = sComp + 512;
         const int ii0 = lane * 16, ibase = i0 + ii0;             // this thread: 16 consecutive bins of its rows
         if (ibase >= n_pad) continue;
         unsigned long long q16[RPW][16];
@@ -161,8 +187,8 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
                 for (int u = 0; u < RPW; ++u) {
                     double acc = 0.0;
 #pragma unroll
-                    for (int b = 0; b < kNumTerms; ++b) acc = fma(sC[r0 + u][b], wv[b], acc);
-                    v[u] = acc * sRate[r0 + u][cmp] * scl;       // N' / 2^tau_i
+                    for (int b = 0; b < kNumTerms; ++b) acc = fma(sC[(r0 + u) * kCoefStride + b], wv[b], acc);
+                    v[u] = acc * sRate[(r0 + u) * RW_MAX_COMPONENTS + cmp] * scl;       // N' / 2^tau_i
                 }
             } else {
                 const double nm = sW[0][sj] * scl;
@@ -298,13 +324,14 @@ k_row_bound(const double *__restrict__ coef, const double *__restrict__ rate, in
 // tau_i = binary exponent of the mean of N_mc over the 33 bins around i (0 where that mean is 0): the per-bin
 // rescaling shared by both operands.  The window keeps tau smooth: it follows the shape of the MC spectrum, which
 // is what spans decades, without passing bin-to-bin noise of N_mc on to the columns of R.
-__global__ void k_tau(const double *__restrict__ N_mc, int n_T, int *__restrict__ tau)
+__global__ void k_tau(const double *__restrict__ N_mc, int n_T, int *__restrict__ tau, int8_t *__restrict__ tau_b)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_T) return;
     double acc = 0.0;
     for (int j = max(0, i - 16); j <= min(n_T - 1, i + 16); ++j) acc += N_mc[j];
-    tau[i] = max(-120, min(120, i8_exponent(acc / 33.0)));      // any tau is valid (shared by both operands); keep 2^-tau an FP32 normal
+    tau[i] = max(-120, min(120, i8_exponent(acc / 33.0)));
+    tau_b[i] = (int8_t)tau[i];                                   // byte copy, zero-padded to 512 bins, for k_slice_A's cp.async      // any tau is valid (shared by both operands); keep 2^-tau an FP32 normal
 }
 
 __global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n_rec, const int *__restrict__ tau,
@@ -665,10 +692,16 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
     const Layout &L = ctx->lay;
     const int KT = L.KT8, n_cols = L.NT8 * 64;                  // NT8 counts 64-column units and is even
     const size_t per = (size_t)(L.NT8 / 2) * KT * L.ns8 * kI8SliceBytesB;
+    // zero-padded byte copies of tau and comp8 (k_slice_A stages them 512 bins at a time with cp.async)
+    if (cudaMemsetAsync(ctx->tau8b, 0, (size_t)ctx->D * L.KP512, s) != cudaSuccess ||
+        cudaMemsetAsync(ctx->comp8p, 0, (size_t)L.KP512, s) != cudaSuccess ||
+        cudaMemcpyAsync(ctx->comp8p, ctx->comp8, (size_t)ctx->n_T, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+        return fail(ctx, RW_ERR_CUDA, "slicing setup: %s", cudaGetErrorString(cudaGetLastError()));
     for (int d = 0; d < ctx->D; ++d) {
         const double *Rd = ctx->R + (size_t)d * ctx->R_period_stride;
         int *f = ctx->f_col8 + (size_t)d * ctx->n_rec, *tau = ctx->tau8 + (size_t)d * ctx->n_T;
-        k_tau<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T, tau);
+        k_tau<<<(ctx->n_T + 255) / 256, 256, 0, s>>>(ctx->N_mc + (size_t)d * ctx->n_T, ctx->n_T, tau,
+                                                     ctx->tau8b + (size_t)d * L.KP512);
         k_block_tables<<<KT, 32, 0, s>>>(ctx->What + (size_t)d * kCoefStride * ctx->n_T, tau, ctx->comp8, ctx->n_T, KT,
                                          ctx->blk_hl8 + (size_t)d * 2 * kNumTerms * KT,
                                          ctx->blk_hl8 + ((size_t)d * 2 + 1) * kNumTerms * KT, ctx->blk_cm8);
@@ -683,6 +716,8 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fold_i8<7, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_slice_A<1, 0, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_slice_smem(0));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_slice_A<1, 0, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, i8_slice_smem(0));
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_i8): %s", cudaGetErrorString(e));
     return RW_OK;
 }
@@ -697,11 +732,12 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     const int64_t rows_pad = (Pc + kI8BM - 1) / kI8BM * kI8BM;
     uint8_t *As = reinterpret_cast<uint8_t *>(ctx->A_packed);     // 8 slice bytes per (point, bin): fits the FP64 N'
     const double *What = ctx->What + (size_t)d * kCoefStride * ctx->n_T;
-    const int *tau = ctx->tau8 + (size_t)d * ctx->n_T;
     const unsigned sgrid = (unsigned)(rows_pad / kI8SliceRows);
+    const int8_t *tau_b = ctx->tau8b + (size_t)d * L.KP512;
     const int nst = fast ? 4 : L.ns8;
 #define RW_SLICE_LAUNCH(PASS, SRC, NS, c0, r0, m0, pp, W0)                                                          \
-    k_slice_A<PASS, SRC, NS><<<sgrid, 256, 0, s>>>(c0, r0, m0, pp, Pc, W0, tau, ctx->n_T, KT, nst, ctx->e_row8, As)
+    k_slice_A<PASS, SRC, NS><<<sgrid, 256, i8_slice_smem(SRC), s>>>(c0, r0, ctx->comp8p, pp, Pc, W0, tau_b, ctx->n_T, KT, \
+                                                                    nst, ctx->e_row8, As)
     if (w) {
         const double *N_mc = ctx->N_mc + (size_t)d * ctx->n_T;
         if (L.ns8 == 8) { RW_SLICE_LAUNCH(0, 1, 8, w, nullptr, nullptr, 0, N_mc); RW_SLICE_LAUNCH(1, 1, 8, w, nullptr, nullptr, 0, N_mc); }

@@ -48,7 +48,8 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part, comp8, rate;
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof, R32;
-    size_t B8, f_col8, e_row8, tau8, blk_hl8, blk_cm8;
+    size_t B8, f_col8, e_row8, tau8, blk_hl8, blk_cm8, tau8b, comp8p;
+    int KP512;            // n_T rounded up to 512 bins (staging chunk of k_slice_A)
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
     int KPAD;             // n_T rounded up to kBK
@@ -98,6 +99,8 @@ struct rw_ctx {
     int *tau8;                // [D][n_T] per-bin rescaling exponents (2^tau ~ N_mc)
     double *blk_hl8;          // [D][2: hi, lo][11][KT8] block-wise max / min of W^_b 2^-tau (row-exponent bound)
     int *blk_cm8;             // [KT8] components present in each 32-bin block
+    int8_t *tau8b;            // [D][KP512] tau as bytes, zero-padded (cp.async staging of k_slice_A)
+    uint8_t *comp8p;          // [KP512] comp8, zero-padded
     float *R32;               // [D][2 (hi, lo)][n_rec][KP32] transposed TF32 split of R (RW_CREATE_FP32)
     CUtensorMap tmapA32[2];   // hi, lo of N' (aliases A_packed)
     CUtensorMap *tmapB32;     // host array [2 D]
