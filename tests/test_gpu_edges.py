@@ -213,19 +213,20 @@ def test_eval_batch_is_cuda_graph_capturable(rw, orc):
     inp = wl.make("cfg1_tiny_nsi")
     params, kinds = wl.scan_points("cfg1_tiny_nsi")
     ref = orc.eval_batch(inp, params, kinds, nthreads=4)
-    ctx = rw.Reweighter(inp, max_batch=121)
-    for P, mode in ((1, "auto"), (121, "auto"), (121, "collapsed")):
+    ctx = rw.Reweighter(inp, max_batch=121, sliced=True)
+    for P, mode in ((1, "auto"), (121, "auto"), (121, "collapsed"), (121, "sliced")):
         buf = _cuda(params[:P].copy())
         out = torch.empty(P, dtype=torch.float64, device="cuda")
+        kw = dict(mode="gemm", sliced=True) if mode == "sliced" else dict(mode=mode)
         side = torch.cuda.Stream()
         side.wait_stream(torch.cuda.current_stream())
         with torch.cuda.stream(side):
-            ctx.eval_batch(buf, kinds, out=out, mode=mode)          # warm-up outside capture
+            ctx.eval_batch(buf, kinds, out=out, **kw)               # warm-up outside capture
         torch.cuda.current_stream().wait_stream(side)
         torch.cuda.synchronize()
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g):
-            ctx.eval_batch(buf, kinds, out=out, mode=mode)
+            ctx.eval_batch(buf, kinds, out=out, **kw)
         for lo in (0, 60):                                           # replay with other points in the same buffer
             sel = np.arange(lo, lo + P) % 121
             buf.copy_(_cuda(params[sel]))
