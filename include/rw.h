@@ -173,7 +173,8 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
  * parameters, flux shapes: PAPER.md:220).
  *   w          [P][n_T] row-major DEVICE pointer, finite and >= 0 (not validated; garbage in, garbage out)
  *   out_m2lnL  [P] device pointer;  out_mu NULL or [P][D][n_rec] device pointer
- *   flags      RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM (COLLAPSED, RW_PARAM_HOST, RW_OUT_HOST: RW_ERR_UNSUPPORTED)
+ *   flags      RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM, RW_SLICED / RW_SLICED_FAST (dense fold of more than 4 points)
+ *              (COLLAPSED, RW_FP32, RW_PARAM_HOST, RW_OUT_HOST: RW_ERR_UNSUPPORTED)
  * Asynchronous and stream-ordered like rw_eval_batch; P may be 0 and may exceed max_batch. */
 int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
                     uint32_t flags, void *cuda_stream);
@@ -187,7 +188,7 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
  *   param, param_kind, P, k   as rw_eval_batch (DEVICE param; kinds RW_EPS_* and RW_MU_NU only)
  *   P_e_pts                   [P][n_E] device pointer, values in [0,1] (not validated)
  *   out_m2lnL [P], out_mu NULL or [P][D][n_rec]   device pointers
- *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM
+ *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM, RW_SLICED / RW_SLICED_FAST
  * Needs a single-component context created without explicit P_mu / P_tau.  Asynchronous and stream-ordered. */
 int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                 const double *P_e_pts, double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
@@ -202,7 +203,8 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
  *   param, param_kind, P, k   as rw_eval_batch (DEVICE param only)
  *   s0, sigma                 centre and width of the Gaussian pull on s; sigma <= 0 or +inf-like: no pull
  *   out_m2lnL [P], out_scale [P] or NULL   device pointers
- *   flags                     RW_FULL_EQ18; RW_MODE_AUTO/STREAM/GEMM (dense fold) or RW_MODE_COLLAPSED
+ *   flags                     RW_FULL_EQ18; RW_MODE_AUTO/STREAM/GEMM (dense fold) or RW_MODE_COLLAPSED; RW_FP32,
+ *                             RW_SLICED, RW_SLICED_FAST select the contraction of the dense fold as in rw_eval_batch
  * Asynchronous and stream-ordered; P may exceed max_batch. */
 int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                     double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,
@@ -213,7 +215,8 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
  * Eq. (4)/(8) and in the rates of Eq. (17), so d mu / d theta_m is the same fold applied to derivative coefficients;
  *     out_grad[p][m] = sum over bins and periods of 2 (1 - n/mu) d mu / d theta_m      (n = 0: 2 d mu / d theta_m).
  * A point costs 1 + k rows of the batched fold.  DEVICE pointers only; flags: RW_FULL_EQ18 (value only) and the
- * fold modes; max_batch must be >= 1 + k.  Asynchronous and stream-ordered; P may exceed max_batch. */
+ * fold modes (RW_FP32, RW_SLICED, RW_SLICED_FAST: RW_ERR_UNSUPPORTED, derivative rows change sign); max_batch must be
+ * >= 1 + k.  Asynchronous and stream-ordered; P may exceed max_batch. */
 int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                  double *out_m2lnL, double *out_grad /*[P][k]*/, uint32_t flags, void *cuda_stream);
 
