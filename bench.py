@@ -190,7 +190,7 @@ def main():
                for key in ("E", "flux_w", "P_e", "T", "N_mc", "R", "bkg", "counts")}
     dev_inp["f_tau"] = inp["f_tau"]
     max_batch = args.max_batch or (16384 if name == "cfg5_joint6" else P)
-    sliced_ok = n_T <= 18560
+    sliced_ok = True
     ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=True, sliced=sliced_ok)   # + operand copies for the opt-in legs
     param_dev = torch.from_numpy(params).to(dev)
     out_dev = torch.empty(P, dtype=torch.float64, device=dev)

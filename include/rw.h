@@ -96,8 +96,7 @@ enum {
 /* rw_inputs.create_flags */
 enum {
     RW_CREATE_FP32 = 1u << 0,  /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
-    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into 8 (7 for n_T > 8192) INT8 slices (at most the bytes of R) for RW_SLICED;
-                                  n_T <= 18560 */
+    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into 8 (7 for n_T > 8192) INT8 slices (at most the bytes of R) for RW_SLICED */
 };
 
 /* Physical constants.  The paper prints symbols only; any field that is 0

@@ -431,9 +431,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: TF32 split of R failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
     if (rc == RW_OK && L.sliced) {
-        if (ctx->n_T > 18560)
-            rc = fail(nullptr, RW_ERR_UNSUPPORTED, "rw_create: RW_CREATE_SLICED needs n_T <= 18560 (exact int32 accumulation)");
-        if (rc == RW_OK) rc = i8_setup(ctx, s);
+        rc = i8_setup(ctx, s);
         if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: slicing R failed: %s", cudaGetErrorString(cudaGetLastError()));
     }

@@ -8,7 +8,8 @@
 // with BALANCED digits: a_0 in [0, 129] (unsigned; one spare bit keeps the carry), a_s in [-128, 127] for s > 0.
 // The contraction becomes NS (NS + 1) / 2 INT8 tensor-core products with EXACT int32 accumulation (tcgen05.mma
 // kind::i8, accumulators in TMEM; |digit product| <= 129 x 128, NS pairs per accumulator:
-// 7 x 16512 x 18560 bins < 2^31 and 8 x 16512 x 8192 < 2^31):
+// 7 x 16512 x 18560 bins < 2^31 and 8 x 16512 x 8192 < 2^31; contractions longer than 16384 bins are accumulated in
+// segments, drained and summed in FP64 by the epilogue):
 //     mu[p][k] - bkg[k] = 2^(e_p + f_k - 14) sum_{d=0..NS-1} 2^(-8d) sum_{s+t=d} sum_i a_s[p][i] b_t[i][k].
 // Balanced digits are what lets 8-bit slices through at n_T = 16384 (unsigned ones would need 7-bit slices, i.e.
 // 8 slices and 36 products for the same 55 bits that 7 slices and 28 products give here).
@@ -40,6 +41,8 @@ constexpr int kI8Threads = 320;                                 // TMA warp, MMA
 #endif
 constexpr int kI8SlotBytes = 65536, kI8Stages = RW_I8_STAGES;   // a slot: N' slices in its first half, R slices in its second
 constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 4 * kI8BN * 8 + 256 + 1024;
+constexpr int kI8SegKT = 512;       // k-blocks (16384 bins) accumulated in int32 before the epilogue drains TMEM:
+                                    // 7 pairs x 129 x 128 x 16384 bins < 2^31; longer contractions go in segments
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
 
 // ---------------------------------------------------------------------------------------------- slicing
@@ -555,11 +558,13 @@ k_fold_i8(const I8Work W)
             const uint32_t idesc = (2u << 4) | ((uint32_t)(kI8BN >> 3) << 17) | ((uint32_t)(kI8BM >> 4) << 24);
             int stage = 0; uint32_t phase = 0, pseq = 0;
             for (int t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-                // ---- pass 0: diagonals 0..3 into accumulators 0..3
-                i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);        // the epilogue has drained the previous pass
+                // ---- pass 0: diagonals 0..3 into accumulators 0..3, one segment of <= 16384 bins at a time
+                for (int k0 = 0; k0 < KT; k0 += kI8SegKT) {
+                const int k1 = min(KT, k0 + kI8SegKT);
+                i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);        // the epilogue has drained the previous segment / pass
                 ++pseq;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                for (int kt = 0; kt < KT; kt += 2) {
+                for (int kt = k0; kt < k1; kt += 2) {
                     i8_mbar_wait(full_bar + 8 * stage, phase);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const int nk = min(2, KT - kt);
@@ -572,18 +577,20 @@ k_fold_i8(const I8Work W)
                                 umma_i8(tmem_base + d * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
                                         i8_desc(sb + (d - s) * kI8SliceBytesB, 2048, 128),
                                         idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u),
-                                        (kt + h > 0 || s > 0) ? 1u : 0u);
+                                        (kt + h > k0 || s > 0) ? 1u : 0u);
                     }
                     i8_commit(empty_bar + 8 * stage);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
                 i8_commit(tfull_bar);
-                if (FAST) continue;
+                }
                 // ---- pass 1: diagonals 4..NS-1 into accumulators 0..NS-5
+                for (int k0 = 0; k0 < (FAST ? 0 : KT); k0 += kI8SegKT) {
+                const int k1 = min(KT, k0 + kI8SegKT);
                 i8_mbar_wait(tempty_bar, (pseq & 1) ^ 1);
                 ++pseq;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                for (int kt = 0; kt < KT; ++kt) {
+                for (int kt = k0; kt < k1; ++kt) {
                     i8_mbar_wait(full_bar + 8 * stage, phase);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t sa = sbase + stage * kSlot, sb = sa + kBOff;
@@ -593,11 +600,12 @@ k_fold_i8(const I8Work W)
                         for (int s = 0; s <= d; ++s)
                             umma_i8(tmem_base + (d - 4) * kI8BN, i8_desc(sa + s * kI8SliceBytesA, 2048, 128),
                                     i8_desc(sb + (d - s) * kI8SliceBytesB, 2048, 128),
-                                    idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u), (kt > 0 || s > 0) ? 1u : 0u);
+                                    idesc | (s > 0 ? 1u << 7 : 0u) | (d - s > 0 ? 1u << 10 : 0u), (kt > k0 || s > 0) ? 1u : 0u);
                     i8_commit(empty_bar + 8 * stage);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
                 i8_commit(tfull_bar);
+                }
             }
         }
     } else {
@@ -626,20 +634,30 @@ k_fold_i8(const I8Work W)
             const double rscale = (e == kI8BadRow) ? __longlong_as_double(0x7ff8000000000000LL) : ldexp(1.0, e - 14);
             const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + 64 * half;
             double v[4][16];
-            // ---- pass 0: v = sum_{d=0..3} 2^(-8d) acc_d, kept in registers
-            i8_mbar_wait(tfull_bar, pseq & 1);
-            ++pseq;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-            for (int g = 0; g < 4; ++g) {
+            for (int g = 0; g < 4; ++g)
 #pragma unroll
-                for (int d = 3; d >= 0; --d) i8_horner16(taddr + d * kI8BN + 16 * g, v[g], d == 3);
+                for (int j = 0; j < 16; ++j) v[g][j] = 0.0;
+            // ---- pass 0: v = sum_{d=0..3} 2^(-8d) acc_d, kept in registers (summed over the <= 16384-bin segments)
+            const int nseg = (KT + kI8SegKT - 1) / kI8SegKT;
+            for (int seg = 0; seg < nseg; ++seg) {
+                i8_mbar_wait(tfull_bar, pseq & 1);
+                ++pseq;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    double u[16];
+#pragma unroll
+                    for (int d = 3; d >= 0; --d) i8_horner16(taddr + d * kI8BN + 16 * g, u, d == 3);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[g][j] += u[j];
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) i8_mbar_arrive(tempty_bar);
             }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) i8_mbar_arrive(tempty_bar);
             // ---- pass 1: v += 2^-32 sum_{d=4..NS-1} 2^(-8(d-4)) acc_(d-4)
-            if (!FAST) {
+            for (int seg = 0; seg < (FAST ? 0 : nseg); ++seg) {
                 i8_mbar_wait(tfull_bar, pseq & 1);
                 ++pseq;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");

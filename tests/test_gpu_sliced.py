@@ -241,3 +241,13 @@ def test_sliced_degenerate_and_boundary_shapes_against_the_oracle(orc, n_T, n_re
     params, kinds = wl.random_points(P, [wl.EPS_EE_L, wl.EPS_MM_L, wl.MU_NU], seed=162 + n_T)
     ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
     _check(inp, params, kinds, ref, mu_ref, scale)
+
+
+def test_sliced_contraction_longer_than_one_int32_segment(orc):
+    """n_T = 20000 > 16384: the int32 accumulators are drained after 512 k-blocks (16384 bins: 7 pairs x 129 x 128 x
+    16384 < 2^31) and the segments are summed in FP64 in the epilogue's registers; both passes, and the fast mode."""
+    inp = wl.make_custom(n_E=24, n_T=20000, n_rec=70, n_periods=1, seed=171, tail=0.0)
+    params, kinds = wl.random_points(130, [wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU], seed=172)
+    ref, mu_ref, scale = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=CORES)
+    _check(inp, params, kinds, ref, mu_ref, scale)
+    _check_fast(orc, inp, params, kinds)
