@@ -395,6 +395,33 @@ def main():
     except Exception as exc:               # noqa: BLE001
         sliced_leg = {"unavailable": str(exc)[:160]}
 
+    # the other entry points of the same path, timed on a slice of the same scan: context only
+    next_rows = None
+    try:
+        if P > 4 and rank == 0:
+            kin = [int(x) for x in kinds]
+            nr = {}
+            Pp = int(min(P, max_batch, 4096))
+            pp = param_dev[:Pp].contiguous()
+            t = timed(lambda: ctx.eval_profile(pp, kinds, s0=1.0, sigma=0.05), 3)
+            nr["profile"] = {"points": Pp, "ms_per_call": t, "evals_per_s": Pp / t * 1e3,
+                             "note": "rw_eval_profile: fold with mu to a scratch + Newton per point (k_profile)"}
+            Pg = int(min(P, max(1, min(max_batch, 4096) // (1 + k))))
+            pg = param_dev[:Pg].contiguous()
+            t = timed(lambda: ctx.eval_grad(pg, kinds), 3)
+            nr["gradient"] = {"points": Pg, "fold_rows": Pg * (1 + k), "ms_per_call": t, "evals_per_s": Pg / t * 1e3,
+                              "note": "rw_eval_grad: 1 + k fold rows per point, then k_grad"}
+            if ctx.n_periods >= 1 and all(x < 7 for x in kin) and "P_mu" not in inp and int(inp.get("n_comp", 1) or 1) == 1:
+                Pe = int(min(P, max_batch, 1024))
+                pe = param_dev[:Pe].contiguous()
+                tab = torch.from_numpy(np.ascontiguousarray(inp["P_e"])).to(dev)[None, :].repeat(Pe, 1).contiguous()
+                t = timed(lambda: ctx.eval_pee(pe, kinds, tab), 3)
+                nr["per_point_pee"] = {"points": Pe, "n_E": int(tab.shape[1]), "ms_per_call": t, "evals_per_s": Pe / t * 1e3,
+                                       "note": "rw_eval_pee: spectrum on the (E x T) grid per point (FP64 ALU), then the dense fold"}
+            next_rows = nr
+    except Exception as exc:                   # noqa: BLE001
+        next_rows = {"unavailable": str(exc)[:160]}
+
     # library DGEMM of the shape of one chunk of the fold (cuBLAS FP64 as a reference point for the
     # denominator).  Context only: no N' generation, no Poisson epilogue, no reduction, and mu goes to HBM.
     lib_dgemm = None
@@ -450,7 +477,7 @@ def main():
                         "matches_device_path": same},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "single_eval": single,
                 "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg, "sliced_mode": sliced_leg,
-                "library_dgemm": lib_dgemm, "clocks": clocks, "all_finite": finite,
+                "library_dgemm": lib_dgemm, "next_rows": next_rows, "clocks": clocks, "all_finite": finite,
                 "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
                                  "the authors' own multi-component model; other hardware and inputs, not comparable"}
         print(json.dumps(line))
