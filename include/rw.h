@@ -68,11 +68,14 @@ enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
 enum {
     RW_DEVIANCE    = 0u,       /* default: 2 sum [mu - n + n ln(n/mu)] (Eq. 18 minus its saturated value) */
     RW_FULL_EQ18   = 1u << 0,  /* literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)] */
-    RW_MODE_AUTO   = 0u,       /* <= 4 points: one-launch streaming path; else: DMMA batched contraction */
-    RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P) */
-    RW_MODE_GEMM   = 2u << 4,  /* force the FP64 tensor-core (DMMA) contraction */
+    RW_MODE_AUTO   = 0u,       /* <= 4 points: one-launch streaming path; <= 64: one-launch streaming DMMA kernel;
+                                  else: tiled DMMA batched contraction */
+    RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P, groups of 16 points per launch) */
+    RW_MODE_GEMM   = 2u << 4,  /* force the tiled FP64 tensor-core (DMMA) contraction */
     RW_MODE_COLLAPSED = 3u << 4, /* opt-in: rank-K prefolded templates (exact, O(K n_rec) per point); see below */
-    RW_MODE_MASK   = 3u << 4,
+    RW_MODE_RIDGE  = 4u << 4,  /* force the streaming DMMA kernel (any P, groups of 64 points per launch): R is read
+                                  from HBM once per group and contracted on the FP64 tensor cores in the same pass */
+    RW_MODE_MASK   = 7u << 4,
     RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
     RW_OUT_HOST    = 1u << 9,  /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
     RW_FP32        = 1u << 10, /* opt-in reduced precision for the batched contraction (rw_eval_batch, > 4 points, dense

@@ -67,6 +67,12 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     L->stream_splits = splits;
+    L->ridge_strips = (int)((n_rec + kRidgeCols - 1) / kRidgeCols);
+    size_t ridge_rows_max = 0;           // rows of the parked partial tiles: ranges x tile height, largest variant
+    for (int v = 0; v < 4; ++v) {
+        const int ns = ridge_plan((int)n_T, (int)n_rec, (int)D, v, kPlanSMs, &L->ridge_rows[v]);
+        if ((size_t)ns * (8u << v) > ridge_rows_max) ridge_rows_max = (size_t)ns * (8u << v);
+    }
     const size_t nstrip2 = (n_rec + 255) / 256;
     const size_t mu_ld = (n_rec + 1) & ~(size_t)1;
 
@@ -98,7 +104,12 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
     size_t part_gemm = D * (size_t)(L->sliced ? L->NT8 : L->n_tiles_n) * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
-    L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
+    {
+        size_t rows_stream = (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB;
+        L->mu_part = take(D * (rows_stream > ridge_rows_max ? rows_stream : ridge_rows_max) * mu_ld * 8);
+    }
+    L->ridge_cnt = take((D * (size_t)L->ridge_strips + 1) * 4);
+    L->ridge_part = take(D * (size_t)L->ridge_strips * kRidgeMaxP * 8);
     L->out_stage = take((size_t)max_batch * 8);
     {   // split-K scratch: at most 8 work items per SM, and never more than 16 k-ranges of every 16-point tile
         int64_t items = (int64_t)L->n_tiles_n * ((L->MC + 15) / 16) * 16;
@@ -160,9 +171,19 @@ static const char *flag_message(int f)
     return "invalid input";
 }
 
-// RW_MODE_AUTO: the one-launch HBM-streaming path for up to 4 points (measured on B200: it wins there at every
-// response size), the DMMA contraction (tile height 16..128, split-K) beyond.
-static bool auto_stream(const rw_ctx *, int64_t P) { return P <= 4; }
+// RW_MODE_AUTO (measured on B200, config-4 size): one point -> the one-launch HBM-streaming kernel; 2..16 points ->
+// the one-launch streaming DMMA kernel (R read once at HBM speed, contraction on the FP64 tensor cores); beyond -> the
+// tiled DMMA contraction (tile height 32..128, split-K).  The opt-in contractions (prec != 0) replace the last two.
+constexpr int kAutoRidgeMax = 16;
+static bool auto_stream(const rw_ctx *, int64_t P, int prec) { return prec == 0 ? P <= 1 : P <= 4; }
+static bool use_stream(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
+{
+    return mode == RW_MODE_STREAM || (mode == RW_MODE_AUTO && auto_stream(ctx, P, prec));
+}
+static bool use_ridge(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
+{
+    return mode == RW_MODE_RIDGE || (mode == RW_MODE_AUTO && prec == 0 && !auto_stream(ctx, P, prec) && P <= kAutoRidgeMax);
+}
 
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
@@ -173,7 +194,7 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
-    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps));
+    const bool stream_mode = use_stream(ctx, mode, Ps, prec);
     if (mode == RW_MODE_COLLAPSED) {
         const int nstrip = (n_rec + 511) / 512;
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
@@ -188,6 +209,13 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
                                             dout + g0, full, mu, s));
+        }
+    } else if (use_ridge(ctx, mode, Ps, prec)) {
+        for (int64_t g0 = 0; g0 < Ps; g0 += kRidgeMaxP) {
+            const int Pb = (int)((Ps - g0 < kRidgeMaxP) ? Ps - g0 : kRidgeMaxP);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
+                                           dout + g0, full, mu, s));
         }
     } else {
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
@@ -344,6 +372,8 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->G = (double *)(ws + L.G);          ctx->ident = (double *)(ws + L.ident);
     ctx->stream_cnt = (int *)(ws + L.stream_cnt);
     ctx->strip_part = (double *)(ws + L.strip_part);
+    ctx->ridge_cnt = (int *)(ws + L.ridge_cnt);
+    ctx->ridge_part = (double *)(ws + L.ridge_part);
     ctx->param_stage = (double *)(ws + L.param_stage);
     ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);
     ctx->partial = (double *)(ws + L.partial);
@@ -406,6 +436,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
     if (n_comp > 1 && !host) RW_TRY(launch_comp8(ctx, in->comp_of_T, s));
     RW_TRY(cudaMemsetAsync(ctx->stream_cnt, 0, (D * (size_t)L.stream_strips + 1) * 4, s));
+    RW_TRY(cudaMemsetAsync(ctx->ridge_cnt, 0, (D * (size_t)L.ridge_strips + 1) * 4, s));
     RW_TRY(launch_flavour(ctx, have_mt ? 1 : 0, f_tau, s));
     if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
     RW_TRY(launch_setup(ctx, s));
@@ -493,20 +524,26 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             }
         }
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
-        if ((mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, Ps))) {
-            // a handful of points: one launch per <= 16 points does a1-a4 (coefficients computed in the kernel)
+        const bool stream_mode = use_stream(ctx, mode, Ps, prec);
+        if (stream_mode || use_ridge(ctx, mode, Ps, prec)) {
+            // up to 64 points: ONE launch per group does a1-a4 (coefficients computed in the kernel) -- the
+            // HBM-streaming kernel (groups of 16) or the streaming DMMA kernel (groups of 64)
             Kinds kd;
             kd.k = k;
             for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
-            for (int64_t g0 = 0; g0 < Ps; g0 += kStreamMaxPB) {
-                const int Pb = (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB);
+            const int group = stream_mode ? kStreamMaxPB : kRidgeMaxP;
+            for (int64_t g0 = 0; g0 < Ps; g0 += group) {
+                const int Pb = (int)((Ps - g0 < group) ? Ps - g0 : group);
                 double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
-                if (k > 0)
-                    RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, dparam + g0 * k, &kd, nullptr, Pb, dout + g0, full, mu, s));
-                else {
+                const double *cf = nullptr, *pr = (k > 0) ? dparam + g0 * k : nullptr;
+                if (k == 0) {
                     RW_CUDA(ctx, launch_coef(ctx, nullptr, Pb, 0, kinds, s));
-                    RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef, nullptr, nullptr, nullptr, Pb, dout + g0, full, mu, s));
+                    cf = ctx->coef;
                 }
+                if (stream_mode)
+                    RW_CUDA(ctx, launch_fold_stream(ctx, cf, pr, k > 0 ? &kd : nullptr, nullptr, Pb, dout + g0, full, mu, s));
+                else
+                    RW_CUDA(ctx, launch_fold_ridge(ctx, cf, pr, k > 0 ? &kd : nullptr, nullptr, Pb, dout + g0, full, mu, s));
             }
         } else {
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
@@ -594,12 +631,17 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
     const size_t n_T = ctx->n_T;
-    const bool stream_mode = (mode == RW_MODE_STREAM) || (mode == RW_MODE_AUTO && auto_stream(ctx, P));
-    if (stream_mode) {
+    if (use_stream(ctx, mode, P, prec)) {
         for (int64_t g0 = 0; g0 < P; g0 += kStreamMaxPB) {
             const int Pb = (int)((P - g0 < kStreamMaxPB) ? P - g0 : kStreamMaxPB);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
+        }
+    } else if (use_ridge(ctx, mode, P, prec)) {
+        for (int64_t g0 = 0; g0 < P; g0 += kRidgeMaxP) {
+            const int Pb = (int)((P - g0 < kRidgeMaxP) ? P - g0 : kRidgeMaxP);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
     } else {
         for (int64_t c0 = 0; c0 < P; c0 += L.MC) {

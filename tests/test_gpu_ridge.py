@@ -1,0 +1,166 @@
+"""GPU parity of the streaming DMMA kernel (k_fold_ridge, RW_MODE_RIDGE and RW_MODE_AUTO for 5..64 points) against
+the CPU oracle, element by element through the C ABI.  Same bars as tests/test_gpu_parity.py: mu within 1e-12
+relative, -2lnL within 1e-9 + 1e-12 x sum_k 2|term_k| (reading T)."""
+import numpy as np
+import pytest
+
+from paper_2607_00488_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MU_RTOL = 1e-12
+
+
+def m2lnl_tol(abs_scale):
+    return 1e-9 + 1e-12 * abs_scale
+
+
+@pytest.fixture(scope="module")
+def rw():
+    import torch
+    from paper_2607_00488_b200 import binding
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    binding.load_library()
+    return binding
+
+
+def _cuda(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _check(rw, orc, inp, params, kinds, mode="ridge", max_batch=None, full_eq18=False):
+    import torch
+    P = params.shape[0]
+    ref, mu_ref, ab = orc.eval_batch(inp, params, kinds, want_mu=True, want_abs=True, nthreads=8, full_eq18=full_eq18)
+    ctx = rw.Reweighter(inp, max_batch=max_batch or max(1, P))
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode=mode, full_eq18=full_eq18)
+    out2 = ctx.eval_batch(_cuda(params), kinds, mode=mode, full_eq18=full_eq18)          # without mu; tickets reset
+    torch.cuda.synchronize()
+    out, mu, out2 = out.cpu().numpy(), mu.cpu().numpy(), out2.cpu().numpy()
+    ctx.close()
+    rel = np.abs(mu - mu_ref) / np.abs(mu_ref)
+    assert np.all(rel <= MU_RTOL), "mu rel err max %.3e" % rel.max()
+    err = np.abs(out - ref)
+    assert np.all(err <= m2lnl_tol(ab)), "-2lnL abs err max %.3e (ref %.6e)" % (err.max(), ref[err.argmax()])
+    assert np.array_equal(out, out2), "a second launch on the same context must reproduce the first bit for bit"
+
+
+@pytest.mark.parametrize("P", [1, 5, 8, 9, 16, 17, 32, 33, 64])
+def test_every_tile_height_on_a_ragged_shape(rw, orc, P):
+    """Tile heights 8 / 16 / 32 / 64 with ragged point counts; n_T = 1500 (several row ranges, the last chunk of
+    every range partial, n_T not a multiple of 4), n_rec = 330 (two 256-column strips, ragged, 16-column groups
+    partly outside), two periods, dead bins, all seven parameter kinds."""
+    inp = wl.make_custom(n_E=24, n_T=1501, n_rec=330, n_periods=2, seed=17, dead_fraction=0.1)
+    params, kinds = wl.random_points(P, list(range(7)), seed=18 + P)
+    _check(rw, orc, inp, params, kinds, mode="ridge")
+    if P > 4:
+        _check(rw, orc, inp, params, kinds, mode="auto")
+
+
+def test_odd_n_rec_single_range_and_groups_of_64(rw, orc):
+    """n_rec = 53 (odd: padded copy of R), n_T = 77 (one row range, one partial chunk), 150 points forced through
+    the kernel in groups of 64 + 64 + 22, with the library slicing at max_batch = 100 on top."""
+    inp = wl.make_custom(n_E=31, n_T=77, n_rec=53, n_periods=2, seed=5)
+    params, kinds = wl.random_points(150, [wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU], seed=6)
+    _check(rw, orc, inp, params, kinds, mode="ridge", max_batch=100)
+
+
+def test_literal_eq18_and_zero_count_bins(rw, orc):
+    inp = wl.make_custom(n_E=25, n_T=300, n_rec=290, n_periods=1, seed=24)
+    inp["counts"][0, :7] = 0.0                       # n = 0 => term = mu
+    params, kinds = wl.random_points(40, [0, 4, 6], seed=25)
+    _check(rw, orc, inp, params, kinds, mode="ridge", full_eq18=True)
+
+
+def test_zero_mu_nan_parameters(rw, orc):
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=48, n_rec=32, n_periods=1, seed=24)
+    inp["R"][0][:, 3] = 0.0
+    inp["bkg"][0, 3] = 0.0                           # mu = 0 < n in that bin => +inf
+    inp["counts"][0, 3] = 4.0
+    params, kinds = wl.random_points(20, [0, 4], seed=25)
+    ctx = rw.Reweighter(inp, max_batch=32)
+    out = ctx.eval_batch(_cuda(params), kinds, mode="ridge")
+    torch.cuda.synchronize()
+    assert np.all(np.isposinf(out.cpu().numpy()))
+    inp2 = wl.make_custom(n_E=25, n_T=48, n_rec=32, n_periods=1, seed=24)
+    ref, scale = orc.eval_batch(inp2, params, kinds, want_abs=True)
+    bad = params.copy()
+    bad[7, 1] = np.nan
+    ctx2 = rw.Reweighter(inp2, max_batch=32)
+    out = ctx2.eval_batch(_cuda(bad), kinds, mode="ridge").cpu().numpy()
+    ok = np.arange(20) != 7
+    assert np.isnan(out[7]) and np.all(np.abs(out[ok] - ref[ok]) <= m2lnl_tol(scale[ok]))
+    ctx.close()
+    ctx2.close()
+
+
+def test_components_and_rates(rw, orc):
+    """Eq. 17 structure: three signal components with their own flux / flavour tables and per-point rate scales."""
+    import torch
+    inp = wl.make_components(n_comp=3, n_E=41, n_T=200, n_rec=270, n_periods=2, seed=77)
+    kinds = [wl.EPS_EE_L, wl.EPS_MM_R, wl.MU_NU, rw.RW_RATE_0, rw.RW_RATE_0 + 2]
+    params, kinds = wl.random_points(23, kinds, seed=78)
+    ref, mu_ref, ab = orc.eval_components(inp, params, kinds, want_mu=True, want_abs=True)
+    ctx = rw.Reweighter(inp, max_batch=64)
+    out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="ridge")
+    torch.cuda.synchronize()
+    rel = np.abs(mu.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= MU_RTOL
+    assert np.all(np.abs(out.cpu().numpy() - ref) <= m2lnl_tol(ab))
+    ctx.close()
+
+
+def test_caller_weights_profile_and_gradient_take_the_same_kernel(rw, orc):
+    """rw_eval_weights, rw_eval_profile and rw_eval_grad with 5..64 fold rows run on k_fold_ridge in RW_MODE_AUTO."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=410, n_rec=300, n_periods=2, seed=31)
+    rng = np.random.default_rng(32)
+    w = rng.uniform(0.2, 3.0, size=(19, 410))
+    ref, mu_ref, ab = orc.eval_weights(inp, w, want_mu=True, want_abs=True)
+    ctx = rw.Reweighter(inp, max_batch=64)
+    out, mu = ctx.eval_weights(_cuda(w), want_mu=True)
+    torch.cuda.synchronize()
+    rel = np.abs(mu.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= MU_RTOL
+    assert np.all(np.abs(out.cpu().numpy() - ref) <= m2lnl_tol(ab))
+    params, kinds = wl.random_points(6, [0, 1, 4, 6], seed=33)          # 6 x (1 + 4) = 30 fold rows
+    val, grad = ctx.eval_grad(_cuda(params), kinds)
+    torch.cuda.synchronize()
+    v_ref, g_ref = orc.eval_grad(inp, params, kinds)
+    assert np.all(np.abs(val.cpu().numpy() - v_ref) <= 1e-9 + 1e-11 * np.abs(v_ref))
+    floor = 1e-11 * np.asarray(inp["bkg"]).sum()      # derivative rows come back as (d mu + bkg) - bkg
+    assert np.all(np.abs(grad.cpu().numpy() - g_ref) <= 1e-10 * np.abs(g_ref) + floor)
+    prof, shat = ctx.eval_profile(_cuda(params), kinds, s0=1.0, sigma=0.1)
+    torch.cuda.synchronize()
+    p_ref, s_ref, p_abs = orc.eval_profile(inp, params, kinds, s0=1.0, sigma=0.1, want_abs=True)
+    assert np.all(np.abs(shat.cpu().numpy() - s_ref) <= 1e-10 * np.maximum(s_ref, 1e-3))
+    assert np.all(np.abs(prof.cpu().numpy() - p_ref) <= 1e-9 + 1e-12 * (p_abs + np.abs(p_ref)))
+    ctx.close()
+
+
+def test_cuda_graph_capture_of_a_ridge_call(rw, orc):
+    """The kernel only enqueues work and resets its own tickets: a 16-point call replays from a CUDA graph."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=300, n_rec=130, n_periods=1, seed=41)
+    params, kinds = wl.random_points(16, [0, 1], seed=42)
+    ref, scale = orc.eval_batch(inp, params, kinds, want_abs=True)
+    ctx = rw.Reweighter(inp, max_batch=16)
+    p = _cuda(params)
+    out = torch.empty(16, dtype=torch.float64, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        ctx.eval_batch(p, kinds, out=out)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        ctx.eval_batch(p, kinds, out=out)
+    for _ in range(3):
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.all(np.abs(out.cpu().numpy() - ref) <= m2lnl_tol(scale))
+    ctx.close()
