@@ -145,7 +145,11 @@ int rw_workspace_bytes(const rw_inputs *in, int64_t max_batch, size_t *bytes);
 
 /* Validate inputs, place tables in the workspace, run the setup kernels (basis spectra, S_SM,
  * pre-scaled basis W^, saturated constant) on `cuda_stream`, and synchronise that stream once.
- * dev_workspace: device pointer, 256-byte aligned, >= rw_workspace_bytes; owned by ctx until destroy. */
+ * dev_workspace: device pointer, 256-byte aligned, >= rw_workspace_bytes; owned by ctx until destroy.
+ * max_batch (an addition to the north_star signature): the library never allocates device memory, so the per-call
+ * scratch (coefficients, the reweighted spectrum of a chunk, partial sums) is part of the workspace and has to be
+ * sized when the workspace is; it must equal the value given to rw_workspace_bytes.  Calls with more points are
+ * processed in slices of max_batch. */
 int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_t workspace_bytes,
               void *cuda_stream, rw_ctx **out);
 
@@ -244,10 +248,6 @@ int rw_destroy(rw_ctx *ctx);
 
 const char *rw_strerror(int status);
 const char *rw_last_error(const rw_ctx *ctx); /* ctx may be NULL: last rw_create failure of this thread */
-
-/* Measurement helper (not part of the method): register-resident FP64 issue-rate probe.
- * kind 0 = DFMA, 1 = DMMA m8n8k4.  Runs on `cuda_stream`, synchronises, returns TFLOP/s. */
-int rw_probe_fp64_peak(int32_t kind, int32_t iters, double *tflops, void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -29,7 +29,7 @@ _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, 
 
 EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_eval_pee", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
-           "rw_last_error", "rw_probe_fp64_peak")
+           "rw_last_error")
 
 _dp = C.POINTER(C.c_double)
 
@@ -100,9 +100,8 @@ def load_library():
     L.rw_strerror.restype = C.c_char_p
     L.rw_last_error.argtypes = [C.c_void_p]
     L.rw_last_error.restype = C.c_char_p
-    L.rw_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
     for f in ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
-              "rw_destroy", "rw_probe_fp64_peak", "rw_profile_begin", "rw_profile_end"):
+              "rw_destroy", "rw_profile_begin", "rw_profile_end"):
         getattr(L, f).restype = C.c_int
     _lib = L
     return L
@@ -110,16 +109,6 @@ def load_library():
 
 def _stream_ptr():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
-
-
-def probe_fp64_peak(kind, iters=20000):
-    """TFLOP/s of the register-resident FP64 probe (0 = DFMA, 1 = DMMA m8n8k4)."""
-    L = load_library()
-    out = C.c_double(0.0)
-    rc = L.rw_probe_fp64_peak(int(kind), int(iters), C.byref(out), _stream_ptr())
-    if rc != 0:
-        raise RwError(rc, L.rw_strerror(rc).decode())
-    return out.value
 
 
 class _DevicePointer:

@@ -10,7 +10,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librw.so")
-SOURCES = ["rw_api.cu", "rw_setup.cu", "rw_coef.cu", "rw_fold_stream.cu", "rw_fold_gemm.cu", "rw_fold_ridge.cu", "rw_fold_tf32.cu", "rw_fold_i8.cu", "rw_collapsed.cu", "rw_profile.cu", "rw_grad.cu", "rw_pee.cu", "rw_probe.cu"]
+SOURCES = ["rw_api.cu", "rw_setup.cu", "rw_coef.cu", "rw_fold_stream.cu", "rw_fold_gemm.cu", "rw_fold_ridge.cu", "rw_fold_tf32.cu", "rw_fold_i8.cu", "rw_collapsed.cu", "rw_profile.cu", "rw_grad.cu", "rw_pee.cu"]
+PROBE_LIB = os.path.join(HERE, "librw_probe.so")      # bench-only FP64 peak probe (include/rw_probe.h)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -22,9 +23,22 @@ def _newer(target, deps):
     return all(os.path.getmtime(d) <= t for d in deps)
 
 
+def build_probe(force=False):
+    src = os.path.join(CSRC, "rw_probe.cu")
+    hdr = os.path.join(HERE, "..", "include", "rw_probe.h")
+    if not force and _newer(PROBE_LIB, [src, hdr]):
+        return PROBE_LIB
+    p = subprocess.run(["nvcc"] + [f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")] + ["-shared", src, "-o", PROBE_LIB],
+                       capture_output=True, text=True)
+    if p.returncode != 0:
+        raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, p.stdout, p.stderr))
+    return PROBE_LIB
+
+
 def build(force=False, verbose=False):
     hdrs = [os.path.join(CSRC, "rw_internal.h"), os.path.join(HERE, "..", "include", "rw.h")]
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
+    build_probe(force)
     if not force and _newer(LIB, srcs + hdrs):
         return LIB
     objdir = os.path.join(HERE, "build")

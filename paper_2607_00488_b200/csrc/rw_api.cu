@@ -117,12 +117,18 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         L->mu_tile_items = (int)items;
         L->mu_tile = take((size_t)items * kBM * kBN * 8);
     }
-    {   // rw_eval_profile scratch: mu of one pass, about 256 MB (at least 128 points, at most max_batch)
+    {   // rw_eval_profile scratch: mu of one pass, about 256 MB (at least 128 points, at most max_batch); rw_eval_pee
+        // keeps the weights w[pee_rows][n_T] of a pass in the same scratch, so it also holds min(max_batch, those
+        // rows) rows of n_T doubles (a context made for single evaluations, max_batch = 1, can still call it)
         int64_t rows = ((int64_t)256 << 20) / (int64_t)(D * n_rec * 8);
         if (rows < 128) rows = 128;
         if (rows > max_batch) rows = max_batch;
         L->prof_rows = rows;
-        L->mu_prof = take((size_t)rows * D * n_rec * 8);
+        size_t doubles = (size_t)rows * D * n_rec;
+        if (doubles < (size_t)rows * n_T) doubles = (size_t)rows * n_T;
+        int64_t pr = (int64_t)(doubles / n_T);
+        L->pee_rows = pr < max_batch ? pr : max_batch;
+        L->mu_prof = take(doubles * 8);
     }
     L->R32 = take(L->fp32 ? D * 2 * n_rec * (size_t)L->KP32 * 4 : 0);
     L->B8 = take(L->sliced ? D * (size_t)L->NT8 * L->KT8 * 16384 : 0);
@@ -401,10 +407,11 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         cudaError_t e__ = (call);                                                               \
         if (e__ != cudaSuccess) {                                                               \
             fail(nullptr, RW_ERR_CUDA, "rw_create: %s failed: %s", #call, cudaGetErrorString(e__)); \
-            free(ctx->tmapR); free(ctx);                                                        \
+            free(comp_host); free(ctx->tmapR); free(ctx);                                       \
             return RW_ERR_CUDA;                                                                 \
         }                                                                                       \
     } while (0)
+    uint8_t *comp_host = nullptr;                              // host staging of comp_of_T, freed after the sync
     RW_TRY(cudaMemcpyAsync(ctx->E, in->E_MeV, n_E * 8, kind, s));
     RW_TRY(cudaMemcpyAsync(ctx->fw, in->flux_w, n_comp * n_E * 8, kind, s));
     for (size_t q = 0; q < n_comp; ++q) {                      // [n_comp][n_E] tables -> P3[n_comp][3][n_E]
@@ -414,7 +421,6 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
             RW_TRY(cudaMemcpyAsync(ctx->P3 + q * 3 * n_E + 2 * n_E, in->P_tau + q * n_E, n_E * 8, kind, s));
         }
     }
-    uint8_t *comp_host = nullptr;                              // host staging of comp_of_T, freed after the sync
     if (n_comp == 1) RW_TRY(cudaMemsetAsync(ctx->comp8, 0, n_T, s));
     if (n_comp > 1) {
         RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
@@ -481,14 +487,21 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
     if (mem_kind == RW_MEM_HOST && host_bad_nonneg(counts, n))
         return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts must be finite and >= 0");
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (mem_kind == RW_MEM_DEVICE) {
+        // validate the caller's array BEFORE the context changes: a rejected call leaves counts and the saturated
+        // constant as they were
+        int flag = 0;
+        RW_CUDA(ctx, cudaMemsetAsync(ctx->flag, 0, 4, s));
+        RW_CUDA(ctx, launch_validate_counts(ctx, counts, s));
+        RW_CUDA(ctx, cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
+        RW_CUDA(ctx, cudaStreamSynchronize(s));
+        if (flag) return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts must be finite and >= 0");
+    }
     RW_CUDA(ctx, cudaMemsetAsync(ctx->flag, 0, 4, s));
     RW_CUDA(ctx, cudaMemcpyAsync(ctx->counts, counts, n * 8,
                                  mem_kind == RW_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
     RW_CUDA(ctx, launch_sat_const(ctx, s));
-    int flag = 0;
-    RW_CUDA(ctx, cudaMemcpyAsync(&flag, ctx->flag, 4, cudaMemcpyDeviceToHost, s));
     RW_CUDA(ctx, cudaStreamSynchronize(s));
-    if (flag) return fail(ctx, RW_ERR_INVALID, "rw_set_counts: counts must be finite and >= 0");
     return RW_OK;
 }
 
@@ -698,11 +711,8 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
         if (kinds[a] >= RW_RATE_0) return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: rate kinds are not accepted");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
-    // passes sized by the mu scratch, which holds the weights w[Pq][n_T] here
-    int64_t per_pass = (int64_t)((size_t)L.prof_rows * ctx->D * ctx->n_rec / (size_t)ctx->n_T);
-    if (per_pass > L.max_batch) per_pass = L.max_batch;
-    if (per_pass < 1)
-        return fail(ctx, RW_ERR_WORKSPACE, "rw_eval_pee: the scratch cannot hold one row of weights (n_T = %d)", ctx->n_T);
+    // passes sized by the mu scratch, which holds the weights w[Pq][n_T] here (plan(): at least one row)
+    const int64_t per_pass = L.pee_rows;
     for (int64_t q0 = 0; q0 < P; q0 += per_pass) {
         const int64_t Pq = (P - q0 < per_pass) ? P - q0 : per_pass;
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));

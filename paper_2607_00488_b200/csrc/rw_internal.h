@@ -72,6 +72,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int KT8, NT8;         // k-blocks of 32 recoil bins; 64-column units = 2 x (128-column tiles) (rw_fold_i8.cu)
     bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
+    int64_t pee_rows;     // points per pass of rw_eval_pee (rows of n_T weights the same scratch holds)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
     int ldG;              // row pitch of the prefolded templates G[D][12][ldG] (n_rec rounded up to even)
     int64_t max_batch;
@@ -142,6 +143,7 @@ int fail(rw_ctx *ctx, int status, const char *fmt, ...);
 // kernels' host launchers (each returns a cudaError_t from the launch) ---------------------------
 cudaError_t launch_setup(rw_ctx *ctx, cudaStream_t s);                       // rw_setup.cu
 cudaError_t launch_sat_const(rw_ctx *ctx, cudaStream_t s);                   // rw_setup.cu
+cudaError_t launch_validate_counts(rw_ctx *ctx, const double *counts_dev, cudaStream_t s);   // rw_setup.cu
 cudaError_t launch_comp8(rw_ctx *ctx, const int32_t *comp_dev, cudaStream_t s);   // rw_setup.cu
 cudaError_t launch_validate_device(rw_ctx *ctx, const double *R_src, int ld_src,
                                    size_t period_stride_src, cudaStream_t s); // rw_setup.cu

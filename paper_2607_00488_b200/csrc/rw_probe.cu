@@ -1,8 +1,11 @@
-// rw_probe.cu -- measurement helper, not part of the method: register-resident FP64 issue-rate
-// probes that give the denominators of the FP64 roofline.
+// rw_probe.cu -- measurement helper of bench.py (include/rw_probe.h), built as librw_probe.so and not linked
+// into librw.so: register-resident FP64 issue-rate probes that give the denominators of the FP64 roofline
+// (DESIGN.md section 6).
 //   kind 0: DFMA chains (16 independent accumulators per thread)
 //   kind 1: DMMA m8n8k4 (8 independent accumulator tiles per warp)
-#include "rw_internal.h"
+#include <cuda_runtime.h>
+
+#include "../../include/rw_probe.h"
 
 namespace rw {
 
@@ -40,20 +43,29 @@ __global__ void __launch_bounds__(256) k_probe_dmma(double *out, int iters, doub
 
 }  // namespace rw
 
-extern "C" int rw_probe_fp64_peak(int32_t kind, int32_t iters, double *tflops, void *cuda_stream)
+static int probe_grid()
 {
-    if (!tflops || iters <= 0 || (kind != 0 && kind != 1)) return RW_ERR_INVALID;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-        return RW_ERR_CUDA;
-    const int grid = sms * 2;
-    double *buf = nullptr;
-    if (cudaMallocAsync(&buf, (size_t)grid * 256 * sizeof(double), s) != cudaSuccess) return RW_ERR_CUDA;
+        return 0;
+    return sms * 2;
+}
+
+extern "C" size_t rw_probe_scratch_bytes(void) { return (size_t)probe_grid() * 256 * sizeof(double); }
+
+extern "C" int rw_probe_fp64_peak(int32_t kind, int32_t iters, void *scratch_dev, size_t scratch_bytes, double *tflops,
+                                  void *cuda_stream)
+{
+    const int grid = probe_grid();
+    if (grid == 0) return -3;
+    if (!tflops || !scratch_dev || iters <= 0 || (kind != 0 && kind != 1) ||
+        scratch_bytes < (size_t)grid * 256 * sizeof(double))
+        return -1;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    double *buf = (double *)scratch_dev;
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -3;
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0, s);
@@ -67,11 +79,9 @@ extern "C" int rw_probe_fp64_peak(int32_t kind, int32_t iters, double *tflops, v
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFreeAsync(buf, s);
-    cudaStreamSynchronize(s);
-    if (cudaGetLastError() != cudaSuccess) return RW_ERR_CUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess || cudaGetLastError() != cudaSuccess) return -3;
     const double flop = (kind == 0) ? 2.0 * 16 * (double)iters * 256.0 * grid
                                     : 512.0 * 8 * (double)iters * 8.0 * grid;
     *tflops = flop / (best * 1e-3) / 1e12;
-    return RW_OK;
+    return 0;
 }

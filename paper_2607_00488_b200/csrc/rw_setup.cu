@@ -228,6 +228,15 @@ cudaError_t launch_comp8(rw_ctx *ctx, const int32_t *comp_dev, cudaStream_t s)
     return cudaGetLastError();
 }
 
+// Sets F_CNT in ctx->flag when a device array of D * n_rec counts holds a negative or non-finite value.
+cudaError_t launch_validate_counts(rw_ctx *ctx, const double *counts_dev, cudaStream_t s)
+{
+    int64_t nB = (int64_t)ctx->D * ctx->n_rec;
+    k_validate_counts<<<(unsigned)((nB + 255) / 256), 256, 0, s>>>(nB, counts_dev, ctx->flag);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_sat_const(rw_ctx *ctx, cudaStream_t s)
 {
     int64_t nB = (int64_t)ctx->D * ctx->n_rec;

@@ -266,3 +266,25 @@ def test_every_regime_is_bit_reproducible_run_to_run(rw):
     twice(lambda: ctx.eval_profile(p[:200], kinds, s0=1.0, sigma=0.1))
     twice(lambda: ctx.eval_grad(p[:100], kinds))
     ctx.close()
+
+
+def test_rejected_device_counts_leave_the_context_unchanged(rw, orc):
+    """rw_set_counts validates a device array before it touches the context: after RW_ERR_INVALID the old counts
+    and the old saturated constant (literal Eq. 18) are still in force."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=48, n_rec=32, n_periods=1, seed=24)
+    params, kinds = wl.random_points(6, [0, 4], seed=25)
+    ctx = rw.Reweighter(inp, max_batch=8)
+    before = ctx.eval_batch(_cuda(params), kinds, full_eq18=True).cpu().numpy()
+    bad = torch.full((1, 32), 3.0, dtype=torch.float64, device="cuda")
+    bad[0, 5] = -1.0
+    with pytest.raises(rw.RwError):
+        ctx.set_counts(bad)
+    bad[0, 5] = float("nan")
+    with pytest.raises(rw.RwError):
+        ctx.set_counts(bad)
+    after = ctx.eval_batch(_cuda(params), kinds, full_eq18=True).cpu().numpy()
+    assert np.array_equal(before, after)
+    ref = orc.eval_batch(inp, params, kinds, full_eq18=True)
+    assert np.all(np.abs(after - ref) <= 1e-9 + 1e-12 * np.abs(ref))
+    ctx.close()

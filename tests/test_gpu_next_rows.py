@@ -366,3 +366,20 @@ def test_per_point_survival_probability_config3_size(rw, orc):
     ref, scale = orc.eval_pee(inp, params[idx], kinds, Pp[idx], want_abs=True, nthreads=CORES)
     assert np.all(np.abs(out.cpu().numpy()[idx] - ref) <= 1e-9 + 1e-12 * scale)
     ctx.close()
+
+
+def test_per_point_survival_probability_with_a_single_evaluation_context(rw, orc):
+    """A context made for single evaluations (max_batch = 1) on a shape with n_T > n_rec: the weights of a pass
+    live in the mu scratch, which must hold at least one row of n_T doubles."""
+    import torch
+    inp = wl.make_custom(n_E=60, n_T=600, n_rec=37, n_periods=1, seed=111)
+    params, kinds = wl.random_points(3, [wl.EPS_EE_L, wl.MU_NU], seed=112)
+    rng = np.random.default_rng(113)
+    Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.2, 0.2, size=(3, 60)), 0.0, 1.0)
+    ref, mu_ref, scale = orc.eval_pee(inp, params, kinds, Pp, want_mu=True, want_abs=True)
+    for mb in (1, 2):
+        ctx = rw.Reweighter(inp, max_batch=mb)
+        out, mu = ctx.eval_pee(_cuda(params), kinds, _cuda(Pp), want_mu=True)      # 3 points => passes of mb
+        torch.cuda.synchronize()
+        _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+        ctx.close()

@@ -15,8 +15,8 @@ from paper_2607_00488_b200 import sharding, workloads as wl
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_functions():
-    text = open(os.path.join(ROOT, "include", "rw.h")).read()
+def _declared_functions(header="rw.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(rw_[a-z0-9_]+)\s*\(", text)))
 
@@ -31,6 +31,14 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, n), "librw.so does not export %s" % n
     from paper_2607_00488_b200 import binding
     assert set(binding.EXPORTS) == set(names)
+    # the bench-only probe library (include/rw_probe.h) is separate: librw.so must not carry it
+    from paper_2607_00488_b200 import probe
+    plib = ctypes.CDLL(build.build_probe())
+    pnames = _declared_functions("rw_probe.h")
+    assert set(probe.EXPORTS) == set(pnames) and pnames
+    for n in pnames:
+        assert hasattr(plib, n), "librw_probe.so does not export %s" % n
+        assert not hasattr(lib, n), "librw.so exports the measurement helper %s" % n
 
 
 def test_binding_constants_match_the_header():
