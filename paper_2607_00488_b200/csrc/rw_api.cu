@@ -68,10 +68,11 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     if (splits < 1) splits = 1;
     L->stream_splits = splits;
     L->ridge_strips = (int)((n_rec + kRidgeCols - 1) / kRidgeCols);
-    size_t ridge_rows_max = 0;           // rows of the parked partial tiles: ranges x tile height, largest variant
-    for (int v = 0; v < 4; ++v) {
-        const int ns = ridge_plan((int)n_T, (int)n_rec, (int)D, v, kPlanSMs, &L->ridge_rows[v]);
-        if ((size_t)ns * (8u << v) > ridge_rows_max) ridge_rows_max = (size_t)ns * (8u << v);
+    L->ridge_max_p = max_batch <= 16 ? 16 : max_batch <= 32 ? 32 : kRidgeMaxP;
+    size_t ridge_slot_bytes = 0;         // 3 parked partial tiles per CTA, largest variant
+    for (int v = 0; (8 << v) <= L->ridge_max_p; ++v) {
+        const size_t b = (size_t)3 * ridge_grid((int)n_T, (int)n_rec, (int)D, v, kRidgePlanSMs, nullptr) * (8u << v) * kRidgeCols * 8;
+        if (b > ridge_slot_bytes) ridge_slot_bytes = b;
     }
     const size_t nstrip2 = (n_rec + 255) / 256;
     const size_t mu_ld = (n_rec + 1) & ~(size_t)1;
@@ -104,10 +105,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
     size_t part_gemm = D * (size_t)(L->sliced ? L->NT8 : L->n_tiles_n) * L->MC, part_stream = D * nstrip2 * kStreamMaxPB;
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
-    {
-        size_t rows_stream = (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB;
-        L->mu_part = take(D * (rows_stream > ridge_rows_max ? rows_stream : ridge_rows_max) * mu_ld * 8);
-    }
+    L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
+    L->ridge_slots = take(ridge_slot_bytes);
     L->ridge_cnt = take((D * (size_t)L->ridge_strips + 1) * 4);
     L->ridge_part = take(D * (size_t)L->ridge_strips * kRidgeMaxP * 8);
     L->out_stage = take((size_t)max_batch * 8);
@@ -177,10 +176,11 @@ static const char *flag_message(int f)
     return "invalid input";
 }
 
-// RW_MODE_AUTO (measured on B200, config-4 size): one point -> the one-launch HBM-streaming kernel; 2..16 points ->
+// RW_MODE_AUTO (measured on B200, config-4 size): one point -> the one-launch HBM-streaming kernel; 2..32 points ->
 // the one-launch streaming DMMA kernel (R read once at HBM speed, contraction on the FP64 tensor cores); beyond -> the
-// tiled DMMA contraction (tile height 32..128, split-K).  The opt-in contractions (prec != 0) replace the last two.
-constexpr int kAutoRidgeMax = 16;
+// tiled DMMA contraction (tile height 64 / 128, split-K: 0.57 ms against 0.61 ms at 64 points).  The opt-in
+// contractions (prec != 0) replace the last two.
+constexpr int kAutoRidgeMax = 32;
 static bool auto_stream(const rw_ctx *, int64_t P, int prec) { return prec == 0 ? P <= 1 : P <= 4; }
 static bool use_stream(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
 {
@@ -217,8 +217,8 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
                                             dout + g0, full, mu, s));
         }
     } else if (use_ridge(ctx, mode, Ps, prec)) {
-        for (int64_t g0 = 0; g0 < Ps; g0 += kRidgeMaxP) {
-            const int Pb = (int)((Ps - g0 < kRidgeMaxP) ? Ps - g0 : kRidgeMaxP);
+        for (int64_t g0 = 0; g0 < Ps; g0 += L.ridge_max_p) {
+            const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
                                            dout + g0, full, mu, s));
@@ -380,6 +380,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->strip_part = (double *)(ws + L.strip_part);
     ctx->ridge_cnt = (int *)(ws + L.ridge_cnt);
     ctx->ridge_part = (double *)(ws + L.ridge_part);
+    ctx->ridge_slots = (double *)(ws + L.ridge_slots);
     ctx->param_stage = (double *)(ws + L.param_stage);
     ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);
     ctx->partial = (double *)(ws + L.partial);
@@ -544,7 +545,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             Kinds kd;
             kd.k = k;
             for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
-            const int group = stream_mode ? kStreamMaxPB : kRidgeMaxP;
+            const int group = stream_mode ? kStreamMaxPB : L.ridge_max_p;
             for (int64_t g0 = 0; g0 < Ps; g0 += group) {
                 const int Pb = (int)((Ps - g0 < group) ? Ps - g0 : group);
                 double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
@@ -651,8 +652,8 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
     } else if (use_ridge(ctx, mode, P, prec)) {
-        for (int64_t g0 = 0; g0 < P; g0 += kRidgeMaxP) {
-            const int Pb = (int)((P - g0 < kRidgeMaxP) ? P - g0 : kRidgeMaxP);
+        for (int64_t g0 = 0; g0 < P; g0 += L.ridge_max_p) {
+            const int Pb = (int)((P - g0 < L.ridge_max_p) ? P - g0 : L.ridge_max_p);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }

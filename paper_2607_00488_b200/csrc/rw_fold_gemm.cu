@@ -111,6 +111,7 @@ __device__ __forceinline__ TileCoord tile_coord(int t, int tiles_m, int tiles_n)
 struct GemmWork {
     int n_T, n_rec, tiles_m, tiles_n, tile0, n_tiles, S, kps, D, d;
     int64_t Pc, part_stride;
+    int zero;                 // 0, opaque to the compiler (release of a pipeline stage, tile heights 16..64)
     const double *bkg, *counts;
     double *partial, *out_mu, *mu_tile;
 };
@@ -192,7 +193,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
     for (int s = 0; s < 2; ++s)
         b_off[s] = Cfg::StageBytesA + (uint32_t)(c + 4 * s) * kRowBytesB + (uint32_t)(32 * wn + 2 * r) * 8;
 
-    int stage = 0;
+    int stage = 0, release = -1;   // `release`: the stage consumed in the previous iteration, not yet handed back
     uint32_t phase = 0;
     uint32_t ready = 0;      // result of the early poll of the next stage's full barrier
     for (int item = blockIdx.x; item < total_items; item += gridDim.x) {
@@ -211,6 +212,7 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
             produce_step();
             if (!ready) mbar_wait(full_bar + 8 * stage, phase);
             const uint32_t st = sbase + stage * Cfg::StageBytes;
+            uint32_t dep = 0;
 #pragma unroll
             for (int kb = 0; kb < kKB; ++kb) {
                 double2 a[MB], b[2][2];
@@ -226,6 +228,12 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                         asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];"
                                      : "=d"(b[sj][s].x), "=d"(b[sj][s].y)
                                      : "r"(st + b_off[s] + (uint32_t)sj * 128 + (uint32_t)kb * (8 * kRowBytesB)));
+                if constexpr (MB < 8) {
+#pragma unroll
+                    for (int mb = 0; mb < MB; ++mb) dep |= (uint32_t)__double2hiint(a[mb].x);
+                    dep |= (uint32_t)__double2hiint(b[0][0].x) | (uint32_t)__double2hiint(b[0][1].x) |
+                           (uint32_t)__double2hiint(b[1][0].x) | (uint32_t)__double2hiint(b[1][1].x);
+                }
                 if (kb == kKB - 1) {
                     // poll the next stage's barrier now: the result is back by the time the last
                     // DMMA block of this stage has issued, so the wait above costs no pipe bubble
@@ -244,8 +252,20 @@ k_fold_gemm(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ C
                         }
                     }
             }
+            // A stage may be handed back only when every fragment load of it has RETURNED: released right behind the
+            // loop, ptxas places the arrive directly after the last LDS issue, and in k_fold_ridge the producer's refill
+            // has been seen to overtake such a load (rw_fold_ridge.cu).  128-row tiles (no register to spare, deep
+            // slack): one iteration late, behind the next stage's barrier wait -- every DMMA reading the stage has been
+            // issued by then, and the TMA issue, Stages - 2 ahead, still finds its slot released an iteration earlier.
+            // Smaller tiles (HBM-bound, every stage in flight counts): at once, the arrive's address depending on the
+            // loaded registers (& 0 the compiler cannot see; lane 0's registers stand for the warp-wide LDS).
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar + 8 * stage);
+            if constexpr (MB == 8) {
+                if (lane == 0 && release >= 0) mbar_arrive(empty_bar + 8 * release);
+                release = stage;
+            } else {
+                if (lane == 0) mbar_arrive(empty_bar + 8 * stage + (dep & (uint32_t)W.zero));
+            }
             if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
 
@@ -465,6 +485,7 @@ cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int
     W.n_T = ctx->n_T; W.n_rec = ctx->n_rec; W.D = ctx->D; W.d = d;
     W.tiles_m = (int)((Pc + BM - 1) / BM);
     W.tiles_n = L.n_tiles_n;
+    W.zero = 0;
     W.Pc = Pc; W.part_stride = L.MC;
     W.bkg = ctx->bkg + (size_t)d * ctx->n_rec;
     W.counts = ctx->counts + (size_t)d * ctx->n_rec;

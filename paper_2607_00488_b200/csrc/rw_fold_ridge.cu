@@ -1,41 +1,45 @@
-// rw_fold_ridge.cu -- the whole path for 5..64 points in ONE kernel: the regime around the ridge of the
+// rw_fold_ridge.cu -- the whole path for 2..64 points in ONE kernel: the regime around the ridge of the
 // roofline (P* = 4 F / BW ~ 23 points on B200), where the fold
 //   mu[p][k] = sum_i N'[p][i] R[i][k] + bkg[k]                                  (Eq. 11)
 // has to read every byte of R exactly once at HBM speed AND do 2 P flop per 8 bytes, more than scalar DFMA
 // can issue next to the loads.  Design:
-//   * decomposition of k_fold_stream: a CTA owns a 256-column strip x a range of recoil rows (grid =
-//     strips x row ranges x periods, one wave of one or two CTAs per SM), so R streams from HBM exactly once;
-//   * a producer warp keeps a ring of 4-6 stages of 8 or 16 rows in flight (up to 200 KB per SM -- registers
-//     cannot hold that much, a first version with the loads going straight into the fragments stayed at 5.4 TB/s):
-//     one plain bulk copy (cp.async.bulk, mbarrier completion) per row, 2 KB long requests, exactly the strip's
-//     bytes; the rows land at a pitch of 2080 bytes (= 32 mod 128), which makes the fragment loads below
-//     conflict free without a swizzle;
-//   * the arithmetic of k_fold_gemm: mma.sync.m8n8k4.f64 (DMMA.8x8x4).  Eight consumer warps own 32 columns
-//     each and all points of the tile; lane (r = lane / 4, c = lane % 4) reads the 16 bytes
-//     R[i + c][col + 2 r .. + 1] -- one B fragment for the even and one for the odd columns of a 16-column group;
-//   * N' of 64 recoil rows x 8 MB points (steps a1 + a2: coefficients from the raw parameters, Eq. 6, PAPER.md:79;
-//     N' = sum_b c_b W^_b, Eq. 14 / Eq. 1) is formed on the fly into shared memory, double
-//     buffered, pitch 68 doubles so that the A-fragment loads are conflict free;
-//   * a4 as in k_fold_stream: the partial tile of a row range is parked; the LAST CTA of a strip (ticket) adds
-//     the ranges in a fixed order, adds bkg and reduces the Poisson terms of Eq. (18); the last
-//     strip adds strips and periods in a fixed order and writes -2lnL.  One launch per call, deterministic.
-#include <type_traits>
-
+//   * stream-K decomposition: the work is the sequence of (period, 256-column strip, block of RS recoil rows)
+//     units, strip-major; CTA j of G takes the units [j U / G, (j + 1) U / G) -- one wave, every SM streams the
+//     same number of bytes whatever the shape.  A span that crosses a strip boundary is cut into segments; a strip
+//     shared by several CTAs is finished by whichever of them arrives last (ticket), adding the parked partial tiles
+//     in CTA order, so the result does not depend on the arrival order;
+//   * a producer warp keeps a ring of 4-6 stages of RS rows in flight (up to 200 KB per SM -- registers cannot
+//     hold that much: a first version with the loads going straight into the fragments stayed at 5.4 TB/s): one plain
+//     bulk copy (cp.async.bulk, mbarrier completion, L2 evict-first) per row, 2 KB requests, exactly the strip's
+//     bytes; the rows land at a pitch of 2064 bytes (= 16 mod 64: the rows 2 c + j a quarter-warp reads fall in four
+//     different 32-byte bank groups), which makes the fragment loads conflict free without a swizzle;
+//   * the arithmetic of k_fold_gemm: mma.sync.m8n8k4.f64 (DMMA.8x8x4).  Eight consumer warps own 32 columns each
+//     and all points of the tile; lane (r = lane / 4, c = lane % 4) reads the 16 bytes R[i + 2 c + j][col + 2 r .. + 1]
+//     -- one B fragment for the even and one for the odd columns of a 16-column group;
+//   * N' of the next 64 recoil rows x 8 MB points (steps a1 + a2: coefficients from the raw parameters, Eq. 6,
+//     PAPER.md:79; N' = sum_b c_b W^_b, Eq. 14 / Eq. 1) is itself a [8 MB x 12] x [12 x 8] DMMA per
+//     8 rows -- consumer warp w forms the 8-row block w of the next chunk (operands prefetched a chunk ahead) -- whose
+//     C fragment (point r, rows 2 c and 2 c + 1) IS the A fragment of the fold's two k-steps when k-step j takes the
+//     rows {2 c + j}: the lanes store and reload their own 16 bytes (double-buffered, lane-linear: no bank conflicts,
+//     no transposition).  3 MB DMMAs per warp and chunk instead of 22 MB DFMAs per thread: with scalar staging the
+//     tensor pipe was 75 % busy at 64 points, and separate scalar stager warps could not keep up at all;
+//   * at 64 points setmaxnreg moves the registers of the producer warpgroup to the consumers (128 accumulators);
+//   * a4: the finishing CTA of a strip adds bkg and reduces the Poisson terms of Eq. (18) of its 256
+//     columns; the last strip adds strips and periods in a fixed order and writes -2lnL.  One launch per call.
 #include "rw_internal.h"
 
 namespace rw {
 
-constexpr int kRgWarps = 8;                           // consumer (DMMA) warps
+constexpr int kRgWarps = 8;                           // consumer (DMMA) warps: two warpgroups
 constexpr int kRgConsumers = kRgWarps * 32;
 constexpr int kRgThreads = kRgConsumers + 32;         // + the producer warp (tile heights 8, 16, 32)
-constexpr int kRgThreads64 = kRgConsumers + 128;      // tile height 64: a producer warpgroup, so that setmaxnreg can
-                                                      // move its registers to the consumers (128 accumulators each)
+constexpr int kRgThreads64 = kRgConsumers + 128;      // tile height 64: a producer warpgroup for setmaxnreg (3 warps idle)
 constexpr int kRgWarpCols = 32;                       // two 16-column groups per warp
-constexpr int kRgCols = kRgWarps * kRgWarpCols;       // 256 columns per CTA strip
-constexpr int kRgKC = 64;                             // recoil rows of N' staged per chunk
-constexpr int kRgPitch = kRgKC + 4;                   // = 4 (mod 16) doubles: the A-fragment rows land in distinct banks
-constexpr int kRgRowBytes = kRgCols * 8 + 32;         // ring pitch 2080 B = 32 (mod 128): rows c = 0..3 -> 4 bank groups
-static_assert(kRgCols == kRidgeCols && kRgKC == kRidgeRowQuantum * 4, "plan() in rw_api.cu assumes this geometry");
+constexpr int kRgCols = kRgWarps * kRgWarpCols;       // 256 columns per strip
+constexpr int kRgKC = 64;                             // recoil rows of N' per chunk: one 8-row block per consumer warp
+constexpr int kRgNB = 2;                              // N' buffers
+constexpr int kRgRowBytes = kRgCols * 8 + 16;         // ring pitch 2064 B = 16 (mod 64): rows 2 c + j -> 4 bank groups
+static_assert(kRgCols == kRidgeCols, "plan() in rw_api.cu assumes this strip width");
 
 struct RidgeArgs {
     const double *R; size_t R_period_stride; int ldR, n_T, n_rec, D;
@@ -45,10 +49,12 @@ struct RidgeArgs {
     const double *rate;       // [Pb][4] rate scales matching `coef`, or NULL
     const uint8_t *comp8;     // [n_T] component of every recoil bin
     const double *What, *N_mc, *bkg, *counts, *sat_const;
-    int Pb, rows_per_split, n_splits, mu_ld;
-    double *mu_part;          // [D][n_splits][8 MB][mu_ld]
-    double *strip_part;       // [D * strips][64]
-    int *cnt;                 // [D * strips] strip tickets, then one global ticket
+    int Pb, n_strips, nblk;   // strips per period; blocks of RS rows per strip
+    int zero_ring;            // ragged strip or row tail: the ring is read where no copy lands
+    int zero;                 // 0, opaque to the compiler (release of a ring stage at 16 points)
+    double *slots;            // [3 G][8 MB][256] parked partial tiles
+    double *strip_part;       // [D * strips][64] Poisson sums per tile
+    int *cnt;                 // [D * strips] tile tickets, then one global ticket
     double *out;              // [Pb]
     double *out_mu;           // NULL or [Pb][D][n_rec]
 };
@@ -90,17 +96,44 @@ __device__ __forceinline__ void rg_bulk_row(uint32_t dst, const void *src, uint3
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
+__device__ __forceinline__ void rg_bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(kRgConsumers) : "memory"); }
 
 template <int MB> struct RidgeCfg {
     static constexpr int PP = 8 * MB;                                  // points of the tile
-    static constexpr int RS = (MB <= 2) ? 8 : 16;                      // recoil rows per ring stage
+    static constexpr int RS = (MB <= 2) ? 8 : 16;                      // recoil rows per ring stage (= per work unit)
     static constexpr int NS = (MB == 1) ? 6 : (MB == 8) ? 4 : 5;       // ring stages
     static constexpr int MinCtas = (MB <= 2) ? 2 : 1;
+    // How a ring stage is handed back safely (see the consumer loop): one iteration late (free, but one stage less in
+    // flight), or at once through a register dependence on its fragment loads (16 points: five 16 KB stages per CTA
+    // are too few to give one away -- 0.199 ms against 0.214 ms on config 4)
+    static constexpr bool LateRelease = (MB != 2);
     static constexpr int Threads = (MB == 8) ? kRgThreads64 : kRgThreads;
+    // tile height 64: setmaxnreg redistributes the registers the CTA was LAUNCHED with (384 x 168): 256 ConsumerRegs +
+    // 128 HelperRegs must not exceed that pool, or the consumers wait for ever
+    static constexpr int ConsumerRegs = 224, HelperRegs = 40;
+    static_assert(kRgConsumers * ConsumerRegs + 128 * HelperRegs <= kRgThreads64 * 168, "setmaxnreg pool");
     static constexpr int StageBytes = RS * kRgRowBytes;
     static constexpr int RingBytes = NS * StageBytes;
-    static constexpr int SmemDoubles = 2 * PP * kRgPitch + PP * kCoefStride + PP * RW_MAX_COMPONENTS + kRgWarps * PP;
-    static constexpr int Smem = RingBytes + SmemDoubles * 8 + 2 * NS * 8;           // + barriers
+    static constexpr int NBytes = kRgNB * (kRgKC / 8) * MB * 512;      // N' fragments: [buffer][8-row block][mb][lane] x 16 B
+    static constexpr int SmemDoubles = PP * kCoefStride + PP * RW_MAX_COMPONENTS + kRgWarps * PP;
+    static constexpr int Smem = RingBytes + NBytes + SmemDoubles * 8 + 2 * NS * 8;
+};
+
+// Work split shared by the three roles.  Units u = tile * nblk + block; CTA j owns [u0(j), u0(j + 1)).
+struct RidgeSplit {
+    long long U;
+    int G, nblk;
+    __device__ __forceinline__ long long u0(int j) const { return (long long)j * U / G; }
+    __device__ __forceinline__ int cta_of(long long u) const { return (int)(((u + 1) * G - 1) / U); }
+    // slot of CTA j's partial tile of `tile`: 3 j + {0: the tile its span starts in, 2: the tile it ends in, 1: a
+    // whole tile in between (private, reused)}
+    __device__ __forceinline__ int slot_of(int j, int tile) const
+    {
+        const long long a = u0(j), b = u0(j + 1) - 1;
+        if (tile == (int)(a / nblk)) return 3 * j;
+        if (tile == (int)(b / nblk)) return 3 * j + 2;
+        return 3 * j + 1;
+    }
 };
 
 template <int MB>
@@ -108,31 +141,25 @@ __global__ void __launch_bounds__(RidgeCfg<MB>::Threads, RidgeCfg<MB>::MinCtas)
 k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
 {
     using Cfg = RidgeCfg<MB>;
-    constexpr int PP = Cfg::PP, RS = Cfg::RS, NS = Cfg::NS, kThreads = Cfg::Threads;
+    constexpr int PP = Cfg::PP, RS = Cfg::RS, NS = Cfg::NS;
     // 128-byte aligned so that the bank analysis of the ring pitch holds; indexed directly (a re-aligned pointer
     // would lose its address space and turn the fragment loads into generic LD)
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t ring = rg_smem_u32(smem);
-    double *sN = reinterpret_cast<double *>(smem + Cfg::RingBytes);     // [2][PP][kRgPitch]
-    double *sC = sN + 2 * PP * kRgPitch;                               // [PP][12]
+    const uint32_t sN = ring + Cfg::RingBytes;                         // [2 buffers][8 blocks][MB][32 lanes] double2
+    double *sC = reinterpret_cast<double *>(smem + Cfg::RingBytes + Cfg::NBytes);   // [PP][12]
     double *sRate = sC + PP * kCoefStride;                             // [PP][4]
     double *red = sRate + PP * RW_MAX_COMPONENTS;                      // [8 warps][PP]
-    const uint32_t full_bar = rg_smem_u32(red + kRgWarps * PP);
+    const uint32_t full_bar = rg_smem_u32(red + kRgWarps * PP);        // ring: NS full, NS empty
     const uint32_t empty_bar = full_bar + NS * 8;
-    __shared__ int s_last;
+    __shared__ int s_flag;
 
-    const int d = blockIdx.z, split = blockIdx.y, strip = blockIdx.x;
     const int n_T = A.n_T, n_rec = A.n_rec, Pb = A.Pb;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int r = lane >> 2, c = lane & 3;
-    const int i0 = split * A.rows_per_split;
-    const int i1 = min(n_T, i0 + A.rows_per_split);
-    const int nrows = i1 - i0;
-    const int n_iters = (nrows + RS - 1) / RS;                         // ring stage-iterations of this CTA
-    const double *Rd = A.R + (size_t)d * A.R_period_stride;
-    const double *Wd = A.What + (size_t)d * kCoefStride * n_T;
-    const double *wts = A.wts;
-    const int cols_avail = min(kRgCols, A.ldR - strip * kRgCols);      // even; the pad column of a copied R is zero
+    const int n_tiles = A.D * A.n_strips;
+    RidgeSplit sp;
+    sp.nblk = A.nblk; sp.U = (long long)n_tiles * A.nblk; sp.G = gridDim.x;
+    const long long ua = sp.u0(blockIdx.x), ub = sp.u0(blockIdx.x + 1);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NS; ++s) {
@@ -141,15 +168,49 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    // ragged strip or row range: the ring is also read where no copy ever lands (times N' = 0), so it must hold
-    // finite numbers there
-    if (cols_avail < kRgCols || (nrows % RS) != 0) {
-        for (int q = threadIdx.x; q < Cfg::RingBytes / 16; q += kThreads)
+    if (A.zero_ring) {               // the ring is also read where no copy ever lands (times N' = 0): finite numbers
+        for (int q = threadIdx.x; q < Cfg::RingBytes / 16; q += Cfg::Threads)
             reinterpret_cast<double2 *>(smem)[q] = make_double2(0.0, 0.0);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
+    __syncthreads();
 
+    if (warp >= kRgWarps) {
+        if constexpr (MB == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(Cfg::HelperRegs));
+        if (warp == kRgWarps) {
+            // ------------------------------------------------------------ producer: lane l copies row l of a stage
+            uint64_t policy;
+            asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+            int stage = 0;
+            uint32_t phase = 0;
+            for (long long u = ua; u < ub;) {
+                const int tile = (int)(u / sp.nblk), b0 = (int)(u - (long long)tile * sp.nblk);
+                const int nb = (int)min((long long)(sp.nblk - b0), ub - u);
+                const int d = tile / A.n_strips, strip = tile - d * A.n_strips;
+                const int row0 = b0 * RS, nrows = min(n_T, (b0 + nb) * RS) - row0;
+                const uint32_t row_bytes = (uint32_t)min(kRgCols, A.ldR - strip * kRgCols) * 8;   // even; a copied R is zero-padded
+                const double *src = A.R + (size_t)d * A.R_period_stride + (size_t)(row0 + lane) * A.ldR + (size_t)strip * kRgCols;
+                for (int q = 0; q < nb; ++q) {
+                    rg_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
+                    const int rows = min(RS, nrows - q * RS);
+                    const uint32_t fb = full_bar + 8 * stage;
+                    if (lane == 0) rg_mbar_expect_tx(fb, (uint32_t)rows * row_bytes);
+                    __syncwarp();
+                    if (lane < rows)
+                        rg_bulk_row(ring + stage * Cfg::StageBytes + lane * kRgRowBytes, src + (size_t)q * RS * A.ldR,
+                                    row_bytes, fb, policy);
+                    if (++stage == NS) { stage = 0; phase ^= 1; }
+                }
+                u += nb;
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------- consumers
+    if constexpr (MB == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::ConsumerRegs));
     // ---------------------------------------------------------------- a1: coefficients of the tile's points
+    const double *wts = A.wts;
     if (!wts) {
         if (A.param) {
             if (threadIdx.x < PP) {
@@ -168,68 +229,64 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
                 for (int q = 0; q < RW_MAX_COMPONENTS; ++q) sRate[threadIdx.x * RW_MAX_COMPONENTS + q] = rr[q];
             }
         } else {
-            for (int q = threadIdx.x; q < PP * kCoefStride; q += kThreads) {
-                const int p = q / kCoefStride;
-                sC[q] = (p < Pb) ? A.coef[q] : 0.0;
-            }
-            for (int q = threadIdx.x; q < PP * RW_MAX_COMPONENTS; q += kThreads) {
-                const int p = q / RW_MAX_COMPONENTS;
-                sRate[q] = (p < Pb && A.rate) ? A.rate[q] : 1.0;
-            }
+            for (int q = threadIdx.x; q < PP * kCoefStride; q += kRgConsumers) sC[q] = (q / kCoefStride < Pb) ? A.coef[q] : 0.0;
+            for (int q = threadIdx.x; q < PP * RW_MAX_COMPONENTS; q += kRgConsumers)
+                sRate[q] = (q / RW_MAX_COMPONENTS < Pb && A.rate) ? A.rate[q] : 1.0;
         }
     }
-    __syncthreads();                                                // barriers, zeroed ring, sC, sRate
+    rg_bar_consumers();                              // (the producer is already streaming R)
+    const int r = lane >> 2, c = lane & 3;
+    // B fragments: rows 2 c + j of an 8-row block, columns 32 warp + 16 g + 2 r + {0, 1}
+    const uint32_t b_off = (uint32_t)(2 * c) * kRgRowBytes + (uint32_t)(kRgWarpCols * warp + 2 * r) * 8;
+    int stage = 0, release = -1;      // `release`: the stage consumed in the previous iteration, not yet handed back
+    uint32_t phase = 0;
+    for (long long u = ua; u < ub;) {
+        const int tile = (int)(u / sp.nblk), b0 = (int)(u - (long long)tile * sp.nblk);
+        const int nb = (int)min((long long)(sp.nblk - b0), ub - u);
+        const int d = tile / A.n_strips, strip = tile - d * A.n_strips;
+        const int row0 = b0 * RS, row1 = min(n_T, (b0 + nb) * RS), nrows = row1 - row0;
+        u += nb;
 
-    if (warp >= kRgWarps) {
-        // ------------------------------------------------------------ producer warp: lane l copies row l of a stage
-        if constexpr (MB == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == kRgWarps) {                                      // (the other warps of that group idle)
-            uint64_t policy;
-            asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-            const uint32_t row_bytes = (uint32_t)cols_avail * 8;
-            const double *src = Rd + (size_t)(i0 + lane) * A.ldR + (size_t)strip * kRgCols;
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int q = 0; q < n_iters; ++q) {
-                rg_mbar_wait(empty_bar + 8 * stage, phase ^ 1);
-                const int rows = min(RS, nrows - q * RS);
-                const uint32_t fb = full_bar + 8 * stage;
-                if (lane == 0) rg_mbar_expect_tx(fb, (uint32_t)rows * row_bytes);
-                __syncwarp();
-                if (lane < rows)
-                    rg_bulk_row(ring + stage * Cfg::StageBytes + lane * kRgRowBytes, src + (size_t)q * RS * A.ldR, row_bytes, fb,
-                                policy);
-                if (++stage == NS) { stage = 0; phase ^= 1; }
-            }
-        }
-    } else {
-        if constexpr (MB == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
-        // ------------------------------------------------------------ a2: N' of a 64-row chunk -> sN[buf][p][row]
-        // thread = (row, quarter of the points): the 11 basis values of its row are loaded once for all its points
-        auto stage_n = [&](int ic, int buf) {
-            const int row = threadIdx.x & (kRgKC - 1), pq = threadIdx.x >> 6;
-            const int i = ic + row;
-            const bool ok = i < i1;
-            double *dst = sN + (size_t)buf * PP * kRgPitch + row;
-            if (wts) {
-                const double nm = ok ? A.N_mc[(size_t)d * n_T + i] : 0.0;
+        // ------------------------------------------------------------ a2: this warp's 8-row block of a 64-row chunk
+        // Lane (r, c): the B fragment of the staging product is W^[4 ks + c][i + r], the A fragment c[8 mb + r][4 ks + c],
+        // and the C fragment N'[8 mb + r][i + 2 c], N'[8 mb + r][i + 2 c + 1] is what the same lane of every warp loads
+        // back as the A fragment of the fold.  fetch() runs a chunk ahead of form().
+        const double *Wd = A.What + (size_t)d * kCoefStride * n_T;
+        double bw[3];
+        int cq0 = 0, cq1 = 0;
+        auto fetch = [&](int ic) {
+            const int i0 = ic + 8 * warp, ia = i0 + 2 * c;
 #pragma unroll
-                for (int j = 0; j < PP / 4; ++j) {
-                    const int p = pq + 4 * j;
-                    dst[p * kRgPitch] = (ok && p < Pb) ? wts[(size_t)p * n_T + i] * nm : 0.0;
+            for (int ks = 0; ks < 3; ++ks) {
+                const int b = 4 * ks + c;
+                bw[ks] = (!wts && b < kNumTerms && i0 + r < row1) ? __ldg(Wd + (size_t)b * n_T + i0 + r) : 0.0;
+            }
+            cq0 = (ia < row1) ? A.comp8[ia] : 0;
+            cq1 = (ia + 1 < row1) ? A.comp8[ia + 1] : 0;
+        };
+        auto form = [&](int ic, int buf) {
+            const int ia = ic + 8 * warp + 2 * c;
+            const uint32_t dst = sN + (uint32_t)((buf * (kRgKC / 8) + warp) * MB) * 512 + lane * 16;
+            if (wts) {
+                const double n0 = (ia < row1) ? A.N_mc[(size_t)d * n_T + ia] : 0.0;
+                const double n1 = (ia + 1 < row1) ? A.N_mc[(size_t)d * n_T + ia + 1] : 0.0;
+#pragma unroll
+                for (int mb = 0; mb < MB; ++mb) {
+                    const int p = 8 * mb + r;
+                    const double v0 = (p < Pb && ia < row1) ? wts[(size_t)p * n_T + ia] * n0 : 0.0;
+                    const double v1 = (p < Pb && ia + 1 < row1) ? wts[(size_t)p * n_T + ia + 1] * n1 : 0.0;
+                    asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(dst + mb * 512), "d"(v0), "d"(v1) : "memory");
                 }
             } else {
-                double w[kNumTerms];
 #pragma unroll
-                for (int b = 0; b < kNumTerms; ++b) w[b] = ok ? __ldg(Wd + (size_t)b * n_T + i) : 0.0;
-                const int cq = ok ? A.comp8[i] : 0;
+                for (int mb = 0; mb < MB; ++mb) {
+                    const int p = 8 * mb + r;
+                    double v0 = 0.0, v1 = 0.0;
 #pragma unroll
-                for (int j = 0; j < PP / 4; ++j) {
-                    const int p = pq + 4 * j;
-                    double v = 0.0;
-#pragma unroll
-                    for (int b = 0; b < kNumTerms; ++b) v = fma(sC[p * kCoefStride + b], w[b], v);
-                    dst[p * kRgPitch] = v * sRate[p * RW_MAX_COMPONENTS + cq];     // rate_k of Eq. (17); 1 when not scanned
+                    for (int ks = 0; ks < 3; ++ks) rg_dmma(v0, v1, sC[p * kCoefStride + 4 * ks + c], bw[ks]);
+                    v0 *= sRate[p * RW_MAX_COMPONENTS + cq0];     // rate_k of Eq. (17); 1 when not scanned
+                    v1 *= sRate[p * RW_MAX_COMPONENTS + cq1];
+                    asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(dst + mb * 512), "d"(v0), "d"(v1) : "memory");
                 }
             }
         };
@@ -241,132 +298,169 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
 #pragma unroll
             for (int g = 0; g < 2; ++g)
 #pragma unroll
-                for (int nb = 0; nb < 2; ++nb) acc[mb][g][nb][0] = acc[mb][g][nb][1] = 0.0;
-        // B fragments: row 4 ks + c of the stage, columns 32 warp + 16 g + 2 r + {0, 1}
-        const uint32_t b_off = (uint32_t)c * kRgRowBytes + (uint32_t)(kRgWarpCols * warp + 2 * r) * 8;
-        if (nrows > 0) stage_n(i0, 0);
-        int stage = 0, buf = 0, q = 0;
-        uint32_t phase = 0;
-        for (int ch = 0; ch * kRgKC < nrows; ++ch, buf ^= 1) {
-            asm volatile("bar.sync 1, %0;" ::"n"(kRgConsumers) : "memory");   // sN[buf] staged; sN[buf ^ 1] no longer read
-            const double *sA = sN + (size_t)buf * PP * kRgPitch + r * kRgPitch + c;
+                for (int e = 0; e < 2; ++e) acc[mb][g][e][0] = acc[mb][g][e][1] = 0.0;
+        fetch(row0);
+        form(row0, 0);
+        int q = 0, nbuf = 0;
+        for (int ic = row0; ic < row1; ic += kRgKC, nbuf ^= 1) {
+            rg_bar_consumers();                      // N'[nbuf] formed by all warps; N'[nbuf ^ 1] no longer read
+            const bool more = ic + kRgKC < row1;
+            if (more) fetch(ic + kRgKC);
+            const uint32_t sA = sN + (uint32_t)(nbuf * (kRgKC / 8) * MB) * 512 + lane * 16;
 #pragma unroll
             for (int sq = 0; sq < kRgKC / RS; ++sq) {
-                if (q < n_iters) {
+                if (q < nb) {
                     rg_mbar_wait(full_bar + 8 * stage, phase);
                     const uint32_t st = ring + stage * Cfg::StageBytes + b_off;
+                    uint32_t dep = 0;
 #pragma unroll
-                    for (int ks = 0; ks < RS / 4; ++ks) {
-                        double a[MB];
-                        double2 b[2];
-#pragma unroll
-                        for (int g = 0; g < 2; ++g)
-                            asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(b[g].x), "=d"(b[g].y)
-                                         : "r"(st + (uint32_t)ks * (4 * kRgRowBytes) + (uint32_t)g * 128));
-#pragma unroll
-                        for (int mb = 0; mb < MB; ++mb) a[mb] = sA[mb * 8 * kRgPitch + sq * RS + 4 * ks];
+                    for (int hb = 0; hb < RS / 8; ++hb) {              // 8-row blocks of this stage
+                        double2 a[MB];
 #pragma unroll
                         for (int mb = 0; mb < MB; ++mb)
+                            asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(a[mb].x), "=d"(a[mb].y)
+                                         : "r"(sA + (uint32_t)((sq * (RS / 8) + hb) * MB + mb) * 512));
 #pragma unroll
-                            for (int g = 0; g < 2; ++g) {
-                                rg_dmma(acc[mb][g][0][0], acc[mb][g][0][1], a[mb], b[g].x);
-                                rg_dmma(acc[mb][g][1][0], acc[mb][g][1][1], a[mb], b[g].y);
+                        for (int j = 0; j < 2; ++j) {                  // k-step j: rows 2 c + j of the block
+                            double2 b[2];
+#pragma unroll
+                            for (int g = 0; g < 2; ++g)
+                                asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(b[g].x), "=d"(b[g].y)
+                                             : "r"(st + (uint32_t)(8 * hb + j) * kRgRowBytes + (uint32_t)g * 128));
+                            if constexpr (!Cfg::LateRelease)
+                                dep |= (uint32_t)__double2hiint(b[0].x) | (uint32_t)__double2hiint(b[1].x);
+#pragma unroll
+                            for (int mb = 0; mb < MB; ++mb) {
+                                const double av = j ? a[mb].y : a[mb].x;
+#pragma unroll
+                                for (int g = 0; g < 2; ++g) {
+                                    rg_dmma(acc[mb][g][0][0], acc[mb][g][0][1], av, b[g].x);
+                                    rg_dmma(acc[mb][g][1][0], acc[mb][g][1][1], av, b[g].y);
+                                }
                             }
+                        }
                     }
+                    // A stage may be handed back only when every fragment load of it has RETURNED.  Released right behind
+                    // the loop, ptxas issues the arrive directly after the last LDS, and the producer's next copy into the
+                    // stage has been seen to overtake that load (two CTAs per SM, 16 points: 32-byte pieces of a later row
+                    // in one fragment, -2lnL off by 1e-8 .. 1e-3 relative in every other run).  Either the arrive comes one
+                    // iteration late, behind the next stage's barrier wait (every DMMA reading the stage has been issued
+                    // by then), or its address depends on the loaded registers (& 0 the compiler cannot see; a warp-wide
+                    // LDS completes as one instruction, so lane 0's registers stand for the warp).
                     __syncwarp();
-                    if (lane == 0) rg_mbar_arrive(empty_bar + 8 * stage);
+                    if constexpr (Cfg::LateRelease) {
+                        if (lane == 0 && release >= 0) rg_mbar_arrive(empty_bar + 8 * release);
+                        release = stage;
+                    } else {
+                        if (lane == 0) rg_mbar_arrive(empty_bar + 8 * stage + (dep & (uint32_t)A.zero));
+                    }
                     if (++stage == NS) { stage = 0; phase ^= 1; }
                     ++q;
                 }
             }
-            if ((ch + 1) * kRgKC < nrows) stage_n(i0 + (ch + 1) * kRgKC, buf ^ 1);
+            if (more) form(ic + kRgKC, nbuf ^ 1);
         }
 
-        // ------------------------------------------------------------ park the partial tile of this row range
-        // column 4 c + 2 e + nb of a 16-column group holds acc[.][.][nb][e]
-        const int colw = strip * kRgCols + warp * kRgWarpCols;
+        // ------------------------------------------------------------ park the partial tile of this segment
+        // column 4 c + 2 e + nb of a 16-column group holds acc[.][.][nb][e]; tile-local layout [8 MB][256]
+        {
+            double *slot = A.slots + (size_t)sp.slot_of(blockIdx.x, tile) * (PP * kRgCols);
 #pragma unroll
-        for (int mb = 0; mb < MB; ++mb)
+            for (int mb = 0; mb < MB; ++mb)
 #pragma unroll
-            for (int g = 0; g < 2; ++g) {
-                const int col = colw + 16 * g + 4 * c;
-                double *dst = A.mu_part + (((size_t)d * A.n_splits + split) * PP + 8 * mb + r) * A.mu_ld + col;
-                if (col < n_rec)
+                for (int g = 0; g < 2; ++g) {
+                    double *dst = slot + (8 * mb + r) * kRgCols + warp * kRgWarpCols + 16 * g + 4 * c;
                     __stcg(reinterpret_cast<double2 *>(dst), make_double2(acc[mb][g][0][0], acc[mb][g][1][0]));
-                if (col + 2 < n_rec)
                     __stcg(reinterpret_cast<double2 *>(dst + 2), make_double2(acc[mb][g][0][1], acc[mb][g][1][1]));
-            }
-    }
+                }
+        }
+        // ------------------------------------------------------------ who finishes this tile?
+        const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
+        __threadfence();
+        rg_bar_consumers();
+        if (jl > jf) {
+            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + tile, 1);
+            rg_bar_consumers();
+            const bool last = (s_flag == jl - jf);
+            rg_bar_consumers();                                        // s_flag is rewritten below / next segment
+            if (!last) continue;
+            __threadfence();
+            if (threadIdx.x == 0) A.cnt[tile] = 0;                     // every contributor has arrived: ready for the next launch
+        }
 
-    // ---------------------------------------------------------------- last CTA of this strip: a4 for 256 columns
-    const int n_splits = A.n_splits, mu_ld = A.mu_ld;
-    const int n_strips = gridDim.x, sid = d * n_strips + strip;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(A.cnt + sid, 1) == n_splits - 1);
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    if (warp < kRgWarps) {
-        const int col = strip * kRgCols + threadIdx.x;
-        const bool col_ok = col < n_rec;
-        double bk = 0.0, cn = 0.0;
-        if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
+        // ------------------------------------------------------------ a4 for the 256 columns of this tile
+        {
+            const int col = strip * kRgCols + threadIdx.x;
+            const bool col_ok = col < n_rec;
+            double bk = 0.0, cn = 0.0;
+            if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
 #pragma unroll 1
-        for (int pb = 0; pb < MB; ++pb) {
-            double m[8];
+            for (int pb = 0; pb < MB; ++pb) {
+                double m[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) m[q] = 0.0;
-            if (col_ok) {
-                const double *src = A.mu_part + ((size_t)d * n_splits * PP + 8 * pb) * mu_ld + col;
-                for (int s = 0; s < n_splits; ++s) {      // row ranges in a fixed order; the 8 loads of a step overlap
+                for (int e = 0; e < 8; ++e) m[e] = 0.0;
+                // contributors in CTA order (the sum is the same whoever finishes); four of them = 32 loads in flight
+                for (int j0 = jf; j0 <= jl; j0 += 4) {
+                    double v[4][8];
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) m[q] += __ldcg(src + ((size_t)s * PP + q) * mu_ld);
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const int j = min(j0 + jj, jl);
+                        const double *src = A.slots + (size_t)sp.slot_of(j, tile) * (PP * kRgCols) + (8 * pb) * kRgCols + threadIdx.x;
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) v[jj][e] = __ldcg(src + e * kRgCols);
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj)
+                        if (j0 + jj <= jl) {
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) m[e] += v[jj][e];
+                        }
+                }
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int p = 8 * pb + e;
+                    double t = 0.0;
+                    if (col_ok && p < Pb) {
+                        const double a = m[e] + bk;
+                        if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
+                        t = poisson_term(a, cn);
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                    if (lane == 0) red[warp * PP + p] = t;
                 }
             }
+            rg_bar_consumers();
+            if (threadIdx.x < PP) {
+                double v = 0.0;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const int p = 8 * pb + q;
-                double t = 0.0;
-                if (col_ok && p < Pb) {
-                    const double a = m[q] + bk;
-                    if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
-                    t = poisson_term(a, cn);
+                for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
+                __stcg(A.strip_part + (size_t)tile * kRidgeMaxP + threadIdx.x, v);
+            }
+            // -------------------------------------------------------- last tile: sum strips and periods, write
+            __threadfence();
+            rg_bar_consumers();
+            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + n_tiles, 1);
+            rg_bar_consumers();
+            const bool all_done = (s_flag == n_tiles - 1);
+            rg_bar_consumers();
+            if (all_done) {
+                __threadfence();
+                if (threadIdx.x < Pb) {
+                    double v = 0.0;
+                    for (int t = 0; t < n_tiles; ++t) v += __ldcg(A.strip_part + (size_t)t * kRidgeMaxP + threadIdx.x);
+                    v *= 2.0;
+                    if (A.sat_const) v += A.sat_const[0];
+                    A.out[threadIdx.x] = v;
                 }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                if (lane == 0) red[warp * PP + p] = t;
+                if (threadIdx.x == 0) A.cnt[n_tiles] = 0;                  // ready for the next launch
             }
         }
     }
-    __syncthreads();
-    if (threadIdx.x < PP) {
-        double v = 0.0;
-#pragma unroll
-        for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
-        __stcg(A.strip_part + (size_t)sid * kRidgeMaxP + threadIdx.x, v);
-    }
-
-    // ---------------------------------------------------------------- last strip: sum strips and periods, write
-    const int n_sid = n_strips * A.D;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(A.cnt + n_sid, 1) == n_sid - 1);
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    if (threadIdx.x < Pb) {
-        double v = 0.0;
-        for (int q = 0; q < n_sid; ++q) v += __ldcg(A.strip_part + (size_t)q * kRidgeMaxP + threadIdx.x);
-        v *= 2.0;
-        if (A.sat_const) v += A.sat_const[0];
-        A.out[threadIdx.x] = v;
-    }
-    for (int q = threadIdx.x; q <= n_sid; q += kThreads) A.cnt[q] = 0;       // ready for the next launch
 }
 
 template <int MB>
-static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Consts &cst, dim3 grid, cudaStream_t s)
+static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Consts &cst, int grid, cudaStream_t s)
 {
     static bool attr_set = false;          // per instantiation; the attribute is per device function
     if (!attr_set) {
@@ -379,23 +473,25 @@ static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Con
     return cudaSuccess;
 }
 
-int ridge_plan(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *rows_per_split)
+// Grid of k_fold_ridge for tile height 8 << mb_log2: one wave of the SM slots, but at least ~256 recoil rows of one
+// strip per CTA (a smaller share is not worth a partial tile).  Host arithmetic only; also sizes the slot scratch.
+int ridge_grid(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *nblk_out)
 {
+    const int RS = (mb_log2 <= 1) ? 8 : 16;
     const int strips = (n_rec + kRgCols - 1) / kRgCols;
-    const int slots = num_sms * ((mb_log2 <= 1) ? 2 : 1);           // resident CTAs (RidgeCfg::MinCtas)
-    const int max_splits = n_T / kRgKC > 1 ? n_T / kRgKC : 1;       // at least one 64-row chunk per CTA
-    int best = 1;
-    double best_eff = 0.0;
-    for (int S = 1; S <= max_splits; ++S) {
-        const int64_t ctas = (int64_t)strips * D * S;
-        if (ctas > 2 * (int64_t)slots && S > 1) break;              // at most two waves: partial tiles cost traffic
-        const double eff = (double)ctas / (double)((ctas + slots - 1) / slots * slots);
-        if (eff > best_eff + 0.01) { best_eff = eff; best = S; }
-    }
-    int rows = (n_T + best - 1) / best;
-    rows = (rows + kRidgeRowQuantum - 1) / kRidgeRowQuantum * kRidgeRowQuantum;
-    *rows_per_split = rows;
-    return (n_T + rows - 1) / rows;
+    const int nblk = (n_T + RS - 1) / RS;
+    const long long U = (long long)strips * D * nblk;
+    const int slots = num_sms * ((mb_log2 <= 1) ? 2 : 1);
+    long long G = U / (256 / RS);
+    if (G > slots) G = slots;
+    // a whole number of CTAs per strip when that still fills >= 95 % of the slots: the strips then advance through the
+    // recoil rows in step, so that the 2 KB row segments in flight belong to few, complete 8 n_rec-byte rows of R
+    // (measured on config 4, 4 / 16 points: 0.181 / 0.186 ms with 288 CTAs, 0.187 / 0.197 ms with 296)
+    const long long n_tiles = (long long)strips * D;
+    if (G == slots && n_tiles <= slots && (slots / n_tiles) * n_tiles * 20 >= (long long)slots * 19) G = (slots / n_tiles) * n_tiles;
+    if (G < 1) G = 1;
+    if (nblk_out) *nblk_out = nblk;
+    return (int)G;
 }
 
 cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
@@ -407,6 +503,8 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     if (coef && coef >= ctx->coef && coef < ctx->coef + (size_t)ctx->lay.max_batch * kCoefStride)
         rate = ctx->rate + (coef - ctx->coef) / kCoefStride * RW_MAX_COMPONENTS;
     const Layout &L = ctx->lay;
+    if (Pb > L.ridge_max_p) return cudaErrorInvalidValue;               // the slot scratch is sized by max_batch (plan())
+    const int mbl = Pb <= 8 ? 0 : Pb <= 16 ? 1 : Pb <= 32 ? 2 : 3;     // tile height 8 << mbl
     RidgeArgs A;
     A.R = ctx->R; A.R_period_stride = ctx->R_period_stride; A.ldR = ctx->ldR;
     A.n_T = ctx->n_T; A.n_rec = ctx->n_rec; A.D = ctx->D;
@@ -415,17 +513,17 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     A.What = ctx->What; A.N_mc = ctx->N_mc; A.bkg = ctx->bkg; A.counts = ctx->counts;
     A.sat_const = full_eq18 ? ctx->sat_const : nullptr;
     A.Pb = Pb;
-    const int mbl = Pb <= 8 ? 0 : Pb <= 16 ? 1 : Pb <= 32 ? 2 : 3;     // tile height 8 << mbl
-    A.rows_per_split = L.ridge_rows[mbl];
-    A.n_splits = (ctx->n_T + A.rows_per_split - 1) / A.rows_per_split;
-    A.mu_ld = (ctx->n_rec + 1) & ~1;
-    A.mu_part = ctx->mu_part; A.strip_part = ctx->ridge_part; A.cnt = ctx->ridge_cnt;
+    A.n_strips = L.ridge_strips;
+    const int grid = ridge_grid(ctx->n_T, ctx->n_rec, ctx->D, mbl, kRidgePlanSMs, &A.nblk);
+    const int RS = (mbl <= 1) ? 8 : 16;
+    A.zero_ring = (ctx->ldR - (L.ridge_strips - 1) * kRgCols < kRgCols) || (ctx->n_T % RS != 0);
+    A.zero = 0;
+    A.slots = ctx->ridge_slots; A.strip_part = ctx->ridge_part; A.cnt = ctx->ridge_cnt;
     A.out = out; A.out_mu = out_mu;
     Kinds none;
     none.k = 0;
     for (int a = 0; a < RW_N_KINDS; ++a) none.kind[a] = -1;
     const Kinds &k = kd ? *kd : none;
-    dim3 grid(L.ridge_strips, A.n_splits, ctx->D);
     cudaError_t e;
     {
         ProfScope prof(ctx, s);

@@ -35,9 +35,9 @@ constexpr int kStreamCols = 2 * kStreamThreads;   // columns per CTA strip (one 
 constexpr int kStreamMaxPB = 16;                  // points folded per pass over R
 
 // ---- streaming DMMA fold geometry (rw_fold_ridge.cu) -------------------------------------------
-constexpr int kRidgeCols = 256;                   // columns per CTA strip (8 warps x 32)
-constexpr int kRidgeRowQuantum = 16;              // a row range is a multiple of 16 recoil rows
+constexpr int kRidgeCols = 256;                   // columns per strip (8 warps x 32)
 constexpr int kRidgeMaxP = 64;                    // points per launch (tile heights 8, 16, 32, 64)
+constexpr int kRidgePlanSMs = 148;                // B200: the stream-K grid is one wave of these SMs' slots
 
 struct Consts {
     double sin2w, m_e, G_F, alpha;
@@ -64,8 +64,8 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int stream_strips;    // ceil(n_rec / kStreamCols)
     int stream_splits;    // row splits of the streaming fold
     int ridge_strips;     // ceil(n_rec / kRidgeCols)
-    int ridge_rows[4];    // recoil rows per CTA of k_fold_ridge for tile heights 8, 16, 32, 64 (ridge_plan)
-    size_t ridge_cnt, ridge_part;
+    int ridge_max_p;      // largest tile height of k_fold_ridge the slot scratch was sized for (16, 32 or 64)
+    size_t ridge_cnt, ridge_part, ridge_slots;
     int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
     bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
     int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 2048, else 7 (rw_api.cu plan())
@@ -100,6 +100,7 @@ struct rw_ctx {
     int *stream_cnt;          // last-CTA-done tickets of the streaming fold: [D * strips] + 1, self-resetting
     int *ridge_cnt;           // the same for k_fold_ridge: [D * ridge_strips] + 1
     double *ridge_part;       // [D * ridge_strips][64] Poisson sums per column strip of k_fold_ridge
+    double *ridge_slots;      // [3 G][tile height][256] parked partial tiles of k_fold_ridge
     double *strip_part;       // [D * strips][16] Poisson sums per column strip
     double *G, *ident;        // prefolded templates [D][12][ldG]; identity coefficients [16][12] used to fold them
     int *flag;
@@ -162,9 +163,8 @@ cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *pa
 cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
                               const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
                               cudaStream_t s);                               // rw_fold_ridge.cu
-// Row ranges of k_fold_ridge for tile height 8 << mb_log2: rows per CTA (multiple of 16) such that strips x ranges x D
-// CTAs fill one or two waves of the SM slots; returns the number of ranges.  Host arithmetic only.
-int ridge_plan(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *rows_per_split);   // rw_fold_ridge.cu
+// Grid (CTAs) of k_fold_ridge for tile height 8 << mb_log2 and the number of row blocks per strip.  Host arithmetic only.
+int ridge_grid(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *nblk_out);         // rw_fold_ridge.cu
 cudaError_t launch_gen_A_weights(rw_ctx *ctx, int d, const double *w, int64_t Pc, cudaStream_t s);  // rw_coef.cu
 cudaError_t launch_prefold(rw_ctx *ctx, cudaStream_t s);                     // rw_collapsed.cu
 cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, double s0, double sigma,

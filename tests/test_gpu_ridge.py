@@ -164,3 +164,30 @@ def test_cuda_graph_capture_of_a_ridge_call(rw, orc):
         torch.cuda.synchronize()
         assert np.all(np.abs(out.cpu().numpy() - ref) <= m2lnl_tol(scale))
     ctx.close()
+
+
+@pytest.mark.parametrize("P", [4, 16, 32, 64])
+def test_run_to_run_identical_when_streaming_from_hbm(rw, orc, P):
+    """Regression test for a pipeline race found in round 2: a ring stage was handed back to the producer while a fragment
+    load of it was still in flight (ptxas issues the mbarrier arrive right behind the last LDS), and with two CTAs per
+    SM the refill overtook that load -- -2lnL off by 1e-8 .. 1e-3 relative in every other run at 9..16 points on a
+    response much larger than the L2.  400 MB response (8 periods), 25 repetitions must agree bit for bit with each
+    other and with the tiled contraction to rounding; sampled points against the oracle."""
+    import torch
+    rng = np.random.default_rng(77)
+    inp = wl.make_custom(n_E=24, n_T=3072, n_rec=2048, n_periods=8, seed=91)
+    params, kinds = wl.random_points(P, [0, 1, 4, 6], seed=92 + P)
+    ctx = rw.Reweighter(inp, max_batch=64)
+    p = _cuda(params)
+    ref = ctx.eval_batch(p, kinds, mode="gemm").cpu().numpy()
+    first = None
+    for rep in range(25):
+        out = ctx.eval_batch(p, kinds, mode="ridge").cpu().numpy()
+        if first is None:
+            first = out
+        assert np.array_equal(out, first), "repetition %d differs from the first" % rep
+    assert np.all(np.abs(first - ref) <= 1e-12 * np.abs(ref))
+    idx = np.array([0, P - 1])
+    o_ref, o_abs = orc.eval_batch(inp, params[idx], kinds, want_abs=True, nthreads=8)
+    assert np.all(np.abs(first[idx] - o_ref) <= m2lnl_tol(o_abs))
+    ctx.close()
