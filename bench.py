@@ -611,6 +611,9 @@ def main():
                 _, mu64 = ctx.eval_batch(param_dev[:ns].contiguous(), kinds, want_mu=True, mode="gemm")
                 rel = ((mu32 - mu64).abs() / mu64.abs())
                 fp32_leg = {"ms_per_call": t_f, "evals_per_s": P / t_f * 1e3,
+                            "what": "RW_FP32 = RW_SLICED_FAST | RW_SLICED_STRICT at 1e-5 (one stream synchronisation per chunk; "
+                                    "the TF32 x 3 kernel of round 1 is gone: slower and less accurate than this)",
+                            "strict_fallback_points": ctx.strict_fallback_count(),
                             "effective_fold_tflops": fold_flops(inp, P) / t_f / 1e9,
                             "mu_rel_err_vs_fp64_max": float(rel.max().item()), "mu_rel_err_vs_fp64_mean": float(rel.mean().item())}
         except Exception as exc:               # noqa: BLE001
@@ -636,6 +639,20 @@ def main():
                 fast_leg = {"ms_per_call": t_f, "evals_per_s": P / t_f * 1e3,
                             "effective_fold_tflops": fold_flops(inp, P) / t_f / 1e9,
                             "mu_rel_err_vs_fp64_max": float(relf.max().item()), "int8_products_per_k_step": 10}
+                # certificate: rigorous per-point bound on max_k |mu~ - mu| / mu, and the strict call that enforces the bar
+                _, bnd = ctx.eval_certified(param_dev, kinds, sliced=True)
+                _, bnd_f = ctx.eval_certified(param_dev, kinds, sliced="fast")
+                fb0 = ctx.strict_fallback_count()
+                out_st = torch.empty(P, dtype=torch.float64, device=dev)
+                t_st = timed(lambda: ctx.eval_batch(param_dev, kinds, out=out_st, sliced="strict"), 3)
+                fb_calls = 5                                                # timed(): 2 warm-up + 3 timed calls
+                cert = {"bound_max": float(bnd.max().item()), "bound_median": float(bnd.median().item()),
+                        "points_over_1e-12": int((bnd > 1e-12).sum().item()), "points": P,
+                        "fast_bound_max": float(bnd_f.max().item()), "fast_points_over_1e-5": int((bnd_f > 1e-5).sum().item()),
+                        "strict_ms_per_call": t_st, "strict_evals_per_s": P / t_st * 1e3,
+                        "strict_fallback_points_per_call": (ctx.strict_fallback_count() - fb0) / fb_calls,
+                        "strict_max_abs_diff_m2lnL_vs_dmma": float((out_st - out_dev).abs().max().item()),
+                        "note": "rw_eval_certified; strict = RW_SLICED | RW_SLICED_STRICT: points over the bar are recomputed by the DMMA path"}
                 n_sl = 8 if n_T <= 2048 else 7                              # balanced 8-bit slices per operand (rw_fold_i8.cu)
                 n_prod = n_sl * (n_sl + 1) // 2
                 sliced_leg = {"ms_per_call": t_s, "evals_per_s": P / t_s * 1e3, "bound": "tensor (int8)",
@@ -644,7 +661,7 @@ def main():
                               "executed_int8_tops": n_prod * fold_flops(inp, P) / t_s / 1e9,
                               "mu_rel_diff_vs_dmma_max": float(rel.max().item()),
                               "max_abs_diff_m2lnL_vs_dmma": float((out_s - out_dev).abs().max().item()),
-                              "slices": n_sl, "int8_products_per_k_step": n_prod, "fast": fast_leg,
+                              "slices": n_sl, "int8_products_per_k_step": n_prod, "fast": fast_leg, "certificate": cert,
                               "note": "%d balanced 8-bit slices per operand, %d tcgen05.mma.kind::i8 products per k-step with exact "
                                       "int32 accumulation in TMEM; FP64 DMMA peak is %.1f TFLOP/s" % (n_sl, n_prod, dmma_peak)}
         except Exception as exc:               # noqa: BLE001

@@ -21,9 +21,9 @@
  *   - the library never allocates device memory: the caller passes one workspace
  *     (rw_workspace_bytes) which the context owns until rw_destroy.
  *   - rw_eval_batch is asynchronous and stream-ordered: it only enqueues work on
- *     `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and never synchronises,
- *     except when RW_PARAM_HOST / RW_OUT_HOST ask for pageable/pinned host buffers, in
- *     which case the copies are enqueued on the same stream (pinned memory => still async).
+ *     `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and never synchronises
+ *     (RW_PARAM_HOST / RW_OUT_HOST copies are enqueued on the same stream: pinned memory => still
+ *     async).  The one exception is the opt-in RW_SLICED_STRICT / RW_FP32, see the flag.
  *   - one context must not be used from two streams at once; several contexts may coexist.
  */
 #ifndef RW_H_
@@ -78,28 +78,40 @@ enum {
     RW_MODE_MASK   = 7u << 4,
     RW_PARAM_HOST  = 1u << 8,  /* `param` is a host pointer (copied H2D on the stream) */
     RW_OUT_HOST    = 1u << 9,  /* `out_m2lnL` (and `out_mu`) are host pointers (copied D2H on the stream) */
-    RW_FP32        = 1u << 10, /* opt-in reduced precision for the batched contraction (rw_eval_batch, > 4 points, dense
-                                  fold): operands split in two TF32 pieces, three tcgen05 tensor-core products, FP32
-                                  accumulation in 128-bin chunks; mu within 1e-5 relative of the FP64 path (values below
-                                  the FP32 range flush to 0).  Needs a context created with RW_CREATE_FP32. */
+    RW_FP32        = 1u << 10, /* opt-in reduced precision for the batched contraction (rw_eval_batch / rw_eval_profile, dense
+                                  fold of more than 4 points): mu within 1e-5 relative of the FP64 path, GUARANTEED -- it is
+                                  RW_SLICED_FAST | RW_SLICED_STRICT: the top four 8-bit slices of both operands on the INT8
+                                  tensor cores, and any point whose certified error exceeds 1e-5 is recomputed in FP64.
+                                  Needs a context created with RW_CREATE_FP32 or RW_CREATE_SLICED.  (Round 1 had a separate
+                                  TF32 x 3 kernel here; the fast sliced contraction is 1.7x faster and more accurate.) */
     RW_SLICED      = 1u << 11, /* opt-in FP64-by-slicing for the batched contraction: rows of N' and columns of R in fixed point
                                   (8 balanced base-256 digits for n_T <= 2048, else 7: 63 / 55 bits below their own maximum),
-                                  36 / 28 INT8 tensor-core products per 32 recoil bins with exact int32 accumulation.  Error bound 2^-53 (row max)(column max) n_T per bin instead of a relative
-                                  one: ~1e-13 of mu for responses spread over many recoil bins.
-                                  Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point).  Accepted by
-                                  rw_eval_batch, rw_eval_profile, rw_eval_weights and rw_eval_pee (dense fold only; the
-                                  streaming and collapsed regimes ignore it); rw_eval_grad refuses it. */
-    RW_SLICED_FAST = 1u << 12  /* opt-in reduced precision on the same slices: only their top four (31-bit fixed point) and
+                                  36 / 28 INT8 tensor-core products per 32 recoil bins with exact int32 accumulation.  The error
+                                  is bounded in terms of (row max)(column max), not of mu: ~1e-13 of mu for responses spread
+                                  over many recoil bins; the certified per-point bound is what
+                                  rw_eval_certified returns, and RW_SLICED_STRICT enforces 1e-12.
+                                  Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point, or the FP64 result
+                                  under RW_SLICED_STRICT).  Accepted by rw_eval_batch, rw_eval_certified, rw_eval_profile,
+                                  rw_eval_weights and rw_eval_pee (dense fold only; the streaming, ridge and collapsed regimes
+                                  ignore it); rw_eval_grad refuses it. */
+    RW_SLICED_FAST = 1u << 12, /* opt-in reduced precision on the same slices: only their top four (31-bit fixed point) and
                                   the four leading diagonals, 10 INT8 products per 32 recoil bins.  Error
                                   ~1e-9 (row max)(column max) n_T per bin: mu within 1e-5 relative wherever RW_SLICED
                                   holds 1e-12 (the FP32 bar of this library).  Same requirements and scope as RW_SLICED,
                                   which it excludes. */
+    RW_SLICED_STRICT = 1u << 13 /* with RW_SLICED / RW_SLICED_FAST: never silently less accurate than promised.  Every point
+                                  carries a rigorous bound on max_k |mu~ - mu| / mu from the fixed-point scales (rw_fold_i8.cu);
+                                  a point whose bound exceeds 1e-12 (RW_SLICED) or 1e-5 (RW_SLICED_FAST) is recomputed by the
+                                  FP64 DMMA path, so every result meets the bar of its mode whatever the response looks like.
+                                  The library reads the number of such points back: ONE stream synchronisation per chunk of
+                                  <= 32768 points (the only calls that synchronise; they cannot be captured in a CUDA graph). */
 };
 
 /* rw_inputs.create_flags */
 enum {
-    RW_CREATE_FP32 = 1u << 0,  /* also keep a transposed TF32 hi/lo copy of R (same bytes as R) for RW_FP32 */
-    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into 8 (7 for n_T > 8192) INT8 slices (at most the bytes of R) for RW_SLICED */
+    RW_CREATE_FP32 = 1u << 0,  /* same as RW_CREATE_SLICED (RW_FP32 runs on the INT8 slices) */
+    RW_CREATE_SLICED = 1u << 1 /* also keep R cut into 8 (n_T <= 2048) or 7 INT8 slices (at most the bytes of R) and the
+                                  per-column certificate constants, for RW_SLICED / RW_SLICED_FAST / RW_FP32 */
 };
 
 /* Physical constants.  The paper prints symbols only; any field that is 0
@@ -166,6 +178,18 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
 int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                   double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
 
+/* rw_eval_certified: rw_eval_batch for the sliced contractions (flags must hold RW_SLICED, RW_SLICED_FAST or RW_FP32;
+ * DEVICE pointers only, no out_mu) that also returns, per point, the certified bound
+ *     out_bound[p] >= max over bins and periods of |mu~ - mu| / mu
+ * of what the INT8 contraction computed (0 for points that went through an FP64 path: <= 4 points, the 5..32-point
+ * kernel, or recomputed under RW_SLICED_STRICT; +inf where a bin's bound reaches its mu or the row could not be sliced).
+ * The bound is rigorous for the arithmetic of rw_fold_i8.cu and pessimistic by 10-100x on smooth inputs. */
+int rw_eval_certified(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                      double *out_m2lnL, double *out_bound, uint32_t flags, void *cuda_stream);
+
+/* Points recomputed in FP64 by strict sliced calls of this context so far (instrumentation, like rw_launch_count). */
+int64_t rw_strict_fallback_count(const rw_ctx *ctx);
+
 /* RW_MODE_COLLAPSED (rw_eval_batch only).  Eq. (4) is quadratic in the couplings, Eq. (8)
  * linear in mu_nu^2 and the fold of Eq. (11) linear in the spectrum, so
  *   mu[p][d][k] - bkg[d][k] = sum_b c_b(theta_p) G[d][b][k],   G[d][b][k] = sum_i W^[d][b][i] R[d][i][k]
@@ -179,7 +203,8 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
  * parameters, flux shapes: PAPER.md:220).
  *   w          [P][n_T] row-major DEVICE pointer, finite and >= 0 (not validated; garbage in, garbage out)
  *   out_m2lnL  [P] device pointer;  out_mu NULL or [P][D][n_rec] device pointer
- *   flags      RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM, RW_SLICED / RW_SLICED_FAST (dense fold of more than 4 points)
+ *   flags      RW_FULL_EQ18, RW_MODE_AUTO/STREAM/RIDGE/GEMM, RW_SLICED / RW_SLICED_FAST (+ RW_SLICED_STRICT: a chunk
+ *              with an uncertified point is recomputed as a whole in FP64)
  *              (COLLAPSED, RW_FP32, RW_PARAM_HOST, RW_OUT_HOST: RW_ERR_UNSUPPORTED)
  * Asynchronous and stream-ordered like rw_eval_batch; P may be 0 and may exceed max_batch. */
 int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, double *out_mu,
@@ -194,7 +219,7 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
  *   param, param_kind, P, k   as rw_eval_batch (DEVICE param; kinds RW_EPS_* and RW_MU_NU only)
  *   P_e_pts                   [P][n_E] device pointer, values in [0,1] (not validated)
  *   out_m2lnL [P], out_mu NULL or [P][D][n_rec]   device pointers
- *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/GEMM, RW_SLICED / RW_SLICED_FAST
+ *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/RIDGE/GEMM, RW_SLICED / RW_SLICED_FAST (+ RW_SLICED_STRICT)
  * Needs a single-component context created without explicit P_mu / P_tau.  Asynchronous and stream-ordered. */
 int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                 const double *P_e_pts, double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
@@ -209,8 +234,8 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
  *   param, param_kind, P, k   as rw_eval_batch (DEVICE param only)
  *   s0, sigma                 centre and width of the Gaussian pull on s; sigma <= 0 or +inf-like: no pull
  *   out_m2lnL [P], out_scale [P] or NULL   device pointers
- *   flags                     RW_FULL_EQ18; RW_MODE_AUTO/STREAM/GEMM (dense fold) or RW_MODE_COLLAPSED; RW_FP32,
- *                             RW_SLICED, RW_SLICED_FAST select the contraction of the dense fold as in rw_eval_batch
+ *   flags                     RW_FULL_EQ18; RW_MODE_AUTO/STREAM/RIDGE/GEMM (dense fold) or RW_MODE_COLLAPSED; RW_FP32,
+ *                             RW_SLICED, RW_SLICED_FAST (+ RW_SLICED_STRICT) select the contraction as in rw_eval_batch
  * Asynchronous and stream-ordered; P may exceed max_batch. */
 int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                     double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,

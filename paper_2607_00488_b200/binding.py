@@ -21,13 +21,13 @@ RW_RATE_0 = 7        # RW_RATE_0 + c: rate scale of signal component c
 RW_MEM_HOST, RW_MEM_DEVICE = 0, 1
 RW_FULL_EQ18 = 1 << 0
 RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED, RW_MODE_RIDGE = 0, 1 << 4, 2 << 4, 3 << 4, 4 << 4
-RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED, RW_SLICED_FAST = 1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12
+RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED, RW_SLICED_FAST, RW_SLICED_STRICT = 1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12, 1 << 13
 RW_CREATE_FP32, RW_CREATE_SLICED = 1, 2
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED,
           "ridge": RW_MODE_RIDGE}
 
-EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_eval_pee", "rw_get_table",
+EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_certified", "rw_strict_fallback_count", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_eval_pee", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
            "rw_last_error")
 
@@ -49,9 +49,12 @@ class rw_inputs(C.Structure):
 
 
 def _sliced_flag(sliced):
-    """sliced = False | True (FP64-grade, RW_SLICED) | "fast" (top four slices, FP32-grade, RW_SLICED_FAST)."""
-    if sliced == "fast":
-        return RW_SLICED_FAST
+    """sliced = False | True (FP64-grade, RW_SLICED) | "fast" (top four slices, FP32-grade, RW_SLICED_FAST) |
+    "strict" / "fast-strict" (the same with RW_SLICED_STRICT: uncertified points are recomputed in FP64)."""
+    if sliced in ("fast", "fast-strict"):
+        return RW_SLICED_FAST | (RW_SLICED_STRICT if sliced == "fast-strict" else 0)
+    if sliced == "strict":
+        return RW_SLICED | RW_SLICED_STRICT
     return RW_SLICED if sliced else 0
 
 
@@ -79,6 +82,11 @@ def load_library():
     L.rw_set_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.rw_eval_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32),
                                 C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_certified.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32),
+                                    C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    L.rw_eval_certified.restype = C.c_int
+    L.rw_strict_fallback_count.argtypes = [C.c_void_p]
+    L.rw_strict_fallback_count.restype = C.c_int64
     L.rw_eval_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     L.rw_eval_weights.restype = C.c_int
     L.rw_eval_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.c_double,
@@ -242,6 +250,29 @@ class Reweighter:
         self._check(rc, self._ctx)
         self._last_param = param          # keep alive until the stream has consumed it
         return (out, out_mu) if (want_mu or out_mu is not None) else out
+
+    def eval_certified(self, param, kinds, sliced=True, full_eq18=False, mode="auto", fp32=False):
+        """(-2lnL[P], bound[P]) through a sliced contraction (rw_eval_certified): bound[p] is the certified
+        max over bins of |mu~ - mu| / mu (0 where an FP64 path ran).  CUDA param[P][k] only."""
+        if not (isinstance(param, torch.Tensor) and param.is_cuda):
+            raise RwError(-4, "eval_certified needs a CUDA tensor param[P][k]")
+        param = param.to(torch.float64).contiguous()
+        if param.ndim == 1:
+            param = param[:, None]
+        P, k = param.shape
+        assert k == len(kinds)
+        kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
+        out = torch.empty(P, dtype=torch.float64, device=self.device)
+        bound = torch.empty(P, dtype=torch.float64, device=self.device)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | (RW_FP32 if fp32 else _sliced_flag(sliced))
+        rc = self._L.rw_eval_certified(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr,
+                                       C.c_void_p(out.data_ptr()), C.c_void_p(bound.data_ptr()), flags, _stream_ptr())
+        self._check(rc, self._ctx)
+        self._last_param = param
+        return out, bound
+
+    def strict_fallback_count(self):
+        return int(self._L.rw_strict_fallback_count(self._ctx))
 
     def eval_profile(self, param, kinds, s0=1.0, sigma=0.0, full_eq18=False, mode="auto", sliced=False):
         """(-2lnL[P] with the overall signal normalisation profiled out, s_hat[P]) for CUDA param[P][k]

@@ -46,9 +46,7 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->ldR = L->copy_R ? (int)((n_rec + 1) & ~(size_t)1) : (int)n_rec;
     L->KPAD = (int)((n_T + 31) / 32 * 32);      // k-stages of 16 (DMMA) and 32 (INT8 slices) both divide it
     L->A_pitch = (int64_t)L->KPAD * 8;
-    L->KP32 = (int)((n_T + 3) / 4 * 4);
-    L->fp32 = (in->create_flags & RW_CREATE_FP32) != 0;
-    L->sliced = (in->create_flags & RW_CREATE_SLICED) != 0;
+    L->sliced = (in->create_flags & (RW_CREATE_SLICED | RW_CREATE_FP32)) != 0;     // RW_FP32 runs on the same slices
     L->KT8 = (int)((n_T + 31) / 32);
     // 8 slices (63 bits) are exact in int32 up to n_T = 8192; they are used where the contraction is too short for
     // the tensor pipe to matter.  Beyond, 7 slices (55 bits, 28 instead of 36 products): measured 5e-15 .. 1.2e-13 of mu
@@ -129,7 +127,6 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
         L->pee_rows = pr < max_batch ? pr : max_batch;
         L->mu_prof = take(doubles * 8);
     }
-    L->R32 = take(L->fp32 ? D * 2 * n_rec * (size_t)L->KP32 * 4 : 0);
     L->B8 = take(L->sliced ? D * (size_t)L->NT8 * L->KT8 * 16384 : 0);
     L->f_col8 = take(L->sliced ? D * n_rec * 4 : 0);
     L->e_row8 = take(L->sliced ? (size_t)L->MC * 4 : 0);
@@ -139,6 +136,13 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->KP512 = (int)((n_T + 511) / 512 * 512);
     L->tau8b = take(L->sliced ? D * (size_t)L->KP512 : 0);
     L->comp8p = take(L->sliced ? (size_t)L->KP512 : 0);
+    L->gcol8 = take(L->sliced ? D * 2 * n_rec * 8 : 0);
+    L->cert_part = take(L->sliced ? D * (size_t)L->NT8 * L->MC * 8 : 0);
+    L->bound_stage = take(L->sliced ? (size_t)max_batch * 8 : 0);
+    L->fb_idx = take(L->sliced ? ((size_t)L->MC + 1) * 4 : 0);
+    L->coef_fb = take(L->sliced ? (size_t)L->MC * kCoefStride * 8 : 0);
+    L->rate_fb = take(L->sliced ? (size_t)L->MC * RW_MAX_COMPONENTS * 8 : 0);
+    L->out_fb = take(L->sliced ? (size_t)L->MC * 8 : 0);
     L->total = off;
     return RW_OK;
 }
@@ -191,16 +195,24 @@ static bool use_ridge(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
     return mode == RW_MODE_RIDGE || (mode == RW_MODE_AUTO && prec == 0 && !auto_stream(ctx, P, prec) && P <= kAutoRidgeMax);
 }
 
+// Options of the sliced contraction (prec 2 / 3): tol > 0 = strict (RW_SLICED_STRICT, RW_FP32): a point whose certified
+// relative error exceeds tol is recomputed by the FP64 DMMA path; bound = device array [Ps] that receives the certified
+// bound of every point (0 for points that went through an FP64 path), or NULL.
+struct SlicedOpt { double tol = 0.0; double *bound = nullptr; };
+
 // Steps a2-a4 for the Ps <= max_batch points whose coefficients are in ctx->coef: -2lnL -> dout[Ps], and mu ->
 // out_mu[Ps][D][n_rec] when asked.
-// prec: 0 = FP64 DMMA, 1 = TF32 x 3 (RW_FP32), 2 = INT8 slices (RW_SLICED), 3 = their top four (RW_SLICED_FAST);
-// only the contraction regime differs
+// prec: 0 = FP64 DMMA, 2 = INT8 slices (RW_SLICED), 3 = their top four (RW_SLICED_FAST, RW_FP32); only the contraction
+// regime differs
 static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double *dout, double *out_mu, cudaStream_t s,
-                      int prec = 0)
+                      int prec = 0, const SlicedOpt &opt = SlicedOpt())
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
     const bool stream_mode = use_stream(ctx, mode, Ps, prec);
+    const bool contraction = mode != RW_MODE_COLLAPSED && !stream_mode && !use_ridge(ctx, mode, Ps, prec);
+    if (opt.bound && !(contraction && prec >= 2))                  // every other regime is an FP64 path
+        RW_CUDA(ctx, cudaMemsetAsync(opt.bound, 0, (size_t)Ps * 8, s));
     if (mode == RW_MODE_COLLAPSED) {
         const int nstrip = (n_rec + 511) / 512;
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
@@ -216,7 +228,7 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             RW_CUDA(ctx, launch_fold_stream(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
                                             dout + g0, full, mu, s));
         }
-    } else if (use_ridge(ctx, mode, Ps, prec)) {
+    } else if (!contraction) {
         for (int64_t g0 = 0; g0 < Ps; g0 += L.ridge_max_p) {
             const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
@@ -224,38 +236,70 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
                                            dout + g0, full, mu, s));
         }
     } else {
+        const bool certify = prec >= 2 && (opt.tol > 0.0 || opt.bound);
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {
             const int64_t Pc = (Ps - c0 < L.MC) ? Ps - c0 : L.MC;
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
-                if (prec == 1) {
-                    RW_CUDA(ctx, launch_fold_tf32(ctx, d, c0, Pc, mu, s));
-                } else if (prec >= 2) {
-                    RW_CUDA(ctx, launch_fold_i8(ctx, d, c0, Pc, mu, s, nullptr, prec == 3));
+                if (prec >= 2) {
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, c0, Pc, mu, s, nullptr, prec == 3, certify));
                 } else {
                     RW_CUDA(ctx, launch_gen_A(ctx, d, c0, Pc, s));
                     RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
                 }
             }
             RW_CUDA(ctx, launch_reduce(ctx, D * (prec >= 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, dout + c0, full, s));
+            if (!certify) continue;
+            double *bnd = opt.bound ? opt.bound + c0 : ctx->bound_stage + c0;
+            RW_CUDA(ctx, launch_reduce_max(ctx, D * L.NT8, L.MC, Pc, bnd, s));
+            if (!(opt.tol > 0.0)) continue;
+            // ---- strict: how many points of this chunk are not certified?  (the one place the library reads a number
+            // back: the stream is synchronised once per chunk, so a strict call cannot be captured in a CUDA graph)
+            double *coef_all = ctx->coef, *rate_all = ctx->rate;
+            ctx->coef = coef_all + c0 * kCoefStride; ctx->rate = rate_all + c0 * RW_MAX_COMPONENTS;
+            cudaError_t e = launch_collect_uncertified(ctx, bnd, Pc, opt.tol, true, s);
+            ctx->coef = coef_all; ctx->rate = rate_all;
+            RW_CUDA(ctx, e);
+            int n_bad = 0;
+            RW_CUDA(ctx, cudaMemcpyAsync(&n_bad, ctx->fb_idx + L.MC, 4, cudaMemcpyDeviceToHost, s));
+            RW_CUDA(ctx, cudaStreamSynchronize(s));
+            ctx->strict_fallbacks += n_bad;
+            if (n_bad == 0) continue;
+            if (mu) {            // mu rows cannot be scattered: the whole chunk goes through the DMMA path again
+                ctx->coef = coef_all + c0 * kCoefStride; ctx->rate = rate_all + c0 * RW_MAX_COMPONENTS;
+                int rc = fold_slice(ctx, Pc, RW_MODE_GEMM, full, dout + c0, mu, s, 0);
+                ctx->coef = coef_all; ctx->rate = rate_all;
+                if (rc != RW_OK) return rc;
+                if (opt.bound) RW_CUDA(ctx, cudaMemsetAsync(opt.bound + c0, 0, (size_t)Pc * 8, s));
+            } else {             // only the uncertified points, from their gathered coefficient rows
+                ctx->coef = ctx->coef_fb; ctx->rate = ctx->rate_fb;
+                int rc = fold_slice(ctx, n_bad, RW_MODE_AUTO, full, ctx->out_fb, nullptr, s, 0);
+                ctx->coef = coef_all; ctx->rate = rate_all;
+                if (rc != RW_OK) return rc;
+                RW_CUDA(ctx, launch_scatter_fallback(ctx, n_bad, dout + c0, opt.bound ? opt.bound + c0 : nullptr, s));
+            }
         }
     }
     return RW_OK;
 }
 
-// Contraction regime asked for by the flags: 0 = FP64 DMMA, 1 = RW_FP32, 2 = RW_SLICED, 3 = RW_SLICED_FAST.
-static int pick_prec(rw_ctx *ctx, const char *fn, uint32_t flags, bool fp32_ok, int *prec)
+// Contraction regime asked for by the flags: 0 = FP64 DMMA, 2 = RW_SLICED, 3 = RW_SLICED_FAST / RW_FP32; *tol > 0 when
+// the call is strict (RW_SLICED_STRICT; RW_FP32 always is: its contract is a relative error, not a scale bound).
+static int pick_prec(rw_ctx *ctx, const char *fn, uint32_t flags, bool fp32_ok, int *prec, double *tol)
 {
-    const bool fp32 = flags & RW_FP32, fast = flags & RW_SLICED_FAST, sliced = (flags & RW_SLICED) || fast;
+    const bool fp32 = flags & RW_FP32, fast = (flags & RW_SLICED_FAST) || fp32, sliced = (flags & RW_SLICED) || fast;
     if ((flags & RW_SLICED) && fast)
-        return fail(ctx, RW_ERR_INVALID, "%s: RW_SLICED and RW_SLICED_FAST exclude each other", fn);
+        return fail(ctx, RW_ERR_INVALID, "%s: RW_SLICED, RW_SLICED_FAST and RW_FP32 exclude each other", fn);
+    if (fp32 && (flags & RW_SLICED_FAST))
+        return fail(ctx, RW_ERR_INVALID, "%s: RW_SLICED, RW_SLICED_FAST and RW_FP32 exclude each other", fn);
     if (fp32 && !fp32_ok) return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 is not supported here", fn);
-    if (fp32 && !ctx->lay.fp32)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_FP32 needs a context created with RW_CREATE_FP32", fn);
-    if (sliced && (!ctx->lay.sliced || fp32))
-        return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_SLICED needs a context created with RW_CREATE_SLICED "
-                                             "and excludes RW_FP32", fn);
-    *prec = fast ? 3 : (sliced ? 2 : (fp32 ? 1 : 0));
+    if ((flags & RW_SLICED_STRICT) && !sliced)
+        return fail(ctx, RW_ERR_INVALID, "%s: RW_SLICED_STRICT goes with RW_SLICED or RW_SLICED_FAST", fn);
+    if (sliced && !ctx->lay.sliced)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "%s: RW_SLICED / RW_SLICED_FAST / RW_FP32 need a context created with "
+                                             "RW_CREATE_SLICED (or RW_CREATE_FP32)", fn);
+    *prec = fast ? 3 : (sliced ? 2 : 0);
+    *tol = (fp32 || (flags & RW_SLICED_STRICT)) ? (fast ? 1e-5 : 1e-12) : 0.0;
     return RW_OK;
 }
 
@@ -388,7 +432,13 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->out_stage = (double *)(ws + L.out_stage);
     ctx->mu_tile = (double *)(ws + L.mu_tile);
     ctx->mu_prof = (double *)(ws + L.mu_prof);
-    ctx->R32 = (float *)(ws + L.R32);
+    ctx->gcol8 = (double *)(ws + L.gcol8);
+    ctx->cert_part = (double *)(ws + L.cert_part);
+    ctx->bound_stage = (double *)(ws + L.bound_stage);
+    ctx->fb_idx = (int *)(ws + L.fb_idx);
+    ctx->coef_fb = (double *)(ws + L.coef_fb);
+    ctx->rate_fb = (double *)(ws + L.rate_fb);
+    ctx->out_fb = (double *)(ws + L.out_fb);
     ctx->B8 = (uint8_t *)(ws + L.B8);
     ctx->f_col8 = (int *)(ws + L.f_col8);
     ctx->e_row8 = (int *)(ws + L.e_row8);
@@ -461,19 +511,12 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     }
     rc = make_tensor_maps(ctx);
     if (rc == RW_OK) rc = profile_setup(ctx);
-    if (rc == RW_OK && L.fp32) {
-        ctx->tmapB32 = (CUtensorMap *)calloc(2 * D, sizeof(CUtensorMap));
-        if (!ctx->tmapB32) rc = fail(nullptr, RW_ERR_NOMEM, "rw_create: out of host memory");
-        if (rc == RW_OK) rc = tf32_setup(ctx, s);
-        if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
-            rc = fail(nullptr, RW_ERR_CUDA, "rw_create: TF32 split of R failed: %s", cudaGetErrorString(cudaGetLastError()));
-    }
     if (rc == RW_OK && L.sliced) {
         rc = i8_setup(ctx, s);
         if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
             rc = fail(nullptr, RW_ERR_CUDA, "rw_create: slicing R failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
-    if (rc != RW_OK) { free(ctx->tmapB32); free(ctx->tmapR); free(ctx); return rc; }
+    if (rc != RW_OK) { free(ctx->tmapR); free(ctx); return rc; }
     ctx->err[0] = 0;
     *out = ctx;
     return RW_OK;
@@ -506,8 +549,8 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
     return RW_OK;
 }
 
-int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
-                  double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
+static int eval_batch_impl(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                           double *out_m2lnL, double *out_mu, double *out_bound, uint32_t flags, void *cuda_stream)
 {
     if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_batch: ctx is NULL");
     if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: P < 0 or k outside [0,11]");
@@ -522,7 +565,9 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
     if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_MODE_COLLAPSED needs a single signal component");
     int prec = 0;
-    { int rc = pick_prec(ctx, "rw_eval_batch", flags, true, &prec); if (rc != RW_OK) return rc; }
+    double tol = 0.0;
+    { int rc = pick_prec(ctx, "rw_eval_batch", flags, true, &prec, &tol); if (rc != RW_OK) return rc; }
+    if (mode > RW_MODE_RIDGE) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: unknown mode in flags");
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -540,6 +585,7 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
         double *dout = out_host ? ctx->out_stage : out_m2lnL + s0;
         const bool stream_mode = use_stream(ctx, mode, Ps, prec);
         if (stream_mode || use_ridge(ctx, mode, Ps, prec)) {
+            if (out_bound) RW_CUDA(ctx, cudaMemsetAsync(out_bound + s0, 0, (size_t)Ps * 8, s));       // FP64 paths
             // up to 64 points: ONE launch per group does a1-a4 (coefficients computed in the kernel) -- the
             // HBM-streaming kernel (groups of 16) or the streaming DMMA kernel (groups of 64)
             Kinds kd;
@@ -561,13 +607,36 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
             }
         } else {
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
-        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, prec); if (rc != RW_OK) return rc; }
+        SlicedOpt opt;
+        opt.tol = tol; opt.bound = out_bound ? out_bound + s0 : nullptr;
+        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, prec, opt); if (rc != RW_OK) return rc; }
         }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
     }
     return RW_OK;
 }
+
+int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                  double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
+{
+    return eval_batch_impl(ctx, param, P, k, param_kind, out_m2lnL, out_mu, nullptr, flags, cuda_stream);
+}
+
+int rw_eval_certified(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+                      double *out_m2lnL, double *out_bound, uint32_t flags, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_certified: ctx is NULL");
+    if (!out_bound && P > 0) return fail(ctx, RW_ERR_INVALID, "rw_eval_certified: out_bound is NULL");
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_certified: host buffers are not supported");
+    if (!(flags & (RW_SLICED | RW_SLICED_FAST | RW_FP32)))
+        return fail(ctx, RW_ERR_INVALID, "rw_eval_certified: needs RW_SLICED, RW_SLICED_FAST or RW_FP32 (the FP64 paths "
+                                         "have no input-dependent bound)");
+    return eval_batch_impl(ctx, param, P, k, param_kind, out_m2lnL, nullptr, out_bound, flags, cuda_stream);
+}
+
+int64_t rw_strict_fallback_count(const rw_ctx *ctx) { return ctx ? ctx->strict_fallbacks : 0; }
 
 int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                     double s0, double sigma, double *out_m2lnL, double *out_scale, uint32_t flags,
@@ -589,14 +658,15 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool full = flags & RW_FULL_EQ18;
     int prec = 0;
-    { int rc = pick_prec(ctx, "rw_eval_profile", flags, true, &prec); if (rc != RW_OK) return rc; }
+    SlicedOpt opt;
+    { int rc = pick_prec(ctx, "rw_eval_profile", flags, true, &prec, &opt.tol); if (rc != RW_OK) return rc; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
     // passes of <= prof_rows points: fold with mu written to the scratch, then one CTA per point profiles s
     for (int64_t q0 = 0; q0 < P; q0 += L.prof_rows) {
         const int64_t Pq = (P - q0 < L.prof_rows) ? P - q0 : L.prof_rows;
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
-        int rc = fold_slice(ctx, Pq, mode, false, ctx->out_stage, ctx->mu_prof, s, prec);
+        int rc = fold_slice(ctx, Pq, mode, false, ctx->out_stage, ctx->mu_prof, s, prec, opt);
         if (rc != RW_OK) return rc;
         RW_CUDA(ctx, launch_profile(ctx, ctx->mu_prof, Pq, s0, sigma, full, out_m2lnL + q0,
                                     out_scale ? out_scale + q0 : nullptr, s));
@@ -640,7 +710,7 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
 
 // Dense fold + likelihood for P rows of caller-visible weights w[P][n_T] (device).
 static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, bool full, double *out, double *out_mu,
-                        cudaStream_t s, int prec)
+                        cudaStream_t s, int prec, double tol = 0.0)
 {
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
@@ -663,13 +733,30 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             double *mu = out_mu ? out_mu + (size_t)c0 * D * n_rec : nullptr;
             for (int d = 0; d < D; ++d) {
                 if (prec >= 2) {
-                    RW_CUDA(ctx, launch_fold_i8(ctx, d, 0, Pc, mu, s, w + (size_t)c0 * n_T, prec == 3));
+                    RW_CUDA(ctx, launch_fold_i8(ctx, d, 0, Pc, mu, s, w + (size_t)c0 * n_T, prec == 3, tol > 0.0));
                 } else {
                     RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
                     RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
                 }
             }
             RW_CUDA(ctx, launch_reduce(ctx, D * (prec >= 2 ? L.NT8 : L.n_tiles_n), L.MC, Pc, out + c0, full, s));
+            if (prec >= 2 && tol > 0.0) {
+                // strict: arbitrary weights have no coefficient rows to gather, so a chunk with ANY uncertified point
+                // goes through the DMMA path again as a whole (one stream synchronisation per chunk)
+                RW_CUDA(ctx, launch_reduce_max(ctx, D * L.NT8, L.MC, Pc, ctx->out_fb, s));
+                RW_CUDA(ctx, launch_collect_uncertified(ctx, ctx->out_fb, Pc, tol, false, s));
+                int n_bad = 0;
+                RW_CUDA(ctx, cudaMemcpyAsync(&n_bad, ctx->fb_idx + L.MC, 4, cudaMemcpyDeviceToHost, s));
+                RW_CUDA(ctx, cudaStreamSynchronize(s));
+                ctx->strict_fallbacks += n_bad;
+                if (n_bad > 0) {
+                    for (int d = 0; d < D; ++d) {
+                        RW_CUDA(ctx, launch_gen_A_weights(ctx, d, w + (size_t)c0 * n_T, Pc, s));
+                        RW_CUDA(ctx, launch_fold_gemm(ctx, d, Pc, mu, 0, s));
+                    }
+                    RW_CUDA(ctx, launch_reduce(ctx, D * L.n_tiles_n, L.MC, Pc, out + c0, full, s));
+                }
+            }
         }
     }
     return RW_OK;
@@ -687,8 +774,9 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_weights: collapsed mode, RW_FP32 and host buffers are not supported "
                                              "(arbitrary weights are not low-rank; w is a device array)");
     int prec = 0;
-    { int rc = pick_prec(ctx, "rw_eval_weights", flags, false, &prec); if (rc != RW_OK) return rc; }
-    return weights_rows(ctx, w, P, mode, flags & RW_FULL_EQ18, out_m2lnL, out_mu, (cudaStream_t)cuda_stream, prec);
+    double tol = 0.0;
+    { int rc = pick_prec(ctx, "rw_eval_weights", flags, false, &prec, &tol); if (rc != RW_OK) return rc; }
+    return weights_rows(ctx, w, P, mode, flags & RW_FULL_EQ18, out_m2lnL, out_mu, (cudaStream_t)cuda_stream, prec, tol);
 }
 
 int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
@@ -706,8 +794,9 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: needs a single component created without explicit P_mu/P_tau "
                                              "(the point's 1 - P_e is split by f_tau)");
     int kinds[RW_N_KINDS], prec = 0;
+    double tol = 0.0;
     { int rc = check_kinds(ctx, "rw_eval_pee", k, param_kind, kinds); if (rc != RW_OK) return rc; }
-    { int rc = pick_prec(ctx, "rw_eval_pee", flags, false, &prec); if (rc != RW_OK) return rc; }
+    { int rc = pick_prec(ctx, "rw_eval_pee", flags, false, &prec, &tol); if (rc != RW_OK) return rc; }
     for (int a = 0; a < k; ++a)
         if (kinds[a] >= RW_RATE_0) return fail(ctx, RW_ERR_INVALID, "rw_eval_pee: rate kinds are not accepted");
     cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -719,7 +808,7 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
         RW_CUDA(ctx, launch_weights_pee(ctx, P_e_pts + (size_t)q0 * ctx->n_E, Pq, ctx->mu_prof, s));
         int rc = weights_rows(ctx, ctx->mu_prof, Pq, mode, flags & RW_FULL_EQ18, out_m2lnL + q0,
-                              out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s, prec);
+                              out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s, prec, tol);
         if (rc != RW_OK) return rc;
     }
     return RW_OK;
@@ -777,7 +866,6 @@ int rw_destroy(rw_ctx *ctx)
         for (int q = 0; q < 2 * ctx->prof_cap; ++q) cudaEventDestroy(ctx->prof_ev[q]);
         free(ctx->prof_ev);
     }
-    free(ctx->tmapB32);
     free(ctx->tmapR);
     free(ctx);
     return RW_OK;

@@ -21,6 +21,17 @@
 // else, so the error is a bound in terms of the scales, not of the individual mu: for responses whose columns
 // spread over many recoil bins (all BASELINE configurations) it is < 1e-13 of mu; see DESIGN.md section 3.3.
 //
+// CERTIFICATE.  With A_i = N'[p][i] 2^-tau_i < 2^e_p, B_i = R[i][k] 2^tau_i < 2^f_k, K'_k the number of recoil bins
+// whose fixed-point R entry is non-zero and S_k = sum_i B_i 2^-f_k (<= K'_k):
+//   rounding of A:  sum_i |A_i - A~_i| B_i   <= 2^(e_p - 8 NS) 2^f_k S_k          (half an ulp of 2^(e_p - 8 NS + 1) each)
+//   rounding of B:  sum_i A~_i |B_i - B~_i|  <= 2^(f_k - 8 NS) 2^e_p K'_k
+//   dropped pairs s + t >= NS (|digits| <= 129, 128; both digits are lower ones):
+//                   K'_k 2^(e_p + f_k - 14) 16512 sum_{d >= NS} (2 NS - 1 - d) 2^(-8 d)  <=  1.01 NS K'_k 2^(e_p + f_k - 8 NS)
+// so |mu~ - mu| <= 2^e_p g_k with the per-column constant g_k = 2^(f_k - 8 NS) (S_k + (1 + 1.01 NS) K'_k), computed once
+// at rw_create (k_col_bound); the fast mode adds the diagonals 4 .. NS - 1 it leaves out: 5.07 K'_k 2^(e_p + f_k - 32).
+// The epilogue turns it into the certified relative error max_k delta / (mu~ - delta) (+ 2e-15 for its own FP64
+// rounding) of every point, which rw_eval_certified returns and RW_SLICED_STRICT acts on (rw_api.cu).
+//
 // One CTA per SM, 320 threads (TMA warp, MMA warp, 8 epilogue warps), tile 128 points x 128 bins, 32 recoil bins per
 // k-block.  The slices are stored in global memory already in the tensor core's canonical K-major no-swizzle layout
 // (8 x 16-byte core matrices), all slices of a (tile, k-block) contiguous: a stage is plain bulk copies into a 64 KB
@@ -40,7 +51,7 @@ constexpr int kI8Threads = 320;                                 // TMA warp, MMA
 #define RW_I8_STAGES 3              // measured: 2 slots cost 0.7 %, a 4th does not fit
 #endif
 constexpr int kI8SlotBytes = 65536, kI8Stages = RW_I8_STAGES;   // a slot: N' slices in its first half, R slices in its second
-constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 4 * kI8BN * 8 + 256 + 1024;
+constexpr int kI8Smem = kI8Stages * kI8SlotBytes + 5 * kI8BN * 8 + 256 + 1024;
 constexpr int kI8SegKT = 512;       // k-blocks (16384 bins) accumulated in int32 before the epilogue drains TMEM:
                                     // 7 pairs x 129 x 128 x 16384 bins < 2^31; longer contractions go in segments
 constexpr int kI8BadRow = INT_MAX;                              // exponent marker: the row holds a non-finite / negative value
@@ -347,6 +358,27 @@ __global__ void k_colexp_B(const double *__restrict__ R, int ldR, int n_T, int n
     f_col[k] = i8_exponent(vmax);
 }
 
+// g_k of the certificate (header comment): per column, the number of recoil bins whose fixed-point entry is non-zero
+// and the sum of the rescaled entries.  gcol[0][k]: full contraction, gcol[1][k]: fast mode.
+__global__ void k_col_bound(const double *__restrict__ R, int ldR, int n_T, int n_rec, int ns, const int *__restrict__ tau,
+                            const int *__restrict__ f_col, double *__restrict__ gcol /*[2][n_rec]*/)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_rec) return;
+    const int f = f_col[k];
+    const double scale2 = ldexp(1.0, 8 * ns - 1 - f);
+    double sum = 0.0, cnt = 0.0;
+    for (int i = 0; i < n_T; ++i) {
+        const double v = ldexp(R[(size_t)i * ldR + k], tau[i]);
+        sum += v;
+        if (__double2ull_rn(v * scale2) != 0ull) cnt += 1.0;
+    }
+    const double S = ldexp(sum, -f) * (1.0 + 1e-9);                  // its own summation rounding
+    const double full = ldexp(S + (1.0 + 1.01 * ns) * cnt, f - 8 * ns) * (1.0 + 1e-6);
+    gcol[k] = full;
+    gcol[(size_t)n_rec + k] = full + ldexp(5.07 * cnt, f - 32);
+}
+
 // Slices of R in  Bs[n-tile][k-block][slice][chunk c][column group g][column r8][16]  (K-major core matrices,
 // "rows" of the B operand are reconstructed bins).  Thread = (column, 16 consecutive recoil bins).
 __global__ void __launch_bounds__(256)
@@ -452,7 +484,9 @@ struct I8Work {
     const uint8_t *As, *Bs;
     const int *e_row, *f_col;
     const double *bkg, *counts;
+    const double *gcol;       // [n_rec] certificate constants of this period and mode, or NULL
     double *partial, *out_mu;
+    double *cert;             // [2 tiles_n][part_stride] certified relative error per (half tile, point), or NULL
 };
 
 __device__ __forceinline__ void i8_tile_coord(int t, int tiles_m, int tiles_n, int &tm, int &tn)
@@ -495,10 +529,11 @@ k_fold_i8(const I8Work W)
     const uint32_t sbase = i8_smem_u32(smem);
     double *s_bkg = reinterpret_cast<double *>(smem + kStages * kSlot);                // [128] per tile
     double *s_cnt = s_bkg + kI8BN, *s_inv = s_cnt + kI8BN, *s_scl = s_inv + kI8BN;    // counts, 1/counts, 2^f_k
-    const uint32_t bars = sbase + kStages * kSlot + 4 * kI8BN * 8;
+    double *s_g = s_scl + kI8BN;                                                      // certificate constants g_k
+    const uint32_t bars = sbase + kStages * kSlot + 5 * kI8BN * 8;
     const uint32_t full_bar = bars, empty_bar = bars + 8 * kStages;
     const uint32_t tfull_bar = empty_bar + 8 * kStages, tempty_bar = tfull_bar + 8;
-    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kStages * kSlot + 4 * kI8BN * 8 + 128);
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kStages * kSlot + 5 * kI8BN * 8 + 128);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -627,6 +662,7 @@ k_fold_i8(const I8Work W)
                 s_cnt[et] = n;
                 s_inv[et] = n > 0.0 ? 1.0 / n : 0.0;
                 s_scl[et] = ok ? ldexp(1.0, W.f_col[col]) : 0.0;
+                s_g[et] = (ok && W.gcol) ? W.gcol[col] : 0.0;
             }
             asm volatile("bar.sync 1, 256;" ::: "memory");
             const int64_t row = (int64_t)tm * kI8BM + lrow;
@@ -673,7 +709,8 @@ k_fold_i8(const I8Work W)
                 __syncwarp();
                 if (lane == 0) i8_mbar_arrive(tempty_bar);       // the next tile's products run under the Poisson terms
             }
-            double tot = 0.0;
+            double tot = 0.0, worst = 0.0;
+            const double escale = (e == kI8BadRow) ? 0.0 : ldexp(1.0, e);      // delta_k = 2^e_p g_k
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
 #pragma unroll
@@ -683,6 +720,15 @@ k_fold_i8(const I8Work W)
                     const double m1 = fma(v[g][j + 1] * rscale, s_scl[c0 + 1], s_bkg[c0 + 1]);
                     const double m2 = fma(v[g][j + 2] * rscale, s_scl[c0 + 2], s_bkg[c0 + 2]);
                     const double m3 = fma(v[g][j + 3] * rscale, s_scl[c0 + 3], s_bkg[c0 + 3]);
+                    if (W.cert) {        // certified |mu~ - mu| / mu <= delta / (mu~ - delta); +inf where delta >= mu~ > 0
+                        const double mm[4] = {m0, m1, m2, m3};
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const double dl = escale * s_g[c0 + u];
+                            const double rel = (dl > 0.0) ? ((mm[u] > dl) ? dl / (mm[u] - dl) : __longlong_as_double(0x7ff0000000000000LL)) : 0.0;
+                            worst = fmax(worst, rel);
+                        }
+                    }
                     if (W.out_mu && row < W.Pc) {
                         const int col = tn * kI8BN + c0;
                         double *dst = W.out_mu + ((size_t)row * W.D + W.d) * W.n_rec + col;
@@ -696,6 +742,9 @@ k_fold_i8(const I8Work W)
                 }
             }
             if (row < W.Pc) W.partial[(size_t)(2 * tn + half) * W.part_stride + row] = tot;
+            if (W.cert && row < W.Pc)       // a row that could not be sliced (NaN result) certifies nothing
+                W.cert[(size_t)(2 * tn + half) * W.part_stride + row] =
+                    (e == kI8BadRow) ? __longlong_as_double(0x7ff0000000000000LL) : worst + 2e-15;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -725,9 +774,11 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
                                          ctx->blk_hl8 + ((size_t)d * 2 + 1) * kNumTerms * KT, ctx->blk_cm8);
         ctx->launches++;
         k_colexp_B<<<(ctx->n_rec + 127) / 128, 128, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, tau, f);
+        k_col_bound<<<(ctx->n_rec + 127) / 128, 128, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, L.ns8, tau, f,
+                                                              ctx->gcol8 + (size_t)d * 2 * ctx->n_rec);
         dim3 grid((n_cols + 255) / 256, KT * 2);
         k_slice_B<<<grid, 256, 0, s>>>(Rd, ctx->ldR, ctx->n_T, ctx->n_rec, n_cols, KT, L.ns8, tau, f, ctx->B8 + (size_t)d * per);
-        ctx->launches += 3;
+        ctx->launches += 4;
     }
     if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "slicing R failed at launch");
     cudaError_t e = cudaFuncSetAttribute(k_fold_i8<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kI8Smem);
@@ -743,7 +794,7 @@ int i8_setup(rw_ctx *ctx, cudaStream_t s)
 // Steps a1-a4 for the Pc points at coef[p0..] and period d through the sliced INT8 contraction.
 // With `w` (weights of the chunk's Pc points, [Pc][n_T]) the rows are N' = w N_mc instead of the coefficient rows.
 cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s, const double *w,
-                           bool fast)
+                           bool fast, bool certify)
 {
     const Layout &L = ctx->lay;
     const int KT = L.KT8;
@@ -782,6 +833,8 @@ cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *o
     W.counts = ctx->counts + (size_t)d * ctx->n_rec;
     W.partial = ctx->partial + (size_t)d * L.NT8 * L.MC;       // [D][NT8][MC]: 64-column half tiles in this mode
     W.out_mu = out_mu;
+    W.gcol = certify ? ctx->gcol8 + ((size_t)d * 2 + (fast ? 1 : 0)) * ctx->n_rec : nullptr;
+    W.cert = certify ? ctx->cert_part + (size_t)d * L.NT8 * L.MC : nullptr;
     const int total = W.tiles_m * W.tiles_n;
     const int grid = total < ctx->num_sms ? total : ctx->num_sms;
     {

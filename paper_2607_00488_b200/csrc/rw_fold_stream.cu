@@ -273,6 +273,86 @@ __global__ void k_reduce(const double *__restrict__ partial, int n_parts, int64_
     out[p] = v;
 }
 
+// bound[p] = max over parts of cert[part][p]: the certified relative error of the sliced contraction per point.
+__global__ void k_reduce_max(const double *__restrict__ cert, int n_parts, int64_t part_stride, int64_t Pc,
+                             double *__restrict__ bound)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= Pc) return;
+    double v = 0.0;
+    for (int q = 0; q < n_parts; ++q) v = fmax(v, cert[(size_t)q * part_stride + p]);
+    bound[p] = v;
+}
+
+cudaError_t launch_reduce_max(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *bound, cudaStream_t s)
+{
+    k_reduce_max<<<(unsigned)((Pc + 255) / 256), 256, 0, s>>>(ctx->cert_part, n_parts, part_stride, Pc, bound);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+// Strict mode: the points of a slice whose certified bound exceeds `tol` (NaN bounds included) -> compact list.
+// idx[0 .. *count) ascending (one thread block scans in order, so the list -- and with it the fallback -- is
+// deterministic); their coefficient and rate rows are gathered next to it.
+__global__ void __launch_bounds__(1024)
+k_collect_uncertified(const double *__restrict__ bound, int64_t Ps, double tol, const double *__restrict__ coef,
+                      const double *__restrict__ rate, int *__restrict__ idx, int *__restrict__ count,
+                      double *__restrict__ coef_fb, double *__restrict__ rate_fb)
+{
+    __shared__ int s_warp[32], s_base;
+    if (threadIdx.x == 0) s_base = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int64_t p0 = 0; p0 < Ps; p0 += 1024) {
+        const int64_t p = p0 + threadIdx.x;
+        const bool bad = p < Ps && !(bound[p] <= tol);
+        const unsigned m = __ballot_sync(0xffffffffu, bad);
+        if (lane == 0) s_warp[warp] = __popc(m);
+        __syncthreads();
+        int off = s_base;
+        for (int w = 0; w < warp; ++w) off += s_warp[w];
+        if (bad) {
+            const int q = off + __popc(m & ((1u << lane) - 1));
+            idx[q] = (int)p;
+            if (coef) {
+#pragma unroll
+            for (int b = 0; b < kCoefStride; ++b) coef_fb[(size_t)q * kCoefStride + b] = coef[(size_t)p * kCoefStride + b];
+#pragma unroll
+            for (int c = 0; c < RW_MAX_COMPONENTS; ++c) rate_fb[(size_t)q * RW_MAX_COMPONENTS + c] = rate[(size_t)p * RW_MAX_COMPONENTS + c];
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) { int t = 0; for (int w = 0; w < 32; ++w) t += s_warp[w]; s_base += t; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *count = s_base;
+}
+
+// out[idx[q]] = out_fb[q], bound[idx[q]] = 0 (recomputed in FP64 by the DMMA path)
+__global__ void k_scatter_fallback(const int *__restrict__ idx, int n, const double *__restrict__ out_fb,
+                                   double *__restrict__ out, double *__restrict__ bound)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n) return;
+    out[idx[q]] = out_fb[q];
+    if (bound) bound[idx[q]] = 0.0;
+}
+
+cudaError_t launch_collect_uncertified(rw_ctx *ctx, const double *bound, int64_t Ps, double tol, bool gather, cudaStream_t s)
+{
+    k_collect_uncertified<<<1, 1024, 0, s>>>(bound, Ps, tol, gather ? ctx->coef : nullptr, ctx->rate, ctx->fb_idx, ctx->fb_idx + ctx->lay.MC,
+                                             ctx->coef_fb, ctx->rate_fb);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_fallback(rw_ctx *ctx, int n, double *out, double *bound, cudaStream_t s)
+{
+    k_scatter_fallback<<<(n + 255) / 256, 256, 0, s>>>(ctx->fb_idx, n, ctx->out_fb, out, bound);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
                           bool full_eq18, cudaStream_t s)
 {

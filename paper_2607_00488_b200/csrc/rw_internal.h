@@ -52,8 +52,9 @@ struct Kinds { int k; int kind[RW_N_KINDS]; };
 struct Layout {           // byte offsets into the workspace (all 256-byte aligned)
     size_t E, fw, P3, T, Tmax_invE, N_mc, bkg, counts, R_copy;
     size_t basis, S_sm, What, sat_const, flag, G, ident, stream_cnt, strip_part, comp8, rate;
-    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof, R32;
+    size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof;
     size_t B8, f_col8, e_row8, tau8, blk_hl8, blk_cm8, tau8b, comp8p;
+    size_t gcol8, cert_part, bound_stage, fb_idx, coef_fb, rate_fb, out_fb;
     int KP512;            // n_T rounded up to 512 bins (staging chunk of k_slice_A)
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
@@ -66,11 +67,9 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int ridge_strips;     // ceil(n_rec / kRidgeCols)
     int ridge_max_p;      // largest tile height of k_fold_ridge the slot scratch was sized for (16, 32 or 64)
     size_t ridge_cnt, ridge_part, ridge_slots;
-    int KP32;             // row pitch (floats) of the FP32 operands: n_T rounded up to 4
     bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
     int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 2048, else 7 (rw_api.cu plan())
     int KT8, NT8;         // k-blocks of 32 recoil bins; 64-column units = 2 x (128-column tiles) (rw_fold_i8.cu)
-    bool fp32;            // RW_CREATE_FP32: the TF32 hi/lo copy of R is in the workspace
     int64_t prof_rows;    // points per pass of rw_eval_profile (rows of the mu scratch)
     int64_t pee_rows;     // points per pass of rw_eval_pee (rows of n_T weights the same scratch holds)
     int mu_tile_items;    // capacity of the split-K scratch in (tile, k-range) work items
@@ -113,15 +112,18 @@ struct rw_ctx {
     int *blk_cm8;             // [KT8] components present in each 32-bin block
     int8_t *tau8b;            // [D][KP512] tau as bytes, zero-padded (cp.async staging of k_slice_A)
     uint8_t *comp8p;          // [KP512] comp8, zero-padded
-    float *R32;               // [D][2 (hi, lo)][n_rec][KP32] transposed TF32 split of R (RW_CREATE_FP32)
-    CUtensorMap tmapA32[2];   // hi, lo of N' (aliases A_packed)
-    CUtensorMap *tmapB32;     // host array [2 D]
+    double *gcol8;            // [D][2: full, fast][n_rec] certificate constants g_k of the sliced contraction
+    double *cert_part;        // [D][NT8][MC] certified relative error per (half tile, point)
+    double *bound_stage;      // [max_batch] certified bound per point of a slice (strict mode without a caller array)
+    int *fb_idx;              // [MC] + 1: uncertified points of a chunk (ascending), then their count
+    double *coef_fb, *rate_fb, *out_fb;   // [MC][12], [MC][4], [MC]: their coefficient rows / recomputed values
     double *mu_prof;          // rw_eval_profile scratch: mu[prof_rows][D][n_rec]
     double *mu_tile;          // split-K scratch: [mu_tile_items][<=128][128] parked accumulators
     CUtensorMap *tmapR;       // host array [D]
     CUtensorMap tmapA[4];     // N' maps for tile heights 16, 32, 64, 128
     int num_sms;
     int64_t launches;
+    int64_t strict_fallbacks; // points recomputed by the DMMA path in strict sliced calls so far
     // measurement hooks (rw_profile_begin/end)
     cudaEvent_t *prof_ev;     // pairs: [2q] before, [2q+1] after fold launch q
     int prof_cap, prof_n;     // pairs allocated / recorded
@@ -177,9 +179,11 @@ cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool 
                         double *grad, cudaStream_t s);                       // rw_grad.cu
 int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
 cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s,
-                           const double *w = nullptr, bool fast = false);    // rw_fold_i8.cu
-int tf32_setup(rw_ctx *ctx, cudaStream_t s);                                 // rw_fold_tf32.cu
-cudaError_t launch_fold_tf32(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s);  // rw_fold_tf32.cu
+                           const double *w = nullptr, bool fast = false, bool certify = false);    // rw_fold_i8.cu
+cudaError_t launch_reduce_max(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *bound,
+                              cudaStream_t s);                               // rw_fold_stream.cu
+cudaError_t launch_collect_uncertified(rw_ctx *ctx, const double *bound, int64_t Ps, double tol, bool gather, cudaStream_t s);   // rw_fold_stream.cu
+cudaError_t launch_scatter_fallback(rw_ctx *ctx, int n, double *out, double *bound, cudaStream_t s);               // rw_fold_stream.cu
 cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu,
                              cudaStream_t s);                                // rw_collapsed.cu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
