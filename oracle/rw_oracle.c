@@ -41,6 +41,9 @@
  *   orc_eval_pee      reference P_ee for every point reproduces orc_eval_batch; equals orc_eval_weights fed
  *                     the spectrum ratio computed with orc_spectrum on the point's table; P_ee = 1 / 0 on a
  *                     single line give the pure nu_e / nu_mu,tau cross-section ratio of Eq. (4)
+ *   orc_eval_pee_components  single component without explicit tables reproduces orc_eval_pee; the nominal
+ *                     tables for every point reproduce orc_eval_components (explicit tables included, so the rho
+ *                     split returns exactly P_mu, P_tau); a component's bins follow its own table only
  *   orc_eval_weights  equals orc_eval_batch when fed orc_weights(theta); numpy matmul +
  *                     scipy Poisson on random weights; w == 1 gives the SM prediction
  * No function here is "parity unpinned".
@@ -685,6 +688,84 @@ int orc_eval_pee(const orc_consts *c, int n_E, const double *E, const double *fl
         xreal *S = (xreal *)malloc(sizeof(xreal) * (size_t)(2 * n_T + n_rec + 1));
         xreal *w = S + n_T, *mu = w + n_T;
         xspectrum(c, n_E, E, flux_w, Pp, Pm, Pt, n_T, T, theta, S);
+        xweights(n_T, S, S0, w);
+        xreal total = 0.0L, total_abs = 0.0L;
+        for (int d = 0; d < n_periods; ++d) {
+            const double *Cd = counts + (size_t)d * n_rec;
+            xfold(n_T, n_rec, w, N_mc + (size_t)d * n_T, R + (size_t)d * n_T * n_rec, bkg + (size_t)d * n_rec, mu);
+            total += full_eq18 ? xeq18(n_rec, mu, Cd) : xdeviance(n_rec, mu, Cd);
+            if (mu_out)
+                for (int q = 0; q < n_rec; ++q) mu_out[((size_t)p * n_periods + d) * n_rec + q] = (double)mu[q];
+            if (abs_out)
+                for (int q = 0; q < n_rec; ++q) total_abs += fabsl(xdeviance(1, mu + q, Cd + q));
+        }
+        out[p] = (double)total;
+        if (abs_out) abs_out[p] = (double)total_abs;
+        free(S);
+        free(Pm);
+    }
+    free(S0);
+    free(Pm0);
+    return 0;
+}
+
+/* Per-point survival probabilities with several signal components and / or explicit nominal nu_mu, nu_tau tables
+ * (Eq. 17, on top of the per-point physics update of PAPER.md:220).  P_e_pts[p][q][.] is the nu_e
+ * survival probability of point p for component q on the shared E grid.  The paper does not say how the rest,
+ * 1 - P_e, of a point is shared between nu_mu and nu_tau when the analysis was set up with explicit tables:
+ * DESIGN.md reading R17 keeps the nominal tables' mu : tau ratio at every energy,
+ *     P_mu^p(E) = (1 - P_e^p(E)) P_mu(E) / (P_mu(E) + P_tau(E)),   P_tau^p likewise
+ * (where P_mu + P_tau = 0, and when no explicit tables were given: the f_tau split of reading R3).  The SM reference of
+ * a bin is computed from the NOMINAL tables of its component (reading R16).  Single-component calls without
+ * explicit tables reduce to orc_eval_pee. */
+int orc_eval_pee_components(const orc_consts *c, int n_E, const double *E, int n_comp, const double *flux_w,
+                            const double *P_e, const double *P_mu, const double *P_tau, int have_mu_tau, double f_tau,
+                            int n_T, const double *T, const int32_t *comp_of_T, int n_rec, int n_periods,
+                            const double *N_mc, const double *R, const double *bkg, const double *counts,
+                            int64_t P, int k, const int32_t *kinds, const double *params, const double *P_e_pts,
+                            double *out, double *mu_out, double *abs_out, int full_eq18, int nthreads)
+{
+    static const double zero[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+    if (n_comp < 1 || n_comp > 4) return -1;
+    for (int a = 0; a < k; ++a) {
+        if (kinds[a] < 0 || kinds[a] >= ORC_N_KINDS) return -1;
+        for (int b = 0; b < a; ++b) if (kinds[a] == kinds[b]) return -1;
+    }
+    for (int i = 0; i < n_T; ++i) if (comp_of_T[i] < 0 || comp_of_T[i] >= n_comp) return -1;
+    size_t nT = (size_t)(n_T > 0 ? n_T : 1), nE = (size_t)(n_E > 0 ? n_E : 1);
+    /* nominal nu_mu / nu_tau tables (given, or the f_tau split) and the share rho of 1 - P_e each flavour takes */
+    double *Pm0 = (double *)malloc(sizeof(double) * 4 * nE * (size_t)n_comp);
+    double *Pt0 = Pm0 + nE * n_comp, *rho_m = Pt0 + nE * n_comp, *rho_t = rho_m + nE * n_comp;
+    for (size_t j = 0; j < nE * (size_t)n_comp; ++j) {
+        if (have_mu_tau) { Pm0[j] = P_mu[j]; Pt0[j] = P_tau[j]; }
+        else { Pm0[j] = (1.0 - P_e[j]) * (1.0 - f_tau); Pt0[j] = (1.0 - P_e[j]) * f_tau; }
+        double sum = Pm0[j] + Pt0[j];
+        if (have_mu_tau && sum > 0.0) { rho_m[j] = Pm0[j] / sum; rho_t[j] = Pt0[j] / sum; }
+        else { rho_m[j] = 1.0 - f_tau; rho_t[j] = f_tau; }
+    }
+    xreal *S0 = (xreal *)malloc(sizeof(xreal) * nT * 2), *tmp0 = S0 + nT;
+    for (int q = 0; q < n_comp; ++q) {
+        xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, P_e + (size_t)q * n_E, Pm0 + (size_t)q * n_E,
+                  Pt0 + (size_t)q * n_E, n_T, T, zero, tmp0);
+        for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S0[i] = tmp0[i];
+    }
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int64_t p = 0; p < P; ++p) {
+        double theta[ORC_N_KINDS] = {0, 0, 0, 0, 0, 0, 0};
+        for (int a = 0; a < k; ++a) theta[kinds[a]] = params[p * k + a];
+        double *Pm = (double *)malloc(sizeof(double) * 2 * nE), *Pt = Pm + nE;
+        xreal *S = (xreal *)malloc(sizeof(xreal) * (3 * nT + (size_t)n_rec + 1));
+        xreal *tmp = S + nT, *w = tmp + nT, *mu = w + nT;
+        for (int q = 0; q < n_comp; ++q) {
+            const double *Pp = P_e_pts + ((size_t)p * n_comp + q) * n_E;
+            for (int j = 0; j < n_E; ++j) {
+                Pm[j] = (1.0 - Pp[j]) * rho_m[(size_t)q * n_E + j];
+                Pt[j] = (1.0 - Pp[j]) * rho_t[(size_t)q * n_E + j];
+            }
+            xspectrum(c, n_E, E, flux_w + (size_t)q * n_E, Pp, Pm, Pt, n_T, T, theta, tmp);
+            for (int i = 0; i < n_T; ++i) if (comp_of_T[i] == q) S[i] = tmp[i];
+        }
         xweights(n_T, S, S0, w);
         xreal total = 0.0L, total_abs = 0.0L;
         for (int d = 0; d < n_periods; ++d) {

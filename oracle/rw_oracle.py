@@ -404,3 +404,53 @@ def eval_pee(inp, params, kinds, P_e_pts, want_mu=False, want_abs=False, full_eq
     if want_abs:
         res.append(ab)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def eval_pee_components(inp, params, kinds, P_e_pts, want_mu=False, want_abs=False, full_eq18=False, nthreads=1,
+                        consts=None):
+    """Per-point survival probabilities with several components and / or explicit nominal P_mu, P_tau tables
+    (reading R17).  ``inp`` as for eval_components; P_e_pts is [P][n_comp][n_E] ([P][n_E] for one)."""
+    c = consts or default_consts()
+    E, T = _a(inp["E"]), _a(inp["T"])
+    fw = np.atleast_2d(_a(inp["flux_w"]))
+    n_comp, n_E = fw.shape
+    P_e = np.atleast_2d(_a(inp["P_e"]))
+    have = inp.get("P_mu") is not None and inp.get("P_tau") is not None
+    f_tau = float(inp.get("f_tau", 0.5))
+    if have:
+        P_mu, P_tau = np.atleast_2d(_a(inp["P_mu"])), np.atleast_2d(_a(inp["P_tau"]))
+    else:
+        P_mu, P_tau = _a((1.0 - P_e) * (1.0 - f_tau)), _a((1.0 - P_e) * f_tau)
+    comp = np.ascontiguousarray(inp.get("comp_of_T", np.zeros(T.size)), dtype=np.int32)
+    R = _a(inp["R"])
+    if R.ndim == 2:
+        R = R[None]
+    D, n_T, n_rec = R.shape
+    N_mc = _a(inp["N_mc"]).reshape(D, n_T)
+    bkg = _a(inp["bkg"]).reshape(D, n_rec)
+    counts = _a(inp["counts"]).reshape(D, n_rec)
+    params = _a(params)
+    if params.ndim == 1:
+        params = params[:, None]
+    P, k = params.shape
+    pts = _a(P_e_pts).reshape(P, n_comp, n_E)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    out = np.empty(P)
+    mu = np.empty((P, D, n_rec)) if want_mu else None
+    ab = np.empty(P) if want_abs else None
+    L = lib()
+    L.orc_eval_pee_components.restype = C.c_int
+    rc = L.orc_eval_pee_components(
+        C.byref(c), C.c_int(n_E), _p(E), C.c_int(n_comp), _p(fw), _p(P_e), _p(P_mu), _p(P_tau),
+        C.c_int(1 if have else 0), C.c_double(f_tau), C.c_int(n_T), _p(T), comp.ctypes.data_as(C.POINTER(C.c_int32)),
+        C.c_int(n_rec), C.c_int(D), _p(N_mc), _p(R), _p(bkg), _p(counts), C.c_int64(P), C.c_int(k),
+        kinds.ctypes.data_as(C.POINTER(C.c_int32)), _p(params), _p(pts), _p(out), _p(mu) if want_mu else None,
+        _p(ab) if want_abs else None, C.c_int(1 if full_eq18 else 0), C.c_int(int(nthreads)))
+    if rc != 0:
+        raise ValueError("orc_eval_pee_components: invalid kinds / component indices")
+    res = [out]
+    if want_mu:
+        res.append(mu)
+    if want_abs:
+        res.append(ab)
+    return res[0] if len(res) == 1 else tuple(res)

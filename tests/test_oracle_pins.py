@@ -533,6 +533,65 @@ def test_eval_pee_pins(orc):
     assert abs(mu1[1, 0, 0] - (1.0 + 0.9 * 100.0 * sm / nominal)) < 1e-12 * mu1[1, 0, 0]
 
 
+def test_eval_pee_components_pins(orc):
+    """Per-point survival probabilities with components / explicit nominal nu_mu, nu_tau tables (reading R17):
+    (i) one component, no explicit tables = orc_eval_pee; (ii) the nominal P_e for every point = orc_eval_components,
+    with explicit tables too (the rho split then returns exactly P_mu, P_tau); (iii) = eval_weights fed spectrum
+    ratios built with orc.spectrum from hand-split tables P_mu^p = (1 - P_e^p) P_mu / (P_mu + P_tau);
+    (iv) changing the table of component 1 leaves the bins of component 0 untouched; (v) a single line with
+    explicit tables in ratio 3 : 1: P_e^p = 0 gives the 3/4 nu_mu + 1/4 nu_tau cross-section mixture."""
+    inp = _small_problem(D=2)
+    params, kinds = wl.random_points(3, [orc.EPS_EE_L, orc.EPS_MM_R, orc.EPS_TT_L, orc.MU_NU], seed=61)
+    n_E = inp["E"].size
+    rng = np.random.default_rng(62)
+    Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.2, 0.2, size=(3, n_E)), 0.0, 1.0)
+    a, mu_a = orc.eval_pee(inp, params, kinds, Pp, want_mu=True)
+    b, mu_b = orc.eval_pee_components(inp, params, kinds, Pp, want_mu=True)
+    assert np.array_equal(a, b) and np.array_equal(mu_a, mu_b)                                   # (i)
+    mc = wl.make_components(n_comp=2, n_E=21, n_T=30, n_rec=17, n_periods=1, seed=63)
+    frac = rng.uniform(0.2, 0.8, size=mc["P_e"].shape)
+    mc["P_mu"] = (1.0 - mc["P_e"]) * frac
+    mc["P_tau"] = (1.0 - mc["P_e"]) * (1.0 - frac)
+    ref, mu_ref = orc.eval_components(mc, params, kinds, want_mu=True)
+    nom = np.tile(mc["P_e"][None], (3, 1, 1))
+    out, mu = orc.eval_pee_components(mc, params, kinds, nom, want_mu=True)
+    assert np.all(np.abs(mu / mu_ref - 1) < 1e-14) and np.all(np.abs(out - ref) <= 1e-11 * np.abs(ref))   # (ii)
+    pts = np.clip(nom + rng.uniform(-0.2, 0.2, size=nom.shape), 0.0, 1.0)
+    out, mu = orc.eval_pee_components(mc, params, kinds, pts, want_mu=True, nthreads=2)
+    comp = mc["comp_of_T"]
+    w = np.ones((3, mc["T"].size))
+    for q in range(2):
+        one = dict(mc, flux_w=mc["flux_w"][q], P_e=mc["P_e"][q], P_mu=mc["P_mu"][q], P_tau=mc["P_tau"][q])
+        S0 = orc.spectrum(one, np.zeros(7))
+        for p in range(3):
+            share = mc["P_mu"][q] / (mc["P_mu"][q] + mc["P_tau"][q])
+            tab = dict(one, P_e=pts[p, q], P_mu=(1 - pts[p, q]) * share, P_tau=(1 - pts[p, q]) * (1 - share))
+            S = orc.spectrum(tab, orc.theta_vector(params[p], kinds))
+            sel = (comp == q) & (S0 > 0)
+            w[p, sel] = S[sel] / S0[sel]
+    out_w, mu_w = orc.eval_weights(mc, w, want_mu=True)
+    assert np.all(np.abs(mu / mu_w - 1) < 1e-14) and np.all(np.abs(out / out_w - 1) < 1e-12)              # (iii)
+    pts2 = pts.copy()
+    pts2[:, 1] = np.clip(pts[:, 1] + 0.1, 0.0, 1.0)
+    # a response that keeps the components apart in the observable: identity-like rows
+    iso = dict(mc, R=np.eye(mc["T"].size)[None], bkg=np.ones((1, mc["T"].size)), counts=np.ones((1, mc["T"].size)))
+    _, m1 = orc.eval_pee_components(iso, params, kinds, pts, want_mu=True)
+    _, m2 = orc.eval_pee_components(iso, params, kinds, pts2, want_mu=True)
+    assert np.array_equal(m1[:, 0, comp == 0], m2[:, 0, comp == 0]) and not np.allclose(m1[:, 0, comp == 1], m2[:, 0, comp == 1])  # (iv)
+    E0, T0, pe0 = 0.862, 0.3, 0.54
+    gL, gR = orc.sm_couplings()
+    line = dict(E=np.array([E0]), flux_w=np.array([2.0]), P_e=np.array([pe0]), P_mu=np.array([0.75 * (1 - pe0)]),
+                P_tau=np.array([0.25 * (1 - pe0)]), T=np.array([T0]), N_mc=np.array([[100.0]]), R=np.array([[[0.9]]]),
+                bkg=np.array([[1.0]]), counts=np.array([[50.0]]))
+    eps_tt = 0.2                                                     # makes nu_tau differ from nu_mu
+    se = orc.dsigma_weak(E0, T0, gL[0], gR[0])
+    sm = orc.dsigma_weak(E0, T0, gL[1], gR[1])
+    st = orc.dsigma_weak(E0, T0, gL[2] + eps_tt, gR[2])
+    nominal = pe0 * se + (1 - pe0) * (0.75 * sm + 0.25 * orc.dsigma_weak(E0, T0, gL[2], gR[2]))
+    _, mu1 = orc.eval_pee_components(line, np.full((1, 1), eps_tt), [orc.EPS_TT_L], np.array([[0.0]]), want_mu=True)
+    assert abs(mu1[0, 0, 0] - (1.0 + 0.9 * 100.0 * (0.75 * sm + 0.25 * st) / nominal)) < 1e-12 * mu1[0, 0, 0]       # (v)
+
+
 def test_sm_point_gives_sm_prediction(orc):
     inp = _small_problem(D=2)
     _, mu = orc.eval_batch(inp, np.zeros((1, 1)), [orc.EPS_EE_L], want_mu=True)
