@@ -212,15 +212,16 @@ int rw_eval_weights(rw_ctx *ctx, const double *w, int64_t P, double *out_m2lnL, 
 
 /* rw_eval_pee: the path with a survival-probability table per point (the "physics update" of PAPER.md:220 evaluates
  * the oscillation probabilities for every parameter vector; here they arrive tabulated on the flux grid).
- *     w[p][i] = S_theta_p(T_i; P_e_pts[p]) / S_SM(T_i; nominal P_e)       (Eq. 12 / Eq. 14; the MC sample and the SM
- * reference stay those of the nominal table given to rw_create), P_mu, P_tau = (1 - P_e)(1 - f_tau), (1 - P_e) f_tau.
- * The spectrum is computed on the (E_nu x T) grid per point (these weights are not low-rank), then folded by the
- * dense path of rw_eval_weights.
+ *     w[p][i] = S_theta_p(T_i; P_e_pts[p]) / S_SM(T_i; nominal tables)       (Eq. 12 / Eq. 14; the MC sample and the SM
+ * reference stay those of the nominal tables given to rw_create, reading R16).  The rest 1 - P_e of a point goes
+ * to nu_mu and nu_tau by f_tau, or -- in a context created with explicit P_mu / P_tau -- in the nominal tables' mu : tau
+ * ratio at every energy (reading R17).  These weights are not low-rank; they are built per point from three suffix sums
+ * over the flux grid sorted by T_max (O(n_E + n_T) per point, rw_pee.cu) and folded by the dense path of rw_eval_weights.
  *   param, param_kind, P, k   as rw_eval_batch (DEVICE param; kinds RW_EPS_* and RW_MU_NU only)
- *   P_e_pts                   [P][n_E] device pointer, values in [0,1] (not validated)
+ *   P_e_pts                   [P][n_comp][n_E] device pointer ([P][n_E] for one component), values in [0,1] (not validated)
  *   out_m2lnL [P], out_mu NULL or [P][D][n_rec]   device pointers
  *   flags                     RW_FULL_EQ18, RW_MODE_AUTO/STREAM/RIDGE/GEMM, RW_SLICED / RW_SLICED_FAST (+ RW_SLICED_STRICT)
- * Needs a single-component context created without explicit P_mu / P_tau.  Asynchronous and stream-ordered. */
+ * Several components or explicit tables need n_E <= ~8500 (the scans live in shared memory).  Asynchronous, stream-ordered. */
 int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                 const double *P_e_pts, double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream);
 

@@ -303,7 +303,7 @@ class Reweighter:
             param = param[:, None]
         P, k = param.shape
         pts = P_e_pts.to(torch.float64).contiguous()
-        assert pts.shape == (P, self.n_E) and k == len(kinds)
+        assert pts.numel() == P * self.n_comp * self.n_E and k == len(kinds), "P_e_pts must be [P][n_comp][n_E]"
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, device=self.device) if want_mu else None

@@ -136,6 +136,13 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->KP512 = (int)((n_T + 511) / 512 * 512);
     L->tau8b = take(L->sliced ? D * (size_t)L->KP512 : 0);
     L->comp8p = take(L->sliced ? (size_t)L->KP512 : 0);
+    L->pee_scan = 3 * (n_E + 1) * 8 <= (size_t)200 << 10;
+    L->pee_perm = take(L->pee_scan ? n_E * 4 : 0);
+    L->pee_j0 = take(L->pee_scan ? n_T * 4 : 0);
+    L->pee_TmaxS = take(L->pee_scan ? n_E * 8 : 0);
+    L->pee_fS = take(L->pee_scan ? n_comp * 3 * n_E * 8 : 0);
+    L->pee_rho = take(L->pee_scan ? n_comp * 2 * n_E * 8 : 0);
+    L->pee_Y = take(L->pee_scan ? n_comp * 9 * (n_E + 1) * 8 : 0);
     L->gcol8 = take(L->sliced ? D * 2 * n_rec * 8 : 0);
     L->cert_part = take(L->sliced ? D * (size_t)L->NT8 * L->MC * 8 : 0);
     L->bound_stage = take(L->sliced ? (size_t)max_batch * 8 : 0);
@@ -432,6 +439,9 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->out_stage = (double *)(ws + L.out_stage);
     ctx->mu_tile = (double *)(ws + L.mu_tile);
     ctx->mu_prof = (double *)(ws + L.mu_prof);
+    ctx->pee_perm = (int *)(ws + L.pee_perm);      ctx->pee_j0 = (int *)(ws + L.pee_j0);
+    ctx->pee_TmaxS = (double *)(ws + L.pee_TmaxS); ctx->pee_fS = (double *)(ws + L.pee_fS);
+    ctx->pee_rho = (double *)(ws + L.pee_rho);     ctx->pee_Y = (double *)(ws + L.pee_Y);
     ctx->gcol8 = (double *)(ws + L.gcol8);
     ctx->cert_part = (double *)(ws + L.cert_part);
     ctx->bound_stage = (double *)(ws + L.bound_stage);
@@ -511,6 +521,11 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     }
     rc = make_tensor_maps(ctx);
     if (rc == RW_OK) rc = profile_setup(ctx);
+    if (rc == RW_OK) {
+        rc = pee_setup(ctx, s);
+        if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
+            rc = fail(nullptr, RW_ERR_CUDA, "rw_create: per-point P_ee tables failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     if (rc == RW_OK && L.sliced) {
         rc = i8_setup(ctx, s);
         if (rc == RW_OK && cudaStreamSynchronize(s) != cudaSuccess)
@@ -790,9 +805,9 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
     const uint32_t mode = flags & RW_MODE_MASK;
     if (mode == RW_MODE_COLLAPSED || (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32)))
         return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: collapsed mode, RW_FP32 and host buffers are not supported");
-    if (ctx->n_comp > 1 || ctx->have_mu_tau)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: needs a single component created without explicit P_mu/P_tau "
-                                             "(the point's 1 - P_e is split by f_tau)");
+    if ((ctx->n_comp > 1 || ctx->have_mu_tau) && !ctx->lay.pee_scan)
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_pee: several components / explicit P_mu, P_tau need the sorted-grid "
+                                             "path, i.e. a flux grid of at most ~8500 entries (n_E = %d)", ctx->n_E);
     int kinds[RW_N_KINDS], prec = 0;
     double tol = 0.0;
     { int rc = check_kinds(ctx, "rw_eval_pee", k, param_kind, kinds); if (rc != RW_OK) return rc; }
@@ -806,7 +821,7 @@ int rw_eval_pee(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const in
     for (int64_t q0 = 0; q0 < P; q0 += per_pass) {
         const int64_t Pq = (P - q0 < per_pass) ? P - q0 : per_pass;
         RW_CUDA(ctx, launch_coef(ctx, k > 0 ? param + q0 * k : nullptr, Pq, k, kinds, s));
-        RW_CUDA(ctx, launch_weights_pee(ctx, P_e_pts + (size_t)q0 * ctx->n_E, Pq, ctx->mu_prof, s));
+        RW_CUDA(ctx, launch_weights_pee(ctx, P_e_pts + (size_t)q0 * ctx->n_comp * ctx->n_E, Pq, ctx->mu_prof, s));
         int rc = weights_rows(ctx, ctx->mu_prof, Pq, mode, flags & RW_FULL_EQ18, out_m2lnL + q0,
                               out_mu ? out_mu + (size_t)q0 * ctx->D * ctx->n_rec : nullptr, s, prec, tol);
         if (rc != RW_OK) return rc;

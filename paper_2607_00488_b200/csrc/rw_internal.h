@@ -55,6 +55,8 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     size_t param_stage, coef, A_packed, partial, mu_part, out_stage, mu_stage, mu_tile, mu_prof;
     size_t B8, f_col8, e_row8, tau8, blk_hl8, blk_cm8, tau8b, comp8p;
     size_t gcol8, cert_part, bound_stage, fb_idx, coef_fb, rate_fb, out_fb;
+    size_t pee_perm, pee_j0, pee_TmaxS, pee_fS, pee_rho, pee_Y;
+    bool pee_scan;        // the sorted-grid suffix-sum tables of rw_eval_pee exist (3 (n_E + 1) doubles fit in shared memory)
     int KP512;            // n_T rounded up to 512 bins (staging chunk of k_slice_A)
     size_t total;
     int ldR;              // row pitch of the workspace copy of R (doubles)
@@ -112,6 +114,8 @@ struct rw_ctx {
     int *blk_cm8;             // [KT8] components present in each 32-bin block
     int8_t *tau8b;            // [D][KP512] tau as bytes, zero-padded (cp.async staging of k_slice_A)
     uint8_t *comp8p;          // [KP512] comp8, zero-padded
+    int *pee_perm, *pee_j0;   // flux grid sorted by T_max; first sorted entry that passes the cut, per recoil bin
+    double *pee_TmaxS, *pee_fS, *pee_rho, *pee_Y;   // sorted T_max; f E^-n [n_comp][3][n_E]; rho [n_comp][2][n_E]; totals [n_comp][9][n_E + 1]
     double *gcol8;            // [D][2: full, fast][n_rec] certificate constants g_k of the sliced contraction
     double *cert_part;        // [D][NT8][MC] certified relative error per (half tile, point)
     double *bound_stage;      // [max_batch] certified bound per point of a slice (strict mode without a caller array)
@@ -177,6 +181,7 @@ cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k,
                              cudaStream_t s);                                // rw_grad.cu
 cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,
                         double *grad, cudaStream_t s);                       // rw_grad.cu
+int pee_setup(rw_ctx *ctx, cudaStream_t s);                                  // rw_pee.cu
 int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
 cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s,
                            const double *w = nullptr, bool fast = false, bool certify = false);    // rw_fold_i8.cu

@@ -383,3 +383,29 @@ def test_per_point_survival_probability_with_a_single_evaluation_context(rw, orc
         torch.cuda.synchronize()
         _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
         ctx.close()
+
+
+@pytest.mark.parametrize("explicit", [False, True])
+def test_per_point_survival_probability_components_and_explicit_tables(rw, orc, explicit):
+    """rw_eval_pee with three signal components (their own flux / survival tables, P_e_pts[P][3][n_E]) and, when
+    `explicit`, nominal nu_mu / nu_tau tables whose mu : tau ratio every point keeps (reading R17); against
+    orc.eval_pee_components.  The flux grid is NOT sorted (a line is appended last): the sorted-grid scan must not care."""
+    import torch
+    inp = wl.make_components(n_comp=3, n_E=150, n_T=240, n_rec=130, n_periods=2, seed=121)
+    rng = np.random.default_rng(122)
+    if explicit:
+        frac = rng.uniform(0.2, 0.8, size=inp["P_e"].shape)
+        inp["P_mu"] = (1.0 - inp["P_e"]) * frac
+        inp["P_tau"] = (1.0 - inp["P_e"]) * (1.0 - frac)
+    P = 37
+    params, kinds = wl.random_points(P, [wl.EPS_EE_L, wl.EPS_MM_R, wl.EPS_TT_L, wl.MU_NU], seed=123)
+    pts = np.clip(inp["P_e"][None] + rng.uniform(-0.25, 0.25, size=(P, 3, 150)), 0.0, 1.0)
+    pts[0] = inp["P_e"]
+    ref, mu_ref, scale = orc.eval_pee_components(inp, params, kinds, pts, want_mu=True, want_abs=True, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=64)
+    out, mu = ctx.eval_pee(_cuda(params), kinds, _cuda(pts), want_mu=True)
+    plain = ctx.eval_batch(_cuda(params[:1]), kinds)
+    torch.cuda.synchronize()
+    _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    assert abs(plain.item() - out[0].item()) <= 1e-9 + 1e-11 * abs(plain.item())     # nominal tables = ordinary path
+    ctx.close()
