@@ -148,7 +148,7 @@ typedef struct {
                                With n_comp > 1, flux_w, P_e (and P_mu, P_tau) are [n_comp][n_E] tables on the shared
                                E grid, and the recoil bins of all components are concatenated along n_T. */
     const int32_t *comp_of_T; /* [n_T] component of every recoil bin (same memory kind as the other arrays);
-                               ignored (may be NULL) when n_comp <= 1.  RW_MODE_COLLAPSED needs n_comp <= 1. */
+                               ignored (may be NULL) when n_comp <= 1. */
 } rw_inputs;
 
 /* Bytes of device workspace rw_create needs for these inputs and batches of up to max_batch points.
@@ -192,8 +192,8 @@ int64_t rw_strict_fallback_count(const rw_ctx *ctx);
 
 /* RW_MODE_COLLAPSED (rw_eval_batch only).  Eq. (4) is quadratic in the couplings, Eq. (8)
  * linear in mu_nu^2 and the fold of Eq. (11) linear in the spectrum, so
- *   mu[p][d][k] - bkg[d][k] = sum_b c_b(theta_p) G[d][b][k],   G[d][b][k] = sum_i W^[d][b][i] R[d][i][k]
- * exactly (up to rounding order).  rw_create folds the 11 templates G once; this mode then evaluates a point
+ *   mu[p][d][k] - bkg[d][k] = sum_q rate_q sum_b c_b(theta_p) G[d][q][b][k],   G[d][q][b][k] = sum_{i in component q} W^[d][b][i] R[d][i][k]
+ * exactly (up to rounding order).  rw_create folds the 11 templates G of every component once; this mode then evaluates a point
  * in O(11 n_rec D) instead of O(n_T n_rec D).  It is NOT what RW_MODE_AUTO/STREAM/GEMM run (those execute the
  * full fold for every point, which is the only valid path once weights are not low-rank -- rw_eval_weights).
  *
@@ -256,7 +256,7 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
  *   RW_TABLE_S_SM   [n_T]        SM recoil spectrum S_SM(T_i) (Eq. 12 at theta = 0)
  *   RW_TABLE_BASIS  [10][n_T]    basis spectra A_e,B_e,C_e,A_mu,...,C_tau,D
  *   RW_TABLE_WHAT   [D][12][n_T] pre-scaled basis W^ = basis * N_mc / S_SM (+ dead-bin row)
- *   RW_TABLE_G      [D][12][ldG] prefolded templates G (ldG = n_rec rounded up to even; rows 11 unused) */
+ *   RW_TABLE_G      [D][n_comp][12][ldG] prefolded templates G (ldG = n_rec rounded up to even; rows 11 unused) */
 enum { RW_TABLE_S_SM = 0, RW_TABLE_BASIS = 1, RW_TABLE_WHAT = 2, RW_TABLE_G = 3 };
 int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64_t *n_elems);
 

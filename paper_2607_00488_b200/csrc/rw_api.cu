@@ -94,10 +94,10 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->sat_const = take(8);
     L->flag = take(4);
     L->ldG = (int)mu_ld;
-    L->G = take(D * kCoefStride * mu_ld * 8);
+    L->G = take(D * n_comp * kCoefStride * mu_ld * 8);              // templates [D][n_comp][12][ldG]
     L->stream_cnt = take((D * (size_t)L->stream_strips + 1) * 4);
     L->strip_part = take(D * (size_t)L->stream_strips * kStreamMaxPB * 8);
-    L->ident = take(kStreamMaxPB * kCoefStride * 8);
+    L->ident = take(kStreamMaxPB * (kCoefStride + RW_MAX_COMPONENTS) * 8);     // unit coefficient rows + one rate row set
     L->param_stage = take((size_t)max_batch * RW_N_KINDS * 8);
     L->coef = take((size_t)max_batch * kCoefStride * 8);
     L->A_packed = take((size_t)(L->MC / 8) * L->A_pitch * 8);
@@ -577,8 +577,6 @@ static int eval_batch_impl(rw_ctx *ctx, const double *param, int64_t P, int32_t 
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
     if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
-    if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: RW_MODE_COLLAPSED needs a single signal component");
     int prec = 0;
     double tol = 0.0;
     { int rc = pick_prec(ctx, "rw_eval_batch", flags, true, &prec, &tol); if (rc != RW_OK) return rc; }
@@ -659,8 +657,6 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
 {
     if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_profile: ctx is NULL");
     if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: P < 0 or k outside [0,11]");
-    if ((flags & RW_MODE_MASK) == RW_MODE_COLLAPSED && ctx->n_comp > 1)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_profile: RW_MODE_COLLAPSED needs a single signal component");
     if (P == 0) return RW_OK;
     if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
         return fail(ctx, RW_ERR_INVALID, "rw_eval_profile: param, param_kind or out_m2lnL is NULL");
@@ -703,8 +699,6 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
     int kinds[RW_N_KINDS];
     { int rc = check_kinds(ctx, "rw_eval_grad", k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
-    if (mode == RW_MODE_COLLAPSED && ctx->n_comp > 1)
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: RW_MODE_COLLAPSED needs a single signal component");
     const bool full = flags & RW_FULL_EQ18;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -836,7 +830,7 @@ int rw_get_table(const rw_ctx *ctx, int32_t which, const double **dev_ptr, int64
     case RW_TABLE_S_SM: *dev_ptr = ctx->S_sm; *n_elems = ctx->n_T; return RW_OK;
     case RW_TABLE_BASIS: *dev_ptr = ctx->basis; *n_elems = (int64_t)kNumBasis * ctx->n_T; return RW_OK;
     case RW_TABLE_WHAT: *dev_ptr = ctx->What; *n_elems = (int64_t)ctx->D * kCoefStride * ctx->n_T; return RW_OK;
-    case RW_TABLE_G: *dev_ptr = ctx->G; *n_elems = (int64_t)ctx->D * kCoefStride * ctx->lay.ldG; return RW_OK;
+    case RW_TABLE_G: *dev_ptr = ctx->G; *n_elems = (int64_t)ctx->D * ctx->n_comp * kCoefStride * ctx->lay.ldG; return RW_OK;
     default: return RW_ERR_INVALID;
     }
 }

@@ -221,12 +221,12 @@ static void launch_stream_t(const StreamArgs &A, const Kinds &kd, const Consts &
 
 cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
                                const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
-                               cudaStream_t s)
+                               cudaStream_t s, const double *rate_rows)
 {
     // `coef` is ctx->coef + 12 g0 for the group starting at point g0 (or the identity of the prefold, which is
     // never run with several components): its rates are ctx->rate + 4 g0
-    const double *rate = nullptr;
-    if (coef && ctx->comp8 && coef >= ctx->coef && coef < ctx->coef + (size_t)ctx->lay.max_batch * kCoefStride)
+    const double *rate = rate_rows;
+    if (!rate && coef && ctx->comp8 && coef >= ctx->coef && coef < ctx->coef + (size_t)ctx->lay.max_batch * kCoefStride)
         rate = ctx->rate + (coef - ctx->coef) / kCoefStride * RW_MAX_COMPONENTS;
     const Layout &L = ctx->lay;
     StreamArgs A;

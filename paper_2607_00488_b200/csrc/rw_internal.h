@@ -164,7 +164,7 @@ cudaError_t launch_fold_gemm(rw_ctx *ctx, int d, int64_t Pc, double *out_mu, int
 // `param` (+ kinds; step a1 then runs inside the kernel) or caller weights `wts`.  out == NULL: fold only (prefold).
 cudaError_t launch_fold_stream(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
                                const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,
-                               cudaStream_t s);                              // rw_fold_stream.cu
+                               cudaStream_t s, const double *rate_rows = nullptr);   // rw_fold_stream.cu
 // The same contract for Pb <= 64 points on the streaming DMMA kernel (rw_fold_ridge.cu); out must not be NULL.
 cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *param, const Kinds *kd,
                               const double *wts, int Pb, double *out, bool full_eq18, double *out_mu,

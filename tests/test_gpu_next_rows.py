@@ -78,7 +78,7 @@ def test_collapsed_templates_are_the_fold_of_the_prescaled_basis(rw):
     ctx = rw.Reweighter(inp, max_batch=4)
     D, n_T, n_rec = inp["R"].shape
     What = ctx.table(rw.RW_TABLE_WHAT).reshape(D, 12, n_T)
-    G = ctx.table(rw.RW_TABLE_G).reshape(D, 12, -1)
+    G = ctx.table(rw.RW_TABLE_G).reshape(D, 12, -1)              # one component: [D][1][12][ldG]
     R = _cuda(inp["R"])
     for d in range(D):
         ref = What[d, :11] @ R[d]
@@ -252,8 +252,10 @@ def test_multi_component_rates(rw, orc, mode, P):
     out, mu = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode=mode)
     torch.cuda.synchronize()
     _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
-    with pytest.raises(rw.RwError):
-        ctx.eval_batch(_cuda(params), kinds, mode="collapsed")
+    # the rank-K identity holds per component (11 n_comp templates, the rates applied to the template sums)
+    out_c, mu_c = ctx.eval_batch(_cuda(params), kinds, want_mu=True, mode="collapsed")
+    torch.cuda.synchronize()
+    _assert_parity(out_c.cpu().numpy(), mu_c.cpu().numpy(), ref, mu_ref, scale)
     with pytest.raises(rw.RwError):
         ctx.eval_batch(_cuda(params[:, :1]), [10])               # rate of a component that does not exist
     ctx.close()
@@ -317,6 +319,7 @@ def test_gradient_multi_component_and_asimov_zero(rw, orc):
     kinds = np.array([0, 2, 3, 6, 7, 8, 9], np.int32)
     params, _ = wl.random_points(40, kinds, seed=94)
     _grad_check(rw, orc, inp, params, kinds, "auto", max_batch=300)
+    _grad_check(rw, orc, inp, params, kinds, "collapsed", max_batch=300)      # per-component templates, rate derivatives
     _, mu = orc.eval_components(inp, params[:1], kinds, want_mu=True)
     asim = dict(inp, counts=mu[0])
     ctx = rw.Reweighter(asim, max_batch=16)
