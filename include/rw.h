@@ -92,8 +92,8 @@ enum {
                                   rw_eval_certified returns, and RW_SLICED_STRICT enforces 1e-12.
                                   Needs RW_CREATE_SLICED; non-negative finite N' (else NaN for that point, or the FP64 result
                                   under RW_SLICED_STRICT).  Accepted by rw_eval_batch, rw_eval_certified, rw_eval_profile,
-                                  rw_eval_weights and rw_eval_pee (dense fold only; the streaming, ridge and collapsed regimes
-                                  ignore it); rw_eval_grad refuses it. */
+                                  rw_eval_weights, rw_eval_pee and rw_eval_grad (dense fold only; the streaming, ridge and
+                                  collapsed regimes ignore it). */
     RW_SLICED_FAST = 1u << 12, /* opt-in reduced precision on the same slices: only their top four (31-bit fixed point) and
                                   the four leading diagonals, 10 INT8 products per 32 recoil bins.  Error
                                   ~1e-9 (row max)(column max) n_T per bin: mu within 1e-5 relative wherever RW_SLICED
@@ -246,9 +246,12 @@ int rw_eval_profile(rw_ctx *ctx, const double *param, int64_t P, int32_t k, cons
  * (the paper minimises Eq. 18 with MIGRAD).  The path is linear in the coefficient vector of
  * Eq. (4)/(8) and in the rates of Eq. (17), so d mu / d theta_m is the same fold applied to derivative coefficients;
  *     out_grad[p][m] = sum over bins and periods of 2 (1 - n/mu) d mu / d theta_m      (n = 0: 2 d mu / d theta_m).
- * A point costs 1 + k rows of the batched fold.  DEVICE pointers only; flags: RW_FULL_EQ18 (value only) and the
- * fold modes (RW_FP32, RW_SLICED, RW_SLICED_FAST: RW_ERR_UNSUPPORTED, derivative rows change sign); max_batch must be
- * >= 1 + k.  Asynchronous and stream-ordered; P may exceed max_batch. */
+ * A point costs 1 + k rows of the batched fold.  DEVICE pointers only; flags: RW_FULL_EQ18 (value only), the fold
+ * modes, and RW_SLICED / RW_SLICED_FAST: a derivative row changes sign along the recoil bins and the sliced contraction
+ * wants non-negative rows, so there it is folded as its positive and its negative part (1 + 2k rows per point) and the
+ * two folds are subtracted; each part carries the contraction's error relative to its own size.  RW_SLICED_STRICT and
+ * RW_FP32: RW_ERR_UNSUPPORTED (a difference of two folds has no per-point certificate).  max_batch must be >= 1 + k
+ * (1 + 2k with the sliced flags).  Asynchronous and stream-ordered; P may exceed max_batch. */
 int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                  double *out_m2lnL, double *out_grad /*[P][k]*/, uint32_t flags, void *cuda_stream);
 

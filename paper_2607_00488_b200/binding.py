@@ -315,8 +315,9 @@ class Reweighter:
         self._last_param = (param, pts)
         return (out, mu) if want_mu else out
 
-    def eval_grad(self, param, kinds, full_eq18=False, mode="auto"):
-        """(-2lnL[P], gradient[P][k]) for CUDA param[P][k] (rw_eval_grad)."""
+    def eval_grad(self, param, kinds, full_eq18=False, mode="auto", sliced=False):
+        """(-2lnL[P], gradient[P][k]) for CUDA param[P][k] (rw_eval_grad).  sliced = True | "fast": the rows go through
+        the INT8 contraction, every derivative row as its positive and its negative part."""
         if not (isinstance(param, torch.Tensor) and param.is_cuda):
             raise RwError(-4, "eval_grad needs a CUDA tensor param[P][k]")
         param = param.to(torch.float64).contiguous()
@@ -327,7 +328,7 @@ class Reweighter:
         kinds_arr = (C.c_int32 * max(1, len(kinds)))(*[int(x) for x in kinds])
         out = torch.empty(P, dtype=torch.float64, device=self.device)
         grad = torch.empty((P, k), dtype=torch.float64, device=self.device)
-        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0)
+        flags = _MODES[mode] | (RW_FULL_EQ18 if full_eq18 else 0) | _sliced_flag(sliced)
         rc = self._L.rw_eval_grad(self._ctx, C.c_void_p(param.data_ptr()), P, k, kinds_arr,
                                   C.c_void_p(out.data_ptr()), C.c_void_p(grad.data_ptr()), flags, _stream_ptr())
         self._check(rc, self._ctx)

@@ -693,26 +693,36 @@ int rw_eval_grad(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const i
     if (P == 0) return RW_OK;
     if (!out_m2lnL || !out_grad || !param || !param_kind)
         return fail(ctx, RW_ERR_INVALID, "rw_eval_grad: param, param_kind, out_m2lnL or out_grad is NULL");
-    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32 | RW_SLICED | RW_SLICED_FAST))
-        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers, RW_FP32 and RW_SLICED are not supported "
-                                             "(derivative rows change sign)");
+    if (flags & (RW_PARAM_HOST | RW_OUT_HOST | RW_FP32 | RW_SLICED_STRICT))
+        return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_grad: host buffers, RW_FP32 and RW_SLICED_STRICT are not supported "
+                                             "(a derivative row has no certificate: it is a difference of two folds)");
     int kinds[RW_N_KINDS];
     { int rc = check_kinds(ctx, "rw_eval_grad", k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
+    int prec = 0;
+    double tol = 0.0;
+    { int rc = pick_prec(ctx, "rw_eval_grad", flags, false, &prec, &tol); if (rc != RW_OK) return rc; }
     const bool full = flags & RW_FULL_EQ18;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
-    // a point is 1 + k rows of the ordinary fold (value row + one derivative row per parameter)
-    int64_t per_pass = L.prof_rows / (1 + k);
+    // a point is 1 + k rows of the ordinary fold (value row + one derivative row per parameter); where the rows go
+    // through the sliced contraction every derivative row goes as its positive and its negative part: 1 + 2 k rows
+    const int max_rows_per_point = 1 + ((prec >= 2 && mode != RW_MODE_COLLAPSED) ? 2 : 1) * k;
+    const int64_t per_pass = L.prof_rows / max_rows_per_point;
     if (per_pass < 1)
-        return fail(ctx, RW_ERR_WORKSPACE, "rw_eval_grad: max_batch (%lld) is smaller than 1 + k = %d rows",
-                    (long long)L.max_batch, 1 + k);
+        return fail(ctx, RW_ERR_WORKSPACE, "rw_eval_grad: max_batch (%lld) is smaller than %d rows per point",
+                    (long long)L.max_batch, max_rows_per_point);
     for (int64_t q0 = 0; q0 < P; q0 += per_pass) {
         const int64_t Pq = (P - q0 < per_pass) ? P - q0 : per_pass;
-        RW_CUDA(ctx, launch_coef_grad(ctx, param + q0 * k, Pq, k, kinds, s));
-        int rc = fold_slice(ctx, Pq * (1 + k), mode, false, ctx->out_stage, ctx->mu_prof, s);
+        // a pass small enough for the streaming kernels is folded in FP64 by fold_slice whatever the flags: no split
+        const int64_t plain_rows = Pq * (1 + k);
+        const bool split = max_rows_per_point > 1 + k && !use_stream(ctx, mode, plain_rows, prec) &&
+                           !use_ridge(ctx, mode, plain_rows, prec);
+        const int64_t rows = split ? Pq * max_rows_per_point : plain_rows;
+        RW_CUDA(ctx, launch_coef_grad(ctx, param + q0 * k, Pq, k, kinds, s, split));
+        int rc = fold_slice(ctx, rows, mode, false, ctx->out_stage, ctx->mu_prof, s, split ? prec : 0);
         if (rc != RW_OK) return rc;
-        RW_CUDA(ctx, launch_grad(ctx, ctx->mu_prof, Pq, k, full, out_m2lnL + q0, out_grad + q0 * k, s));
+        RW_CUDA(ctx, launch_grad(ctx, ctx->mu_prof, Pq, k, full, out_m2lnL + q0, out_grad + q0 * k, s, split));
     }
     return RW_OK;
 }

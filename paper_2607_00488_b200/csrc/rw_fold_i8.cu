@@ -203,6 +203,8 @@ k_slice_A(const double *__restrict__ coef, const double *__restrict__ rate, cons
 #pragma unroll
                     for (int b = 0; b < kNumTerms; ++b) acc = fma(sC[(r0 + u) * kCoefStride + b], wv[b], acc);
                     v[u] = acc * sRate[(r0 + u) * RW_MAX_COMPONENTS + cmp] * scl;       // N' / 2^tau_i
+                    // derivative rows of rw_eval_grad (slot 11 = 1): the positive part of the row, negatives -> 0
+                    if (sC[(r0 + u) * kCoefStride + kCoefStride - 1] != 0.0) v[u] = fmax(v[u], 0.0);
                 }
             } else {
                 const double nm = sW[0][sj] * scl;

@@ -178,9 +178,9 @@ cudaError_t launch_profile(rw_ctx *ctx, const double *mu_rows, int64_t rows, dou
 int profile_setup(rw_ctx *ctx);                                              // rw_profile.cu
 cudaError_t launch_weights_pee(rw_ctx *ctx, const double *P_e_pts, int64_t Pq, double *w, cudaStream_t s);  // rw_pee.cu
 cudaError_t launch_coef_grad(rw_ctx *ctx, const double *param, int64_t P, int k, const int *kinds,
-                             cudaStream_t s);                                // rw_grad.cu
+                             cudaStream_t s, bool split = false);            // rw_grad.cu
 cudaError_t launch_grad(rw_ctx *ctx, const double *rows, int64_t P, int k, bool full_eq18, double *out,
-                        double *grad, cudaStream_t s);                       // rw_grad.cu
+                        double *grad, cudaStream_t s, bool split = false);   // rw_grad.cu
 int pee_setup(rw_ctx *ctx, cudaStream_t s);                                  // rw_pee.cu
 int i8_setup(rw_ctx *ctx, cudaStream_t s);                                   // rw_fold_i8.cu
 cudaError_t launch_fold_i8(rw_ctx *ctx, int d, int64_t p0, int64_t Pc, double *out_mu, cudaStream_t s,

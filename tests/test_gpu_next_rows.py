@@ -330,6 +330,36 @@ def test_gradient_multi_component_and_asimov_zero(rw, orc):
     ctx.close()
 
 
+def test_gradient_through_the_sliced_contraction(rw, orc):
+    """RW_SLICED on rw_eval_grad: a derivative row changes sign along the recoil bins, so it is folded as its positive
+    and its negative part (1 + 2k rows per point) and k_grad takes the difference.  n_T = 2300 > 2048: seven slices;
+    several passes of the row scratch; a last pass small enough for the FP64 streaming kernels (no split there)."""
+    import torch
+    inp = wl.make_custom(n_E=31, n_T=2300, n_rec=140, n_periods=2, seed=95, dead_fraction=0.1)
+    kinds = np.array([0, 1, 2, 5, 6, 7], np.int32)
+    params, _ = wl.random_points(43, kinds, seed=96)
+    ref, gref = orc.eval_grad(inp, params, kinds, nthreads=CORES)
+    ctx = rw.Reweighter(inp, max_batch=14 * 13, sliced=True)        # 14 points per pass (1 + 2*6 rows each); 43 = 3*14 + 1
+    floor = 1e-11 * np.asarray(inp["bkg"]).sum()
+    for sliced, rel in ((True, 1e-11), ("fast", 1e-5)):
+        out, grad = ctx.eval_grad(_cuda(params), kinds, mode="auto", sliced=sliced)
+        out_g, grad_g = ctx.eval_grad(_cuda(params), kinds, mode="gemm", sliced=sliced)
+        torch.cuda.synchronize()
+        for o, g in ((out, grad), (out_g, grad_g)):
+            o, g = o.cpu().numpy(), g.cpu().numpy()
+            tol_v = 1e-9 + 1e-11 * np.abs(ref) if sliced is True else 1e-4 * np.abs(ref) + 1.0
+            assert np.all(np.abs(o - ref) <= tol_v), np.abs(o - ref).max()
+            # each part carries the relative error of the contraction on ITS size; the gradient is their difference
+            # summed over bins with weights 2 (1 - n/mu): compare on the scale of the whole gradient vector's row
+            scale = np.abs(gref) + np.abs(gref).max(axis=1, keepdims=True) * 1e-3
+            err = np.abs(g - gref) / scale
+            print("grad sliced=%s: max rel err %.2e" % (sliced, err.max()))
+            assert np.all(np.abs(g - gref) <= rel * scale + floor), err.max()
+    with pytest.raises(rw.RwError, match="RW_SLICED_STRICT"):
+        ctx.eval_grad(_cuda(params), kinds, sliced="strict")
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------- f-3 per-point survival probabilities
 @pytest.mark.parametrize("mode,P", [("stream", 3), ("gemm", 45), ("auto", 150)])
 def test_per_point_survival_probability(rw, orc, mode, P):
