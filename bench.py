@@ -484,15 +484,14 @@ def main():
 
     gathered = None
     if strong:
-        shard_max = -(-P_job // world)
+        shard_max = sharding.shard_pad(P_job, world)
         pad = torch.zeros(shard_max, dtype=torch.float64, device=dev)
         gathered = torch.empty(world * shard_max, dtype=torch.float64, device=dev)
 
     def step_dev():
         ctx.eval_batch(param_dev, kinds, out=out_dev)
         if strong:                            # the caller wants the whole scan: gather the slices (8 P_job bytes)
-            pad[:P].copy_(out_dev)
-            dist.all_gather_into_tensor(gathered, pad)
+            sharding.gather_shards(out_dev, pad, gathered, P_job, world)
 
     def step_host():
         ctx.eval_batch(param_pin, kinds, out=out_pin)

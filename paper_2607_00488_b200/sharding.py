@@ -24,6 +24,29 @@ def shard_range(P, rank, world):
     return lo, lo + base + (1 if rank < rem else 0)
 
 
+def shard_pad(P, world):
+    """Length every rank's slice is padded to for the gather (the largest shard)."""
+    return -(-int(P) // int(world))
+
+
+def gather_shards(out_local, pad, gathered, P, world):
+    """Strong scaling's only exchange, 8 P bytes per scan: every rank's out[lo:hi) -> the whole scan's out[P] on every
+    rank.  `pad` [shard_pad] and `gathered` [world * shard_pad] are caller-owned buffers on out_local's device (no
+    allocation per step); returns a tensor of P values in scan order (a fresh one unless the shards are equal-sized,
+    where it is a view of `gathered`)."""
+    import torch
+    import torch.distributed as dist
+    n = out_local.numel()
+    pad[:n].copy_(out_local)
+    dist.all_gather_into_tensor(gathered, pad) if gathered.is_cuda else dist.all_gather(
+        list(gathered.view(world, -1).unbind(0)), pad)
+    sp = pad.numel()
+    if P == world * sp:
+        return gathered
+    return torch.cat([gathered[r * sp: r * sp + (shard_range(P, r, world)[1] - shard_range(P, r, world)[0])]
+                      for r in range(world)])
+
+
 def max_over_ranks(x, device, world):
     """max of a python float over all ranks (device-timed durations are combined this way)."""
     if world == 1:

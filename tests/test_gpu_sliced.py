@@ -141,16 +141,10 @@ def test_sliced_weights_profile_and_pee(orc):
     torch.cuda.synchronize()
     out = out.cpu().numpy()
     assert np.isnan(out[4]) and np.all(np.isfinite(np.delete(out, 4)))
-    with pytest.raises(binding.RwError):
-        flags = binding.RW_SLICED
-        import ctypes as C
-        p = _cuda(params)
-        o = torch.empty(45, dtype=torch.float64, device="cuda")
-        g = torch.empty((45, 4), dtype=torch.float64, device="cuda")
-        ka = (C.c_int32 * 4)(*[int(x) for x in kinds])
-        rc = ctx._L.rw_eval_grad(ctx._ctx, C.c_void_p(p.data_ptr()), 45, 4, ka, C.c_void_p(o.data_ptr()),
-                                 C.c_void_p(g.data_ptr()), flags, None)
-        ctx._check(rc, ctx._ctx)
+    # the gradient accepts the sliced contraction (tests/test_gpu_next_rows.py) but not its strict form or RW_FP32
+    for bad in ("strict", "fast-strict"):
+        with pytest.raises(binding.RwError, match="RW_SLICED_STRICT"):
+            ctx.eval_grad(_cuda(params), kinds, sliced=bad)
     ctx.close()
 
 

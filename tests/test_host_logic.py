@@ -158,6 +158,23 @@ ms = sharding.max_over_ranks(10.0 + 5.0 * rank, "cpu", world)
 assert ms == 15.0, ms
 v = sharding.whole_job_value(world, 121, 4, ms)
 assert abs(v - 2 * 121 * 4 / 0.015) < 1e-9
+# strong scaling: one scan split into contiguous shards (61 + 60 points), every rank evaluates its own (here with the CPU
+# oracle -- there is no GPU on this box), the shards are gathered into out[P] in scan order on every rank
+import numpy as np
+from oracle import rw_oracle as orc
+from paper_2607_00488_b200 import workloads as wl
+orc.build()
+inp = wl.make("cfg1_tiny_nsi")
+params, kinds = wl.scan_points("cfg1_tiny_nsi")
+P = params.shape[0]
+lo, hi = sharding.shard_range(P, rank, world)
+assert (lo, hi) == ((0, 61) if rank == 0 else (61, 121))
+mine = torch.from_numpy(np.asarray(orc.eval_batch(inp, params[lo:hi], kinds)))
+pad = torch.zeros(sharding.shard_pad(P, world), dtype=torch.float64)
+gathered = torch.empty(world * pad.numel(), dtype=torch.float64)
+whole = sharding.gather_shards(mine, pad, gathered, P, world)
+ref = torch.from_numpy(np.asarray(orc.eval_batch(inp, params, kinds)))
+assert whole.shape == (P,) and torch.equal(whole, ref), (whole - ref).abs().max()
 dist.barrier()
 dist.destroy_process_group()
 sys.stdout.write("rank" + str(rank) + "-ok\n")
