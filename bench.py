@@ -38,8 +38,12 @@ L2_BYTES = 126e6
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from committed `ncu --set full` captures (NOT measured in
 # this run: bench.py cannot run under ncu).  kernel -> (bytes per launch, file under profiles/)
 NCU_TRAFFIC = {
-    "k_fold_gemm<8>": (69.584991e9 + 0.032040e9, "profiles/r01c_fold_gemm_full.md"),
-    "k_fold_stream<1>": (1.075726e9 + 0.0112768e9, "profiles/r01e_fold_stream_full.md"),
+    "k_fold_gemm<8>": (64.519372e9 + 0.033138e9, "profiles/r02_folds.md"),
+    "k_fold_gemm<4>": (1.120025e9 + 0.032784e9, "profiles/r02_folds.md"),
+    "k_fold_stream<1>": (1.075720e9 + 0.011437e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<1>": (1.075512e9 + 0.007054e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<2>": (1.075595e9 + 0.008221e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<4>": (1.075435e9 + 0.005559e9, "profiles/r02_folds.md"),
 }
 
 
@@ -313,11 +317,15 @@ def ridge_regimes(torch, ctx, timer, param_dev, kinds, dev, inp, peaks, dmma_pea
         hbm_ms = r_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
         ten_ms = fold_flops(inp, Pb) / (dmma_peak * 1e12) * 1e3
         bound_ms = max(hbm_ms, ten_ms)
-        res.append({"regime": "ridge", "points": Pb, "kernel": policy_kernel(Pb),
-                    "bound": "hbm" if hbm_ms >= ten_ms else "tensor", "bound_ms": bound_ms, "ms_per_call": ms,
-                    "fold_kernel_ms": k_ms, "frac": bound_ms / ms, "kernel_frac": bound_ms / k_ms if k_ms > 0 else None,
-                    "evals_per_s": Pb / ms * 1e3, "fold_tflops": fold_flops(inp, Pb) / ms / 1e9,
-                    "response_gbs": r_bytes / ms / 1e6})
+        blk = {"regime": "ridge", "points": Pb, "kernel": policy_kernel(Pb),
+               "bound": "hbm" if hbm_ms >= ten_ms else "tensor", "bound_ms": bound_ms, "ms_per_call": ms,
+               "fold_kernel_ms": k_ms, "frac": bound_ms / ms, "kernel_frac": bound_ms / k_ms if k_ms > 0 else None,
+               "evals_per_s": Pb / ms * 1e3, "fold_tflops": fold_flops(inp, Pb) / ms / 1e9,
+               "response_gbs": r_bytes / ms / 1e6}
+        tr = NCU_TRAFFIC.get(blk["kernel"])
+        if tr and r_bytes == 1073741824:
+            blk["traffic"], blk["traffic_source"] = tr[0], tr[1] + " (ncu capture, not measured in this run)"
+        res.append(blk)
     return res
 
 
@@ -393,6 +401,39 @@ def bench_config(name, dev, steps, warmup, peaks, dmma_peak, cores, quick):
     return res
 
 
+def kernel_tour(torch, ctx, param_dev, kinds, inp, dev, max_batch):
+    """Two calls (the first warms caches, clocks and lazily loaded modules) of every regime and entry point on the
+    context the bench times: the launches an `ncu --set full -k regex:...` capture picks from.  Nothing is timed."""
+    P, k = param_dev.shape
+    calls = []
+
+    def twice(label, fn):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        calls.append(label)
+
+    for Pb in (1, 2, 8, 16, 32, 64):
+        pb = param_dev[:Pb].contiguous()
+        twice("rw_eval_batch P=%d auto -> %s" % (Pb, policy_kernel(Pb)), lambda: ctx.eval_batch(pb, kinds))
+    twice("rw_eval_batch P=%d auto -> %s" % (P, policy_kernel(min(P, max_batch))), lambda: ctx.eval_batch(param_dev, kinds))
+    twice("rw_eval_batch P=%d RW_SLICED -> k_slice_A + k_fold_i8" % P, lambda: ctx.eval_batch(param_dev, kinds, sliced=True))
+    twice("rw_eval_batch P=%d RW_SLICED_FAST" % P, lambda: ctx.eval_batch(param_dev, kinds, sliced="fast"))
+    twice("rw_eval_batch P=%d RW_MODE_COLLAPSED -> k_collapsed" % P, lambda: ctx.eval_batch(param_dev, kinds, mode="collapsed"))
+    Pp = int(min(P, max_batch, 4096))
+    pp = param_dev[:Pp].contiguous()
+    twice("rw_eval_profile P=%d -> fold + k_profile" % Pp, lambda: ctx.eval_profile(pp, kinds, s0=1.0, sigma=0.05))
+    Pg = int(min(P, max(1, min(max_batch, 4096) // (1 + k))))
+    pg = param_dev[:Pg].contiguous()
+    twice("rw_eval_grad P=%d -> k_coef_grad + fold + k_grad" % Pg, lambda: ctx.eval_grad(pg, kinds))
+    if all(int(x) < 7 for x in kinds):
+        Pe = int(min(P, max_batch, 1024))
+        pe = param_dev[:Pe].contiguous()
+        tab = torch.from_numpy(np.ascontiguousarray(inp["P_e"])).to(dev)[None, :].repeat(Pe, 1).contiguous()
+        twice("rw_eval_pee P=%d n_E=%d -> k_pee_scan + fold" % (Pe, tab.shape[1]), lambda: ctx.eval_pee(pe, kinds, tab))
+    return calls
+
+
 def self_launch(args):
     """Started as a plain process with --gpus N > 1: re-execute under torch.distributed.run, one rank per GPU."""
     port = 29500 + (os.getpid() % 2000)
@@ -412,6 +453,9 @@ def main():
     ap.add_argument("--config", default="cfg4_dense")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tour", action="store_true",
+                    help="no timing: two calls of every entry point / regime on the bench context, for `ncu -k ...` captures "
+                         "(profiles/*.md name the command); prints the list of calls")
     ap.add_argument("--quick", action="store_true", help="headline, e2e and rooflines only: no context legs, no other configs")
     ap.add_argument("--max-batch", type=int, default=0,
                     help="points per library slice (default: the whole scan; 16384 for cfg5_joint6, as BASELINE.json says)")
@@ -469,6 +513,12 @@ def main():
     out_pin = torch.empty(P, dtype=torch.float64).pin_memory()
     peaks = load_peaks()
     r_bytes = D * n_T * n_rec * 8
+    if args.tour:
+        assert world == 1, "--tour is a single-GPU profiling aid"
+        calls = kernel_tour(torch, ctx, param_dev, kinds, inp, dev, max_batch)
+        print(json.dumps({"tour": calls, "config": name, "launches": int(ctx.launch_count())}))
+        ctx.close()
+        return
 
     def barrier():
         torch.cuda.synchronize()
