@@ -126,7 +126,7 @@ struct RidgeSplit {
     __device__ __forceinline__ long long u0(int j) const { return (long long)j * U / G; }
     __device__ __forceinline__ int cta_of(long long u) const { return (int)(((u + 1) * G - 1) / U); }
     // slot of CTA j's partial tile of `tile`: 3 j + {0: the tile its span starts in, 2: the tile it ends in, 1: a
-    // whole tile in between (private, reused)}
+    // whole tile in between (private, reused)}.  Four 64-bit divisions: never inside a loop over contributors.
     __device__ __forceinline__ int slot_of(int j, int tile) const
     {
         const long long a = u0(j), b = u0(j + 1) - 1;
@@ -153,6 +153,7 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     const uint32_t full_bar = rg_smem_u32(red + kRgWarps * PP);        // ring: NS full, NS empty
     const uint32_t empty_bar = full_bar + NS * 8;
     __shared__ int s_flag;
+    __shared__ int s_slot[2 * kRidgePlanSMs + 8];                       // slots of the contributors of the tile being finished
 
     const int n_T = A.n_T, n_rec = A.n_rec, Pb = A.Pb;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -160,6 +161,7 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     RidgeSplit sp;
     sp.nblk = A.nblk; sp.U = (long long)n_tiles * A.nblk; sp.G = gridDim.x;
     const long long ua = sp.u0(blockIdx.x), ub = sp.u0(blockIdx.x + 1);
+    const int tile_a = (int)(ua / sp.nblk), tile_b = (int)((ub - 1) / sp.nblk);   // first and last tile of this CTA's span
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NS; ++s) {
@@ -238,13 +240,104 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     const int r = lane >> 2, c = lane & 3;
     // B fragments: rows 2 c + j of an 8-row block, columns 32 warp + 16 g + 2 r + {0, 1}
     const uint32_t b_off = (uint32_t)(2 * c) * kRgRowBytes + (uint32_t)(kRgWarpCols * warp + 2 * r) * 8;
+    // ---------------------------------------------------------------- a4 for the 256 columns of one tile whose
+    // contributors have all parked their partial tiles
+    auto finish_tile = [&](const int tile) {
+        const int d = tile / A.n_strips, strip = tile - d * A.n_strips;
+        const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
+        // where the contributors parked: one slot_of (four 64-bit divisions) per thread -- inside the summation loop they
+        // were 9 / 21 / 30 us of a 0.18 / 0.21 / 0.32 ms call at 4 / 16 / 32 points
+        for (int t = threadIdx.x; t <= jl - jf; t += kRgConsumers) s_slot[t] = sp.slot_of(jf + t, tile);
+        __threadfence();
+        rg_bar_consumers();
+        {
+            const int col = strip * kRgCols + threadIdx.x;
+            const bool col_ok = col < n_rec;
+            double bk = 0.0, cn = 0.0;
+            if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
+#pragma unroll 1
+            for (int pb = 0; pb < MB; ++pb) {
+                double m[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) m[e] = 0.0;
+                // contributors in CTA order (the sum is the same whoever finishes); four of them = 32 loads in flight
+                for (int j0 = jf; j0 <= jl; j0 += 4) {
+                    double v[4][8];
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const int j = min(j0 + jj, jl);
+                        const double *src = A.slots + (size_t)s_slot[j - jf] * (PP * kRgCols) + (8 * pb) * kRgCols + threadIdx.x;
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) v[jj][e] = __ldcg(src + e * kRgCols);
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj)
+                        if (j0 + jj <= jl) {
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) m[e] += v[jj][e];
+                        }
+                }
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int p = 8 * pb + e;
+                    double t = 0.0;
+                    if (col_ok && p < Pb) {
+                        const double a = m[e] + bk;
+                        if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
+                        t = poisson_term(a, cn);
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                    if (lane == 0) red[warp * PP + p] = t;
+                }
+            }
+            rg_bar_consumers();
+            if (threadIdx.x < PP) {
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
+                __stcg(A.strip_part + (size_t)tile * kRidgeMaxP + threadIdx.x, v);
+            }
+            // -------------------------------------------------------- last tile: sum strips and periods, write
+            __threadfence();
+            rg_bar_consumers();
+            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + n_tiles, 1);
+            rg_bar_consumers();
+            const bool all_done = (s_flag == n_tiles - 1);
+            rg_bar_consumers();
+            if (all_done) {
+                __threadfence();
+                // warp w adds the tiles w, w + 8, ... for point `lane` (+ 32), then the eight warps in order: a fixed
+                // order, and one round trip to L2 instead of n_tiles / 4
+#pragma unroll
+                for (int h = 0; h < (PP + 31) / 32; ++h) {
+                    const int p = 32 * h + lane;
+                    double v = 0.0;
+                    if (p < Pb)
+                        for (int t = warp; t < n_tiles; t += kRgWarps) v += __ldcg(A.strip_part + (size_t)t * kRidgeMaxP + p);
+                    if (p < PP) red[warp * PP + p] = v;
+                }
+                rg_bar_consumers();
+                if (threadIdx.x < Pb) {
+                    double v = 0.0;
+#pragma unroll
+                    for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
+                    v *= 2.0;
+                    if (A.sat_const) v += A.sat_const[0];
+                    A.out[threadIdx.x] = v;
+                }
+                if (threadIdx.x == 0) A.cnt[n_tiles] = 0;                  // ready for the next launch
+            }
+        }
+    };
+    int pending = 0;                  // shared tiles this CTA arrived at last: bit 0 the first of its span, bit 1 the last
     int stage = 0, release = -1;      // `release`: the stage consumed in the previous iteration, not yet handed back
     uint32_t phase = 0;
     for (long long u = ua; u < ub;) {
         const int tile = (int)(u / sp.nblk), b0 = (int)(u - (long long)tile * sp.nblk);
         const int nb = (int)min((long long)(sp.nblk - b0), ub - u);
-        const int d = tile / A.n_strips, strip = tile - d * A.n_strips;
-        const int row0 = b0 * RS, row1 = min(n_T, (b0 + nb) * RS), nrows = row1 - row0;
+        const int d = tile / A.n_strips;
+        const int row0 = b0 * RS, row1 = min(n_T, (b0 + nb) * RS);
         u += nb;
 
         // ------------------------------------------------------------ a2: this warp's 8-row block of a 64-row chunk
@@ -364,7 +457,8 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
         // ------------------------------------------------------------ park the partial tile of this segment
         // column 4 c + 2 e + nb of a 16-column group holds acc[.][.][nb][e]; tile-local layout [8 MB][256]
         {
-            double *slot = A.slots + (size_t)sp.slot_of(blockIdx.x, tile) * (PP * kRgCols);
+            const int my_slot = 3 * blockIdx.x + (tile == tile_a ? 0 : tile == tile_b ? 2 : 1);     // = sp.slot_of(blockIdx.x, tile)
+            double *slot = A.slots + (size_t)my_slot * (PP * kRgCols);
 #pragma unroll
             for (int mb = 0; mb < MB; ++mb)
 #pragma unroll
@@ -375,6 +469,10 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
                 }
         }
         // ------------------------------------------------------------ who finishes this tile?
+        // A tile shared with other CTAs is finished by its last contributor -- but not now: a CTA that still has a
+        // segment to stream would stall its ring for the whole of a4 (and pay a4 again for its last tile); the tile
+        // waits in its slots until this CTA has streamed everything.  A tile this CTA owns alone is finished at once
+        // (its slot 3 j + 1 is reused by the next whole tile).
         const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
         __threadfence();
         rg_bar_consumers();
@@ -382,81 +480,17 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
             if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + tile, 1);
             rg_bar_consumers();
             const bool last = (s_flag == jl - jf);
-            rg_bar_consumers();                                        // s_flag is rewritten below / next segment
-            if (!last) continue;
-            __threadfence();
-            if (threadIdx.x == 0) A.cnt[tile] = 0;                     // every contributor has arrived: ready for the next launch
-        }
-
-        // ------------------------------------------------------------ a4 for the 256 columns of this tile
-        {
-            const int col = strip * kRgCols + threadIdx.x;
-            const bool col_ok = col < n_rec;
-            double bk = 0.0, cn = 0.0;
-            if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
-#pragma unroll 1
-            for (int pb = 0; pb < MB; ++pb) {
-                double m[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) m[e] = 0.0;
-                // contributors in CTA order (the sum is the same whoever finishes); four of them = 32 loads in flight
-                for (int j0 = jf; j0 <= jl; j0 += 4) {
-                    double v[4][8];
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        const int j = min(j0 + jj, jl);
-                        const double *src = A.slots + (size_t)sp.slot_of(j, tile) * (PP * kRgCols) + (8 * pb) * kRgCols + threadIdx.x;
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) v[jj][e] = __ldcg(src + e * kRgCols);
-                    }
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj)
-                        if (j0 + jj <= jl) {
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) m[e] += v[jj][e];
-                        }
-                }
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int p = 8 * pb + e;
-                    double t = 0.0;
-                    if (col_ok && p < Pb) {
-                        const double a = m[e] + bk;
-                        if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
-                        t = poisson_term(a, cn);
-                    }
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                    if (lane == 0) red[warp * PP + p] = t;
-                }
+            rg_bar_consumers();                                        // s_flag is rewritten by the next segment
+            if (last) {
+                if (threadIdx.x == 0) A.cnt[tile] = 0;                 // every contributor has arrived: ready for the next launch
+                pending |= (tile == tile_a) ? 1 : 2;                   // a shared tile is the first or the last of the span
             }
-            rg_bar_consumers();
-            if (threadIdx.x < PP) {
-                double v = 0.0;
-#pragma unroll
-                for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
-                __stcg(A.strip_part + (size_t)tile * kRidgeMaxP + threadIdx.x, v);
-            }
-            // -------------------------------------------------------- last tile: sum strips and periods, write
-            __threadfence();
-            rg_bar_consumers();
-            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + n_tiles, 1);
-            rg_bar_consumers();
-            const bool all_done = (s_flag == n_tiles - 1);
-            rg_bar_consumers();
-            if (all_done) {
-                __threadfence();
-                if (threadIdx.x < Pb) {
-                    double v = 0.0;
-                    for (int t = 0; t < n_tiles; ++t) v += __ldcg(A.strip_part + (size_t)t * kRidgeMaxP + threadIdx.x);
-                    v *= 2.0;
-                    if (A.sat_const) v += A.sat_const[0];
-                    A.out[threadIdx.x] = v;
-                }
-                if (threadIdx.x == 0) A.cnt[n_tiles] = 0;                  // ready for the next launch
-            }
+        } else {
+            finish_tile(tile);
         }
     }
+    if (pending & 1) finish_tile(tile_a);
+    if (pending & 2) finish_tile(tile_b);
 }
 
 template <int MB>
@@ -483,7 +517,7 @@ int ridge_grid(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *nblk_ou
     const long long U = (long long)strips * D * nblk;
     const int slots = num_sms * ((mb_log2 <= 1) ? 2 : 1);
     long long G = U / (256 / RS);
-    if (G > slots) G = slots;
+    if (G > slots) G = slots;                                          // <= 2 kRidgePlanSMs: s_slot[] in the kernel
     // a whole number of CTAs per strip when that still fills >= 95 % of the slots: the strips then advance through the
     // recoil rows in step, so that the 2 KB row segments in flight belong to few, complete 8 n_rec-byte rows of R
     // (measured on config 4, 4 / 16 points: 0.181 / 0.186 ms with 288 CTAs, 0.187 / 0.197 ms with 296)

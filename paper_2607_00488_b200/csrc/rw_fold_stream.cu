@@ -162,15 +162,28 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
     double m0[PB], m1[PB];
 #pragma unroll
     for (int p = 0; p < PB; ++p) m0[p] = m1[p] = 0.0;
-    if (col_ok)
-        for (int s = 0; s < n_splits; ++s) {          // row ranges in a fixed order; the PB loads of a step overlap
+    if (col_ok) {
+        // row ranges in a fixed order, kBatch of them (16 loads) in flight: left to the compiler the loop ran ~4 loads
+        // deep, ten dependent round trips to L2 for the 37 row ranges of a config-4 strip (~10 us of a 0.17 ms call)
+        constexpr int kBatch = (PB >= 16) ? 1 : 16 / PB;
+        for (int s0 = 0; s0 < n_splits; s0 += kBatch) {
+            double2 v[kBatch][PB];
 #pragma unroll
-            for (int p = 0; p < PB; ++p) {
-                const double2 v = __ldcg(reinterpret_cast<const double2 *>(
-                    A.mu_part + (((size_t)d * n_splits + s) * PB + p) * mu_ld + col));
-                m0[p] += v.x; m1[p] += v.y;
+            for (int u = 0; u < kBatch; ++u) {
+                const int s = min(s0 + u, n_splits - 1);
+#pragma unroll
+                for (int p = 0; p < PB; ++p)
+                    v[u][p] = __ldcg(reinterpret_cast<const double2 *>(
+                        A.mu_part + (((size_t)d * n_splits + s) * PB + p) * mu_ld + col));
             }
+#pragma unroll
+            for (int u = 0; u < kBatch; ++u)
+                if (s0 + u < n_splits) {
+#pragma unroll
+                    for (int p = 0; p < PB; ++p) { m0[p] += v[u][p].x; m1[p] += v[u][p].y; }
+                }
         }
+    }
 #pragma unroll
     for (int p = 0; p < PB; ++p) {
         double t = 0.0;
@@ -203,9 +216,17 @@ k_fold_stream(const StreamArgs A, const Kinds kd, const Consts cst)
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    {   // warp w adds the strips w, w + 8, ... of point `lane`, then the eight warps in order: fixed order, one round trip
+        double v = 0.0;
+        if (lane < Pb)
+            for (int q = warp; q < n_sid; q += kStreamThreads / 32) v += __ldcg(A.strip_part + (size_t)q * kStreamMaxPB + lane);
+        if (lane < PB) red[warp][lane] = v;
+    }
+    __syncthreads();
     if (threadIdx.x < Pb) {
         double v = 0.0;
-        for (int q = 0; q < n_sid; ++q) v += __ldcg(A.strip_part + (size_t)q * kStreamMaxPB + threadIdx.x);
+#pragma unroll
+        for (int w = 0; w < kStreamThreads / 32; ++w) v += red[w][threadIdx.x];
         v *= 2.0;
         if (A.sat_const) v += A.sat_const[0];
         A.out[threadIdx.x] = v;
