@@ -105,8 +105,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->partial = take((part_gemm > part_stream ? part_gemm : part_stream) * 8);
     L->mu_part = take(D * (size_t)(max_splits < splits ? max_splits : splits) * kStreamMaxPB * mu_ld * 8);
     L->ridge_slots = take(ridge_slot_bytes);
-    L->ridge_cnt = take((D * (size_t)L->ridge_strips + 1) * 4);
-    L->ridge_part = take(D * (size_t)L->ridge_strips * kRidgeMaxP * 8);
+    L->ridge_cnt = take((2 * D * (size_t)L->ridge_strips + 1) * 4);
+    L->ridge_part = take((size_t)2 * kRidgePlanSMs * kRidgeMaxP * 8);
     L->out_stage = take((size_t)max_batch * 8);
     {   // split-K scratch: at most 8 work items per SM, and never more than 16 k-ranges of every 16-point tile
         int64_t items = (int64_t)L->n_tiles_n * ((L->MC + 15) / 16) * 16;
@@ -503,7 +503,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     RW_TRY(cudaMemsetAsync(ctx->flag, 0, 4, s));
     if (n_comp > 1 && !host) RW_TRY(launch_comp8(ctx, in->comp_of_T, s));
     RW_TRY(cudaMemsetAsync(ctx->stream_cnt, 0, (D * (size_t)L.stream_strips + 1) * 4, s));
-    RW_TRY(cudaMemsetAsync(ctx->ridge_cnt, 0, (D * (size_t)L.ridge_strips + 1) * 4, s));
+    RW_TRY(cudaMemsetAsync(ctx->ridge_cnt, 0, (2 * D * (size_t)L.ridge_strips + 1) * 4, s));
     RW_TRY(launch_flavour(ctx, have_mt ? 1 : 0, f_tau, s));
     if (!host) RW_TRY(launch_validate_device(ctx, ctx->R, ctx->ldR, ctx->R_period_stride, s));
     RW_TRY(launch_setup(ctx, s));

@@ -53,8 +53,8 @@ struct RidgeArgs {
     int zero_ring;            // ragged strip or row tail: the ring is read where no copy lands
     int zero;                 // 0, opaque to the compiler (release of a ring stage at 16 points)
     double *slots;            // [3 G][8 MB][256] parked partial tiles
-    double *strip_part;       // [D * strips][64] Poisson sums per tile
-    int *cnt;                 // [D * strips] tile tickets, then one global ticket
+    double *strip_part;       // [G][64] Poisson sums of everything a CTA finished
+    int *cnt;                 // [D * strips] "parked" tickets, [D * strips] "left" tickets, one global ticket
     double *out;              // [Pb]
     double *out_mu;           // NULL or [Pb][D][n_rec]
 };
@@ -240,94 +240,78 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     const int r = lane >> 2, c = lane & 3;
     // B fragments: rows 2 c + j of an 8-row block, columns 32 warp + 16 g + 2 r + {0, 1}
     const uint32_t b_off = (uint32_t)(2 * c) * kRgRowBytes + (uint32_t)(kRgWarpCols * warp + 2 * r) * 8;
-    // ---------------------------------------------------------------- a4 for the 256 columns of one tile whose
-    // contributors have all parked their partial tiles
-    auto finish_tile = [&](const int tile) {
+    // ---------------------------------------------------------------- a4, shared out among the contributors of a tile
+    // Once every contributor [jf, jl] of `tile` has parked its partial tile, contributor ci = j - jf finishes the points
+    // [ci PPc, (ci + 1) PPc) of it for all 256 columns: sums the parked partials in CTA order (the result does not
+    // depend on who arrives when), adds bkg, reduces the Poisson terms of Eq. (18).  One round trip to L2 per CTA instead
+    // of one per contributor in a single finishing CTA (which cost 7 / 15 / 21 us of a 0.18 / 0.19 / 0.32 ms call at
+    // 4 / 16 / 32 points).  Thread t keeps the running sum of point t over everything this CTA finishes.
+    double my_part = 0.0;
+    auto finish_slice = [&](const int tile, const int jf, const int jl) {
         const int d = tile / A.n_strips, strip = tile - d * A.n_strips;
-        const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
-        // where the contributors parked: one slot_of (four 64-bit divisions) per thread -- inside the summation loop they
-        // were 9 / 21 / 30 us of a 0.18 / 0.21 / 0.32 ms call at 4 / 16 / 32 points
-        for (int t = threadIdx.x; t <= jl - jf; t += kRgConsumers) s_slot[t] = sp.slot_of(jf + t, tile);
-        __threadfence();
-        rg_bar_consumers();
-        {
-            const int col = strip * kRgCols + threadIdx.x;
-            const bool col_ok = col < n_rec;
-            double bk = 0.0, cn = 0.0;
-            if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
+        const int ncon = jl - jf + 1, ci = blockIdx.x - jf;
+        const int PPc = (Pb + ncon - 1) / ncon;
+        const int p_lo = ci * PPc, p_hi = min(Pb, p_lo + PPc);
+        if (p_lo >= p_hi) return;                                       // (uniform) more contributors than points
+        const int col = strip * kRgCols + threadIdx.x;
+        const bool col_ok = col < n_rec;
+        double bk = 0.0, cn = 0.0;
+        if (col_ok) { bk = A.bkg[(size_t)d * n_rec + col]; cn = A.counts[(size_t)d * n_rec + col]; }
 #pragma unroll 1
-            for (int pb = 0; pb < MB; ++pb) {
-                double m[8];
+        for (int p0 = p_lo; p0 < p_hi; p0 += 4) {
+            double m[4] = {0.0, 0.0, 0.0, 0.0};
+            for (int j0 = 0; j0 < ncon; j0 += 8) {                      // 4 points x 8 contributors = 32 loads in flight
+                double v[8][4];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) m[e] = 0.0;
-                // contributors in CTA order (the sum is the same whoever finishes); four of them = 32 loads in flight
-                for (int j0 = jf; j0 <= jl; j0 += 4) {
-                    double v[4][8];
+                for (int jj = 0; jj < 8; ++jj) {
+                    const double *src = A.slots + (size_t)s_slot[min(j0 + jj, ncon - 1)] * (PP * kRgCols) + threadIdx.x;
 #pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        const int j = min(j0 + jj, jl);
-                        const double *src = A.slots + (size_t)s_slot[j - jf] * (PP * kRgCols) + (8 * pb) * kRgCols + threadIdx.x;
+                    for (int e = 0; e < 4; ++e) v[jj][e] = __ldcg(src + (size_t)min(p0 + e, p_hi - 1) * kRgCols);
+                }
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) v[jj][e] = __ldcg(src + e * kRgCols);
+                for (int jj = 0; jj < 8; ++jj)
+                    if (j0 + jj < ncon) {
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) m[e] += v[jj][e];
                     }
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj)
-                        if (j0 + jj <= jl) {
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) m[e] += v[jj][e];
-                        }
-                }
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int p = 8 * pb + e;
-                    double t = 0.0;
-                    if (col_ok && p < Pb) {
-                        const double a = m[e] + bk;
-                        if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
-                        t = poisson_term(a, cn);
-                    }
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                    if (lane == 0) red[warp * PP + p] = t;
-                }
             }
-            rg_bar_consumers();
-            if (threadIdx.x < PP) {
-                double v = 0.0;
 #pragma unroll
-                for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
-                __stcg(A.strip_part + (size_t)tile * kRidgeMaxP + threadIdx.x, v);
-            }
-            // -------------------------------------------------------- last tile: sum strips and periods, write
-            __threadfence();
-            rg_bar_consumers();
-            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + n_tiles, 1);
-            rg_bar_consumers();
-            const bool all_done = (s_flag == n_tiles - 1);
-            rg_bar_consumers();
-            if (all_done) {
-                __threadfence();
-                // warp w adds the tiles w, w + 8, ... for point `lane` (+ 32), then the eight warps in order: a fixed
-                // order, and one round trip to L2 instead of n_tiles / 4
-#pragma unroll
-                for (int h = 0; h < (PP + 31) / 32; ++h) {
-                    const int p = 32 * h + lane;
-                    double v = 0.0;
-                    if (p < Pb)
-                        for (int t = warp; t < n_tiles; t += kRgWarps) v += __ldcg(A.strip_part + (size_t)t * kRidgeMaxP + p);
-                    if (p < PP) red[warp * PP + p] = v;
+            for (int e = 0; e < 4; ++e) {
+                const int p = p0 + e;
+                double t = 0.0;
+                if (col_ok && p < p_hi) {
+                    const double a = m[e] + bk;
+                    if (A.out_mu) A.out_mu[((size_t)p * A.D + d) * n_rec + col] = a;
+                    t = poisson_term(a, cn);
                 }
-                rg_bar_consumers();
-                if (threadIdx.x < Pb) {
-                    double v = 0.0;
 #pragma unroll
-                    for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
-                    v *= 2.0;
-                    if (A.sat_const) v += A.sat_const[0];
-                    A.out[threadIdx.x] = v;
-                }
-                if (threadIdx.x == 0) A.cnt[n_tiles] = 0;                  // ready for the next launch
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                if (lane == 0 && p < p_hi) red[warp * PP + p] = t;
             }
+        }
+        rg_bar_consumers();
+        if ((int)threadIdx.x >= p_lo && (int)threadIdx.x < p_hi) {
+#pragma unroll
+            for (int w = 0; w < kRgWarps; ++w) my_part += red[w * PP + threadIdx.x];
+        }
+        rg_bar_consumers();                                             // red is rewritten by the next tile
+    };
+    // a shared tile: wait until all its contributors have parked (they are co-resident: one wave, cooperative launch),
+    // finish this CTA's share, and let the last one to leave reset the two tickets for the next launch
+    auto finish_shared = [&](const int tile) {
+        const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
+        const int ncon = jl - jf + 1;
+        for (int t = threadIdx.x; t < ncon; t += kRgConsumers) s_slot[t] = sp.slot_of(jf + t, tile);   // four 64-bit divisions each
+        if (threadIdx.x == 0) {
+            const volatile int *tk = A.cnt + tile;
+            while (*tk < ncon) __nanosleep(64);
+        }
+        rg_bar_consumers();
+        __threadfence();
+        finish_slice(tile, jf, jl);
+        if (threadIdx.x == 0 && atomicAdd(A.cnt + n_tiles + tile, 1) == ncon - 1) {
+            A.cnt[tile] = 0;                                            // everyone is past the wait above
+            A.cnt[n_tiles + tile] = 0;
         }
     };
     int pending = 0;                  // shared tiles this CTA arrived at last: bit 0 the first of its span, bit 1 the last
@@ -468,29 +452,62 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
                     __stcg(reinterpret_cast<double2 *>(dst + 2), make_double2(acc[mb][g][0][1], acc[mb][g][1][1]));
                 }
         }
-        // ------------------------------------------------------------ who finishes this tile?
-        // A tile shared with other CTAs is finished by its last contributor -- but not now: a CTA that still has a
-        // segment to stream would stall its ring for the whole of a4 (and pay a4 again for its last tile); the tile
-        // waits in its slots until this CTA has streamed everything.  A tile this CTA owns alone is finished at once
-        // (its slot 3 j + 1 is reused by the next whole tile).
+        // ------------------------------------------------------------ a4
+        // A tile shared with other CTAs is finished by all of them together -- but not now: a CTA that still has a
+        // segment to stream would stall its ring; the partial tile waits in its slot until this CTA has streamed
+        // everything.  A tile this CTA owns alone is finished at once (its slot 3 j + 1 is reused by the next one).
         const int jf = sp.cta_of((long long)tile * sp.nblk), jl = sp.cta_of((long long)(tile + 1) * sp.nblk - 1);
         __threadfence();
         rg_bar_consumers();
         if (jl > jf) {
-            if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + tile, 1);
-            rg_bar_consumers();
-            const bool last = (s_flag == jl - jf);
-            rg_bar_consumers();                                        // s_flag is rewritten by the next segment
-            if (last) {
-                if (threadIdx.x == 0) A.cnt[tile] = 0;                 // every contributor has arrived: ready for the next launch
-                pending |= (tile == tile_a) ? 1 : 2;                   // a shared tile is the first or the last of the span
-            }
+            if (threadIdx.x == 0) atomicAdd(A.cnt + tile, 1);          // parked
+            pending |= (tile == tile_a) ? 1 : 2;                       // a shared tile is the first or the last of the span
         } else {
-            finish_tile(tile);
+            if (threadIdx.x == 0) s_slot[0] = 3 * blockIdx.x + (tile == tile_a ? 0 : tile == tile_b ? 2 : 1);
+            rg_bar_consumers();
+            finish_slice(tile, jf, jl);
         }
     }
-    if (pending & 1) finish_tile(tile_a);
-    if (pending & 2) finish_tile(tile_b);
+    if (pending & 1) finish_shared(tile_a);
+    if (pending & 2) finish_shared(tile_b);
+
+    // ---------------------------------------------------------------- the last CTA adds the CTAs' sums and writes -2lnL
+    if (threadIdx.x < PP) __stcg(A.strip_part + (size_t)blockIdx.x * kRidgeMaxP + threadIdx.x, my_part);
+    __threadfence();
+    rg_bar_consumers();
+    if (threadIdx.x == 0) s_flag = atomicAdd(A.cnt + 2 * n_tiles, 1);
+    rg_bar_consumers();
+    if (s_flag != (int)gridDim.x - 1) return;
+    __threadfence();
+    // warp w adds the CTAs w, w + 8, ... for point `lane` (+ 32), eight loads in flight, then the eight warps in order
+#pragma unroll
+    for (int h = 0; h < (PP + 31) / 32; ++h) {
+        const int p = 32 * h + lane;
+        double v = 0.0;
+        if (p < Pb) {
+            for (int j0 = warp; j0 < (int)gridDim.x; j0 += 8 * kRgWarps) {
+                double x[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int j = j0 + u * kRgWarps;
+                    x[u] = (j < (int)gridDim.x) ? __ldcg(A.strip_part + (size_t)j * kRidgeMaxP + p) : 0.0;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v += x[u];
+            }
+        }
+        if (p < PP) red[warp * PP + p] = v;
+    }
+    rg_bar_consumers();
+    if (threadIdx.x < Pb) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < kRgWarps; ++w) v += red[w * PP + threadIdx.x];
+        v *= 2.0;
+        if (A.sat_const) v += A.sat_const[0];
+        A.out[threadIdx.x] = v;
+    }
+    if (threadIdx.x == 0) A.cnt[2 * n_tiles] = 0;                      // ready for the next launch
 }
 
 template <int MB>
@@ -503,8 +520,19 @@ static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Con
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    k_fold_ridge<MB><<<grid, RidgeCfg<MB>::Threads, RidgeCfg<MB>::Smem, s>>>(A, kd, cst);
-    return cudaSuccess;
+    // cooperative: the contributors of a tile wait for one another, so the whole grid (one wave by construction,
+    // ridge_grid) must be resident at once; the launch fails instead of hanging where it could not be
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(RidgeCfg<MB>::Threads);
+    cfg.dynamicSmemBytes = RidgeCfg<MB>::Smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_fold_ridge<MB>, A, kd, cst);
 }
 
 // Grid of k_fold_ridge for tile height 8 << mb_log2: one wave of the SM slots, but at least ~256 recoil rows of one

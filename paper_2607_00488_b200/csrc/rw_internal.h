@@ -99,8 +99,8 @@ struct rw_ctx {
     size_t R_period_stride;   // doubles between periods
     double *basis, *S_sm, *What, *sat_const;
     int *stream_cnt;          // last-CTA-done tickets of the streaming fold: [D * strips] + 1, self-resetting
-    int *ridge_cnt;           // the same for k_fold_ridge: [D * ridge_strips] + 1
-    double *ridge_part;       // [D * ridge_strips][64] Poisson sums per column strip of k_fold_ridge
+    int *ridge_cnt;           // tickets of k_fold_ridge: 2 x [D * ridge_strips] + 1
+    double *ridge_part;       // [2 kRidgePlanSMs][64] Poisson sums per CTA of k_fold_ridge
     double *ridge_slots;      // [3 G][tile height][256] parked partial tiles of k_fold_ridge
     double *strip_part;       // [D * strips][16] Poisson sums per column strip
     double *G, *ident;        // prefolded templates [D][12][ldG]; identity coefficients [16][12] used to fold them
