@@ -188,9 +188,9 @@ def policy_kernel(P):
     """The fold kernel RW_MODE_AUTO picks for a call of P points (label only; mirrors rw_api.cu)."""
     if P <= 1:
         return "k_fold_stream<1>"
-    if P <= 32:
-        return "k_fold_ridge<%d>" % (1 if P <= 8 else 2 if P <= 16 else 4)
-    return "k_fold_gemm<%d>" % (4 if P <= 64 else 8)
+    if P <= 64:
+        return "k_fold_ridge<%d>" % (1 if P <= 8 else 2 if P <= 16 else 4 if P <= 32 else 8)
+    return "k_fold_gemm<8>"
 
 
 def parity_indices(name, P, max_batch, n):

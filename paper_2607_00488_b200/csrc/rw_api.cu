@@ -107,6 +107,8 @@ static int plan(const rw_inputs *in, int64_t max_batch, Layout *L)
     L->ridge_slots = take(ridge_slot_bytes);
     L->ridge_cnt = take((2 * D * (size_t)L->ridge_strips + 1) * 4);
     L->ridge_part = take((size_t)2 * kRidgePlanSMs * kRidgeMaxP * 8);
+    // N' in fragment order for the ridge kernel's tile heights 32 and 64: [D][n_T / 8 + 8 blocks][points / 8][32] x 16 B
+    L->ridge_frag = take(L->ridge_max_p >= 32 ? D * ((n_T + 7) / 8 + 8) * (size_t)(L->ridge_max_p / 8) * 512 : 0);
     L->out_stage = take((size_t)max_batch * 8);
     {   // split-K scratch: at most 8 work items per SM, and never more than 16 k-ranges of every 16-point tile
         int64_t items = (int64_t)L->n_tiles_n * ((L->MC + 15) / 16) * 16;
@@ -187,11 +189,11 @@ static const char *flag_message(int f)
     return "invalid input";
 }
 
-// RW_MODE_AUTO (measured on B200, config-4 size): one point -> the one-launch HBM-streaming kernel; 2..32 points ->
-// the one-launch streaming DMMA kernel (R read once at HBM speed, contraction on the FP64 tensor cores); beyond -> the
-// tiled DMMA contraction (tile height 64 / 128, split-K: 0.57 ms against 0.61 ms at 64 points).  The opt-in
-// contractions (prec != 0) replace the last two.
-constexpr int kAutoRidgeMax = 32;
+// RW_MODE_AUTO (measured on B200, config-4 size): one point -> the one-launch HBM-streaming kernel; 2..64 points ->
+// the streaming DMMA kernel (R read once at HBM speed, contraction on the FP64 tensor cores; one launch up to 16
+// points, N' from k_ridge_frag above: 64 points 0.536 ms against 0.574 ms for the tiled contraction); beyond -> the
+// tiled DMMA contraction (tile height 128, split-K).  The opt-in contractions (prec != 0) replace the last two.
+constexpr int kAutoRidgeMax = 64;
 static bool auto_stream(const rw_ctx *, int64_t P, int prec) { return prec == 0 ? P <= 1 : P <= 4; }
 static bool use_stream(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
 {
@@ -431,6 +433,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
     ctx->strip_part = (double *)(ws + L.strip_part);
     ctx->ridge_cnt = (int *)(ws + L.ridge_cnt);
     ctx->ridge_part = (double *)(ws + L.ridge_part);
+    ctx->ridge_frag = (double *)(ws + L.ridge_frag);
     ctx->ridge_slots = (double *)(ws + L.ridge_slots);
     ctx->param_stage = (double *)(ws + L.param_stage);
     ctx->coef = (double *)(ws + L.coef);    ctx->A_packed = (double *)(ws + L.A_packed);

@@ -23,6 +23,10 @@
 //     rows {2 c + j}: the lanes store and reload their own 16 bytes (double-buffered, lane-linear: no bank conflicts,
 //     no transposition).  3 MB DMMAs per warp and chunk instead of 22 MB DFMAs per thread: with scalar staging the
 //     tensor pipe was 75 % busy at 64 points, and separate scalar stager warps could not keep up at all;
+//   * tile heights 32 and 64 (17..64 points) take N' ready-made instead: k_ridge_frag writes it once per call in the
+//     fragment layout and one more warp copies it chunk by chunk (one bulk copy) into the two buffers -- formed in the
+//     consumer warps, the dependent chain load -> 3 DMMA -> store and its bar.sync cost 10 % of the kernel there, and
+//     stager warps (DMMA or scalar) only queue behind the consumers: on B200 DFMA and DMMA share one pipe;
 //   * at 64 points setmaxnreg moves the registers of the producer warpgroup to the consumers (128 accumulators);
 //   * a4: the finishing CTA of a strip adds bkg and reduces the Poisson terms of Eq. (18) of its 256
 //     columns; the last strip adds strips and periods in a fixed order and writes -2lnL.  One launch per call.
@@ -52,6 +56,8 @@ struct RidgeArgs {
     int Pb, n_strips, nblk;   // strips per period; blocks of RS rows per strip
     int zero_ring;            // ragged strip or row tail: the ring is read where no copy lands
     int zero;                 // 0, opaque to the compiler (release of a ring stage at 16 points)
+    double *frag;             // tile heights 32, 64: N' as DMMA fragments [D][nblk8][MB][32 lanes] x 16 B (k_ridge_frag)
+    int nblk8;                // 8-row blocks per period in `frag` (n_T / 8 rounded up, + 8 zero blocks)
     double *slots;            // [3 G][8 MB][256] parked partial tiles
     double *strip_part;       // [G][64] Poisson sums of everything a CTA finished
     int *cnt;                 // [D * strips] "parked" tickets, [D * strips] "left" tickets, one global ticket
@@ -107,7 +113,11 @@ template <int MB> struct RidgeCfg {
     // flight), or at once through a register dependence on its fragment loads (16 points: five 16 KB stages per CTA
     // are too few to give one away -- 0.199 ms against 0.214 ms on config 4)
     static constexpr bool LateRelease = (MB != 2);
-    static constexpr int Threads = (MB == 8) ? kRgThreads64 : kRgThreads;
+    // Tile heights 32 and 64 read N' ready-made (k_ridge_frag writes it once per call instead of once per column strip
+    // in every CTA; in the consumer warps the chain load W^ -> 3 DMMA -> store and the bar.sync behind it idled the
+    // tensor pipe for 10 % of the kernel there): one more warp copies it chunk by chunk into the two N' buffers
+    static constexpr bool Prefab = (MB >= 4);
+    static constexpr int Threads = (MB == 8) ? kRgThreads64 : Prefab ? kRgThreads + 32 : kRgThreads;
     // tile height 64: setmaxnreg redistributes the registers the CTA was LAUNCHED with (384 x 168): 256 ConsumerRegs +
     // 128 HelperRegs must not exceed that pool, or the consumers wait for ever
     static constexpr int ConsumerRegs = 224, HelperRegs = 40;
@@ -116,7 +126,7 @@ template <int MB> struct RidgeCfg {
     static constexpr int RingBytes = NS * StageBytes;
     static constexpr int NBytes = kRgNB * (kRgKC / 8) * MB * 512;      // N' fragments: [buffer][8-row block][mb][lane] x 16 B
     static constexpr int SmemDoubles = PP * kCoefStride + PP * RW_MAX_COMPONENTS + kRgWarps * PP;
-    static constexpr int Smem = RingBytes + NBytes + SmemDoubles * 8 + 2 * NS * 8;
+    static constexpr int Smem = RingBytes + NBytes + SmemDoubles * 8 + 2 * NS * 8 + 2 * kRgNB * 8;
 };
 
 // Work split shared by the three roles.  Units u = tile * nblk + block; CTA j owns [u0(j), u0(j + 1)).
@@ -152,6 +162,8 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     double *red = sRate + PP * RW_MAX_COMPONENTS;                      // [8 warps][PP]
     const uint32_t full_bar = rg_smem_u32(red + kRgWarps * PP);        // ring: NS full, NS empty
     const uint32_t empty_bar = full_bar + NS * 8;
+    const uint32_t nfull_bar = empty_bar + NS * 8;                     // the two N' buffers (tile heights 32, 64)
+    const uint32_t nempty_bar = nfull_bar + kRgNB * 8;
     __shared__ int s_flag;
     __shared__ int s_slot[2 * kRidgePlanSMs + 8];                       // slots of the contributors of the tile being finished
 
@@ -167,6 +179,10 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
         for (int s = 0; s < NS; ++s) {
             rg_mbar_init(full_bar + 8 * s, 1);
             rg_mbar_init(empty_bar + 8 * s, kRgWarps);
+        }
+        for (int s = 0; s < kRgNB; ++s) {
+            rg_mbar_init(nfull_bar + 8 * s, 1);
+            rg_mbar_init(nempty_bar + 8 * s, kRgWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -205,6 +221,26 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
                 }
                 u += nb;
             }
+        } else if (Cfg::Prefab && warp == kRgWarps + 1 && lane == 0) {
+            // ------------------------------------------------------------ N' loader: chunk n -> buffer n & 1
+            uint64_t policy;
+            asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(policy));    // read by every strip
+            uint32_t n = 0;
+            for (long long u = ua; u < ub;) {
+                const int tile = (int)(u / sp.nblk), b0 = (int)(u - (long long)tile * sp.nblk);
+                const int nb = (int)min((long long)(sp.nblk - b0), ub - u);
+                const int d = tile / A.n_strips;
+                const int row0 = b0 * RS, row1 = min(n_T, (b0 + nb) * RS);
+                u += nb;
+                for (int ic = row0; ic < row1; ic += kRgKC, ++n) {
+                    const uint32_t buf = n & 1;
+                    rg_mbar_wait(nempty_bar + 8 * buf, ((n >> 1) & 1) ^ 1);     // the consumers are done with chunk n - 2
+                    constexpr uint32_t bytes = (kRgKC / 8) * MB * 512;
+                    rg_mbar_expect_tx(nfull_bar + 8 * buf, bytes);
+                    rg_bulk_row(sN + buf * bytes, A.frag + ((size_t)d * A.nblk8 + ic / 8) * (MB * 64), bytes,
+                                nfull_bar + 8 * buf, policy);
+                }
+            }
         }
         return;
     }
@@ -213,7 +249,7 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     if constexpr (MB == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::ConsumerRegs));
     // ---------------------------------------------------------------- a1: coefficients of the tile's points
     const double *wts = A.wts;
-    if (!wts) {
+    if (!wts && !Cfg::Prefab) {
         if (A.param) {
             if (threadIdx.x < PP) {
                 double cc[kCoefStride], rr[RW_MAX_COMPONENTS];
@@ -314,6 +350,8 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
             A.cnt[n_tiles + tile] = 0;
         }
     };
+    uint32_t chunk_n = 0;             // chunks folded so far (tile heights 32, 64: N' buffer chunk_n & 1, phase (chunk_n >> 1) & 1)
+    int nrelease = -1;                // N' buffer of the previous chunk, not yet handed back to the loader
     int pending = 0;                  // shared tiles this CTA arrived at last: bit 0 the first of its span, bit 1 the last
     int stage = 0, release = -1;      // `release`: the stage consumed in the previous iteration, not yet handed back
     uint32_t phase = 0;
@@ -376,18 +414,33 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
             for (int g = 0; g < 2; ++g)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) acc[mb][g][e][0] = acc[mb][g][e][1] = 0.0;
-        fetch(row0);
-        form(row0, 0);
+        if constexpr (!Cfg::Prefab) {
+            fetch(row0);
+            form(row0, 0);
+        }
         int q = 0, nbuf = 0;
         for (int ic = row0; ic < row1; ic += kRgKC, nbuf ^= 1) {
-            rg_bar_consumers();                      // N'[nbuf] formed by all warps; N'[nbuf ^ 1] no longer read
             const bool more = ic + kRgKC < row1;
-            if (more) fetch(ic + kRgKC);
+            if constexpr (Cfg::Prefab) {
+                nbuf = (int)(chunk_n & 1);
+                rg_mbar_wait(nfull_bar + 8 * nbuf, (chunk_n >> 1) & 1);        // N' of this chunk has landed
+            } else {
+                rg_bar_consumers();                  // N'[nbuf] formed by all warps; N'[nbuf ^ 1] no longer read
+                if (more) fetch(ic + kRgKC);
+            }
             const uint32_t sA = sN + (uint32_t)(nbuf * (kRgKC / 8) * MB) * 512 + lane * 16;
 #pragma unroll
             for (int sq = 0; sq < kRgKC / RS; ++sq) {
                 if (q < nb) {
                     rg_mbar_wait(full_bar + 8 * stage, phase);
+                    if constexpr (Cfg::Prefab) {
+                        // the N' buffer of the previous chunk goes back to the loader only now: every DMMA that read it
+                        // has been issued, so its fragment loads have returned (the hazard described at the ring release)
+                        if (nrelease >= 0) {
+                            if (lane == 0) rg_mbar_arrive(nempty_bar + 8 * nrelease);
+                            nrelease = -1;
+                        }
+                    }
                     const uint32_t st = ring + stage * Cfg::StageBytes + b_off;
                     uint32_t dep = 0;
 #pragma unroll
@@ -435,7 +488,13 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
                     ++q;
                 }
             }
-            if (more) form(ic + kRgKC, nbuf ^ 1);
+            if constexpr (Cfg::Prefab) {
+                __syncwarp();
+                nrelease = nbuf;
+                ++chunk_n;
+            } else {
+                if (more) form(ic + kRgKC, nbuf ^ 1);
+            }
         }
 
         // ------------------------------------------------------------ park the partial tile of this segment
@@ -510,6 +569,75 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     if (threadIdx.x == 0) A.cnt[2 * n_tiles] = 0;                      // ready for the next launch
 }
 
+// a1 + a2 for tile heights 32 and 64: N' of all recoil rows, once per call, in the fragment layout of the fold --
+// block of 8 rows, 8-point group mb, lane (r, c): { N'[8 mb + r][8 blk + 2 c], N'[8 mb + r][8 blk + 2 c + 1] }.
+// One CTA per 64 rows and period; thread (blk_local, lane), all mb.  Rows >= n_T and points >= Pb are zero.
+__global__ void __launch_bounds__(256)
+k_ridge_frag(const RidgeArgs A, const Kinds kd, const Consts cst, const int MB)
+{
+    __shared__ double sC[kRidgeMaxP * kCoefStride];
+    __shared__ double sRate[kRidgeMaxP * RW_MAX_COMPONENTS];
+    const int PP = 8 * MB, Pb = A.Pb, n_T = A.n_T, d = blockIdx.y;
+    if (!A.wts) {
+        if (A.param) {
+            if ((int)threadIdx.x < PP) {
+                double cc[kCoefStride], rr[RW_MAX_COMPONENTS];
+                if ((int)threadIdx.x < Pb) {
+                    coef_from_param(A.param + (size_t)threadIdx.x * kd.k, kd, cst, cc, rr);
+                } else {
+#pragma unroll
+                    for (int b = 0; b < kCoefStride; ++b) cc[b] = 0.0;
+#pragma unroll
+                    for (int q = 0; q < RW_MAX_COMPONENTS; ++q) rr[q] = 1.0;
+                }
+#pragma unroll
+                for (int b = 0; b < kCoefStride; ++b) sC[threadIdx.x * kCoefStride + b] = cc[b];
+#pragma unroll
+                for (int q = 0; q < RW_MAX_COMPONENTS; ++q) sRate[threadIdx.x * RW_MAX_COMPONENTS + q] = rr[q];
+            }
+        } else {
+            for (int q = threadIdx.x; q < PP * kCoefStride; q += 256) sC[q] = (q / kCoefStride < Pb) ? A.coef[q] : 0.0;
+            for (int q = threadIdx.x; q < PP * RW_MAX_COMPONENTS; q += 256)
+                sRate[q] = (q / RW_MAX_COMPONENTS < Pb && A.rate) ? A.rate[q] : 1.0;
+        }
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
+    const int blk = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (blk >= A.nblk8) return;
+    const int ia = 8 * blk + 2 * c;
+    const bool ok0 = ia < n_T, ok1 = ia + 1 < n_T;
+    double2 *dst = reinterpret_cast<double2 *>(A.frag) + ((size_t)d * A.nblk8 + blk) * (MB * 32) + lane;
+    if (A.wts) {
+        const double n0 = ok0 ? A.N_mc[(size_t)d * n_T + ia] : 0.0, n1 = ok1 ? A.N_mc[(size_t)d * n_T + ia + 1] : 0.0;
+        for (int mb = 0; mb < MB; ++mb) {
+            const int p = 8 * mb + r;
+            dst[mb * 32] = make_double2((p < Pb && ok0) ? A.wts[(size_t)p * n_T + ia] * n0 : 0.0,
+                                        (p < Pb && ok1) ? A.wts[(size_t)p * n_T + ia + 1] * n1 : 0.0);
+        }
+        return;
+    }
+    const double *Wd = A.What + (size_t)d * kCoefStride * n_T;
+    double w0[kNumTerms], w1[kNumTerms];
+#pragma unroll
+    for (int b = 0; b < kNumTerms; ++b) {
+        w0[b] = ok0 ? __ldg(Wd + (size_t)b * n_T + ia) : 0.0;
+        w1[b] = ok1 ? __ldg(Wd + (size_t)b * n_T + ia + 1) : 0.0;
+    }
+    const int cq0 = ok0 ? A.comp8[ia] : 0, cq1 = ok1 ? A.comp8[ia + 1] : 0;
+    for (int mb = 0; mb < MB; ++mb) {
+        const int p = 8 * mb + r;
+        double v0 = 0.0, v1 = 0.0;
+#pragma unroll
+        for (int b = 0; b < kNumTerms; ++b) {
+            const double cb = sC[p * kCoefStride + b];
+            v0 = fma(cb, w0[b], v0);
+            v1 = fma(cb, w1[b], v1);
+        }
+        dst[mb * 32] = make_double2(v0 * sRate[p * RW_MAX_COMPONENTS + cq0], v1 * sRate[p * RW_MAX_COMPONENTS + cq1]);   // rate_k of Eq. (17)
+    }
+}
+
 template <int MB>
 static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Consts &cst, int grid, cudaStream_t s)
 {
@@ -582,6 +710,8 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     A.zero = 0;
     A.slots = ctx->ridge_slots; A.strip_part = ctx->ridge_part; A.cnt = ctx->ridge_cnt;
     A.out = out; A.out_mu = out_mu;
+    A.frag = ctx->ridge_frag;
+    A.nblk8 = (ctx->n_T + 7) / 8 + 8;
     Kinds none;
     none.k = 0;
     for (int a = 0; a < RW_N_KINDS; ++a) none.kind[a] = -1;
@@ -589,6 +719,10 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     cudaError_t e;
     {
         ProfScope prof(ctx, s);
+        if (mbl >= 2) {                  // tile heights 32, 64: N' once per call
+            k_ridge_frag<<<dim3((unsigned)((A.nblk8 + 7) / 8), (unsigned)ctx->D), 256, 0, s>>>(A, k, ctx->cst, 1 << mbl);
+            ctx->launches++;
+        }
         if (mbl == 0) e = launch_ridge_t<1>(A, k, ctx->cst, grid, s);
         else if (mbl == 1) e = launch_ridge_t<2>(A, k, ctx->cst, grid, s);
         else if (mbl == 2) e = launch_ridge_t<4>(A, k, ctx->cst, grid, s);

@@ -68,7 +68,7 @@ struct Layout {           // byte offsets into the workspace (all 256-byte align
     int stream_splits;    // row splits of the streaming fold
     int ridge_strips;     // ceil(n_rec / kRidgeCols)
     int ridge_max_p;      // largest tile height of k_fold_ridge the slot scratch was sized for (16, 32 or 64)
-    size_t ridge_cnt, ridge_part, ridge_slots;
+    size_t ridge_cnt, ridge_part, ridge_slots, ridge_frag;
     bool sliced;          // RW_CREATE_SLICED: the INT8 slices of R are in the workspace
     int ns8;              // 8-bit balanced slices per operand: 8 when n_T <= 2048, else 7 (rw_api.cu plan())
     int KT8, NT8;         // k-blocks of 32 recoil bins; 64-column units = 2 x (128-column tiles) (rw_fold_i8.cu)
@@ -102,6 +102,7 @@ struct rw_ctx {
     int *ridge_cnt;           // tickets of k_fold_ridge: 2 x [D * ridge_strips] + 1
     double *ridge_part;       // [2 kRidgePlanSMs][64] Poisson sums per CTA of k_fold_ridge
     double *ridge_slots;      // [3 G][tile height][256] parked partial tiles of k_fold_ridge
+    double *ridge_frag;       // N' as DMMA fragments for its tile heights 32 and 64 (k_ridge_frag)
     double *strip_part;       // [D * strips][16] Poisson sums per column strip
     double *G, *ident;        // prefolded templates [D][12][ldG]; identity coefficients [16][12] used to fold them
     int *flag;
