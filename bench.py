@@ -39,11 +39,11 @@ L2_BYTES = 126e6
 # this run: bench.py cannot run under ncu).  kernel -> (bytes per launch, file under profiles/)
 NCU_TRAFFIC = {
     "k_fold_gemm<8>": (64.519372e9 + 0.033138e9, "profiles/r02_folds.md"),
-    "k_fold_gemm<4>": (1.120025e9 + 0.032784e9, "profiles/r02_folds.md"),
-    "k_fold_stream<1>": (1.075720e9 + 0.011437e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<1>": (1.075512e9 + 0.007054e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<2>": (1.075595e9 + 0.008221e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<4>": (1.075435e9 + 0.005559e9, "profiles/r02_folds.md"),
+    "k_fold_stream<1>": (1.075719e9 + 0.011484e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<1>": (1.075498e9 + 0.005801e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<2>": (1.075463e9 + 0.006756e9, "profiles/r02_folds.md"),
+    "k_fold_ridge<4>": (1.078194e9 + 0.004309e9 + 0.001488e9, "profiles/r02_folds.md (k_ridge_frag included)"),
+    "k_fold_ridge<8>": (1.082517e9 + 0.005428e9 + 0.001489e9, "profiles/r02_folds.md (k_ridge_frag included)"),
 }
 
 
@@ -250,8 +250,9 @@ def single_eval_block(torch, ctx, timer, param_dev, kinds, dev, r_bytes, peaks, 
     fn = lambda: ctx.eval_batch(one, kinds, out=out1)                   # RW_MODE_AUTO: the one-launch streaming kernel
     for _ in range(5):
         fn()
-    ctx.profile_begin()
-    ms = timer.total_ms(fn, reps) / reps
+    ms = timer.total_ms(fn, reps) / reps                               # call level: without the library's event hooks
+    ctx.profile_begin()                                                 # (they cost ~5 us per call on the stream)
+    timer.total_ms(fn, reps)
     k_ms, k_n = ctx.profile_end()
     k_ms = k_ms / max(1, k_n)
     graph_us = None
@@ -310,8 +311,9 @@ def ridge_regimes(torch, ctx, timer, param_dev, kinds, dev, inp, peaks, dmma_pea
         fn = lambda: ctx.eval_batch(pb, kinds, out=ob)
         for _ in range(3):
             fn()
+        ms = timer.total_ms(fn, 20) / 20                                # call level: without the library's event hooks
         ctx.profile_begin()
-        ms = timer.total_ms(fn, 20) / 20
+        timer.total_ms(fn, 20)
         k_ms, k_n = ctx.profile_end()
         k_ms = k_ms / 20                                               # all fold launches of one call
         hbm_ms = r_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
@@ -384,6 +386,22 @@ def bench_config(name, dev, steps, warmup, peaks, dmma_peak, cores, quick):
         res["frac"] = None
         res["note"] = ("%.1e flop per scan is microseconds of tensor work: the scan is bound by its %d kernel launches; "
                        "no roofline fraction is claimed" % (fold_flops(inp, P), launches))
+        try:                                   # the same scan replayed from a CUDA graph: launch gaps gone, kernels remain
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                scan()
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                scan()
+            g_ms = timer.per_call_ms(g.replay, 20, warm=5)
+            res["graph_replay_ms_per_scan"] = g_ms
+            res["graph_replay_evals_per_s"] = P / g_ms * 1e3
+            res["graph_replay_call_frac"] = fold_flops(inp, P) / (g_ms * 1e-3) / 1e12 / dmma_peak
+        except Exception as exc:               # noqa: BLE001
+            res["graph_replay_ms_per_scan"] = "unavailable: %s" % str(exc)[:80]
     else:
         res["bound"] = "tensor"
         res["frac"] = achieved / dmma_peak

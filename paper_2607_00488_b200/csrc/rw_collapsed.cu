@@ -104,7 +104,9 @@ k_collapsed_multi(const double *__restrict__ G, int ldG, int n_rec, int D, int n
     }
 }
 
-__global__ void __launch_bounds__(kColThreads)
+// (three CTAs per SM: 80 registers and 48 bytes of spills beat 91 registers and two CTAs by 9 % -- the kernel is bound
+// by the FP64 pipe behind the dependent chain of its log1p, profiles/r02_alu_kernels.md)
+__global__ void __launch_bounds__(kColThreads, 3)
 k_collapsed(const double *__restrict__ G, int ldG, int n_rec, int D, const double *__restrict__ coef,
             const double *__restrict__ rate /*[.][4]: rate[.][0] scales the single component*/, int64_t Pc, const double *__restrict__ bkg, const double *__restrict__ counts,
             double *__restrict__ partial, int64_t part_stride, double *__restrict__ out_mu)

@@ -140,15 +140,17 @@ def test_caller_weights_profile_and_gradient_take_the_same_kernel(rw, orc):
     ctx.close()
 
 
-def test_cuda_graph_capture_of_a_ridge_call(rw, orc):
-    """The kernel only enqueues work and resets its own tickets: a 16-point call replays from a CUDA graph."""
+@pytest.mark.parametrize("P", [16, 40])
+def test_cuda_graph_capture_of_a_ridge_call(rw, orc, P):
+    """The kernel only enqueues work and resets its own tickets: a call replays from a CUDA graph -- the one-launch form
+    (16 points) and the two-launch form with N' written first (40 points); both are cooperative launches."""
     import torch
     inp = wl.make_custom(n_E=25, n_T=300, n_rec=130, n_periods=1, seed=41)
-    params, kinds = wl.random_points(16, [0, 1], seed=42)
+    params, kinds = wl.random_points(P, [0, 1], seed=42)
     ref, scale = orc.eval_batch(inp, params, kinds, want_abs=True)
-    ctx = rw.Reweighter(inp, max_batch=16)
+    ctx = rw.Reweighter(inp, max_batch=P)
     p = _cuda(params)
-    out = torch.empty(16, dtype=torch.float64, device="cuda")
+    out = torch.empty(P, dtype=torch.float64, device="cuda")
     side = torch.cuda.Stream()
     side.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(side):
