@@ -361,7 +361,7 @@ def test_gradient_through_the_sliced_contraction(rw, orc):
 
 
 # ------------------------------------------------------------------------------------- f-3 per-point survival probabilities
-@pytest.mark.parametrize("mode,P", [("stream", 3), ("gemm", 45), ("auto", 150)])
+@pytest.mark.parametrize("mode,P", [("stream", 3), ("gemm", 45), ("auto", 150), ("auto", 12), ("auto", 40)])
 def test_per_point_survival_probability(rw, orc, mode, P):
     """P_ee table per point: spectrum on the (E_nu x T) grid per point (n_E = 300: three staging chunks with a
     ragged tail; dead bins), then the dense fold; against orc.eval_pee."""
