@@ -68,8 +68,10 @@ enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
 enum {
     RW_DEVIANCE    = 0u,       /* default: 2 sum [mu - n + n ln(n/mu)] (Eq. 18 minus its saturated value) */
     RW_FULL_EQ18   = 1u << 0,  /* literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)] */
-    RW_MODE_AUTO   = 0u,       /* 1 point: one-launch streaming path; 2..32: one-launch streaming DMMA kernel;
-                                  more: tiled DMMA batched contraction */
+    RW_MODE_AUTO   = 0u,       /* 1 point: one-launch streaming path; 2..64: streaming DMMA kernel (one launch up to 16
+                                  points, two above: N' is written first); more: tiled DMMA batched contraction.  The
+                                  streaming DMMA kernel is a cooperative launch (its CTAs share out the epilogue of a
+                                  column strip and wait for one another); it can be captured in a CUDA graph */
     RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P, groups of 16 points per launch) */
     RW_MODE_GEMM   = 2u << 4,  /* force the tiled FP64 tensor-core (DMMA) contraction */
     RW_MODE_COLLAPSED = 3u << 4, /* opt-in: rank-K prefolded templates (exact, O(K n_rec) per point); see below */
