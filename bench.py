@@ -184,12 +184,17 @@ class Timer:
         return self.total_ms(fn, reps) / reps
 
 
-def policy_kernel(P):
-    """The fold kernel RW_MODE_AUTO picks for a call of P points (label only; mirrors rw_api.cu)."""
+def policy_kernel(P, inp=None):
+    """The fold kernel RW_MODE_AUTO picks for a call of P points (label only; mirrors rw_api.cu).  With `inp` the label
+    also names the ridge-kernel tail of a batch that is not a multiple of 128 points."""
     if P <= 1:
         return "k_fold_stream<1>"
     if P <= 64:
         return "k_fold_ridge<%d>" % (1 if P <= 8 else 2 if P <= 16 else 4 if P <= 32 else 8)
+    if inp is not None and 0 < P % 128 <= 96:           # fold_slice() in rw_api.cu: where the tail pays
+        D, n_T, n_rec = inp["R"].shape
+        if (P <= 16384 and n_T * n_rec >= 4e7) or (P <= 256 and n_T * n_rec * D >= 4e6):
+            return ("k_fold_gemm<8> + " if P >= 128 else "") + "k_fold_ridge for the last %d points" % (P % 128)
     return "k_fold_gemm<8>"
 
 
@@ -651,13 +656,13 @@ def main():
     sweep, collapsed, fp32_leg, sliced_leg, next_rows, lib_dgemm = None, None, None, None, None, None
     if not lite:
         sweep = []
-        for Pb in (1, 4, 16, 64, 256, 2048):
+        for Pb in (1, 4, 16, 64, 192, 256, 300, 2048):
             if Pb > P:
                 break
             pb = param_dev[:Pb].contiguous()
             ob = torch.empty(Pb, dtype=torch.float64, device=dev)
             t = timed(lambda: ctx.eval_batch(pb, kinds, out=ob), 20 if Pb <= 256 else 5)
-            sweep.append({"points": Pb, "ms_per_call": t, "evals_per_s": Pb / t * 1e3, "kernel": policy_kernel(Pb),
+            sweep.append({"points": Pb, "ms_per_call": t, "evals_per_s": Pb / t * 1e3, "kernel": policy_kernel(Pb, inp),
                           "fold_tflops": fold_flops(inp, Pb) / t / 1e9, "response_gbs": r_bytes / t / 1e6})
         # opt-in rank-K collapsed mode: exact, O(11 n_rec) per point, FP64-ALU bound; never mixed into `value`
         out_c = torch.empty(P, dtype=torch.float64, device=dev)

@@ -194,6 +194,8 @@ static const char *flag_message(int f)
 // points, N' from k_ridge_frag above: 64 points 0.536 ms against 0.574 ms for the tiled contraction); beyond -> the
 // tiled DMMA contraction (tile height 128, split-K).  The opt-in contractions (prec != 0) replace the last two.
 constexpr int kAutoRidgeMax = 64;
+constexpr int kAutoTailRows = 96;        // left-over points of a batch (P mod 128) that go to the ridge kernel in RW_MODE_AUTO
+constexpr int64_t kAutoTailMax = 16384;  // ... for batches up to this size (beyond, one more row of tiles is < 1 %)
 static bool auto_stream(const rw_ctx *, int64_t P, int prec) { return prec == 0 ? P <= 1 : P <= 4; }
 static bool use_stream(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
 {
@@ -222,6 +224,32 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
     const bool contraction = mode != RW_MODE_COLLAPSED && !stream_mode && !use_ridge(ctx, mode, Ps, prec);
     if (opt.bound && !(contraction && prec >= 2))                  // every other regime is an FP64 path
         RW_CUDA(ctx, cudaMemsetAsync(opt.bound, 0, (size_t)Ps * 8, s));
+    // RW_MODE_AUTO, FP64: the tiled contraction works in rows of 128 points, and a partly filled last row costs as much
+    // as a full one (config-4 size: 1.07 ms per row of tiles; 192 points 2.02 ms).  Up to 96 left-over points go through
+    // the streaming DMMA kernel instead (0.18 / 0.27 / 0.53 ms for <= 16 / 32 / 64 points): 192 points 1.60 ms, 65 points
+    // 0.71 instead of 1.07 ms.  Scans of "a few hundred" points are the paper's own use.
+    // Where it pays (measured): responses large enough that a row of tiles is a sizeable part of a wave of the machine
+    // (n_T n_rec >= 4e7 per period: config-4 class), and any batch of <= 256 points unless the response is so small
+    // that the call is bound by its launches (n_T n_rec D < 4e6: config 2 and below), where the extra launches lose.
+    const double cells = (double)ctx->n_T * (double)n_rec;
+    const bool tail_pays = (Ps <= kAutoTailMax && cells >= 4e7) || (Ps <= 256 && cells * D >= 4e6);
+    if (contraction && mode == RW_MODE_AUTO && prec == 0 && L.ridge_max_p >= kRidgeMaxP && tail_pays) {
+        const int64_t rem = Ps % kBM;
+        if (rem > 0 && rem <= kAutoTailRows) {
+            const int64_t main = Ps - rem;
+            if (main > 0) {
+                const int rc = fold_slice(ctx, main, RW_MODE_GEMM, full, dout, out_mu, s, 0, opt);
+                if (rc != RW_OK) return rc;
+            }
+            for (int64_t g0 = main; g0 < Ps; g0 += L.ridge_max_p) {
+                const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
+                double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+                RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
+                                               dout + g0, full, mu, s));
+            }
+            return RW_OK;
+        }
+    }
     if (mode == RW_MODE_COLLAPSED) {
         const int nstrip = (n_rec + 511) / 512;
         for (int64_t c0 = 0; c0 < Ps; c0 += L.MC) {

@@ -58,6 +58,16 @@ def test_every_tile_height_on_a_ragged_shape(rw, orc, P):
         _check(rw, orc, inp, params, kinds, mode="auto")
 
 
+@pytest.mark.parametrize("P", [65, 192, 230])
+def test_auto_sends_the_left_over_points_of_a_batch_through_the_ridge_kernel(rw, orc, P):
+    """RW_MODE_AUTO beyond 64 points: the tiled contraction takes the full rows of 128 points, up to 96 left-over points
+    go through k_fold_ridge (65 = 64 + 1 with no tiled part at all, 192 = 128 + 64, 230 = 128 + 102: no split).  -2lnL and
+    the mu rows of both parts against the oracle."""
+    inp = wl.make_custom(n_E=31, n_T=2300, n_rec=1810, n_periods=1, seed=61, dead_fraction=0.05)
+    params, kinds = wl.random_points(P, [0, 1, 4, 6], seed=62 + P)
+    _check(rw, orc, inp, params, kinds, mode="auto", max_batch=256)
+
+
 def test_odd_n_rec_single_range_and_groups_of_64(rw, orc):
     """n_rec = 53 (odd: padded copy of R), n_T = 77 (one row range, one partial chunk), 150 points forced through
     the kernel in groups of 64 + 64 + 22, with the library slicing at max_batch = 100 on top."""
