@@ -206,6 +206,24 @@ static bool use_ridge(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
     return mode == RW_MODE_RIDGE || (mode == RW_MODE_AUTO && prec == 0 && !auto_stream(ctx, P, prec) && P <= kAutoRidgeMax);
 }
 
+// RW_MODE_AUTO, FP64, beyond 64 points: the number of left-over points (P mod 128, at most 96) that go through the
+// streaming DMMA kernel instead of a partly filled row of tiles, or 0.  The tiled contraction works in rows of 128
+// points and a partly filled last row costs as much as a full one (config-4 size: 1.07 ms per row; 192 points 2.02 ms,
+// 65 points 1.07 ms); the ridge kernel does <= 16 / 32 / 64 points in 0.18 / 0.27 / 0.53 ms there (192 points 1.60 ms,
+// 65 points 0.71 ms).  Scans of "a few hundred" points are the paper's own use.
+// Where it pays (measured, never a loss from 1000 x 500 to 16384 x 8192): responses large enough that a row of tiles is
+// a sizeable part of a wave of the machine (n_T n_rec >= 4e7 per period: config-4 class), and any batch of <= 256 points
+// unless the response is so small that the call is bound by its launches (n_T n_rec D < 4e6: config 2 and below).
+static int64_t auto_tail(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
+{
+    const Layout &L = ctx->lay;
+    if (mode != RW_MODE_AUTO || prec != 0 || P <= kAutoRidgeMax || L.ridge_max_p < kRidgeMaxP) return 0;
+    const double cells = (double)ctx->n_T * (double)ctx->n_rec;
+    const bool pays = (P <= kAutoTailMax && cells >= 4e7) || (P <= 256 && cells * ctx->D >= 4e6);
+    const int64_t rem = P % kBM;
+    return (pays && rem <= kAutoTailRows) ? rem : 0;
+}
+
 // Options of the sliced contraction (prec 2 / 3): tol > 0 = strict (RW_SLICED_STRICT, RW_FP32): a point whose certified
 // relative error exceeds tol is recomputed by the FP64 DMMA path; bound = device array [Ps] that receives the certified
 // bound of every point (0 for points that went through an FP64 path), or NULL.
@@ -224,31 +242,19 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
     const bool contraction = mode != RW_MODE_COLLAPSED && !stream_mode && !use_ridge(ctx, mode, Ps, prec);
     if (opt.bound && !(contraction && prec >= 2))                  // every other regime is an FP64 path
         RW_CUDA(ctx, cudaMemsetAsync(opt.bound, 0, (size_t)Ps * 8, s));
-    // RW_MODE_AUTO, FP64: the tiled contraction works in rows of 128 points, and a partly filled last row costs as much
-    // as a full one (config-4 size: 1.07 ms per row of tiles; 192 points 2.02 ms).  Up to 96 left-over points go through
-    // the streaming DMMA kernel instead (0.18 / 0.27 / 0.53 ms for <= 16 / 32 / 64 points): 192 points 1.60 ms, 65 points
-    // 0.71 instead of 1.07 ms.  Scans of "a few hundred" points are the paper's own use.
-    // Where it pays (measured): responses large enough that a row of tiles is a sizeable part of a wave of the machine
-    // (n_T n_rec >= 4e7 per period: config-4 class), and any batch of <= 256 points unless the response is so small
-    // that the call is bound by its launches (n_T n_rec D < 4e6: config 2 and below), where the extra launches lose.
-    const double cells = (double)ctx->n_T * (double)n_rec;
-    const bool tail_pays = (Ps <= kAutoTailMax && cells >= 4e7) || (Ps <= 256 && cells * D >= 4e6);
-    if (contraction && mode == RW_MODE_AUTO && prec == 0 && L.ridge_max_p >= kRidgeMaxP && tail_pays) {
-        const int64_t rem = Ps % kBM;
-        if (rem > 0 && rem <= kAutoTailRows) {
-            const int64_t main = Ps - rem;
-            if (main > 0) {
-                const int rc = fold_slice(ctx, main, RW_MODE_GEMM, full, dout, out_mu, s, 0, opt);
-                if (rc != RW_OK) return rc;
-            }
-            for (int64_t g0 = main; g0 < Ps; g0 += L.ridge_max_p) {
-                const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
-                double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
-                RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
-                                               dout + g0, full, mu, s));
-            }
-            return RW_OK;
+    if (const int64_t rem = contraction ? auto_tail(ctx, mode, Ps, prec) : 0) {
+        const int64_t main = Ps - rem;
+        if (main > 0) {
+            const int rc = fold_slice(ctx, main, RW_MODE_GEMM, full, dout, out_mu, s, 0, opt);
+            if (rc != RW_OK) return rc;
         }
+        for (int64_t g0 = main; g0 < Ps; g0 += L.ridge_max_p) {
+            const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
+                                           dout + g0, full, mu, s));
+        }
+        return RW_OK;
     }
     if (mode == RW_MODE_COLLAPSED) {
         const int nstrip = (n_rec + 511) / 512;
@@ -773,6 +779,17 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
         }
     } else if (use_ridge(ctx, mode, P, prec)) {
         for (int64_t g0 = 0; g0 < P; g0 += L.ridge_max_p) {
+            const int Pb = (int)((P - g0 < L.ridge_max_p) ? P - g0 : L.ridge_max_p);
+            double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
+            RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
+        }
+    } else if (const int64_t rem = auto_tail(ctx, mode, P, prec)) {     // full rows of tiles, then the left-over points
+        const int64_t main = P - rem;
+        if (main > 0) {
+            const int rc = weights_rows(ctx, w, main, RW_MODE_GEMM, full, out, out_mu, s, prec, tol);
+            if (rc != RW_OK) return rc;
+        }
+        for (int64_t g0 = main; g0 < P; g0 += L.ridge_max_p) {
             const int Pb = (int)((P - g0 < L.ridge_max_p) ? P - g0 : L.ridge_max_p);
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));

@@ -68,6 +68,21 @@ def test_auto_sends_the_left_over_points_of_a_batch_through_the_ridge_kernel(rw,
     _check(rw, orc, inp, params, kinds, mode="auto", max_batch=256)
 
 
+def test_left_over_rows_of_caller_weights_take_the_ridge_kernel_too(rw, orc):
+    """rw_eval_weights with 150 rows in RW_MODE_AUTO: 128 through the tiled contraction, 22 through k_fold_ridge."""
+    import torch
+    inp = wl.make_custom(n_E=25, n_T=2300, n_rec=1810, n_periods=1, seed=63)
+    w = np.random.default_rng(64).uniform(0.2, 3.0, size=(150, 2300))
+    ref, mu_ref, ab = orc.eval_weights(inp, w, want_mu=True, want_abs=True, nthreads=8)
+    ctx = rw.Reweighter(inp, max_batch=256)
+    out, mu = ctx.eval_weights(_cuda(w), want_mu=True)
+    torch.cuda.synchronize()
+    rel = np.abs(mu.cpu().numpy() - mu_ref) / np.abs(mu_ref)
+    assert rel.max() <= MU_RTOL
+    assert np.all(np.abs(out.cpu().numpy() - ref) <= m2lnl_tol(ab))
+    ctx.close()
+
+
 def test_odd_n_rec_single_range_and_groups_of_64(rw, orc):
     """n_rec = 53 (odd: padded copy of R), n_T = 77 (one row range, one partial chunk), 150 points forced through
     the kernel in groups of 64 + 64 + 22, with the library slicing at max_batch = 100 on top."""
