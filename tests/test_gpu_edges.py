@@ -288,3 +288,32 @@ def test_rejected_device_counts_leave_the_context_unchanged(rw, orc):
     ref = orc.eval_batch(inp, params, kinds, full_eq18=True)
     assert np.all(np.abs(after - ref) <= 1e-9 + 1e-12 * np.abs(ref))
     ctx.close()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_a_scan_split_with_shard_range_reassembles_to_the_single_call(rw, orc, world):
+    """Strong scaling on one GPU: the shards that `bench.py --scaling strong` hands to the ranks (sharding.shard_range),
+    each through its own context, concatenated in rank order, against the one-call scan and the oracle.  The shards
+    start new rows of tiles, so the tiled contraction may split its k-ranges differently: equal to rounding, not to
+    the bit."""
+    import torch
+    from paper_2607_00488_b200 import sharding
+    inp = wl.make_custom(n_E=31, n_T=700, n_rec=390, n_periods=2, seed=171)
+    params, kinds = wl.random_points(301, [0, 1, 4, 6], seed=172)
+    ref, scale = orc.eval_batch(inp, params, kinds, want_abs=True, nthreads=8)
+    whole_ctx = rw.Reweighter(inp, max_batch=301)
+    whole = whole_ctx.eval_batch(_cuda(params), kinds).cpu().numpy()
+    whole_ctx.close()
+    parts, seen = [], 0
+    for rank in range(world):
+        lo, hi = sharding.shard_range(301, rank, world)
+        assert lo == seen
+        seen = hi
+        ctx = rw.Reweighter(inp, max_batch=hi - lo)                   # a rank's own context, sized for its shard
+        parts.append(ctx.eval_batch(_cuda(params[lo:hi]), kinds).cpu().numpy())
+        ctx.close()
+    torch.cuda.synchronize()
+    assert seen == 301
+    cat = np.concatenate(parts)
+    assert np.all(np.abs(cat - whole) <= 1e-12 * np.abs(whole))
+    assert np.all(np.abs(cat - ref) <= 1e-9 + 1e-12 * scale)
