@@ -279,6 +279,36 @@ int rw_profile_end(rw_ctx *ctx, double *fold_ms_total, int64_t *fold_launches);
 
 int rw_destroy(rw_ctx *ctx);
 
+/* rw_fold_weights_static: steps a2 + a3 + a4 for ONE point and ONE period on caller weights, for callers that cannot
+ * allocate device memory at all -- so cannot even provide the workspace rw_create wants.  Examples: a likelihood
+ * plugged into a host application whose own memory pool already owns the device and which hands a plugin only its
+ * input and output buffers; a fit next to latency-critical streams that a cudaMalloc / cudaFree (both synchronise the
+ * device) would stall; a process whose memory budget was fixed before this library was loaded.
+ *     mu[k]  = sum_i w[i] N_mc[i] R[i][k] + bkg[k]           (Eq. 1; Eq. 11)
+ *     out    = 2 sum_k [mu_k - n_k + n_k ln(n_k / mu_k)]     (Eq. 18, relative to its saturated value)
+ * the same numbers as rw_eval_weights with P = 1, D = 1, RW_MODE_STREAM (up to the order of the row-range sums).
+ * No rw_ctx, no workspace: the call and everything under it uses no cudaMalloc, cudaFree or allocating library
+ * routine.  The scratch of the streaming fold (partial sums per row range, completion tickets) is a fixed
+ * 4 MiB + 512 B __device__ array inside librw.so; every GPU that loads the library holds it until the process exits.
+ *   w [n_T], N_mc [n_T], bkg [n_rec], counts [n_rec]   DEVICE pointers, FP64
+ *   R                    DEVICE pointer, [n_T] rows of pitch ldR doubles, rec index fastest; 16-byte aligned, ldR even
+ *                        and >= n_rec
+ *   out_m2lnL            DEVICE pointer to one double;  out_mu: NULL or DEVICE [n_rec]
+ *   n_rec <= RW_STATIC_MAX_N_REC (the scratch is compiled for that many columns): larger => RW_ERR_INVALID with a
+ *   message saying so (rw_last_error(NULL)); n_T is not limited.  n_T = 0 gives mu = bkg, n_rec = 0 gives 0.
+ * Asynchronous and stream-ordered on `cuda_stream`, never synchronises.  Numerical outcomes are values as in
+ * rw_eval_batch (mu_k = 0 < n_k: +inf; NaN in: NaN out).
+ * First call on a device: looks up the device address of the built-in array (cudaGetSymbolAddress, once per device,
+ * for the device that is current at the call) -- make that first call outside any stream capture.
+ * One array per GPU serves every call and keeps what the previous call left in it; the call clears the tickets it
+ * needs at zero on the stream before the kernel.  Two calls of this process that can overlap on one GPU (issued on
+ * different streams, or from different host threads without ordering) race on it and give garbage: keep all calls
+ * on a GPU ordered one after the other.  Other processes have their own copy of the array. */
+enum { RW_STATIC_MAX_N_REC = 8192 };
+int rw_fold_weights_static(const double *w, const double *N_mc, const double *R, int64_t ldR, int32_t n_T,
+                           int32_t n_rec, const double *bkg, const double *counts, double *out_m2lnL,
+                           double *out_mu, void *cuda_stream);
+
 const char *rw_strerror(int status);
 const char *rw_last_error(const rw_ctx *ctx); /* ctx may be NULL: last rw_create failure of this thread */
 

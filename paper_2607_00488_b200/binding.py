@@ -24,12 +24,13 @@ RW_MODE_AUTO, RW_MODE_STREAM, RW_MODE_GEMM, RW_MODE_COLLAPSED, RW_MODE_RIDGE = 0
 RW_PARAM_HOST, RW_OUT_HOST, RW_FP32, RW_SLICED, RW_SLICED_FAST, RW_SLICED_STRICT = 1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12, 1 << 13
 RW_CREATE_FP32, RW_CREATE_SLICED = 1, 2
 RW_TABLE_S_SM, RW_TABLE_BASIS, RW_TABLE_WHAT, RW_TABLE_G = 0, 1, 2, 3
+RW_STATIC_MAX_N_REC = 8192
 _MODES = {"auto": RW_MODE_AUTO, "stream": RW_MODE_STREAM, "gemm": RW_MODE_GEMM, "collapsed": RW_MODE_COLLAPSED,
           "ridge": RW_MODE_RIDGE}
 
 EXPORTS = ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_eval_certified", "rw_strict_fallback_count", "rw_eval_weights", "rw_eval_profile", "rw_eval_grad", "rw_eval_pee", "rw_get_table",
            "rw_launch_count", "rw_profile_begin", "rw_profile_end", "rw_destroy", "rw_strerror",
-           "rw_last_error")
+           "rw_last_error", "rw_fold_weights_static")
 
 _dp = C.POINTER(C.c_double)
 
@@ -108,6 +109,9 @@ def load_library():
     L.rw_strerror.restype = C.c_char_p
     L.rw_last_error.argtypes = [C.c_void_p]
     L.rw_last_error.restype = C.c_char_p
+    L.rw_fold_weights_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.rw_fold_weights_static.restype = C.c_int
     for f in ("rw_workspace_bytes", "rw_create", "rw_set_counts", "rw_eval_batch", "rw_get_table",
               "rw_destroy", "rw_profile_begin", "rw_profile_end"):
         getattr(L, f).restype = C.c_int
@@ -125,6 +129,40 @@ class _DevicePointer:
     def __init__(self, ptr, n):
         self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f8", "data": (int(ptr), False),
                                          "version": 3, "strides": None}
+
+
+def fold_weights_static(w, N_mc, R, bkg, counts, out=None, out_mu=None, want_mu=False):
+    """rw_fold_weights_static: -2lnL (and mu) of one point and one period for caller weights w[n_T], without a
+    Reweighter and without any workspace -- for users who cannot allocate device memory (a plugin inside an
+    application whose memory pool owns the GPU, a fit that must not trigger the device-wide synchronisation of
+    cudaMalloc).  The library's built-in 4 MiB scratch serves all calls, so n_rec <= RW_STATIC_MAX_N_REC, and calls
+    on one GPU must not overlap (keep them on one stream).  All arguments are CUDA float64 tensors; R is
+    [n_T][n_rec] (a row pitch is taken from R.stride(0); it must be even).  Pass `out` (1 element) and `out_mu`
+    ([n_rec]) to keep this wrapper allocation-free as well; they are created with torch.empty otherwise.
+    Asynchronous on the current stream."""
+    L = load_library()
+    for name, t in (("w", w), ("N_mc", N_mc), ("R", R), ("bkg", bkg), ("counts", counts)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
+            raise RwError(-1, "fold_weights_static: %s must be a CUDA float64 tensor" % name)
+    n_T, n_rec = (int(x) for x in R.shape)
+    if R.stride(1) != 1 and n_rec > 1:
+        raise RwError(-1, "fold_weights_static: the reconstructed index of R must be contiguous")
+    ldR = int(R.stride(0)) if n_T > 1 else max(n_rec + (n_rec & 1), int(R.stride(0)))
+    assert w.numel() == n_T and N_mc.numel() == n_T and bkg.numel() == n_rec and counts.numel() == n_rec
+    for t in (w, N_mc, bkg, counts):
+        assert t.is_contiguous()
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=R.device)
+    if want_mu and out_mu is None:
+        out_mu = torch.empty(n_rec, dtype=torch.float64, device=R.device)
+    with torch.cuda.device(R.device):
+        rc = L.rw_fold_weights_static(C.c_void_p(w.data_ptr()), C.c_void_p(N_mc.data_ptr()), C.c_void_p(R.data_ptr()),
+                                      ldR, n_T, n_rec, C.c_void_p(bkg.data_ptr()), C.c_void_p(counts.data_ptr()),
+                                      C.c_void_p(out.data_ptr()),
+                                      C.c_void_p(out_mu.data_ptr()) if out_mu is not None else None, _stream_ptr())
+    if rc != 0:
+        raise RwError(rc, L.rw_last_error(None).decode() or L.rw_strerror(rc).decode())
+    return (out, out_mu) if (want_mu or out_mu is not None) else out
 
 
 class Reweighter:

@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librw.so")
-SOURCES = ["rw_api.cu", "rw_setup.cu", "rw_coef.cu", "rw_fold_stream.cu", "rw_fold_gemm.cu", "rw_fold_ridge.cu", "rw_fold_i8.cu", "rw_collapsed.cu", "rw_profile.cu", "rw_grad.cu", "rw_pee.cu"]
+SOURCES = ["rw_api.cu", "rw_setup.cu", "rw_coef.cu", "rw_fold_stream.cu", "rw_fold_gemm.cu", "rw_fold_ridge.cu", "rw_fold_i8.cu", "rw_collapsed.cu", "rw_profile.cu", "rw_grad.cu", "rw_pee.cu", "rw_noalloc.cu"]
 PROBE_LIB = os.path.join(HERE, "librw_probe.so")      # bench-only FP64 peak probe (include/rw_probe.h)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
