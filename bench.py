@@ -35,16 +35,111 @@ METRIC = "likelihood evals/sec (batched)"
 UNIT = "evals/s"
 L2_BYTES = 126e6
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from committed `ncu --set full` captures (NOT measured in
-# this run: bench.py cannot run under ncu).  kernel -> (bytes per launch, file under profiles/)
-NCU_TRAFFIC = {
-    "k_fold_gemm<8>": (64.519372e9 + 0.033138e9, "profiles/r02_folds.md"),
-    "k_fold_stream<1>": (1.075719e9 + 0.011484e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<1>": (1.075498e9 + 0.005801e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<2>": (1.075463e9 + 0.006756e9, "profiles/r02_folds.md"),
-    "k_fold_ridge<4>": (1.078194e9 + 0.004309e9 + 0.001488e9, "profiles/r02_folds.md (k_ridge_frag included)"),
-    "k_fold_ridge<8>": (1.082517e9 + 0.005428e9 + 0.001489e9, "profiles/r02_folds.md (k_ridge_frag included)"),
-}
+NCU_CSV = os.path.join("profiles", "r03_folds_raw.csv")
+REGIME_POINTS = (2, 3, 8, 12, 16, 17, 24, 32, 33, 40, 48, 56, 64, 65, 72, 96, 127, 128, 192, 300)
+DETAIL_FILE = "bench_detail.json"      # everything measured, prose included; the stdout line names it
+LINE_LIMIT = 4096                      # bytes of the contract line (the driver keeps only a tail of stdout)
+
+
+def load_ncu_traffic(path=None):
+    """kernel -> dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed reduction of an
+    `ncu --set full` capture of `bench.py --tour` on config 4 (profiles/r03_folds.md names the command).  NOT measured in
+    this run: bench.py cannot run under ncu.  Of a kernel's captures inside plain rw_eval_batch calls (rows whose `call`
+    names no flag), the longest one with a DRAM figure counts: the main launch of a chunk (ncu returned no counters for
+    the 1.6 ms split-K tail launches of k_fold_gemm<8>).  Missing file or kernel: no traffic figure."""
+    import csv
+    path = path or os.path.join(ROOT, NCU_CSV)
+    res, best = {}, {}
+    if not os.path.exists(path):
+        return res
+    with open(path, newline="") as f:
+        for row in csv.DictReader(f):
+            call = row.get("call", "rw_eval_batch")
+            if not call.startswith("rw_eval_batch") or "RW_" in call:
+                continue
+            try:
+                t, tr = float(row["time_ms"]), float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+            except (KeyError, ValueError):
+                continue
+            if t >= best.get(row["kernel"], 0.0):
+                best[row["kernel"]], res[row["kernel"]] = t, tr
+    return res
+
+
+NCU_TRAFFIC = load_ncu_traffic()
+
+
+def _clean(x, digits=6):
+    """JSON-safe copy: non-finite floats -> None, floats rounded to `digits` significant digits, numpy scalars unwrapped."""
+    if isinstance(x, dict):
+        return {str(k): _clean(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_clean(v, digits) for v in x]
+    if isinstance(x, (bool, np.bool_)):
+        return bool(x)
+    if isinstance(x, (int, np.integer)):
+        return int(x)
+    if isinstance(x, (float, np.floating)):
+        x = float(x)
+        if x != x or x in (float("inf"), float("-inf")):
+            return None
+        return float("%.*g" % (digits, x))
+    return x
+
+
+def contract_line(full):
+    """The ONE line the driver parses: built from the dict of everything measured (`full`, which goes to
+    bench_detail.json as it is), numbers only, no prose, at most LINE_LIMIT bytes, strict JSON.
+    roofline.regimes rows: [points, kernel, bound, ms_per_call, frac]; roofline.per_config values:
+    [evals_per_s, bound, frac, single_eval_ms, mu_rel_max, m2lnl_err_over_bound_max, parity pass]."""
+    def pick(d, keys):
+        return {k: d.get(k) for k in keys if d is not None and k in d} if d else None
+
+    line = {k: full.get(k) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                                      "higher_is_better", "scaling", "vs_baseline", "dtype", "data")}
+    cfg = full.get("config") or {}
+    line["config"] = dict(cfg)
+    line["gpu_launches"] = full.get("gpu_launches")
+    line["clocks"] = pick(full.get("clocks"), ("sm_mhz", "sm_max_mhz", "reasons"))
+    line["e2e"] = pick(full.get("e2e"), ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step",
+                                         "matches_device_path"))
+    rf = full.get("roofline") or {}
+    roof = pick(rf, ("bound", "kernel", "achieved", "peak", "unit", "frac", "call_frac", "traffic", "avg_launch_ms",
+                     "launches_timed", "kernel_share_of_step", "ridge_points"))
+    if rf.get("regimes"):
+        roof["regimes"] = [[r.get("points"), r.get("kernel"), r.get("bound"), r.get("ms_per_call"), r.get("frac")]
+                           for r in rf["regimes"]]
+    if rf.get("per_config"):
+        pc = {}
+        for name, r in rf["per_config"].items():
+            par = r.get("parity") or {}
+            pc[name] = [r.get("evals_per_s"), r.get("bound"), r.get("frac"), r.get("single_eval_ms"),
+                        par.get("mu_rel_max"), par.get("m2lnl_err_over_bound_max"), par.get("pass")] \
+                if "unavailable" not in r else None
+        roof["per_config"] = pc
+    line["roofline"] = roof
+    cpu = full.get("cpu_baseline")
+    if cpu:
+        line["cpu_baseline"] = pick(cpu, ("value", "unit", "cores", "kind", "sample"))
+        if cpu.get("single_thread"):
+            line["cpu_baseline"]["single_thread_value"] = cpu["single_thread"].get("value")
+    else:
+        line["cpu_baseline"] = None
+    line["parity"] = pick(full.get("parity"), ("points", "mu_rel_max", "m2lnl_abs_max", "m2lnl_err_over_bound_max", "pass"))
+    line["all_finite"] = full.get("all_finite")
+    line["bench_wall_s"] = full.get("bench_wall_s")
+    line["detail"] = full.get("detail")
+    if full.get("errors"):
+        line["errors"] = len(full["errors"])
+    text = json.dumps(_clean(line, 7), allow_nan=False, separators=(",", ":"))
+    if len(text) > LINE_LIMIT:                       # never let context take the contract down: drop it, largest first
+        for key in ("regimes", "per_config"):
+            if line["roofline"] and key in line["roofline"]:
+                del line["roofline"][key]
+                text = json.dumps(_clean(line, 7), allow_nan=False, separators=(",", ":"))
+                if len(text) <= LINE_LIMIT:
+                    break
+    return text
 
 
 def load_peaks():
@@ -98,17 +193,18 @@ class ClockSampler:
 
 
 def workload_config(name, inp, P, n_gpus, max_batch=0, scaling="weak"):
+    """The `config` object of the line; both arms (ours and --impl reference) print exactly this."""
     D, n_T, n_rec = inp["R"].shape
     if scaling == "strong":
-        par = "one scan of %d points split over %d GPU(s) (contiguous shards), tables replicated, -2lnL slices gathered" % (P, n_gpus)
+        par = "one scan split over %d GPU(s), tables replicated, -2lnL slices gathered" % n_gpus
     else:
         par = "points sharded over %d GPU(s), tables replicated, no collective" % n_gpus
     return {"workload": name, "n_E": int(inp["E"].size), "n_T": int(n_T), "n_rec": int(n_rec), "n_periods": int(D),
             "points_per_step_per_gpu": int(P), "response_bytes": int(D * n_T * n_rec * 8),
             "library_slice_points": int(max_batch) if max_batch else int(P), "parallelism": par,
-            "l2": ("response (%.2f GB) and reweighted spectrum exceed the 126 MB L2: no flush needed" % (D * n_T * n_rec * 8 / 1e9))
-                  if D * n_T * n_rec * 8 + 8.0 * P * n_T > 2 * L2_BYTES else
-                  "working set fits the 126 MB L2: a 256 MB buffer is rewritten between timed steps (L2 flush)"}
+            # working set beyond 2 x the 126 MB L2: nothing survives between steps, no flush needed; else a 256 MB buffer
+            # is rewritten between timed steps
+            "l2_flush": bool(D * n_T * n_rec * 8 + 8.0 * P * n_T <= 2 * L2_BYTES)}
 
 
 def default_max_batch(name, P):
@@ -145,7 +241,7 @@ def run_reference(args, rank, world):
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
-    print(json.dumps(line))
+    print(json.dumps(_clean(line, 9), allow_nan=False), flush=True)
 
 
 # ------------------------------------------------------------------------------------------------ helpers (GPU arm)
@@ -194,7 +290,7 @@ def policy_kernel(P, inp=None):
     if inp is not None and 0 < P % 128 <= 96:           # fold_slice() in rw_api.cu: where the tail pays
         D, n_T, n_rec = inp["R"].shape
         if (P <= 16384 and n_T * n_rec >= 4e7) or (P <= 256 and n_T * n_rec * D >= 4e6):
-            return ("k_fold_gemm<8> + " if P >= 128 else "") + "k_fold_ridge for the last %d points" % (P % 128)
+            return ("k_fold_gemm<8>+" if P >= 128 else "") + "k_fold_ridge[last %d]" % (P % 128)
     return "k_fold_gemm<8>"
 
 
@@ -215,7 +311,7 @@ def parity_indices(name, P, max_batch, n):
 
 def parity_block(orc, wl, torch, ctx, name, inp, params, kinds, out_scan, dev, max_batch, n_sample, cores):
     """Raw error maxima of the timed scan against the CPU oracle on a sample: -2lnL from the timed scan's own output,
-    mu from a 256-point call on the same kernel family (128-row tiles) that contains the sample points.
+    mu from 256-point RW_MODE_AUTO calls (the mode the scan ran in) that contain the sample points.
     Returns (dict, oracle seconds, points)."""
     P = params.shape[0]
     idx = parity_indices(name, P, max_batch, n_sample)
@@ -230,8 +326,7 @@ def parity_block(orc, wl, torch, ctx, name, inp, params, kinds, out_scan, dev, m
         sel = idx[lo:lo + 256]
         pad = np.setdiff1d(np.arange(min(P, 512)), sel)[:max(0, min(P, 256) - sel.size)]
         batch = np.concatenate([sel, pad]).astype(np.int64)
-        _, mu = ctx.eval_batch(torch.from_numpy(params[batch]).to(dev), kinds, want_mu=True,
-                               mode="gemm" if batch.size > 64 else "auto")
+        _, mu = ctx.eval_batch(torch.from_numpy(params[batch]).to(dev), kinds, want_mu=True, mode="auto")
         torch.cuda.synchronize()
         rel = np.abs(mu.cpu().numpy()[:sel.size] - mu_ref[lo:lo + sel.size]) / np.abs(mu_ref[lo:lo + sel.size])
         mu_max = float(rel.max()) if mu_max is None else max(mu_max, float(rel.max()))
@@ -287,7 +382,7 @@ def single_eval_block(torch, ctx, timer, param_dev, kinds, dev, r_bytes, peaks, 
                        "includes the last-CTA reduction; call_frac divides by the call-level time" % (r_bytes / 1e9))
         tr = NCU_TRAFFIC.get("k_fold_stream<1>")
         if tr and r_bytes == 1073741824:
-            blk["traffic"], blk["traffic_source"] = tr[0], tr[1] + " (ncu capture, not measured in this run)"
+            blk["traffic"], blk["traffic_source"] = tr, NCU_CSV + " (ncu capture, not measured in this run)"
     else:
         blk["bound"] = "l2/latency"
         blk["frac"] = None
@@ -324,14 +419,14 @@ def ridge_regimes(torch, ctx, timer, param_dev, kinds, dev, inp, peaks, dmma_pea
         hbm_ms = r_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
         ten_ms = fold_flops(inp, Pb) / (dmma_peak * 1e12) * 1e3
         bound_ms = max(hbm_ms, ten_ms)
-        blk = {"regime": "ridge", "points": Pb, "kernel": policy_kernel(Pb),
+        blk = {"regime": "ridge" if Pb <= 64 else "small batch", "points": Pb, "kernel": policy_kernel(Pb, inp),
                "bound": "hbm" if hbm_ms >= ten_ms else "tensor", "bound_ms": bound_ms, "ms_per_call": ms,
                "fold_kernel_ms": k_ms, "frac": bound_ms / ms, "kernel_frac": bound_ms / k_ms if k_ms > 0 else None,
                "evals_per_s": Pb / ms * 1e3, "fold_tflops": fold_flops(inp, Pb) / ms / 1e9,
                "response_gbs": r_bytes / ms / 1e6}
         tr = NCU_TRAFFIC.get(blk["kernel"])
         if tr and r_bytes == 1073741824:
-            blk["traffic"], blk["traffic_source"] = tr[0], tr[1] + " (ncu capture, not measured in this run)"
+            blk["traffic"], blk["traffic_source"] = tr, NCU_CSV + " (ncu capture, not measured in this run)"
         res.append(blk)
     return res
 
@@ -372,16 +467,17 @@ def bench_config(name, dev, steps, warmup, peaks, dmma_peak, cores, quick):
     ms = timer.total_ms(scan, n_steps) / n_steps
     fold_ms, fold_n = ctx.profile_end()
     launches = (ctx.launch_count() - launches0) // n_steps
-    if not big:
+    ms_e2e, same = None, None
+    if not big:                                                        # (config 5: one timed scan only, a scan takes seconds)
         ctx.eval_batch(param_pin, kinds, out=out_pin)
-    ms_e2e = timer.total_ms(lambda: ctx.eval_batch(param_pin, kinds, out=out_pin), n_steps) / n_steps
-    torch.cuda.synchronize()
-    same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
+        ms_e2e = timer.total_ms(lambda: ctx.eval_batch(param_pin, kinds, out=out_pin), n_steps) / n_steps
+        torch.cuda.synchronize()
+        same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
     achieved = fold_flops(inp, P) * n_steps / (fold_ms * 1e-3) / 1e12
     launch_bound = fold_flops(inp, P) < 5e10                            # < ~1.5 us of DMMA work per SM
     res = {"points": P, "k": k, "n_T": n_T, "n_rec": n_rec, "n_periods": D, "response_bytes": int(r_bytes),
            "library_slice_points": int(max_batch), "steps": n_steps, "warmup": "3 library slices" if big else n_warm,
-           "evals_per_s": P / ms * 1e3, "ms_per_scan": ms, "e2e_evals_per_s": P / ms_e2e * 1e3, "e2e_ms_per_scan": ms_e2e,
+           "evals_per_s": P / ms * 1e3, "ms_per_scan": ms, "e2e_evals_per_s": P / ms_e2e * 1e3 if ms_e2e else None, "e2e_ms_per_scan": ms_e2e,
            "e2e_h2d_bytes": int(P * k * 8), "e2e_d2h_bytes": int(P * 8), "e2e_matches_device_path": same,
            "gpu_launches_per_scan": int(launches), "l2_flush_between_steps": bool(need_flush),
            "dominant_kernel": policy_kernel(min(P, max_batch)), "fold_launches_per_scan": int(fold_n // n_steps),
@@ -479,7 +575,11 @@ def main():
     ap.add_argument("--tour", action="store_true",
                     help="no timing: two calls of every entry point / regime on the bench context, for `ncu -k ...` captures "
                          "(profiles/*.md name the command); prints the list of calls")
-    ap.add_argument("--quick", action="store_true", help="headline, e2e and rooflines only: no context legs, no other configs")
+    ap.add_argument("--quick", action="store_true", help="headline, e2e and rooflines only: no other configs")
+    ap.add_argument("--full", action="store_true",
+                    help="also time the opt-in legs (batch sweep, collapsed, FP32, sliced + certificate, profile / gradient / P_ee, "
+                         "library DGEMM); they go to bench_detail.json only, never into the stdout line")
+    ap.add_argument("--detail", default=DETAIL_FILE, help="where everything measured is written (JSON, relative to the repo root)")
     ap.add_argument("--max-batch", type=int, default=0,
                     help="points per library slice (default: the whole scan; 16384 for cfg5_joint6, as BASELINE.json says)")
     args = ap.parse_args()
@@ -522,6 +622,7 @@ def main():
         P_job = params.shape[0] * world
     P, k = params.shape
     lite = args.quick or world > 1          # multi-rank runs time the headline and e2e legs only
+    extras = (args.full or args.tour) and not lite         # opt-in legs (sliced / fp32 / collapsed / profile / gradient / P_ee / DGEMM): detail file only
 
     # tables resident in HBM before anything is timed (R is borrowed by the context, not copied)
     dev_inp = {key: torch.from_numpy(np.ascontiguousarray(inp[key])).to(dev)
@@ -529,7 +630,7 @@ def main():
     dev_inp["f_tau"] = inp["f_tau"]
     max_batch = args.max_batch or default_max_batch(name, params.shape[0] if not strong else P_job)
     max_batch = min(max_batch, max(P, 1))
-    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=not lite, sliced=not lite)   # + operand copies for the opt-in legs
+    ctx = binding.Reweighter(dev_inp, max_batch=max_batch, device=dev, fp32=extras, sliced=extras)   # + operand copies for the opt-in legs
     param_dev = torch.from_numpy(params).to(dev)
     out_dev = torch.empty(P, dtype=torch.float64, device=dev)
     param_pin = torch.from_numpy(params).pin_memory()
@@ -600,6 +701,33 @@ def main():
     same = bool(np.array_equal(out_pin.numpy(), out_dev.cpu().numpy()))
     out_scan = out_dev.cpu().numpy()
 
+    # everything measured goes into `full` (-> bench_detail.json); the stdout line is contract_line(full).  From here on
+    # no leg may take the line down: each runs under guard() and a failure is recorded in full["errors"].
+    sec = {"headline+e2e": time.perf_counter() - t_start}
+    full = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(name, inp, P_job if strong else P, world,
+                                      max_batch=default_max_batch(name, P_job if strong else P),
+                                      scaling="strong" if strong else "weak"),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(P * k * 8),
+                    "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps, "matches_device_path": same},
+            "gpu_launches": int(launches), "clocks": clocks, "all_finite": finite, "errors": [],
+            "detail": args.detail if rank == 0 else None, "section_wall_s": sec}
+    if rank == 0:       # insurance for a human reader if a later leg hangs: the headline so far, on stderr (stdout carries ONE line)
+        sys.stderr.write("bench.py headline so far: " + contract_line(full) + "\n")
+        sys.stderr.flush()
+
+    def guard(label, fn):
+        t0 = time.perf_counter()
+        try:
+            return fn()
+        except Exception as exc:               # noqa: BLE001
+            full["errors"].append("%s: %s" % (label, str(exc)[:200]))
+            return None
+        finally:
+            sec[label] = time.perf_counter() - t0
+
     # ---------------------------------------------------------------- roofline of the dominant kernel + the other regimes
     def tprobe(kind, prev):
         return max(prev, probe.fp64_peak(kind))
@@ -610,51 +738,58 @@ def main():
     dom = policy_kernel(min(P, max_batch))
     tr = NCU_TRAFFIC.get(dom) if name == "cfg4_dense" else None
     roofline = {"bound": "tensor", "kernel": dom, "achieved": achieved, "peak": dmma_peak, "unit": "TFLOP/s",
-                "frac": achieved / dmma_peak, "traffic": tr[0] if tr else None,
-                "traffic_source": (tr[1] + " (ncu --set full capture of this kernel on this workload; not measured in this run)") if tr else None,
+                "frac": achieved / dmma_peak, "traffic": tr,
+                "traffic_source": (NCU_CSV + " (ncu --set full capture of this kernel on this workload; not measured in this run)") if tr else None,
                 "peak_source": "FP64 DMMA.8x8x4 issue-rate probe measured live (librw_probe.so); DFMA probe %.2f; "
                                "bf16 %s peak x nominal FP64/bf16 ratio (45/2250) = %.1f burst / %.1f sustained"
                                % (dfma_peak, peaks["source"], peaks["bf16"] * 0.02, (peaks["bf16_sus"] or 0) * 0.02),
                 "launches_timed": int(fold_launches), "avg_launch_ms": fold_ms / max(1, fold_launches),
                 "flops_per_launch": flops_timed / max(1, fold_launches),
                 "kernel_share_of_step": fold_ms / ms,
-                "call_frac": flops_timed / (ms * 1e-3) / 1e12 / dmma_peak}
+                "call_frac": flops_timed / (ms * 1e-3) / 1e12 / dmma_peak,
+                "ridge_points": 4.0 * dmma_peak * 1e12 / (peaks["hbm_gbs"] * 1e9)}
+    full["roofline"] = roofline
     single = None
-    if rank == 0:
-        single = single_eval_block(torch, ctx, timer, param_dev, kinds, dev, r_bytes, peaks)
-        regimes = [single]
-        regimes += ridge_regimes(torch, ctx, timer, param_dev, kinds, dev, inp, peaks, dmma_peak, (2, 4, 8, 16, 32, 64))
+    if rank == 0 and world == 1:
+        single = guard("single_eval", lambda: single_eval_block(torch, ctx, timer, param_dev, kinds, dev, r_bytes, peaks))
+        regimes = [single] if single else []
+        regimes += guard("regimes", lambda: ridge_regimes(torch, ctx, timer, param_dev, kinds, dev, inp, peaks, dmma_peak,
+                                                          REGIME_POINTS)) or []
         regimes.append({"regime": "batched", "points": P, "kernel": dom, "bound": "tensor", "achieved_tflops": achieved,
                         "peak_tflops": dmma_peak, "frac": achieved / dmma_peak, "avg_launch_ms": roofline["avg_launch_ms"],
                         "flops_per_launch": roofline["flops_per_launch"], "ms_per_call": ms / args.steps})
         roofline["regimes"] = regimes
-        roofline["ridge_points"] = 4.0 * dmma_peak * 1e12 / (peaks["hbm_gbs"] * 1e9)
 
     # ---------------------------------------------------------------- parity maxima + CPU oracle beside it
-    cpu, parity = None, None
     cores = os.cpu_count() or 1
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import rw_oracle as orc
-        orc.build()
-        n_par = min(P, 2 * cores)
-        parity, secs, n_done = parity_block(orc, wl, torch, ctx, name, inp, params, kinds, out_scan, dev, max_batch,
-                                            n_par, cores)
-        cpu = {"value": n_done / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "%d sampled scan points of %d (the parity sample: slice/chunk edges + seeded draws), OpenMP "
-                         "over points on %d threads, %.1f s wall, mu and conditioning scale returned" % (n_done, P, cores, secs)}
-        n1 = 2 if fold_flops(inp, 1) > 1e8 else min(P, 64)
-        t0 = time.perf_counter()
-        orc.eval_batch(inp, params[:n1], kinds, nthreads=1)
-        s1 = time.perf_counter() - t0
-        cpu["single_thread"] = {"value": n1 / s1, "unit": UNIT, "cores": 1,
-                                "sample": "first %d scan points on one thread, %.1f s wall" % (n1, s1)}
+        def cpu_leg():
+            from oracle import rw_oracle as orc
+            orc.build()
+            n_par = min(P, 2 * cores)
+            parity, secs, n_done = parity_block(orc, wl, torch, ctx, name, inp, params, kinds, out_scan, dev, max_batch,
+                                                n_par, cores)
+            full["parity"] = parity
+            cpu = {"value": n_done / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": "%d of %d scan points, %d threads, %.1f s" % (n_done, P, cores, secs),
+                   "sample_detail": "the parity sample (slice/chunk edges + seeded draws), OpenMP over points, mu and "
+                                    "conditioning scale returned"}
+            full["cpu_baseline"] = cpu
+            n1 = 1 if fold_flops(inp, 1) > 1e8 else min(P, 64)
+            t0 = time.perf_counter()
+            orc.eval_batch(inp, params[:n1], kinds, nthreads=1)
+            s1 = time.perf_counter() - t0
+            cpu["single_thread"] = {"value": n1 / s1, "unit": UNIT, "cores": 1,
+                                    "sample": "first %d scan points on one thread, %.1f s wall" % (n1, s1)}
+        guard("parity+cpu_baseline", cpu_leg)
 
     # ---------------------------------------------------------------- other regimes of the same path (context lines)
     def timed(fn, reps):
         return timer.per_call_ms(fn, reps)
 
     sweep, collapsed, fp32_leg, sliced_leg, next_rows, lib_dgemm = None, None, None, None, None, None
-    if not lite:
+    t_extras = time.perf_counter()
+    if extras:
         sweep = []
         for Pb in (1, 4, 16, 64, 192, 256, 300, 2048):
             if Pb > P:
@@ -784,43 +919,41 @@ def main():
             except RuntimeError as exc:                                  # out of memory on a crowded box: context only
                 lib_dgemm = {"unavailable": str(exc)[:120]}
 
+    sec["extras"] = time.perf_counter() - t_extras
     ctx.close()
     del dev_inp, param_dev
     torch.cuda.empty_cache()
 
     # ---------------------------------------------------------------- every other BASELINE config, briefly
-    per_config = None
     if not lite and rank == 0:
         per_config = {name: {"see": "top level of this line (value, e2e, roofline, parity)", "evals_per_s": value,
                              "ms_per_scan": ms / args.steps, "dominant_kernel": dom, "bound": "tensor", "achieved": achieved,
                              "peak": dmma_peak, "unit": "TFLOP/s", "frac": achieved / dmma_peak,
-                             "single_eval_ms": single["ms_per_call"] if single else None}}
+                             "single_eval_ms": single["ms_per_call"] if single else None, "parity": full.get("parity")}}
         for other in wl.CONFIG_NAMES:
             if other == name:
                 continue
-            try:
-                per_config[other] = bench_config(other, dev, args.steps, args.warmup, peaks, dmma_peak, cores, args.quick)
-            except Exception as exc:               # noqa: BLE001  (a context leg never takes the line down)
-                per_config[other] = {"unavailable": str(exc)[:200]}
+            r = guard(other, lambda: bench_config(other, dev, min(args.steps, 5), 3, peaks, dmma_peak, cores, True))
+            per_config[other] = r if r is not None else {"unavailable": full["errors"][-1]}
         roofline["per_config"] = per_config
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-                "scaling": "strong" if strong else "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": workload_config(name, inp, P_job if strong else P, world, max_batch=default_max_batch(name, P_job if strong else P),
-                                          scaling="strong" if strong else "weak"),
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(P * k * 8),
-                        "d2h_bytes_per_step": int(P * 8), "ms_per_step": ms_e2e / args.steps,
-                        "matches_device_path": same},
-                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "parity": parity,
-                "single_eval": single, "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg,
-                "sliced_mode": sliced_leg, "library_dgemm": lib_dgemm, "next_rows": next_rows, "clocks": clocks,
-                "all_finite": finite, "bench_wall_s": time.perf_counter() - t_start,
-                "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
-                                 "the authors' own multi-component model; other hardware and inputs, not comparable"}
-        print(json.dumps(line))
+        full.update({"single_eval": single, "batch_sweep": sweep, "collapsed_mode": collapsed, "fp32_mode": fp32_leg,
+                     "sliced_mode": sliced_leg, "library_dgemm": lib_dgemm, "next_rows": next_rows,
+                     "bench_wall_s": time.perf_counter() - t_start,
+                     "paper_context": "PAPER.md Table I: 86.8 ms (RTX 3080 Ti) / 52.4 ms (A30X) per single evaluation of "
+                                      "the authors' own multi-component model; other hardware and inputs, not comparable"})
+        full.setdefault("cpu_baseline", None)
+        full.setdefault("parity", None)
+        if full["detail"]:
+            try:
+                with open(os.path.join(ROOT, args.detail), "w") as f:
+                    json.dump(_clean(full, 9), f, indent=1, allow_nan=False)
+            except OSError as exc:
+                full["detail"] = None
+                full["errors"].append("detail file: %s" % exc)
+        sys.stdout.flush()
+        print(contract_line(full), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
