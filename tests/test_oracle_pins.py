@@ -640,3 +640,33 @@ def test_config2_stored_derived_inputs(orc):
     p, kinds = wl.scan_points("cfg2_mm_lowE")
     assert p.shape == (1000, 1) and list(kinds) == [6]
     assert abs(p[0, 0] / 1e-12 - 1) < 1e-12 and abs(p[-1, 0] / 1e-10 - 1) < 1e-12
+
+
+def test_tolerance_scale_equals_the_deviance_two_sided(orc):
+    """`abs_out` = sum_k 2|term_k| sets every -2lnL tolerance of the GPU tests (1e-9 + 1e-12 x scale, reading T), so an
+    inflated scale would loosen every parity bar unnoticed.  Every deviance term of Eq. (18) is >= 0,
+    hence in deviance mode the scale must EQUAL the value to rounding -- in every oracle entry point that returns one;
+    for the profiled value it equals the value minus the Gaussian pull at the minimiser."""
+    tol = 4e-16
+    inp = _small_problem(D=2)
+    params, kinds = wl.random_points(6, [orc.EPS_EE_L, orc.EPS_TT_R, orc.MU_NU], seed=91)
+    out, ab = orc.eval_batch(inp, params, kinds, want_abs=True)
+    assert np.all(out > 0) and np.all(np.abs(ab - out) <= tol * out)
+    w = np.random.default_rng(92).uniform(0.1, 3.0, size=(4, inp["T"].size))
+    out, ab = orc.eval_weights(inp, w, want_abs=True)
+    assert np.all(out > 0) and np.all(np.abs(ab - out) <= tol * out)
+    mc = wl.make_components(n_comp=3, n_E=30, n_T=60, n_rec=31, n_periods=2, seed=42)
+    kinds3 = np.array([orc.EPS_EE_L, orc.MU_NU, orc.RATE_0, orc.RATE_0 + 2], np.int32)
+    p3, _ = wl.random_points(3, kinds3, seed=93)
+    out, ab = orc.eval_components(mc, p3, kinds3, want_abs=True)
+    assert np.all(out > 0) and np.all(np.abs(ab - out) <= tol * out)
+    Pp = np.clip(inp["P_e"][None, :] + np.random.default_rng(94).uniform(-0.2, 0.2, size=(6, inp["E"].size)), 0.0, 1.0)
+    out, ab = orc.eval_pee(inp, params, kinds, Pp, want_abs=True)
+    assert np.all(out > 0) and np.all(np.abs(ab - out) <= tol * out)
+    # profiled: no pull -> the scale is the value; with a pull -> the value minus ((s^ - s0)/sigma)^2
+    out, sc, ab = orc.eval_profile(inp, params, kinds, want_abs=True)
+    assert np.all(out > 0) and np.all(np.abs(ab - out) <= tol * out)
+    s0, sigma = 1.0, 0.05
+    out, sc, ab = orc.eval_profile(inp, params, kinds, s0=s0, sigma=sigma, want_abs=True)
+    pull = ((sc - s0) / sigma) ** 2
+    assert np.all(pull > 0) and np.all(np.abs(ab + pull - out) <= 4 * tol * out)
