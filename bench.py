@@ -286,7 +286,7 @@ def policy_kernel(P, inp=None):
     if P <= 1:
         return "k_fold_stream<1>"
     if P <= 64:
-        return "k_fold_ridge<%d>" % (1 if P <= 8 else 2 if P <= 16 else 4 if P <= 32 else 8)
+        return "k_fold_ridge<%d>" % ((P + 7) // 8)               # one instantiation per multiple of 8 points
     if inp is not None and 0 < P % 128 <= 96:           # fold_slice() in rw_api.cu: where the tail pays
         D, n_T, n_rec = inp["R"].shape
         if (P <= 16384 and n_T * n_rec >= 4e7) or (P <= 256 and n_T * n_rec * D >= 4e6):

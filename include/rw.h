@@ -185,8 +185,8 @@ int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const 
 /* rw_eval_certified: rw_eval_batch for the sliced contractions (flags must hold RW_SLICED, RW_SLICED_FAST or RW_FP32;
  * DEVICE pointers only, no out_mu) that also returns, per point, the certified bound
  *     out_bound[p] >= max over bins and periods of |mu~ - mu| / mu
- * of what the INT8 contraction computed (0 for points that went through an FP64 path: <= 4 points, the 5..32-point
- * kernel, or recomputed under RW_SLICED_STRICT; +inf where a bin's bound reaches its mu or the row could not be sliced).
+ * of what the INT8 contraction computed (0 for points that went through an FP64 path: calls of up to 64 points, which
+ * RW_MODE_AUTO gives to the streaming kernels, or points recomputed under RW_SLICED_STRICT; +inf where a bin's bound reaches its mu or the row could not be sliced).
  * The bound is rigorous for the arithmetic of rw_fold_i8.cu and pessimistic by 10-100x on smooth inputs. */
 int rw_eval_certified(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                       double *out_m2lnL, double *out_bound, uint32_t flags, void *cuda_stream);
@@ -310,7 +310,10 @@ int rw_fold_weights_static(const double *w, const double *N_mc, const double *R,
                            double *out_mu, void *cuda_stream);
 
 const char *rw_strerror(int status);
-const char *rw_last_error(const rw_ctx *ctx); /* ctx may be NULL: last rw_create failure of this thread */
+const char *rw_last_error(const rw_ctx *ctx); /* ctx may be NULL: the last failure without a context (rw_create,
+                                                 rw_fold_weights_static, a NULL ctx) of the CALLING THREAD -- that one
+                                                 buffer is thread-local state, the only state outside contexts besides
+                                                 the built-in scratch of rw_fold_weights_static */
 
 #ifdef __cplusplus
 }

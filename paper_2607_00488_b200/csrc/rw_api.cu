@@ -557,6 +557,7 @@ int rw_create(const rw_inputs *in, int64_t max_batch, void *dev_workspace, size_
         return RW_ERR_INVALID;
     }
     rc = make_tensor_maps(ctx);
+    if (rc == RW_OK) rc = ridge_setup(ctx);
     if (rc == RW_OK) rc = profile_setup(ctx);
     if (rc == RW_OK) {
         rc = pee_setup(ctx, s);
@@ -601,23 +602,23 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
     return RW_OK;
 }
 
-static int eval_batch_impl(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
+static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                            double *out_m2lnL, double *out_mu, double *out_bound, uint32_t flags, void *cuda_stream)
 {
-    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "rw_eval_batch: ctx is NULL");
-    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: P < 0 or k outside [0,11]");
+    if (!ctx) return fail(nullptr, RW_ERR_INVALID, "%s: ctx is NULL", fn);
+    if (P < 0 || k < 0 || k > RW_N_KINDS) return fail(ctx, RW_ERR_INVALID, "%s: P < 0 or k outside [0,11]", fn);
     if (P == 0) return RW_OK;
     if (!out_m2lnL || (k > 0 && (!param || !param_kind)))
-        return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: param, param_kind or out_m2lnL is NULL");
+        return fail(ctx, RW_ERR_INVALID, "%s: param, param_kind or out_m2lnL is NULL", fn);
     int kinds[RW_N_KINDS];
-    { int rc = check_kinds(ctx, "rw_eval_batch", k, param_kind, kinds); if (rc != RW_OK) return rc; }
+    { int rc = check_kinds(ctx, fn, k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
-    if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "rw_eval_batch: out_mu with RW_OUT_HOST is not supported");
+    if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "%s: out_mu with RW_OUT_HOST is not supported", fn);
     int prec = 0;
     double tol = 0.0;
-    { int rc = pick_prec(ctx, "rw_eval_batch", flags, true, &prec, &tol); if (rc != RW_OK) return rc; }
-    if (mode > RW_MODE_RIDGE) return fail(ctx, RW_ERR_INVALID, "rw_eval_batch: unknown mode in flags");
+    { int rc = pick_prec(ctx, fn, flags, true, &prec, &tol); if (rc != RW_OK) return rc; }
+    if (mode > RW_MODE_RIDGE) return fail(ctx, RW_ERR_INVALID, "%s: unknown mode in flags", fn);
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
@@ -670,7 +671,7 @@ static int eval_batch_impl(rw_ctx *ctx, const double *param, int64_t P, int32_t 
 int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
                   double *out_m2lnL, double *out_mu, uint32_t flags, void *cuda_stream)
 {
-    return eval_batch_impl(ctx, param, P, k, param_kind, out_m2lnL, out_mu, nullptr, flags, cuda_stream);
+    return eval_batch_impl("rw_eval_batch", ctx, param, P, k, param_kind, out_m2lnL, out_mu, nullptr, flags, cuda_stream);
 }
 
 int rw_eval_certified(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,
@@ -683,7 +684,7 @@ int rw_eval_certified(rw_ctx *ctx, const double *param, int64_t P, int32_t k, co
     if (!(flags & (RW_SLICED | RW_SLICED_FAST | RW_FP32)))
         return fail(ctx, RW_ERR_INVALID, "rw_eval_certified: needs RW_SLICED, RW_SLICED_FAST or RW_FP32 (the FP64 paths "
                                          "have no input-dependent bound)");
-    return eval_batch_impl(ctx, param, P, k, param_kind, out_m2lnL, nullptr, out_bound, flags, cuda_stream);
+    return eval_batch_impl("rw_eval_certified", ctx, param, P, k, param_kind, out_m2lnL, nullptr, out_bound, flags, cuda_stream);
 }
 
 int64_t rw_strict_fallback_count(const rw_ctx *ctx) { return ctx ? ctx->strict_fallbacks : 0; }

@@ -106,19 +106,22 @@ __device__ __forceinline__ void rg_bar_consumers() { asm volatile("bar.sync 1, %
 
 template <int MB> struct RidgeCfg {
     static constexpr int PP = 8 * MB;                                  // points of the tile
-    static constexpr int RS = (MB <= 2) ? 8 : 16;                      // recoil rows per ring stage (= per work unit)
-    static constexpr int NS = (MB == 1) ? 6 : (MB == 8) ? 4 : 5;       // ring stages
-    static constexpr int MinCtas = (MB <= 2) ? 2 : 1;
+    // Tile heights 24 .. 64 (MB >= 3) read N' ready-made (k_ridge_frag writes it once per call instead of once per column
+    // strip in every CTA; in the consumer warps the chain load W^ -> 3 DMMA -> store and the bar.sync behind it idled the
+    // tensor pipe for 10 % of the kernel there): one more warp copies it chunk by chunk into the two N' buffers.
+    // Every multiple of 8 points has its own instantiation: above 16 points the kernel is bound by the DMMA pipe, so its
+    // time follows the tile height, not the number of points (33 points in a 64-row tile ran at 0.46 of the bound).
+    static constexpr bool Prefab = (MB >= 3);
+    static constexpr bool Big = (MB >= 7);                             // 112 / 128 accumulator registers: setmaxnreg
+    static constexpr int RS = Prefab ? 16 : 8;                         // recoil rows per ring stage (= per work unit)
+    static constexpr int NS = (MB == 1) ? 6 : Big ? 4 : 5;             // ring stages
+    static constexpr int MinCtas = Prefab ? 1 : 2;
     // How a ring stage is handed back safely (see the consumer loop): one iteration late (free, but one stage less in
     // flight), or at once through a register dependence on its fragment loads (16 points: five 16 KB stages per CTA
     // are too few to give one away -- 0.199 ms against 0.214 ms on config 4)
     static constexpr bool LateRelease = (MB != 2);
-    // Tile heights 32 and 64 read N' ready-made (k_ridge_frag writes it once per call instead of once per column strip
-    // in every CTA; in the consumer warps the chain load W^ -> 3 DMMA -> store and the bar.sync behind it idled the
-    // tensor pipe for 10 % of the kernel there): one more warp copies it chunk by chunk into the two N' buffers
-    static constexpr bool Prefab = (MB >= 4);
-    static constexpr int Threads = (MB == 8) ? kRgThreads64 : Prefab ? kRgThreads + 32 : kRgThreads;
-    // tile height 64: setmaxnreg redistributes the registers the CTA was LAUNCHED with (384 x 168): 256 ConsumerRegs +
+    static constexpr int Threads = Big ? kRgThreads64 : Prefab ? kRgThreads + 32 : kRgThreads;
+    // tile heights 56, 64: setmaxnreg redistributes the registers the CTA was LAUNCHED with (384 x 168): 256 ConsumerRegs +
     // 128 HelperRegs must not exceed that pool, or the consumers wait for ever
     static constexpr int ConsumerRegs = 224, HelperRegs = 40;
     static_assert(kRgConsumers * ConsumerRegs + 128 * HelperRegs <= kRgThreads64 * 168, "setmaxnreg pool");
@@ -194,7 +197,7 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     __syncthreads();
 
     if (warp >= kRgWarps) {
-        if constexpr (MB == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(Cfg::HelperRegs));
+        if constexpr (Cfg::Big) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(Cfg::HelperRegs));
         if (warp == kRgWarps) {
             // ------------------------------------------------------------ producer: lane l copies row l of a stage
             uint64_t policy;
@@ -246,7 +249,7 @@ k_fold_ridge(const RidgeArgs A, const Kinds kd, const Consts cst)
     }
 
     // ---------------------------------------------------------------- consumers
-    if constexpr (MB == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::ConsumerRegs));
+    if constexpr (Cfg::Big) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::ConsumerRegs));
     // ---------------------------------------------------------------- a1: coefficients of the tile's points
     const double *wts = A.wts;
     if (!wts && !Cfg::Prefab) {
@@ -641,13 +644,7 @@ k_ridge_frag(const RidgeArgs A, const Kinds kd, const Consts cst, const int MB)
 template <int MB>
 static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Consts &cst, int grid, cudaStream_t s)
 {
-    static bool attr_set = false;          // per instantiation; the attribute is per device function
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_fold_ridge<MB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             RidgeCfg<MB>::Smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // (the > 48 KB dynamic shared memory attribute is set by ridge_setup() at rw_create, for the device of the context)
     // cooperative: the contributors of a tile wait for one another, so the whole grid (one wave by construction,
     // ridge_grid) must be resident at once; the launch fails instead of hanging where it could not be
     cudaLaunchConfig_t cfg = {};
@@ -663,7 +660,28 @@ static cudaError_t launch_ridge_t(const RidgeArgs &A, const Kinds &kd, const Con
     return cudaLaunchKernelEx(&cfg, k_fold_ridge<MB>, A, kd, cst);
 }
 
-// Grid of k_fold_ridge for tile height 8 << mb_log2: one wave of the SM slots, but at least ~256 recoil rows of one
+template <int MB> static cudaError_t ridge_attr_t()
+{
+    return cudaFuncSetAttribute(k_fold_ridge<MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, RidgeCfg<MB>::Smem);
+}
+
+// rw_create: the function attributes belong to the device that is current, not to the process -- a context on a
+// second GPU of the same process needs them set again, so no "done once" flag.
+int ridge_setup(rw_ctx *ctx)
+{
+    cudaError_t e = ridge_attr_t<1>();
+    if (e == cudaSuccess) e = ridge_attr_t<2>();
+    if (e == cudaSuccess) e = ridge_attr_t<3>();
+    if (e == cudaSuccess) e = ridge_attr_t<4>();
+    if (e == cudaSuccess) e = ridge_attr_t<5>();
+    if (e == cudaSuccess) e = ridge_attr_t<6>();
+    if (e == cudaSuccess) e = ridge_attr_t<7>();
+    if (e == cudaSuccess) e = ridge_attr_t<8>();
+    if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_fold_ridge): %s", cudaGetErrorString(e));
+    return RW_OK;
+}
+
+// Grid of k_fold_ridge for tile height 8 << mb_log2 (mb_log2 >= 2: any of the heights 24 .. 64): one wave of the SM slots, but at least ~256 recoil rows of one
 // strip per CTA (a smaller share is not worth a partial tile).  Host arithmetic only; also sizes the slot scratch.
 int ridge_grid(int n_T, int n_rec, int D, int mb_log2, int num_sms, int *nblk_out)
 {
@@ -694,7 +712,8 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
         rate = ctx->rate + (coef - ctx->coef) / kCoefStride * RW_MAX_COMPONENTS;
     const Layout &L = ctx->lay;
     if (Pb > L.ridge_max_p) return cudaErrorInvalidValue;               // the slot scratch is sized by max_batch (plan())
-    const int mbl = Pb <= 8 ? 0 : Pb <= 16 ? 1 : Pb <= 32 ? 2 : 3;     // tile height 8 << mbl
+    const int MB = (Pb + 7) / 8;                                        // tile height 8 MB: the points rounded up to 8
+    const int mbl = MB <= 1 ? 0 : MB == 2 ? 1 : 2;                      // geometry class: 2 CTAs per SM x 8-row stages | 1 x 16
     RidgeArgs A;
     A.R = ctx->R; A.R_period_stride = ctx->R_period_stride; A.ldR = ctx->ldR;
     A.n_T = ctx->n_T; A.n_rec = ctx->n_rec; A.D = ctx->D;
@@ -704,7 +723,8 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     A.sat_const = full_eq18 ? ctx->sat_const : nullptr;
     A.Pb = Pb;
     A.n_strips = L.ridge_strips;
-    const int grid = ridge_grid(ctx->n_T, ctx->n_rec, ctx->D, mbl, kRidgePlanSMs, &A.nblk);
+    // the slot scratch is sized for kRidgePlanSMs (plan() runs without a device); fewer SMs only shrink the grid
+    const int grid = ridge_grid(ctx->n_T, ctx->n_rec, ctx->D, mbl, ctx->num_sms < kRidgePlanSMs ? ctx->num_sms : kRidgePlanSMs, &A.nblk);
     const int RS = (mbl <= 1) ? 8 : 16;
     A.zero_ring = (ctx->ldR - (L.ridge_strips - 1) * kRgCols < kRgCols) || (ctx->n_T % RS != 0);
     A.zero = 0;
@@ -719,14 +739,20 @@ cudaError_t launch_fold_ridge(rw_ctx *ctx, const double *coef, const double *par
     cudaError_t e;
     {
         ProfScope prof(ctx, s);
-        if (mbl >= 2) {                  // tile heights 32, 64: N' once per call
-            k_ridge_frag<<<dim3((unsigned)((A.nblk8 + 7) / 8), (unsigned)ctx->D), 256, 0, s>>>(A, k, ctx->cst, 1 << mbl);
+        if (MB >= 3) {                   // tile heights 24 .. 64: N' once per call
+            k_ridge_frag<<<dim3((unsigned)((A.nblk8 + 7) / 8), (unsigned)ctx->D), 256, 0, s>>>(A, k, ctx->cst, MB);
             ctx->launches++;
         }
-        if (mbl == 0) e = launch_ridge_t<1>(A, k, ctx->cst, grid, s);
-        else if (mbl == 1) e = launch_ridge_t<2>(A, k, ctx->cst, grid, s);
-        else if (mbl == 2) e = launch_ridge_t<4>(A, k, ctx->cst, grid, s);
-        else e = launch_ridge_t<8>(A, k, ctx->cst, grid, s);
+        switch (MB) {
+        case 1: e = launch_ridge_t<1>(A, k, ctx->cst, grid, s); break;
+        case 2: e = launch_ridge_t<2>(A, k, ctx->cst, grid, s); break;
+        case 3: e = launch_ridge_t<3>(A, k, ctx->cst, grid, s); break;
+        case 4: e = launch_ridge_t<4>(A, k, ctx->cst, grid, s); break;
+        case 5: e = launch_ridge_t<5>(A, k, ctx->cst, grid, s); break;
+        case 6: e = launch_ridge_t<6>(A, k, ctx->cst, grid, s); break;
+        case 7: e = launch_ridge_t<7>(A, k, ctx->cst, grid, s); break;
+        default: e = launch_ridge_t<8>(A, k, ctx->cst, grid, s); break;
+        }
     }
     if (e != cudaSuccess) return e;
     ctx->launches++;

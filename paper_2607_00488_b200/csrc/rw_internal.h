@@ -36,7 +36,7 @@ constexpr int kStreamMaxPB = 16;                  // points folded per pass over
 
 // ---- streaming DMMA fold geometry (rw_fold_ridge.cu) -------------------------------------------
 constexpr int kRidgeCols = 256;                   // columns per strip (8 warps x 32)
-constexpr int kRidgeMaxP = 64;                    // points per launch (tile heights 8, 16, 32, 64)
+constexpr int kRidgeMaxP = 64;                    // points per launch (tile heights 8, 16, 24, ... 64)
 constexpr int kRidgePlanSMs = 148;                // B200: the stream-K grid is one wave of these SMs' slots
 
 struct Consts {
@@ -195,6 +195,7 @@ cudaError_t launch_collapsed(rw_ctx *ctx, int64_t p0, int64_t Pc, double *out_mu
 cudaError_t launch_reduce(rw_ctx *ctx, int n_parts, int64_t part_stride, int64_t Pc, double *out,
                           bool full_eq18, cudaStream_t s);                   // rw_fold_stream.cu
 int make_tensor_maps(rw_ctx *ctx);                                           // rw_fold_gemm.cu
+int ridge_setup(rw_ctx *ctx);                                                // rw_fold_ridge.cu
 int gemm_rows_per_warp_block(int64_t Pc);                                    // rw_fold_gemm.cu
 int gemm_tail_split(int tail, int num_sms, int k_iters, int max_items);      // rw_fold_gemm.cu
 

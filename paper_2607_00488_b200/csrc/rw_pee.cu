@@ -336,7 +336,9 @@ int pee_setup(rw_ctx *ctx, cudaStream_t s)
     k_pee_j0<<<(n_T + 127) / 128, 128, 0, s>>>(n_T, ctx->T, n_E, ctx->pee_TmaxS, ctx->pee_j0);
     ctx->launches += 4;
     if (cudaGetLastError() != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "per-point P_ee tables failed at launch");
-    cudaError_t e = cudaFuncSetAttribute(k_pee_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * (n_E + 1) * 8);
+    // The attribute belongs to the function on this device, not to the context: always raise it to the cap plan() admits
+    // (L.pee_scan), so that a later context with a smaller flux grid cannot lower it under a live context's launches.
+    cudaError_t e = cudaFuncSetAttribute(k_pee_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 << 10);
     if (e != cudaSuccess) return fail(ctx, RW_ERR_CUDA, "cudaFuncSetAttribute(k_pee_scan): %s", cudaGetErrorString(e));
     return RW_OK;
 }

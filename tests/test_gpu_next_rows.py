@@ -442,3 +442,28 @@ def test_per_point_survival_probability_components_and_explicit_tables(rw, orc, 
     _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
     assert abs(plain.item() - out[0].item()) <= 1e-9 + 1e-11 * abs(plain.item())     # nominal tables = ordinary path
     ctx.close()
+
+
+def test_per_point_survival_probability_two_live_contexts_of_different_flux_grids(rw, orc):
+    """k_pee_scan keeps its three suffix sums in dynamic shared memory: 3 (n_E + 1) doubles, 62 KB at n_E = 2600 -- more than
+    the 48 KB a kernel gets without cudaFuncAttributeMaxDynamicSharedMemorySize.  That attribute belongs to the function,
+    not to a context: a context created LATER with a small flux grid must not lower it under the first one."""
+    import torch
+    big = wl.make_custom(n_E=2600, n_T=90, n_rec=70, n_periods=1, seed=131)
+    small = wl.make_custom(n_E=120, n_T=77, n_rec=53, n_periods=1, seed=132)
+    kin = [wl.EPS_EE_L, wl.EPS_TT_R, wl.MU_NU]
+    rng = np.random.default_rng(133)
+    cases = []
+    for inp, P, seed in ((big, 9, 134), (small, 7, 135)):
+        params, kinds = wl.random_points(P, kin, seed=seed)
+        Pp = np.clip(inp["P_e"][None, :] + rng.uniform(-0.2, 0.2, size=(P, inp["E"].size)), 0.0, 1.0)
+        cases.append((inp, params, kinds, Pp) + orc.eval_pee(inp, params, kinds, Pp, want_mu=True, want_abs=True, nthreads=CORES))
+    ctx_big = rw.Reweighter(big, max_batch=16)
+    ctx_small = rw.Reweighter(small, max_batch=16)          # created second: its rw_create sets the attribute last
+    for _ in range(2):                                      # alternately, twice
+        for ctx, (inp, params, kinds, Pp, ref, mu_ref, scale) in zip((ctx_big, ctx_small), cases):
+            out, mu = ctx.eval_pee(_cuda(params), kinds, _cuda(Pp), want_mu=True)
+            torch.cuda.synchronize()
+            _assert_parity(out.cpu().numpy(), mu.cpu().numpy(), ref, mu_ref, scale)
+    ctx_small.close()
+    ctx_big.close()

@@ -46,9 +46,10 @@ def _check(rw, orc, inp, params, kinds, mode="ridge", max_batch=None, full_eq18=
     assert np.array_equal(out, out2), "a second launch on the same context must reproduce the first bit for bit"
 
 
-@pytest.mark.parametrize("P", [1, 5, 8, 9, 16, 17, 32, 33, 64])
+@pytest.mark.parametrize("P", [1, 5, 8, 9, 16, 17, 24, 25, 32, 33, 40, 41, 48, 49, 56, 57, 64])
 def test_every_tile_height_on_a_ragged_shape(rw, orc, P):
-    """Tile heights 8 / 16 / 32 / 64 with ragged point counts; n_T = 1500 (several row ranges, the last chunk of
+    """Every tile height 8, 16, 24, ... 64 (one instantiation per multiple of 8 points), full and with one point in the
+    next height; n_T = 1500 (several row ranges, the last chunk of
     every range partial, n_T not a multiple of 4), n_rec = 330 (two 256-column strips, ragged, 16-column groups
     partly outside), two periods, dead bins, all seven parameter kinds."""
     inp = wl.make_custom(n_E=24, n_T=1501, n_rec=330, n_periods=2, seed=17, dead_fraction=0.1)
@@ -193,7 +194,7 @@ def test_cuda_graph_capture_of_a_ridge_call(rw, orc, P):
     ctx.close()
 
 
-@pytest.mark.parametrize("P", [4, 16, 32, 64])
+@pytest.mark.parametrize("P", [4, 16, 24, 32, 44, 56, 64])
 def test_run_to_run_identical_when_streaming_from_hbm(rw, orc, P):
     """Regression test for a pipeline race found in round 2: a ring stage was handed back to the producer while a fragment
     load of it was still in flight (ptxas issues the mbarrier arrive right behind the last LDS), and with two CTAs per
