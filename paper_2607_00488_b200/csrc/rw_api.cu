@@ -206,6 +206,18 @@ static bool use_ridge(const rw_ctx *ctx, uint32_t mode, int64_t P, int prec)
     return mode == RW_MODE_RIDGE || (mode == RW_MODE_AUTO && prec == 0 && !auto_stream(ctx, P, prec) && P <= kAutoRidgeMax);
 }
 
+// Points of the next call of the streaming DMMA kernel when `rem` are left.  Its time follows the tile height (a
+// multiple of 8 points) but never drops below one pass over R (config 4: 0.18 / 0.22 / 0.27 / 0.34 / 0.40 / 0.47 /
+// 0.53 ms for <= 16 / 24 / 32 / 40 / 48 / 56 / 64 points), so when two calls are left they share the points evenly
+// instead of 64 + rest: 65 points = 40 + 25 (0.34 + 0.27 ms) rather than 64 + 1 (0.53 + 0.18 ms).
+static int ridge_group(int64_t rem, int max_p)
+{
+    if (rem <= max_p) return (int)rem;
+    if (rem > 2 * (int64_t)max_p) return max_p;
+    const int half = (int)(((rem + 1) / 2 + 7) / 8 * 8);
+    return half < max_p ? half : max_p;
+}
+
 // RW_MODE_AUTO, FP64, beyond 64 points: the number of left-over points (P mod 128, at most 96) that go through the
 // streaming DMMA kernel instead of a partly filled row of tiles, or 0.  The tiled contraction works in rows of 128
 // points and a partly filled last row costs as much as a full one (config-4 size: 1.07 ms per row; 192 points 2.02 ms,
@@ -248,8 +260,9 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
             const int rc = fold_slice(ctx, main, RW_MODE_GEMM, full, dout, out_mu, s, 0, opt);
             if (rc != RW_OK) return rc;
         }
-        for (int64_t g0 = main; g0 < Ps; g0 += L.ridge_max_p) {
-            const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
+        for (int64_t g0 = main, step = 0; g0 < Ps; g0 += step) {
+            const int Pb = ridge_group(Ps - g0, L.ridge_max_p);
+            step = Pb;
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
                                            dout + g0, full, mu, s));
@@ -272,8 +285,9 @@ static int fold_slice(rw_ctx *ctx, int64_t Ps, uint32_t mode, bool full, double 
                                             dout + g0, full, mu, s));
         }
     } else if (!contraction) {
-        for (int64_t g0 = 0; g0 < Ps; g0 += L.ridge_max_p) {
-            const int Pb = (int)((Ps - g0 < L.ridge_max_p) ? Ps - g0 : L.ridge_max_p);
+        for (int64_t g0 = 0, step = 0; g0 < Ps; g0 += step) {
+            const int Pb = ridge_group(Ps - g0, L.ridge_max_p);
+            step = Pb;
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, ctx->coef + g0 * kCoefStride, nullptr, nullptr, nullptr, Pb,
                                            dout + g0, full, mu, s));
@@ -642,9 +656,10 @@ static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int
             Kinds kd;
             kd.k = k;
             for (int a = 0; a < RW_N_KINDS; ++a) kd.kind[a] = (a < k) ? kinds[a] : -1;
-            const int group = stream_mode ? kStreamMaxPB : L.ridge_max_p;
-            for (int64_t g0 = 0; g0 < Ps; g0 += group) {
-                const int Pb = (int)((Ps - g0 < group) ? Ps - g0 : group);
+            for (int64_t g0 = 0, step = 0; g0 < Ps; g0 += step) {
+                const int Pb = stream_mode ? (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB)
+                                           : ridge_group(Ps - g0, L.ridge_max_p);
+                step = Pb;
                 double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
                 const double *cf = nullptr, *pr = (k > 0) ? dparam + g0 * k : nullptr;
                 if (k == 0) {
@@ -779,8 +794,9 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             RW_CUDA(ctx, launch_fold_stream(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
     } else if (use_ridge(ctx, mode, P, prec)) {
-        for (int64_t g0 = 0; g0 < P; g0 += L.ridge_max_p) {
-            const int Pb = (int)((P - g0 < L.ridge_max_p) ? P - g0 : L.ridge_max_p);
+        for (int64_t g0 = 0, step = 0; g0 < P; g0 += step) {
+            const int Pb = ridge_group(P - g0, L.ridge_max_p);
+            step = Pb;
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
@@ -790,8 +806,9 @@ static int weights_rows(rw_ctx *ctx, const double *w, int64_t P, uint32_t mode, 
             const int rc = weights_rows(ctx, w, main, RW_MODE_GEMM, full, out, out_mu, s, prec, tol);
             if (rc != RW_OK) return rc;
         }
-        for (int64_t g0 = main; g0 < P; g0 += L.ridge_max_p) {
-            const int Pb = (int)((P - g0 < L.ridge_max_p) ? P - g0 : L.ridge_max_p);
+        for (int64_t g0 = main, step = 0; g0 < P; g0 += step) {
+            const int Pb = ridge_group(P - g0, L.ridge_max_p);
+            step = Pb;
             double *mu = out_mu ? out_mu + (size_t)g0 * D * n_rec : nullptr;
             RW_CUDA(ctx, launch_fold_ridge(ctx, nullptr, nullptr, nullptr, w + (size_t)g0 * n_T, Pb, out + g0, full, mu, s));
         }
