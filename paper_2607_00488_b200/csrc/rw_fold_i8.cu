@@ -24,10 +24,13 @@
 // CERTIFICATE.  With A_i = N'[p][i] 2^-tau_i < 2^e_p, B_i = R[i][k] 2^tau_i < 2^f_k, K'_k the number of recoil bins
 // whose fixed-point R entry is non-zero and S_k = sum_i B_i 2^-f_k (<= K'_k):
 //   rounding of A:  sum_i |A_i - A~_i| B_i   <= 2^(e_p - 8 NS) 2^f_k S_k          (half an ulp of 2^(e_p - 8 NS + 1) each)
-//   rounding of B:  sum_i A~_i |B_i - B~_i|  <= 2^(f_k - 8 NS) 2^e_p K'_k
+//   rounding of B:  sum_i A~_i |B_i - B~_i|  <= 2^(f_k - 8 NS) 2^e_p K'_k + 2^e_p L_k,   L_k = the sum of the entries
+//                   0 < B_i < 2^(f_k - 8 NS) that round to zero: they are not among the K'_k, and each loses all of
+//                   A~_i B_i (a floor below the resolution over thousands of live bins, next to a few large entries
+//                   that meet N' = 0, is otherwise certified while the column's whole signal is gone)
 //   dropped pairs s + t >= NS (|digits| <= 129, 128; both digits are lower ones):
 //                   K'_k 2^(e_p + f_k - 14) 16512 sum_{d >= NS} (2 NS - 1 - d) 2^(-8 d)  <=  1.01 NS K'_k 2^(e_p + f_k - 8 NS)
-// so |mu~ - mu| <= 2^e_p g_k with the per-column constant g_k = 2^(f_k - 8 NS) (S_k + (1 + 1.01 NS) K'_k), computed once
+// so |mu~ - mu| <= 2^e_p g_k with the per-column constant g_k = 2^(f_k - 8 NS) (S_k + (1 + 1.01 NS) K'_k) + L_k, computed once
 // at rw_create (k_col_bound); the fast mode adds the diagonals 4 .. NS - 1 it leaves out: 5.07 K'_k 2^(e_p + f_k - 32).
 // The epilogue turns it into the certified relative error max_k delta / (mu~ - delta) (+ 2e-15 for its own FP64
 // rounding) of every point, which rw_eval_certified returns and RW_SLICED_STRICT acts on (rw_api.cu).
@@ -369,14 +372,15 @@ __global__ void k_col_bound(const double *__restrict__ R, int ldR, int n_T, int 
     if (k >= n_rec) return;
     const int f = f_col[k];
     const double scale2 = ldexp(1.0, 8 * ns - 1 - f);
-    double sum = 0.0, cnt = 0.0;
+    double sum = 0.0, cnt = 0.0, lost = 0.0;
     for (int i = 0; i < n_T; ++i) {
         const double v = ldexp(R[(size_t)i * ldR + k], tau[i]);
         sum += v;
         if (__double2ull_rn(v * scale2) != 0ull) cnt += 1.0;
+        else lost += v;                                              // below the resolution: the whole entry is the error
     }
     const double S = ldexp(sum, -f) * (1.0 + 1e-9);                  // its own summation rounding
-    const double full = ldexp(S + (1.0 + 1.01 * ns) * cnt, f - 8 * ns) * (1.0 + 1e-6);
+    const double full = (ldexp(S + (1.0 + 1.01 * ns) * cnt, f - 8 * ns) + lost) * (1.0 + 1e-6);
     gcol[k] = full;
     gcol[(size_t)n_rec + k] = full + ldexp(5.07 * cnt, f - 32);
 }

@@ -154,3 +154,39 @@ def test_strict_weights_path_and_flag_errors(rw, orc):
         plain.eval_batch(_cuda(params), kinds, mode="gemm", sliced="strict")
     plain.close()
     ctx.close()
+
+
+def test_entries_below_the_fixed_point_resolution_are_charged_to_the_bound(rw):
+    """Columns 5..9: three large entries (0.4) in recoil bins where the MC spectrum is empty (N' = 0 there, so they add
+    nothing to mu but set the column's fixed-point scale), and a floor of 2^-68 in all 2260 live bins -- below the
+    resolution 2^-58 of the seven-slice fixed point even after the rescaling by 2^tau = 512, so every one of them is
+    rounded to zero and the column's whole signal (~2e-15 on a background of 2e-4: ~1e-11 relative) is lost.  The bound
+    must own up to that: measured error <= certified bound with NO slack, against the FP64 DMMA path (same N', so the
+    oracle-vs-GPU rounding of N' does not enter), and the strict mode must recompute these points."""
+    import torch
+    inp = wl.make_custom(n_E=24, n_T=2300, n_rec=140, n_periods=1, seed=331, tail=0.0)
+    inp["N_mc"][0, :2260] = 256.0
+    inp["N_mc"][0, 2260:] = 0.0                                     # tau = 0 for the last bins (33-bin window all empty)
+    inp["R"][0][:, 5:10] = 0.0
+    inp["R"][0][:2260, 5:10] = 2.0 ** -68
+    inp["R"][0][-3:, 5:10] = 0.4
+    inp["bkg"][0, 5:10] = 2e-4
+    inp["counts"][0, 5:10] = 0.0
+    params, kinds = wl.random_points(24, [0, 1, 6], seed=332)
+    ctx = rw.Reweighter(inp, max_batch=32, sliced=True)
+    p = _cuda(params)
+    _, mu64 = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm")
+    _, mu8 = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm", sliced=True)
+    _, bound = ctx.eval_certified(p, kinds, sliced=True, mode="gemm")
+    torch.cuda.synchronize()
+    mu64, mu8, bound = mu64.cpu().numpy(), mu8.cpu().numpy(), bound.cpu().numpy()
+    worst = _mu_rel(mu8, mu64).max(axis=(1, 2))
+    lost = _mu_rel(mu8[:, 0, 5:10], mu64[:, 0, 5:10]).max(axis=1)
+    assert np.all(lost > 1e-12), "the construction must lose the floor: %.3e" % lost.min()
+    assert np.all(worst <= bound), "error %.3e above its certified bound %.3e" % (worst.max(), bound[worst.argmax()])
+    before = ctx.strict_fallback_count()
+    _, mu_s = ctx.eval_batch(p, kinds, want_mu=True, mode="gemm", sliced="strict")
+    torch.cuda.synchronize()
+    assert ctx.strict_fallback_count() - before == 24               # every point holds such columns
+    assert _mu_rel(mu_s.cpu().numpy(), mu64).max() <= 1e-14
+    ctx.close()
