@@ -68,10 +68,11 @@ enum { RW_MEM_HOST = 0, RW_MEM_DEVICE = 1 };
 enum {
     RW_DEVIANCE    = 0u,       /* default: 2 sum [mu - n + n ln(n/mu)] (Eq. 18 minus its saturated value) */
     RW_FULL_EQ18   = 1u << 0,  /* literal first sum of Eq. (18): 2 sum [mu - n ln mu + lnGamma(n+1)] */
-    RW_MODE_AUTO   = 0u,       /* 1 point: one-launch streaming path; 2..64: streaming DMMA kernel (one launch up to 16
-                                  points, two above: N' is written first); more: tiled DMMA batched contraction (on large
-                                  responses the last P mod 128 <= 96 points of a batch go through the streaming DMMA
-                                  kernel instead of a partly filled row of tiles).  The
+    RW_MODE_AUTO   = 0u,       /* 1 point: one-launch streaming path; 2..64: streaming DMMA kernel, tile height = the points
+                                  rounded up to 8 (one launch up to 16 points, two above: N' is written first); more: tiled
+                                  DMMA batched contraction (on large responses the last P mod 128 <= 96 points of a batch go
+                                  through the streaming DMMA kernel instead of a partly filled row of tiles; when that takes
+                                  two calls they share the points evenly, e.g. 65 = 40 + 25).  The
                                   streaming DMMA kernel is a cooperative launch (its CTAs share out the epilogue of a
                                   column strip and wait for one another); it can be captured in a CUDA graph */
     RW_MODE_STREAM = 1u << 4,  /* force the HBM-streaming fold (any P, groups of 16 points per launch) */
