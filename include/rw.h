@@ -177,7 +177,8 @@ int rw_set_counts(rw_ctx *ctx, const double *counts, int32_t mem_kind, void *cud
  *   param       [P][k] row-major, device pointer (host if RW_PARAM_HOST)
  *   param_kind  host [k], distinct values in RW_EPS_EE_L..RW_MU_NU (absent: 0) and RW_RATE_0 + c, c < n_comp (absent: 1)
  *   out_m2lnL   [P] device pointer (host if RW_OUT_HOST)
- *   out_mu      NULL, or [P][D][n_rec] predicted counts mu (same memory kind as out_m2lnL)
+ *   out_mu      NULL, or [P][D][n_rec] predicted counts mu (same memory kind as out_m2lnL); with RW_OUT_HOST it is staged
+ *               through the workspace in slices and copied D2H on the stream
  * P may be 0 (no-op) and may exceed max_batch (processed in slices).  Per-point numerical outcomes
  * are values, not errors: mu_k = 0 with n_k > 0 gives +inf; non-finite parameters give NaN. */
 int rw_eval_batch(rw_ctx *ctx, const double *param, int64_t P, int32_t k, const int32_t *param_kind,

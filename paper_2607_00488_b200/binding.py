@@ -269,8 +269,8 @@ class Reweighter:
             if out is None:
                 out = torch.empty(P, dtype=torch.float64, pin_memory=True)
             flags |= RW_PARAM_HOST | RW_OUT_HOST
-            if want_mu or out_mu is not None:
-                raise RwError(-4, "out_mu is only available with device-resident params/out")
+            if want_mu and out_mu is None:
+                out_mu = torch.empty((P, self.n_periods, self.n_rec), dtype=torch.float64, pin_memory=True)
         else:
             param = param.to(torch.float64).contiguous()
             if param.ndim == 1:

@@ -628,7 +628,6 @@ static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int
     { int rc = check_kinds(ctx, fn, k, param_kind, kinds); if (rc != RW_OK) return rc; }
     const uint32_t mode = flags & RW_MODE_MASK;
     const bool param_host = flags & RW_PARAM_HOST, out_host = flags & RW_OUT_HOST, full = flags & RW_FULL_EQ18;
-    if (out_host && out_mu) return fail(ctx, RW_ERR_UNSUPPORTED, "%s: out_mu with RW_OUT_HOST is not supported", fn);
     int prec = 0;
     double tol = 0.0;
     { int rc = pick_prec(ctx, fn, flags, true, &prec, &tol); if (rc != RW_OK) return rc; }
@@ -637,8 +636,13 @@ static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Layout &L = ctx->lay;
     const int D = ctx->D, n_rec = ctx->n_rec;
-    for (int64_t s0 = 0; s0 < P; s0 += L.max_batch) {
-        const int64_t Ps = (P - s0 < L.max_batch) ? P - s0 : L.max_batch;
+    // mu for a host caller is staged through the scratch of rw_eval_profile (prof_rows points of D n_rec doubles),
+    // slice by slice, and copied D2H on the stream like -2lnL
+    const bool mu_host = out_host && out_mu;
+    const int64_t slice = (mu_host && L.prof_rows < L.max_batch) ? L.prof_rows : L.max_batch;
+    for (int64_t s0 = 0; s0 < P; s0 += slice) {
+        const int64_t Ps = (P - s0 < slice) ? P - s0 : slice;
+        double *dmu = !out_mu ? nullptr : mu_host ? ctx->mu_prof : out_mu + (size_t)s0 * D * n_rec;
         const double *dparam = nullptr;
         if (k > 0) {
             dparam = param + s0 * k;
@@ -660,7 +664,7 @@ static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int
                 const int Pb = stream_mode ? (int)((Ps - g0 < kStreamMaxPB) ? Ps - g0 : kStreamMaxPB)
                                            : ridge_group(Ps - g0, L.ridge_max_p);
                 step = Pb;
-                double *mu = out_mu ? out_mu + (size_t)(s0 + g0) * D * n_rec : nullptr;
+                double *mu = dmu ? dmu + (size_t)g0 * D * n_rec : nullptr;
                 const double *cf = nullptr, *pr = (k > 0) ? dparam + g0 * k : nullptr;
                 if (k == 0) {
                     RW_CUDA(ctx, launch_coef(ctx, nullptr, Pb, 0, kinds, s));
@@ -675,10 +679,13 @@ static int eval_batch_impl(const char *fn, rw_ctx *ctx, const double *param, int
         RW_CUDA(ctx, launch_coef(ctx, dparam, Ps, k, kinds, s));
         SlicedOpt opt;
         opt.tol = tol; opt.bound = out_bound ? out_bound + s0 : nullptr;
-        { int rc = fold_slice(ctx, Ps, mode, full, dout, out_mu ? out_mu + (size_t)s0 * D * n_rec : nullptr, s, prec, opt); if (rc != RW_OK) return rc; }
+        { int rc = fold_slice(ctx, Ps, mode, full, dout, dmu, s, prec, opt); if (rc != RW_OK) return rc; }
         }
         if (out_host)
             RW_CUDA(ctx, cudaMemcpyAsync(out_m2lnL + s0, ctx->out_stage, (size_t)Ps * 8, cudaMemcpyDeviceToHost, s));
+        if (mu_host)
+            RW_CUDA(ctx, cudaMemcpyAsync(out_mu + (size_t)s0 * D * n_rec, ctx->mu_prof, (size_t)Ps * D * n_rec * 8,
+                                         cudaMemcpyDeviceToHost, s));
     }
     return RW_OK;
 }

@@ -317,3 +317,24 @@ def test_a_scan_split_with_shard_range_reassembles_to_the_single_call(rw, orc, w
     cat = np.concatenate(parts)
     assert np.all(np.abs(cat - whole) <= 1e-12 * np.abs(whole))
     assert np.all(np.abs(cat - ref) <= 1e-9 + 1e-12 * scale)
+
+
+def test_host_buffers_can_return_mu(rw, orc):
+    """rw_eval_batch with RW_PARAM_HOST | RW_OUT_HOST and out_mu: mu is staged through the workspace slice by slice (the
+    context is sized for 128 points, the call has 300: slices of 128, 128 and 44) and copied D2H on the stream; bit-equal
+    to the device-resident call, and within the bars of the oracle on sampled points around the slice edges."""
+    import torch
+    inp = wl.make_custom(n_E=31, n_T=203, n_rec=130, n_periods=2, seed=181)
+    params, kinds = wl.random_points(300, [0, 1, 4, 6], seed=182)
+    ctx = rw.Reweighter(inp, max_batch=128)
+    out_d, mu_d = ctx.eval_batch(torch.from_numpy(params).cuda(), kinds, want_mu=True)
+    out_h, mu_h = ctx.eval_batch(torch.from_numpy(params).pin_memory(), kinds, want_mu=True)
+    torch.cuda.synchronize()
+    assert not out_h.is_cuda and not mu_h.is_cuda
+    assert np.array_equal(out_h.numpy(), out_d.cpu().numpy())
+    assert np.array_equal(mu_h.numpy(), mu_d.cpu().numpy())
+    idx = np.array([0, 127, 128, 255, 256, 299])
+    ref, mu_ref, scale = orc.eval_batch(inp, params[idx], kinds, want_mu=True, want_abs=True, nthreads=4)
+    assert np.all(np.abs(mu_h.numpy()[idx] - mu_ref) <= 1e-12 * np.abs(mu_ref))
+    assert np.all(np.abs(out_h.numpy()[idx] - ref) <= 1e-9 + 1e-12 * scale)
+    ctx.close()
